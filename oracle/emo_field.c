@@ -1,0 +1,103 @@
+/* ORACLE (test infrastructure).  Charged-track propagation in a uniform magnetic
+ * field ("on-device propagation of particles through arbitrary
+ * magnetic fields ... different integration algorithms"; BASELINE.json
+ * configs[3]: "adaptive RK4 (1e-6 mm miss-distance tolerance)").  The paper gives
+ * no algorithm: classical RK4 with step doubling (Press et al.) plus a chord /
+ * secant boundary search -> DESIGN.md R-C9.
+ * State y = (x, u);  dy/ds = (u, kappa u x Bhat),  kappa = q*CB*|B|/p.
+ */
+#include <math.h>
+#include "emo.h"
+
+static void rhs(const double u[3], double kappa, const double B[3], double dx[3], double du[3]) {
+    dx[0] = u[0]; dx[1] = u[1]; dx[2] = u[2];
+    du[0] = kappa * (u[1] * B[2] - u[2] * B[1]);
+    du[1] = kappa * (u[2] * B[0] - u[0] * B[2]);
+    du[2] = kappa * (u[0] * B[1] - u[1] * B[0]);
+}
+
+static void rk4(const double x[3], const double u[3], double kappa, const double B[3], double h,
+                double xo[3], double uo[3]) {
+    double k1x[3], k1u[3], k2x[3], k2u[3], k3x[3], k3u[3], k4x[3], k4u[3], ut[3];
+    rhs(u, kappa, B, k1x, k1u);
+    for (int i = 0; i < 3; ++i) ut[i] = u[i] + 0.5 * h * k1u[i];
+    rhs(ut, kappa, B, k2x, k2u);
+    for (int i = 0; i < 3; ++i) ut[i] = u[i] + 0.5 * h * k2u[i];
+    rhs(ut, kappa, B, k3x, k3u);
+    for (int i = 0; i < 3; ++i) ut[i] = u[i] + h * k3u[i];
+    rhs(ut, kappa, B, k4x, k4u);
+    for (int i = 0; i < 3; ++i) {
+        xo[i] = x[i] + (h / 6.0) * (k1x[i] + 2.0 * k2x[i] + 2.0 * k3x[i] + k4x[i]);
+        uo[i] = u[i] + (h / 6.0) * (k1u[i] + 2.0 * k2u[i] + 2.0 * k3u[i] + k4u[i]);
+    }
+}
+
+/* one step of h versus two of h/2; err = |x_full - x_half|; result = the two-half-step
+ * state with u renormalised */
+void emo_rk4_doubling(const double x[3], const double u[3], double kappa, const double B[3], double h,
+                      double x1[3], double u1[3], double *err) {
+    double xf[3], uf[3], xm[3], um[3];
+    rk4(x, u, kappa, B, h, xf, uf);
+    rk4(x, u, kappa, B, 0.5 * h, xm, um);
+    rk4(xm, um, kappa, B, 0.5 * h, x1, u1);
+    double dx = xf[0] - x1[0], dy = xf[1] - x1[1], dz = xf[2] - x1[2];
+    *err = sqrt(dx * dx + dy * dy + dz * dz);
+    double n = sqrt(u1[0] * u1[0] + u1[1] * u1[1] + u1[2] * u1[2]);
+    u1[0] /= n; u1[1] /= n; u1[2] /= n;
+}
+
+/* propagate up to s_max inside cell `vol`; returns the arc length travelled,
+ * *hit = surface reached (-1: none).  x, u are updated in place. */
+double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x[3], double u[3],
+                           double kappa, double s_max, int *hit) {
+    const double eps = p->ph.field_eps;
+    double s_done = 0.0;
+    int surf = *surf_io;
+    double h = 0.25 / fabs(kappa);
+    if (s_max < h) h = s_max;
+    *hit = -1;
+    for (int attempt = 0; attempt < p->ph.max_substeps; ++attempt) {
+        double rem = s_max - s_done;
+        if (h > rem) h = rem;
+        double x1[3], u1[3], err;
+        emo_rk4_doubling(x, u, kappa, p->Bhat, h, x1, u1, &err);
+        if (err > eps && h > 1e-9) {
+            double f = 0.9 * pow(eps / err, 0.2);
+            h *= (f > 0.2 ? f : 0.2);
+            continue;
+        }
+        double c[3] = { x1[0] - x[0], x1[1] - x[1], x1[2] - x[2] };
+        double L = sqrt(c[0] * c[0] + c[1] * c[1] + c[2] * c[2]);
+        if (!(L > 0.0)) { s_done += h; break; }
+        double cd[3] = { c[0] / L, c[1] / L, c[2] / L };
+        int S;
+        double d = emo_distance(p, vol, x, cd, surf, &S);
+        if (d <= eps) {
+            /* chord bends back across the surface the track sits on: shorten and retry */
+            if (d == 0.0 && S == surf && h > 1e-9) { h *= 0.5; continue; }
+            *hit = S;                                  /* immediate (re-)crossing, nothing travelled */
+            *surf_io = surf;
+            return s_done;
+        }
+        if (d > L) {                                   /* chord stays inside the cell: accept */
+            x[0] = x1[0]; x[1] = x1[1]; x[2] = x1[2];
+            u[0] = u1[0]; u[1] = u1[1]; u[2] = u1[2];
+            s_done += h; surf = -1;
+            if (s_done >= s_max * (1.0 - 1e-14)) break;
+            double e = err > eps / 3125.0 ? err : eps / 3125.0;
+            double f = 0.9 * pow(eps / e, 0.2);
+            h *= (f < 5.0 ? f : 5.0);
+            continue;
+        }
+        if (L - d <= eps) {                            /* landed on S within tolerance */
+            x[0] = x1[0]; x[1] = x1[1]; x[2] = x1[2];
+            u[0] = u1[0]; u[1] = u1[1]; u[2] = u1[2];
+            *hit = S;
+            *surf_io = S;
+            return s_done + h;
+        }
+        h *= d / L;                                    /* secant: aim the chord end at S */
+    }
+    *surf_io = surf;
+    return s_done;
+}

@@ -1,0 +1,222 @@
+"""Pins for the oracle's geometry and uniform-field propagation (C9)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2203_09467_b200 import workloads as W
+
+
+def _inside(desc, vol, x):
+    """Brute-force point-in-cell test written directly from the surface definitions."""
+    for S, sense in zip(desc["volumes"][vol]["surf"], desc["volumes"][vol]["sense"]):
+        t, v = desc["surfaces"][S]
+        f = x[0] ** 2 + x[1] ** 2 - v * v if t == W.CZ else x[t] - v
+        if (1 if f > 0 else -1) != sense:
+            return False
+    return True
+
+
+def _march(desc, vol, x, u, smax, ds):
+    s = 0.0
+    while s < smax:
+        if not _inside(desc, vol, x + (s + ds) * u):
+            lo, hi = s, s + ds
+            for _ in range(60):
+                mid = 0.5 * (lo + hi)
+                if _inside(desc, vol, x + mid * u):
+                    lo = mid
+                else:
+                    hi = mid
+            return 0.5 * (lo + hi)
+        s += ds
+    return math.inf
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 4])
+def test_distance_against_ray_marching(emo, cfg):
+    desc, _ = W.get(cfg, 4)
+    P = emo.Problem(desc)
+    rng = np.random.default_rng(cfg)
+    checked = 0
+    for _ in range(300):
+        if cfg == 4:
+            r = rng.uniform(0, 294); ph = rng.uniform(0, 2 * math.pi)
+            x = np.array([r * math.cos(ph), r * math.sin(ph), rng.uniform(-149, 149)])
+        elif cfg == 2:
+            x = np.array([rng.uniform(-29, 29), rng.uniform(-29, 29), rng.uniform(-9, 49)])
+        else:
+            x = np.array([rng.uniform(-49, 49), rng.uniform(-49, 49), rng.uniform(1, 99)])
+        vol = P.locate(x)
+        assert vol >= 0 and _inside(desc, vol, x)
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        d, hit = P.distance(vol, x, u)
+        ref = _march(desc, vol, x, u, 700.0, 0.011)
+        if math.isfinite(ref) and ref > 0.05:       # marching can step over grazing chords shorter than ds
+            assert d == pytest.approx(ref, rel=1e-9, abs=1e-9)
+            checked += 1
+            # the landing point lies on the reported surface
+            t, v = desc["surfaces"][hit]
+            y = x + d * u
+            f = math.hypot(y[0], y[1]) - v if t == W.CZ else y[t] - v
+            assert abs(f) < 1e-9
+    assert checked > 200
+
+
+def test_cylinder_chord_and_on_surface_rules(emo):
+    desc, _ = W.config4(4)
+    P = emo.Problem(desc)
+    R = desc["surfaces"][0][1]          # 5 cm, cell 0 is inside it
+    # chord through the axis plane at impact parameter b: length 2 sqrt(R^2 - b^2) / sin(theta)
+    for b, uz in ((0.0, 0.0), (3.0, 0.0), (4.9, 0.3)):
+        s = math.sqrt(1 - uz * uz)
+        x = np.array([-math.sqrt(R * R - b * b), b, 0.0])      # on the cylinder
+        u = np.array([s, 0.0, uz])
+        d, hit = P.distance(0, x, u, surf=0)
+        assert hit == 0 and d == pytest.approx(2 * math.sqrt(R * R - b * b) / s, rel=1e-13)
+    # flagged on the cylinder and pointing outwards from the inside cell: immediate re-crossing, d = 0
+    d, hit = P.distance(0, np.array([R, 0.0, 0.0]), np.array([1.0, 0.0, 0.0]), surf=0)
+    assert (d, hit) == (0.0, 0)
+    # outside cell (cell 1 = Si shell between CZ0 and CZ1), flagged on CZ0, moving outwards: CZ0 is skipped
+    d, hit = P.distance(1, np.array([R, 0.0, 0.0]), np.array([1.0, 0.0, 0.0]), surf=0)
+    assert hit == 1 and d == pytest.approx(0.03, rel=1e-12)
+    # parallel to the axis: only the end planes
+    d, hit = P.distance(0, np.array([1.0, 1.0, 0.0]), np.array([0.0, 0.0, 1.0]))
+    assert hit == 84 and d == pytest.approx(150.0)
+
+
+def test_straight_track_through_the_calorimeter_stack(emo):
+    desc, _ = W.config2(4)
+    P = emo.Problem(desc)
+    u = np.array([0.05, -0.02, 1.0]); u /= np.linalg.norm(u)
+    x = np.array([0.0, 0.0, -0.1]); vol, surf = 100, -1
+    path = {}
+    seq = []
+    for _ in range(300):
+        d, hit = P.distance(vol, x, u, surf)
+        path[vol] = path.get(vol, 0.0) + d
+        x = x + d * u
+        nv = P.neighbour(x, u, hit)
+        seq.append(vol)
+        if nv < 0:
+            break
+        vol, surf = nv, hit
+    assert seq == [100] + list(range(100)) + [101]       # front vacuum, layers 0..99 in order, back vacuum
+    for layer in range(100):
+        thick = 0.23 if layer % 2 == 0 else 0.57
+        assert path[layer] == pytest.approx(thick / u[2], rel=1e-12)
+    assert sum(path.values()) == pytest.approx(50.1 / u[2], rel=1e-13)
+
+
+def test_neighbour_sideways_exit_and_world_escape(emo):
+    desc, _ = W.config2(4)
+    P = emo.Problem(desc)
+    # leave layer 10 through x = +20 -> right vacuum box (103), then through x = +30 -> outside
+    x = np.array([20.0, 1.0, 4.1]); u = np.array([1.0, 0.0, 0.0])
+    assert P.neighbour(x, u, 105) == 103
+    assert P.neighbour(np.array([30.0, 1.0, 4.1]), u, 106) == -1
+    # crossing back into the stack from the side box lands in the right layer
+    assert P.neighbour(x, -u, 105) == 10      # z = 4.1 lies in Pb_5 = [4.0, 4.23] = volume 10
+    # on an edge (also on a z plane): direction decides
+    x = np.array([20.0, 0.0, 0.8]); ud = np.array([-0.6, 0.0, 0.8])
+    assert P.neighbour(x, ud, 105) == 2
+    assert P.neighbour(x, np.array([-0.6, 0.0, -0.8]), 105) == 1
+
+
+# ---------------- field ----------------
+
+def _helix(x0, u0, kappa, Bhat, s):
+    """Analytic solution of du/ds = kappa u x Bhat."""
+    Bhat = np.asarray(Bhat, float)
+    upar = (u0 @ Bhat) * Bhat
+    uperp = u0 - upar
+    w = np.cross(uperp, Bhat)
+    x = x0 + upar * s + (uperp * math.sin(kappa * s) + w * (1 - math.cos(kappa * s))) / kappa
+    u = upar + uperp * math.cos(kappa * s) + w * math.sin(kappa * s)
+    return x, u
+
+
+def _open_problem(emo, B):
+    surfaces = [(W.PX, -1e4), (W.PX, 1e4), (W.PY, -1e4), (W.PY, 1e4), (W.PZ, -1e4), (W.PZ, 1e4)]
+    d = dict(materials=[W.PB], surfaces=surfaces,
+             volumes=[dict(surf=list(range(6)), sense=[1, -1, 1, -1, 1, -1], material=-1, tally=-1)],
+             field=B, physics=W.physics(n_E=16))
+    return emo.Problem(d)
+
+
+def test_rk4_doubling_error_estimate(emo):
+    import ctypes as C
+    L = emo.lib()
+    dp = C.POINTER(C.c_double)
+    x0 = np.zeros(3); u0 = np.array([0.6, 0.0, 0.8]); Bh = np.array([0.0, 0.0, 1.0])
+    kappa = -2.5
+    for h in (0.02, 0.05, 0.1):
+        x1 = np.zeros(3); u1 = np.zeros(3); err = C.c_double()
+        L.emo_rk4_doubling(x0.ctypes.data_as(dp), u0.ctypes.data_as(dp), kappa, Bh.ctypes.data_as(dp), h,
+                           x1.ctypes.data_as(dp), u1.ctypes.data_as(dp), C.byref(err))
+        xe, ue = _helix(x0, u0, kappa, Bh, h)
+        true = np.linalg.norm(x1 - xe)
+        assert true <= err.value / 10          # Richardson: the half-step result is ~16x better
+        assert abs(np.linalg.norm(u1) - 1) < 1e-15
+        assert abs(u1 @ Bh - u0 @ Bh) < 1e-4 * (h * kappa) ** 6 + 1e-15   # pitch: only the RK4 norm drift (renormalised)
+
+
+@pytest.mark.parametrize("B,q", [((0, 1.0, 0), -1), ((0, 0, 4.0), 1), ((0.3, -0.2, 0.5), -1)])
+def test_propagation_follows_the_analytic_helix(emo, B, q):
+    P = _open_problem(emo, B)
+    Bm = np.linalg.norm(B); Bh = np.array(B) / Bm
+    p = 5.0                                     # MeV/c
+    kappa = q * 2.99792458e-3 * Bm / p
+    assert 1 / abs(kappa) == pytest.approx(p / (2.99792458e-3 * Bm))
+    x0 = np.array([1.0, -2.0, 0.5]); u0 = np.array([0.48, 0.6, 0.64])
+    s_max = 30.0 / abs(kappa) if abs(kappa) * 30 < 200 else 100.0
+    s_max = min(s_max, 500.0)
+    s, hit, x, u = P.propagate_field(0, -1, x0, u0, kappa, s_max)
+    assert hit == -1 and s == pytest.approx(s_max, rel=1e-13)
+    xe, ue = _helix(x0, u0, kappa, Bh, s)
+    nsub = s_max * abs(kappa) / 0.05 + 10       # crude bound on the number of substeps
+    assert np.linalg.norm(x - xe) < 1e-7 * nsub / 15 + 1e-9
+    assert np.linalg.norm(u - ue) < 1e-6
+
+
+def test_radius_of_curvature_1T_1MeV(emo):
+    # r = p / (2.99792458e-3 B): 0.33356 cm for 1 MeV/c in 1 T
+    assert 1.0 / (2.99792458 * 1.0) == pytest.approx(0.33356, rel=1e-4)
+    P = _open_problem(emo, (0, 0, 1.0))
+    kappa = -2.99792458e-3 / 1e-3 * 1e-3        # p = 1 MeV/c, q = -1
+    x0 = np.zeros(3); u0 = np.array([1.0, 0.0, 0.0])
+    s, hit, x, u = P.propagate_field(0, -1, x0, u0, kappa, math.pi / abs(kappa))   # half a turn
+    assert np.linalg.norm(x - x0) == pytest.approx(2 * 333.56, rel=1e-3)
+
+
+def test_weak_field_limit_is_a_straight_line(emo):
+    P = _open_problem(emo, (0, 1e-12, 0))
+    x0 = np.array([0.0, 0.0, 0.0]); u0 = np.array([0.0, 0.6, 0.8])
+    s, hit, x, u = P.propagate_field(0, -1, x0, u0, -1e-15, 50.0)
+    assert s == pytest.approx(50.0, rel=1e-13) and np.allclose(x, 50.0 * u0, atol=1e-9) and np.allclose(u, u0, atol=1e-12)
+
+
+def test_boundary_landing_in_field(emo):
+    desc, _ = W.config3(4)
+    P = emo.Problem(desc)
+    eps = desc["physics"]["field_eps"]
+    rng = np.random.default_rng(11)
+    n_hit = 0
+    for _ in range(200):
+        layer = int(rng.integers(0, 100))
+        z0, z1 = desc["surfaces"][layer][1], desc["surfaces"][layer + 1][1]
+        x0 = np.array([rng.uniform(-5, 5), rng.uniform(-5, 5), rng.uniform(z0 + 1e-3, z1 - 1e-3)])
+        u0 = rng.normal(size=3); u0 /= np.linalg.norm(u0)
+        p = 10 ** rng.uniform(-0.5, 2)
+        kappa = -2.99792458e-3 * 1.0 / p
+        s, hit, x, u = P.propagate_field(layer, -1, x0, u0, kappa, 5.0)
+        xe, ue = _helix(x0, u0, kappa, np.array([0, 1.0, 0]), s)
+        assert np.linalg.norm(x - xe) < 1e-5          # on the true helix
+        if hit >= 0:
+            n_hit += 1
+            t, v = desc["surfaces"][hit]
+            assert abs(x[t] - v) <= 2 * eps           # landed within tolerance of the surface
+            assert hit in (layer, layer + 1, 104, 105, 108, 109)
+        else:
+            assert s == pytest.approx(5.0, rel=1e-13) and z0 < x[2] < z1
+    assert n_hit > 150
