@@ -1,0 +1,264 @@
+/* emx.h -- C-ABI boundary of the B200-native EM-shower step loop.
+ *
+ * The hot path of arxiv 2203.09467 ("Celeritas"): the per-track Monte Carlo step
+ * loop of a coupled gamma / e- / e+ electromagnetic shower.  The calls follow the
+ * paper's statement of the problem -- inputs are geometry, physics, events,
+ * cutoff thresholds and scoring regions (scoring API
+ * PAPER.md:152); the loop is PAPER.md:114 ("six characteristics")
+ * (tabulated cross sections, per-model interaction kernels)
+ * (secondary stack allocator), PAPER.md:204-212 (slots, queued initializers,
+ * iteration until nothing is left), PAPER.md:142 (surfaces + CSG cells) and
+ * PAPER.md:144 (field propagation).  The readings of everything the paper
+ * leaves open are listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - plain C, no torch types.  Every pointer is marked HOST or DEVICE.
+ *   - units: MeV, cm, g/cm3, tesla.  Particle codes 0 = gamma, 1 = e-, 2 = e+.
+ *   - all floating point is IEEE fp64; integers are 32 bit unless stated.
+ *   - every call returns 0 (or a non-negative id) on success and a negative
+ *     EMX_E_* code on failure; emx_last_error() gives the text.  Nothing
+ *     throws or aborts across the boundary.
+ *   - bulk device memory (primaries, workspace = track store + queues +
+ *     tallies) is allocated by the CALLER and passed as raw device pointers
+ *     together with the CUDA stream handle (cudaStream_t as void*; NULL = the
+ *     legacy default stream).  The library owns only the problem description
+ *     and one small (< 1 MB) device block holding tables and geometry.
+ *   - calls on one emx_problem are not thread-safe.
+ *   - there is NO CPU fallback: without a CUDA device every compute call
+ *     returns EMX_E_CUDA.
+ */
+#ifndef EMX_H
+#define EMX_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EMX_MAX_ELEM 4   /* elements per material */
+#define EMX_MAX_FACES 8  /* faces per cell */
+
+/* error codes */
+#define EMX_OK 0
+#define EMX_E_ARG (-1)      /* invalid argument */
+#define EMX_E_STATE (-2)    /* call out of order (e.g. tables not built) */
+#define EMX_E_CUDA (-3)     /* CUDA runtime error or no device */
+#define EMX_E_CAPACITY (-4) /* workspace too small / secondary stack cannot make progress */
+#define EMX_E_NOMEM (-5)
+
+/* surface types ("quadric surfaces", restricted): f = x_a - v (planes), x^2+y^2 - v^2 (CZ) */
+#define EMX_S_PX 0
+#define EMX_S_PY 1
+#define EMX_S_PZ 2
+#define EMX_S_CZ 3
+
+/* process mask bits (Table 2) */
+#define EMX_M_COMPTON 1u
+#define EMX_M_PHOTO 2u
+#define EMX_M_PAIR 4u
+#define EMX_M_IONI 8u   /* Moller + Bhabha */
+#define EMX_M_BREMS 16u
+#define EMX_M_ANNIH 32u
+
+/* process ids (interaction counters, step results) */
+#define EMX_P_COMPTON 0
+#define EMX_P_PHOTO 1
+#define EMX_P_PAIR 2
+#define EMX_P_MOLLER 3
+#define EMX_P_BHABHA 4
+#define EMX_P_BREMS 5
+#define EMX_P_ANNIH 6
+#define EMX_P_REST 7 /* e+ annihilation at rest */
+#define EMX_NPROC 8
+
+/* what limited the step */
+#define EMX_A_NONE 0
+#define EMX_A_DISCRETE 1
+#define EMX_A_LOSS 2
+#define EMX_A_BOUNDARY 3
+#define EMX_A_TRUNC 4 /* vacuum step cap / field substeps exhausted */
+
+/* table kinds per material, each n_E doubles on the log grid */
+#define EMX_T_COMPTON 0
+#define EMX_T_PHOTO 1
+#define EMX_T_PAIR 2
+#define EMX_T_MOLLER 3
+#define EMX_T_BREMS_EM 4
+#define EMX_T_DEDX_EM 5
+#define EMX_T_RANGE_EM 6
+#define EMX_T_BHABHA 7
+#define EMX_T_BREMS_EP 8
+#define EMX_T_ANNIH 9
+#define EMX_T_DEDX_EP 10
+#define EMX_T_RANGE_EP 11
+#define EMX_T_PAIR_ELEM0 12 /* + element index: n_i * sigma_pair(Z_i) for element selection */
+#define EMX_NTABLE (EMX_T_PAIR_ELEM0 + EMX_MAX_ELEM)
+
+typedef struct emx_problem emx_problem; /* opaque, owned by the library */
+
+/* physics switches and numerical parameters (PAPER.md:114 ii, iii, vi; PAPER.md:236 cutoffs).
+ * emx_create() fills in the defaults quoted in DESIGN.md (R9, R14). */
+typedef struct {
+    uint32_t process_mask;      /* EMX_M_* */
+    double E_min, E_max;        /* energy grid, MeV */
+    int32_t n_E;                /* grid points, >= 2 */
+    double E_trk;               /* tracking cut, MeV */
+    double prod_cut_cm;         /* > 0: derive per-material production thresholds from this length */
+    double alpha_R, rho_R;      /* continuous-loss step function (rho_R in cm) */
+    double lin_loss;            /* linear-loss limit as a fraction of E */
+    double field_eps;           /* cm: RK4 local error and boundary landing tolerance */
+    int32_t max_substeps;       /* field substep attempts per step */
+    double vacuum_step;         /* cm: step cap in vacuum */
+    int32_t max_steps;          /* per track; then the track is killed into looper_lost */
+    int32_t deposit_e_at_creation; /* 1: every e- is deposited where it is born (BASELINE configs[0]) */
+} emx_physics;
+
+/* run totals (PAPER.md:176 energy deposition; Fig. 5 diagnostics PAPER.md:204-212) */
+typedef struct {
+    double escaped, below_cut, looper, E_in; /* MeV */
+    uint64_t steps[3];                       /* track-steps by particle type */
+    uint64_t tracks[3];                      /* tracks created by particle type (primaries included) */
+    uint64_t inter[EMX_NPROC];               /* discrete interactions by process id */
+    uint64_t null_int;                       /* kinematically impossible (null) interactions */
+    uint64_t track_steps;                    /* sum of steps[] */
+    uint64_t stalls;                         /* steps re-executed because the secondary stack was full */
+    uint64_t iterations;                     /* step iterations of the loop */
+    uint64_t peak_live, peak_queue;          /* max tracks in flight / queued initializers */
+} emx_scalars;
+
+/* one track, array-of-structures form used only by the level-2 parity hook emx_step_batch */
+typedef struct {
+    double x[3], u[3], E;
+    uint64_t tid;
+    uint32_t prim, step;
+    int32_t vol, surf, ptype, alive;
+} emx_track;
+
+/* everything one step produces (emx_step_batch output) */
+typedef struct {
+    emx_track trk;          /* updated track, alive = 0 if killed */
+    int32_t action;         /* EMX_A_* */
+    int32_t process;        /* EMX_P_* or -1 */
+    int32_t n_sec;
+    emx_track sec[4];       /* allocated secondaries in ordinal order */
+    int32_t sec_ord[4];
+    double edep;            /* MeV deposited, belongs to cell edep_vol */
+    int32_t edep_vol;
+    double below_cut;       /* part of edep from tracking-cut kills / births */
+    double escaped, looper;
+    double s;               /* step length travelled, cm */
+    int32_t n_draws;        /* uniforms consumed */
+    int32_t null_int;
+    int32_t rest;           /* e+ annihilated at rest in this step */
+} emx_step_result;
+
+/* ---- problem description (host side; arrays are HOST pointers, copied during the call) ---- */
+
+/* New problem with default physics.  *out receives the handle. */
+int emx_create(emx_problem **out);
+void emx_destroy(emx_problem *p);
+
+/* Material (PAPER.md:114 i "material-dependent physical properties"): n_elem <= EMX_MAX_ELEM elements
+ * with atomic number Z, molar mass A (g/mol) and mass fraction; density g/cm3; mean excitation energy in
+ * eV (> 0).  Returns the material id (>= 0); vacuum is material -1 and is never added. */
+int emx_add_material(emx_problem *p, int n_elem, const int *Z, const double *A, const double *mass_frac,
+                     double density_g_cm3, double mean_exc_energy_eV);
+
+/* Surface: type EMX_S_*, value = plane position or cylinder radius (cm).  Returns its id. */
+int emx_add_surface(emx_problem *p, int type, double value_cm);
+
+/* Cell = conjunction of n_faces <= EMX_MAX_FACES half-spaces (surface id, sense -1: f < 0 side, +1: f > 0
+ * side); material id or -1 (vacuum); tally id or -1 (not scored).  Cells must tile the world without
+ * overlap; leaving every cell = escape.  Returns the cell id. */
+int emx_add_volume(emx_problem *p, int n_faces, const int *surf, const int *sense, int material, int tally);
+
+/* Uniform magnetic field in tesla; all zero = no field. */
+int emx_set_field(emx_problem *p, double Bx_T, double By_T, double Bz_T);
+
+int emx_get_physics(const emx_problem *p, emx_physics *out);
+int emx_set_physics(emx_problem *p, const emx_physics *ph);
+
+/* Explicit production thresholds (MeV) for one material instead of the cut-length conversion. */
+int emx_set_cuts(emx_problem *p, int material, double Tcut_MeV, double kcut_MeV);
+
+/* ---- tables (BASELINE configs[0] "tabulated from closed forms") ---- */
+
+/* Runs the table-builder kernels on `stream`, uploads geometry, and synchronises the stream. */
+int emx_build_tables(emx_problem *p, void *stream);
+
+/* Copies one table (n == n_E doubles) of a material to HOST memory. */
+int emx_get_table(const emx_problem *p, int material, int kind, double *host_out, int n);
+
+/* host_out8 = { n_e [1/cm3], I [MeV], plasma energy [MeV], X0 [cm], Tcut [MeV], kcut [MeV], rho, n_elem } */
+int emx_get_material_info(const emx_problem *p, int material, double *host_out8);
+
+int emx_n_tally(const emx_problem *p);
+
+/* ---- transport ---- */
+
+/* Bytes of caller-provided DEVICE workspace for a track store of n_slots and secondary stacks holding
+ * queue_capacity records in total.  0 on invalid arguments. */
+size_t emx_workspace_bytes(const emx_problem *p, long n_slots, long queue_capacity);
+
+/* Transport n_primaries primaries to completion.  ptype[n], E[n] (MeV), pos3[3n], dir3[3n] (unit vectors),
+ * start_vol[n] (cell ids), start_surf[n] (surface the primary sits on or -1; may be NULL = all -1) are
+ * DEVICE pointers in array-of-xyz layout; they are read, never written.  `workspace` is a DEVICE buffer of
+ * at least emx_workspace_bytes() bytes, 256-byte aligned, owned by the caller; its contents are
+ * overwritten.  Work is enqueued on `stream`; the call returns after the loop has finished and the run
+ * totals are on the host (the loop itself is device-driven; the host waits once at the end).
+ * Tallies accumulate in the problem's device block until emx_reset_tallies(). */
+int emx_transport(emx_problem *p, long n_primaries, const int *ptype, const double *E, const double *pos3,
+                  const double *dir3, const int *start_vol, const int *start_surf, uint64_t seed,
+                  long n_slots, long queue_capacity, void *workspace, size_t workspace_bytes, void *stream);
+
+/* Same call with every primary array in HOST memory (pageable or pinned): uploads on `stream`,
+ * transports, and leaves the tallies readable.  This is the end-to-end entry bench.py times as `e2e`. */
+int emx_transport_host(emx_problem *p, long n_primaries, const int *ptype, const double *E,
+                       const double *pos3, const double *dir3, const int *start_vol, const int *start_surf,
+                       uint64_t seed, long n_slots, long queue_capacity, void *workspace,
+                       size_t workspace_bytes, void *stream);
+
+int emx_reset_tallies(emx_problem *p, void *stream);
+
+/* edep_host[n_tally] (MeV per tally id) and the run totals, copied to HOST memory. */
+int emx_read_tallies(const emx_problem *p, double *edep_host, emx_scalars *out);
+
+/* Milliseconds the last emx_transport spent between its first launch and the end of the loop,
+ * measured with CUDA events on the caller's stream; < 0 if none. */
+double emx_last_transport_ms(const emx_problem *p);
+
+/* Per-iteration diagnostics of the last transport (Fig. 5): up to `max_iter` rows of
+ * { live tracks, queued initializers } as uint32 pairs in HOST memory; returns rows written. */
+long emx_get_iteration_log(const emx_problem *p, uint32_t *host_out, long max_iter);
+
+/* ---- parity hooks ---- */
+
+/* Level-2 parity hook: one step of each of n tracks with the same device step function the loop uses.
+ * in[n] and out[n] are DEVICE pointers (AoS). */
+int emx_step_batch(emx_problem *p, uint64_t seed, long n, const emx_track *in, emx_step_result *out,
+                   void *stream);
+
+/* Level-1 parity hooks (integer work).  All pointers DEVICE.
+ * emx_philox_batch: out[4i..4i+3] = Philox4x32-10(ctr[4i..], key[2i..]).
+ * emx_draw_batch:   u[i] = draw number n[i] of (seed, prim[i], tid[i], step[i]); child[i] = child track id
+ *                   for ordinal n[i] (either output may be NULL). */
+int emx_philox_batch(long n, const uint32_t *ctr4, const uint32_t *key2, uint32_t *out4, void *stream);
+int emx_draw_batch(uint64_t seed, long n, const uint32_t *prim, const uint64_t *tid, const uint32_t *step,
+                   const uint32_t *nn, double *u, uint64_t *child, void *stream);
+
+/* Level-1 hook for the refill / compaction step: applies one refill pass to a pool
+ * of `n_live` slots whose alive flags are alive[n_live] (uint8, DEVICE) with `n_queue` queued records and
+ * room for `capacity` slots, and writes, for every slot index < new_n_live, src[i] (int32, DEVICE,
+ * capacity entries): -1 = untouched live track, q >= 0 = filled from queue record q,
+ * -2 - j = moved from slot j.  counts_host[3] = { new_n_live, new_n_queue, n_moved }. */
+int emx_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
+                    long *counts_host, void *stream);
+
+const char *emx_last_error(const emx_problem *p);
+const char *emx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EMX_H */

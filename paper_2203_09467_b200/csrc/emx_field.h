@@ -1,0 +1,110 @@
+// emx_field.h -- charged-track propagation in a uniform magnetic field (step A5 of DESIGN.md).
+// PAPER.md:144 "on-device propagation of particles through arbitrary magnetic fields ... different
+// integration algorithms"; BASELINE.json configs[3]: "adaptive RK4 (1e-6 mm miss-distance tolerance)".
+// Algorithm (C9): classical RK4 with step doubling for the local error, plus a chord /
+// secant search for the boundary landing point.  y = (x, u), dy/ds = (u, kappa u x Bhat).
+#pragma once
+#include "emx_core.h"
+#include "emx_geom.h"
+
+namespace emx {
+
+EMX_HD Vec3 lorentz(const Vec3 &u, double kappa, const double B[3]) {
+    return {kappa * (u.y * B[2] - u.z * B[1]), kappa * (u.z * B[0] - u.x * B[2]), kappa * (u.x * B[1] - u.y * B[0])};
+}
+
+// one classical RK4 step of length h.  dx/ds = u, so the x-stages are the u-stage arguments.
+EMX_HD void rk4_step(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, Vec3 &xo, Vec3 &uo) {
+    const Vec3 k1u = lorentz(u, kappa, B);
+    const Vec3 u2 = u + (0.5 * h) * k1u;
+    const Vec3 k2u = lorentz(u2, kappa, B);
+    const Vec3 u3 = u + (0.5 * h) * k2u;
+    const Vec3 k3u = lorentz(u3, kappa, B);
+    const Vec3 u4 = u + h * k3u;
+    const Vec3 k4u = lorentz(u4, kappa, B);
+    const double h6 = h / 6.0;
+    xo.x = x.x + h6 * (u.x + 2.0 * u2.x + 2.0 * u3.x + u4.x);
+    xo.y = x.y + h6 * (u.y + 2.0 * u2.y + 2.0 * u3.y + u4.y);
+    xo.z = x.z + h6 * (u.z + 2.0 * u2.z + 2.0 * u3.z + u4.z);
+    uo.x = u.x + h6 * (k1u.x + 2.0 * k2u.x + 2.0 * k3u.x + k4u.x);
+    uo.y = u.y + h6 * (k1u.y + 2.0 * k2u.y + 2.0 * k3u.y + k4u.y);
+    uo.z = u.z + h6 * (k1u.z + 2.0 * k2u.z + 2.0 * k3u.z + k4u.z);
+}
+
+// one step of h against two of h/2: err = |x_full - x_half|, result = half-step state, u renormalised
+EMX_HD void rk4_doubling(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, Vec3 &x1, Vec3 &u1,
+                         double &err) {
+    Vec3 xf, uf, xm, um;
+    rk4_step(x, u, kappa, B, h, xf, uf);
+    rk4_step(x, u, kappa, B, 0.5 * h, xm, um);
+    rk4_step(xm, um, kappa, B, 0.5 * h, x1, u1);
+    err = norm(xf - x1);
+    const double n = norm(u1);
+    u1.x /= n;
+    u1.y /= n;
+    u1.z /= n;
+}
+
+// Propagate up to s_max inside cell `vol`.  Returns the arc length travelled; hit = surface reached
+// (-1 none).  x, u are updated; on_surf is the surface the track starts on.
+EMX_HD double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
+                              int &hit) {
+    const double eps = P.ph.field_eps;
+    double s_done = 0.0;
+    int surf = on_surf;
+    double h = 0.25 / fabs(kappa);
+    if (s_max < h) h = s_max;
+    hit = -1;
+    const int max_attempts = P.ph.max_substeps;
+    for (int attempt = 0; attempt < max_attempts; ++attempt) {
+        const double rem = s_max - s_done;
+        if (h > rem) h = rem;
+        Vec3 x1, u1;
+        double err;
+        rk4_doubling(x, u, kappa, P.Bhat, h, x1, u1, err);
+        if (err > eps && h > 1e-9) {  // too inaccurate: shrink and retry
+            const double f = 0.9 * pow(eps / err, 0.2);
+            h *= (f > 0.2 ? f : 0.2);
+            continue;
+        }
+        const Vec3 c = x1 - x;
+        const double L = norm(c);
+        if (!(L > 0.0)) {
+            s_done += h;
+            break;
+        }
+        const Vec3 cd = {c.x / L, c.y / L, c.z / L};
+        int S;
+        const double d = distance_to_boundary(P, vol, x, cd, surf, S);
+        if (d <= eps) {
+            // chord bends back across the surface the track sits on: shorten and retry
+            if (d == 0.0 && S == surf && h > 1e-9) {
+                h *= 0.5;
+                continue;
+            }
+            hit = S;  // immediate (re-)crossing, nothing more travelled
+            return s_done;
+        }
+        if (d > L) {  // chord stays inside the cell: accept
+            x = x1;
+            u = u1;
+            s_done += h;
+            surf = -1;
+            if (s_done >= s_max * (1.0 - 1e-14)) break;
+            const double e = err > eps / 3125.0 ? err : eps / 3125.0;
+            const double f = 0.9 * pow(eps / e, 0.2);
+            h *= (f < 5.0 ? f : 5.0);
+            continue;
+        }
+        if (L - d <= eps) {  // landed on S within tolerance
+            x = x1;
+            u = u1;
+            hit = S;
+            return s_done + h;
+        }
+        h *= d / L;  // secant: aim the chord end at S
+    }
+    return s_done;
+}
+
+}  // namespace emx

@@ -1,0 +1,249 @@
+// emx_interact.h -- the six discrete interactors of PAPER.md:110-111 (Table 2): Klein-Nishina Compton,
+// photoelectric, Bethe-Heitler pair production, bremsstrahlung, Moller / Bhabha ionisation and
+// two-photon annihilation (step A7 of DESIGN.md).  The paper names the models only; the samplers are
+// the readings of DESIGN.md C6.  Uniforms are consumed strictly in the order written there.
+#pragma once
+#include "emx_core.h"
+#include "emx_xs.h"
+
+namespace emx {
+
+EMX_HD void normalise(Vec3 &v, const Vec3 &fallback) {
+    const double n = norm(v);
+    if (n > 0.0) {
+        v.x /= n;
+        v.y /= n;
+        v.z /= n;
+    } else {
+        v = fallback;
+    }
+}
+
+EMX_HD void sincos_(double a, double &s, double &c) {
+#if defined(__CUDA_ARCH__)
+    sincos(a, &s, &c);
+#else
+    s = sin(a);
+    c = cos(a);
+#endif
+}
+
+// rotate u by polar cosine mu (sine s) and azimuth (cphi, sphi) -- C6 "Common"
+EMX_HD Vec3 rotate(const Vec3 &u, double mu, double s, double cphi, double sphi) {
+    Vec3 o;
+    const double rho2 = u.x * u.x + u.y * u.y;
+    if (rho2 > 1e-30) {
+        const double rho = sqrt(rho2);
+        o.x = u.x * mu + s * (u.x * u.z * cphi - u.y * sphi) / rho;
+        o.y = u.y * mu + s * (u.y * u.z * cphi + u.x * sphi) / rho;
+        o.z = u.z * mu - s * rho * cphi;
+    } else {
+        o.x = s * cphi;
+        o.y = s * sphi;
+        o.z = (u.z > 0.0 ? mu : -mu);
+    }
+    normalise(o, u);
+    return o;
+}
+EMX_HD Vec3 rotate_mu_phi(const Vec3 &u, double mu, double phi) {
+    double sp, cp;
+    sincos_(phi, sp, cp);
+    return rotate(u, mu, sqrt((1.0 - mu) * (1.0 + mu)), cp, sp);
+}
+
+EMX_HD double beta_of(double T) { return sqrt(T * (T + 2.0 * kMe)) / (T + kMe); }
+EMX_HD double clamp1(double m) { return m > 1.0 ? 1.0 : (m < -1.0 ? -1.0 : m); }
+// exact inverse CDF of p(mu) ~ (1 - beta mu)^-2 (R30)
+EMX_HD double boosted_iso(double xi, double beta) { return clamp1((2.0 * xi - 1.0 + beta) / (beta * (2.0 * xi - 1.0) + 1.0)); }
+
+// ---- Compton, Klein-Nishina (C6.1): photon E -> E1 along u1, electron Te along ue
+EMX_HD void compton(Rng &r, double E, const Vec3 &u, double &E1, Vec3 &u1, double &Te, Vec3 &ue) {
+    const double k = E / kMe;
+    const double e0 = 1.0 / (1.0 + 2.0 * k);
+    const double a1 = -log(e0), a2 = 0.5 * (1.0 - e0 * e0);
+    double eps, t;
+    for (;;) {
+        const double x1 = r.next(), x2 = r.next(), x3 = r.next();
+        if (x1 * (a1 + a2) < a1) eps = exp(-a1 * x2);
+        else eps = sqrt(e0 * e0 + (1.0 - e0 * e0) * x2);
+        t = (1.0 - eps) / (k * eps);
+        if (x3 <= 1.0 - eps * t * (2.0 - t) / (1.0 + eps * eps)) break;
+    }
+    const double mu = 1.0 - t;
+    const double s2 = t * (2.0 - t);
+    const double s = s2 > 0.0 ? sqrt(s2) : 0.0;
+    double sp, cp;
+    sincos_(2.0 * kPi * r.next(), sp, cp);
+    u1 = rotate(u, mu, s, cp, sp);
+    E1 = eps * E;
+    Te = E - E1;
+    ue = E * u - E1 * u1;
+    normalise(ue, u);
+}
+
+// ---- photoelectron direction, leading Sauter term p(mu) ~ (1 - mu^2) / (1 - beta mu)^4 (C6.2)
+EMX_HD Vec3 photo_dir(Rng &r, double E, const Vec3 &u) {
+    const double g = E / kMe + 1.0;
+    const double b = beta_of(E);
+    const double A = 1.0 / (g * g * b * (1.0 + b));
+    double nu;
+    for (;;) {
+        const double x1 = r.next(), x2 = r.next();
+        nu = 1.0 / (1.0 / A - x1 * (1.0 / A - 1.0 / (A + 2.0))) - A;
+        if (x2 <= A * (2.0 + A) * nu * (2.0 - nu) / ((A + nu) * (A + nu))) break;
+    }
+    const double s2 = nu * (2.0 - nu);
+    double sp, cp;
+    sincos_(2.0 * kPi * r.next(), sp, cp);
+    return rotate(u, 1.0 - nu, s2 > 0.0 ? sqrt(s2) : 0.0, cp, sp);
+}
+
+// ---- Bethe-Heitler pair production on element Z (C6.3).  false = null interaction.
+EMX_HD double pair_F1(double d, double F) {
+    double a, b;
+    screening(d, a, b);
+    return 3.0 * a - b - F;
+}
+EMX_HD double pair_F2(double d, double F) {
+    double a, b;
+    screening(d, a, b);
+    return 1.5 * a + 0.5 * b - F;
+}
+EMX_HD bool pair_production(Rng &r, int Z, double E, const Vec3 &u, double &Tm, Vec3 &um, double &Tp, Vec3 &up) {
+    const double e0 = kMe / E;
+    const double c = 136.0 * pow((double)Z, -1.0 / 3.0) * e0;
+    const double F = pair_F(Z, E);
+    const double dmin = 4.0 * c;
+    const double dmax = exp((42.24 - F) / 8.368) - 0.952;
+    if (!(E > 2.0 * kMe) || dmin >= dmax) return false;
+    const double e1 = 0.5 - 0.5 * sqrt(1.0 - dmin / dmax);
+    const double emin = e0 > e1 ? e0 : e1;
+    const double F10 = pair_F1(dmin, F), F20 = pair_F2(dmin, F);
+    const double N1 = (0.5 - emin) * (0.5 - emin) * F10, N2 = 1.5 * F20;
+    double eps;
+    for (;;) {
+        const double x1 = r.next(), x2 = r.next(), x3 = r.next();
+        if (x1 * (N1 + N2) < N1) {
+            eps = 0.5 - (0.5 - emin) * cbrt(x2);
+            if (x3 * F10 <= pair_F1(c / (eps * (1.0 - eps)), F)) break;
+        } else {
+            eps = emin + (0.5 - emin) * x2;
+            if (x3 * F20 <= pair_F2(c / (eps * (1.0 - eps)), F)) break;
+        }
+    }
+    const double x4 = r.next();
+    const double ee = (x4 < 0.5) ? eps : 1.0 - eps;  // the electron's share
+    double tm = ee * E - kMe;
+    if (tm < 0.0) tm = 0.0;
+    double tp = E - tm - 2.0 * kMe;
+    if (tp < 0.0) tp = 0.0;
+    Tm = tm;
+    Tp = tp;
+    const double mum = boosted_iso(r.next(), beta_of(tm));
+    const double mup = boosted_iso(r.next(), beta_of(tp));
+    double sp, cp;
+    sincos_(2.0 * kPi * r.next(), sp, cp);
+    um = rotate(u, mum, sqrt((1.0 - mum) * (1.0 + mum)), cp, sp);
+    up = rotate(u, mup, sqrt((1.0 - mup) * (1.0 + mup)), -cp, -sp);
+    return true;
+}
+
+// ---- bremsstrahlung, complete-screening shape (C6.4).  false = null (T <= kc).
+EMX_HD bool bremsstrahlung(Rng &r, double T, double kc, const Vec3 &u, double &k, Vec3 &ug, double &T1, Vec3 &u1) {
+    if (!(T > kc)) return false;
+    const double lr = log(T / kc);
+    double kk;
+    for (;;) {
+        const double x1 = r.next(), x2 = r.next();
+        kk = kc * exp(x1 * lr);
+        if (kk > T) kk = T;
+        const double y = kk / T;
+        if ((4.0 / 3.0) * x2 <= 4.0 / 3.0 - 4.0 * y / 3.0 + y * y) break;
+    }
+    const double mu = boosted_iso(r.next(), beta_of(T));
+    ug = rotate_mu_phi(u, mu, 2.0 * kPi * r.next());
+    const double p = sqrt(T * (T + 2.0 * kMe));
+    k = kk;
+    T1 = T - kk;
+    u1 = p * u - kk * ug;
+    normalise(u1, u);
+    return true;
+}
+
+// exact two-body kinematics of a knock-on electron of energy Td on a free electron at rest (C6.5)
+EMX_HD void knock_on(Rng &r, double T, double Td, const Vec3 &u, Vec3 &ud, double &T1, Vec3 &u1) {
+    const double p = sqrt(T * (T + 2.0 * kMe)), pd = sqrt(Td * (Td + 2.0 * kMe));
+    const double mu = clamp1(Td * (T + 2.0 * kMe) / (p * pd));
+    ud = rotate_mu_phi(u, mu, 2.0 * kPi * r.next());
+    T1 = T - Td;
+    u1 = p * u - pd * ud;
+    normalise(u1, u);
+}
+
+EMX_HD bool moller(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec3 &ud, double &T1, Vec3 &u1) {
+    if (!(T > 2.0 * Tcut)) return false;
+    const double x = Tcut / T, g = T / kMe + 1.0, g2 = g * g;
+    const double c = (2.0 * g - 1.0) / g2, a = (g - 1.0) * (g - 1.0) / g2;
+    const double whalf = 0.25 * (a + 8.0 - 4.0 * c);
+    double eps;
+    for (;;) {
+        const double x1 = r.next(), x2 = r.next();
+        eps = x / (1.0 - x1 * (1.0 - 2.0 * x));
+        const double w = eps * eps * (a + (1.0 / eps) * (1.0 / eps - c) + (1.0 / (1.0 - eps)) * (1.0 / (1.0 - eps) - c));
+        if (x2 * whalf <= w) break;
+    }
+    Td = eps * T;
+    knock_on(r, T, Td, u, ud, T1, u1);
+    return true;
+}
+
+EMX_HD bool bhabha(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec3 &ud, double &T1, Vec3 &u1) {
+    if (!(T > Tcut)) return false;
+    const double x = Tcut / T, g = T / kMe + 1.0, b2 = 1.0 - 1.0 / (g * g);
+    const double y = 1.0 / (g + 1.0), t = 1.0 - 2.0 * y;
+    const double B1 = 2.0 - y * y, B2 = t * (3.0 + y * y), B4 = t * t * t, B3 = t * t + B4;
+    double eps;
+    for (;;) {
+        const double x1 = r.next(), x2 = r.next();
+        eps = x / (1.0 - x1 * (1.0 - x));
+        if (x2 <= 1.0 - b2 * (B1 * eps - B2 * eps * eps + B3 * eps * eps * eps - B4 * eps * eps * eps * eps)) break;
+    }
+    Td = eps * T;
+    knock_on(r, T, Td, u, ud, T1, u1);
+    return true;
+}
+
+// ---- two-photon annihilation in flight, Heitler (C6.6)
+EMX_HD void annih_flight(Rng &r, double T, const Vec3 &u, double &k1, Vec3 &u1, double &k2, Vec3 &u2) {
+    const double g = T / kMe + 1.0;
+    const double rr = sqrt((g - 1.0) / (g + 1.0));
+    const double elo = 0.5 * (1.0 - rr), ehi = 0.5 * (1.0 + rr);
+    const double lr = log(ehi / elo);
+    double eps;
+    for (;;) {
+        const double x1 = r.next(), x2 = r.next();
+        eps = elo * exp(x1 * lr);
+        if (x2 <= 1.0 - eps + (2.0 * g * eps - 1.0) / (eps * (g + 1.0) * (g + 1.0))) break;
+    }
+    const double Etot = T + 2.0 * kMe;
+    const double kk = eps * Etot;
+    const double mu = clamp1((eps * (g + 1.0) - 1.0) / (eps * sqrt(g * g - 1.0)));
+    u1 = rotate_mu_phi(u, mu, 2.0 * kPi * r.next());
+    const double p = sqrt(T * (T + 2.0 * kMe));
+    k1 = kk;
+    k2 = Etot - kk;
+    u2 = p * u - kk * u1;
+    normalise(u2, u);
+}
+
+// ---- annihilation at rest: two back-to-back me photons, isotropic (C6.6, R12/R25)
+EMX_HD void annih_rest(Rng &r, Vec3 &u1, Vec3 &u2) {
+    const double mu = 2.0 * r.next() - 1.0;
+    double sp, cp;
+    sincos_(2.0 * kPi * r.next(), sp, cp);
+    const double s = sqrt((1.0 - mu) * (1.0 + mu));
+    u1 = {s * cp, s * sp, mu};
+    u2 = {-u1.x, -u1.y, -u1.z};
+}
+
+}  // namespace emx
