@@ -26,7 +26,7 @@ constexpr double kAlpha = 7.2973525693e-3;  // fine-structure constant
 constexpr double kNa = 6.02214076e23;       // Avogadro, 1/mol
 constexpr double kCB = 2.99792458e-3;       // curvature [1/cm] = q * kCB * B[T] / p[MeV/c]
 constexpr double kPi = 3.14159265358979323846;
-constexpr double kInf = 1e300 * 1e300;      // +inf without <limits> in device code
+constexpr double kInf = __builtin_huge_val(); // +inf
 
 enum : int { kGamma = 0, kElectron = 1, kPositron = 2 };
 

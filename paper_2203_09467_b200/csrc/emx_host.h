@@ -1,0 +1,103 @@
+// emx_host.h -- host-side problem description behind the C-ABI (include/emx.h): materials, surfaces,
+// cells, field and physics switches (the inputs PAPER.md:235-237 lists), plus the derived quantities that
+// are computed once on the host: material constants (C3), grid constants (C4) and the
+// per-surface neighbour candidate lists used by emx_geom.h.
+#pragma once
+#include <string>
+#include <vector>
+#include "emx_core.h"
+#include "emx_xs.h"
+
+namespace emx {
+
+struct HostProblem {
+    std::vector<Material> mat;
+    std::vector<int> surf_type;
+    std::vector<double> surf_v;
+    std::vector<Volume> vol;
+    emx_physics ph;
+    double B[3] = {0.0, 0.0, 0.0};
+    int n_tally = 0;
+    bool built = false;
+    std::string err;
+
+    HostProblem() {
+        ph.process_mask = 63u;
+        ph.E_min = 1e-3;
+        ph.E_max = 1e4;
+        ph.n_E = 256;
+        ph.E_trk = 1e-3;
+        ph.prod_cut_cm = 0.07;
+        ph.alpha_R = 0.2;   // R9
+        ph.rho_R = 0.1;     // R9
+        ph.lin_loss = 0.01; // R9
+        ph.field_eps = 1e-7;   // R14: 1e-6 mm
+        ph.max_substeps = 1000;
+        ph.vacuum_step = 1e3;
+        ph.max_steps = 10000;
+        ph.deposit_e_at_creation = 0;
+    }
+};
+
+// material constants of C3: number densities, electron density, plasma energy, radiation length
+inline bool derive_material(Material &m, int n_elem, const int *Z, const double *A, const double *w, double rho,
+                            double I_eV) {
+    if (n_elem < 1 || n_elem > EMX_MAX_ELEM || !(rho > 0.0) || !(I_eV > 0.0)) return false;
+    m = Material();
+    m.n_elem = n_elem;
+    m.rho = rho;
+    m.I = I_eV * 1e-6;
+    m.n_e = 0.0;
+    double invX0 = 0.0;
+    for (int i = 0; i < EMX_MAX_ELEM; ++i) {
+        m.Z[i] = 0;
+        m.A[i] = m.w[i] = m.n_i[i] = 0.0;
+    }
+    for (int i = 0; i < n_elem; ++i) {
+        if (Z[i] < 1 || !(A[i] > 0.0) || !(w[i] >= 0.0)) return false;
+        m.Z[i] = Z[i];
+        m.A[i] = A[i];
+        m.w[i] = w[i];
+        m.n_i[i] = rho * kNa * w[i] / A[i];
+        m.n_e += m.n_i[i] * Z[i];
+        invX0 += rho * w[i] / X0_element(Z[i], A[i]);
+    }
+    m.X0 = 1.0 / invX0;
+    m.hwp = (kMe / kAlpha) * sqrt(4.0 * kPi * m.n_e * kRe * kRe * kRe);
+    m.Tcut = -1.0;
+    m.kcut = -1.0;
+    return true;
+}
+
+// nb_off[2 S + (sense > 0)] .. nb_off[2 S + (sense > 0) + 1]: cells listing (S, sense), ascending id
+inline void build_neighbour_lists(const HostProblem &hp, std::vector<int> &off, std::vector<int> &list) {
+    const int ns = (int)hp.surf_type.size();
+    off.assign(2 * ns + 1, 0);
+    list.clear();
+    for (int k = 0; k < 2 * ns; ++k) {
+        const int S = k / 2, sense = (k & 1) ? 1 : -1;
+        off[k] = (int)list.size();
+        for (int c = 0; c < (int)hp.vol.size(); ++c) {
+            const Volume &v = hp.vol[c];
+            for (int i = 0; i < v.n_faces; ++i)
+                if (v.surf[i] == S && v.sense[i] == sense) {
+                    list.push_back(c);
+                    break;
+                }
+        }
+    }
+    off[2 * ns] = (int)list.size();
+}
+
+struct GridConsts {
+    double lnE0, dlnE, inv_dlnE;
+};
+inline GridConsts grid_consts(const emx_physics &ph) {
+    GridConsts g;
+    g.lnE0 = log(ph.E_min);
+    g.dlnE = log(ph.E_max / ph.E_min) / (ph.n_E - 1);
+    g.inv_dlnE = (ph.n_E - 1) / log(ph.E_max / ph.E_min);
+    return g;
+}
+
+}  // namespace emx
