@@ -1,0 +1,35 @@
+// emx_kernels.h -- launchers of the CUDA kernels (emx_kernels.cu, emx_transport.cu), called by emx_api.cu.
+#pragma once
+#include <cuda_runtime.h>
+#include "emx_core.h"
+#include "emx_work.h"
+
+namespace emx {
+
+struct TableCtx;
+
+cudaError_t launch_build_tables(const TableCtx &c, cudaStream_t st);
+cudaError_t launch_step_batch(const Params &P, uint64_t seed, long n, const emx_track *in, emx_step_result *out,
+                              cudaStream_t st);
+cudaError_t launch_philox_batch(long n, const uint32_t *ctr, const uint32_t *key, uint32_t *out, cudaStream_t st);
+cudaError_t launch_draw_batch(uint64_t seed, long n, const uint32_t *prim, const uint64_t *tid, const uint32_t *step,
+                              const uint32_t *nn, double *u, uint64_t *child, cudaStream_t st);
+
+// primaries in DEVICE memory (AoS xyz as in include/emx.h)
+struct Primaries {
+    long n;
+    const int *ptype;
+    const double *E, *pos3, *dir3;
+    const int *vol, *surf;  // surf may be null
+};
+
+// resets the control block and pushes every primary onto the stack of its type (lowest index on top)
+cudaError_t launch_load_primaries(const Work &w, const Primaries &pr, cudaStream_t st);
+// one iteration of the loop: refill (plan, fill, move) then step; tally = device edep array
+cudaError_t launch_iteration(const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st);
+// level-1 hook: the refill index logic alone on a caller-supplied alive[] (see include/emx.h)
+cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
+                               int *scratch, cudaStream_t st);
+size_t refill_plan_scratch_ints(long capacity);
+
+}  // namespace emx

@@ -1,0 +1,557 @@
+// emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the fused
+// per-type step kernel (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
+//
+// One ITERATION = k_plan -> k_fill -> k_move -> k_step<gamma|e-|e+>.  Nothing returns to the host
+// between iterations: pool sizes, stack tops and the done flag live in the device control block.
+#include <cuda_runtime.h>
+#include "emx_kernels.h"
+#include "emx_step.h"
+
+namespace emx {
+
+__device__ __forceinline__ void load_record(const QueueSoA &q, int r, const TrackSoA &t, int i) {
+    t.x[i] = q.x[r];
+    t.y[i] = q.y[r];
+    t.z[i] = q.z[r];
+    t.ux[i] = q.ux[r];
+    t.uy[i] = q.uy[r];
+    t.uz[i] = q.uz[r];
+    t.E[i] = q.E[r];
+    t.tid[i] = q.tid[r];
+    t.prim[i] = q.prim[r];
+    t.step[i] = 0u;
+    t.vol[i] = q.vol[r];
+    t.surf[i] = q.surf[r];
+    t.alive[i] = 2;  // 2 = filled in this refill pass (k_move still ranks it as a hole)
+}
+
+__device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
+    t.x[to] = t.x[from];
+    t.y[to] = t.y[from];
+    t.z[to] = t.z[from];
+    t.ux[to] = t.ux[from];
+    t.uy[to] = t.uy[from];
+    t.uz[to] = t.uz[from];
+    t.E[to] = t.E[from];
+    t.tid[to] = t.tid[from];
+    t.prim[to] = t.prim[from];
+    t.step[to] = t.step[from];
+    t.vol[to] = t.vol[from];
+    t.surf[to] = t.surf[from];
+    t.alive[to] = 2;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Primaries -> stacks.  One block; primaries of each type keep ascending index order from the top of
+// their stack downwards, so they enter the pools in ascending order and only after every secondary above
+// them has been consumed (R8).
+__global__ void __launch_bounds__(1024) k_load_primaries(Work w, Primaries pr) {
+    __shared__ int s_cnt[3][32];
+    __shared__ int s_total[3], s_base[3];
+    __shared__ double s_E[32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    Ctl *c = w.ctl;
+    if (tid == 0) {
+        Ctl z = Ctl();
+        *c = z;
+    }
+    // pass 1: totals per type and the injected energy
+    int cnt[3] = {0, 0, 0};
+    double ein = 0.0;
+    for (long i = tid; i < pr.n; i += blockDim.x) {
+        const int pt = pr.ptype[i];
+        cnt[0] += (pt == 0);
+        cnt[1] += (pt == 1);
+        cnt[2] += (pt == 2);
+        ein += pr.E[i] + (pt == kPositron ? 2.0 * kMe : 0.0);
+    }
+    for (int p = 0; p < 3; ++p) {
+        int v = cnt[p];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) s_cnt[p][wid] = v;
+    }
+    for (int o = 16; o > 0; o >>= 1) ein += __shfl_down_sync(0xffffffffu, ein, o);
+    if (lane == 0) s_E[wid] = ein;
+    __syncthreads();
+    if (tid == 0) {
+        double e = 0.0;
+        for (int k = 0; k < 32; ++k) e += s_E[k];
+        for (int p = 0; p < 3; ++p) {
+            int t = 0;
+            for (int k = 0; k < 32; ++k) t += s_cnt[p][k];
+            s_total[p] = t;
+            s_base[p] = 0;
+            c->q_top[p] = t;
+            c->tracks[p] = (unsigned long long)t;
+            if (t > w.qcap[p]) c->error = EMX_E_CAPACITY;
+        }
+        c->E_in = e;
+    }
+    __syncthreads();
+    if (c->error) return;
+    // pass 2: stable rank of each primary inside its type, tile by tile
+    for (long base = 0; base < pr.n; base += blockDim.x) {
+        const long i = base + tid;
+        const int pt = (i < pr.n) ? pr.ptype[i] : -1;
+        int rank = 0;
+        for (int p = 0; p < 3; ++p) {
+            const unsigned b = __ballot_sync(0xffffffffu, pt == p);
+            if (lane == 0) s_cnt[p][wid] = __popc(b);
+            if (pt == p) rank = __popc(b & ((1u << lane) - 1u));
+        }
+        __syncthreads();
+        if (pt >= 0) {
+            int before = s_base[pt];
+            for (int k = 0; k < wid; ++k) before += s_cnt[pt][k];
+            const int r = s_total[pt] - 1 - (before + rank);  // lowest index on top
+            const QueueSoA &q = w.q[pt];
+            q.x[r] = pr.pos3[3 * i];
+            q.y[r] = pr.pos3[3 * i + 1];
+            q.z[r] = pr.pos3[3 * i + 2];
+            q.ux[r] = pr.dir3[3 * i];
+            q.uy[r] = pr.dir3[3 * i + 1];
+            q.uz[r] = pr.dir3[3 * i + 2];
+            q.E[r] = pr.E[i];
+            q.tid[r] = 0ull;
+            q.prim[r] = (uint32_t)i;
+            q.vol[r] = pr.vol[i];
+            q.surf[r] = pr.surf ? pr.surf[i] : -1;
+        }
+        __syncthreads();
+        if (tid < 3) {
+            int t = 0;
+            for (int k = 0; k < 32; ++k) t += s_cnt[tid][k];
+            s_base[tid] += t;
+        }
+        __syncthreads();
+    }
+}
+
+cudaError_t launch_load_primaries(const Work &w, const Primaries &pr, cudaStream_t st) {
+    k_load_primaries<<<1, 1024, 0, st>>>(w, pr);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// A9 / A12: refill plan and loop control.  One block.  Per pool: exclusive prefix sum of the per-chunk
+// dead counts the step kernel left behind -> rank of every hole; then the sizes of the refill:
+//   a      holes filled from the stack (hole k, ascending slot index, takes record [q - 1 - k]),
+//   h - a  holes left when the stack is dry: the live range shrinks to n_new and the live tracks above
+//          n_new move into the remaining holes below it (j-th live track from the end -> j-th such hole),
+//   extra  records appended above the old range when the stack holds more than the holes.
+__global__ void __launch_bounds__(1024) k_plan(Work w) {
+    __shared__ int s_warp[32];
+    __shared__ int s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    Ctl *c = w.ctl;
+    if (c->done) return;
+    for (int p = 0; p < 3; ++p) {
+        const int n_old = c->n_live[p];
+        const int nch = (n_old + kChunk - 1) / kChunk;
+        if (tid == 0) s_carry = 0;
+        __syncthreads();
+        for (int base = 0; base < nch; base += blockDim.x) {
+            const int k = base + tid;
+            const int v = (k < nch) ? w.chunk_dead[p][k] : 0;
+            int inc = v;  // inclusive warp scan
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (lane == 31) s_warp[wid] = inc;
+            __syncthreads();
+            if (wid == 0) {
+                int x = s_warp[lane], xi = x;
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int t = __shfl_up_sync(0xffffffffu, xi, o);
+                    if (lane >= o) xi += t;
+                }
+                s_warp[lane] = xi - x;  // exclusive warp offsets
+            }
+            __syncthreads();
+            const int off = s_carry + s_warp[wid] + inc - v;
+            if (k < nch) w.chunk_off[p][k] = off;
+            __syncthreads();
+            if (tid == blockDim.x - 1) s_carry = off + v;
+            __syncthreads();
+        }
+        if (tid == 0) {
+            const int h = s_carry;
+            const int q = c->q_top[p];
+            const int a = h < q ? h : q;
+            const int n_new = n_old - (h - a);
+            int extra = 0;
+            if (h == a) {
+                extra = q - a;
+                const int room = w.cap[p] - n_old;
+                if (extra > room) extra = room;
+            }
+            PoolPlan pl;
+            pl.n_old = n_old;
+            pl.h = h;
+            pl.a = a;
+            pl.n_new = n_new;
+            pl.extra = extra;
+            pl.n_final = n_new + extra;
+            pl.q_old = q;
+            pl.q_new = q - a - extra;
+            c->plan[p] = pl;
+            c->n_live[p] = pl.n_final;
+            c->q_top[p] = pl.q_new;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const long long ng = c->n_live[0], ne = c->n_live[1], np = c->n_live[2];
+        const long long live = ng + ne + np;
+        const long long queued = (long long)c->q_top[0] + c->q_top[1] + c->q_top[2];
+        if ((unsigned long long)live > c->peak_live) c->peak_live = (unsigned long long)live;
+        if ((unsigned long long)queued > c->peak_queue) c->peak_queue = (unsigned long long)queued;
+        if (c->iter < (unsigned long long)w.max_log) {
+            w.log[2 * c->iter] = (uint32_t)live;
+            w.log[2 * c->iter + 1] = (uint32_t)queued;
+        }
+        if (live == 0) {
+            c->done = 1;
+            c->m_step[0] = c->m_step[1] = c->m_step[2] = 0;
+        } else {
+            c->iter += 1;
+            // R7: step only as many tracks as the stacks can absorb in the worst case (per parent:
+            // gamma -> 1 e- + 1 e+; e- -> 1 e- or 1 gamma; e+ -> 1 e- + 3 gamma); tracks not stepped keep their
+            // (tid, step) and are re-executed later with the same draws, so capacity never changes the physics
+            const long long need[3] = {ne + 3 * np, ng + ne + np, ng};
+            double f = 1.0;
+            for (int t = 0; t < 3; ++t) {
+                const long long fr = (long long)w.qcap[t] - c->q_top[t];
+                if (need[t] > fr) {
+                    const double ft = (double)fr / (double)need[t];
+                    if (ft < f) f = ft;
+                }
+            }
+            long long m[3] = {ng, ne, np};
+            if (f < 1.0)
+                for (int t = 0; t < 3; ++t) m[t] = (long long)floor((double)m[t] * f);
+            c->m_step[0] = (int)m[0];
+            c->m_step[1] = (int)m[1];
+            c->m_step[2] = (int)m[2];
+            c->stalls += (unsigned long long)(live - m[0] - m[1] - m[2]);
+            if (m[0] + m[1] + m[2] == 0) {
+                c->error = EMX_E_CAPACITY;
+                c->done = 1;
+            }
+        }
+    }
+}
+
+// rank of slot i among the dead slots of its chunk (exclusive), for a block that covers one chunk
+__device__ __forceinline__ int rank_in_chunk(bool dead, int *s_w) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned b = __ballot_sync(0xffffffffu, dead);
+    if (lane == 0) s_w[wid] = __popc(b);
+    __syncthreads();
+    int r = __popc(b & ((1u << lane) - 1u));
+    for (int k = 0; k < wid; ++k) r += s_w[k];
+    __syncthreads();
+    return r;
+}
+
+// A0: fill holes from the stack, list the holes that are left, append records above the old range
+__global__ void __launch_bounds__(kChunk) k_fill(Work w, int32_t *dbg_src) {
+    __shared__ int s_w[kChunk / 32];
+    const int p = blockIdx.y;
+    const Ctl *c = w.ctl;
+    if (c->done) return;
+    const PoolPlan pl = c->plan[p];
+    const int top = pl.n_old > pl.n_final ? pl.n_old : pl.n_final;
+    const int base = blockIdx.x * kChunk;
+    if (base >= top) return;
+    const int i = base + threadIdx.x;
+    const TrackSoA &t = w.trk[p];
+    const bool dead = (i < pl.n_old) && (t.alive[i] == 0);
+    const int k = w.chunk_off[p][blockIdx.x < (pl.n_old + kChunk - 1) / kChunk ? blockIdx.x : 0] + rank_in_chunk(dead, s_w);
+    if (dead) {
+        if (k < pl.a) {
+            const int r = pl.q_old - 1 - k;
+            if (dbg_src) { dbg_src[i] = r; t.alive[i] = 2; }
+            else load_record(w.q[p], r, t, i);
+        } else {
+            w.hole_idx[p][k - pl.a] = i;
+        }
+    } else if (i >= pl.n_old && i < pl.n_old + pl.extra) {
+        const int r = pl.q_old - 1 - pl.a - (i - pl.n_old);
+        if (dbg_src) { dbg_src[i] = r; t.alive[i] = 2; }
+        else load_record(w.q[p], r, t, i);
+    }
+}
+
+// A9: tail compaction when the stack ran dry: live tracks at or above n_new move into the holes below it
+__global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
+    __shared__ int s_w[kChunk / 32];
+    const int p = blockIdx.y;
+    const Ctl *c = w.ctl;
+    if (c->done) return;
+    const PoolPlan pl = c->plan[p];
+    if (pl.h == pl.a) return;  // nothing to compact
+    const int base = blockIdx.x * kChunk;
+    if (base >= pl.n_old || base + kChunk <= pl.n_new) return;
+    const int i = base + threadIdx.x;
+    const TrackSoA &t = w.trk[p];
+    const bool in = i < pl.n_old;
+    const uint8_t al = in ? t.alive[i] : (uint8_t)1;
+    const bool dead = al != 1;  // holes of this pass, whether k_fill has refilled them (2) or not (0)
+    const int dead_before = w.chunk_off[p][blockIdx.x] + rank_in_chunk(dead, s_w);
+    if (in && !dead && i >= pl.n_new) {
+        const int dead_after = pl.h - dead_before;             // dead slots in (i, n_old)
+        const int j = (pl.n_old - 1 - i) - dead_after;         // live tracks in (i, n_old)
+        const int dest = w.hole_idx[p][j];
+        if (dbg_src) { dbg_src[dest] = -2 - i; t.alive[dest] = 2; }
+        else move_slot(t, i, dest);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A1-A8 + A10: one step of every live track of pool PT.  One thread per slot of the dense prefix; the
+// track is read once, stepped in registers and written once.  Secondaries go straight onto the typed
+// stacks: the warp counts its records per type with ballots, one lane reserves the range with a single
+// atomicAdd per type ("atomic addition to unambiguously reserve one or more items"), and the
+// lanes write to consecutive records.  Energy deposition is accumulated per block in shared memory and
+// flushed with one atomic per touched tally.
+struct BlockAcc {
+    double sc[3];           // escaped, below_cut, looper
+    unsigned cnt[16];       // [0..7] interactions, [8] null, [9..11] tracks created by type, [12] steps
+};
+
+__device__ __forceinline__ void push_record(const QueueSoA &q, int r, const Vec3 &x, const Vec3 &u, double E,
+                                            uint64_t tid, uint32_t prim, int vol) {
+    q.x[r] = x.x;
+    q.y[r] = x.y;
+    q.z[r] = x.z;
+    q.ux[r] = u.x;
+    q.uy[r] = u.y;
+    q.uz[r] = u.z;
+    q.E[r] = E;
+    q.tid[r] = tid;
+    q.prim[r] = prim;
+    q.vol[r] = vol;
+    q.surf[r] = -1;
+}
+
+template <int PT>
+__global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params P, const __grid_constant__ Work w,
+                                                 uint64_t seed, double *tally) {
+    extern __shared__ double s_tally[];
+    __shared__ BlockAcc acc;
+    Ctl *c = w.ctl;
+    const int n_live = c->n_live[PT];
+    const int base = blockIdx.x * kChunk;
+    if (base >= n_live) return;
+    const int m = c->m_step[PT];
+    const int i = base + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool use_smem = P.n_tally <= 2048;
+    if (use_smem)
+        for (int k = threadIdx.x; k < P.n_tally; k += kChunk) s_tally[k] = 0.0;
+    if (threadIdx.x < 3) acc.sc[threadIdx.x] = 0.0;
+    if (threadIdx.x < 16) acc.cnt[threadIdx.x] = 0u;
+    __syncthreads();
+
+    const TrackSoA &ts = w.trk[PT];
+    const bool active = i < m;
+    Track t;
+    StepOut o;
+    int vol0 = 0;
+    uint32_t step0 = 0;
+    if (active) {
+        t.x = {ts.x[i], ts.y[i], ts.z[i]};
+        t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
+        t.E = ts.E[i];
+        t.tid = ts.tid[i];
+        t.prim = ts.prim[i];
+        t.step = ts.step[i];
+        t.vol = ts.vol[i];
+        t.surf = ts.surf[i];
+        t.alive = 1;
+        vol0 = t.vol;
+        step0 = t.step;
+        step<PT>(P, seed, t, o);
+    } else {
+        o.s0.ptype = o.s1.ptype = -1;
+        o.rest_alloc = 0;
+        o.process = -1;
+        o.edep = o.below_cut = o.escaped = o.looper = 0.0;
+        o.null_int = o.rest = 0;
+        t.alive = 1;
+    }
+
+    // ---- A8: secondaries -> typed stacks (warp-aggregated reservation)
+    const int ng = (o.s0.ptype == kGamma) + (o.s1.ptype == kGamma) + 2 * o.rest_alloc;
+    const int ne = (o.s0.ptype == kElectron);  // only ordinal 0 is ever an electron
+    const int np = (o.s1.ptype == kPositron);  // only the pair positron
+    {
+        const unsigned lt = (1u << lane) - 1u;
+        // electrons
+        unsigned b = __ballot_sync(0xffffffffu, ne);
+        if (b) {
+            int r0 = 0;
+            if (lane == 0) r0 = atomicAdd(&c->q_top[kElectron], __popc(b));
+            r0 = __shfl_sync(0xffffffffu, r0, 0);
+            if (ne) push_record(w.q[kElectron], r0 + __popc(b & lt), t.x, o.s0.u, o.s0.E,
+                                child_tid((uint32_t)seed, t.prim, t.tid, step0, 0u), t.prim, t.vol);
+        }
+        // positrons
+        b = __ballot_sync(0xffffffffu, np);
+        if (b) {
+            int r0 = 0;
+            if (lane == 0) r0 = atomicAdd(&c->q_top[kPositron], __popc(b));
+            r0 = __shfl_sync(0xffffffffu, r0, 0);
+            if (np) push_record(w.q[kPositron], r0 + __popc(b & lt), t.x, o.s1.u, o.s1.E,
+                                child_tid((uint32_t)seed, t.prim, t.tid, step0, 1u), t.prim, t.vol);
+        }
+        // photons: 0..3 per lane -> inclusive warp scan of the counts
+        b = __ballot_sync(0xffffffffu, ng > 0);
+        if (b) {
+            int inc = ng;
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += v;
+            }
+            const int total = __shfl_sync(0xffffffffu, inc, 31);
+            int r0 = 0;
+            if (lane == 0) r0 = atomicAdd(&c->q_top[kGamma], total);
+            r0 = __shfl_sync(0xffffffffu, r0, 0);
+            int r = r0 + inc - ng;
+            const QueueSoA &q = w.q[kGamma];
+            if (o.s0.ptype == kGamma)
+                push_record(q, r++, t.x, o.s0.u, o.s0.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 0u), t.prim, t.vol);
+            if (o.s1.ptype == kGamma)
+                push_record(q, r++, t.x, o.s1.u, o.s1.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 1u), t.prim, t.vol);
+            if (o.rest_alloc) {
+                const Vec3 mu = {-o.rest_u.x, -o.rest_u.y, -o.rest_u.z};
+                push_record(q, r++, t.x, o.rest_u, kMe, child_tid((uint32_t)seed, t.prim, t.tid, step0, 2u), t.prim, t.vol);
+                push_record(q, r++, t.x, mu, kMe, child_tid((uint32_t)seed, t.prim, t.tid, step0, 3u), t.prim, t.vol);
+            }
+        }
+    }
+
+    // ---- write the track back (A5-A7 results); tid and prim never change
+    if (active) {
+        ts.x[i] = t.x.x;
+        ts.y[i] = t.x.y;
+        ts.z[i] = t.x.z;
+        ts.ux[i] = t.u.x;
+        ts.uy[i] = t.u.y;
+        ts.uz[i] = t.u.z;
+        ts.E[i] = t.E;
+        ts.step[i] = t.step;
+        ts.vol[i] = t.vol;
+        ts.surf[i] = t.surf;
+    }
+    if (i < n_live) ts.alive[i] = (uint8_t)t.alive;
+
+    // ---- A10: tallies and counters
+    if (active) {
+        if (o.edep != 0.0) {
+            const int tl = P.vol[vol0].tally;
+            if (tl >= 0) {
+                if (use_smem) atomicAdd(&s_tally[tl], o.edep);
+                else atomicAdd(&tally[tl], o.edep);
+            }
+        }
+        if (o.escaped != 0.0) atomicAdd(&acc.sc[0], o.escaped);
+        if (o.below_cut != 0.0) atomicAdd(&acc.sc[1], o.below_cut);
+        if (o.looper != 0.0) atomicAdd(&acc.sc[2], o.looper);
+        if (o.process >= 0) atomicAdd(&acc.cnt[o.null_int ? 8 : o.process], 1u);
+        if (o.rest) atomicAdd(&acc.cnt[EMX_P_REST], 1u);
+        if (ng) atomicAdd(&acc.cnt[9], (unsigned)ng);
+        if (ne) atomicAdd(&acc.cnt[10], 1u);
+        if (np) atomicAdd(&acc.cnt[11], 1u);
+    }
+    const int n_dead = __syncthreads_count(i < n_live && !t.alive);
+    if (threadIdx.x == 0) {
+        w.chunk_dead[PT][blockIdx.x] = n_dead;
+        const int n_act = (m - base) < kChunk ? ((m - base) > 0 ? (m - base) : 0) : kChunk;
+        if (n_act) atomicAdd(&c->steps[PT], (unsigned long long)n_act);
+        if (acc.sc[0] != 0.0) atomicAdd(&c->escaped, acc.sc[0]);
+        if (acc.sc[1] != 0.0) atomicAdd(&c->below_cut, acc.sc[1]);
+        if (acc.sc[2] != 0.0) atomicAdd(&c->looper, acc.sc[2]);
+    }
+    if (threadIdx.x < 12) {
+        const unsigned v = acc.cnt[threadIdx.x];
+        if (v) {
+            unsigned long long *dst = threadIdx.x < 8 ? &c->inter[threadIdx.x]
+                                     : (threadIdx.x == 8 ? &c->null_int : &c->tracks[threadIdx.x - 9]);
+            atomicAdd(dst, (unsigned long long)v);
+        }
+    }
+    if (use_smem)
+        for (int k = threadIdx.x; k < P.n_tally; k += kChunk) {
+            const double v = s_tally[k];
+            if (v != 0.0) atomicAdd(&tally[k], v);
+        }
+}
+
+cudaError_t launch_iteration(const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st) {
+    int maxcap = w.cap[0];
+    for (int p = 1; p < 3; ++p) maxcap = w.cap[p] > maxcap ? w.cap[p] : maxcap;
+    const dim3 g3((maxcap + kChunk - 1) / kChunk, 3);
+    k_plan<<<1, 1024, 0, st>>>(w);
+    k_fill<<<g3, kChunk, 0, st>>>(w, nullptr);
+    k_move<<<g3, kChunk, 0, st>>>(w, nullptr);
+    const size_t sm = P.n_tally <= 2048 ? (size_t)P.n_tally * sizeof(double) : 0;
+    k_step<kGamma><<<(w.cap[0] + kChunk - 1) / kChunk, kChunk, sm, st>>>(P, w, seed, tally);
+    k_step<kElectron><<<(w.cap[1] + kChunk - 1) / kChunk, kChunk, sm, st>>>(P, w, seed, tally);
+    k_step<kPositron><<<(w.cap[2] + kChunk - 1) / kChunk, kChunk, sm, st>>>(P, w, seed, tally);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// level-1 hook: the refill index logic (k_plan, k_fill, k_move) on a caller-supplied alive[] array
+__global__ void k_hook_init(Work w, int n_live, int n_queue) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        Ctl z = Ctl();
+        z.n_live[0] = n_live;
+        z.q_top[0] = n_queue;
+        *w.ctl = z;
+    }
+}
+__global__ void __launch_bounds__(kChunk) k_count_dead(Work w, int n_live) {
+    const int i = blockIdx.x * kChunk + threadIdx.x;
+    const int n = __syncthreads_count(i < n_live && w.trk[0].alive[i] == 0);
+    if (threadIdx.x == 0) w.chunk_dead[0][blockIdx.x] = n;
+}
+
+size_t refill_plan_scratch_ints(long capacity) {
+    const size_t nch = (size_t)(capacity + kChunk - 1) / kChunk + 1;
+    return 2 * nch + (size_t)capacity + (sizeof(Ctl) + 3) / 4 + 64 + ((size_t)capacity + 3) / 4 + 64;
+}
+
+cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
+                               int *scratch, cudaStream_t st) {
+    const size_t nch = (size_t)(capacity + kChunk - 1) / kChunk + 1;
+    Work w = Work();
+    int *p = scratch;
+    w.chunk_dead[0] = p; p += nch;
+    w.chunk_off[0] = p; p += nch;
+    w.hole_idx[0] = p; p += capacity;
+    p += (16 - ((uintptr_t)p / 4) % 16) % 16;  // 64-byte alignment for the control block
+    w.ctl = (Ctl *)p; p += (sizeof(Ctl) + 3) / 4;
+    w.trk[0].alive = (uint8_t *)p;
+    w.cap[0] = (int)capacity;
+    w.cap[1] = w.cap[2] = 0;
+    w.qcap[0] = w.qcap[1] = w.qcap[2] = 0x7fffffff;
+    w.log = nullptr;
+    w.max_log = 0;
+    cudaMemsetAsync(w.trk[0].alive, 0, (size_t)capacity, st);
+    if (n_live > 0) cudaMemcpyAsync(w.trk[0].alive, alive, (size_t)n_live, cudaMemcpyDeviceToDevice, st);
+    cudaMemsetAsync(src, 0xFF, (size_t)capacity * sizeof(int32_t), st);
+    k_hook_init<<<1, 32, 0, st>>>(w, (int)n_live, (int)n_queue);
+    const unsigned g = (unsigned)((n_live + kChunk - 1) / kChunk);
+    if (g) k_count_dead<<<g, kChunk, 0, st>>>(w, (int)n_live);
+    k_plan<<<1, 1024, 0, st>>>(w);
+    const dim3 g3((unsigned)((capacity + kChunk - 1) / kChunk), 1);
+    k_fill<<<g3, kChunk, 0, st>>>(w, src);
+    k_move<<<g3, kChunk, 0, st>>>(w, src);
+    return cudaGetLastError();
+}
+
+}  // namespace emx

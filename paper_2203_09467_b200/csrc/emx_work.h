@@ -1,0 +1,70 @@
+// emx_work.h -- layout of the caller-provided device workspace: the SoA track store ("state" in the paper's
+// params/state split), the secondary stacks ("stack allocator", PAPER.md:204
+// "track initializers"), and the loop's control block.  DESIGN.md section 5.
+//
+// The store is split into one POOL per particle type (gamma, e-, e+): a track never changes type, so each
+// pool is stepped by a kernel instantiated for that type -- particle type is the coarsest "next action"
+// and partitioning by it removes the largest source of warp divergence.  Inside a pool the live tracks
+// always occupy the dense prefix [0, n_live): the refill pass fills holes from the pool's LIFO stack and,
+// when the stack runs dry, from the tail of the pool, so every field access is a coalesced 8-byte stream.
+#pragma once
+#include "emx_core.h"
+
+namespace emx {
+
+constexpr int kChunk = 128;  // slots per thread block of the step / refill kernels
+
+struct TrackSoA {
+    double *x, *y, *z, *ux, *uy, *uz, *E;
+    uint64_t *tid;
+    uint32_t *prim, *step;
+    int *vol, *surf;
+    uint8_t *alive;
+};
+
+struct QueueSoA {  // secondary / primary initializer records (76 B per record)
+    double *x, *y, *z, *ux, *uy, *uz, *E;
+    uint64_t *tid;
+    uint32_t *prim;
+    int *vol, *surf;
+};
+
+struct PoolPlan {
+    int n_old;    // live range before the refill
+    int h;        // holes (dead slots) in [0, n_old)
+    int a;        // holes filled from the stack
+    int n_new;    // live range after tail compaction
+    int extra;    // records appended beyond n_old
+    int n_final;  // live range after the refill
+    int q_old, q_new;
+};
+
+struct Ctl {
+    int n_live[3];
+    int q_top[3];
+    int m_step[3];  // tracks stepped this iteration (< n_live only when a stack is nearly full, R7)
+    PoolPlan plan[3];
+    int done, error;
+    unsigned long long iter;
+    double escaped, below_cut, looper, E_in;
+    unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls, peak_live, peak_queue;
+};
+
+struct Work {
+    TrackSoA trk[3];
+    QueueSoA q[3];
+    int cap[3];   // slots per pool
+    int qcap[3];  // records per stack
+    int *chunk_dead[3];
+    int *chunk_off[3];
+    int *hole_idx[3];
+    Ctl *ctl;
+    uint32_t *log;  // per iteration: live, queued
+    int max_log;
+};
+
+// bytes of one slot / one record, for the workspace carve-up and the roofline arithmetic
+constexpr size_t kSlotBytes = 7 * 8 + 8 + 4 + 4 + 4 + 4 + 1;
+constexpr size_t kRecordBytes = 7 * 8 + 8 + 4 + 4 + 4;
+
+}  // namespace emx
