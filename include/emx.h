@@ -251,7 +251,8 @@ int emx_draw_batch(uint64_t seed, long n, const uint32_t *prim, const uint64_t *
  * of `n_live` slots whose alive flags are alive[n_live] (uint8, DEVICE) with `n_queue` queued records and
  * room for `capacity` slots, and writes, for every slot index < new_n_live, src[i] (int32, DEVICE,
  * capacity entries): -1 = untouched live track, q >= 0 = filled from queue record q,
- * -2 - j = moved from slot j.  counts_host[3] = { new_n_live, new_n_queue, n_moved }. */
+ * -2 - j = moved from slot j.  counts_host[3] = { new_n_live, new_n_queue, holes the stack could not
+ * fill (= old n_live - new n_live when positive) }. */
 int emx_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
                     long *counts_host, void *stream);
 

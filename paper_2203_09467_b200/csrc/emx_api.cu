@@ -496,7 +496,7 @@ int emx_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *ali
     if (e != cudaSuccess) return fail_cuda(p, e, "emx_refill_plan");
     counts_host[0] = hc.plan[0].n_final;
     counts_host[1] = hc.plan[0].q_new;
-    counts_host[2] = hc.plan[0].h - hc.plan[0].a > 0 ? (hc.plan[0].n_old - hc.plan[0].n_new) - (hc.plan[0].h - hc.plan[0].a - 0) : 0;
+    counts_host[2] = hc.plan[0].h - hc.plan[0].a;
     return EMX_OK;
 }
 

@@ -216,29 +216,17 @@ __global__ void __launch_bounds__(1024) k_plan(Work w) {
             c->m_step[0] = c->m_step[1] = c->m_step[2] = 0;
         } else {
             c->iter += 1;
-            // R7: step only as many tracks as the stacks can absorb in the worst case (per parent:
-            // gamma -> 1 e- + 1 e+; e- -> 1 e- or 1 gamma; e+ -> 1 e- + 3 gamma); tracks not stepped keep their
-            // (tid, step) and are re-executed later with the same draws, so capacity never changes the physics
-            const long long need[3] = {ne + 3 * np, ng + ne + np, ng};
-            double f = 1.0;
-            for (int t = 0; t < 3; ++t) {
-                const long long fr = (long long)w.qcap[t] - c->q_top[t];
-                if (need[t] > fr) {
-                    const double ft = (double)fr / (double)need[t];
-                    if (ft < f) f = ft;
-                }
-            }
-            long long m[3] = {ng, ne, np};
-            if (f < 1.0)
-                for (int t = 0; t < 3; ++t) m[t] = (long long)floor((double)m[t] * f);
-            c->m_step[0] = (int)m[0];
-            c->m_step[1] = (int)m[1];
-            c->m_step[2] = (int)m[2];
-            c->stalls += (unsigned long long)(live - m[0] - m[1] - m[2]);
-            if (m[0] + m[1] + m[2] == 0) {
+            // R7: a step whose secondaries do not fit on the stacks is not committed and is re-executed in a
+            // later iteration with the same (tid, step) and hence the same draws; if a whole iteration commits
+            // nothing, the stacks are too small for this problem
+            c->m_step[0] = (int)ng;
+            c->m_step[1] = (int)ne;
+            c->m_step[2] = (int)np;
+            if (c->iter > 1 && c->progress == 0ull) {
                 c->error = EMX_E_CAPACITY;
                 c->done = 1;
             }
+            c->progress = 0ull;
         }
     }
 }
@@ -361,10 +349,12 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
     StepOut o;
     int vol0 = 0;
     uint32_t step0 = 0;
-    if (active) {
+    const double E0 = active ? ts.E[i] : 0.0;
+    const bool tomb = active && E0 < 0.0;  // tombstone record: retire the slot without stepping
+    if (active && !tomb) {
         t.x = {ts.x[i], ts.y[i], ts.z[i]};
         t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
-        t.E = ts.E[i];
+        t.E = E0;
         t.tid = ts.tid[i];
         t.prim = ts.prim[i];
         t.step = ts.step[i];
@@ -383,33 +373,42 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         t.alive = 1;
     }
 
-    // ---- A8: secondaries -> typed stacks (warp-aggregated reservation)
+    // ---- A8: secondaries -> typed stacks.  Warp-aggregated reservation: one atomicAdd per type and warp.  A
+    // reservation that would pass the capacity is rolled back (no other warp can succeed while the top is
+    // above the capacity, so successful ranges stay contiguous) and the lanes that needed it STALL: nothing
+    // of their step is committed (R7).  Records a stalled lane did obtain for another type become tombstones
+    // (E < 0), which the next refill loads and this kernel retires without stepping.
     const int ng = (o.s0.ptype == kGamma) + (o.s1.ptype == kGamma) + 2 * o.rest_alloc;
     const int ne = (o.s0.ptype == kElectron);  // only ordinal 0 is ever an electron
     const int np = (o.s1.ptype == kPositron);  // only the pair positron
+    bool stall = false;
+    int r_e = -1, r_p = -1, r_g = -1;
     {
         const unsigned lt = (1u << lane) - 1u;
-        // electrons
         unsigned b = __ballot_sync(0xffffffffu, ne);
         if (b) {
             int r0 = 0;
-            if (lane == 0) r0 = atomicAdd(&c->q_top[kElectron], __popc(b));
+            if (lane == 0) {
+                const int cnt = __popc(b);
+                r0 = atomicAdd(&c->q_top[kElectron], cnt);
+                if (r0 + cnt > w.qcap[kElectron]) { atomicSub(&c->q_top[kElectron], cnt); r0 = -1; }
+            }
             r0 = __shfl_sync(0xffffffffu, r0, 0);
-            if (ne) push_record(w.q[kElectron], r0 + __popc(b & lt), t.x, o.s0.u, o.s0.E,
-                                child_tid((uint32_t)seed, t.prim, t.tid, step0, 0u), t.prim, t.vol);
+            if (ne) { if (r0 < 0) stall = true; else r_e = r0 + __popc(b & lt); }
         }
-        // positrons
         b = __ballot_sync(0xffffffffu, np);
         if (b) {
             int r0 = 0;
-            if (lane == 0) r0 = atomicAdd(&c->q_top[kPositron], __popc(b));
+            if (lane == 0) {
+                const int cnt = __popc(b);
+                r0 = atomicAdd(&c->q_top[kPositron], cnt);
+                if (r0 + cnt > w.qcap[kPositron]) { atomicSub(&c->q_top[kPositron], cnt); r0 = -1; }
+            }
             r0 = __shfl_sync(0xffffffffu, r0, 0);
-            if (np) push_record(w.q[kPositron], r0 + __popc(b & lt), t.x, o.s1.u, o.s1.E,
-                                child_tid((uint32_t)seed, t.prim, t.tid, step0, 1u), t.prim, t.vol);
+            if (np) { if (r0 < 0) stall = true; else r_p = r0 + __popc(b & lt); }
         }
-        // photons: 0..3 per lane -> inclusive warp scan of the counts
         b = __ballot_sync(0xffffffffu, ng > 0);
-        if (b) {
+        if (b) {  // photons: 0..3 per lane -> inclusive warp scan of the counts
             int inc = ng;
             for (int d = 1; d < 32; d <<= 1) {
                 const int v = __shfl_up_sync(0xffffffffu, inc, d);
@@ -417,10 +416,27 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
             }
             const int total = __shfl_sync(0xffffffffu, inc, 31);
             int r0 = 0;
-            if (lane == 0) r0 = atomicAdd(&c->q_top[kGamma], total);
+            if (lane == 0) {
+                r0 = atomicAdd(&c->q_top[kGamma], total);
+                if (r0 + total > w.qcap[kGamma]) { atomicSub(&c->q_top[kGamma], total); r0 = -1; }
+            }
             r0 = __shfl_sync(0xffffffffu, r0, 0);
-            int r = r0 + inc - ng;
+            if (ng) { if (r0 < 0) stall = true; else r_g = r0 + inc - ng; }
+        }
+    }
+    if (stall) {
+        if (r_e >= 0) w.q[kElectron].E[r_e] = -1.0;
+        if (r_p >= 0) w.q[kPositron].E[r_p] = -1.0;
+        if (r_g >= 0)
+            for (int k = 0; k < ng; ++k) w.q[kGamma].E[r_g + k] = -1.0;
+    } else {
+        if (ne) push_record(w.q[kElectron], r_e, t.x, o.s0.u, o.s0.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 0u),
+                            t.prim, t.vol);
+        if (np) push_record(w.q[kPositron], r_p, t.x, o.s1.u, o.s1.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 1u),
+                            t.prim, t.vol);
+        if (ng) {
             const QueueSoA &q = w.q[kGamma];
+            int r = r_g;
             if (o.s0.ptype == kGamma)
                 push_record(q, r++, t.x, o.s0.u, o.s0.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 0u), t.prim, t.vol);
             if (o.s1.ptype == kGamma)
@@ -432,9 +448,10 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
             }
         }
     }
+    const bool commit = active && !tomb && !stall;
 
     // ---- write the track back (A5-A7 results); tid and prim never change
-    if (active) {
+    if (commit) {
         ts.x[i] = t.x.x;
         ts.y[i] = t.x.y;
         ts.z[i] = t.x.z;
@@ -446,10 +463,11 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         ts.vol[i] = t.vol;
         ts.surf[i] = t.surf;
     }
-    if (i < n_live) ts.alive[i] = (uint8_t)t.alive;
+    const int alive_out = tomb ? 0 : (commit ? t.alive : 1);
+    if (i < n_live) ts.alive[i] = (uint8_t)alive_out;
 
     // ---- A10: tallies and counters
-    if (active) {
+    if (commit) {
         if (o.edep != 0.0) {
             const int tl = P.vol[vol0].tally;
             if (tl >= 0) {
@@ -466,11 +484,15 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         if (ne) atomicAdd(&acc.cnt[10], 1u);
         if (np) atomicAdd(&acc.cnt[11], 1u);
     }
-    const int n_dead = __syncthreads_count(i < n_live && !t.alive);
+    const int n_dead = __syncthreads_count(i < n_live && !alive_out);
+    const int n_commit = __syncthreads_count(commit);
+    const int n_tomb = __syncthreads_count(tomb);
+    const int n_stall = __syncthreads_count(active && stall);
     if (threadIdx.x == 0) {
         w.chunk_dead[PT][blockIdx.x] = n_dead;
-        const int n_act = (m - base) < kChunk ? ((m - base) > 0 ? (m - base) : 0) : kChunk;
-        if (n_act) atomicAdd(&c->steps[PT], (unsigned long long)n_act);
+        if (n_commit) atomicAdd(&c->steps[PT], (unsigned long long)n_commit);
+        if (n_commit + n_tomb) atomicAdd(&c->progress, (unsigned long long)(n_commit + n_tomb));
+        if (n_stall) atomicAdd(&c->stalls, (unsigned long long)n_stall);
         if (acc.sc[0] != 0.0) atomicAdd(&c->escaped, acc.sc[0]);
         if (acc.sc[1] != 0.0) atomicAdd(&c->below_cut, acc.sc[1]);
         if (acc.sc[2] != 0.0) atomicAdd(&c->looper, acc.sc[2]);

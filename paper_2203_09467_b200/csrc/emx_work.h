@@ -42,10 +42,11 @@ struct PoolPlan {
 struct Ctl {
     int n_live[3];
     int q_top[3];
-    int m_step[3];  // tracks stepped this iteration (< n_live only when a stack is nearly full, R7)
+    int m_step[3];  // tracks to step this iteration (= n_live)
     PoolPlan plan[3];
     int done, error;
     unsigned long long iter;
+    unsigned long long progress;  // steps committed + tombstones retired in the current iteration (R7)
     double escaped, below_cut, looper, E_in;
     unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls, peak_live, peak_queue;
 };
