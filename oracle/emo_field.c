@@ -79,7 +79,7 @@ double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x
             *surf_io = surf;
             return s_done;
         }
-        if (d > L) {                                   /* chord stays inside the cell: accept */
+        if (d > L + eps) {                             /* chord ends inside the cell, clear of S: accept */
             x[0] = x1[0]; x[1] = x1[1]; x[2] = x1[2];
             u[0] = u1[0]; u[1] = u1[1]; u[2] = u1[2];
             s_done += h; surf = -1;
@@ -89,7 +89,10 @@ double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x
             h *= (f < 5.0 ? f : 5.0);
             continue;
         }
-        if (L - d <= eps) {                            /* landed on S within tolerance */
+        if (L - d <= eps) {                            /* |L - d| <= eps: landed on S within tolerance, whether just
+                                                          past it or just short of it.  (A point accepted as "inside"
+                                                          a hair short of S can round onto S unflagged, and the next
+                                                          chord then sees S at distance 0 and walks through it.) */
             x[0] = x1[0]; x[1] = x1[1]; x[2] = x1[2];
             u[0] = u1[0]; u[1] = u1[1]; u[2] = u1[2];
             *hit = S;

@@ -85,7 +85,7 @@ EMX_HD double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Ve
             hit = S;  // immediate (re-)crossing, nothing more travelled
             return s_done;
         }
-        if (d > L) {  // chord stays inside the cell: accept
+        if (d > L + eps) {  // chord ends inside the cell, clear of S: accept
             x = x1;
             u = u1;
             s_done += h;
@@ -96,7 +96,7 @@ EMX_HD double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Ve
             h *= (f < 5.0 ? f : 5.0);
             continue;
         }
-        if (L - d <= eps) {  // landed on S within tolerance
+        if (L - d <= eps) {  // |L - d| <= eps: landed on S, just past it or just short of it
             x = x1;
             u = u1;
             hit = S;

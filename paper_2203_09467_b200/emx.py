@@ -4,8 +4,10 @@ PyTorch provides device memory and the CUDA stream; every step of the path runs 
 libemx.so.  There is no CPU fallback: if the library is missing or no CUDA device is present the calls
 raise.  Problem descriptions are the plain dicts produced by `workloads` (inputs only).
 """
+import atexit
 import ctypes as C
 import os
+import weakref
 
 import numpy as np
 
@@ -61,6 +63,7 @@ def lib():
         if not os.path.exists(LIB_PATH):
             raise RuntimeError("libemx.so not built: run `python -m paper_2203_09467_b200.build` (needs nvcc); "
                                "this package has no CPU path")
+        import torch  # noqa: F401  -- load torch's CUDA libraries before ours (device memory and streams are torch's)
         L = C.CDLL(LIB_PATH)
         vp, i, l, d, u64 = C.c_void_p, C.c_int, C.c_long, C.c_double, C.c_uint64
         sig = {
@@ -111,6 +114,16 @@ class EmxError(RuntimeError):
     pass
 
 
+_live = weakref.WeakSet()
+
+
+@atexit.register
+def _destroy_all():
+    """Free every problem while the CUDA runtime is still up (not from __del__ at interpreter teardown)."""
+    for p in list(_live):
+        p.close()
+
+
 class Problem:
     """create -> add materials / surfaces / volumes -> set field / physics -> build tables."""
 
@@ -119,6 +132,8 @@ class Problem:
         h = C.c_void_p()
         self._check(L.emx_create(C.byref(h)), None)
         self.h = h
+        self._destroy = L.emx_destroy
+        _live.add(self)
         self.desc = desc
         for m in desc["materials"]:
             Z, A, w = _np(m["Z"], np.int32), _np(m["A"], np.float64), _np(m["w"], np.float64)
@@ -149,10 +164,17 @@ class Problem:
             raise EmxError("emx error %d: %s" % (rc, (lib().emx_last_error(hh) or b"").decode()))
         return rc
 
+    def close(self):
+        h, self.h = getattr(self, "h", None), None
+        if h:
+            self._ws = None
+            self._destroy(h)
+
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().emx_destroy(self.h)
-            self.h = None
+        try:
+            self.close()
+        except Exception:
+            pass
 
     def build_tables(self):
         _torch()
@@ -244,7 +266,9 @@ class Problem:
         tout = torch.empty(n * C.sizeof(StepResult), dtype=torch.uint8, device="cuda")
         self._check(lib().emx_step_batch(self.h, seed, n, C.c_void_p(tin.data_ptr()), C.c_void_p(tout.data_ptr()), _stream()))
         torch.cuda.synchronize()
-        C.memmove(out, tout.cpu().numpy().ctypes.data, n * C.sizeof(StepResult))
+        host = tout.cpu().numpy()          # keep the host copy alive while ctypes reads from it
+        C.memmove(out, host.ctypes.data, n * C.sizeof(StepResult))
+        del host
         return out
 
 

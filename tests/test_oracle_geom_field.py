@@ -220,3 +220,38 @@ def test_boundary_landing_in_field(emo):
         else:
             assert s == pytest.approx(5.0, rel=1e-13) and z0 < x[2] < z1
     assert n_hit > 150
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 6000), (4, 6000)])
+def test_field_steps_never_leave_their_cell(emo, cfg, n):
+    """Invariant (C9): a step ends inside or on the boundary of the cell it started in -- a
+    boundary may be reached, never passed.  Pins the landing rule |L - d| <= eps: with the one-sided rule
+    L - d <= eps a chord end a hair SHORT of a surface was accepted as interior, rounded onto the surface
+    unflagged, and the next chord walked through it (seen as end points 7 cm outside the cell)."""
+    import states
+    desc, _ = W.get(cfg, 4)
+    P = emo.Problem(desc)
+    tr = states.random_states(emo, P, desc, n, seed=1000 + cfg, ptypes=(1, 2))
+    res = P.step_batch(tr, desc["seed"])
+    worst = 0.0
+    for t, r in zip(tr, res):
+        vol = desc["volumes"][t.vol]
+        x = r.trk.x
+        for S, sense in zip(vol["surf"], vol["sense"]):
+            ty, v = desc["surfaces"][S]
+            f = (math.hypot(x[0], x[1]) - v) if ty == 3 else (x[ty] - v)
+            worst = max(worst, -sense * f)          # > 0: outside this face by that many cm
+    assert worst <= 2e-7                             # landing tolerance eps = 1e-7 cm
+
+
+def test_field_landing_regression_state(emo):
+    """The state that exposed the one-sided landing rule: a 4 keV e- in the bottom vacuum box of the
+    calorimeter world, B = 1 T along y; it must stop on the y = -30 cm face (surface 107)."""
+    desc, _ = W.get(3, 4)
+    P = emo.Problem(desc)
+    t = emo.Track()
+    t.x[:] = [15.723231344610966, -26.661460451909164, 6.158366420181668]
+    t.u[:] = [-0.7636925592807772, -0.26691181033127387, 0.5878194964484071]
+    t.E = 0.003987383479174055; t.vol = 104; t.surf = -1; t.ptype = 1; t.alive = 1
+    r = P.step_batch((emo.Track * 1)(t), 3)[0]
+    assert r.action == 3 and r.trk.surf == 107 and abs(r.trk.x[1] + 30.0) <= 1e-7 and r.trk.alive == 0
