@@ -1,0 +1,268 @@
+"""bench.py -- track-steps/s and primaries/s of the EM-shower step loop on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--primaries n] [--impl reference]
+
+One "step" = one pass of the whole hot path (refill, step kernels, secondaries, tallies, until no track is
+left) over one batch of synthetic primaries: by default the full BASELINE config 4 ("throughput stress":
+barrel detector in a 4 T field, 100 000 primaries of 1-100 GeV, 2^20 track slots), the largest
+single-GPU configuration.  Inputs are seeded and synthetic (paper_2203_09467_b200/workloads.py).
+`value` is device-timed with the primaries already resident in HBM; `e2e` is the same metric through
+emx_transport_host with HOST buffers (uploads and the tally read-back inside the timed region).
+N > 1 (torchrun): independent replicas, one per GPU, different seeds ("replicas only").
+`--impl reference` times the oracle (plain fp64 C, oracle/) on the host cores on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+from paper_2203_09467_b200 import workloads as W  # noqa: E402
+
+METRIC, UNIT = "track_steps_per_sec", "track-steps/s"
+# algorithmic DRAM bytes of the step kernel: per track-step the slot is read once
+# (x, u, E, tid, prim, step, vol, surf = 80 B) and written once (x, u, E, step, vol, surf, alive = 69 B);
+# per secondary one 76-byte record is written.
+B_STEP, B_SEC = 80 + 69, 76
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--primaries", type=int, default=0, help="0 = the config's full count")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload(args):
+    desc, prim = W.get(args.config) if args.primaries <= 0 else W.get(args.config, args.primaries)
+    return desc, prim
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[k] for r in self.rows if len(r) >= 7 for k in range(4) if r[3 + k].lower() == "active"})
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=reasons, samples=len(sm))
+
+
+def oracle_run(desc, prim, n_sample, threads=None):
+    """The oracle as it stands on the host cores: (track_steps, seconds, threads)."""
+    from oracle import emo
+    P = emo.Problem(desc)
+    threads = threads or (os.cpu_count() or 1)
+    sub = W.prefix(prim, n_sample)
+    t0 = time.perf_counter()
+    r = P.transport(sub, desc["seed"], n_threads=threads)
+    dt = time.perf_counter() - t0
+    return r["track_steps"], dt, threads
+
+
+def oracle_sample_size(desc, prim, threads):
+    """primaries whose oracle transport takes roughly 10-30 s: probe with a few, then scale"""
+    n0 = min(len(prim["E"]), 4 * threads)
+    steps, dt, _ = oracle_run(desc, prim, n0, threads)
+    rate = max(n0 / max(dt, 1e-3), 1e-9)          # primaries / s
+    return int(max(n0, min(len(prim["E"]), rate * 15.0)))
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step = a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    desc, prim = workload(args)
+    threads = os.cpu_count() or 1
+    n_s = oracle_sample_size(desc, prim, threads)
+    for _ in range(args.warmup):
+        oracle_run(desc, prim, max(1, n_s // 8), threads)
+    tot_steps, tot_t = 0, 0.0
+    for _ in range(args.steps):
+        s, dt, _ = oracle_run(desc, prim, n_s, threads)
+        tot_steps += s
+        tot_t += dt
+    v = tot_steps / tot_t
+    sample = "first %d of %d primaries of %s per step" % (n_s, len(prim["E"]), desc["name"])
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": desc["name"], "primaries_per_step": n_s},
+        "primaries_per_sec": n_s * args.steps / tot_t,
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2203_09467_b200 import emx
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the emx path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    desc, prim = workload(args)
+    n_prim = len(prim["E"])
+    seed = desc["seed"] + 1000 * rank          # replicas: same problem, independent histories
+    G = emx.Problem(desc)
+    pdev = G.upload_primaries(prim)
+    pinned = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in prim.items()}
+    phost = {k: v.numpy() for k, v in pinned.items()}
+    h2d = sum(v.numel() * v.element_size() for v in pinned.values())
+    d2h = 8 * G.n_tally + 200
+
+    G.set_profile(False)
+    for _ in range(args.warmup):
+        G.transport(pdev, seed)
+    barrier()
+
+    # ---- timed region: K steps, device-resident inputs, per-kernel events on
+    G.set_profile(True)
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tot = dict(steps=0, sec=0, kms=np.zeros(4), launches=0, per_type=np.zeros(3), sec_type=np.zeros(3), iters=0)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        r = G.transport(pdev, seed)
+        pr = G.profile()
+        tot["steps"] += r["track_steps"]
+        tot["per_type"] += r["steps"].astype(np.float64)
+        sec = r["tracks"].astype(np.float64).copy()
+        for k in range(3):
+            sec[k] -= float((prim["ptype"] == k).sum())
+        tot["sec_type"] += sec
+        tot["kms"] += np.array(pr["ms"])
+        tot["launches"] += pr["launches"]
+        tot["iters"] += r["iterations"]
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clk = clocks.stop() if rank == 0 else None
+    last = r
+
+    # ---- e2e: host buffers in, tallies out, through the public entry point
+    G.set_profile(False)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = 0
+    for _ in range(args.steps):
+        r2 = G.transport_host(phost, seed)
+        e2e_steps += r2["track_steps"]
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+        c = torch.tensor([float(tot["steps"]), float(e2e_steps)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        all_steps, all_e2e = float(c[0]), float(c[1])
+    else:
+        all_steps, all_e2e = float(tot["steps"]), float(e2e_steps)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = all_steps / (ms * 1e-3)
+    # roofline of the dominant kernel: the fused step kernel of the pool that took the most time
+    dom = int(np.argmax(tot["kms"][:3]))
+    names = ["k_step<gamma>", "k_step<e->", "k_step<e+>"]
+    # secondaries written by pool `dom`: gamma pool makes e-/e+, e- pool makes e-/gamma, e+ pool e-/gamma -- the split by
+    # parent type is not counted separately, so attribute all secondaries in proportion to the steps
+    share = tot["per_type"][dom] / max(tot["per_type"].sum(), 1.0)
+    alg_bytes = tot["per_type"][dom] * B_STEP + tot["sec_type"].sum() * share * B_SEC
+    k_s = tot["kms"][dom] * 1e-3
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    ach = alg_bytes / k_s / 1e9 if k_s > 0 else 0.0
+    n_launch_dom = max(tot["iters"], 1)
+    roof = {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "traffic": None, "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s",
+            "algorithmic_bytes_per_launch": alg_bytes / n_launch_dom, "avg_launch_ms": tot["kms"][dom] / n_launch_dom,
+            "kernel_ms_per_step": {"k_step_gamma": tot["kms"][0] / args.steps, "k_step_eminus": tot["kms"][1] / args.steps,
+                                   "k_step_eplus": tot["kms"][2] / args.steps, "refill": tot["kms"][3] / args.steps},
+            "step_kernel_share_of_step": float(tot["kms"][:3].sum() / ms)}
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": desc["name"], "primaries_per_step": n_prim, "n_slots": desc["n_slots"],
+                      "queue_capacity": desc["queue_capacity"], "parallelism": "replicas x%d" % world,
+                      "l2": "inputs larger than L2: track store + stacks > 126 MB, every step re-reads the stacks"},
+           "primaries_per_sec": n_prim * args.steps * world / (ms * 1e-3),
+           "iterations_per_step": tot["iters"] / args.steps, "peak_live": last["peak_live"], "peak_queue": last["peak_queue"],
+           "e2e": {"value": all_e2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+           "gpu_launches": int(tot["launches"]), "clocks": clk, "roofline": roof}
+    if not args.no_cpu_baseline and world == 1:
+        threads = os.cpu_count() or 1
+        n_s = oracle_sample_size(desc, prim, threads)
+        s, dt, _ = oracle_run(desc, prim, n_s, threads)
+        out["cpu_baseline"] = {"value": s / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+                               "sample": "first %d of %d primaries of %s, %.1f s" % (n_s, n_prim, desc["name"], dt)}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -34,6 +34,11 @@ struct emx_problem {
     // pinned staging for the control block
     Ctl *h_ctl = nullptr;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    // optional per-kernel timing of the loop (emx_set_profile)
+    bool profile = false;
+    std::vector<cudaEvent_t> prof_ev;
+    double prof_ms[4] = {0, 0, 0, 0};  // k_step gamma, e-, e+, refill (plan + fill + move)
+    long launches = 0, iterations_launched = 0;
 };
 
 namespace {
@@ -150,6 +155,7 @@ void emx_destroy(emx_problem *p) {
     if (p->h_ctl) cudaFreeHost(p->h_ctl);
     if (p->ev0) cudaEventDestroy(p->ev0);
     if (p->ev1) cudaEventDestroy(p->ev1);
+    for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
     delete p;
 }
 
@@ -353,11 +359,41 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     if (need > workspace_bytes) return fail(p, EMX_E_CAPACITY, "emx_transport: workspace smaller than emx_workspace_bytes()");
     CU(cudaEventRecord(p->ev0, st));
     CU(launch_load_primaries(w, pr, st));
+    p->launches = 1;
+    p->iterations_launched = 0;
+    for (double &v : p->prof_ms) v = 0.0;
     int batch = 8;
     for (;;) {
-        for (int k = 0; k < batch; ++k) CU(launch_iteration(p->P, w, seed, p->d_tally, st));
+        size_t ne = 0;
+        if (p->profile) {
+            while (p->prof_ev.size() < (size_t)batch * 5) {
+                cudaEvent_t e;
+                CU(cudaEventCreate(&e));
+                p->prof_ev.push_back(e);
+            }
+        }
+        for (int k = 0; k < batch; ++k) {
+            if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
+            CU(launch_refill(w, st));
+            for (int pt = 0; pt < 3; ++pt) {
+                if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
+                CU(launch_step(pt, p->P, w, seed, p->d_tally, st));
+            }
+            if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
+        }
+        p->launches += (long)batch * kLaunchesPerIteration;
+        p->iterations_launched += batch;
         CU(cudaMemcpyAsync(p->h_ctl, w.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
+        if (p->profile)
+            for (int k = 0; k < batch; ++k) {
+                float ms;
+                const cudaEvent_t *e = &p->prof_ev[(size_t)k * 5];
+                CU(cudaEventElapsedTime(&ms, e[0], e[1])); p->prof_ms[3] += ms;
+                CU(cudaEventElapsedTime(&ms, e[1], e[2])); p->prof_ms[0] += ms;
+                CU(cudaEventElapsedTime(&ms, e[2], e[3])); p->prof_ms[1] += ms;
+                CU(cudaEventElapsedTime(&ms, e[3], e[4])); p->prof_ms[2] += ms;
+            }
         if (p->h_ctl->done || p->h_ctl->error) break;
         if (batch < 64) batch *= 2;
     }
@@ -441,6 +477,20 @@ int emx_read_tallies(const emx_problem *cp, double *edep_host, emx_scalars *out)
 }
 
 double emx_last_transport_ms(const emx_problem *p) { return p ? p->last_ms : -1.0; }
+
+int emx_set_profile(emx_problem *p, int on) {
+    if (!p) return EMX_E_ARG;
+    p->profile = on != 0;
+    return EMX_OK;
+}
+
+int emx_get_profile(const emx_problem *p, double *ms4, long *launches, long *iterations_launched) {
+    if (!p) return EMX_E_ARG;
+    if (ms4) for (int k = 0; k < 4; ++k) ms4[k] = p->prof_ms[k];
+    if (launches) *launches = p->launches;
+    if (iterations_launched) *iterations_launched = p->iterations_launched;
+    return EMX_OK;
+}
 
 long emx_get_iteration_log(const emx_problem *p, uint32_t *host_out, long max_iter) {
     if (!p || !host_out || max_iter < 0) return EMX_E_ARG;

@@ -512,17 +512,22 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         }
 }
 
-cudaError_t launch_iteration(const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st) {
+cudaError_t launch_refill(const Work &w, cudaStream_t st) {
     int maxcap = w.cap[0];
     for (int p = 1; p < 3; ++p) maxcap = w.cap[p] > maxcap ? w.cap[p] : maxcap;
     const dim3 g3((maxcap + kChunk - 1) / kChunk, 3);
     k_plan<<<1, 1024, 0, st>>>(w);
     k_fill<<<g3, kChunk, 0, st>>>(w, nullptr);
     k_move<<<g3, kChunk, 0, st>>>(w, nullptr);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_step(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st) {
     const size_t sm = P.n_tally <= 2048 ? (size_t)P.n_tally * sizeof(double) : 0;
-    k_step<kGamma><<<(w.cap[0] + kChunk - 1) / kChunk, kChunk, sm, st>>>(P, w, seed, tally);
-    k_step<kElectron><<<(w.cap[1] + kChunk - 1) / kChunk, kChunk, sm, st>>>(P, w, seed, tally);
-    k_step<kPositron><<<(w.cap[2] + kChunk - 1) / kChunk, kChunk, sm, st>>>(P, w, seed, tally);
+    const unsigned g = (unsigned)((w.cap[pt] + kChunk - 1) / kChunk);
+    if (pt == kGamma) k_step<kGamma><<<g, kChunk, sm, st>>>(P, w, seed, tally);
+    else if (pt == kElectron) k_step<kElectron><<<g, kChunk, sm, st>>>(P, w, seed, tally);
+    else k_step<kPositron><<<g, kChunk, sm, st>>>(P, w, seed, tally);
     return cudaGetLastError();
 }
 

@@ -120,12 +120,21 @@ def test_single_step_parity(emx, emo, cfg, n):
     gin = (emx.Track * n).from_buffer_copy(bytes(tr))
     got = states.result_arrays(G.step_batch(gin, desc["seed"]))
     E_in = np.array([t.E for t in tr])
-    n_bad, worst, rep = states.compare_steps(ref, got, E_in)
+    # field steps that end because the substep budget ran out (action TRUNC) return "whatever was travelled":
+    # the sum of ~1000 adaptive substeps whose sizes depend on pow() of an ill-conditioned error estimate, so
+    # they agree only to ~1e-9; they are compared separately and counted
+    trunc = (ref["action"] == 4) & (got["action"] == 4) & (np.array([t.ptype for t in tr]) != 0) & (cfg >= 3)
+    n_bad, worst, rep = states.compare_steps(ref, got, E_in, skip=trunc)
     # level 1: action, process, secondary counts and ids, draw counts, cells: bit-exact.  States whose
     # outcome hinges on a comparison within rounding of equality may differ; they are counted (expected 0)
-    assert n_bad <= max(1, n // 20000), rep
+    assert n_bad <= (0 if cfg < 3 else 2), rep
     big = {k: v for k, v in rep.items() if isinstance(v, float) and v > 1e-13}
-    assert worst <= (RTOL2 if cfg < 3 else 1e-9), big          # field steps: see DESIGN.md section 6
+    # level 2: 1e-12; multi-substep field steps accumulate up to ~100 substeps of rounding: 1e-11
+    assert worst <= (RTOL2 if cfg < 3 else 1e-11), big
+    if trunc.any():
+        _, w2, rep2 = states.compare_steps(ref, got, E_in, skip=~trunc)
+        assert w2 <= 1e-6, rep2
+        assert trunc.sum() <= n // 100
     # coverage of the branches
     acts = np.bincount(ref["action"], minlength=5)
     assert acts[1] > 0 and (cfg == 0 or acts[3] > 0)
