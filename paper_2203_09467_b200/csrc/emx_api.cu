@@ -357,8 +357,14 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     Work w;
     const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog);
     if (need > workspace_bytes) return fail(p, EMX_E_CAPACITY, "emx_transport: workspace smaller than emx_workspace_bytes()");
+    // admission limits (R8): about 20 MeV of shower energy in flight per queued record at the peak of
+    // the queue (measured on configs 1-4), with a factor 4 of headroom below the capacity
+    w.n_primaries = pr.n;
+    w.wave = (int)(n_slots / 256 < 256 ? 256 : (n_slots / 256 > 4096 ? 4096 : n_slots / 256));
+    w.queue_soft = queue_capacity / 4;
+    w.inflight_cap = 5.0 * (double)queue_capacity;
     CU(cudaEventRecord(p->ev0, st));
-    CU(launch_load_primaries(w, pr, st));
+    CU(launch_init(w, pr, st));
     p->launches = 1;
     p->iterations_launched = 0;
     for (double &v : p->prof_ms) v = 0.0;
@@ -374,7 +380,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         }
         for (int k = 0; k < batch; ++k) {
             if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
-            CU(launch_refill(w, st));
+            CU(launch_refill(w, pr, st));
             for (int pt = 0; pt < 3; ++pt) {
                 if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
                 CU(launch_step(pt, p->P, w, seed, p->d_tally, st));

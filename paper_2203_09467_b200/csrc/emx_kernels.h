@@ -23,13 +23,13 @@ struct Primaries {
     const int *vol, *surf;  // surf may be null
 };
 
-// resets the control block and pushes every primary onto the stack of its type (lowest index on top)
-cudaError_t launch_load_primaries(const Work &w, const Primaries &pr, cudaStream_t st);
-// one iteration of the loop = launch_refill (k_plan, k_fill, k_move) then launch_step for the three pools;
-// tally = device edep array
-cudaError_t launch_refill(const Work &w, cudaStream_t st);
+// resets the control block, totals the injected energy
+cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st);
+// one iteration of the loop = launch_refill (k_admit, k_plan, k_fill, k_move) then launch_step for the three
+// pools; tally = device edep array
+cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st);
 cudaError_t launch_step(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st);
-constexpr int kLaunchesPerIteration = 6;
+constexpr int kLaunchesPerIteration = 7;
 // level-1 hook: the refill index logic alone on a caller-supplied alive[] (see include/emx.h)
 cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
                                int *scratch, cudaStream_t st);

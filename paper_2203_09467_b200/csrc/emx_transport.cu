@@ -42,20 +42,12 @@ __device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Primaries -> stacks.  One block; primaries of each type keep ascending index order from the top of
-// their stack downwards, so they enter the pools in ascending order and only after every secondary above
-// them has been consumed (R8).
-__global__ void __launch_bounds__(1024) k_load_primaries(Work w, Primaries pr) {
+// Loop start: clear the control block, total the injected energy and the primaries per type.
+__global__ void __launch_bounds__(1024) k_init(Work w, Primaries pr) {
     __shared__ int s_cnt[3][32];
-    __shared__ int s_total[3], s_base[3];
     __shared__ double s_E[32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     Ctl *c = w.ctl;
-    if (tid == 0) {
-        Ctl z = Ctl();
-        *c = z;
-    }
-    // pass 1: totals per type and the injected energy
     int cnt[3] = {0, 0, 0};
     double ein = 0.0;
     for (long i = tid; i < pr.n; i += blockDim.x) {
@@ -74,25 +66,74 @@ __global__ void __launch_bounds__(1024) k_load_primaries(Work w, Primaries pr) {
     if (lane == 0) s_E[wid] = ein;
     __syncthreads();
     if (tid == 0) {
+        Ctl z = Ctl();
         double e = 0.0;
         for (int k = 0; k < 32; ++k) e += s_E[k];
         for (int p = 0; p < 3; ++p) {
             int t = 0;
             for (int k = 0; k < 32; ++k) t += s_cnt[p][k];
+            z.tracks[p] = (unsigned long long)t;
+        }
+        z.E_in = e;
+        *c = z;
+    }
+}
+
+// A0, first half: admission of primaries (R8).  One block, run at the start of every iteration.  While the
+// shower energy in flight and the stacks are below their soft limits, the next `wave` primaries are pushed
+// onto the stacks of their types, lowest index on top, so they enter the pools in ascending order at the
+// refill that follows.  Histories do not depend on when a primary is admitted (keyed RNG, C2); admission only
+// bounds the number of queued records (the queue had to hold 2.5e7 initializers).
+__global__ void __launch_bounds__(1024) k_admit(Work w, Primaries pr) {
+    __shared__ int s_cnt[3][32];
+    __shared__ int s_total[3], s_base[3];
+    __shared__ double s_E[32];
+    __shared__ int s_go;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    Ctl *c = w.ctl;
+    if (c->done) return;
+    const long long next = c->next_primary;
+    if (next >= pr.n) return;
+    const long long queued = (long long)c->q_top[0] + c->q_top[1] + c->q_top[2];
+    const double inflight = c->E_admitted - (c->edep_total + c->escaped + c->looper);
+    if (inflight >= w.inflight_cap || queued >= w.queue_soft) return;
+    const long long A = (pr.n - next) < (long long)w.wave ? (pr.n - next) : (long long)w.wave;
+    // pass 1: counts per type and energy of the window
+    int cnt[3] = {0, 0, 0};
+    double ein = 0.0;
+    for (long long k = tid; k < A; k += blockDim.x) {
+        const int pt = pr.ptype[next + k];
+        cnt[0] += (pt == 0);
+        cnt[1] += (pt == 1);
+        cnt[2] += (pt == 2);
+        ein += pr.E[next + k] + (pt == kPositron ? 2.0 * kMe : 0.0);
+    }
+    for (int p = 0; p < 3; ++p) {
+        int v = cnt[p];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) s_cnt[p][wid] = v;
+    }
+    for (int o = 16; o > 0; o >>= 1) ein += __shfl_down_sync(0xffffffffu, ein, o);
+    if (lane == 0) s_E[wid] = ein;
+    __syncthreads();
+    if (tid == 0) {
+        int go = 1;
+        for (int p = 0; p < 3; ++p) {
+            int t = 0;
+            for (int k = 0; k < 32; ++k) t += s_cnt[p][k];
             s_total[p] = t;
             s_base[p] = 0;
-            c->q_top[p] = t;
-            c->tracks[p] = (unsigned long long)t;
-            if (t > w.qcap[p]) c->error = EMX_E_CAPACITY;
+            if (c->q_top[p] + t > w.qcap[p]) go = 0;  // no room: try again in a later iteration
         }
-        c->E_in = e;
+        s_go = go;
     }
     __syncthreads();
-    if (c->error) return;
+    if (!s_go) return;
     // pass 2: stable rank of each primary inside its type, tile by tile
-    for (long base = 0; base < pr.n; base += blockDim.x) {
-        const long i = base + tid;
-        const int pt = (i < pr.n) ? pr.ptype[i] : -1;
+    for (long long base = 0; base < A; base += blockDim.x) {
+        const long long k = base + tid;
+        const long long i = next + k;
+        const int pt = (k < A) ? pr.ptype[i] : -1;
         int rank = 0;
         for (int p = 0; p < 3; ++p) {
             const unsigned b = __ballot_sync(0xffffffffu, pt == p);
@@ -102,8 +143,8 @@ __global__ void __launch_bounds__(1024) k_load_primaries(Work w, Primaries pr) {
         __syncthreads();
         if (pt >= 0) {
             int before = s_base[pt];
-            for (int k = 0; k < wid; ++k) before += s_cnt[pt][k];
-            const int r = s_total[pt] - 1 - (before + rank);  // lowest index on top
+            for (int q = 0; q < wid; ++q) before += s_cnt[pt][q];
+            const int r = c->q_top[pt] + s_total[pt] - 1 - (before + rank);  // lowest index on top
             const QueueSoA &q = w.q[pt];
             q.x[r] = pr.pos3[3 * i];
             q.y[r] = pr.pos3[3 * i + 1];
@@ -120,15 +161,22 @@ __global__ void __launch_bounds__(1024) k_load_primaries(Work w, Primaries pr) {
         __syncthreads();
         if (tid < 3) {
             int t = 0;
-            for (int k = 0; k < 32; ++k) t += s_cnt[tid][k];
+            for (int q = 0; q < 32; ++q) t += s_cnt[tid][q];
             s_base[tid] += t;
         }
         __syncthreads();
     }
+    if (tid == 0) {
+        double e = 0.0;
+        for (int k = 0; k < 32; ++k) e += s_E[k];
+        for (int p = 0; p < 3; ++p) c->q_top[p] += s_total[p];
+        c->next_primary = next + A;
+        c->E_admitted += e;
+    }
 }
 
-cudaError_t launch_load_primaries(const Work &w, const Primaries &pr, cudaStream_t st) {
-    k_load_primaries<<<1, 1024, 0, st>>>(w, pr);
+cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st) {
+    k_init<<<1, 1024, 0, st>>>(w, pr);
     return cudaGetLastError();
 }
 
@@ -211,21 +259,22 @@ __global__ void __launch_bounds__(1024) k_plan(Work w) {
             w.log[2 * c->iter] = (uint32_t)live;
             w.log[2 * c->iter + 1] = (uint32_t)queued;
         }
-        if (live == 0) {
+        if (live == 0 && c->next_primary >= w.n_primaries) {
             c->done = 1;
             c->m_step[0] = c->m_step[1] = c->m_step[2] = 0;
         } else {
             c->iter += 1;
             // R7: a step whose secondaries do not fit on the stacks is not committed and is re-executed in a
             // later iteration with the same (tid, step) and hence the same draws; if a whole iteration commits
-            // nothing, the stacks are too small for this problem
+            // nothing although tracks are live, the stacks are too small for this problem
             c->m_step[0] = (int)ng;
             c->m_step[1] = (int)ne;
             c->m_step[2] = (int)np;
-            if (c->iter > 1 && c->progress == 0ull) {
+            if (c->had_live && c->progress == 0ull) {
                 c->error = EMX_E_CAPACITY;
                 c->done = 1;
             }
+            c->had_live = live > 0 ? 1 : 0;
             c->progress = 0ull;
         }
     }
@@ -305,7 +354,7 @@ __global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
 // lanes write to consecutive records.  Energy deposition is accumulated per block in shared memory and
 // flushed with one atomic per touched tally.
 struct BlockAcc {
-    double sc[3];           // escaped, below_cut, looper
+    double sc[4];           // escaped, below_cut, looper, deposited
     unsigned cnt[16];       // [0..7] interactions, [8] null, [9..11] tracks created by type, [12] steps
 };
 
@@ -339,7 +388,7 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
     const bool use_smem = P.n_tally <= 2048;
     if (use_smem)
         for (int k = threadIdx.x; k < P.n_tally; k += kChunk) s_tally[k] = 0.0;
-    if (threadIdx.x < 3) acc.sc[threadIdx.x] = 0.0;
+    if (threadIdx.x < 4) acc.sc[threadIdx.x] = 0.0;
     if (threadIdx.x < 16) acc.cnt[threadIdx.x] = 0u;
     __syncthreads();
 
@@ -469,6 +518,7 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
     // ---- A10: tallies and counters
     if (commit) {
         if (o.edep != 0.0) {
+            atomicAdd(&acc.sc[3], o.edep);
             const int tl = P.vol[vol0].tally;
             if (tl >= 0) {
                 if (use_smem) atomicAdd(&s_tally[tl], o.edep);
@@ -496,6 +546,7 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         if (acc.sc[0] != 0.0) atomicAdd(&c->escaped, acc.sc[0]);
         if (acc.sc[1] != 0.0) atomicAdd(&c->below_cut, acc.sc[1]);
         if (acc.sc[2] != 0.0) atomicAdd(&c->looper, acc.sc[2]);
+        if (acc.sc[3] != 0.0) atomicAdd(&c->edep_total, acc.sc[3]);
     }
     if (threadIdx.x < 12) {
         const unsigned v = acc.cnt[threadIdx.x];
@@ -512,7 +563,8 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         }
 }
 
-cudaError_t launch_refill(const Work &w, cudaStream_t st) {
+cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
+    k_admit<<<1, 1024, 0, st>>>(w, pr);
     int maxcap = w.cap[0];
     for (int p = 1; p < 3; ++p) maxcap = w.cap[p] > maxcap ? w.cap[p] : maxcap;
     const dim3 g3((maxcap + kChunk - 1) / kChunk, 3);
@@ -568,6 +620,7 @@ cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const u
     w.qcap[0] = w.qcap[1] = w.qcap[2] = 0x7fffffff;
     w.log = nullptr;
     w.max_log = 0;
+    w.n_primaries = 0;
     cudaMemsetAsync(w.trk[0].alive, 0, (size_t)capacity, st);
     if (n_live > 0) cudaMemcpyAsync(w.trk[0].alive, alive, (size_t)n_live, cudaMemcpyDeviceToDevice, st);
     cudaMemsetAsync(src, 0xFF, (size_t)capacity * sizeof(int32_t), st);

@@ -44,9 +44,12 @@ struct Ctl {
     int q_top[3];
     int m_step[3];  // tracks to step this iteration (= n_live)
     PoolPlan plan[3];
-    int done, error;
+    int done, error, had_live;
     unsigned long long iter;
     unsigned long long progress;  // steps committed + tombstones retired in the current iteration (R7)
+    long long next_primary;       // primaries [0, next_primary) have been admitted
+    double E_admitted;            // energy of the admitted primaries (e+ with their 2 me)
+    double edep_total;            // all energy deposited so far (every cell, tallied or not)
     double escaped, below_cut, looper, E_in;
     unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls, peak_live, peak_queue;
 };
@@ -62,6 +65,12 @@ struct Work {
     Ctl *ctl;
     uint32_t *log;  // per iteration: live, queued
     int max_log;
+    // admission of primaries (R8): up to `wave` primaries enter per iteration while the energy in
+    // flight (admitted - deposited - escaped) is below inflight_cap and fewer than queue_soft records wait
+    long long n_primaries;
+    int wave;
+    long long queue_soft;
+    double inflight_cap;
 };
 
 // bytes of one slot / one record, for the workspace carve-up and the roofline arithmetic
