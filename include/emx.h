@@ -228,10 +228,12 @@ int emx_read_tallies(const emx_problem *p, double *edep_host, emx_scalars *out);
  * measured with CUDA events on the caller's stream; < 0 if none. */
 double emx_last_transport_ms(const emx_problem *p);
 
-/* Per-kernel timing of the loop.  With profiling on, emx_transport brackets every launch group of every
+/* Per-kernel timing of the loop.  Normally emx_transport runs the loop as a CUDA graph (8 iterations per
+ * graph, the three step kernels as parallel branches) on internal streams ordered after `stream`.  With
+ * profiling on (on = 1) it launches kernel by kernel on `stream` instead and brackets every launch group of every
  * iteration with CUDA events on the caller's stream and sums the elapsed times.  emx_get_profile: ms4[4] =
- * milliseconds of the last transport spent in { step kernel gamma, step kernel e-, step kernel e+, refill
- * (plan + fill + move) }; *launches = kernels launched by the last transport (always counted);
+ * milliseconds of the last transport spent in { the step kernel, the refill kernels (admit + count + plan +
+ * fill + move), 0, 0 }; *launches = kernels launched by the last transport (always counted);
  * *iterations_launched = iterations enqueued (>= iterations needed: the host checks the done flag once per
  * batch).  Any output pointer may be NULL. */
 int emx_set_profile(emx_problem *p, int on);
@@ -240,6 +242,11 @@ int emx_get_profile(const emx_problem *p, double *ms4, long *launches, long *ite
 /* Per-iteration diagnostics of the last transport (Fig. 5): up to `max_iter` rows of
  * { live tracks, queued initializers } as uint32 pairs in HOST memory; returns rows written. */
 long emx_get_iteration_log(const emx_problem *p, uint32_t *host_out, long max_iter);
+
+/* Time per step iteration of the last transport (Fig. 5b), recorded when profiling is on:
+ * up to `max_iter` rows of { refill ms, step-kernel ms } as float pairs in HOST memory; returns rows written
+ * (iterations enqueued after the loop finished are included and cost only their launch overhead). */
+long emx_get_iteration_times(const emx_problem *p, float *host_out, long max_iter);
 
 /* ---- parity hooks ---- */
 

@@ -22,7 +22,7 @@ struct emx_problem {
     Volume *d_vol = nullptr;
     double *d_tab = nullptr;
     double *d_scratch = nullptr;
-    int *d_nb_off = nullptr, *d_nb_list = nullptr;
+    int *d_nb_off = nullptr, *d_nb_list = nullptr, *d_nb2_off = nullptr, *d_nb2_list = nullptr;
     double *d_tally = nullptr;
     Params P;
     // results of the last transport
@@ -37,8 +37,14 @@ struct emx_problem {
     // optional per-kernel timing of the loop (emx_set_profile)
     bool profile = false;
     std::vector<cudaEvent_t> prof_ev;
-    double prof_ms[4] = {0, 0, 0, 0};  // k_step gamma, e-, e+, refill (plan + fill + move)
+    double prof_ms[4] = {0, 0, 0, 0};  // k_step_all, refill (admit + count + plan + fill + move), unused, unused
+    int n_sm = 148;
     long launches = 0, iterations_launched = 0;
+    std::vector<float> iter_ms;  // per iteration: refill ms, step ms (profiling on)
+    // iteration graph: internal streams (the caller's stream may be the legacy stream, which cannot be captured)
+    cudaStream_t s0 = nullptr, s1 = nullptr, s2 = nullptr;
+    cudaEvent_t evFork = nullptr, evJ1 = nullptr, evJ2 = nullptr, evIn = nullptr, evOut = nullptr;
+    bool use_graph = true;
 };
 
 namespace {
@@ -156,6 +162,10 @@ void emx_destroy(emx_problem *p) {
     if (p->ev0) cudaEventDestroy(p->ev0);
     if (p->ev1) cudaEventDestroy(p->ev1);
     for (cudaEvent_t e : p->prof_ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : {p->evFork, p->evJ1, p->evJ2, p->evIn, p->evOut})
+        if (e) cudaEventDestroy(e);
+    for (cudaStream_t s : {p->s0, p->s1, p->s2})
+        if (s) cudaStreamDestroy(s);
     delete p;
 }
 
@@ -251,6 +261,8 @@ int emx_build_tables(emx_problem *p, void *stream) {
 
     std::vector<int> nb_off, nb_list;
     build_neighbour_lists(hp, nb_off, nb_list);
+    std::vector<int> nb2_off, nb2_list;
+    build_nonlisting_lists(hp, nb2_off, nb2_list);
     const size_t n = (size_t)hp.ph.n_E, nm = hp.mat.size(), ns = hp.surf_v.size(), nv = hp.vol.size();
     Carve c{nullptr};
     auto layout = [&](Carve &cv) {
@@ -262,6 +274,8 @@ int emx_build_tables(emx_problem *p, void *stream) {
         p->d_scratch = cv.take<double>((nm ? nm : 1) * n);
         p->d_nb_off = cv.take<int>(nb_off.size());
         p->d_nb_list = cv.take<int>(nb_list.size() ? nb_list.size() : 1);
+        p->d_nb2_off = cv.take<int>(nb2_off.size());
+        p->d_nb2_list = cv.take<int>(nb2_list.size() ? nb2_list.size() : 1);
         p->d_tally = cv.take<double>(hp.n_tally ? hp.n_tally : 1);
     };
     layout(c);
@@ -279,6 +293,9 @@ int emx_build_tables(emx_problem *p, void *stream) {
     CU(cudaMemcpyAsync(p->d_nb_off, nb_off.data(), nb_off.size() * sizeof(int), cudaMemcpyHostToDevice, st));
     if (!nb_list.empty())
         CU(cudaMemcpyAsync(p->d_nb_list, nb_list.data(), nb_list.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(p->d_nb2_off, nb2_off.data(), nb2_off.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+    if (!nb2_list.empty())
+        CU(cudaMemcpyAsync(p->d_nb2_list, nb2_list.data(), nb2_list.size() * sizeof(int), cudaMemcpyHostToDevice, st));
 
     const GridConsts g = grid_consts(hp.ph);
     if (nm) {
@@ -309,15 +326,30 @@ int emx_build_tables(emx_problem *p, void *stream) {
     P.tab = p->d_tab;
     P.nb_off = p->d_nb_off;
     P.nb_list = p->d_nb_list;
+    P.nb2_off = p->d_nb2_off;
+    P.nb2_list = p->d_nb2_list;
     const double bm = sqrt(hp.B[0] * hp.B[0] + hp.B[1] * hp.B[1] + hp.B[2] * hp.B[2]);
     P.Bmag = bm;
     for (int i = 0; i < 3; ++i) P.Bhat[i] = bm > 0.0 ? hp.B[i] / bm : 0.0;
     P.lnE0 = g.lnE0;
     P.dlnE = g.dlnE;
     P.inv_dlnE = g.inv_dlnE;
+    {
+        int dev = 0, sms = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        p->n_sm = sms > 0 ? sms : 148;
+    }
     if (!p->h_ctl) CU(cudaMallocHost(&p->h_ctl, sizeof(Ctl)));
     if (!p->ev0) CU(cudaEventCreate(&p->ev0));
     if (!p->ev1) CU(cudaEventCreate(&p->ev1));
+    if (!p->s0) {
+        CU(cudaStreamCreateWithFlags(&p->s0, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&p->s1, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&p->s2, cudaStreamNonBlocking));
+        for (cudaEvent_t *e : {&p->evFork, &p->evJ1, &p->evJ2, &p->evIn, &p->evOut})
+            CU(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    }
     hp.built = true;
     p->have_ctl = false;
     return EMX_OK;
@@ -368,11 +400,57 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     p->launches = 1;
     p->iterations_launched = 0;
     for (double &v : p->prof_ms) v = 0.0;
+    p->iter_ms.clear();
+    if (p->use_graph && !p->profile) {
+        // ---- device-driven path: kIterPerGraph iterations captured once as a CUDA graph; inside an iteration
+        // the three step kernels are parallel branches, so the tail of one pool overlaps the start of the next.
+        // The host only looks at the done flag between graph launches.
+        constexpr int kIterPerGraph = 8;
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t exec = nullptr;
+        CU(cudaEventRecord(p->evIn, st));
+        CU(cudaStreamWaitEvent(p->s0, p->evIn, 0));
+        CU(cudaStreamBeginCapture(p->s0, cudaStreamCaptureModeThreadLocal));
+        cudaError_t ce = cudaSuccess;
+        for (int k = 0; k < kIterPerGraph && ce == cudaSuccess; ++k) {
+            ce = launch_refill(w, pr, p->s0);
+            if (ce == cudaSuccess) ce = cudaEventRecord(p->evFork, p->s0);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s1, p->evFork, 0);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s2, p->evFork, 0);
+            if (ce == cudaSuccess) ce = launch_step_pool(kPositron, p->P, w, seed, p->d_tally, p->n_sm, p->s1);
+            if (ce == cudaSuccess) ce = launch_step_pool(kElectron, p->P, w, seed, p->d_tally, p->n_sm, p->s2);
+            if (ce == cudaSuccess) ce = launch_step_pool(kGamma, p->P, w, seed, p->d_tally, p->n_sm, p->s0);
+            if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ1, p->s1);
+            if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ2, p->s2);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ1, 0);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ2, 0);
+        }
+        cudaError_t ce2 = cudaStreamEndCapture(p->s0, &graph);
+        if (ce != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return fail_cuda(p, ce, "emx_transport: graph capture"); }
+        CU(ce2);
+        ce = cudaGraphInstantiate(&exec, graph, 0);
+        if (ce != cudaSuccess) { cudaGraphDestroy(graph); return fail_cuda(p, ce, "cudaGraphInstantiate"); }
+        int batch = 1;
+        for (;;) {
+            for (int k = 0; k < batch && ce == cudaSuccess; ++k) ce = cudaGraphLaunch(exec, p->s0);
+            p->launches += (long)batch * kIterPerGraph * kLaunchesPerIteration;
+            p->iterations_launched += (long)batch * kIterPerGraph;
+            if (ce == cudaSuccess) ce = cudaMemcpyAsync(p->h_ctl, w.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, p->s0);
+            if (ce == cudaSuccess) ce = cudaStreamSynchronize(p->s0);
+            if (ce != cudaSuccess || p->h_ctl->done || p->h_ctl->error) break;
+            if (batch < 8) batch *= 2;
+        }
+        cudaGraphExecDestroy(exec);
+        cudaGraphDestroy(graph);
+        if (ce != cudaSuccess) return fail_cuda(p, ce, "emx_transport: iteration graph");
+        CU(cudaEventRecord(p->evOut, p->s0));
+        CU(cudaStreamWaitEvent(st, p->evOut, 0));
+    } else {
     int batch = 8;
     for (;;) {
         size_t ne = 0;
         if (p->profile) {
-            while (p->prof_ev.size() < (size_t)batch * 5) {
+            while (p->prof_ev.size() < (size_t)batch * 3) {
                 cudaEvent_t e;
                 CU(cudaEventCreate(&e));
                 p->prof_ev.push_back(e);
@@ -381,10 +459,8 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         for (int k = 0; k < batch; ++k) {
             if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
             CU(launch_refill(w, pr, st));
-            for (int pt = 0; pt < 3; ++pt) {
-                if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
-                CU(launch_step(pt, p->P, w, seed, p->d_tally, st));
-            }
+            if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
+            CU(launch_step(p->P, w, seed, p->d_tally, p->n_sm, st));
             if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
         }
         p->launches += (long)batch * kLaunchesPerIteration;
@@ -394,14 +470,13 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         if (p->profile)
             for (int k = 0; k < batch; ++k) {
                 float ms;
-                const cudaEvent_t *e = &p->prof_ev[(size_t)k * 5];
-                CU(cudaEventElapsedTime(&ms, e[0], e[1])); p->prof_ms[3] += ms;
-                CU(cudaEventElapsedTime(&ms, e[1], e[2])); p->prof_ms[0] += ms;
-                CU(cudaEventElapsedTime(&ms, e[2], e[3])); p->prof_ms[1] += ms;
-                CU(cudaEventElapsedTime(&ms, e[3], e[4])); p->prof_ms[2] += ms;
+                const cudaEvent_t *e = &p->prof_ev[(size_t)k * 3];
+                CU(cudaEventElapsedTime(&ms, e[0], e[1])); p->prof_ms[1] += ms; p->iter_ms.push_back(ms);
+                CU(cudaEventElapsedTime(&ms, e[1], e[2])); p->prof_ms[0] += ms; p->iter_ms.push_back(ms);
             }
         if (p->h_ctl->done || p->h_ctl->error) break;
         if (batch < 64) batch *= 2;
+    }
     }
     CU(cudaEventRecord(p->ev1, st));
     CU(cudaEventSynchronize(p->ev1));
@@ -486,7 +561,8 @@ double emx_last_transport_ms(const emx_problem *p) { return p ? p->last_ms : -1.
 
 int emx_set_profile(emx_problem *p, int on) {
     if (!p) return EMX_E_ARG;
-    p->profile = on != 0;
+    p->profile = (on & 1) != 0;
+    p->use_graph = (on & 2) == 0;  // bit 1: plain stream launches without profiling (diagnostics)
     return EMX_OK;
 }
 
@@ -503,6 +579,14 @@ long emx_get_iteration_log(const emx_problem *p, uint32_t *host_out, long max_it
     long n = (long)(p->iter_log.size() / 2);
     if (n > max_iter) n = max_iter;
     if (n) memcpy(host_out, p->iter_log.data(), (size_t)n * 2 * sizeof(uint32_t));
+    return n;
+}
+
+long emx_get_iteration_times(const emx_problem *p, float *host_out, long max_iter) {
+    if (!p || !host_out || max_iter < 0) return EMX_E_ARG;
+    long n = (long)(p->iter_ms.size() / 2);
+    if (n > max_iter) n = max_iter;
+    if (n) memcpy(host_out, p->iter_ms.data(), (size_t)n * 2 * sizeof(float));
     return n;
 }
 

@@ -11,10 +11,19 @@
 
 #if defined(__CUDACC__)
 #define EMX_HD __host__ __device__ __forceinline__
-#define EMX_HDN __host__ __device__ __noinline__
+// shared, out-of-line building blocks: the fused step kernel is instruction-cache bound when everything is
+// inlined (345 KB of SASS), so the routines with many call sites exist once
+#ifndef EMX_OUTLINE
+#define EMX_OUTLINE 0
+#endif
+#if EMX_OUTLINE
+#define EMX_NI inline __host__ __device__ __noinline__
+#else
+#define EMX_NI __host__ __device__ __forceinline__
+#endif
 #else
 #define EMX_HD inline
-#define EMX_HDN
+#define EMX_NI inline
 #endif
 
 namespace emx {
@@ -56,9 +65,25 @@ struct Params {
     const double *tab;      // [n_mat][EMX_NTABLE][n_E]
     const int *nb_off;      // neighbour candidates: cells having face (S, sense); index 2*S + (sense > 0)
     const int *nb_list;
+    const int *nb2_off;     // per surface S: cells that do not list S at all (the only other cells that can match)
+    const int *nb2_list;
     double Bmag, Bhat[3];
     double lnE0, dlnE, inv_dlnE;  // grid: x_j = lnE0 + j * dlnE
 };
+
+// libm calls of the step path, out of line (one copy each instead of one per call site)
+EMX_NI double m_log(double x) { return log(x); }
+EMX_NI double m_exp(double x) { return exp(x); }
+EMX_NI double m_pow(double x, double y) { return pow(x, y); }
+EMX_NI double m_cbrt(double x) { return cbrt(x); }
+EMX_NI void m_sincos(double a, double &s, double &c) {
+#if defined(__CUDA_ARCH__)
+    sincos(a, &s, &c);
+#else
+    s = sin(a);
+    c = cos(a);
+#endif
+}
 
 struct Vec3 {
     double x, y, z;
@@ -76,7 +101,7 @@ struct Philox4 {
     uint32_t w[4];
 };
 
-EMX_HD Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
+EMX_NI Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const uint64_t p0 = (uint64_t)0xD2511F53u * c0;

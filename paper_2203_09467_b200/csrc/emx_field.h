@@ -32,7 +32,7 @@ EMX_HD void rk4_step(const Vec3 &x, const Vec3 &u, double kappa, const double B[
 }
 
 // one step of h against two of h/2: err = |x_full - x_half|, result = half-step state, u renormalised
-EMX_HD void rk4_doubling(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, Vec3 &x1, Vec3 &u1,
+EMX_NI void rk4_doubling(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, Vec3 &x1, Vec3 &u1,
                          double &err) {
     Vec3 xf, uf, xm, um;
     rk4_step(x, u, kappa, B, h, xf, uf);
@@ -47,7 +47,7 @@ EMX_HD void rk4_doubling(const Vec3 &x, const Vec3 &u, double kappa, const doubl
 
 // Propagate up to s_max inside cell `vol`.  Returns the arc length travelled; hit = surface reached
 // (-1 none).  x, u are updated; on_surf is the surface the track starts on.
-EMX_HD double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
+EMX_NI double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
                               int &hit) {
     const double eps = P.ph.field_eps;
     double s_done = 0.0;
@@ -63,7 +63,7 @@ EMX_HD double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Ve
         double err;
         rk4_doubling(x, u, kappa, P.Bhat, h, x1, u1, err);
         if (err > eps && h > 1e-9) {  // too inaccurate: shrink and retry
-            const double f = 0.9 * pow(eps / err, 0.2);
+            const double f = 0.9 * m_pow(eps / err, 0.2);
             h *= (f > 0.2 ? f : 0.2);
             continue;
         }
@@ -92,7 +92,7 @@ EMX_HD double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Ve
             surf = -1;
             if (s_done >= s_max * (1.0 - 1e-14)) break;
             const double e = err > eps / 3125.0 ? err : eps / 3125.0;
-            const double f = 0.9 * pow(eps / e, 0.2);
+            const double f = 0.9 * m_pow(eps / e, 0.2);
             h *= (f < 5.0 ? f : 5.0);
             continue;
         }

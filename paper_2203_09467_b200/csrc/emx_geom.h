@@ -19,7 +19,7 @@ EMX_HD double surf_g(int type, const Vec3 &x, const Vec3 &u) {
 
 // Distance along u from x to the nearest face of cell `vol`; on_surf = surface the track is flagged on
 // (-1 none).  Returns +inf and hit = -1 when no face is ahead.  Ties -> lowest surface id.
-EMX_HD double distance_to_boundary(const Params &P, int vol, const Vec3 &x, const Vec3 &u, int on_surf, int &hit) {
+EMX_NI double distance_to_boundary(const Params &P, int vol, const Vec3 &x, const Vec3 &u, int on_surf, int &hit) {
     const Volume &c = P.vol[vol];
     double best = kInf;
     int bs = -1;
@@ -97,20 +97,22 @@ EMX_HD bool cell_matches(const Params &P, int cid, const Vec3 &x, const Vec3 &u,
 }
 
 // Cell entered when crossing surface S at x with direction u; -1 = left the world.
-// Definition (C8): the lowest cell id whose faces all agree.  Cells that list (S, newsense) as a
-// face are tried first (precomputed per-surface lists, ascending id): in a world tiled without overlap the
-// answer is one of them, except at edges/corners where another surface lies within the tolerance -- then no
-// candidate matches and every cell is scanned in id order, which is the definition itself.
-EMX_HD int neighbour(const Params &P, const Vec3 &x, const Vec3 &u, int S) {
+// Definition (C8): the lowest cell id whose faces all agree.  A cell that lists S with the other
+// sense can never agree, so only two precomputed lists (ascending id) have to be looked at: the cells that
+// list (S, newsense) -- in a world tiled without overlap the answer is one of them -- and, if none of those
+// matches (edges and corners where another surface lies within the tolerance), the cells that do not list S
+// at all.  For a world tiled without overlap this returns the id of the full scan in id order.
+EMX_NI int neighbour(const Params &P, const Vec3 &x, const Vec3 &u, int S) {
     const int newsense = surf_g(P.surf_type[S], x, u) > 0.0 ? 1 : -1;
     const int k = 2 * S + (newsense > 0 ? 1 : 0);
-    const int b = P.nb_off[k], e = P.nb_off[k + 1];
-    for (int j = b; j < e; ++j) {
+    for (int j = P.nb_off[k], e = P.nb_off[k + 1]; j < e; ++j) {
         const int cid = P.nb_list[j];
         if (cell_matches(P, cid, x, u, S, newsense)) return cid;
     }
-    for (int cid = 0; cid < P.n_vol; ++cid)
+    for (int j = P.nb2_off[S], e = P.nb2_off[S + 1]; j < e; ++j) {
+        const int cid = P.nb2_list[j];
         if (cell_matches(P, cid, x, u, S, newsense)) return cid;
+    }
     return -1;
 }
 

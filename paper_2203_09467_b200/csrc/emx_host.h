@@ -89,6 +89,23 @@ inline void build_neighbour_lists(const HostProblem &hp, std::vector<int> &off, 
     off[2 * ns] = (int)list.size();
 }
 
+// off2[S] .. off2[S + 1]: cells that do not list S with either sense, ascending id
+inline void build_nonlisting_lists(const HostProblem &hp, std::vector<int> &off2, std::vector<int> &list2) {
+    const int ns = (int)hp.surf_type.size();
+    off2.assign(ns + 1, 0);
+    list2.clear();
+    for (int S = 0; S < ns; ++S) {
+        off2[S] = (int)list2.size();
+        for (int c = 0; c < (int)hp.vol.size(); ++c) {
+            const Volume &v = hp.vol[c];
+            bool lists = false;
+            for (int i = 0; i < v.n_faces; ++i) lists = lists || (v.surf[i] == S);
+            if (!lists) list2.push_back(c);
+        }
+    }
+    off2[ns] = (int)list2.size();
+}
+
 struct GridConsts {
     double lnE0, dlnE, inv_dlnE;
 };

@@ -19,17 +19,10 @@ EMX_HD void normalise(Vec3 &v, const Vec3 &fallback) {
     }
 }
 
-EMX_HD void sincos_(double a, double &s, double &c) {
-#if defined(__CUDA_ARCH__)
-    sincos(a, &s, &c);
-#else
-    s = sin(a);
-    c = cos(a);
-#endif
-}
+EMX_HD void sincos_(double a, double &s, double &c) { m_sincos(a, s, c); }
 
 // rotate u by polar cosine mu (sine s) and azimuth (cphi, sphi) -- C6 "Common"
-EMX_HD Vec3 rotate(const Vec3 &u, double mu, double s, double cphi, double sphi) {
+EMX_NI Vec3 rotate(const Vec3 &u, double mu, double s, double cphi, double sphi) {
     Vec3 o;
     const double rho2 = u.x * u.x + u.y * u.y;
     if (rho2 > 1e-30) {
@@ -57,14 +50,14 @@ EMX_HD double clamp1(double m) { return m > 1.0 ? 1.0 : (m < -1.0 ? -1.0 : m); }
 EMX_HD double boosted_iso(double xi, double beta) { return clamp1((2.0 * xi - 1.0 + beta) / (beta * (2.0 * xi - 1.0) + 1.0)); }
 
 // ---- Compton, Klein-Nishina (C6.1): photon E -> E1 along u1, electron Te along ue
-EMX_HD void compton(Rng &r, double E, const Vec3 &u, double &E1, Vec3 &u1, double &Te, Vec3 &ue) {
+EMX_NI void compton(Rng &r, double E, const Vec3 &u, double &E1, Vec3 &u1, double &Te, Vec3 &ue) {
     const double k = E / kMe;
     const double e0 = 1.0 / (1.0 + 2.0 * k);
-    const double a1 = -log(e0), a2 = 0.5 * (1.0 - e0 * e0);
+    const double a1 = -m_log(e0), a2 = 0.5 * (1.0 - e0 * e0);
     double eps, t;
     for (;;) {
         const double x1 = r.next(), x2 = r.next(), x3 = r.next();
-        if (x1 * (a1 + a2) < a1) eps = exp(-a1 * x2);
+        if (x1 * (a1 + a2) < a1) eps = m_exp(-a1 * x2);
         else eps = sqrt(e0 * e0 + (1.0 - e0 * e0) * x2);
         t = (1.0 - eps) / (k * eps);
         if (x3 <= 1.0 - eps * t * (2.0 - t) / (1.0 + eps * eps)) break;
@@ -82,7 +75,7 @@ EMX_HD void compton(Rng &r, double E, const Vec3 &u, double &E1, Vec3 &u1, doubl
 }
 
 // ---- photoelectron direction, leading Sauter term p(mu) ~ (1 - mu^2) / (1 - beta mu)^4 (C6.2)
-EMX_HD Vec3 photo_dir(Rng &r, double E, const Vec3 &u) {
+EMX_NI Vec3 photo_dir(Rng &r, double E, const Vec3 &u) {
     const double g = E / kMe + 1.0;
     const double b = beta_of(E);
     const double A = 1.0 / (g * g * b * (1.0 + b));
@@ -109,12 +102,12 @@ EMX_HD double pair_F2(double d, double F) {
     screening(d, a, b);
     return 1.5 * a + 0.5 * b - F;
 }
-EMX_HD bool pair_production(Rng &r, int Z, double E, const Vec3 &u, double &Tm, Vec3 &um, double &Tp, Vec3 &up) {
+EMX_NI bool pair_production(Rng &r, int Z, double E, const Vec3 &u, double &Tm, Vec3 &um, double &Tp, Vec3 &up) {
     const double e0 = kMe / E;
-    const double c = 136.0 * pow((double)Z, -1.0 / 3.0) * e0;
+    const double c = 136.0 * m_pow((double)Z, -1.0 / 3.0) * e0;
     const double F = pair_F(Z, E);
     const double dmin = 4.0 * c;
-    const double dmax = exp((42.24 - F) / 8.368) - 0.952;
+    const double dmax = m_exp((42.24 - F) / 8.368) - 0.952;
     if (!(E > 2.0 * kMe) || dmin >= dmax) return false;
     const double e1 = 0.5 - 0.5 * sqrt(1.0 - dmin / dmax);
     const double emin = e0 > e1 ? e0 : e1;
@@ -124,7 +117,7 @@ EMX_HD bool pair_production(Rng &r, int Z, double E, const Vec3 &u, double &Tm, 
     for (;;) {
         const double x1 = r.next(), x2 = r.next(), x3 = r.next();
         if (x1 * (N1 + N2) < N1) {
-            eps = 0.5 - (0.5 - emin) * cbrt(x2);
+            eps = 0.5 - (0.5 - emin) * m_cbrt(x2);
             if (x3 * F10 <= pair_F1(c / (eps * (1.0 - eps)), F)) break;
         } else {
             eps = emin + (0.5 - emin) * x2;
@@ -149,13 +142,13 @@ EMX_HD bool pair_production(Rng &r, int Z, double E, const Vec3 &u, double &Tm, 
 }
 
 // ---- bremsstrahlung, complete-screening shape (C6.4).  false = null (T <= kc).
-EMX_HD bool bremsstrahlung(Rng &r, double T, double kc, const Vec3 &u, double &k, Vec3 &ug, double &T1, Vec3 &u1) {
+EMX_NI bool bremsstrahlung(Rng &r, double T, double kc, const Vec3 &u, double &k, Vec3 &ug, double &T1, Vec3 &u1) {
     if (!(T > kc)) return false;
-    const double lr = log(T / kc);
+    const double lr = m_log(T / kc);
     double kk;
     for (;;) {
         const double x1 = r.next(), x2 = r.next();
-        kk = kc * exp(x1 * lr);
+        kk = kc * m_exp(x1 * lr);
         if (kk > T) kk = T;
         const double y = kk / T;
         if ((4.0 / 3.0) * x2 <= 4.0 / 3.0 - 4.0 * y / 3.0 + y * y) break;
@@ -171,7 +164,7 @@ EMX_HD bool bremsstrahlung(Rng &r, double T, double kc, const Vec3 &u, double &k
 }
 
 // exact two-body kinematics of a knock-on electron of energy Td on a free electron at rest (C6.5)
-EMX_HD void knock_on(Rng &r, double T, double Td, const Vec3 &u, Vec3 &ud, double &T1, Vec3 &u1) {
+EMX_NI void knock_on(Rng &r, double T, double Td, const Vec3 &u, Vec3 &ud, double &T1, Vec3 &u1) {
     const double p = sqrt(T * (T + 2.0 * kMe)), pd = sqrt(Td * (Td + 2.0 * kMe));
     const double mu = clamp1(Td * (T + 2.0 * kMe) / (p * pd));
     ud = rotate_mu_phi(u, mu, 2.0 * kPi * r.next());
@@ -180,7 +173,7 @@ EMX_HD void knock_on(Rng &r, double T, double Td, const Vec3 &u, Vec3 &ud, doubl
     normalise(u1, u);
 }
 
-EMX_HD bool moller(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec3 &ud, double &T1, Vec3 &u1) {
+EMX_NI bool moller(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec3 &ud, double &T1, Vec3 &u1) {
     if (!(T > 2.0 * Tcut)) return false;
     const double x = Tcut / T, g = T / kMe + 1.0, g2 = g * g;
     const double c = (2.0 * g - 1.0) / g2, a = (g - 1.0) * (g - 1.0) / g2;
@@ -197,7 +190,7 @@ EMX_HD bool moller(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec
     return true;
 }
 
-EMX_HD bool bhabha(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec3 &ud, double &T1, Vec3 &u1) {
+EMX_NI bool bhabha(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec3 &ud, double &T1, Vec3 &u1) {
     if (!(T > Tcut)) return false;
     const double x = Tcut / T, g = T / kMe + 1.0, b2 = 1.0 - 1.0 / (g * g);
     const double y = 1.0 / (g + 1.0), t = 1.0 - 2.0 * y;
@@ -214,15 +207,15 @@ EMX_HD bool bhabha(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec
 }
 
 // ---- two-photon annihilation in flight, Heitler (C6.6)
-EMX_HD void annih_flight(Rng &r, double T, const Vec3 &u, double &k1, Vec3 &u1, double &k2, Vec3 &u2) {
+EMX_NI void annih_flight(Rng &r, double T, const Vec3 &u, double &k1, Vec3 &u1, double &k2, Vec3 &u2) {
     const double g = T / kMe + 1.0;
     const double rr = sqrt((g - 1.0) / (g + 1.0));
     const double elo = 0.5 * (1.0 - rr), ehi = 0.5 * (1.0 + rr);
-    const double lr = log(ehi / elo);
+    const double lr = m_log(ehi / elo);
     double eps;
     for (;;) {
         const double x1 = r.next(), x2 = r.next();
-        eps = elo * exp(x1 * lr);
+        eps = elo * m_exp(x1 * lr);
         if (x2 <= 1.0 - eps + (2.0 * g * eps - 1.0) / (eps * (g + 1.0) * (g + 1.0))) break;
     }
     const double Etot = T + 2.0 * kMe;
@@ -237,7 +230,7 @@ EMX_HD void annih_flight(Rng &r, double T, const Vec3 &u, double &k1, Vec3 &u1, 
 }
 
 // ---- annihilation at rest: two back-to-back me photons, isotropic (C6.6, R12/R25)
-EMX_HD void annih_rest(Rng &r, Vec3 &u1, Vec3 &u2) {
+EMX_NI void annih_rest(Rng &r, Vec3 &u1, Vec3 &u2) {
     const double mu = 2.0 * r.next() - 1.0;
     double sp, cp;
     sincos_(2.0 * kPi * r.next(), sp, cp);

@@ -44,7 +44,7 @@ struct GridPos {
     double f;
 };
 EMX_HD GridPos grid_pos(const Params &P, double E) {
-    const double t = (log(E) - P.lnE0) * P.inv_dlnE;
+    const double t = (m_log(E) - P.lnE0) * P.inv_dlnE;
     int j = (int)floor(t);
     const int n = P.ph.n_E;
     if (j < 0) j = 0;
@@ -60,10 +60,10 @@ EMX_HD const double *table(const Params &P, int mat, int kind) {
 }
 
 // exact inverse of the forward lookup on a range table (C5.9)
-EMX_HD double range_inverse(const Params &P, const double *R, double r) {
+EMX_NI double range_inverse(const Params &P, const double *R, double r) {
     const int n = P.ph.n_E;
-    if (r <= R[0]) return exp(P.lnE0) * (r / R[0]);  // constant dE/dx below the grid (R24)
-    if (r >= R[n - 1]) return exp(P.lnE0 + (n - 1) * P.dlnE);
+    if (r <= R[0]) return m_exp(P.lnE0) * (r / R[0]);  // constant dE/dx below the grid (R24)
+    if (r >= R[n - 1]) return m_exp(P.lnE0 + (n - 1) * P.dlnE);
     int lo = 0, hi = n - 1;  // R[lo] <= r < R[hi]
     while (hi - lo > 1) {
         const int mid = (lo + hi) / 2;
@@ -71,7 +71,7 @@ EMX_HD double range_inverse(const Params &P, const double *R, double r) {
         else hi = mid;
     }
     const double f = (r - R[lo]) / (R[lo + 1] - R[lo]);
-    return exp(P.lnE0 + (lo + f) * P.dlnE);
+    return m_exp(P.lnE0 + (lo + f) * P.dlnE);
 }
 
 // C10: a secondary of type pt; deposited locally instead when below the tracking cut (gamma, e-) or when
@@ -170,7 +170,7 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o) {
         Stot = (PT == kElectron) ? (Sig0 + Sig1) : (Sig0 + Sig1 + Sig2);
         // 4. limits: interaction length resampled every step (R27); continuous-loss step function (R9)
         const double xi = rng.next();
-        s_phys = Stot > 0.0 ? -log(xi) / Stot : kInf;
+        s_phys = Stot > 0.0 ? -m_log(xi) / Stot : kInf;
         action = EMX_A_DISCRETE;
         if (PT != kGamma) {
             double s_loss;

@@ -1,7 +1,7 @@
 // emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the fused
 // per-type step kernel (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
 //
-// One ITERATION = k_plan -> k_fill -> k_move -> k_step<gamma|e-|e+>.  Nothing returns to the host
+// One ITERATION = k_admit -> k_count_dead_pools -> k_plan -> k_fill -> k_move -> k_step_pool<e+|e-|gamma>.  Nothing returns to the host
 // between iterations: pool sizes, stack tops and the done flag live in the device control block.
 #include <cuda_runtime.h>
 #include "emx_kernels.h"
@@ -276,6 +276,7 @@ __global__ void __launch_bounds__(1024) k_plan(Work w) {
             }
             c->had_live = live > 0 ? 1 : 0;
             c->progress = 0ull;
+            c->work_ctr3[0] = c->work_ctr3[1] = c->work_ctr3[2] = 0;
         }
     }
 }
@@ -347,16 +348,23 @@ __global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// A1-A8 + A10: one step of every live track of pool PT.  One thread per slot of the dense prefix; the
-// track is read once, stepped in registers and written once.  Secondaries go straight onto the typed
-// stacks: the warp counts its records per type with ballots, one lane reserves the range with a single
-// atomicAdd per type ("atomic addition to unambiguously reserve one or more items"), and the
-// lanes write to consecutive records.  Energy deposition is accumulated per block in shared memory and
-// flushed with one atomic per touched tally.
-struct BlockAcc {
-    double sc[4];           // escaped, below_cut, looper, deposited
-    unsigned cnt[16];       // [0..7] interactions, [8] null, [9..11] tracks created by type, [12] steps
-};
+// A1-A8 + A10: one step of every live track.  One PERSISTENT launch per pool (e+, e-, gamma): the grid is a
+// fixed number of single-warp blocks (16 per SM: what 128 registers per thread allow) and each warp pulls
+// 32-slot chunks of the pool from a device-side work counter until none are left.  A warp never waits for
+// another warp: there is no block-wide barrier and no shared memory.  One pool per launch keeps the code of a
+// single particle type in the instruction caches (a merged kernel for the three types was instruction-fetch
+// bound: profiles/r1_v2_*); the three launches are parallel branches of the iteration graph.
+//   per lane: the track is read once, stepped in registers (step<PT>) and written once;
+//   secondaries go straight onto the typed stacks: the warp counts its records per type with ballots, one
+//   lane reserves the range with one atomic per type ("atomic addition to unambiguously reserve
+//   one or more items") and the lanes write consecutive records;
+//   tallies: lanes that deposit into the same tally are reduced with warp shuffles and one lane issues the
+//   fp64 atomic (north_star "warp-shuffle reductions for tallies"); run counters are kept in registers, one
+//   counter per lane, across all chunks of the warp and flushed once at the end of the launch.
+#ifndef EMX_WARPS_PER_SM
+#define EMX_WARPS_PER_SM 16
+#endif
+constexpr int kStepWarpsPerSM = EMX_WARPS_PER_SM;
 
 __device__ __forceinline__ void push_record(const QueueSoA &q, int r, const Vec3 &x, const Vec3 &u, double E,
                                             uint64_t tid, uint32_t prim, int vol) {
@@ -373,27 +381,60 @@ __device__ __forceinline__ void push_record(const QueueSoA &q, int r, const Vec3
     q.surf[r] = -1;
 }
 
-template <int PT>
-__global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params P, const __grid_constant__ Work w,
-                                                 uint64_t seed, double *tally) {
-    extern __shared__ double s_tally[];
-    __shared__ BlockAcc acc;
-    Ctl *c = w.ctl;
-    const int n_live = c->n_live[PT];
-    const int base = blockIdx.x * kChunk;
-    if (base >= n_live) return;
-    const int m = c->m_step[PT];
-    const int i = base + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    const bool use_smem = P.n_tally <= 2048;
-    if (use_smem)
-        for (int k = threadIdx.x; k < P.n_tally; k += kChunk) s_tally[k] = 0.0;
-    if (threadIdx.x < 4) acc.sc[threadIdx.x] = 0.0;
-    if (threadIdx.x < 16) acc.cnt[threadIdx.x] = 0u;
-    __syncthreads();
+__device__ __forceinline__ double warp_sum(double v) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
 
+// per-warp accumulators, spread over the lanes: lane k owns integer counter k (0..7 interactions by process,
+// 8 null interactions, 9..11 tracks created by type, 12..14 steps by type, 15 progress, 16 stalls) and lanes
+// 0..3 own the doubles escaped, below_cut, looper, deposited
+struct WarpAcc {
+    unsigned long long n;
+    double d;
+};
+
+// Reserve `cnt` records (warp total) on stack ty; returns the base index or -1 when the stack is full.
+// Far from the capacity one atomicAdd does it: kReserveSlack bounds what all resident warps of
+// the three step kernels can request at the same time (one outstanding reservation of <= 96 records each), so
+// the top cannot pass the capacity.  Near the capacity the reservation is a compare-and-swap that never
+// moves the top past the capacity.  Nothing is ever rolled back: an add-then-subtract scheme lets a
+// reservation succeed above a top that a concurrent failure has inflated, and strands its records.
+constexpr int kReserveSlack = 148 * 3 * 32 * 96;
+
+__device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, int lane) {
+    int r0 = -1;
+    if (lane == 0) {
+        const int cap = w.qcap[ty];
+        int old = *(volatile int *)&c->q_top[ty];
+        if ((long long)old + cnt + kReserveSlack <= (long long)cap) {
+            r0 = atomicAdd(&c->q_top[ty], cnt);
+        } else {
+            while (old + cnt <= cap) {
+                const int prev = atomicCAS(&c->q_top[ty], old, old + cnt);
+                if (prev == old) {
+                    r0 = old;
+                    break;
+                }
+                old = prev;
+            }
+        }
+    }
+    return __shfl_sync(0xffffffffu, r0, 0);
+}
+
+template <int PT>
+__device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
+                                               int n_live) {
+    WarpAcc acc;
+    acc.n = 0ull;
+    acc.d = 0.0;
+    Ctl *c = w.ctl;
+    const int lane = threadIdx.x;
+    const unsigned lt = (1u << lane) - 1u;
+    const int i = base + lane;
     const TrackSoA &ts = w.trk[PT];
-    const bool active = i < m;
+    const bool active = i < n_live;
     Track t;
     StepOut o;
     int vol0 = 0;
@@ -422,55 +463,45 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         t.alive = 1;
     }
 
-    // ---- A8: secondaries -> typed stacks.  Warp-aggregated reservation: one atomicAdd per type and warp.  A
-    // reservation that would pass the capacity is rolled back (no other warp can succeed while the top is
-    // above the capacity, so successful ranges stay contiguous) and the lanes that needed it STALL: nothing
-    // of their step is committed (R7).  Records a stalled lane did obtain for another type become tombstones
-    // (E < 0), which the next refill loads and this kernel retires without stepping.
+    // ---- A8: secondaries -> typed stacks.  When a stack cannot take the warp's records the lanes that needed
+    // it STALL: nothing of their step is committed (R7).  Records a stalled lane did obtain
+    // for another type become tombstones (E < 0), which the next refill loads and this kernel retires.
     const int ng = (o.s0.ptype == kGamma) + (o.s1.ptype == kGamma) + 2 * o.rest_alloc;
     const int ne = (o.s0.ptype == kElectron);  // only ordinal 0 is ever an electron
     const int np = (o.s1.ptype == kPositron);  // only the pair positron
     bool stall = false;
     int r_e = -1, r_p = -1, r_g = -1;
-    {
-        const unsigned lt = (1u << lane) - 1u;
-        unsigned b = __ballot_sync(0xffffffffu, ne);
-        if (b) {
-            int r0 = 0;
-            if (lane == 0) {
-                const int cnt = __popc(b);
-                r0 = atomicAdd(&c->q_top[kElectron], cnt);
-                if (r0 + cnt > w.qcap[kElectron]) { atomicSub(&c->q_top[kElectron], cnt); r0 = -1; }
-            }
-            r0 = __shfl_sync(0xffffffffu, r0, 0);
-            if (ne) { if (r0 < 0) stall = true; else r_e = r0 + __popc(b & lt); }
+    unsigned b = __ballot_sync(0xffffffffu, ne);
+    if (b) {
+        const int r0 = reserve(c, w, kElectron, __popc(b), lane);
+        if (ne) {
+            if (r0 < 0) stall = true;
+            else r_e = r0 + __popc(b & lt);
         }
+    }
+    if (PT == kGamma) {  // only photons make positrons
         b = __ballot_sync(0xffffffffu, np);
         if (b) {
-            int r0 = 0;
-            if (lane == 0) {
-                const int cnt = __popc(b);
-                r0 = atomicAdd(&c->q_top[kPositron], cnt);
-                if (r0 + cnt > w.qcap[kPositron]) { atomicSub(&c->q_top[kPositron], cnt); r0 = -1; }
+            const int r0 = reserve(c, w, kPositron, __popc(b), lane);
+            if (np) {
+                if (r0 < 0) stall = true;
+                else r_p = r0 + __popc(b & lt);
             }
-            r0 = __shfl_sync(0xffffffffu, r0, 0);
-            if (np) { if (r0 < 0) stall = true; else r_p = r0 + __popc(b & lt); }
         }
+    }
+    if (PT != kGamma) {  // only e+- make photons: 0..3 per lane -> inclusive warp scan of the counts
         b = __ballot_sync(0xffffffffu, ng > 0);
-        if (b) {  // photons: 0..3 per lane -> inclusive warp scan of the counts
+        if (b) {
             int inc = ng;
             for (int d = 1; d < 32; d <<= 1) {
                 const int v = __shfl_up_sync(0xffffffffu, inc, d);
                 if (lane >= d) inc += v;
             }
-            const int total = __shfl_sync(0xffffffffu, inc, 31);
-            int r0 = 0;
-            if (lane == 0) {
-                r0 = atomicAdd(&c->q_top[kGamma], total);
-                if (r0 + total > w.qcap[kGamma]) { atomicSub(&c->q_top[kGamma], total); r0 = -1; }
+            const int r0 = reserve(c, w, kGamma, __shfl_sync(0xffffffffu, inc, 31), lane);
+            if (ng) {
+                if (r0 < 0) stall = true;
+                else r_g = r0 + inc - ng;
             }
-            r0 = __shfl_sync(0xffffffffu, r0, 0);
-            if (ng) { if (r0 < 0) stall = true; else r_g = r0 + inc - ng; }
         }
     }
     if (stall) {
@@ -512,55 +543,104 @@ __global__ void __launch_bounds__(kChunk) k_step(const __grid_constant__ Params 
         ts.vol[i] = t.vol;
         ts.surf[i] = t.surf;
     }
-    const int alive_out = tomb ? 0 : (commit ? t.alive : 1);
-    if (i < n_live) ts.alive[i] = (uint8_t)alive_out;
+    if (active) ts.alive[i] = (uint8_t)(tomb ? 0 : (commit ? t.alive : 1));
 
-    // ---- A10: tallies and counters
-    if (commit) {
-        if (o.edep != 0.0) {
-            atomicAdd(&acc.sc[3], o.edep);
-            const int tl = P.vol[vol0].tally;
-            if (tl >= 0) {
-                if (use_smem) atomicAdd(&s_tally[tl], o.edep);
-                else atomicAdd(&tally[tl], o.edep);
-            }
-        }
-        if (o.escaped != 0.0) atomicAdd(&acc.sc[0], o.escaped);
-        if (o.below_cut != 0.0) atomicAdd(&acc.sc[1], o.below_cut);
-        if (o.looper != 0.0) atomicAdd(&acc.sc[2], o.looper);
-        if (o.process >= 0) atomicAdd(&acc.cnt[o.null_int ? 8 : o.process], 1u);
-        if (o.rest) atomicAdd(&acc.cnt[EMX_P_REST], 1u);
-        if (ng) atomicAdd(&acc.cnt[9], (unsigned)ng);
-        if (ne) atomicAdd(&acc.cnt[10], 1u);
-        if (np) atomicAdd(&acc.cnt[11], 1u);
-    }
-    const int n_dead = __syncthreads_count(i < n_live && !alive_out);
-    const int n_commit = __syncthreads_count(commit);
-    const int n_tomb = __syncthreads_count(tomb);
-    const int n_stall = __syncthreads_count(active && stall);
-    if (threadIdx.x == 0) {
-        w.chunk_dead[PT][blockIdx.x] = n_dead;
-        if (n_commit) atomicAdd(&c->steps[PT], (unsigned long long)n_commit);
-        if (n_commit + n_tomb) atomicAdd(&c->progress, (unsigned long long)(n_commit + n_tomb));
-        if (n_stall) atomicAdd(&c->stalls, (unsigned long long)n_stall);
-        if (acc.sc[0] != 0.0) atomicAdd(&c->escaped, acc.sc[0]);
-        if (acc.sc[1] != 0.0) atomicAdd(&c->below_cut, acc.sc[1]);
-        if (acc.sc[2] != 0.0) atomicAdd(&c->looper, acc.sc[2]);
-        if (acc.sc[3] != 0.0) atomicAdd(&c->edep_total, acc.sc[3]);
-    }
-    if (threadIdx.x < 12) {
-        const unsigned v = acc.cnt[threadIdx.x];
-        if (v) {
-            unsigned long long *dst = threadIdx.x < 8 ? &c->inter[threadIdx.x]
-                                     : (threadIdx.x == 8 ? &c->null_int : &c->tracks[threadIdx.x - 9]);
-            atomicAdd(dst, (unsigned long long)v);
+    // ---- A10: per-volume tally.  Lanes with the same tally id are summed with shuffles; one atomic per group.
+    {
+        const int tl = (commit && o.edep != 0.0) ? P.vol[vol0].tally : -1;
+        unsigned m = __ballot_sync(0xffffffffu, tl >= 0);
+        while (m) {
+            const int leader = __ffs(m) - 1;
+            const int key = __shfl_sync(0xffffffffu, tl, leader);
+            const bool mine = (tl == key);
+            const unsigned grp = __ballot_sync(0xffffffffu, mine);
+            const double s = warp_sum(mine ? o.edep : 0.0);
+            if (lane == leader) atomicAdd(&tally[key], s);
+            m &= ~grp;
         }
     }
-    if (use_smem)
-        for (int k = threadIdx.x; k < P.n_tally; k += kChunk) {
-            const double v = s_tally[k];
-            if (v != 0.0) atomicAdd(&tally[k], v);
+    // ---- run totals, accumulated in registers (lane k owns counter k)
+    {
+        const double e0 = commit ? o.escaped : 0.0, e1 = commit ? o.below_cut : 0.0, e2 = commit ? o.looper : 0.0,
+                     e3 = commit ? o.edep : 0.0;
+        if (__ballot_sync(0xffffffffu, e0 != 0.0 || e1 != 0.0 || e2 != 0.0 || e3 != 0.0)) {
+            const double s0 = warp_sum(e0), s1 = warp_sum(e1), s2 = warp_sum(e2), s3 = warp_sum(e3);
+            acc.d += (lane == 0) ? s0 : (lane == 1) ? s1 : (lane == 2) ? s2 : (lane == 3) ? s3 : 0.0;
         }
+        const int proc = (commit && o.process >= 0) ? (o.null_int ? 8 : o.process) : -1;
+        unsigned add = 0;
+        for (int k = 0; k < 9; ++k) {
+            const unsigned cnt = __popc(__ballot_sync(0xffffffffu, proc == k));
+            if (lane == k) add = cnt;
+        }
+        const unsigned n_rest = __popc(__ballot_sync(0xffffffffu, commit && o.rest));
+        if (lane == EMX_P_REST) add += n_rest;
+        const unsigned n_e = __popc(__ballot_sync(0xffffffffu, commit && ne));
+        const unsigned n_p = __popc(__ballot_sync(0xffffffffu, commit && np));
+        unsigned n_g = commit ? (unsigned)ng : 0u;
+        for (int o2 = 16; o2 > 0; o2 >>= 1) n_g += __shfl_xor_sync(0xffffffffu, n_g, o2);
+        const unsigned n_commit = __popc(__ballot_sync(0xffffffffu, commit));
+        const unsigned n_tomb = __popc(__ballot_sync(0xffffffffu, tomb));
+        const unsigned n_stall = __popc(__ballot_sync(0xffffffffu, active && stall));
+        if (lane == 9) add = n_g;
+        if (lane == 10) add = n_e;
+        if (lane == 11) add = n_p;
+        if (lane == 12 + PT) add = n_commit;
+        if (lane == 15) add = n_commit + n_tomb;
+        if (lane == 16) add = n_stall;
+        acc.n += add;
+    }
+    return acc;
+}
+
+// one pool per launch: the code of a single particle type stays resident in the instruction caches
+template <int PT>
+__global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_constant__ Params P,
+                                                                  const __grid_constant__ Work w, uint64_t seed,
+                                                                  double *tally) {
+    Ctl *c = w.ctl;
+    const int lane = threadIdx.x;
+    const int nl = c->m_step[PT];
+    const int total = (nl + 31) >> 5;
+    WarpAcc acc;
+    acc.n = 0ull;
+    acc.d = 0.0;
+    int k_next = 0;
+    if (lane == 0) k_next = atomicAdd(&c->work_ctr3[PT], 1);
+    for (;;) {
+        const int k = __shfl_sync(0xffffffffu, k_next, 0);
+        if (k >= total) break;
+        if (lane == 0) k_next = atomicAdd(&c->work_ctr3[PT], 1);
+        const WarpAcc d = step_chunk<PT>(P, w, seed, tally, k << 5, nl);
+        acc.n += d.n;
+        acc.d += d.d;
+    }
+    if (acc.n) {
+        unsigned long long *dst = lane < 8    ? &c->inter[lane]
+                                  : lane == 8 ? &c->null_int
+                                  : lane < 12 ? &c->tracks[lane - 9]
+                                  : lane < 15 ? &c->steps[lane - 12]
+                                  : lane == 15 ? &c->progress
+                                               : &c->stalls;
+        if (lane <= 16) atomicAdd(dst, acc.n);
+    }
+    if (acc.d != 0.0 && lane < 4) {
+        double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
+        atomicAdd(dst, acc.d);
+    }
+}
+
+// dead slots per 128-slot chunk of the live ranges, for the refill plan
+__global__ void __launch_bounds__(kChunk) k_count_dead_pools(Work w) {
+    const int p = blockIdx.y;
+    const Ctl *c = w.ctl;
+    if (c->done) return;
+    const int n_live = c->n_live[p];
+    const int base = blockIdx.x * kChunk;
+    if (base >= n_live) return;
+    const int i = base + threadIdx.x;
+    const int n = __syncthreads_count(i < n_live && w.trk[p].alive[i] == 0);
+    if (threadIdx.x == 0) w.chunk_dead[p][blockIdx.x] = n;
 }
 
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
@@ -568,18 +648,27 @@ cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
     int maxcap = w.cap[0];
     for (int p = 1; p < 3; ++p) maxcap = w.cap[p] > maxcap ? w.cap[p] : maxcap;
     const dim3 g3((maxcap + kChunk - 1) / kChunk, 3);
+    k_count_dead_pools<<<g3, kChunk, 0, st>>>(w);
     k_plan<<<1, 1024, 0, st>>>(w);
     k_fill<<<g3, kChunk, 0, st>>>(w, nullptr);
     k_move<<<g3, kChunk, 0, st>>>(w, nullptr);
     return cudaGetLastError();
 }
 
-cudaError_t launch_step(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st) {
-    const size_t sm = P.n_tally <= 2048 ? (size_t)P.n_tally * sizeof(double) : 0;
-    const unsigned g = (unsigned)((w.cap[pt] + kChunk - 1) / kChunk);
-    if (pt == kGamma) k_step<kGamma><<<g, kChunk, sm, st>>>(P, w, seed, tally);
-    else if (pt == kElectron) k_step<kElectron><<<g, kChunk, sm, st>>>(P, w, seed, tally);
-    else k_step<kPositron><<<g, kChunk, sm, st>>>(P, w, seed, tally);
+cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st) {
+    k_step_pool<kPositron><<<n_sm * kStepWarpsPerSM, 32, 0, st>>>(P, w, seed, tally);
+    k_step_pool<kElectron><<<n_sm * kStepWarpsPerSM, 32, 0, st>>>(P, w, seed, tally);
+    k_step_pool<kGamma><<<n_sm * kStepWarpsPerSM, 32, 0, st>>>(P, w, seed, tally);
+    return cudaGetLastError();
+}
+
+// the step kernel of one pool on its own stream (fork / join branches of the iteration graph)
+cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
+                             cudaStream_t st) {
+    const int g = n_sm * kStepWarpsPerSM;
+    if (pt == kGamma) k_step_pool<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
+    else if (pt == kElectron) k_step_pool<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
+    else k_step_pool<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
     return cudaGetLastError();
 }
 

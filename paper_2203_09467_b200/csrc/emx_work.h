@@ -45,6 +45,7 @@ struct Ctl {
     int m_step[3];  // tracks to step this iteration (= n_live)
     PoolPlan plan[3];
     int done, error, had_live;
+    int work_ctr3[3];  // next 32-slot chunk of each pool's step kernel
     unsigned long long iter;
     unsigned long long progress;  // steps committed + tombstones retired in the current iteration (R7)
     long long next_primary;       // primaries [0, next_primary) have been admitted

@@ -69,11 +69,11 @@ EMX_HD void screening(double d, double &phi1, double &phi2) {
         phi1 = 20.867 - 3.242 * d + 0.625 * d * d;
         phi2 = 20.209 - 1.930 * d - 0.086 * d * d;
     } else {
-        phi1 = phi2 = 21.12 - 4.184 * log(d + 0.952);
+        phi1 = phi2 = 21.12 - 4.184 * m_log(d + 0.952);
     }
 }
 EMX_HD double pair_F(int Z, double E) {
-    double F = (8.0 / 3.0) * log((double)Z);
+    double F = (8.0 / 3.0) * m_log((double)Z);
     if (E >= 50.0) F += 8.0 * coulomb_fc(Z);
     return F;
 }

@@ -12,7 +12,7 @@ import weakref
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libemx.so")
+LIB_PATH = os.environ.get("EMX_LIB_PATH") or os.path.join(HERE, "libemx.so")   # override: kernel experiments
 MAX_ELEM, MAX_FACES, NPROC, NTABLE = 4, 8, 8, 16
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
            "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3"]
@@ -50,7 +50,7 @@ EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "
            "emx_get_physics", "emx_set_physics", "emx_set_cuts", "emx_build_tables", "emx_get_table",
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
            "emx_reset_tallies", "emx_read_tallies", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile",
-           "emx_get_iteration_log",
+           "emx_get_iteration_log", "emx_get_iteration_times",
            "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_last_error",
            "emx_version"]
 
@@ -79,6 +79,7 @@ def lib():
             "emx_transport_host": (i, [vp, l, vp, vp, vp, vp, vp, vp, u64, l, l, vp, C.c_size_t, vp]),
             "emx_reset_tallies": (i, [vp, vp]), "emx_read_tallies": (i, [vp, vp, C.POINTER(Scalars)]),
             "emx_last_transport_ms": (d, [vp]), "emx_get_iteration_log": (l, [vp, vp, l]),
+            "emx_get_iteration_times": (l, [vp, vp, l]),
             "emx_set_profile": (i, [vp, i]), "emx_get_profile": (i, [vp, vp, vp, vp]),
             "emx_step_batch": (i, [vp, u64, l, vp, vp, vp]),
             "emx_philox_batch": (i, [l, vp, vp, vp, vp]),
@@ -253,7 +254,7 @@ class Problem:
                     ms=lib().emx_last_transport_ms(self.h))
 
     def set_profile(self, on):
-        self._check(lib().emx_set_profile(self.h, int(bool(on))))
+        self._check(lib().emx_set_profile(self.h, int(on)))
 
     def profile(self):
         """dict(ms=[step gamma, step e-, step e+, refill], launches, iterations_launched) of the last transport"""
@@ -262,6 +263,12 @@ class Problem:
         self._check(lib().emx_get_profile(self.h, C.cast(ms, C.c_void_p), C.cast(C.byref(nl), C.c_void_p),
                                           C.cast(C.byref(ni), C.c_void_p)))
         return dict(ms=list(ms), launches=nl.value, iterations_launched=ni.value)
+
+    def iteration_times(self, max_iter=1 << 16):
+        """(n, 2) float32: refill ms, step-kernel ms per iteration of the last transport (profiling on)"""
+        out = np.zeros((max_iter, 2), dtype=np.float32)
+        n = lib().emx_get_iteration_times(self.h, _hp(out), max_iter)
+        return out[:max(n, 0)]
 
     def iteration_log(self, max_iter=1 << 16):
         out = np.zeros((max_iter, 2), dtype=np.uint32)
