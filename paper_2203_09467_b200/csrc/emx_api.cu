@@ -2,6 +2,7 @@
 // Host logic only; every computation of the path runs in the kernels of emx_kernels.cu / emx_transport.cu.
 #include <cuda_runtime.h>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -45,6 +46,8 @@ struct emx_problem {
     cudaStream_t s0 = nullptr, s1 = nullptr, s2 = nullptr;
     cudaEvent_t evFork = nullptr, evJ1 = nullptr, evJ2 = nullptr, evIn = nullptr, evOut = nullptr;
     bool use_graph = true;
+    long slice_above = -1;  // < 0: n_slots / 32
+    int slice_budget = 2;
 };
 
 namespace {
@@ -123,6 +126,14 @@ size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
         t.prim = c.take<uint32_t>(n); t.step = c.take<uint32_t>(n);
         t.vol = c.take<int>(n); t.surf = c.take<int>(n);
         t.alive = c.take<uint8_t>(n);
+        if (p != 0) {
+            t.fs_s = c.take<double>(n);
+            t.fs_h = c.take<double>(n);
+            t.fs_a = c.take<int>(n);
+        } else {
+            t.fs_s = t.fs_h = nullptr;
+            t.fs_a = nullptr;
+        }
         QueueSoA &s = w.q[p];
         s.x = c.take<double>(q); s.y = c.take<double>(q); s.z = c.take<double>(q);
         s.ux = c.take<double>(q); s.uy = c.take<double>(q); s.uz = c.take<double>(q);
@@ -151,6 +162,9 @@ int emx_create(emx_problem **out) {
     if (!out) return fail(nullptr, EMX_E_ARG, "emx_create: null output");
     emx_problem *p = new (std::nothrow) emx_problem();
     if (!p) return fail(nullptr, EMX_E_NOMEM, "emx_create: out of memory");
+    // tuning knobs of the scheduler (they never change a result, only when work is done)
+    if (const char *e = getenv("EMX_SLICE_BUDGET")) p->slice_budget = atoi(e) > 0 ? atoi(e) : p->slice_budget;
+    if (const char *e = getenv("EMX_SLICE_ABOVE")) p->slice_above = atol(e);
     *out = p;
     return EMX_OK;
 }
@@ -395,6 +409,8 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     w.wave = (int)(n_slots / 256 < 256 ? 256 : (n_slots / 256 > 4096 ? 4096 : n_slots / 256));
     w.queue_soft = queue_capacity / 4;
     w.inflight_cap = 5.0 * (double)queue_capacity;
+    w.slice_above = p->slice_above >= 0 ? p->slice_above : n_slots / 32;
+    w.slice_budget = p->slice_budget;
     CU(cudaEventRecord(p->ev0, st));
     CU(launch_init(w, pr, st));
     p->launches = 1;

@@ -42,9 +42,13 @@ EMX_HD void step_one(const Params &P, uint64_t seed, const emx_track &in, emx_st
     t.surf = in.surf;
     t.alive = 1;
     StepOut o;
-    if (in.ptype == kGamma) step<kGamma>(P, seed, t, o);
-    else if (in.ptype == kElectron) step<kElectron>(P, seed, t, o);
-    else step<kPositron>(P, seed, t, o);
+    FieldState fs;
+    fs.s_done = fs.h = 0.0;
+    fs.attempt = 0;
+    const int whole = P.ph.max_substeps;  // the hook runs the whole step in one call
+    if (in.ptype == kGamma) step<kGamma>(P, seed, t, o, fs, whole);
+    else if (in.ptype == kElectron) step<kElectron>(P, seed, t, o, fs, whole);
+    else step<kPositron>(P, seed, t, o, fs, whole);
 
     put3(r.trk.x, t.x);
     put3(r.trk.u, t.u);

@@ -45,18 +45,48 @@ EMX_NI void rk4_doubling(const Vec3 &x, const Vec3 &u, double kappa, const doubl
     u1.z /= n;
 }
 
-// Propagate up to s_max inside cell `vol`.  Returns the arc length travelled; hit = surface reached
-// (-1 none).  x, u are updated; on_surf is the surface the track starts on.
-EMX_NI double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
-                              int &hit) {
+// Progress of a propagation that is spread over several iterations of the loop: the
+// arc length done, the current trial step and the substep attempts used.  attempt == 0: none in progress.
+struct FieldState {
+    double s_done, h;
+    int attempt;
+};
+
+// Propagate up to s_max inside cell `vol`.  Returns the arc length travelled so far; hit = surface reached
+// (-1 none).  x, u are updated; on_surf is the surface the track sits on (updated when suspended).
+// The substep loop of C9 runs for at most `budget` attempts per call; if it is not finished by then,
+// `suspended` is set and fs holds the loop variables, so that the next call continues the SAME sequence of
+// substeps: slicing changes when the work is done, never its result.  budget >= max_substeps: one call.
+EMX_NI double propagate_field(const Params &P, int vol, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
+                              int &hit, FieldState &fs, int budget, bool &suspended) {
     const double eps = P.ph.field_eps;
-    double s_done = 0.0;
+    double s_done;
     int surf = on_surf;
-    double h = 0.25 / fabs(kappa);
-    if (s_max < h) h = s_max;
+    double h;
+    int attempt;
+    if (fs.attempt > 0) {  // resume
+        s_done = fs.s_done;
+        h = fs.h;
+        attempt = fs.attempt;
+    } else {
+        s_done = 0.0;
+        h = 0.25 / fabs(kappa);
+        if (s_max < h) h = s_max;
+        attempt = 0;
+    }
     hit = -1;
+    suspended = false;
     const int max_attempts = P.ph.max_substeps;
-    for (int attempt = 0; attempt < max_attempts; ++attempt) {
+    const int stop_at = (budget < max_attempts - attempt) ? attempt + budget : max_attempts;
+    for (; attempt < max_attempts; ++attempt) {
+        if (attempt >= stop_at) {  // out of budget for this iteration: park the loop variables
+            fs.s_done = s_done;
+            fs.h = h;
+            fs.attempt = attempt;
+            on_surf = surf;
+            suspended = true;
+            return s_done;
+        }
         const double rem = s_max - s_done;
         if (h > rem) h = rem;
         Vec3 x1, u1;
@@ -83,6 +113,7 @@ EMX_NI double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Ve
                 continue;
             }
             hit = S;  // immediate (re-)crossing, nothing more travelled
+            fs.attempt = 0;
             return s_done;
         }
         if (d > L + eps) {  // chord ends inside the cell, clear of S: accept
@@ -100,10 +131,12 @@ EMX_NI double propagate_field(const Params &P, int vol, int on_surf, Vec3 &x, Ve
             x = x1;
             u = u1;
             hit = S;
+            fs.attempt = 0;
             return s_done + h;
         }
         h *= d / L;  // secant: aim the chord end at S
     }
+    fs.attempt = 0;
     return s_done;
 }
 

@@ -36,6 +36,7 @@ struct StepOut {
     Vec3 rest_u;
     double edep, below_cut, escaped, looper, s;
     int n_draws, null_int, rest;
+    int suspended;       // field propagation parked for the next iteration: nothing else of the step happened
 };
 
 // grid lookup (C4): bin j and fraction f of ln E, shared by every table of the step
@@ -116,8 +117,10 @@ EMX_HD void kill_below(const Params &P, Rng &rng, Track &t, StepOut &o, double E
 }
 
 // One step of a live track of type PT (C7).  `t` is updated in place; `o` receives everything else.
+// `fs` / `budget`: time slicing of the field propagation (emx_field.h); pass attempt = 0 and a budget
+// >= max_substeps to run the whole step in one call.
 template <int PT>
-EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o) {
+EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
     const emx_physics &ph = P.ph;
     o.action = EMX_A_NONE;
     o.process = -1;
@@ -126,6 +129,7 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o) {
     o.rest_alloc = 0;
     o.edep = o.below_cut = o.escaped = o.looper = o.s = 0.0;
     o.n_draws = o.null_int = o.rest = 0;
+    o.suspended = 0;
     Rng rng;
     rng.init(seed, t.prim, t.tid, t.step);
     const int vol = t.vol;
@@ -204,7 +208,12 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o) {
         const double pm = sqrt(E * (E + 2.0 * kMe));
         const double q = (PT == kElectron) ? -1.0 : 1.0;
         const double kappa = q * kCB * P.Bmag / pm;
-        s = propagate_field(P, vol, t.surf, t.x, t.u, kappa, s_phys, hit);
+        bool susp;
+        s = propagate_field(P, vol, t.surf, t.x, t.u, kappa, s_phys, hit, fs, budget, susp);
+        if (susp) {  // x, u, surf and fs hold the progress; the step continues in the next iteration
+            o.suspended = 1;
+            return;
+        }
         if (hit >= 0) {
             action = EMX_A_BOUNDARY;
             full = false;

@@ -23,6 +23,7 @@ __device__ __forceinline__ void load_record(const QueueSoA &q, int r, const Trac
     t.vol[i] = q.vol[r];
     t.surf[i] = q.surf[r];
     t.alive[i] = 2;  // 2 = filled in this refill pass (k_move still ranks it as a hole)
+    if (t.fs_a) t.fs_a[i] = 0;
 }
 
 __device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
@@ -39,6 +40,11 @@ __device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
     t.vol[to] = t.vol[from];
     t.surf[to] = t.surf[from];
     t.alive[to] = 2;
+    if (t.fs_a) {
+        t.fs_s[to] = t.fs_s[from];
+        t.fs_h[to] = t.fs_h[from];
+        t.fs_a[to] = t.fs_a[from];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -275,6 +281,10 @@ __global__ void __launch_bounds__(1024) k_plan(Work w) {
                 c->done = 1;
             }
             c->had_live = live > 0 ? 1 : 0;
+            // time slicing of the field propagation: with many tracks in flight a track may use only a few
+            // substep attempts per iteration (the rest of its step continues next iteration), so that no warp
+            // holds an iteration open for hundreds of substeps; with few tracks left latency matters more
+            c->field_budget = live > w.slice_above ? w.slice_budget : 0x7fffffff;
             c->progress = 0ull;
             c->work_ctr3[0] = c->work_ctr3[1] = c->work_ctr3[2] = 0;
         }
@@ -425,7 +435,7 @@ __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, i
 
 template <int PT>
 __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
-                                               int n_live) {
+                                               int n_live, int budget) {
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
@@ -453,15 +463,47 @@ __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, ui
         t.alive = 1;
         vol0 = t.vol;
         step0 = t.step;
-        step<PT>(P, seed, t, o);
+        FieldState fs;
+        fs.s_done = fs.h = 0.0;
+        fs.attempt = 0;
+        if (PT != kGamma) {
+            fs.attempt = ts.fs_a[i];
+            if (fs.attempt > 0) {
+                fs.s_done = ts.fs_s[i];
+                fs.h = ts.fs_h[i];
+            }
+        }
+        step<PT>(P, seed, t, o, fs, budget);
+        if (PT != kGamma && o.suspended) {
+            // the propagation continues in the next iteration: park position, direction, surface flag and the
+            // loop variables; nothing else of the step has happened yet
+            ts.x[i] = t.x.x;
+            ts.y[i] = t.x.y;
+            ts.z[i] = t.x.z;
+            ts.ux[i] = t.u.x;
+            ts.uy[i] = t.u.y;
+            ts.uz[i] = t.u.z;
+            ts.surf[i] = t.surf;
+            ts.fs_s[i] = fs.s_done;
+            ts.fs_h[i] = fs.h;
+            ts.fs_a[i] = fs.attempt;
+            o.s0.ptype = o.s1.ptype = -1;
+            o.rest_alloc = 0;
+            o.process = -1;
+            o.edep = o.below_cut = o.escaped = o.looper = 0.0;
+            o.null_int = o.rest = 0;
+            t.alive = 1;
+        }
     } else {
         o.s0.ptype = o.s1.ptype = -1;
         o.rest_alloc = 0;
         o.process = -1;
         o.edep = o.below_cut = o.escaped = o.looper = 0.0;
         o.null_int = o.rest = 0;
+        o.suspended = 0;
         t.alive = 1;
     }
+    const bool parked = active && !tomb && (PT != kGamma) && o.suspended;
 
     // ---- A8: secondaries -> typed stacks.  When a stack cannot take the warp's records the lanes that needed
     // it STALL: nothing of their step is committed (R7).  Records a stalled lane did obtain
@@ -528,7 +570,7 @@ __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, ui
             }
         }
     }
-    const bool commit = active && !tomb && !stall;
+    const bool commit = active && !tomb && !stall && !parked;
 
     // ---- write the track back (A5-A7 results); tid and prim never change
     if (commit) {
@@ -542,6 +584,7 @@ __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, ui
         ts.step[i] = t.step;
         ts.vol[i] = t.vol;
         ts.surf[i] = t.surf;
+        if (PT != kGamma) ts.fs_a[i] = 0;
     }
     if (active) ts.alive[i] = (uint8_t)(tomb ? 0 : (commit ? t.alive : 1));
 
@@ -580,7 +623,7 @@ __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, ui
         unsigned n_g = commit ? (unsigned)ng : 0u;
         for (int o2 = 16; o2 > 0; o2 >>= 1) n_g += __shfl_xor_sync(0xffffffffu, n_g, o2);
         const unsigned n_commit = __popc(__ballot_sync(0xffffffffu, commit));
-        const unsigned n_tomb = __popc(__ballot_sync(0xffffffffu, tomb));
+        const unsigned n_tomb = __popc(__ballot_sync(0xffffffffu, tomb || parked));
         const unsigned n_stall = __popc(__ballot_sync(0xffffffffu, active && stall));
         if (lane == 9) add = n_g;
         if (lane == 10) add = n_e;
@@ -602,6 +645,7 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_
     const int lane = threadIdx.x;
     const int nl = c->m_step[PT];
     const int total = (nl + 31) >> 5;
+    const int budget = c->field_budget;
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
@@ -611,7 +655,7 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_
         const int k = __shfl_sync(0xffffffffu, k_next, 0);
         if (k >= total) break;
         if (lane == 0) k_next = atomicAdd(&c->work_ctr3[PT], 1);
-        const WarpAcc d = step_chunk<PT>(P, w, seed, tally, k << 5, nl);
+        const WarpAcc d = step_chunk<PT>(P, w, seed, tally, k << 5, nl, budget);
         acc.n += d.n;
         acc.d += d.d;
     }

@@ -20,6 +20,10 @@ struct TrackSoA {
     uint32_t *prim, *step;
     int *vol, *surf;
     uint8_t *alive;
+    // field propagation in progress (charged pools only; null for gamma): arc length done, trial step,
+    // substep attempts used (0 = none in progress)
+    double *fs_s, *fs_h;
+    int *fs_a;
 };
 
 struct QueueSoA {  // secondary / primary initializer records (76 B per record)
@@ -46,6 +50,7 @@ struct Ctl {
     PoolPlan plan[3];
     int done, error, had_live;
     int work_ctr3[3];  // next 32-slot chunk of each pool's step kernel
+    int field_budget;  // substep attempts per track and iteration (time slicing of the field propagation)
     unsigned long long iter;
     unsigned long long progress;  // steps committed + tombstones retired in the current iteration (R7)
     long long next_primary;       // primaries [0, next_primary) have been admitted
@@ -72,10 +77,12 @@ struct Work {
     int wave;
     long long queue_soft;
     double inflight_cap;
+    long long slice_above;  // live tracks above which the field propagation is time-sliced
+    int slice_budget;       // substep attempts per track and iteration while sliced
 };
 
 // bytes of one slot / one record, for the workspace carve-up and the roofline arithmetic
-constexpr size_t kSlotBytes = 7 * 8 + 8 + 4 + 4 + 4 + 4 + 1;
+constexpr size_t kSlotBytes = 7 * 8 + 8 + 4 + 4 + 4 + 4 + 1;  // + 20 B in the charged pools (field progress)
 constexpr size_t kRecordBytes = 7 * 8 + 8 + 4 + 4 + 4;
 
 }  // namespace emx
