@@ -126,6 +126,7 @@ size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
         t.prim = c.take<uint32_t>(n); t.step = c.take<uint32_t>(n);
         t.vol = c.take<int>(n); t.surf = c.take<int>(n);
         t.alive = c.take<uint8_t>(n);
+        t.pend = c.take<uint8_t>(n);
         if (p != 0) {
             t.fs_s = c.take<double>(n);
             t.fs_h = c.take<double>(n);
@@ -144,6 +145,7 @@ size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
         w.chunk_dead[p] = c.take<int>(nch);
         w.chunk_off[p] = c.take<int>(nch);
         w.hole_idx[p] = c.take<int>(n);
+        for (int k = 0; k < 3; ++k) w.ilist[p][k] = c.take<int>(n);
     }
     return align_up(c.off, 256);
 }

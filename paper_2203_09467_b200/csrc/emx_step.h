@@ -117,10 +117,26 @@ EMX_HD void kill_below(const Params &P, Rng &rng, Track &t, StepOut &o, double E
 }
 
 // One step of a live track of type PT (C7).  `t` is updated in place; `o` receives everything else.
-// `fs` / `budget`: time slicing of the field propagation (emx_field.h); pass attempt = 0 and a budget
-// >= max_substeps to run the whole step in one call.
+// The step is written in two parts so that the loop can regroup tracks between them:
+//   step_pre      items 1-7 of C7 plus the SELECTION of the discrete process (draws 0 and 1); returns the
+//                 process id (EMX_P_*) if an interaction is pending, else -1 and the step is complete;
+//   step_interact item 8 (the interactor, draws 2...) and item 9 for a track whose interaction is pending.
+// step() = both, back to back (the level-2 hook).  `fs` / `budget`: time slicing of the field propagation
+// (emx_field.h); pass attempt = 0 and a budget >= max_substeps to run the whole propagation in one call.
 template <int PT>
-EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
+EMX_HD void finish_step(const Params &P, Track &t, StepOut &o) {
+    // 9. step counter, looper cap (R14)
+    if (t.alive) {
+        t.step += 1;
+        if ((int)t.step >= P.ph.max_steps) {
+            o.looper += t.E + (PT == kPositron ? 2.0 * kMe : 0.0);
+            t.alive = 0;
+        }
+    }
+}
+
+template <int PT>
+EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
     const emx_physics &ph = P.ph;
     o.action = EMX_A_NONE;
     o.process = -1;
@@ -139,7 +155,7 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
     if (t.E < ph.E_trk) {
         kill_below<PT>(P, rng, t, o, t.E);
         o.n_draws = (int)rng.n;
-        return;
+        return -1;
     }
 
     double Sig0 = 0.0, Sig1 = 0.0, Sig2 = 0.0, Stot = 0.0, D = 0.0, R = 0.0, s_phys;
@@ -212,7 +228,7 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
         s = propagate_field(P, vol, t.surf, t.x, t.u, kappa, s_phys, hit, fs, budget, susp);
         if (susp) {  // x, u, surf and fs hold the progress; the step continues in the next iteration
             o.suspended = 1;
-            return;
+            return -1;
         }
         if (hit >= 0) {
             action = EMX_A_BOUNDARY;
@@ -243,7 +259,7 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
             o.action = action;
             kill_below<PT>(P, rng, t, o, t.E);
             o.n_draws = (int)rng.n;
-            return;
+            return -1;
         }
     }
     o.action = action;
@@ -256,7 +272,7 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
             o.escaped += t.E + (PT == kPositron ? 2.0 * kMe : 0.0);
             t.alive = 0;
             o.n_draws = (int)rng.n;
-            return;
+            return -1;
         }
         t.vol = nv;
     } else {
@@ -266,9 +282,6 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
     // 8. discrete interaction: select with the pre-step cross sections, interact at the post-loss energy (R21)
     if (action == EMX_A_DISCRETE) {
         const double target = rng.next() * Stot;
-        const Material &m = P.mat[mat];
-        const double E1 = t.E;
-        const Vec3 u0 = t.u;
         int k;
         if (PT == kElectron) {
             k = (Sig0 > target) ? 0 : 1;
@@ -279,17 +292,42 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
             if (k == 2 && Sig2 <= 0.0) k = 1;
             if (k == 1 && Sig1 <= 0.0) k = 0;
         }
+        // k-th process of this particle type -> process id
+        int proc;
+        if (PT == kGamma) proc = (k == 0) ? EMX_P_COMPTON : (k == 1 ? EMX_P_PHOTO : EMX_P_PAIR);
+        else if (PT == kElectron) proc = (k == 0) ? EMX_P_MOLLER : EMX_P_BREMS;
+        else proc = (k == 0) ? EMX_P_BHABHA : (k == 1 ? EMX_P_BREMS : EMX_P_ANNIH);
+        o.n_draws = (int)rng.n;
+        return proc;  // interaction pending: the step is finished by step_interact
+    }
+    finish_step<PT>(P, t, o);
+    o.n_draws = (int)rng.n;
+    return -1;
+}
+
+// Item 8 of C7 for a track whose interaction `proc` was selected by step_pre: the interactor runs at the
+// post-loss energy t.E with draws 2, 3, ... of the step, then item 9.
+template <int PT>
+EMX_HD void step_interact(const Params &P, uint64_t seed, Track &t, StepOut &o, int proc) {
+    const emx_physics &ph = P.ph;
+    Rng rng;
+    rng.init(seed, t.prim, t.tid, t.step);
+    rng.n = 2u;  // draws 0 (interaction length) and 1 (process selection) were used by step_pre
+    const int mat = P.vol[t.vol].material;
+    const Material &m = P.mat[mat];
+    const double E1 = t.E;
+    const Vec3 u0 = t.u;
+    o.process = proc;
+    {
         if (PT == kGamma) {
-            if (k == 0) {
-                o.process = EMX_P_COMPTON;
+            if (proc == EMX_P_COMPTON) {
                 double Eg, Te;
                 Vec3 ug, ue;
                 compton(rng, E1, u0, Eg, ug, Te, ue);
                 add_secondary(P, o, o.s0, kElectron, Te, ue, 0);
                 t.E = Eg;
                 t.u = ug;
-            } else if (k == 1) {
-                o.process = EMX_P_PHOTO;
+            } else if (proc == EMX_P_PHOTO) {
                 if (ph.deposit_e_at_creation) {
                     o.edep += E1;
                 } else {
@@ -299,7 +337,6 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
                 t.E = 0.0;
                 t.alive = 0;
             } else {
-                o.process = EMX_P_PAIR;
                 int ie = 0;
                 if (m.n_elem > 1) {  // element selection (R4)
                     const double xe = rng.next();
@@ -331,9 +368,8 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
                 }
             }
         } else {
-            const bool ioni = (k == 0), brem = (k == 1);
+            const bool ioni = (proc == EMX_P_MOLLER || proc == EMX_P_BHABHA), brem = (proc == EMX_P_BREMS);
             if (ioni) {
-                o.process = (PT == kElectron) ? EMX_P_MOLLER : EMX_P_BHABHA;
                 double Td, T1;
                 Vec3 ud, u1;
                 const bool ok = (PT == kElectron) ? moller(rng, E1, m.Tcut, u0, Td, ud, T1, u1)
@@ -346,7 +382,6 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
                     o.null_int = 1;
                 }
             } else if (brem) {
-                o.process = EMX_P_BREMS;
                 double k1, T1;
                 Vec3 ug, u1;
                 if (bremsstrahlung(rng, E1, m.kcut, u0, k1, ug, T1, u1)) {
@@ -357,7 +392,6 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
                     o.null_int = 1;
                 }
             } else {
-                o.process = EMX_P_ANNIH;
                 double k1, k2;
                 Vec3 u1, u2;
                 annih_flight(rng, E1, u0, k1, u1, k2, u2);
@@ -369,16 +403,15 @@ EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldStat
         }
         if (t.alive && t.E < ph.E_trk) kill_below<PT>(P, rng, t, o, t.E);
     }
-
-    // 9. step counter, looper cap (R14)
-    if (t.alive) {
-        t.step += 1;
-        if ((int)t.step >= ph.max_steps) {
-            o.looper += t.E + (PT == kPositron ? 2.0 * kMe : 0.0);
-            t.alive = 0;
-        }
-    }
+    finish_step<PT>(P, t, o);
     o.n_draws = (int)rng.n;
+}
+
+// the whole step in one call
+template <int PT>
+EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
+    const int proc = step_pre<PT>(P, seed, t, o, fs, budget);
+    if (proc >= 0) step_interact<PT>(P, seed, t, o, proc);
 }
 
 }  // namespace emx

@@ -1,7 +1,8 @@
 // emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the fused
 // per-type step kernel (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
 //
-// One ITERATION = k_admit -> k_count_dead_pools -> k_plan -> k_fill -> k_move -> k_step_pool<e+|e-|gamma>.  Nothing returns to the host
+// One ITERATION = k_admit -> k_count_dead_pools -> k_plan -> k_fill -> k_move -> per pool (e+, e-, gamma):
+// k_step_pool<PT> (phase A) -> k_interact<PT> (phase B).  Nothing returns to the host
 // between iterations: pool sizes, stack tops and the done flag live in the device control block.
 #include <cuda_runtime.h>
 #include "emx_kernels.h"
@@ -24,6 +25,7 @@ __device__ __forceinline__ void load_record(const QueueSoA &q, int r, const Trac
     t.surf[i] = q.surf[r];
     t.alive[i] = 2;  // 2 = filled in this refill pass (k_move still ranks it as a hole)
     if (t.fs_a) t.fs_a[i] = 0;
+    if (t.pend) t.pend[i] = 0;
 }
 
 __device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
@@ -40,6 +42,7 @@ __device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
     t.vol[to] = t.vol[from];
     t.surf[to] = t.surf[from];
     t.alive[to] = 2;
+    if (t.pend) t.pend[to] = t.pend[from];
     if (t.fs_a) {
         t.fs_s[to] = t.fs_s[from];
         t.fs_h[to] = t.fs_h[from];
@@ -287,6 +290,9 @@ __global__ void __launch_bounds__(1024) k_plan(Work w) {
             c->field_budget = live > w.slice_above ? w.slice_budget : 0x7fffffff;
             c->progress = 0ull;
             c->work_ctr3[0] = c->work_ctr3[1] = c->work_ctr3[2] = 0;
+            c->work_ctrB[0] = c->work_ctrB[1] = c->work_ctrB[2] = 0;
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b) c->icount[a][b] = 0;
         }
     }
 }
@@ -433,78 +439,34 @@ __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, i
     return __shfl_sync(0xffffffffu, r0, 0);
 }
 
+// index of process `proc` among the processes of particle type PT (the order of C7.8), and back
 template <int PT>
-__device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
-                                               int n_live, int budget) {
+__device__ __forceinline__ int proc_slot(int proc) {
+    if (PT == kGamma) return proc == EMX_P_COMPTON ? 0 : (proc == EMX_P_PHOTO ? 1 : 2);
+    if (PT == kElectron) return proc == EMX_P_MOLLER ? 0 : 1;
+    return proc == EMX_P_BHABHA ? 0 : (proc == EMX_P_BREMS ? 1 : 2);
+}
+template <int PT>
+__device__ __forceinline__ int slot_proc(int k) {
+    if (PT == kGamma) return k == 0 ? EMX_P_COMPTON : (k == 1 ? EMX_P_PHOTO : EMX_P_PAIR);
+    if (PT == kElectron) return k == 0 ? EMX_P_MOLLER : EMX_P_BREMS;
+    return k == 0 ? EMX_P_BHABHA : (k == 1 ? EMX_P_BREMS : EMX_P_ANNIH);
+}
+
+// What both step kernels do with a lane's result: reserve and write the secondaries (A8), write the track
+// back, tally (A10), count.  `pend` >= 0: the lane's step is not finished -- its interaction `pend` was
+// selected and waits for k_interact; only what has happened so far (move, continuous loss) is committed.
+template <int PT>
+__device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint64_t seed, double *tally, int i,
+                                            bool active, bool tomb, bool parked, int pend, Track &t, StepOut &o,
+                                            int vol0, uint32_t step0) {
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
     Ctl *c = w.ctl;
     const int lane = threadIdx.x;
     const unsigned lt = (1u << lane) - 1u;
-    const int i = base + lane;
     const TrackSoA &ts = w.trk[PT];
-    const bool active = i < n_live;
-    Track t;
-    StepOut o;
-    int vol0 = 0;
-    uint32_t step0 = 0;
-    const double E0 = active ? ts.E[i] : 0.0;
-    const bool tomb = active && E0 < 0.0;  // tombstone record: retire the slot without stepping
-    if (active && !tomb) {
-        t.x = {ts.x[i], ts.y[i], ts.z[i]};
-        t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
-        t.E = E0;
-        t.tid = ts.tid[i];
-        t.prim = ts.prim[i];
-        t.step = ts.step[i];
-        t.vol = ts.vol[i];
-        t.surf = ts.surf[i];
-        t.alive = 1;
-        vol0 = t.vol;
-        step0 = t.step;
-        FieldState fs;
-        fs.s_done = fs.h = 0.0;
-        fs.attempt = 0;
-        if (PT != kGamma) {
-            fs.attempt = ts.fs_a[i];
-            if (fs.attempt > 0) {
-                fs.s_done = ts.fs_s[i];
-                fs.h = ts.fs_h[i];
-            }
-        }
-        step<PT>(P, seed, t, o, fs, budget);
-        if (PT != kGamma && o.suspended) {
-            // the propagation continues in the next iteration: park position, direction, surface flag and the
-            // loop variables; nothing else of the step has happened yet
-            ts.x[i] = t.x.x;
-            ts.y[i] = t.x.y;
-            ts.z[i] = t.x.z;
-            ts.ux[i] = t.u.x;
-            ts.uy[i] = t.u.y;
-            ts.uz[i] = t.u.z;
-            ts.surf[i] = t.surf;
-            ts.fs_s[i] = fs.s_done;
-            ts.fs_h[i] = fs.h;
-            ts.fs_a[i] = fs.attempt;
-            o.s0.ptype = o.s1.ptype = -1;
-            o.rest_alloc = 0;
-            o.process = -1;
-            o.edep = o.below_cut = o.escaped = o.looper = 0.0;
-            o.null_int = o.rest = 0;
-            t.alive = 1;
-        }
-    } else {
-        o.s0.ptype = o.s1.ptype = -1;
-        o.rest_alloc = 0;
-        o.process = -1;
-        o.edep = o.below_cut = o.escaped = o.looper = 0.0;
-        o.null_int = o.rest = 0;
-        o.suspended = 0;
-        t.alive = 1;
-    }
-    const bool parked = active && !tomb && (PT != kGamma) && o.suspended;
-
     // ---- A8: secondaries -> typed stacks.  When a stack cannot take the warp's records the lanes that needed
     // it STALL: nothing of their step is committed (R7).  Records a stalled lane did obtain
     // for another type become tombstones (E < 0), which the next refill loads and this kernel retires.
@@ -585,6 +547,7 @@ __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, ui
         ts.vol[i] = t.vol;
         ts.surf[i] = t.surf;
         if (PT != kGamma) ts.fs_a[i] = 0;
+        ts.pend[i] = (uint8_t)(pend >= 0 ? 1 + pend : 0);
     }
     if (active) ts.alive[i] = (uint8_t)(tomb ? 0 : (commit ? t.alive : 1));
 
@@ -623,12 +586,13 @@ __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, ui
         unsigned n_g = commit ? (unsigned)ng : 0u;
         for (int o2 = 16; o2 > 0; o2 >>= 1) n_g += __shfl_xor_sync(0xffffffffu, n_g, o2);
         const unsigned n_commit = __popc(__ballot_sync(0xffffffffu, commit));
+        const unsigned n_done = __popc(__ballot_sync(0xffffffffu, commit && pend < 0));  // completed steps
         const unsigned n_tomb = __popc(__ballot_sync(0xffffffffu, tomb || parked));
         const unsigned n_stall = __popc(__ballot_sync(0xffffffffu, active && stall));
         if (lane == 9) add = n_g;
         if (lane == 10) add = n_e;
         if (lane == 11) add = n_p;
-        if (lane == 12 + PT) add = n_commit;
+        if (lane == 12 + PT) add = n_done;
         if (lane == 15) add = n_commit + n_tomb;
         if (lane == 16) add = n_stall;
         acc.n += add;
@@ -637,6 +601,144 @@ __device__ __forceinline__ WarpAcc step_chunk(const Params &P, const Work &w, ui
 }
 
 // one pool per launch: the code of a single particle type stays resident in the instruction caches
+
+// Phase A of a chunk: items 1-7 of C7 and the selection of the discrete process for 32 consecutive slots.
+// Lanes whose step ends here (boundary, loss-limited, truncated, killed) are committed; lanes with an
+// interaction pending are committed as far as they got and filed in the list of their process, so that
+// k_interact runs every interactor on full warps (B:north_star "partitioned by next action").
+template <int PT>
+__device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
+                                             int n_live, int budget) {
+    Ctl *c = w.ctl;
+    const int lane = threadIdx.x;
+    const unsigned lt = (1u << lane) - 1u;
+    const int i = base + lane;
+    const TrackSoA &ts = w.trk[PT];
+    const bool active = i < n_live;
+    Track t;
+    StepOut o;
+    int vol0 = 0;
+    uint32_t step0 = 0;
+    const double E0 = active ? ts.E[i] : 0.0;
+    const bool tomb = active && E0 < 0.0;  // tombstone record: retire the slot without stepping
+    const int pend_in = (active && !tomb) ? (int)ts.pend[i] - 1 : -1;  // interaction still waiting (stalled)
+    int pend = -1;
+    if (active && !tomb && pend_in < 0) {
+        t.x = {ts.x[i], ts.y[i], ts.z[i]};
+        t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
+        t.E = E0;
+        t.tid = ts.tid[i];
+        t.prim = ts.prim[i];
+        t.step = ts.step[i];
+        t.vol = ts.vol[i];
+        t.surf = ts.surf[i];
+        t.alive = 1;
+        vol0 = t.vol;
+        step0 = t.step;
+        FieldState fs;
+        fs.s_done = fs.h = 0.0;
+        fs.attempt = 0;
+        if (PT != kGamma) {
+            fs.attempt = ts.fs_a[i];
+            if (fs.attempt > 0) {
+                fs.s_done = ts.fs_s[i];
+                fs.h = ts.fs_h[i];
+            }
+        }
+        pend = step_pre<PT>(P, seed, t, o, fs, budget);
+#if defined(EMX_ONE_PHASE)
+        if (pend >= 0) {
+            step_interact<PT>(P, seed, t, o, pend);
+            pend = -1;
+        }
+#endif
+        if (PT != kGamma && o.suspended) {
+            // the propagation continues in the next iteration: park position, direction, surface flag and the
+            // loop variables; nothing else of the step has happened yet
+            ts.x[i] = t.x.x;
+            ts.y[i] = t.x.y;
+            ts.z[i] = t.x.z;
+            ts.ux[i] = t.u.x;
+            ts.uy[i] = t.u.y;
+            ts.uz[i] = t.u.z;
+            ts.surf[i] = t.surf;
+            ts.fs_s[i] = fs.s_done;
+            ts.fs_h[i] = fs.h;
+            ts.fs_a[i] = fs.attempt;
+            o.s0.ptype = o.s1.ptype = -1;
+            o.rest_alloc = 0;
+            o.process = -1;
+            o.edep = o.below_cut = o.escaped = o.looper = 0.0;
+            o.null_int = o.rest = 0;
+            t.alive = 1;
+        }
+    } else {
+        o.s0.ptype = o.s1.ptype = -1;
+        o.rest_alloc = 0;
+        o.process = -1;
+        o.edep = o.below_cut = o.escaped = o.looper = 0.0;
+        o.null_int = o.rest = 0;
+        o.suspended = 0;
+        t.alive = 1;
+    }
+    const bool parked = active && !tomb && (PT != kGamma) && o.suspended;
+    const bool waiting = pend_in >= 0;  // nothing to do in this phase
+
+    WarpAcc acc = epilogue<PT>(P, w, seed, tally, i, active && !waiting, tomb, parked, pend, t, o, vol0, step0);
+    // file the lanes with a pending interaction (new or stalled) in the list of their process
+    {
+        const int pk = waiting ? proc_slot<PT>(pend_in) : (pend >= 0 && !parked ? proc_slot<PT>(pend) : -1);
+        constexpr int nk = (PT == kElectron) ? 2 : 3;
+#pragma unroll
+        for (int k = 0; k < nk; ++k) {
+            const unsigned b = __ballot_sync(0xffffffffu, pk == k);
+            if (b) {
+                int r0 = 0;
+                if (lane == 0) r0 = atomicAdd(&c->icount[PT][k], __popc(b));
+                r0 = __shfl_sync(0xffffffffu, r0, 0);
+                if (pk == k) w.ilist[PT][k][r0 + __popc(b & lt)] = i;
+            }
+        }
+    }
+    return acc;
+}
+
+// Phase B of a chunk: 32 tracks of pool PT waiting for the same interactor (list k of the pool).
+template <int PT>
+__device__ __forceinline__ WarpAcc interact_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int k,
+                                                  int first, int n_list) {
+    const int lane = threadIdx.x;
+    const int idx = first + lane;
+    const TrackSoA &ts = w.trk[PT];
+    const bool active = idx < n_list;
+    const int i = active ? w.ilist[PT][k][idx] : 0;
+    Track t;
+    StepOut o;
+    o.action = EMX_A_DISCRETE;
+    o.process = -1;
+    o.s0.ptype = o.s1.ptype = -1;
+    o.rest_alloc = 0;
+    o.edep = o.below_cut = o.escaped = o.looper = o.s = 0.0;
+    o.n_draws = o.null_int = o.rest = o.suspended = 0;
+    int vol0 = 0;
+    uint32_t step0 = 0;
+    t.alive = 1;
+    if (active) {
+        t.x = {ts.x[i], ts.y[i], ts.z[i]};
+        t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
+        t.E = ts.E[i];
+        t.tid = ts.tid[i];
+        t.prim = ts.prim[i];
+        t.step = ts.step[i];
+        t.vol = ts.vol[i];
+        t.surf = -1;
+        vol0 = t.vol;
+        step0 = t.step;
+        step_interact<PT>(P, seed, t, o, slot_proc<PT>(k));
+    }
+    return epilogue<PT>(P, w, seed, tally, i, active, false, false, -1, t, o, vol0, step0);
+}
+
 template <int PT>
 __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_constant__ Params P,
                                                                   const __grid_constant__ Work w, uint64_t seed,
@@ -655,7 +757,60 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_
         const int k = __shfl_sync(0xffffffffu, k_next, 0);
         if (k >= total) break;
         if (lane == 0) k_next = atomicAdd(&c->work_ctr3[PT], 1);
-        const WarpAcc d = step_chunk<PT>(P, w, seed, tally, k << 5, nl, budget);
+        const WarpAcc d = pre_chunk<PT>(P, w, seed, tally, k << 5, nl, budget);
+        acc.n += d.n;
+        acc.d += d.d;
+    }
+    if (acc.n) {
+        unsigned long long *dst = lane < 8    ? &c->inter[lane]
+                                  : lane == 8 ? &c->null_int
+                                  : lane < 12 ? &c->tracks[lane - 9]
+                                  : lane < 15 ? &c->steps[lane - 12]
+                                  : lane == 15 ? &c->progress
+                                               : &c->stalls;
+        if (lane <= 16) atomicAdd(dst, acc.n);
+    }
+    if (acc.d != 0.0 && lane < 4) {
+        double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
+        atomicAdd(dst, acc.d);
+    }
+}
+
+// Phase B: the interactors.  Persistent single-warp blocks pull 32-entry chunks of the pool's process lists;
+// a warp runs ONE interactor on (up to) 32 tracks that all selected it.
+template <int PT>
+__global__ void __launch_bounds__(32, kStepWarpsPerSM) k_interact(const __grid_constant__ Params P,
+                                                                 const __grid_constant__ Work w, uint64_t seed,
+                                                                 double *tally) {
+    Ctl *c = w.ctl;
+    const int lane = threadIdx.x;
+    constexpr int nk = (PT == kElectron) ? 2 : 3;
+    // order in which the lists are worked off.  The stacks are LIFO, so what is pushed LAST is refilled
+    // first: photons run pair production first (its leptons are the most energetic secondaries and go to the
+    // bottom of this iteration's records) and photoelectric absorption last.  Keeping low-energy tracks on top
+    // is what keeps the queue short ("preferentially selecting lower-energy particles").
+    const int ord0 = (PT == kGamma) ? 2 : 0, ord1 = (PT == kGamma) ? 0 : 1, ord2 = (PT == kGamma) ? 1 : 2;
+    int n[3], cb[4];
+    cb[0] = 0;
+    n[0] = c->icount[PT][ord0];
+    n[1] = c->icount[PT][ord1];
+    n[2] = ord2 < nk ? c->icount[PT][ord2] : 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) cb[k + 1] = cb[k] + ((n[k] + 31) >> 5);
+    const int total = cb[3];
+    WarpAcc acc;
+    acc.n = 0ull;
+    acc.d = 0.0;
+    int k_next = 0;
+    if (lane == 0 && total > 0) k_next = atomicAdd(&c->work_ctrB[PT], 1);
+    for (;;) {
+        const int ch = __shfl_sync(0xffffffffu, k_next, 0);
+        if (ch >= total) break;
+        if (lane == 0) k_next = atomicAdd(&c->work_ctrB[PT], 1);
+        WarpAcc d;
+        if (ch < cb[1]) d = interact_chunk<PT>(P, w, seed, tally, ord0, ch << 5, n[0]);
+        else if (ch < cb[2]) d = interact_chunk<PT>(P, w, seed, tally, ord1, (ch - cb[1]) << 5, n[1]);
+        else d = interact_chunk<PT>(P, w, seed, tally, ord2, (ch - cb[2]) << 5, n[2]);
         acc.n += d.n;
         acc.d += d.d;
     }
@@ -699,10 +854,13 @@ cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
     return cudaGetLastError();
 }
 
+cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
+                             cudaStream_t st);
 cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st) {
-    k_step_pool<kPositron><<<n_sm * kStepWarpsPerSM, 32, 0, st>>>(P, w, seed, tally);
-    k_step_pool<kElectron><<<n_sm * kStepWarpsPerSM, 32, 0, st>>>(P, w, seed, tally);
-    k_step_pool<kGamma><<<n_sm * kStepWarpsPerSM, 32, 0, st>>>(P, w, seed, tally);
+    for (int pt = 2; pt >= 0; --pt) {
+        const cudaError_t e = launch_step_pool(pt, P, w, seed, tally, n_sm, st);
+        if (e != cudaSuccess) return e;
+    }
     return cudaGetLastError();
 }
 
@@ -710,9 +868,16 @@ cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *t
 cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                              cudaStream_t st) {
     const int g = n_sm * kStepWarpsPerSM;
-    if (pt == kGamma) k_step_pool<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
-    else if (pt == kElectron) k_step_pool<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
-    else k_step_pool<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+    if (pt == kGamma) {
+        k_step_pool<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
+        k_interact<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
+    } else if (pt == kElectron) {
+        k_step_pool<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        k_interact<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
+    } else {
+        k_step_pool<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        k_interact<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+    }
     return cudaGetLastError();
 }
 

@@ -20,6 +20,7 @@ struct TrackSoA {
     uint32_t *prim, *step;
     int *vol, *surf;
     uint8_t *alive;
+    uint8_t *pend;  // 0, or 1 + process id of the interaction selected by phase A and not yet run
     // field propagation in progress (charged pools only; null for gamma): arc length done, trial step,
     // substep attempts used (0 = none in progress)
     double *fs_s, *fs_h;
@@ -49,7 +50,9 @@ struct Ctl {
     int m_step[3];  // tracks to step this iteration (= n_live)
     PoolPlan plan[3];
     int done, error, had_live;
-    int work_ctr3[3];  // next 32-slot chunk of each pool's step kernel
+    int work_ctr3[3];  // next 32-slot chunk of each pool's step kernel (phase A)
+    int work_ctrB[3];  // next 32-entry chunk of each pool's interaction lists (phase B)
+    int icount[3][3];  // entries in the interaction lists [pool][process slot]
     int field_budget;  // substep attempts per track and iteration (time slicing of the field propagation)
     unsigned long long iter;
     unsigned long long progress;  // steps committed + tombstones retired in the current iteration (R7)
@@ -68,6 +71,7 @@ struct Work {
     int *chunk_dead[3];
     int *chunk_off[3];
     int *hole_idx[3];
+    int *ilist[3][3];  // slots waiting for an interactor, [pool][process slot], capacity cap[pool] each
     Ctl *ctl;
     uint32_t *log;  // per iteration: live, queued
     int max_log;
