@@ -25,13 +25,13 @@ struct Primaries {
 
 // resets the control block, totals the injected energy
 cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st);
-// one iteration of the loop = launch_refill (k_admit, k_count_dead_pools, k_plan, k_fill, k_move) then
+// one iteration of the loop = launch_refill (k_plan, k_fill, k_move) then
 // launch_step (one persistent kernel per pool); tally = device edep array
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st);
 cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st);
 cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                              cudaStream_t st);
-constexpr int kLaunchesPerIteration = 11;  // 5 refill kernels + 3 x (phase A + phase B)
+constexpr int kLaunchesPerIteration = 9;  // 3 refill kernels + 3 x (phase A + phase B)
 // level-1 hook: the refill index logic alone on a caller-supplied alive[] (see include/emx.h)
 cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
                                int *scratch, cudaStream_t st);

@@ -1,7 +1,7 @@
 // emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the fused
 // per-type step kernel (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
 //
-// One ITERATION = k_admit -> k_count_dead_pools -> k_plan -> k_fill -> k_move -> per pool (e+, e-, gamma):
+// One ITERATION = k_plan (admission + refill plan) -> k_fill -> k_move -> per pool (e+, e-, gamma):
 // k_step_pool<PT> (phase A) -> k_interact<PT> (phase B).  Nothing returns to the host
 // between iterations: pool sizes, stack tops and the done flag live in the device control block.
 #include <cuda_runtime.h>
@@ -86,14 +86,16 @@ __global__ void __launch_bounds__(1024) k_init(Work w, Primaries pr) {
         z.E_in = e;
         *c = z;
     }
+    for (int p = 0; p < 3; ++p)
+        for (int k = tid; k <= w.cap[p] / kChunk; k += blockDim.x) w.chunk_dead[p][k] = 0;
 }
 
-// A0, first half: admission of primaries (R8).  One block, run at the start of every iteration.  While the
+// A0, first half: admission of primaries (R8).  Done by the one block of k_plan at the start of every iteration.  While the
 // shower energy in flight and the stacks are below their soft limits, the next `wave` primaries are pushed
 // onto the stacks of their types, lowest index on top, so they enter the pools in ascending order at the
 // refill that follows.  Histories do not depend on when a primary is admitted (keyed RNG, C2); admission only
 // bounds the number of queued records (the queue had to hold 2.5e7 initializers).
-__global__ void __launch_bounds__(1024) k_admit(Work w, Primaries pr) {
+__device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) {
     __shared__ int s_cnt[3][32];
     __shared__ int s_total[3], s_base[3];
     __shared__ double s_E[32];
@@ -196,12 +198,14 @@ cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st) {
 //   h - a  holes left when the stack is dry: the live range shrinks to n_new and the live tracks above
 //          n_new move into the remaining holes below it (j-th live track from the end -> j-th such hole),
 //   extra  records appended above the old range when the stack holds more than the holes.
-__global__ void __launch_bounds__(1024) k_plan(Work w) {
+__global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
     __shared__ int s_warp[32];
     __shared__ int s_carry;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     Ctl *c = w.ctl;
     if (c->done) return;
+    admit_block(w, pr);
+    __syncthreads();
     for (int p = 0; p < 3; ++p) {
         const int n_old = c->n_live[p];
         const int nch = (n_old + kChunk - 1) / kChunk;
@@ -227,7 +231,10 @@ __global__ void __launch_bounds__(1024) k_plan(Work w) {
             }
             __syncthreads();
             const int off = s_carry + s_warp[wid] + inc - v;
-            if (k < nch) w.chunk_off[p][k] = off;
+            if (k < nch) {
+                w.chunk_off[p][k] = off;
+                w.chunk_dead[p][k] = 0;  // the step kernels count the next iteration's deaths into it
+            }
             __syncthreads();
             if (tid == blockDim.x - 1) s_carry = off + v;
             __syncthreads();
@@ -456,7 +463,7 @@ __device__ __forceinline__ int slot_proc(int k) {
 // What both step kernels do with a lane's result: reserve and write the secondaries (A8), write the track
 // back, tally (A10), count.  `pend` >= 0: the lane's step is not finished -- its interaction `pend` was
 // selected and waits for k_interact; only what has happened so far (move, continuous loss) is committed.
-template <int PT>
+template <int PT, bool CONSEC>
 __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint64_t seed, double *tally, int i,
                                             bool active, bool tomb, bool parked, int pend, Track &t, StepOut &o,
                                             int vol0, uint32_t step0) {
@@ -549,7 +556,15 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
         if (PT != kGamma) ts.fs_a[i] = 0;
         ts.pend[i] = (uint8_t)(pend >= 0 ? 1 + pend : 0);
     }
-    if (active) ts.alive[i] = (uint8_t)(tomb ? 0 : (commit ? t.alive : 1));
+    const bool died = active && (tomb || (commit && !t.alive));
+    if (active) ts.alive[i] = (uint8_t)(died ? 0 : 1);
+    // dead slots per 128-slot chunk, for the refill plan (A9)
+    if (CONSEC) {  // the warp's lanes are 32 consecutive slots of one chunk
+        const unsigned bd = __ballot_sync(0xffffffffu, died);
+        if (bd && lane == 0) atomicAdd(&w.chunk_dead[PT][i / kChunk], __popc(bd));
+    } else if (died) {
+        atomicAdd(&w.chunk_dead[PT][i / kChunk], 1);
+    }
 
     // ---- A10: per-volume tally.  Lanes with the same tally id are summed with shuffles; one atomic per group.
     {
@@ -684,7 +699,7 @@ __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uin
     const bool parked = active && !tomb && (PT != kGamma) && o.suspended;
     const bool waiting = pend_in >= 0;  // nothing to do in this phase
 
-    WarpAcc acc = epilogue<PT>(P, w, seed, tally, i, active && !waiting, tomb, parked, pend, t, o, vol0, step0);
+    WarpAcc acc = epilogue<PT, true>(P, w, seed, tally, i, active && !waiting, tomb, parked, pend, t, o, vol0, step0);
     // file the lanes with a pending interaction (new or stalled) in the list of their process
     {
         const int pk = waiting ? proc_slot<PT>(pend_in) : (pend >= 0 && !parked ? proc_slot<PT>(pend) : -1);
@@ -736,7 +751,7 @@ __device__ __forceinline__ WarpAcc interact_chunk(const Params &P, const Work &w
         step0 = t.step;
         step_interact<PT>(P, seed, t, o, slot_proc<PT>(k));
     }
-    return epilogue<PT>(P, w, seed, tally, i, active, false, false, -1, t, o, vol0, step0);
+    return epilogue<PT, false>(P, w, seed, tally, i, active, false, false, -1, t, o, vol0, step0);
 }
 
 template <int PT>
@@ -829,26 +844,11 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_interact(const __grid_c
     }
 }
 
-// dead slots per 128-slot chunk of the live ranges, for the refill plan
-__global__ void __launch_bounds__(kChunk) k_count_dead_pools(Work w) {
-    const int p = blockIdx.y;
-    const Ctl *c = w.ctl;
-    if (c->done) return;
-    const int n_live = c->n_live[p];
-    const int base = blockIdx.x * kChunk;
-    if (base >= n_live) return;
-    const int i = base + threadIdx.x;
-    const int n = __syncthreads_count(i < n_live && w.trk[p].alive[i] == 0);
-    if (threadIdx.x == 0) w.chunk_dead[p][blockIdx.x] = n;
-}
-
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
-    k_admit<<<1, 1024, 0, st>>>(w, pr);
     int maxcap = w.cap[0];
     for (int p = 1; p < 3; ++p) maxcap = w.cap[p] > maxcap ? w.cap[p] : maxcap;
     const dim3 g3((maxcap + kChunk - 1) / kChunk, 3);
-    k_count_dead_pools<<<g3, kChunk, 0, st>>>(w);
-    k_plan<<<1, 1024, 0, st>>>(w);
+    k_plan<<<1, 1024, 0, st>>>(w, pr);
     k_fill<<<g3, kChunk, 0, st>>>(w, nullptr);
     k_move<<<g3, kChunk, 0, st>>>(w, nullptr);
     return cudaGetLastError();
@@ -925,7 +925,8 @@ cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const u
     k_hook_init<<<1, 32, 0, st>>>(w, (int)n_live, (int)n_queue);
     const unsigned g = (unsigned)((n_live + kChunk - 1) / kChunk);
     if (g) k_count_dead<<<g, kChunk, 0, st>>>(w, (int)n_live);
-    k_plan<<<1, 1024, 0, st>>>(w);
+    Primaries none = Primaries();
+    k_plan<<<1, 1024, 0, st>>>(w, none);
     const dim3 g3((unsigned)((capacity + kChunk - 1) / kChunk), 1);
     k_fill<<<g3, kChunk, 0, st>>>(w, src);
     k_move<<<g3, kChunk, 0, st>>>(w, src);

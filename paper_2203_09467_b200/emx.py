@@ -209,7 +209,7 @@ class Problem:
         """dict of numpy arrays -> dict of CUDA tensors (ptype i32, E, pos (n,3), dir (n,3), vol, surf)."""
         torch = _torch()
         dt = dict(ptype=np.int32, E=np.float64, pos=np.float64, dir=np.float64, vol=np.int32, surf=np.int32)
-        return {k: torch.from_numpy(_np(prim[k], dt[k])).cuda() for k in dt}
+        return {k: torch.from_numpy(np.array(prim[k], dtype=dt[k], order="C")).cuda() for k in dt}
 
     def transport(self, prim_dev, seed, n_slots=None, queue_capacity=None, reset=True):
         """emx_transport on device-resident primaries.  Returns the tallies dict."""
