@@ -316,6 +316,8 @@ __device__ __forceinline__ int rank_in_chunk(bool dead, int *s_w) {
     return r;
 }
 
+constexpr int kRefillBlocks = 1184;  // per pool: 8 x 148 blocks, grid-stride over the chunks
+
 // A0: fill holes from the stack, list the holes that are left, append records above the old range
 __global__ void __launch_bounds__(kChunk) k_fill(Work w, int32_t *dbg_src) {
     __shared__ int s_w[kChunk / 32];
@@ -324,24 +326,31 @@ __global__ void __launch_bounds__(kChunk) k_fill(Work w, int32_t *dbg_src) {
     if (c->done) return;
     const PoolPlan pl = c->plan[p];
     const int top = pl.n_old > pl.n_final ? pl.n_old : pl.n_final;
-    const int base = blockIdx.x * kChunk;
-    if (base >= top) return;
-    const int i = base + threadIdx.x;
+    const int nch_old = (pl.n_old + kChunk - 1) / kChunk;
     const TrackSoA &t = w.trk[p];
-    const bool dead = (i < pl.n_old) && (t.alive[i] == 0);
-    const int k = w.chunk_off[p][blockIdx.x < (pl.n_old + kChunk - 1) / kChunk ? blockIdx.x : 0] + rank_in_chunk(dead, s_w);
-    if (dead) {
-        if (k < pl.a) {
-            const int r = pl.q_old - 1 - k;
+    for (int ch = blockIdx.x; ch * kChunk < top; ch += gridDim.x) {  // grid-stride over 128-slot chunks
+        const int base = ch * kChunk;
+        if (ch < nch_old && base + kChunk <= pl.n_old) {  // chunk inside the old range: skip it if nothing died
+            const int d0 = w.chunk_off[p][ch];
+            const int d1 = (ch + 1 < nch_old) ? w.chunk_off[p][ch + 1] : pl.h;
+            if (d1 == d0) continue;
+        }
+        const int i = base + threadIdx.x;
+        const bool dead = (i < pl.n_old) && (t.alive[i] == 0);
+        const int k = w.chunk_off[p][ch < nch_old ? ch : 0] + rank_in_chunk(dead, s_w);
+        if (dead) {
+            if (k < pl.a) {
+                const int r = pl.q_old - 1 - k;
+                if (dbg_src) { dbg_src[i] = r; t.alive[i] = 2; }
+                else load_record(w.q[p], r, t, i);
+            } else {
+                w.hole_idx[p][k - pl.a] = i;
+            }
+        } else if (i >= pl.n_old && i < pl.n_old + pl.extra) {
+            const int r = pl.q_old - 1 - pl.a - (i - pl.n_old);
             if (dbg_src) { dbg_src[i] = r; t.alive[i] = 2; }
             else load_record(w.q[p], r, t, i);
-        } else {
-            w.hole_idx[p][k - pl.a] = i;
         }
-    } else if (i >= pl.n_old && i < pl.n_old + pl.extra) {
-        const int r = pl.q_old - 1 - pl.a - (i - pl.n_old);
-        if (dbg_src) { dbg_src[i] = r; t.alive[i] = 2; }
-        else load_record(w.q[p], r, t, i);
     }
 }
 
@@ -353,20 +362,21 @@ __global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
     if (c->done) return;
     const PoolPlan pl = c->plan[p];
     if (pl.h == pl.a) return;  // nothing to compact
-    const int base = blockIdx.x * kChunk;
-    if (base >= pl.n_old || base + kChunk <= pl.n_new) return;
-    const int i = base + threadIdx.x;
     const TrackSoA &t = w.trk[p];
-    const bool in = i < pl.n_old;
-    const uint8_t al = in ? t.alive[i] : (uint8_t)1;
-    const bool dead = al != 1;  // holes of this pass, whether k_fill has refilled them (2) or not (0)
-    const int dead_before = w.chunk_off[p][blockIdx.x] + rank_in_chunk(dead, s_w);
-    if (in && !dead && i >= pl.n_new) {
-        const int dead_after = pl.h - dead_before;             // dead slots in (i, n_old)
-        const int j = (pl.n_old - 1 - i) - dead_after;         // live tracks in (i, n_old)
-        const int dest = w.hole_idx[p][j];
-        if (dbg_src) { dbg_src[dest] = -2 - i; t.alive[dest] = 2; }
-        else move_slot(t, i, dest);
+    // grid-stride over the chunks that overlap the tail [n_new, n_old)
+    for (int ch = pl.n_new / kChunk + blockIdx.x; ch * kChunk < pl.n_old; ch += gridDim.x) {
+        const int i = ch * kChunk + threadIdx.x;
+        const bool in = i < pl.n_old;
+        const uint8_t al = in ? t.alive[i] : (uint8_t)1;
+        const bool dead = al != 1;  // holes of this pass, whether k_fill has refilled them (2) or not (0)
+        const int dead_before = w.chunk_off[p][ch] + rank_in_chunk(dead, s_w);
+        if (in && !dead && i >= pl.n_new) {
+            const int dead_after = pl.h - dead_before;      // dead slots in (i, n_old)
+            const int j = (pl.n_old - 1 - i) - dead_after;  // live tracks in (i, n_old)
+            const int dest = w.hole_idx[p][j];
+            if (dbg_src) { dbg_src[dest] = -2 - i; t.alive[dest] = 2; }
+            else move_slot(t, i, dest);
+        }
     }
 }
 
@@ -845,9 +855,7 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_interact(const __grid_c
 }
 
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
-    int maxcap = w.cap[0];
-    for (int p = 1; p < 3; ++p) maxcap = w.cap[p] > maxcap ? w.cap[p] : maxcap;
-    const dim3 g3((maxcap + kChunk - 1) / kChunk, 3);
+    const dim3 g3(kRefillBlocks, 3);
     k_plan<<<1, 1024, 0, st>>>(w, pr);
     k_fill<<<g3, kChunk, 0, st>>>(w, nullptr);
     k_move<<<g3, kChunk, 0, st>>>(w, nullptr);
@@ -927,7 +935,7 @@ cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const u
     if (g) k_count_dead<<<g, kChunk, 0, st>>>(w, (int)n_live);
     Primaries none = Primaries();
     k_plan<<<1, 1024, 0, st>>>(w, none);
-    const dim3 g3((unsigned)((capacity + kChunk - 1) / kChunk), 1);
+    const dim3 g3(kRefillBlocks, 1);
     k_fill<<<g3, kChunk, 0, st>>>(w, src);
     k_move<<<g3, kChunk, 0, st>>>(w, src);
     return cudaGetLastError();
