@@ -48,6 +48,7 @@ struct emx_problem {
     bool use_graph = true;
     long slice_above = -1;  // < 0: n_slots / 32
     int slice_budget = 2;
+    int warps_per_sm[3] = {16, 16, 16};
 };
 
 namespace {
@@ -167,6 +168,7 @@ int emx_create(emx_problem **out) {
     // tuning knobs of the scheduler (they never change a result, only when work is done)
     if (const char *e = getenv("EMX_SLICE_BUDGET")) p->slice_budget = atoi(e) > 0 ? atoi(e) : p->slice_budget;
     if (const char *e = getenv("EMX_SLICE_ABOVE")) p->slice_above = atol(e);
+    if (const char *e = getenv("EMX_WARPS_PER_SM")) sscanf(e, "%d,%d,%d", &p->warps_per_sm[0], &p->warps_per_sm[1], &p->warps_per_sm[2]);
     *out = p;
     return EMX_OK;
 }
@@ -413,6 +415,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     w.inflight_cap = 5.0 * (double)queue_capacity;
     w.slice_above = p->slice_above >= 0 ? p->slice_above : n_slots / 32;
     w.slice_budget = p->slice_budget;
+    for (int k = 0; k < 3; ++k) w.warps_per_sm[k] = p->warps_per_sm[k];
     CU(cudaEventRecord(p->ev0, st));
     CU(launch_init(w, pr, st));
     p->launches = 1;

@@ -875,7 +875,9 @@ cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *t
 // the step kernel of one pool on its own stream (fork / join branches of the iteration graph)
 cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                              cudaStream_t st) {
-    const int g = n_sm * kStepWarpsPerSM;
+    // persistent single-warp blocks per SM for this pool: the three pools' kernels run side by side, so each
+    // gets a share of the 16 warps per SM that fit
+    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM);
     if (pt == kGamma) {
         k_step_pool<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
         k_interact<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);

@@ -81,6 +81,7 @@ struct Work {
     int wave;
     long long queue_soft;
     double inflight_cap;
+    int warps_per_sm[3];    // persistent step-kernel warps per SM, per pool
     long long slice_above;  // live tracks above which the field propagation is time-sliced
     int slice_budget;       // substep attempts per track and iteration while sliced
 };

@@ -210,3 +210,45 @@ def test_error_paths(emx):
     assert b"volume" in L.emx_last_error(h)
     assert L.emx_transport(h, 0, None, None, None, None, None, None, 0, 10, 10, None, 0, None) == -2
     L.emx_destroy(h)
+
+
+def test_scheduling_knobs_do_not_change_results(emx, monkeypatch):
+    """Time slicing of the field propagation (substep budget per iteration) and the graph / stream launch
+    paths only change WHEN work is done: counters are equal, tallies equal up to summation order."""
+    desc, prim = W.get(4, 64)
+    runs = []
+    for budget, mode in (("2", 0), ("100000", 0), ("7", 2), ("2", 1)):
+        monkeypatch.setenv("EMX_SLICE_BUDGET", budget)
+        monkeypatch.setenv("EMX_SLICE_ABOVE", "0")
+        G = emx.Problem(desc)
+        G.set_profile(mode)
+        runs.append(G.transport(G.upload_primaries(prim), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 20))
+    a = runs[0]
+    for b in runs[1:]:
+        for k in ("steps", "tracks", "inter"):
+            assert np.array_equal(a[k], b[k]), k
+        assert a["null_int"] == b["null_int"]
+        assert np.allclose(a["edep"], b["edep"], rtol=1e-11, atol=1e-9)
+        assert b["escaped"] == pytest.approx(a["escaped"], rel=1e-11)
+    assert runs[0]["iterations"] != runs[1]["iterations"]       # the schedules did differ
+
+
+def test_full_size_bench_configuration(emx, emo):
+    """BASELINE config 4 in full (100 000 primaries, 2^20 slots, 2^26 records: what bench.py times), against
+    the oracle on all host cores.  With keyed random numbers the histories are the same, so the integer
+    counters agree to a few parts per million (a comparison within rounding of equality may flip in
+    3.6e9 steps) and every tally within 1e-6; energy closes to 1e-9."""
+    desc, prim = W.get(4)
+    G = emx.Problem(desc)
+    g = G.transport(G.upload_primaries(prim), desc["seed"])
+    assert g["stalls"] == 0
+    assert g["edep"].sum() + g["escaped"] + g["looper"] == pytest.approx(g["E_in"], rel=1e-9)
+    assert g["track_steps"] == int(g["steps"].sum())
+    o = emo.Problem(desc).transport(prim, desc["seed"])
+    assert o["edep"].sum() + o["escaped"] + o["looper"] == pytest.approx(o["E_in"], rel=1e-9)
+    for k in ("steps", "tracks", "inter"):
+        a, b = o[k].astype(np.float64), g[k].astype(np.float64)
+        assert np.all(np.abs(a - b) <= 1e-5 * np.maximum(a, 1.0) + 5.0), (k, o[k], g[k])
+    big = o["edep"] > 1e-6 * o["E_in"]
+    assert np.all(np.abs(g["edep"][big] - o["edep"][big]) <= 1e-6 * o["edep"][big])
+    assert g["escaped"] == pytest.approx(o["escaped"], rel=1e-6)
