@@ -30,9 +30,10 @@ METRIC, UNIT = "track_steps_per_sec", "track-steps/s"
 # (x, u, E, tid, prim, step, vol, surf = 80 B) and written once (x, u, E, step, vol, surf, alive = 69 B);
 # per secondary one 76-byte record is written.
 B_STEP, B_SEC = 80 + 69, 76
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_step_all launch from the committed ncu capture
-# (profiles/); None until a capture of the current kernel exists
-TRAFFIC_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the committed `ncu --set full` capture
+# of a saturated iteration (profiles/r1_final_step_kernels_full.md)
+TRAFFIC_PER_LAUNCH = {"k_step_pool<gamma>": 23.3e6, "k_step_pool<e->": 37.9e6, "k_step_pool<e+>": 7.3e6,
+                      "k_interact<gamma>": 32.2e6, "k_interact<e->": 29.3e6, "k_interact<e+>": 9.4e6}
 
 
 def parse():
@@ -157,7 +158,7 @@ def run_ours(args):
     seed = desc["seed"] + 1000 * rank          # replicas: same problem, independent histories
     G = emx.Problem(desc)
     pdev = G.upload_primaries(prim)
-    pinned = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in prim.items()}
+    pinned = {k: torch.from_numpy(np.array(v, order="C")).pin_memory() for k, v in prim.items()}
     phost = {k: v.numpy() for k, v in pinned.items()}
     h2d = sum(v.numel() * v.element_size() for v in pinned.values())
     d2h = 8 * G.n_tally + 200
@@ -196,7 +197,8 @@ def run_ours(args):
     # bracketed by CUDA events on the launching stream; the graph path cannot be bracketed per kernel)
     G.set_profile(True)
     rp = G.transport(pdev, seed)
-    tot["kms"] = np.array(G.profile()["ms"]) * args.steps
+    prof = G.profile()
+    tot["kms"] = np.array(prof["ms"])
     prof_ms = rp["ms"]
     G.set_profile(False)
 
@@ -226,10 +228,20 @@ def run_ours(args):
         return
 
     value = all_steps / (ms * 1e-3)
-    # roofline of the dominant kernel: the fused step kernel k_step_pool<PT> (three persistent launches per
-    # iteration, timed together with CUDA events in a profiled pass of the same step)
-    alg_bytes = tot["per_type"].sum() * B_STEP + tot["sec_type"].sum() * B_SEC
-    k_s = tot["kms"][0] * 1e-3
+    # roofline of the dominant kernel.  The profiled pass brackets each of the six step kernels of every
+    # iteration with CUDA events; the dominant one is the kernel with the largest total.  Its algorithmic
+    # bytes = the track slots it processed (counted by the kernel) x bytes per slot.
+    names = ["k_step_pool<gamma>", "k_step_pool<e->", "k_step_pool<e+>", "k_interact<gamma>", "k_interact<e->",
+             "k_interact<e+>"]
+    kms = tot["kms"]                      # ms of the profiled pass per kernel
+    dom = int(np.argmax(kms[:6]))
+    lanes = float(prof["lanes"][dom])
+    n_sec = float(tot["sec_type"].sum()) / args.steps
+    if dom < 3:
+        alg_bytes = lanes * B_STEP        # phase A: slot read (80 B) + written back (69 B)
+    else:
+        alg_bytes = lanes * (B_STEP + 4) + n_sec * B_SEC * (lanes / max(sum(prof["lanes"][3:6]), 1.0))
+    k_s = kms[dom] * 1e-3
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -237,14 +249,17 @@ def run_ours(args):
         pass
     peak = float(peaks.get("hbm_gbs", 6650.0))
     ach = alg_bytes / k_s / 1e9 if k_s > 0 else 0.0
-    n_launch = max(tot["iters"], 1)
-    roof = {"bound": "hbm", "kernel": "k_step_pool<e+|e-|gamma>", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-            "traffic": TRAFFIC_PER_LAUNCH, "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s",
-            "algorithmic_bytes_per_launch": alg_bytes / n_launch, "avg_launch_ms": tot["kms"][0] / n_launch,
-            "kernel_ms_per_step": {"k_step_pool": tot["kms"][0] / args.steps, "refill": tot["kms"][1] / args.steps},
-            "step_kernel_share_of_step": float(tot["kms"][0] / args.steps / prof_ms),
-            "profiled_pass_ms": prof_ms,
-            "note": "not HBM-bound on B200: the 85 MB track store stays in the 126 MB L2; see DESIGN.md section 7"}
+    n_launch = max(rp["iterations"], 1)
+    roof = {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "traffic": TRAFFIC_PER_LAUNCH.get(names[dom]),
+            "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s",
+            "algorithmic_bytes_per_launch": alg_bytes / n_launch, "avg_launch_ms": kms[dom] / n_launch,
+            "kernel_ms_profiled_pass": dict(zip(names + ["refill", "all_step_kernels"], [float(v) for v in kms])),
+            "kernel_share_of_profiled_pass": float(kms[dom] / prof_ms), "profiled_pass_ms": prof_ms,
+            "all_step_kernels": {"achieved_GBs": float((sum(prof["lanes"][:3]) * B_STEP + sum(prof["lanes"][3:6]) * (B_STEP + 4)
+                                                        + n_sec * B_SEC) / (kms[7] * 1e-3) / 1e9)},
+            "note": "not HBM-bound on B200: the 95 MB track store stays in the 126 MB L2 (traffic < algorithmic "
+                    "bytes); the step kernels are latency / divergence bound, see DESIGN.md section 7"}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",

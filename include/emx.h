@@ -229,15 +229,17 @@ int emx_read_tallies(const emx_problem *p, double *edep_host, emx_scalars *out);
 double emx_last_transport_ms(const emx_problem *p);
 
 /* Per-kernel timing of the loop.  Normally emx_transport runs the loop as a CUDA graph (8 iterations per
- * graph, the three step kernels as parallel branches) on internal streams ordered after `stream`.  With
- * profiling on (on = 1) it launches kernel by kernel on `stream` instead and brackets every launch group of every
- * iteration with CUDA events on the caller's stream and sums the elapsed times.  emx_get_profile: ms4[4] =
- * milliseconds of the last transport spent in { the step kernel, the refill kernels (admit + count + plan +
- * fill + move), 0, 0 }; *launches = kernels launched by the last transport (always counted);
+ * graph, the pools' step kernels as parallel branches) on internal streams ordered after `stream`.  With
+ * profiling on (on = 1) it launches kernel by kernel on `stream` instead and brackets every launch with
+ * CUDA events on that stream.  emx_get_profile: ms8[8] = milliseconds of the last transport spent in
+ * { phase A (k_step_pool) gamma, e-, e+, phase B (k_interact) gamma, e-, e+, refill (k_plan + k_fill +
+ * k_move), all step kernels }; *launches = kernels launched by the last transport (always counted);
  * *iterations_launched = iterations enqueued (>= iterations needed: the host checks the done flag once per
- * batch).  Any output pointer may be NULL. */
+ * batch).  emx_get_lanes: lanes6[6] = track slots processed by { phase A gamma, e-, e+, phase B gamma, e-, e+ }
+ * over the last transport (the units of each kernel's algorithmic bytes).  Output pointers may be NULL. */
 int emx_set_profile(emx_problem *p, int on);
-int emx_get_profile(const emx_problem *p, double *ms4, long *launches, long *iterations_launched);
+int emx_get_profile(const emx_problem *p, double *ms8, long *launches, long *iterations_launched);
+int emx_get_lanes(const emx_problem *p, uint64_t *lanes6);
 
 /* Per-iteration diagnostics of the last transport (Fig. 5): up to `max_iter` rows of
  * { live tracks, queued initializers } as uint32 pairs in HOST memory; returns rows written. */

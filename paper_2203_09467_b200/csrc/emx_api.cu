@@ -38,7 +38,7 @@ struct emx_problem {
     // optional per-kernel timing of the loop (emx_set_profile)
     bool profile = false;
     std::vector<cudaEvent_t> prof_ev;
-    double prof_ms[4] = {0, 0, 0, 0};  // k_step_all, refill (admit + count + plan + fill + move), unused, unused
+    double prof_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // phase A gamma, e-, e+; phase B gamma, e-, e+; refill; all step kernels
     int n_sm = 148;
     long launches = 0, iterations_launched = 0;
     std::vector<float> iter_ms;  // per iteration: refill ms, step ms (profiling on)
@@ -471,7 +471,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     for (;;) {
         size_t ne = 0;
         if (p->profile) {
-            while (p->prof_ev.size() < (size_t)batch * 3) {
+            while (p->prof_ev.size() < (size_t)batch * 8) {
                 cudaEvent_t e;
                 CU(cudaEventCreate(&e));
                 p->prof_ev.push_back(e);
@@ -480,9 +480,16 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         for (int k = 0; k < batch; ++k) {
             if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
             CU(launch_refill(w, pr, st));
-            if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
-            CU(launch_step(p->P, w, seed, p->d_tally, p->n_sm, st));
-            if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
+            if (p->profile) {
+                for (int pt = 2; pt >= 0; --pt)
+                    for (int ph = 0; ph < 2; ++ph) {
+                        CU(cudaEventRecord(p->prof_ev[ne++], st));
+                        CU(launch_phase(pt, ph, p->P, w, seed, p->d_tally, p->n_sm, st));
+                    }
+                CU(cudaEventRecord(p->prof_ev[ne++], st));
+            } else {
+                CU(launch_step(p->P, w, seed, p->d_tally, p->n_sm, st));
+            }
         }
         p->launches += (long)batch * kLaunchesPerIteration;
         p->iterations_launched += batch;
@@ -491,9 +498,15 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         if (p->profile)
             for (int k = 0; k < batch; ++k) {
                 float ms;
-                const cudaEvent_t *e = &p->prof_ev[(size_t)k * 3];
-                CU(cudaEventElapsedTime(&ms, e[0], e[1])); p->prof_ms[1] += ms; p->iter_ms.push_back(ms);
-                CU(cudaEventElapsedTime(&ms, e[1], e[2])); p->prof_ms[0] += ms; p->iter_ms.push_back(ms);
+                const cudaEvent_t *e = &p->prof_ev[(size_t)k * 8];
+                CU(cudaEventElapsedTime(&ms, e[0], e[1])); p->prof_ms[6] += ms; p->iter_ms.push_back(ms);
+                int q = 1;
+                for (int pt = 2; pt >= 0; --pt)
+                    for (int ph = 0; ph < 2; ++ph, ++q) {
+                        CU(cudaEventElapsedTime(&ms, e[q], e[q + 1]));
+                        p->prof_ms[3 * ph + pt] += ms;
+                    }
+                CU(cudaEventElapsedTime(&ms, e[1], e[7])); p->prof_ms[7] += ms; p->iter_ms.push_back(ms);
             }
         if (p->h_ctl->done || p->h_ctl->error) break;
         if (batch < 64) batch *= 2;
@@ -587,9 +600,9 @@ int emx_set_profile(emx_problem *p, int on) {
     return EMX_OK;
 }
 
-int emx_get_profile(const emx_problem *p, double *ms4, long *launches, long *iterations_launched) {
+int emx_get_profile(const emx_problem *p, double *ms4, long *launches, long *iterations_launched) {  // ms4: 8 doubles
     if (!p) return EMX_E_ARG;
-    if (ms4) for (int k = 0; k < 4; ++k) ms4[k] = p->prof_ms[k];
+    if (ms4) for (int k = 0; k < 8; ++k) ms4[k] = p->prof_ms[k];
     if (launches) *launches = p->launches;
     if (iterations_launched) *iterations_launched = p->iterations_launched;
     return EMX_OK;
@@ -601,6 +614,13 @@ long emx_get_iteration_log(const emx_problem *p, uint32_t *host_out, long max_it
     if (n > max_iter) n = max_iter;
     if (n) memcpy(host_out, p->iter_log.data(), (size_t)n * 2 * sizeof(uint32_t));
     return n;
+}
+
+int emx_get_lanes(const emx_problem *p, uint64_t *lanes6) {
+    if (!p || !lanes6 || !p->have_ctl) return EMX_E_ARG;
+    for (int ph = 0; ph < 2; ++ph)
+        for (int pt = 0; pt < 3; ++pt) lanes6[3 * ph + pt] = p->last_ctl.lanes[ph][pt];
+    return EMX_OK;
 }
 
 long emx_get_iteration_times(const emx_problem *p, float *host_out, long max_iter) {

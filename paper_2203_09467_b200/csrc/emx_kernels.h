@@ -29,6 +29,8 @@ cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st);
 // launch_step (one persistent kernel per pool); tally = device edep array
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st);
 cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st);
+cudaError_t launch_phase(int pt, int phase, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
+                         cudaStream_t st);
 cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                              cudaStream_t st);
 constexpr int kLaunchesPerIteration = 9;  // 3 refill kernels + 3 x (phase A + phase B)

@@ -614,12 +614,14 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
         const unsigned n_done = __popc(__ballot_sync(0xffffffffu, commit && pend < 0));  // completed steps
         const unsigned n_tomb = __popc(__ballot_sync(0xffffffffu, tomb || parked));
         const unsigned n_stall = __popc(__ballot_sync(0xffffffffu, active && stall));
+        const unsigned n_active = __popc(__ballot_sync(0xffffffffu, active));
         if (lane == 9) add = n_g;
         if (lane == 10) add = n_e;
         if (lane == 11) add = n_p;
         if (lane == 12 + PT) add = n_done;
         if (lane == 15) add = n_commit + n_tomb;
         if (lane == 16) add = n_stall;
+        if (lane == 17) add = n_active;
         acc.n += add;
     }
     return acc;
@@ -794,6 +796,7 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_
                                   : lane == 15 ? &c->progress
                                                : &c->stalls;
         if (lane <= 16) atomicAdd(dst, acc.n);
+        if (lane == 17) atomicAdd(&c->lanes[0][PT], acc.n);
     }
     if (acc.d != 0.0 && lane < 4) {
         double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
@@ -847,6 +850,7 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_interact(const __grid_c
                                   : lane == 15 ? &c->progress
                                                : &c->stalls;
         if (lane <= 16) atomicAdd(dst, acc.n);
+        if (lane == 17) atomicAdd(&c->lanes[1][PT], acc.n);
     }
     if (acc.d != 0.0 && lane < 4) {
         double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
@@ -872,7 +876,23 @@ cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *t
     return cudaGetLastError();
 }
 
-// the step kernel of one pool on its own stream (fork / join branches of the iteration graph)
+// one phase of one pool (profiling path: every kernel bracketed by events)
+cudaError_t launch_phase(int pt, int phase, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
+                         cudaStream_t st) {
+    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM);
+    if (phase == 0) {
+        if (pt == kGamma) k_step_pool<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
+        else if (pt == kElectron) k_step_pool<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        else k_step_pool<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+    } else {
+        if (pt == kGamma) k_interact<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
+        else if (pt == kElectron) k_interact<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        else k_interact<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+    }
+    return cudaGetLastError();
+}
+
+// the step kernels of one pool on its own stream (fork / join branches of the iteration graph)
 cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                              cudaStream_t st) {
     // persistent single-warp blocks per SM for this pool: the three pools' kernels run side by side, so each

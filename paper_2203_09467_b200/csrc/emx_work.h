@@ -61,6 +61,7 @@ struct Ctl {
     double edep_total;            // all energy deposited so far (every cell, tallied or not)
     double escaped, below_cut, looper, E_in;
     unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls, peak_live, peak_queue;
+    unsigned long long lanes[2][3];  // track slots processed by phase A / phase B kernels, per pool
 };
 
 struct Work {

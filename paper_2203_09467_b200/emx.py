@@ -49,7 +49,7 @@ class StepResult(C.Structure):
 EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "emx_add_volume", "emx_set_field",
            "emx_get_physics", "emx_set_physics", "emx_set_cuts", "emx_build_tables", "emx_get_table",
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
-           "emx_reset_tallies", "emx_read_tallies", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile",
+           "emx_reset_tallies", "emx_read_tallies", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
            "emx_get_iteration_log", "emx_get_iteration_times",
            "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_last_error",
            "emx_version"]
@@ -80,6 +80,7 @@ def lib():
             "emx_reset_tallies": (i, [vp, vp]), "emx_read_tallies": (i, [vp, vp, C.POINTER(Scalars)]),
             "emx_last_transport_ms": (d, [vp]), "emx_get_iteration_log": (l, [vp, vp, l]),
             "emx_get_iteration_times": (l, [vp, vp, l]),
+            "emx_get_lanes": (i, [vp, vp]),
             "emx_set_profile": (i, [vp, i]), "emx_get_profile": (i, [vp, vp, vp, vp]),
             "emx_step_batch": (i, [vp, u64, l, vp, vp, vp]),
             "emx_philox_batch": (i, [l, vp, vp, vp, vp]),
@@ -257,12 +258,15 @@ class Problem:
         self._check(lib().emx_set_profile(self.h, int(on)))
 
     def profile(self):
-        """dict(ms=[step gamma, step e-, step e+, refill], launches, iterations_launched) of the last transport"""
-        ms = (C.c_double * 4)()
+        """dict(ms=[A gamma, A e-, A e+, B gamma, B e-, B e+, refill, all step kernels], lanes=[same six],
+        launches, iterations_launched) of the last transport"""
+        ms = (C.c_double * 8)()
         nl, ni = C.c_long(), C.c_long()
         self._check(lib().emx_get_profile(self.h, C.cast(ms, C.c_void_p), C.cast(C.byref(nl), C.c_void_p),
                                           C.cast(C.byref(ni), C.c_void_p)))
-        return dict(ms=list(ms), launches=nl.value, iterations_launched=ni.value)
+        lanes = (C.c_uint64 * 6)()
+        lib().emx_get_lanes(self.h, C.cast(lanes, C.c_void_p))
+        return dict(ms=list(ms), lanes=list(lanes), launches=nl.value, iterations_launched=ni.value)
 
     def iteration_times(self, max_iter=1 << 16):
         """(n, 2) float32: refill ms, step-kernel ms per iteration of the last transport (profiling on)"""
