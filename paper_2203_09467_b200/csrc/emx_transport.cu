@@ -10,19 +10,32 @@
 
 namespace emx {
 
+// stack records are written once and read once: streaming stores / loads (evict-first) keep them from
+// displacing the track store in L2
+#ifndef EMX_STREAM_HINTS
+#define EMX_STREAM_HINTS 1
+#endif
+#if EMX_STREAM_HINTS
+#define EMX_ST(p, v) __stcs((p), (v))
+#define EMX_LD(p) __ldcs((p))
+#else
+#define EMX_ST(p, v) (*(p) = (v))
+#define EMX_LD(p) (*(p))
+#endif
+
 __device__ __forceinline__ void load_record(const QueueSoA &q, int r, const TrackSoA &t, int i) {
-    t.x[i] = q.x[r];
-    t.y[i] = q.y[r];
-    t.z[i] = q.z[r];
-    t.ux[i] = q.ux[r];
-    t.uy[i] = q.uy[r];
-    t.uz[i] = q.uz[r];
-    t.E[i] = q.E[r];
-    t.tid[i] = q.tid[r];
-    t.prim[i] = q.prim[r];
+    t.x[i] = EMX_LD(&q.x[r]);
+    t.y[i] = EMX_LD(&q.y[r]);
+    t.z[i] = EMX_LD(&q.z[r]);
+    t.ux[i] = EMX_LD(&q.ux[r]);
+    t.uy[i] = EMX_LD(&q.uy[r]);
+    t.uz[i] = EMX_LD(&q.uz[r]);
+    t.E[i] = EMX_LD(&q.E[r]);
+    t.tid[i] = (uint64_t)EMX_LD((const unsigned long long *)&q.tid[r]);
+    t.prim[i] = EMX_LD(&q.prim[r]);
     t.step[i] = 0u;
-    t.vol[i] = q.vol[r];
-    t.surf[i] = q.surf[r];
+    t.vol[i] = EMX_LD(&q.vol[r]);
+    t.surf[i] = EMX_LD(&q.surf[r]);
     t.alive[i] = 2;  // 2 = filled in this refill pass (k_move still ranks it as a hole)
     if (t.fs_a) t.fs_a[i] = 0;
     if (t.pend) t.pend[i] = 0;
@@ -401,17 +414,17 @@ constexpr int kStepWarpsPerSM = EMX_WARPS_PER_SM;
 
 __device__ __forceinline__ void push_record(const QueueSoA &q, int r, const Vec3 &x, const Vec3 &u, double E,
                                             uint64_t tid, uint32_t prim, int vol) {
-    q.x[r] = x.x;
-    q.y[r] = x.y;
-    q.z[r] = x.z;
-    q.ux[r] = u.x;
-    q.uy[r] = u.y;
-    q.uz[r] = u.z;
-    q.E[r] = E;
-    q.tid[r] = tid;
-    q.prim[r] = prim;
-    q.vol[r] = vol;
-    q.surf[r] = -1;
+    EMX_ST(&q.x[r], x.x);
+    EMX_ST(&q.y[r], x.y);
+    EMX_ST(&q.z[r], x.z);
+    EMX_ST(&q.ux[r], u.x);
+    EMX_ST(&q.uy[r], u.y);
+    EMX_ST(&q.uz[r], u.z);
+    EMX_ST(&q.E[r], E);
+    EMX_ST((unsigned long long *)&q.tid[r], (unsigned long long)tid);
+    EMX_ST(&q.prim[r], prim);
+    EMX_ST(&q.vol[r], vol);
+    EMX_ST(&q.surf[r], -1);
 }
 
 __device__ __forceinline__ double warp_sum(double v) {

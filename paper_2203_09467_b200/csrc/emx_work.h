@@ -82,6 +82,7 @@ struct Work {
     int wave;
     long long queue_soft;
     double inflight_cap;
+    size_t hot_bytes;       // leading part of the workspace that holds the track store, scan arrays and lists
     int warps_per_sm[3];    // persistent step-kernel warps per SM, per pool
     long long slice_above;  // live tracks above which the field propagation is time-sliced
     int slice_budget;       // substep attempts per track and iteration while sliced
