@@ -848,10 +848,10 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_interact(const __grid_c
         const int ch = __shfl_sync(0xffffffffu, k_next, 0);
         if (ch >= total) break;
         if (lane == 0) k_next = atomicAdd(&c->work_ctrB[PT], 1);
-        WarpAcc d;
-        if (ch < cb[1]) d = interact_chunk<PT>(P, w, seed, tally, ord0, ch << 5, n[0]);
-        else if (ch < cb[2]) d = interact_chunk<PT>(P, w, seed, tally, ord1, (ch - cb[1]) << 5, n[1]);
-        else d = interact_chunk<PT>(P, w, seed, tally, ord2, (ch - cb[2]) << 5, n[2]);
+        // one call site: the interactor code exists once per kernel
+        const int sel = ch < cb[1] ? 0 : (ch < cb[2] ? 1 : 2);
+        const int kk = sel == 0 ? ord0 : (sel == 1 ? ord1 : ord2);
+        const WarpAcc d = interact_chunk<PT>(P, w, seed, tally, kk, (ch - cb[sel]) << 5, n[sel]);
         acc.n += d.n;
         acc.d += d.d;
     }
