@@ -398,7 +398,8 @@ int emx_get_material_info(const emx_problem *p, int material, double *o) {
 }
 
 size_t emx_workspace_bytes(const emx_problem *p, long n_slots, long queue_capacity) {
-    if (!p || n_slots < 1 || queue_capacity < 1 || n_slots > (1L << 30) || queue_capacity > (1L << 30)) return 0;
+    // pools hold fewer than 2^21 slots each (packed list counters): n_slots <= 2^21
+    if (!p || n_slots < 1 || queue_capacity < 1 || n_slots > (1L << 21) || queue_capacity > (1L << 30)) return 0;
     Work w;
     return carve_work(nullptr, n_slots, queue_capacity, w, kMaxLog);
 }

@@ -311,8 +311,7 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
             c->progress = 0ull;
             c->work_ctr3[0] = c->work_ctr3[1] = c->work_ctr3[2] = 0;
             c->work_ctrB[0] = c->work_ctrB[1] = c->work_ctrB[2] = 0;
-            for (int a = 0; a < 3; ++a)
-                for (int b = 0; b < 3; ++b) c->icount[a][b] = 0;
+            for (int a = 0; a < 3; ++a) c->icount64[a] = 0ull;
         }
     }
 }
@@ -728,15 +727,21 @@ __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uin
     // file the lanes with a pending interaction (new or stalled) in the list of their process
     {
         const int pk = waiting ? proc_slot<PT>(pend_in) : (pend >= 0 && !parked ? proc_slot<PT>(pend) : -1);
-        constexpr int nk = (PT == kElectron) ? 2 : 3;
-#pragma unroll
-        for (int k = 0; k < nk; ++k) {
-            const unsigned b = __ballot_sync(0xffffffffu, pk == k);
-            if (b) {
-                int r0 = 0;
-                if (lane == 0) r0 = atomicAdd(&c->icount[PT][k], __popc(b));
-                r0 = __shfl_sync(0xffffffffu, r0, 0);
-                if (pk == k) w.ilist[PT][k][r0 + __popc(b & lt)] = i;
+        // the three list counters of a pool are packed into one 64-bit word (21 bits each; pools hold fewer than
+        // 2^21 slots, checked by the host), so one atomic per warp reserves the entries of all three lists
+        const unsigned b0 = __ballot_sync(0xffffffffu, pk == 0);
+        const unsigned b1 = __ballot_sync(0xffffffffu, pk == 1);
+        const unsigned b2 = __ballot_sync(0xffffffffu, pk == 2);
+        if (b0 | b1 | b2) {
+            unsigned long long base = 0ull;
+            if (lane == 0)
+                base = atomicAdd(&c->icount64[PT], (unsigned long long)__popc(b0) | ((unsigned long long)__popc(b1) << 21) |
+                                                       ((unsigned long long)__popc(b2) << 42));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (pk >= 0) {
+                const unsigned bk = pk == 0 ? b0 : (pk == 1 ? b1 : b2);
+                const int r0 = (int)((base >> (21 * pk)) & 0x1fffffull);
+                w.ilist[PT][pk][r0 + __popc(bk & lt)] = i;
             }
         }
     }
@@ -819,8 +824,11 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_
 
 // Phase B: the interactors.  Persistent single-warp blocks pull 32-entry chunks of the pool's process lists;
 // a warp runs ONE interactor on (up to) 32 tracks that all selected it.
+#ifndef EMX_WARPS_B
+#define EMX_WARPS_B EMX_WARPS_PER_SM
+#endif
 template <int PT>
-__global__ void __launch_bounds__(32, kStepWarpsPerSM) k_interact(const __grid_constant__ Params P,
+__global__ void __launch_bounds__(32, EMX_WARPS_B) k_interact(const __grid_constant__ Params P,
                                                                  const __grid_constant__ Work w, uint64_t seed,
                                                                  double *tally) {
     Ctl *c = w.ctl;
@@ -833,9 +841,10 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_interact(const __grid_c
     const int ord0 = (PT == kGamma) ? 2 : 0, ord1 = (PT == kGamma) ? 0 : 1, ord2 = (PT == kGamma) ? 1 : 2;
     int n[3], cb[4];
     cb[0] = 0;
-    n[0] = c->icount[PT][ord0];
-    n[1] = c->icount[PT][ord1];
-    n[2] = ord2 < nk ? c->icount[PT][ord2] : 0;
+    const unsigned long long packed = c->icount64[PT];
+    n[0] = (int)((packed >> (21 * ord0)) & 0x1fffffull);
+    n[1] = (int)((packed >> (21 * ord1)) & 0x1fffffull);
+    n[2] = ord2 < nk ? (int)((packed >> (21 * ord2)) & 0x1fffffull) : 0;
 #pragma unroll
     for (int k = 0; k < 3; ++k) cb[k + 1] = cb[k] + ((n[k] + 31) >> 5);
     const int total = cb[3];

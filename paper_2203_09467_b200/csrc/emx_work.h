@@ -52,7 +52,7 @@ struct Ctl {
     int done, error, had_live;
     int work_ctr3[3];  // next 32-slot chunk of each pool's step kernel (phase A)
     int work_ctrB[3];  // next 32-entry chunk of each pool's interaction lists (phase B)
-    int icount[3][3];  // entries in the interaction lists [pool][process slot]
+    unsigned long long icount64[3];  // entries in the interaction lists of each pool, 3 x 21 bits packed
     int field_budget;  // substep attempts per track and iteration (time slicing of the field propagation)
     unsigned long long iter;
     unsigned long long progress;  // steps committed + tombstones retired in the current iteration (R7)
