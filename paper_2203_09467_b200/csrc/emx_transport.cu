@@ -224,10 +224,16 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
         const int nch = (n_old + kChunk - 1) / kChunk;
         if (tid == 0) s_carry = 0;
         __syncthreads();
-        for (int base = 0; base < nch; base += blockDim.x) {
-            const int k = base + tid;
-            const int v = (k < nch) ? w.chunk_dead[p][k] : 0;
-            int inc = v;  // inclusive warp scan
+        constexpr int kPer = 8;  // chunks per thread: one pass covers 8192 chunks = 2^20 slots
+        for (int base = 0; base < nch; base += blockDim.x * kPer) {
+            const int k0 = base + tid * kPer;
+            int d[kPer], v = 0;
+#pragma unroll
+            for (int q = 0; q < kPer; ++q) {
+                d[q] = (k0 + q < nch) ? w.chunk_dead[p][k0 + q] : 0;
+                v += d[q];
+            }
+            int inc = v;  // inclusive warp scan of the per-thread sums
             for (int o = 1; o < 32; o <<= 1) {
                 const int t = __shfl_up_sync(0xffffffffu, inc, o);
                 if (lane >= o) inc += t;
@@ -243,13 +249,17 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
                 s_warp[lane] = xi - x;  // exclusive warp offsets
             }
             __syncthreads();
-            const int off = s_carry + s_warp[wid] + inc - v;
-            if (k < nch) {
-                w.chunk_off[p][k] = off;
-                w.chunk_dead[p][k] = 0;  // the step kernels count the next iteration's deaths into it
+            int off = s_carry + s_warp[wid] + inc - v;
+#pragma unroll
+            for (int q = 0; q < kPer; ++q) {
+                if (k0 + q < nch) {
+                    w.chunk_off[p][k0 + q] = off;
+                    w.chunk_dead[p][k0 + q] = 0;  // the step kernels count the next iteration's deaths into it
+                }
+                off += d[q];
             }
             __syncthreads();
-            if (tid == blockDim.x - 1) s_carry = off + v;
+            if (tid == blockDim.x - 1) s_carry = off;
             __syncthreads();
         }
         if (tid == 0) {
