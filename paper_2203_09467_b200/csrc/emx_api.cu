@@ -95,7 +95,7 @@ void split3(long n, const double f[3], int out[3]) {
 }
 
 const double kPoolFrac[3] = {0.50, 0.42, 0.08};   // measured live mix of the workloads
-const double kQueueFrac[3] = {0.45, 0.45, 0.10};
+const double kQueueFrac[3] = {0.30, 0.60, 0.10};  // e- secondaries dominate the queued records in every config
 
 struct Carve {
     char *base;

@@ -118,9 +118,10 @@ __device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) 
     if (c->done) return;
     const long long next = c->next_primary;
     if (next >= pr.n) return;
-    const long long queued = (long long)c->q_top[0] + c->q_top[1] + c->q_top[2];
     const double inflight = c->E_admitted - (c->edep_total + c->escaped + c->looper);
-    if (inflight >= w.inflight_cap || queued >= w.queue_soft) return;
+    if (inflight >= w.inflight_cap) return;
+    for (int p = 0; p < 3; ++p)
+        if (4LL * c->q_top[p] >= (long long)w.qcap[p]) return;  // a stack is a quarter full: let it drain first
     const long long A = (pr.n - next) < (long long)w.wave ? (pr.n - next) : (long long)w.wave;
     // pass 1: counts per type and energy of the window
     int cnt[3] = {0, 0, 0};
@@ -452,8 +453,8 @@ struct WarpAcc {
 // Reserve `cnt` records (warp total) on stack ty; returns the base index or -1 when the stack is full.
 // Far from the capacity one atomicAdd does it: kReserveSlack bounds what all resident warps of
 // the three step kernels can request at the same time (one outstanding reservation of <= 96 records each), so
-// the top cannot pass the capacity.  Near the capacity the reservation is a compare-and-swap that never
-// moves the top past the capacity.  Nothing is ever rolled back: an add-then-subtract scheme lets a
+// the top cannot pass the capacity.  Near the capacity a small stack (tests) is reserved by compare-and-swap,
+// which never moves the top past the capacity; a large stack is simply treated as full.  Nothing is ever rolled back: an add-then-subtract scheme lets a
 // reservation succeed above a top that a concurrent failure has inflated, and strands its records.
 constexpr int kReserveSlack = 148 * 3 * 32 * 96;
 
@@ -464,7 +465,8 @@ __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, i
         int old = *(volatile int *)&c->q_top[ty];
         if ((long long)old + cnt + kReserveSlack <= (long long)cap) {
             r0 = atomicAdd(&c->q_top[ty], cnt);
-        } else {
+        } else if (cap < 8 * kReserveSlack) {
+            // small stack: exact accounting by compare-and-swap
             while (old + cnt <= cap) {
                 const int prev = atomicCAS(&c->q_top[ty], old, old + cnt);
                 if (prev == old) {
@@ -474,6 +476,8 @@ __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, i
                 old = prev;
             }
         }
+        // large stack within kReserveSlack of its capacity: treated as full (thousands of warps spinning on one
+        // compare-and-swap cost 10x the iteration; the last 2 % of a large stack are not worth it)
     }
     return __shfl_sync(0xffffffffu, r0, 0);
 }

@@ -156,7 +156,41 @@ def config4(n=100000):
     return desc, _prim(n, pt, E, (0, 0, 0), d, 0, -1)
 
 
-CONFIGS = [config0, config1, config2, config3, config4]
+# ---- the paper's own verification problem as a sixth workload -------------
+GRAPHITE = dict(name="C", Z=[6], A=[12.011], w=[1.0], rho=2.0, I_eV=78.0)
+TI = dict(name="Ti", Z=[22], A=[47.867], w=[1.0], rho=4.54, I_eV=233.0)
+FE = dict(name="Fe", Z=[26], A=[55.845], w=[1.0], rho=7.874, I_eV=286.0)
+
+
+def config5(n=100000, n_zbins=28, half_length=700.0):
+    """"An idealized coarse representation of the main components of the CMS detector, comprising six
+    cylindrical shells centered about the z axis up to 375 cm ... vacuum, Si, Pb, C, Ti, and Fe"; "an isotropic
+    1 GeV photon point source at the origin, composed of 100 events each with 1000 photon primaries";
+    observables: cumulative energy deposition over z, steps per track by particle type.
+    The paper gives neither the radii nor the length: reading = radii 30 / 125 / 175 /
+    275 / 325 / 375 cm, |z| < 700 cm, no field.  The z tally is realised in the geometry: every
+    shell is cut into n_zbins slabs and all cells of a slab share one tally id."""
+    radii = [30.0, 125.0, 175.0, 275.0, 325.0, 375.0]
+    mats = [SI, PB, GRAPHITE, TI, FE]                     # shells outside the vacuum core
+    nr = len(radii)
+    zs = [-half_length + k * (2.0 * half_length / n_zbins) for k in range(n_zbins + 1)]
+    surfaces = [(CZ, r) for r in radii] + [(PZ, z) for z in zs]
+    vols = [dict(surf=[0, nr, nr + n_zbins], sense=[-1, 1, -1], material=-1, tally=-1)]   # vacuum core
+    for i in range(1, nr):
+        for k in range(n_zbins):
+            vols.append(dict(surf=[i - 1, i, nr + k, nr + k + 1], sense=[1, -1, 1, -1], material=i - 1, tally=k))
+    desc = dict(name="config5_paper_verification", seed=5, materials=mats, surfaces=surfaces, volumes=vols,
+                field=(0.0, 0.0, 0.0), physics=physics(), n_slots=1 << 20, queue_capacity=1 << 26)
+    rng = np.random.default_rng(5)
+    xi = rng.random(size=(n, 2))
+    mu = 2.0 * xi[:, 0] - 1.0
+    phi = 2.0 * np.pi * xi[:, 1]
+    s = np.sqrt((1.0 - mu) * (1.0 + mu))
+    d = np.stack([s * np.cos(phi), s * np.sin(phi), mu], axis=1)
+    return desc, _prim(n, 0, 1000.0, (0, 0, 0), d, 0, -1)
+
+
+CONFIGS = [config0, config1, config2, config3, config4, config5]
 
 
 def get(k, n=None):

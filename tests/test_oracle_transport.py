@@ -230,7 +230,7 @@ def test_config0_energy_sum_first_collision_and_step_count(emo):
     assert np.median(depth) == pytest.approx(mfp * math.log(2), rel=0.12)
 
 
-@pytest.mark.parametrize("cfg,n", [(1, 40), (2, 6), (3, 6), (4, 24)])
+@pytest.mark.parametrize("cfg,n", [(1, 40), (2, 6), (3, 6), (4, 24), (5, 60)])
 def test_energy_closure_per_event(emo, cfg, n):
     desc, prim = W.get(cfg, n)
     P = emo.Problem(desc)
@@ -274,3 +274,25 @@ def test_shower_sanity_config2(emo):
     assert 2.0 < zmax < 12.0
     frac_ar = r["edep"][1::2].sum() / r["edep"].sum()
     assert 0.05 < frac_ar < 0.5                                            # sampling fraction of lAr
+
+
+def test_paper_verification_problem_geometry(emo):
+    """SURVEY 8(f) f1 / PAPER.md:172-176: six cylindrical regions to 375 cm cut into z slabs.  A straight
+    radial photon crosses the shells at the declared radii, and the slab tallies of a small run add up to
+    the deposited energy (the z tally lives in the geometry)."""
+    desc, prim = W.get(5, 40)
+    P = emo.Problem(desc)
+    x, u, vol, surf = np.array([0.0, 0.0, 3.0]), np.array([1.0, 0.0, 0.0]), 0, -1
+    radii = []
+    for _ in range(6):
+        d, hit = P.distance(vol, x, u, surf)
+        x = x + d * u
+        radii.append(float(np.hypot(x[0], x[1])))
+        vol, surf = P.neighbour(x, u, hit), hit
+        if vol < 0:
+            break
+    assert radii == pytest.approx([30.0, 125.0, 175.0, 275.0, 325.0, 375.0], abs=1e-9) and vol == -1
+    r = P.transport(prim, desc["seed"], per_primary=True)
+    assert len(r["edep"]) == 28
+    assert r["edep"].sum() + r["escaped"] + r["looper"] == pytest.approx(r["E_in"], rel=1e-11)
+    assert r["edep"][13] + r["edep"][14] > 0.4 * r["E_in"]            # isotropic source: most energy near z = 0
