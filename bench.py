@@ -108,6 +108,25 @@ def oracle_sample_size(desc, prim, threads):
     return int(max(n0, min(len(prim["E"]), rate * 15.0)))
 
 
+def replica_seed(base_seed, rank):
+    """Replicas (N > 1): the same problem on every GPU with independent histories."""
+    return base_seed + 1000 * rank
+
+
+def reduce_over_ranks(times, counts, device):
+    """The only exchange of an N-GPU run: max over ranks of the timed durations, sum over ranks of the work
+    done.  Works on any torch.distributed backend (nccl on GPUs; gloo on CPU in the tests)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(t) for t in times], [float(c) for c in counts]
+    t = torch.tensor([float(x) for x in times], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([float(x) for x in counts], device=device, dtype=torch.float64)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return t.tolist(), c.tolist()
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores; each step = a bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -155,7 +174,7 @@ def run_ours(args):
 
     desc, prim = workload(args)
     n_prim = len(prim["E"])
-    seed = desc["seed"] + 1000 * rank          # replicas: same problem, independent histories
+    seed = replica_seed(desc["seed"], rank)
     G = emx.Problem(desc)
     pdev = G.upload_primaries(prim)
     pinned = {k: torch.from_numpy(np.array(v, order="C")).pin_memory() for k, v in prim.items()}
@@ -213,15 +232,7 @@ def run_ours(args):
     barrier()
     e2e_s = time.perf_counter() - t0
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
-        c = torch.tensor([float(tot["steps"]), float(e2e_steps)], device="cuda", dtype=torch.float64)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        all_steps, all_e2e = float(c[0]), float(c[1])
-    else:
-        all_steps, all_e2e = float(tot["steps"]), float(e2e_steps)
+    (ms, e2e_s), (all_steps, all_e2e) = reduce_over_ranks([ms, e2e_s], [tot["steps"], e2e_steps], "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
