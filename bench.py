@@ -32,8 +32,8 @@ METRIC, UNIT = "track_steps_per_sec", "track-steps/s"
 B_STEP, B_SEC = 80 + 69, 76
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the committed `ncu --set full` capture
 # of a saturated iteration (profiles/r1_final_step_kernels_full.md)
-TRAFFIC_PER_LAUNCH = {"k_step_pool<gamma>": 23.3e6, "k_step_pool<e->": 37.9e6, "k_step_pool<e+>": 7.3e6,
-                      "k_interact<gamma>": 32.2e6, "k_interact<e->": 29.3e6, "k_interact<e+>": 9.4e6}
+TRAFFIC_PER_LAUNCH = {"k_step_pool<gamma>": 23.8e6, "k_step_pool<e->": 37.9e6, "k_step_pool<e+>": 7.3e6,
+                      "k_interact<gamma>": 27.2e6, "k_interact<e->": 27.3e6, "k_interact<e+>": 6.7e6}
 
 
 def parse():

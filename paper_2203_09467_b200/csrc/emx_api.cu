@@ -48,7 +48,7 @@ struct emx_problem {
     bool use_graph = true;
     long slice_above = -1;  // < 0: n_slots / 32
     int slice_budget = 2;
-    int warps_per_sm[3] = {16, 16, 16};
+    int warps_per_sm[3] = {16, 16, 8};  // gamma, e-, e+ (the e+ pool holds 8 % of the slots)
 };
 
 namespace {
@@ -419,7 +419,6 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     // the queue (measured on configs 1-4), with a factor 4 of headroom below the capacity
     w.n_primaries = pr.n;
     w.wave = (int)(n_slots / 256 < 256 ? 256 : (n_slots / 256 > 4096 ? 4096 : n_slots / 256));
-    w.queue_soft = queue_capacity / 4;
     w.inflight_cap = 5.0 * (double)queue_capacity;
     w.slice_above = p->slice_above >= 0 ? p->slice_above : n_slots / 32;
     w.slice_budget = p->slice_budget;

@@ -421,6 +421,13 @@ __global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
 #define EMX_WARPS_PER_SM 16
 #endif
 constexpr int kStepWarpsPerSM = EMX_WARPS_PER_SM;
+// warps of a step-kernel block are independent (no barrier, no shared memory); they are grouped four to a
+// block only because block dispatch is what an idle iteration costs (~2.4 ns per block, 21 000 single-warp
+// blocks per iteration = 50 us)
+#ifndef EMX_STEP_BLOCK
+#define EMX_STEP_BLOCK 128
+#endif
+constexpr int kStepBlock = EMX_STEP_BLOCK;
 
 __device__ __forceinline__ void push_record(const QueueSoA &q, int r, const Vec3 &x, const Vec3 &u, double E,
                                             uint64_t tid, uint32_t prim, int vol) {
@@ -507,7 +514,7 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     acc.n = 0ull;
     acc.d = 0.0;
     Ctl *c = w.ctl;
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const TrackSoA &ts = w.trk[PT];
     // ---- A8: secondaries -> typed stacks.  When a stack cannot take the warp's records the lanes that needed
@@ -663,7 +670,7 @@ template <int PT>
 __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
                                              int n_live, int budget) {
     Ctl *c = w.ctl;
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const int i = base + lane;
     const TrackSoA &ts = w.trk[PT];
@@ -766,7 +773,7 @@ __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uin
 template <int PT>
 __device__ __forceinline__ WarpAcc interact_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int k,
                                                   int first, int n_list) {
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x & 31;
     const int idx = first + lane;
     const TrackSoA &ts = w.trk[PT];
     const bool active = idx < n_list;
@@ -799,11 +806,11 @@ __device__ __forceinline__ WarpAcc interact_chunk(const Params &P, const Work &w
 }
 
 template <int PT>
-__global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_constant__ Params P,
+__global__ void __launch_bounds__(kStepBlock, kStepWarpsPerSM * 32 / kStepBlock) k_step_pool(const __grid_constant__ Params P,
                                                                   const __grid_constant__ Work w, uint64_t seed,
                                                                   double *tally) {
     Ctl *c = w.ctl;
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x & 31;
     const int nl = c->m_step[PT];
     const int total = (nl + 31) >> 5;
     const int budget = c->field_budget;
@@ -842,11 +849,11 @@ __global__ void __launch_bounds__(32, kStepWarpsPerSM) k_step_pool(const __grid_
 #define EMX_WARPS_B EMX_WARPS_PER_SM
 #endif
 template <int PT>
-__global__ void __launch_bounds__(32, EMX_WARPS_B) k_interact(const __grid_constant__ Params P,
+__global__ void __launch_bounds__(kStepBlock, EMX_WARPS_B * 32 / kStepBlock) k_interact(const __grid_constant__ Params P,
                                                                  const __grid_constant__ Work w, uint64_t seed,
                                                                  double *tally) {
     Ctl *c = w.ctl;
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x & 31;
     constexpr int nk = (PT == kElectron) ? 2 : 3;
     // order in which the lists are worked off.  The stacks are LIFO, so what is pushed LAST is refilled
     // first: photons run pair production first (its leptons are the most energetic secondaries and go to the
@@ -915,15 +922,15 @@ cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *t
 // one phase of one pool (profiling path: every kernel bracketed by events)
 cudaError_t launch_phase(int pt, int phase, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                          cudaStream_t st) {
-    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM);
+    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM) * 32 / kStepBlock;
     if (phase == 0) {
-        if (pt == kGamma) k_step_pool<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
-        else if (pt == kElectron) k_step_pool<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
-        else k_step_pool<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        if (pt == kGamma) k_step_pool<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        else if (pt == kElectron) k_step_pool<kElectron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        else k_step_pool<kPositron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
     } else {
-        if (pt == kGamma) k_interact<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
-        else if (pt == kElectron) k_interact<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
-        else k_interact<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        if (pt == kGamma) k_interact<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        else if (pt == kElectron) k_interact<kElectron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        else k_interact<kPositron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
     }
     return cudaGetLastError();
 }
@@ -933,16 +940,16 @@ cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t se
                              cudaStream_t st) {
     // persistent single-warp blocks per SM for this pool: the three pools' kernels run side by side, so each
     // gets a share of the 16 warps per SM that fit
-    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM);
+    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM) * 32 / kStepBlock;
     if (pt == kGamma) {
-        k_step_pool<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
-        k_interact<kGamma><<<g, 32, 0, st>>>(P, w, seed, tally);
+        k_step_pool<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        k_interact<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
     } else if (pt == kElectron) {
-        k_step_pool<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
-        k_interact<kElectron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        k_step_pool<kElectron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        k_interact<kElectron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
     } else {
-        k_step_pool<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
-        k_interact<kPositron><<<g, 32, 0, st>>>(P, w, seed, tally);
+        k_step_pool<kPositron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        k_interact<kPositron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
     }
     return cudaGetLastError();
 }

@@ -77,10 +77,9 @@ struct Work {
     uint32_t *log;  // per iteration: live, queued
     int max_log;
     // admission of primaries (R8): up to `wave` primaries enter per iteration while the energy in
-    // flight (admitted - deposited - escaped) is below inflight_cap and fewer than queue_soft records wait
+    // flight (admitted - deposited - escaped) is below inflight_cap and no stack is more than a quarter full
     long long n_primaries;
     int wave;
-    long long queue_soft;
     double inflight_cap;
     size_t hot_bytes;       // leading part of the workspace that holds the track store, scan arrays and lists
     int warps_per_sm[3];    // persistent step-kernel warps per SM, per pool
