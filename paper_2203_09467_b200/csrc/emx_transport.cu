@@ -63,6 +63,33 @@ __device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
     }
 }
 
+// Optional timeline of the iteration graph (diagnostics, -DEMX_TIMELINE): first block start / last block end
+// of every kernel node, from %globaltimer, for iterations [EMX_TL_FIRST, EMX_TL_FIRST + kTlN).
+#ifdef EMX_TIMELINE
+#ifndef EMX_TL_FIRST
+#define EMX_TL_FIRST 2500
+#endif
+constexpr int kTlN = 64;
+__device__ unsigned long long g_tl[kTlN][9][4];  // min start, max end, sum of block times, blocks
+__device__ __forceinline__ void tl_mark(const Work &w, int node, int which, int iter_off) {
+    __shared__ unsigned long long s_t0;
+    if (threadIdx.x != 0) return;
+    const long long it = (long long)w.ctl->iter - iter_off - EMX_TL_FIRST;
+    if (it < 0 || it >= kTlN) return;
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    atomicMax(&g_tl[it][node][which], which == 0 ? ~t : t);
+    if (which == 0) s_t0 = t;
+    else {
+        atomicAdd(&g_tl[it][node][2], t - s_t0);
+        atomicAdd(&g_tl[it][node][3], 1ull);
+    }
+}
+#define EMX_TL(w, node, which, off) tl_mark(w, node, which, off)
+#else
+#define EMX_TL(w, node, which, off) ((void)0)
+#endif
+
 // ------------------------------------------------------------------------------------------------
 // Loop start: clear the control block, total the injected energy and the primaries per type.
 __global__ void __launch_bounds__(1024) k_init(Work w, Primaries pr) {
@@ -113,7 +140,7 @@ __device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) 
     __shared__ int s_total[3], s_base[3];
     __shared__ double s_E[32];
     __shared__ int s_go;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
     Ctl *c = w.ctl;
     if (c->done) return;
     const long long next = c->next_primary;
@@ -145,7 +172,7 @@ __device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) 
         int go = 1;
         for (int p = 0; p < 3; ++p) {
             int t = 0;
-            for (int k = 0; k < 32; ++k) t += s_cnt[p][k];
+            for (int k = 0; k < nw; ++k) t += s_cnt[p][k];
             s_total[p] = t;
             s_base[p] = 0;
             if (c->q_top[p] + t > w.qcap[p]) go = 0;  // no room: try again in a later iteration
@@ -186,14 +213,14 @@ __device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) 
         __syncthreads();
         if (tid < 3) {
             int t = 0;
-            for (int q = 0; q < 32; ++q) t += s_cnt[tid][q];
+            for (int q = 0; q < nw; ++q) t += s_cnt[tid][q];
             s_base[tid] += t;
         }
         __syncthreads();
     }
     if (tid == 0) {
         double e = 0.0;
-        for (int k = 0; k < 32; ++k) e += s_E[k];
+        for (int k = 0; k < nw; ++k) e += s_E[k];
         for (int p = 0; p < 3; ++p) c->q_top[p] += s_total[p];
         c->next_primary = next + A;
         c->E_admitted += e;
@@ -205,6 +232,8 @@ cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st) {
     return cudaGetLastError();
 }
 
+constexpr int kPlanThreads = 1024;
+
 // ------------------------------------------------------------------------------------------------
 // A9 / A12: refill plan and loop control.  One block.  Per pool: exclusive prefix sum of the per-chunk
 // dead counts the step kernel left behind -> rank of every hole; then the sizes of the refill:
@@ -213,21 +242,23 @@ cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st) {
 //          n_new move into the remaining holes below it (j-th live track from the end -> j-th such hole),
 //   extra  records appended above the old range when the stack holds more than the holes.
 __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
-    __shared__ int s_warp[32];
-    __shared__ int s_carry;
+    constexpr int kGroupWarps = 10;  // warps 0-9 scan the gamma pool, 10-19 e-, 20-29 e+ (side by side)
+    __shared__ int s_warp[3][kGroupWarps];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     Ctl *c = w.ctl;
     if (c->done) return;
+    EMX_TL(w, 0, 0, 0);
     admit_block(w, pr);
     __syncthreads();
-    for (int p = 0; p < 3; ++p) {
+    const int p = wid / kGroupWarps, wig = wid % kGroupWarps;  // pool of this warp, warp index in its group
+    if (p < 3) {
+        const int gt = wig * 32 + lane;  // thread index in the group
         const int n_old = c->n_live[p];
         const int nch = (n_old + kChunk - 1) / kChunk;
-        if (tid == 0) s_carry = 0;
-        __syncthreads();
-        constexpr int kPer = 8;  // chunks per thread: one pass covers 8192 chunks = 2^20 slots
-        for (int base = 0; base < nch; base += blockDim.x * kPer) {
-            const int k0 = base + tid * kPer;
+        constexpr int kPer = 8;  // chunks per thread: one pass of a group covers 2560 chunks
+        int carry = 0;           // dead slots before this pass (every thread of the group keeps its own copy)
+        for (int base = 0; base < nch; base += kGroupWarps * 32 * kPer) {
+            const int k0 = base + gt * kPer;
             int d[kPer], v = 0;
 #pragma unroll
             for (int q = 0; q < kPer; ++q) {
@@ -239,18 +270,16 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
                 const int t = __shfl_up_sync(0xffffffffu, inc, o);
                 if (lane >= o) inc += t;
             }
-            if (lane == 31) s_warp[wid] = inc;
-            __syncthreads();
-            if (wid == 0) {
-                int x = s_warp[lane], xi = x;
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int t = __shfl_up_sync(0xffffffffu, xi, o);
-                    if (lane >= o) xi += t;
-                }
-                s_warp[lane] = xi - x;  // exclusive warp offsets
+            if (lane == 31) s_warp[p][wig] = inc;
+            asm volatile("bar.sync %0, %1;" ::"r"(p + 1), "r"(kGroupWarps * 32) : "memory");
+            int before = 0, total = 0;
+#pragma unroll
+            for (int k = 0; k < kGroupWarps; ++k) {
+                const int x = s_warp[p][k];
+                before += k < wig ? x : 0;
+                total += x;
             }
-            __syncthreads();
-            int off = s_carry + s_warp[wid] + inc - v;
+            int off = carry + before + inc - v;
 #pragma unroll
             for (int q = 0; q < kPer; ++q) {
                 if (k0 + q < nch) {
@@ -259,12 +288,11 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
                 }
                 off += d[q];
             }
-            __syncthreads();
-            if (tid == blockDim.x - 1) s_carry = off;
-            __syncthreads();
+            carry += total;
+            asm volatile("bar.sync %0, %1;" ::"r"(p + 1), "r"(kGroupWarps * 32) : "memory");
         }
-        if (tid == 0) {
-            const int h = s_carry;
+        if (gt == 0) {
+            const int h = carry;
             const int q = c->q_top[p];
             const int a = h < q ? h : q;
             const int n_new = n_old - (h - a);
@@ -287,8 +315,8 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
             c->n_live[p] = pl.n_final;
             c->q_top[p] = pl.q_new;
         }
-        __syncthreads();
     }
+    __syncthreads();
     if (tid == 0) {
         const long long ng = c->n_live[0], ne = c->n_live[1], np = c->n_live[2];
         const long long live = ng + ne + np;
@@ -310,6 +338,7 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
             c->m_step[0] = (int)ng;
             c->m_step[1] = (int)ne;
             c->m_step[2] = (int)np;
+            EMX_TL(w, 0, 1, 1);
             if (c->had_live && c->progress == 0ull) {
                 c->error = EMX_E_CAPACITY;
                 c->done = 1;
@@ -351,6 +380,7 @@ __global__ void __launch_bounds__(kChunk) k_fill(Work w, int32_t *dbg_src) {
     const int top = pl.n_old > pl.n_final ? pl.n_old : pl.n_final;
     const int nch_old = (pl.n_old + kChunk - 1) / kChunk;
     const TrackSoA &t = w.trk[p];
+    EMX_TL(w, 1, 0, 1);
     for (int ch = blockIdx.x; ch * kChunk < top; ch += gridDim.x) {  // grid-stride over 128-slot chunks
         const int base = ch * kChunk;
         if (ch < nch_old && base + kChunk <= pl.n_old) {  // chunk inside the old range: skip it if nothing died
@@ -375,6 +405,7 @@ __global__ void __launch_bounds__(kChunk) k_fill(Work w, int32_t *dbg_src) {
             else load_record(w.q[p], r, t, i);
         }
     }
+    EMX_TL(w, 1, 1, 1);
 }
 
 // A9: tail compaction when the stack ran dry: live tracks at or above n_new move into the holes below it
@@ -384,7 +415,11 @@ __global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
     const Ctl *c = w.ctl;
     if (c->done) return;
     const PoolPlan pl = c->plan[p];
-    if (pl.h == pl.a) return;  // nothing to compact
+    EMX_TL(w, 2, 0, 1);
+    if (pl.h == pl.a) {  // nothing to compact
+        EMX_TL(w, 2, 1, 1);
+        return;
+    }
     const TrackSoA &t = w.trk[p];
     // grid-stride over the chunks that overlap the tail [n_new, n_old)
     for (int ch = pl.n_new / kChunk + blockIdx.x; ch * kChunk < pl.n_old; ch += gridDim.x) {
@@ -401,6 +436,7 @@ __global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
             else move_slot(t, i, dest);
         }
     }
+    EMX_TL(w, 2, 1, 1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -679,32 +715,37 @@ __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uin
     StepOut o;
     int vol0 = 0;
     uint32_t step0 = 0;
-    const double E0 = active ? ts.E[i] : 0.0;
-    const bool tomb = active && E0 < 0.0;  // tombstone record: retire the slot without stepping
-    const int pend_in = (active && !tomb) ? (int)ts.pend[i] - 1 : -1;  // interaction still waiting (stalled)
-    int pend = -1;
-    if (active && !tomb && pend_in < 0) {
+    // every field of the slot is loaded up front, whether or not the lane turns out to need it (tombstone, stalled
+    // interaction, no propagation in progress): one round trip to L2 instead of a chain of four dependent ones
+    double E0 = 0.0;
+    uint8_t pend_b = 0;
+    FieldState fs;
+    fs.s_done = fs.h = 0.0;
+    fs.attempt = 0;
+    if (active) {
+        E0 = ts.E[i];
+        pend_b = ts.pend[i];
         t.x = {ts.x[i], ts.y[i], ts.z[i]};
         t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
-        t.E = E0;
         t.tid = ts.tid[i];
         t.prim = ts.prim[i];
         t.step = ts.step[i];
         t.vol = ts.vol[i];
         t.surf = ts.surf[i];
+        if (PT != kGamma) {
+            fs.attempt = ts.fs_a[i];
+            fs.s_done = ts.fs_s[i];
+            fs.h = ts.fs_h[i];
+        }
+    }
+    const bool tomb = active && E0 < 0.0;  // tombstone record: retire the slot without stepping
+    const int pend_in = (active && !tomb) ? (int)pend_b - 1 : -1;  // interaction still waiting (stalled)
+    int pend = -1;
+    if (active && !tomb && pend_in < 0) {
+        t.E = E0;
         t.alive = 1;
         vol0 = t.vol;
         step0 = t.step;
-        FieldState fs;
-        fs.s_done = fs.h = 0.0;
-        fs.attempt = 0;
-        if (PT != kGamma) {
-            fs.attempt = ts.fs_a[i];
-            if (fs.attempt > 0) {
-                fs.s_done = ts.fs_s[i];
-                fs.h = ts.fs_h[i];
-            }
-        }
         pend = step_pre<PT>(P, seed, t, o, fs, budget);
 #if defined(EMX_ONE_PHASE)
         if (pend >= 0) {
@@ -814,6 +855,7 @@ __global__ void __launch_bounds__(kStepBlock, kStepWarpsPerSM * 32 / kStepBlock)
     const int nl = c->m_step[PT];
     const int total = (nl + 31) >> 5;
     const int budget = c->field_budget;
+    EMX_TL(w, 3 + PT, 0, 1);
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
@@ -837,6 +879,7 @@ __global__ void __launch_bounds__(kStepBlock, kStepWarpsPerSM * 32 / kStepBlock)
         if (lane <= 16) atomicAdd(dst, acc.n);
         if (lane == 17) atomicAdd(&c->lanes[0][PT], acc.n);
     }
+    EMX_TL(w, 3 + PT, 1, 1);
     if (acc.d != 0.0 && lane < 4) {
         double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
         atomicAdd(dst, acc.d);
@@ -869,6 +912,7 @@ __global__ void __launch_bounds__(kStepBlock, EMX_WARPS_B * 32 / kStepBlock) k_i
 #pragma unroll
     for (int k = 0; k < 3; ++k) cb[k + 1] = cb[k] + ((n[k] + 31) >> 5);
     const int total = cb[3];
+    EMX_TL(w, 6 + PT, 0, 1);
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
@@ -895,15 +939,27 @@ __global__ void __launch_bounds__(kStepBlock, EMX_WARPS_B * 32 / kStepBlock) k_i
         if (lane <= 16) atomicAdd(dst, acc.n);
         if (lane == 17) atomicAdd(&c->lanes[1][PT], acc.n);
     }
+    EMX_TL(w, 6 + PT, 1, 1);
     if (acc.d != 0.0 && lane < 4) {
         double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
         atomicAdd(dst, acc.d);
     }
 }
 
+#ifdef EMX_TIMELINE
+extern "C" int emx_debug_timeline(unsigned long long *host, int clear) {
+    if (clear) {
+        void *a = nullptr;
+        cudaGetSymbolAddress(&a, g_tl);
+        return (int)cudaMemset(a, 0, sizeof(g_tl));
+    }
+    return (int)cudaMemcpyFromSymbol(host, g_tl, sizeof(g_tl));
+}
+#endif
+
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
+    k_plan<<<1, kPlanThreads, 0, st>>>(w, pr);
     const dim3 g3(kRefillBlocks, 3);
-    k_plan<<<1, 1024, 0, st>>>(w, pr);
     k_fill<<<g3, kChunk, 0, st>>>(w, nullptr);
     k_move<<<g3, kChunk, 0, st>>>(w, nullptr);
     return cudaGetLastError();
@@ -911,6 +967,12 @@ cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
 
 cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                              cudaStream_t st);
+
+// blocks of a pool's persistent step kernels: warps_per_sm warps per SM, which pull chunks until the pool is done
+static int step_grid(const Work &w, int pt, int n_sm) {
+    return n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM) * 32 / kStepBlock;
+}
+
 cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st) {
     for (int pt = 2; pt >= 0; --pt) {
         const cudaError_t e = launch_step_pool(pt, P, w, seed, tally, n_sm, st);
@@ -922,7 +984,7 @@ cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *t
 // one phase of one pool (profiling path: every kernel bracketed by events)
 cudaError_t launch_phase(int pt, int phase, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                          cudaStream_t st) {
-    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM) * 32 / kStepBlock;
+    const int g = step_grid(w, pt, n_sm);
     if (phase == 0) {
         if (pt == kGamma) k_step_pool<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
         else if (pt == kElectron) k_step_pool<kElectron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
@@ -940,7 +1002,7 @@ cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t se
                              cudaStream_t st) {
     // persistent single-warp blocks per SM for this pool: the three pools' kernels run side by side, so each
     // gets a share of the 16 warps per SM that fit
-    const int g = n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM) * 32 / kStepBlock;
+    const int g = step_grid(w, pt, n_sm);
     if (pt == kGamma) {
         k_step_pool<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
         k_interact<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
