@@ -138,9 +138,11 @@ typedef struct {
     int rest;                    /* 1 if an e+ annihilated at rest in this step */
 } emo_step_result;
 
+#define EMO_NHIST 96
 typedef struct {
     double escaped, below_cut, looper, E_in;
     uint64_t steps[3], tracks[3], inter[EMO_NPROC], null_int, track_steps;
+    uint64_t step_hist[3][EMO_NHIST];   /* tracks by particle type and by emo_step_bin(steps the track took) */
 } emo_scalars;
 
 /* ---- philox.c ---- */
@@ -213,6 +215,11 @@ int emo_step_batch(const emo_problem *p, uint64_t seed, long n, const emo_track 
  * [edep_total, escaped, looper, below_cut, E_in, steps_g, steps_em, steps_ep, trk_g, trk_em, trk_ep]
  * (11 doubles); per_prim_tally (optional) receives n_prim*n_tally doubles. */
 #define EMO_PER_PRIM 11
+/* Steps-per-track histogram ("steps per track ... by particle type", one of the paper's two
+ * verification observables).  Bin of a track that took n >= 1 steps: n itself below 16, then four bins per
+ * octave: 16 + 4 (e - 4) + (the two bits of n below its leading bit), e = floor(log2 n); the last bin
+ * collects everything beyond. */
+int emo_step_bin(uint64_t n);
 int emo_transport(const emo_problem *p, long n_prim, const int *ptype, const double *E,
                   const double *pos3, const double *dir3, const int *start_vol, const int *start_surf,
                   uint64_t seed, int n_threads, double *edep, emo_scalars *sc,

@@ -11,7 +11,7 @@ import numpy as np
 
 from . import build as _build
 
-MAX_ELEM, MAX_FACES, NPROC, PER_PRIM = 4, 8, 8, 11
+MAX_ELEM, MAX_FACES, NPROC, PER_PRIM, NHIST = 4, 8, 8, 11, 96
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
            "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3"]
 T = {n: i for i, n in enumerate(T_NAMES)}
@@ -45,7 +45,7 @@ class Rng(C.Structure):
 class Scalars(C.Structure):
     _fields_ = [("escaped", C.c_double), ("below_cut", C.c_double), ("looper", C.c_double), ("E_in", C.c_double),
                 ("steps", C.c_uint64 * 3), ("tracks", C.c_uint64 * 3), ("inter", C.c_uint64 * NPROC),
-                ("null_int", C.c_uint64), ("track_steps", C.c_uint64)]
+                ("null_int", C.c_uint64), ("track_steps", C.c_uint64), ("step_hist", (C.c_uint64 * NHIST) * 3)]
 
 
 _lib = None
@@ -89,6 +89,7 @@ def lib():
             "emo_bhabha": (i, [C.POINTER(Rng), d, d, dp, dp, dp, dp, dp]),
             "emo_annih_flight": (None, [C.POINTER(Rng), d, dp, dp, dp, dp, dp]),
             "emo_annih_rest": (None, [C.POINTER(Rng), dp, dp]),
+            "emo_step_bin": (i, [C.c_uint64]),
             "emo_step_batch": (i, [p, C.c_uint64, C.c_long, C.POINTER(Track), C.POINTER(StepResult)]),
             "emo_transport": (i, [p, C.c_long, ip, dp, dp, dp, ip, ip, C.c_uint64, i, dp, C.POINTER(Scalars), dp, dp]),
         }
@@ -214,7 +215,8 @@ class Problem:
         res = dict(edep=edep[:self.n_tally], escaped=sc.escaped, below_cut=sc.below_cut, looper=sc.looper,
                    E_in=sc.E_in, steps=np.array(sc.steps[:], dtype=np.uint64),
                    tracks=np.array(sc.tracks[:], dtype=np.uint64), inter=np.array(sc.inter[:], dtype=np.uint64),
-                   null_int=int(sc.null_int), track_steps=int(sc.track_steps))
+                   null_int=int(sc.null_int), track_steps=int(sc.track_steps),
+                   step_hist=np.array([list(sc.step_hist[k]) for k in range(3)], dtype=np.uint64))
         if per_primary:
             res["per_prim"] = pp
             res["per_prim_tally"] = ppt[:, :self.n_tally]

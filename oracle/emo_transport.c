@@ -245,6 +245,17 @@ int emo_step_batch(const emo_problem *p, uint64_t seed, long n, const emo_track 
     return 0;
 }
 
+int emo_step_bin(uint64_t n) {
+    int b;
+    if (n < 16) b = (int)n;
+    else {
+        int e = 0;
+        while ((n >> e) > 1) ++e;                        /* e = floor(log2 n) >= 4 */
+        b = 16 + 4 * (e - 4) + (int)((n >> (e - 2)) & 3);
+    }
+    return b < EMO_NHIST ? b : EMO_NHIST - 1;
+}
+
 typedef struct { emo_track *v; size_t n, cap; } stack_t;
 static int push(stack_t *s, const emo_track *t) {
     if (s->n == s->cap) {
@@ -292,8 +303,10 @@ int emo_transport(const emo_problem *p, long n_prim, const int *ptype, const dou
             ls.tracks[t0.ptype]++; ptr[t0.ptype] += 1.0;
             while (st.n > 0) {
                 emo_track t = st.v[--st.n];
+                uint64_t taken = 0;                       /* steps of this track */
                 while (t.alive) {
                     emo_step(p, seed, &t, r);
+                    ++taken;
                     ls.steps[t.ptype]++; ls.track_steps++; pst[t.ptype] += 1.0;
                     if (r->edep != 0.0) {
                         int tl = p->vol[r->edep_vol].tally;
@@ -309,6 +322,7 @@ int emo_transport(const emo_problem *p, long n_prim, const int *ptype, const dou
                     }
                     t = r->trk;
                 }
+                ls.step_hist[t.ptype][emo_step_bin(taken)]++;
             }
             for (int i = 0; i < nt; ++i) led[i] += ped[i];
             ls.below_cut += pe_bc; ls.escaped += pe_esc; ls.looper += pe_loop; ls.E_in += Ein;
@@ -326,6 +340,8 @@ int emo_transport(const emo_problem *p, long n_prim, const int *ptype, const dou
             for (int i = 0; i < 3; ++i) { sc->steps[i] += ls.steps[i]; sc->tracks[i] += ls.tracks[i]; }
             for (int i = 0; i < EMO_NPROC; ++i) sc->inter[i] += ls.inter[i];
             sc->null_int += ls.null_int; sc->track_steps += ls.track_steps;
+            for (int i = 0; i < 3; ++i)
+                for (int b = 0; b < EMO_NHIST; ++b) sc->step_hist[i][b] += ls.step_hist[i][b];
         }
         free(st.v); free(led); free(ped); free(r);
     }

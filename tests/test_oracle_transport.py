@@ -230,6 +230,35 @@ def test_config0_energy_sum_first_collision_and_step_count(emo):
     assert np.median(depth) == pytest.approx(mfp * math.log(2), rel=0.12)
 
 
+def test_step_bin_edges_by_brute_force(emo):
+    """emo_step_bin against its definition written out with floats and a table: identity below 16, four equal
+    sub-bins per octave above, monotone, every bin non-empty up to the overflow bin."""
+    L = emo.lib()
+    bins = np.array([L.emo_step_bin(n) for n in range(1, 1 << 15)])
+    assert bins[:15].tolist() == list(range(1, 16))
+    assert np.all(np.diff(bins) >= 0) and np.all(np.diff(bins) <= 1)
+    for n in (16, 19, 20, 31, 32, 39, 40, 1000, 1023, 1024, 20000):
+        e = int(math.floor(math.log2(n)))
+        assert L.emo_step_bin(n) == 16 + 4 * (e - 4) + int((n - 2 ** e) / 2 ** (e - 2))
+    # widths: octave e is cut into four bins of 2^(e-2) values each
+    assert [int((bins == b).sum()) for b in range(16, 28)] == [4] * 4 + [8] * 4 + [16] * 4
+    assert L.emo_step_bin(1 << 40) == emo.NHIST - 1 and L.emo_step_bin(0) == 0
+
+
+def test_steps_per_track_histogram_config0(emo):
+    """Config 0 has one track per primary (photons only, electrons deposited at creation), so the histogram
+    of steps per track must be the histogram of the per-primary step counts, which come from another counter."""
+    desc, prim = W.config0()
+    P = emo.Problem(desc)
+    r = P.transport(prim, desc["seed"], n_threads=2, per_primary=True)
+    per_primary = r["per_prim"][:, 5].astype(np.int64)
+    assert per_primary.max() < 16                                          # identity bins: n itself
+    want = np.bincount(per_primary, minlength=emo.NHIST)
+    assert np.array_equal(r["step_hist"][0], want.astype(np.uint64))
+    assert r["step_hist"][1:].sum() == 0
+    assert int((np.arange(emo.NHIST) * r["step_hist"][0]).sum()) == int(r["steps"][0])
+
+
 @pytest.mark.parametrize("cfg,n", [(1, 40), (2, 6), (3, 6), (4, 24), (5, 60)])
 def test_energy_closure_per_event(emo, cfg, n):
     desc, prim = W.get(cfg, n)
@@ -242,6 +271,12 @@ def test_energy_closure_per_event(emo, cfg, n):
     assert np.allclose(r["per_prim_tally"].sum(0), r["edep"], rtol=1e-12)
     assert r["track_steps"] == int(r["steps"].sum()) == int(pp[:, 5:8].sum())
     assert r["tracks"].tolist() == pp[:, 8:11].sum(0).astype(int).tolist()
+    # steps-per-track histogram: one entry per track; the mean steps per track lies inside the bins' bounds
+    assert r["step_hist"].sum(1).tolist() == r["tracks"].tolist()
+    lo = np.array([b if b < 16 else (4 + (b - 16) % 4) << ((b - 16) // 4 + 2) for b in range(emo.NHIST)], dtype=np.float64)
+    hi = np.array([lo[b + 1] - 1 if b + 1 < emo.NHIST else np.inf for b in range(emo.NHIST)])
+    for k in range(3):
+        assert (lo * r["step_hist"][k]).sum() <= r["steps"][k] <= (np.where(r["step_hist"][k] > 0, hi, 0) * r["step_hist"][k]).sum()
     # every e+ ends by annihilation (in flight or at rest) unless it escaped or looped
     if r["escaped"] == 0 and r["looper"] == 0:
         assert r["tracks"][2] == r["inter"][6] + r["inter"][7]
