@@ -72,6 +72,12 @@ extern "C" {
 #define EMX_P_REST 7 /* e+ annihilation at rest */
 #define EMX_NPROC 8
 
+/* Steps-per-track histogram ("steps per track ... by particle type", one of the two observables
+ * of the paper's verification problem).  A track that took n >= 1 steps falls into bin n below 16; above, every
+ * octave has four equal bins: 16 + 4 (e - 4) + (the two bits of n below its leading bit), e = floor(log2 n);
+ * the last bin collects everything beyond. */
+#define EMX_NHIST 96
+
 /* what limited the step */
 #define EMX_A_NONE 0
 #define EMX_A_DISCRETE 1
@@ -223,6 +229,11 @@ int emx_reset_tallies(emx_problem *p, void *stream);
 
 /* edep_host[n_tally] (MeV per tally id) and the run totals, copied to HOST memory. */
 int emx_read_tallies(const emx_problem *p, double *edep_host, emx_scalars *out);
+
+/* hist_host[3 * EMX_NHIST] (HOST memory): tracks of the last transport by particle type (gamma, e-, e+) and by
+ * the bin of the number of steps they took before they ended (absorbed, below the tracking cut, escaped,
+ * looper).  Sums to scalars.tracks[] per type.  EMX_E_STATE before the first transport. */
+int emx_read_step_hist(const emx_problem *p, uint64_t *hist_host);
 
 /* Milliseconds the last emx_transport spent between its first launch and the end of the loop,
  * measured with CUDA events on the caller's stream; < 0 if none. */

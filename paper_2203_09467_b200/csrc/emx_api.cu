@@ -630,6 +630,15 @@ int emx_get_lanes(const emx_problem *p, uint64_t *lanes6) {
     return EMX_OK;
 }
 
+int emx_read_step_hist(const emx_problem *cp, uint64_t *hist_host) {
+    emx_problem *p = const_cast<emx_problem *>(cp);
+    if (!p || !hist_host) return fail(p, EMX_E_ARG, "emx_read_step_hist: null argument");
+    if (!p->have_ctl) return fail(p, EMX_E_STATE, "emx_read_step_hist: no transport yet");
+    for (int pt = 0; pt < 3; ++pt)
+        for (int b = 0; b < EMX_NHIST; ++b) hist_host[pt * EMX_NHIST + b] = p->last_ctl.hist[pt][b];
+    return EMX_OK;
+}
+
 long emx_get_iteration_times(const emx_problem *p, float *host_out, long max_iter) {
     if (!p || !host_out || max_iter < 0) return EMX_E_ARG;
     long n = (long)(p->iter_ms.size() / 2);

@@ -525,6 +525,16 @@ __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, i
     return __shfl_sync(0xffffffffu, r0, 0);
 }
 
+// bin of the steps-per-track histogram (include/emx.h: EMX_NHIST)
+__device__ __forceinline__ int step_bin(uint32_t n) {
+    int b = (int)n;
+    if (n >= 16u) {
+        const int e = 31 - __clz(n);
+        b = 16 + 4 * (e - 4) + (int)((n >> (e - 2)) & 3u);
+    }
+    return b < EMX_NHIST ? b : EMX_NHIST - 1;
+}
+
 // index of process `proc` among the processes of particle type PT (the order of C7.8), and back
 template <int PT>
 __device__ __forceinline__ int proc_slot(int proc) {
@@ -637,6 +647,17 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     }
     const bool died = active && (tomb || (commit && !t.alive));
     if (active) ts.alive[i] = (uint8_t)(died ? 0 : 1);
+    // steps-per-track histogram: a track that ends here took step0 + 1 steps; lanes with the same bin share
+    // one atomic (most tracks end after a few steps: per-lane atomics on those few bins cost 70 % more time)
+    {
+        const bool ended = died && !tomb;
+        const unsigned be = __ballot_sync(0xffffffffu, ended);
+        if (ended) {
+            const int hb = step_bin(step0 + 1u);
+            const unsigned m = __match_any_sync(be, hb);
+            if (lane == __ffs(m) - 1) atomicAdd(&c->hist[PT][hb], (unsigned long long)__popc(m));
+        }
+    }
     // dead slots per 128-slot chunk, for the refill plan (A9)
     if (CONSEC) {  // the warp's lanes are 32 consecutive slots of one chunk
         const unsigned bd = __ballot_sync(0xffffffffu, died);

@@ -62,6 +62,7 @@ struct Ctl {
     double escaped, below_cut, looper, E_in;
     unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls, peak_live, peak_queue;
     unsigned long long lanes[2][3];  // track slots processed by phase A / phase B kernels, per pool
+    unsigned long long hist[3][EMX_NHIST];  // tracks by type and by the bin of the steps they took
 };
 
 struct Work {

@@ -172,9 +172,16 @@ def test_transport_parity_and_energy_closure(emx, emo, cfg, n, n_slots):
         assert np.all(np.abs(a - b) <= 1e-3 * np.maximum(a, 1.0) + 3.0), (k, o[k], g[k])
     assert g["track_steps"] == int(g["steps"].sum())
     assert g["stalls"] == 0
+    # steps-per-track histogram: one entry per track; bins within 3 sigma (Poisson) and 1e-3
+    hg, ho = G.read_step_hist(), o["step_hist"]
+    assert hg.sum(1).tolist() == g["tracks"].tolist()
+    a, b = ho.astype(np.float64), hg.astype(np.float64)
+    assert np.all(np.abs(a - b) <= 1e-3 * a + 3.0 * np.sqrt(np.maximum(a, 1.0)) * (a != b)), (ho, hg)
     if cfg == 0:
         assert g["edep"][0] == pytest.approx(1000 * 10.0, rel=1e-12)
         assert np.array_equal(g["steps"], o["steps"]) and np.array_equal(g["inter"], o["inter"])
+    if np.array_equal(g["steps"], o["steps"]) and np.array_equal(g["tracks"], o["tracks"]):
+        assert np.array_equal(hg, ho)                  # same histories step for step: the same histogram
 
 
 def test_full_stack_stalls_do_not_change_the_physics(emx, emo):
@@ -189,6 +196,9 @@ def test_full_stack_stalls_do_not_change_the_physics(emx, emo):
     assert np.array_equal(a["tracks"], b["tracks"])
     assert b["edep"].sum() == pytest.approx(a["edep"].sum(), rel=1e-12)
     assert b["peak_queue"] <= 6000 * 1.01 + 384
+    hb = G.read_step_hist()
+    G.transport(pd, desc["seed"], n_slots=4096, queue_capacity=1 << 20)
+    assert np.array_equal(hb, G.read_step_hist())      # stalled steps are not counted twice
 
 
 def test_results_do_not_depend_on_slots_or_host_entry(emx):
@@ -210,6 +220,9 @@ def test_error_paths(emx):
     assert L.emx_build_tables(h, None) == -2           # no volume
     assert b"volume" in L.emx_last_error(h)
     assert L.emx_transport(h, 0, None, None, None, None, None, None, 0, 10, 10, None, 0, None) == -2
+    hist = (C.c_uint64 * (3 * emx.NHIST))()
+    assert L.emx_read_step_hist(h, C.cast(hist, C.c_void_p)) == -2      # no transport yet
+    assert L.emx_read_step_hist(h, None) == -1
     L.emx_destroy(h)
 
 
@@ -217,13 +230,15 @@ def test_scheduling_knobs_do_not_change_results(emx, monkeypatch):
     """Time slicing of the field propagation (substep budget per iteration) and the graph / stream launch
     paths only change WHEN work is done: counters are equal, tallies equal up to summation order."""
     desc, prim = W.get(4, 64)
-    runs = []
+    runs, hists = [], []
     for budget, mode in (("2", 0), ("100000", 0), ("7", 2), ("2", 1)):
         monkeypatch.setenv("EMX_SLICE_BUDGET", budget)
         monkeypatch.setenv("EMX_SLICE_ABOVE", "0")
         G = emx.Problem(desc)
         G.set_profile(mode)
         runs.append(G.transport(G.upload_primaries(prim), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 20))
+        hists.append(G.read_step_hist())
+    assert all(np.array_equal(hists[0], h) for h in hists[1:])
     a = runs[0]
     for b in runs[1:]:
         for k in ("steps", "tracks", "inter"):
@@ -253,3 +268,6 @@ def test_full_size_bench_configuration(emx, emo):
     big = o["edep"] > 1e-6 * o["E_in"]
     assert np.all(np.abs(g["edep"][big] - o["edep"][big]) <= 1e-6 * o["edep"][big])
     assert g["escaped"] == pytest.approx(o["escaped"], rel=1e-6)
+    hg, ho = G.read_step_hist().astype(np.float64), o["step_hist"].astype(np.float64)
+    assert hg.sum(1).tolist() == g["tracks"].astype(np.float64).tolist()
+    assert np.all(np.abs(hg - ho) <= 1e-5 * ho + 5.0), np.abs(hg - ho).max()
