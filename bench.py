@@ -32,8 +32,11 @@ METRIC, UNIT = "track_steps_per_sec", "track-steps/s"
 B_STEP, B_SEC = 80 + 69, 76
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the committed `ncu --set full` capture
 # of a saturated iteration (profiles/r1_final_step_kernels_full.md)
-TRAFFIC_PER_LAUNCH = {"k_step_pool<gamma>": 23.8e6, "k_step_pool<e->": 37.9e6, "k_step_pool<e+>": 7.3e6,
-                      "k_interact<gamma>": 27.2e6, "k_interact<e->": 27.3e6, "k_interact<e+>": 6.7e6}
+TRAFFIC_PER_LAUNCH = {"k_step_pool<gamma>": 23.6e6, "k_step_pool<e->": 44.8e6, "k_step_pool<e+>": 8.6e6,
+                      "k_interact<gamma>": 26.9e6, "k_interact<e->": 26.6e6, "k_interact<e+>": 6.7e6}
+# sm__inst_executed_pipe_fp64 (fraction of peak) of the same capture: how far the kernels are from the fp64 ALU roof
+FP64_PIPE_NCU = {"k_step_pool<gamma>": 0.146, "k_step_pool<e->": 0.258, "k_step_pool<e+>": 0.114,
+                 "k_interact<gamma>": 0.136, "k_interact<e->": 0.094, "k_interact<e+>": 0.070}
 
 
 def parse():
@@ -263,6 +266,7 @@ def run_ours(args):
     n_launch = max(rp["iterations"], 1)
     roof = {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
             "traffic": TRAFFIC_PER_LAUNCH.get(names[dom]),
+            "fp64_pipe_frac_ncu": FP64_PIPE_NCU.get(names[dom]),
             "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s",
             "algorithmic_bytes_per_launch": alg_bytes / n_launch, "avg_launch_ms": kms[dom] / n_launch,
             "kernel_ms_profiled_pass": dict(zip(names + ["refill", "all_step_kernels"], [float(v) for v in kms])),
