@@ -684,9 +684,22 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     {
         const double e0 = commit ? o.escaped : 0.0, e1 = commit ? o.below_cut : 0.0, e2 = commit ? o.looper : 0.0,
                      e3 = commit ? o.edep : 0.0;
-        if (__ballot_sync(0xffffffffu, e0 != 0.0 || e1 != 0.0 || e2 != 0.0 || e3 != 0.0)) {
-            const double s0 = warp_sum(e0), s1 = warp_sum(e1), s2 = warp_sum(e2), s3 = warp_sum(e3);
-            acc.d += (lane == 0) ? s0 : (lane == 1) ? s1 : (lane == 2) ? s2 : (lane == 3) ? s3 : 0.0;
+        // escapes, cut kills and loopers are rare: a warp reduction only for the totals that have something to add
+        if (__ballot_sync(0xffffffffu, e0 != 0.0)) {
+            const double s0 = warp_sum(e0);
+            if (lane == 0) acc.d += s0;
+        }
+        if (__ballot_sync(0xffffffffu, e1 != 0.0)) {
+            const double s1 = warp_sum(e1);
+            if (lane == 1) acc.d += s1;
+        }
+        if (__ballot_sync(0xffffffffu, e2 != 0.0)) {
+            const double s2 = warp_sum(e2);
+            if (lane == 2) acc.d += s2;
+        }
+        if (__ballot_sync(0xffffffffu, e3 != 0.0)) {
+            const double s3 = warp_sum(e3);
+            if (lane == 3) acc.d += s3;
         }
         const int proc = (commit && o.process >= 0) ? (o.null_int ? 8 : o.process) : -1;
         unsigned add = 0;
