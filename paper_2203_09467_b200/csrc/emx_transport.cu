@@ -819,26 +819,27 @@ __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uin
     const bool parked = active && !tomb && (PT != kGamma) && o.suspended;
     const bool waiting = pend_in >= 0;  // nothing to do in this phase
 
+    // file the lanes with a pending interaction (new or stalled) in the list of their process.  The three list
+    // counters of a pool are packed into one 64-bit word (21 bits each; pools hold fewer than 2^21 slots, checked
+    // by the host), so one atomic per warp reserves the entries of all three lists.  It is issued BEFORE the
+    // epilogue and its result is used after it: the round trip to L2 runs under the epilogue's work.
+    const int pk = waiting ? proc_slot<PT>(pend_in) : (pend >= 0 && !parked ? proc_slot<PT>(pend) : -1);
+    const unsigned b0 = __ballot_sync(0xffffffffu, pk == 0);
+    const unsigned b1 = __ballot_sync(0xffffffffu, pk == 1);
+    const unsigned b2 = __ballot_sync(0xffffffffu, pk == 2);
+    unsigned long long lbase = 0ull;
+    if ((b0 | b1 | b2) && lane == 0)
+        lbase = atomicAdd(&c->icount64[PT], (unsigned long long)__popc(b0) | ((unsigned long long)__popc(b1) << 21) |
+                                               ((unsigned long long)__popc(b2) << 42));
+
     WarpAcc acc = epilogue<PT, true>(P, w, seed, tally, i, active && !waiting, tomb, parked, pend, t, o, vol0, step0);
-    // file the lanes with a pending interaction (new or stalled) in the list of their process
-    {
-        const int pk = waiting ? proc_slot<PT>(pend_in) : (pend >= 0 && !parked ? proc_slot<PT>(pend) : -1);
-        // the three list counters of a pool are packed into one 64-bit word (21 bits each; pools hold fewer than
-        // 2^21 slots, checked by the host), so one atomic per warp reserves the entries of all three lists
-        const unsigned b0 = __ballot_sync(0xffffffffu, pk == 0);
-        const unsigned b1 = __ballot_sync(0xffffffffu, pk == 1);
-        const unsigned b2 = __ballot_sync(0xffffffffu, pk == 2);
-        if (b0 | b1 | b2) {
-            unsigned long long base = 0ull;
-            if (lane == 0)
-                base = atomicAdd(&c->icount64[PT], (unsigned long long)__popc(b0) | ((unsigned long long)__popc(b1) << 21) |
-                                                       ((unsigned long long)__popc(b2) << 42));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            if (pk >= 0) {
-                const unsigned bk = pk == 0 ? b0 : (pk == 1 ? b1 : b2);
-                const int r0 = (int)((base >> (21 * pk)) & 0x1fffffull);
-                w.ilist[PT][pk][r0 + __popc(bk & lt)] = i;
-            }
+
+    if (b0 | b1 | b2) {
+        lbase = __shfl_sync(0xffffffffu, lbase, 0);
+        if (pk >= 0) {
+            const unsigned bk = pk == 0 ? b0 : (pk == 1 ? b1 : b2);
+            const int r0 = (int)((lbase >> (21 * pk)) & 0x1fffffull);
+            w.ilist[PT][pk][r0 + __popc(bk & lt)] = i;
         }
     }
     return acc;
