@@ -48,6 +48,9 @@ def parse():
     ap.add_argument("--primaries", type=int, default=0, help="0 = the config's full count")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: ONE workload sharded by primaries over the ranks + final all-reduce of the tallies "
+                         "(strong scaling) instead of N replicas (default, weak scaling)")
     return ap.parse_args()
 
 
@@ -176,9 +179,14 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     desc, prim = workload(args)
-    n_prim = len(prim["E"])
-    seed = replica_seed(desc["seed"], rank)
+    sharded = bool(args.shard) and world > 1
+    seed = desc["seed"] if sharded else replica_seed(desc["seed"], rank)
     G = emx.Problem(desc)
+    if sharded:      # contiguous ranges of the primaries, histories as in the unsharded run
+        from paper_2203_09467_b200 import shard
+        first, prim = shard.shard_primaries(prim, rank, world)
+        G.set_primary_offset(first)
+    n_prim = len(prim["E"])
     pdev = G.upload_primaries(prim)
     pinned = {k: torch.from_numpy(np.array(v, order="C")).pin_memory() for k, v in prim.items()}
     phost = {k: v.numpy() for k, v in pinned.items()}
@@ -210,6 +218,8 @@ def run_ours(args):
         tot["sec_type"] += sec
         tot["launches"] += pr["launches"]
         tot["iters"] += r["iterations"]
+        if sharded:  # the one exchange of the job: tallies, totals and counters summed over the ranks
+            shard.all_reduce_results(r, G.read_step_hist(), "cuda")
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
@@ -276,10 +286,11 @@ def run_ours(args):
             "note": "not HBM-bound on B200: the 95 MB track store stays in the 126 MB L2 (traffic < algorithmic "
                     "bytes); the step kernels are latency / divergence bound, see DESIGN.md section 7"}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "f64", "data": "synthetic",
+           "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": desc["name"], "primaries_per_step": n_prim, "n_slots": desc["n_slots"],
-                      "queue_capacity": desc["queue_capacity"], "parallelism": "replicas x%d" % world,
+                      "queue_capacity": desc["queue_capacity"],
+                      "parallelism": ("primaries sharded x%d + final all-reduce" if sharded else "replicas x%d") % world,
                       "l2": "inputs larger than L2: track store + stacks > 126 MB, every step re-reads the stacks"},
            "primaries_per_sec": n_prim * args.steps * world / (ms * 1e-3),
            "iterations_per_step": tot["iters"] / args.steps, "peak_live": last["peak_live"], "peak_queue": last["peak_queue"],

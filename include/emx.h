@@ -227,6 +227,13 @@ int emx_transport_host(emx_problem *p, long n_primaries, const int *ptype, const
 
 int emx_reset_tallies(emx_problem *p, void *stream);
 
+/* Sharding by primaries ("particle events are decomposed across MPI ranks"): the
+ * primaries passed to the following emx_transport calls are the primaries first, first + 1, ... of a longer
+ * list.  A history depends on the seed and on its primary index only, so the tallies and counters of the parts
+ * of a list, transported anywhere in any order with their offsets, sum to those of the whole list.
+ * Default 0.  first + n must stay below 2^32 (EMX_E_ARG otherwise, here or in emx_transport). */
+int emx_set_primary_offset(emx_problem *p, long first);
+
 /* edep_host[n_tally] (MeV per tally id) and the run totals, copied to HOST memory. */
 int emx_read_tallies(const emx_problem *p, double *edep_host, emx_scalars *out);
 

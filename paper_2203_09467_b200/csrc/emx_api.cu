@@ -45,6 +45,7 @@ struct emx_problem {
     // iteration graph: internal streams (the caller's stream may be the legacy stream, which cannot be captured)
     cudaStream_t s0 = nullptr, s1 = nullptr, s2 = nullptr;
     cudaEvent_t evFork = nullptr, evJ1 = nullptr, evJ2 = nullptr, evIn = nullptr, evOut = nullptr;
+    long long prim_first = 0;  // primary index of the first element passed to emx_transport
     bool use_graph = true;
     long slice_above = -1;  // < 0: n_slots / 32
     int slice_budget = 2;
@@ -412,6 +413,7 @@ int emx_reset_tallies(emx_problem *p, void *stream) {
 
 static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, long n_slots, long queue_capacity,
                             void *workspace, size_t workspace_bytes, cudaStream_t st) {
+    if (pr.first + pr.n > 0x100000000LL) return fail(p, EMX_E_ARG, "emx_transport: primary indices beyond 2^32");
     Work w;
     const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog);
     if (need > workspace_bytes) return fail(p, EMX_E_CAPACITY, "emx_transport: workspace smaller than emx_workspace_bytes()");
@@ -539,7 +541,7 @@ int emx_transport(emx_problem *p, long n, const int *ptype, const double *E, con
     if (!p || !p->hp.built) return fail(p, EMX_E_STATE, "emx_transport: tables not built");
     if (n < 0 || (n > 0 && (!ptype || !E || !pos3 || !dir3 || !start_vol)) || !workspace || n_slots < 1 || queue_capacity < 1)
         return fail(p, EMX_E_ARG, "emx_transport: invalid argument");
-    Primaries pr{n, ptype, E, pos3, dir3, start_vol, start_surf};
+    Primaries pr{n, ptype, E, pos3, dir3, start_vol, start_surf, p->prim_first};
     return transport_device(p, pr, seed, n_slots, queue_capacity, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
@@ -571,11 +573,18 @@ int emx_transport_host(emx_problem *p, long n, const int *ptype, const double *E
     int rc;
     if (e != cudaSuccess) rc = fail_cuda(p, e, "emx_transport_host: upload");
     else {
-        Primaries pr{n, d_pt, d_E, d_pos, d_dir, d_vol, start_surf ? d_surf : nullptr};
+        Primaries pr{n, d_pt, d_E, d_pos, d_dir, d_vol, start_surf ? d_surf : nullptr, p->prim_first};
         rc = transport_device(p, pr, seed, n_slots, queue_capacity, workspace, workspace_bytes, st);
     }
     cudaFree(d);
     return rc;
+}
+
+int emx_set_primary_offset(emx_problem *p, long first) {
+    if (!p) return fail(p, EMX_E_ARG, "emx_set_primary_offset: null problem");
+    if (first < 0 || first > 0xffffffffL) return fail(p, EMX_E_ARG, "emx_set_primary_offset: offset outside [0, 2^32)");
+    p->prim_first = first;
+    return EMX_OK;
 }
 
 int emx_read_tallies(const emx_problem *cp, double *edep_host, emx_scalars *out) {

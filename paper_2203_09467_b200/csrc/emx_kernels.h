@@ -21,6 +21,7 @@ struct Primaries {
     const int *ptype;
     const double *E, *pos3, *dir3;
     const int *vol, *surf;  // surf may be null
+    long long first;        // primary index of element 0 (emx_set_primary_offset): element i is primary first + i
 };
 
 // resets the control block, totals the injected energy

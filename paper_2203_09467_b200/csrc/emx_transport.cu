@@ -206,7 +206,7 @@ __device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) 
             q.uz[r] = pr.dir3[3 * i + 2];
             q.E[r] = pr.E[i];
             q.tid[r] = 0ull;
-            q.prim[r] = (uint32_t)i;
+            q.prim[r] = (uint32_t)(pr.first + i);
             q.vol[r] = pr.vol[i];
             q.surf[r] = pr.surf ? pr.surf[i] : -1;
         }

@@ -211,6 +211,36 @@ def test_results_do_not_depend_on_slots_or_host_entry(emx):
     assert a["iterations"] != b["iterations"] or a["peak_live"] != b["peak_live"]
 
 
+def test_shards_of_the_primaries_sum_to_the_whole(emx):
+    """the primaries cut into contiguous parts, each transported with its offset (here one after
+    the other on one GPU, as the ranks of a sharded job would), give the counters of the whole list exactly and
+    its tallies up to summation order."""
+    from paper_2203_09467_b200 import shard
+    desc, prim = W.get(3, 16)
+    G = emx.Problem(desc)
+    whole = G.transport(G.upload_primaries(prim), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 20)
+    h_whole = G.read_step_hist()
+    parts, hists = [], []
+    for rank in range(3):
+        first, sub = shard.shard_primaries(prim, rank, 3)
+        G.set_primary_offset(first)
+        parts.append(G.transport(G.upload_primaries(sub), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 20))
+        hists.append(G.read_step_hist())
+    G.set_primary_offset(0)
+    for k in ("steps", "tracks", "inter"):
+        assert np.array_equal(sum(p[k].astype(np.int64) for p in parts), whole[k].astype(np.int64)), k
+    assert sum(p["null_int"] for p in parts) == whole["null_int"]
+    assert np.array_equal(sum(h.astype(np.int64) for h in hists), h_whole.astype(np.int64))
+    assert np.allclose(sum(p["edep"] for p in parts), whole["edep"], rtol=1e-11, atol=1e-9)
+    assert sum(p["E_in"] for p in parts) == pytest.approx(whole["E_in"], rel=1e-14)
+    # without the offsets the parts are different histories
+    first, sub = shard.shard_primaries(prim, 2, 3)
+    other = G.transport(G.upload_primaries(sub), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 20)
+    assert not np.array_equal(other["steps"], parts[2]["steps"])
+    with pytest.raises(emx.EmxError):
+        G.set_primary_offset(-1)
+
+
 def test_error_paths(emx):
     import ctypes as C
     L = emx.lib()
