@@ -46,6 +46,13 @@ struct emx_problem {
     cudaStream_t s0 = nullptr, s1 = nullptr, s2 = nullptr;
     cudaEvent_t evFork = nullptr, evJ1 = nullptr, evJ2 = nullptr, evIn = nullptr, evOut = nullptr;
     long long prim_first = 0;  // primary index of the first element passed to emx_transport
+    // the instantiated iteration graph is kept for the next emx_transport with the same kernel arguments
+    // (workspace, primaries, seed, tables): capture + instantiation cost about 2 ms
+    cudaGraphExec_t graph_exec = nullptr;
+    Work graph_w;
+    Primaries graph_pr;
+    uint64_t graph_seed = 0;
+    unsigned long long graph_gen = 0, params_gen = 1;
     bool use_graph = true;
     long slice_above = -1;  // < 0: n_slots / 32
     int slice_budget = 2;
@@ -184,6 +191,7 @@ int emx_create(emx_problem **out) {
 void emx_destroy(emx_problem *p) {
     if (!p) return;
     free_device(p);
+    if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
     if (p->h_ctl) cudaFreeHost(p->h_ctl);
     if (p->ev0) cudaEventDestroy(p->ev0);
     if (p->ev1) cudaEventDestroy(p->ev1);
@@ -377,6 +385,7 @@ int emx_build_tables(emx_problem *p, void *stream) {
             CU(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
     }
     hp.built = true;
+    p->params_gen += 1;  // kernel nodes hold Params by value: a kept graph is stale now
     p->have_ctl = false;
     return EMX_OK;
 }
@@ -415,6 +424,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
                             void *workspace, size_t workspace_bytes, cudaStream_t st) {
     if (pr.first + pr.n > 0x100000000LL) return fail(p, EMX_E_ARG, "emx_transport: primary indices beyond 2^32");
     Work w;
+    memset(&w, 0, sizeof(w));  // compared bytewise with the arguments of the kept graph
     const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog);
     if (need > workspace_bytes) return fail(p, EMX_E_CAPACITY, "emx_transport: workspace smaller than emx_workspace_bytes()");
     // admission limits (R8): about 20 MeV of shower energy in flight per queued record at the peak of
@@ -436,30 +446,45 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         // the three step kernels are parallel branches, so the tail of one pool overlaps the start of the next.
         // The host only looks at the done flag between graph launches.
         constexpr int kIterPerGraph = 8;
-        cudaGraph_t graph = nullptr;
-        cudaGraphExec_t exec = nullptr;
         CU(cudaEventRecord(p->evIn, st));
         CU(cudaStreamWaitEvent(p->s0, p->evIn, 0));
-        CU(cudaStreamBeginCapture(p->s0, cudaStreamCaptureModeThreadLocal));
         cudaError_t ce = cudaSuccess;
-        for (int k = 0; k < kIterPerGraph && ce == cudaSuccess; ++k) {
-            ce = launch_refill(w, pr, p->s0);
-            if (ce == cudaSuccess) ce = cudaEventRecord(p->evFork, p->s0);
-            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s1, p->evFork, 0);
-            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s2, p->evFork, 0);
-            if (ce == cudaSuccess) ce = launch_step_pool(kPositron, p->P, w, seed, p->d_tally, p->n_sm, p->s1);
-            if (ce == cudaSuccess) ce = launch_step_pool(kElectron, p->P, w, seed, p->d_tally, p->n_sm, p->s2);
-            if (ce == cudaSuccess) ce = launch_step_pool(kGamma, p->P, w, seed, p->d_tally, p->n_sm, p->s0);
-            if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ1, p->s1);
-            if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ2, p->s2);
-            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ1, 0);
-            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ2, 0);
+        Primaries prz;
+        memset(&prz, 0, sizeof(prz));
+        prz.n = pr.n; prz.ptype = pr.ptype; prz.E = pr.E; prz.pos3 = pr.pos3; prz.dir3 = pr.dir3;
+        prz.vol = pr.vol; prz.surf = pr.surf; prz.first = pr.first;
+        const bool keep = p->graph_exec && p->graph_gen == p->params_gen && p->graph_seed == seed &&
+                          memcmp(&p->graph_w, &w, sizeof(Work)) == 0 && memcmp(&p->graph_pr, &prz, sizeof(Primaries)) == 0;
+        if (!keep) {
+            if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
+            p->graph_exec = nullptr;
+            cudaGraph_t graph = nullptr;
+            CU(cudaStreamBeginCapture(p->s0, cudaStreamCaptureModeThreadLocal));
+            for (int k = 0; k < kIterPerGraph && ce == cudaSuccess; ++k) {
+                ce = launch_refill(w, pr, p->s0);
+                if (ce == cudaSuccess) ce = cudaEventRecord(p->evFork, p->s0);
+                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s1, p->evFork, 0);
+                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s2, p->evFork, 0);
+                if (ce == cudaSuccess) ce = launch_step_pool(kPositron, p->P, w, seed, p->d_tally, p->n_sm, p->s1);
+                if (ce == cudaSuccess) ce = launch_step_pool(kElectron, p->P, w, seed, p->d_tally, p->n_sm, p->s2);
+                if (ce == cudaSuccess) ce = launch_step_pool(kGamma, p->P, w, seed, p->d_tally, p->n_sm, p->s0);
+                if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ1, p->s1);
+                if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ2, p->s2);
+                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ1, 0);
+                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ2, 0);
+            }
+            cudaError_t ce2 = cudaStreamEndCapture(p->s0, &graph);
+            if (ce != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return fail_cuda(p, ce, "emx_transport: graph capture"); }
+            CU(ce2);
+            ce = cudaGraphInstantiate(&p->graph_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (ce != cudaSuccess) { p->graph_exec = nullptr; return fail_cuda(p, ce, "cudaGraphInstantiate"); }
+            p->graph_w = w;
+            p->graph_pr = prz;
+            p->graph_seed = seed;
+            p->graph_gen = p->params_gen;
         }
-        cudaError_t ce2 = cudaStreamEndCapture(p->s0, &graph);
-        if (ce != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return fail_cuda(p, ce, "emx_transport: graph capture"); }
-        CU(ce2);
-        ce = cudaGraphInstantiate(&exec, graph, 0);
-        if (ce != cudaSuccess) { cudaGraphDestroy(graph); return fail_cuda(p, ce, "cudaGraphInstantiate"); }
+        cudaGraphExec_t exec = p->graph_exec;
         int batch = 1;
         for (;;) {
             for (int k = 0; k < batch && ce == cudaSuccess; ++k) ce = cudaGraphLaunch(exec, p->s0);
@@ -470,9 +495,11 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
             if (ce != cudaSuccess || p->h_ctl->done || p->h_ctl->error) break;
             if (batch < 8) batch *= 2;
         }
-        cudaGraphExecDestroy(exec);
-        cudaGraphDestroy(graph);
-        if (ce != cudaSuccess) return fail_cuda(p, ce, "emx_transport: iteration graph");
+        if (ce != cudaSuccess) {
+            cudaGraphExecDestroy(p->graph_exec);
+            p->graph_exec = nullptr;
+            return fail_cuda(p, ce, "emx_transport: iteration graph");
+        }
         CU(cudaEventRecord(p->evOut, p->s0));
         CU(cudaStreamWaitEvent(st, p->evOut, 0));
     } else {
