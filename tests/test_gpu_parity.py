@@ -241,6 +241,32 @@ def test_shards_of_the_primaries_sum_to_the_whole(emx):
         G.set_primary_offset(-1)
 
 
+def test_kept_iteration_graph_is_dropped_when_an_argument_changes(emx):
+    """emx_transport keeps the instantiated graph for the next call with the same kernel arguments; a new seed,
+    new primaries, another workspace size or rebuilt tables must each give the result of a fresh problem."""
+    desc, prim = W.get(1, 24)
+    G = emx.Problem(desc)
+    pd = G.upload_primaries(prim)
+    kw = dict(n_slots=1 << 13, queue_capacity=1 << 18)
+    a1 = G.transport(pd, 11, **kw)
+    a2 = G.transport(pd, 11, **kw)                      # reused graph
+    b = G.transport(pd, 12, **kw)                       # other seed
+    a3 = G.transport(pd, 11, **kw)
+    for x in (a2, a3):
+        assert np.array_equal(x["steps"], a1["steps"]) and np.array_equal(x["inter"], a1["inter"])
+        assert np.allclose(x["edep"], a1["edep"], rtol=1e-12)
+    assert not np.array_equal(b["steps"], a1["steps"])
+    fresh = emx.Problem(desc)
+    f = fresh.transport(fresh.upload_primaries(prim), 12, **kw)
+    assert np.array_equal(b["steps"], f["steps"]) and np.array_equal(b["inter"], f["inter"])
+    prim2 = {k: v[:12].copy() for k, v in prim.items()}
+    c = G.transport(G.upload_primaries(prim2), 11, **kw)            # other primaries
+    f2 = fresh.transport(fresh.upload_primaries(prim2), 11, **kw)
+    assert np.array_equal(c["steps"], f2["steps"]) and c["E_in"] == pytest.approx(a1["E_in"] / 2)
+    d = G.transport(pd, 11, n_slots=1 << 12, queue_capacity=1 << 18)  # other workspace carve-up
+    assert np.array_equal(d["steps"], a1["steps"])
+
+
 def test_error_paths(emx):
     import ctypes as C
     L = emx.lib()
