@@ -53,6 +53,8 @@ struct emx_problem {
     Primaries graph_pr;
     uint64_t graph_seed = 0;
     unsigned long long graph_gen = 0, params_gen = 1;
+    int loop_node = 1;         // 1: the whole loop is one graph with a WHILE node; 0: flat graphs + host polling
+    bool graph_is_loop = false;
     bool use_graph = true;
     long slice_above = -1;  // < 0: n_slots / 32
     int slice_budget = 2;
@@ -183,6 +185,7 @@ int emx_create(emx_problem **out) {
     // tuning knobs of the scheduler (they never change a result, only when work is done)
     if (const char *e = getenv("EMX_SLICE_BUDGET")) p->slice_budget = atoi(e) > 0 ? atoi(e) : p->slice_budget;
     if (const char *e = getenv("EMX_SLICE_ABOVE")) p->slice_above = atol(e);
+    if (const char *e = getenv("EMX_LOOP_NODE")) p->loop_node = atoi(e);
     if (const char *e = getenv("EMX_WARPS_PER_SM")) sscanf(e, "%d,%d,%d", &p->warps_per_sm[0], &p->warps_per_sm[1], &p->warps_per_sm[2]);
     *out = p;
     return EMX_OK;
@@ -454,46 +457,105 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         prz.n = pr.n; prz.ptype = pr.ptype; prz.E = pr.E; prz.pos3 = pr.pos3; prz.dir3 = pr.dir3;
         prz.vol = pr.vol; prz.surf = pr.surf; prz.first = pr.first;
         const bool keep = p->graph_exec && p->graph_gen == p->params_gen && p->graph_seed == seed &&
+                          p->graph_is_loop == (p->loop_node != 0) &&
                           memcmp(&p->graph_w, &w, sizeof(Work)) == 0 && memcmp(&p->graph_pr, &prz, sizeof(Primaries)) == 0;
+        // kIterPerGraph iterations of the loop, captured from s0 (fork / join over s1, s2)
+        auto capture_iterations = [&]() -> cudaError_t {
+            cudaError_t e = cudaSuccess;
+            for (int k = 0; k < kIterPerGraph && e == cudaSuccess; ++k) {
+                e = launch_refill(w, pr, p->s0);
+                if (e == cudaSuccess) e = cudaEventRecord(p->evFork, p->s0);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s1, p->evFork, 0);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s2, p->evFork, 0);
+                if (e == cudaSuccess) e = launch_step_pool(kPositron, p->P, w, seed, p->d_tally, p->n_sm, p->s1);
+                if (e == cudaSuccess) e = launch_step_pool(kElectron, p->P, w, seed, p->d_tally, p->n_sm, p->s2);
+                if (e == cudaSuccess) e = launch_step_pool(kGamma, p->P, w, seed, p->d_tally, p->n_sm, p->s0);
+                if (e == cudaSuccess) e = cudaEventRecord(p->evJ1, p->s1);
+                if (e == cudaSuccess) e = cudaEventRecord(p->evJ2, p->s2);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s0, p->evJ1, 0);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s0, p->evJ2, 0);
+            }
+            return e;
+        };
         if (!keep) {
             if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
             p->graph_exec = nullptr;
             cudaGraph_t graph = nullptr;
-            CU(cudaStreamBeginCapture(p->s0, cudaStreamCaptureModeThreadLocal));
-            for (int k = 0; k < kIterPerGraph && ce == cudaSuccess; ++k) {
-                ce = launch_refill(w, pr, p->s0);
-                if (ce == cudaSuccess) ce = cudaEventRecord(p->evFork, p->s0);
-                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s1, p->evFork, 0);
-                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s2, p->evFork, 0);
-                if (ce == cudaSuccess) ce = launch_step_pool(kPositron, p->P, w, seed, p->d_tally, p->n_sm, p->s1);
-                if (ce == cudaSuccess) ce = launch_step_pool(kElectron, p->P, w, seed, p->d_tally, p->n_sm, p->s2);
-                if (ce == cudaSuccess) ce = launch_step_pool(kGamma, p->P, w, seed, p->d_tally, p->n_sm, p->s0);
-                if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ1, p->s1);
-                if (ce == cudaSuccess) ce = cudaEventRecord(p->evJ2, p->s2);
-                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ1, 0);
-                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(p->s0, p->evJ2, 0);
+            bool looped = false;
+            if (p->loop_node) {
+                // the whole loop as ONE graph: a WHILE node whose body is kIterPerGraph iterations followed by
+                // a one-thread kernel that sets the node's condition from the done flag -- nothing returns to
+                // the host until the transport is over
+                cudaGraphConditionalHandle handle = 0;
+                cudaGraphNode_t node = nullptr;
+                cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+                ce = cudaGraphCreate(&graph, 0);
+                if (ce == cudaSuccess) ce = cudaGraphConditionalHandleCreate(&handle, graph, 1, cudaGraphCondAssignDefault);
+                if (ce == cudaSuccess) {
+                    np.type = cudaGraphNodeTypeConditional;
+                    np.conditional.handle = handle;
+                    np.conditional.type = cudaGraphCondTypeWhile;
+                    np.conditional.size = 1;
+                    ce = cudaGraphAddNode(&node, graph, nullptr, 0, &np);
+                }
+                if (ce == cudaSuccess)
+                    ce = cudaStreamBeginCaptureToGraph(p->s0, np.conditional.phGraph_out[0], nullptr, nullptr, 0,
+                                                       cudaStreamCaptureModeThreadLocal);
+                if (ce == cudaSuccess) {
+                    ce = capture_iterations();
+                    if (ce == cudaSuccess) ce = launch_loop_condition(w, (unsigned long long)handle, p->s0);
+                    cudaGraph_t body = nullptr;
+                    const cudaError_t ce2 = cudaStreamEndCapture(p->s0, &body);
+                    if (ce == cudaSuccess) ce = ce2;
+                }
+                if (ce == cudaSuccess) ce = cudaGraphInstantiate(&p->graph_exec, graph, 0);
+                if (ce == cudaSuccess) looped = true;
+                else {  // no conditional nodes on this driver: fall back to flat graphs
+                    cudaGetLastError();
+                    if (graph) cudaGraphDestroy(graph);
+                    graph = nullptr;
+                    p->graph_exec = nullptr;
+                    p->loop_node = 0;
+                    ce = cudaSuccess;
+                }
             }
-            cudaError_t ce2 = cudaStreamEndCapture(p->s0, &graph);
-            if (ce != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return fail_cuda(p, ce, "emx_transport: graph capture"); }
-            CU(ce2);
-            ce = cudaGraphInstantiate(&p->graph_exec, graph, 0);
+            if (!looped) {
+                CU(cudaStreamBeginCapture(p->s0, cudaStreamCaptureModeThreadLocal));
+                ce = capture_iterations();
+                cudaError_t ce2 = cudaStreamEndCapture(p->s0, &graph);
+                if (ce != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return fail_cuda(p, ce, "emx_transport: graph capture"); }
+                CU(ce2);
+                ce = cudaGraphInstantiate(&p->graph_exec, graph, 0);
+            }
             cudaGraphDestroy(graph);
             if (ce != cudaSuccess) { p->graph_exec = nullptr; return fail_cuda(p, ce, "cudaGraphInstantiate"); }
             p->graph_w = w;
             p->graph_pr = prz;
             p->graph_seed = seed;
             p->graph_gen = p->params_gen;
+            p->graph_is_loop = looped;
         }
         cudaGraphExec_t exec = p->graph_exec;
-        int batch = 1;
-        for (;;) {
-            for (int k = 0; k < batch && ce == cudaSuccess; ++k) ce = cudaGraphLaunch(exec, p->s0);
-            p->launches += (long)batch * kIterPerGraph * kLaunchesPerIteration;
-            p->iterations_launched += (long)batch * kIterPerGraph;
+        if (p->graph_is_loop) {
+            ce = cudaGraphLaunch(exec, p->s0);
             if (ce == cudaSuccess) ce = cudaMemcpyAsync(p->h_ctl, w.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, p->s0);
             if (ce == cudaSuccess) ce = cudaStreamSynchronize(p->s0);
-            if (ce != cudaSuccess || p->h_ctl->done || p->h_ctl->error) break;
-            if (batch < 8) batch *= 2;
+            if (ce == cudaSuccess) {
+                const long bodies = (long)((p->h_ctl->iter + kIterPerGraph) / kIterPerGraph);  // the last one finds done
+                p->launches += bodies * (kIterPerGraph * kLaunchesPerIteration + 1);
+                p->iterations_launched += bodies * kIterPerGraph;
+            }
+        } else {
+            int batch = 1;
+            for (;;) {
+                for (int k = 0; k < batch && ce == cudaSuccess; ++k) ce = cudaGraphLaunch(exec, p->s0);
+                p->launches += (long)batch * kIterPerGraph * kLaunchesPerIteration;
+                p->iterations_launched += (long)batch * kIterPerGraph;
+                if (ce == cudaSuccess) ce = cudaMemcpyAsync(p->h_ctl, w.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, p->s0);
+                if (ce == cudaSuccess) ce = cudaStreamSynchronize(p->s0);
+                if (ce != cudaSuccess || p->h_ctl->done || p->h_ctl->error) break;
+                if (batch < 8) batch *= 2;
+            }
         }
         if (ce != cudaSuccess) {
             cudaGraphExecDestroy(p->graph_exec);

@@ -29,6 +29,8 @@ cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st);
 // one iteration of the loop = launch_refill (k_plan, k_fill, k_move) then
 // launch_step (one persistent kernel per pool); tally = device edep array
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st);
+// sets the condition of a graph WHILE node (handle from cudaGraphConditionalHandleCreate): go on unless done
+cudaError_t launch_loop_condition(const Work &w, unsigned long long handle, cudaStream_t st);
 cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st);
 cudaError_t launch_phase(int pt, int phase, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                          cudaStream_t st);

@@ -1000,6 +1000,15 @@ cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
     return cudaGetLastError();
 }
 
+// A12 when the loop is a graph WHILE node: after the last iteration of the body, continue unless done
+__global__ void k_loop_condition(Work w, cudaGraphConditionalHandle handle) {
+    cudaGraphSetConditional(handle, w.ctl->done ? 0u : 1u);
+}
+cudaError_t launch_loop_condition(const Work &w, unsigned long long handle, cudaStream_t st) {
+    k_loop_condition<<<1, 1, 0, st>>>(w, (cudaGraphConditionalHandle)handle);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
                              cudaStream_t st);
 

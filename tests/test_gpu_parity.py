@@ -283,13 +283,15 @@ def test_error_paths(emx):
 
 
 def test_scheduling_knobs_do_not_change_results(emx, monkeypatch):
-    """Time slicing of the field propagation (substep budget per iteration) and the graph / stream launch
-    paths only change WHEN work is done: counters are equal, tallies equal up to summation order."""
+    """Time slicing of the field propagation (substep budget per iteration) and the launch paths (the loop as
+    one graph with a WHILE node, flat iteration graphs polled by the host, plain stream launches, profiled
+    launches) only change WHEN work is done: counters are equal, tallies equal up to summation order."""
     desc, prim = W.get(4, 64)
     runs, hists = [], []
-    for budget, mode in (("2", 0), ("100000", 0), ("7", 2), ("2", 1)):
+    for budget, mode, loop_node in (("2", 0, "1"), ("100000", 0, "1"), ("7", 2, "1"), ("2", 1, "1"), ("2", 0, "0")):
         monkeypatch.setenv("EMX_SLICE_BUDGET", budget)
         monkeypatch.setenv("EMX_SLICE_ABOVE", "0")
+        monkeypatch.setenv("EMX_LOOP_NODE", loop_node)      # 0: flat iteration graphs polled by the host
         G = emx.Problem(desc)
         G.set_profile(mode)
         runs.append(G.transport(G.upload_primaries(prim), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 20))
