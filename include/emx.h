@@ -246,14 +246,15 @@ int emx_read_step_hist(const emx_problem *p, uint64_t *hist_host);
  * measured with CUDA events on the caller's stream; < 0 if none. */
 double emx_last_transport_ms(const emx_problem *p);
 
-/* Per-kernel timing of the loop.  Normally emx_transport runs the loop as a CUDA graph (8 iterations per
- * graph, the pools' step kernels as parallel branches) on internal streams ordered after `stream`.  With
+/* Per-kernel timing of the loop.  Normally emx_transport runs the whole loop as ONE CUDA graph (a WHILE node
+ * whose body is 8 iterations, the pools' step kernels as parallel branches, and a kernel that sets the node's
+ * condition from the done flag) on internal streams ordered after `stream`.  With
  * profiling on (on = 1) it launches kernel by kernel on `stream` instead and brackets every launch with
  * CUDA events on that stream.  emx_get_profile: ms8[8] = milliseconds of the last transport spent in
  * { phase A (k_step_pool) gamma, e-, e+, phase B (k_interact) gamma, e-, e+, refill (k_plan + k_fill +
  * k_move), all step kernels }; *launches = kernels launched by the last transport (always counted);
- * *iterations_launched = iterations enqueued (>= iterations needed: the host checks the done flag once per
- * batch).  emx_get_lanes: lanes6[6] = track slots processed by { phase A gamma, e-, e+, phase B gamma, e-, e+ }
+ * *iterations_launched = iterations run, empty ones included (>= iterations needed: the done flag is looked at
+ * once per 8 iterations in the graph, once per batch of launches otherwise).  emx_get_lanes: lanes6[6] = track slots processed by { phase A gamma, e-, e+, phase B gamma, e-, e+ }
  * over the last transport (the units of each kernel's algorithmic bytes).  Output pointers may be NULL. */
 int emx_set_profile(emx_problem *p, int on);
 int emx_get_profile(const emx_problem *p, double *ms8, long *launches, long *iterations_launched);
