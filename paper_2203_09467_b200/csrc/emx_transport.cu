@@ -233,6 +233,7 @@ cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st) {
 }
 
 constexpr int kPlanThreads = 1024;
+constexpr int kPatience = 64;  // iterations without progress before the loop gives up (R7)
 
 // ------------------------------------------------------------------------------------------------
 // A9 / A12: refill plan and loop control.  One block.  Per pool: exclusive prefix sum of the per-chunk
@@ -333,13 +334,16 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
         } else {
             c->iter += 1;
             // R7: a step whose secondaries do not fit on the stacks is not committed and is re-executed in a
-            // later iteration with the same (tid, step) and hence the same draws; if a whole iteration commits
-            // nothing although tracks are live, the stacks are too small for this problem
+            // later iteration with the same (tid, step) and hence the same draws.  Progress = steps committed or
+            // field propagations advanced; retiring a tombstone is none (stalled warps can push and retire
+            // tombstones for ever).  kPatience iterations in a row without progress although tracks are live:
+            // the stacks are too small for this problem
             c->m_step[0] = (int)ng;
             c->m_step[1] = (int)ne;
             c->m_step[2] = (int)np;
             EMX_TL(w, 0, 1, 1);
-            if (c->had_live && c->progress == 0ull) {
+            c->idle_iters = (c->had_live && c->progress == 0ull) ? c->idle_iters + 1 : 0;
+            if (c->idle_iters >= kPatience) {
                 c->error = EMX_E_CAPACITY;
                 c->done = 1;
             }
@@ -715,14 +719,14 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
         for (int o2 = 16; o2 > 0; o2 >>= 1) n_g += __shfl_xor_sync(0xffffffffu, n_g, o2);
         const unsigned n_commit = __popc(__ballot_sync(0xffffffffu, commit));
         const unsigned n_done = __popc(__ballot_sync(0xffffffffu, commit && pend < 0));  // completed steps
-        const unsigned n_tomb = __popc(__ballot_sync(0xffffffffu, tomb || parked));
+        const unsigned n_parked = __popc(__ballot_sync(0xffffffffu, parked));
         const unsigned n_stall = __popc(__ballot_sync(0xffffffffu, active && stall));
         const unsigned n_active = __popc(__ballot_sync(0xffffffffu, active));
         if (lane == 9) add = n_g;
         if (lane == 10) add = n_e;
         if (lane == 11) add = n_p;
         if (lane == 12 + PT) add = n_done;
-        if (lane == 15) add = n_commit + n_tomb;
+        if (lane == 15) add = n_commit + n_parked;
         if (lane == 16) add = n_stall;
         if (lane == 17) add = n_active;
         acc.n += add;

@@ -50,6 +50,7 @@ struct Ctl {
     int m_step[3];  // tracks to step this iteration (= n_live)
     PoolPlan plan[3];
     int done, error, had_live;
+    int idle_iters;  // consecutive iterations without progress although tracks are live (R7)
     int work_ctr3[3];  // next 32-slot chunk of each pool's step kernel (phase A)
     int work_ctrB[3];  // next 32-entry chunk of each pool's interaction lists (phase B)
     unsigned long long icount64[3];  // entries in the interaction lists of each pool, 3 x 21 bits packed

@@ -201,6 +201,20 @@ def test_full_stack_stalls_do_not_change_the_physics(emx, emo):
     assert np.array_equal(hb, G.read_step_hist())      # stalled steps are not counted twice
 
 
+def test_hopelessly_small_workspace_is_an_error_not_a_hang(emx):
+    """R7: 100 GeV showers in 384 slots with 1000 stack records dead-lock (every live track waits for room on a
+    full stack, and stalled warps keep pushing and retiring tombstones).  The loop must notice that no step is
+    committed any more and return EMX_E_CAPACITY; the same problem with room runs."""
+    desc, prim = W.get(4, 8)
+    G = emx.Problem(desc)
+    pd = G.upload_primaries(prim)
+    with pytest.raises(emx.EmxError, match="-4"):
+        G.transport(pd, desc["seed"], n_slots=384, queue_capacity=1000)
+    ok = G.transport(pd, desc["seed"], n_slots=384, queue_capacity=1 << 20)
+    assert ok["stalls"] == 0 and ok["track_steps"] > 100000
+    assert ok["edep"].sum() + ok["escaped"] + ok["looper"] == pytest.approx(ok["E_in"], rel=1e-9)
+
+
 def test_results_do_not_depend_on_slots_or_host_entry(emx):
     desc, prim = W.get(2, 12)
     G = emx.Problem(desc)
