@@ -201,6 +201,44 @@ def test_full_stack_stalls_do_not_change_the_physics(emx, emo):
     assert np.array_equal(hb, G.read_step_hist())      # stalled steps are not counted twice
 
 
+@pytest.mark.parametrize("case", ["none", "one", "escape_at_once", "positrons_below_cut", "photons_below_cut", "grid_top"])
+def test_degenerate_primaries_against_the_oracle(emx, emo, case):
+    """Edge cases of the loop: no primary, one primary, primaries that leave the world in their first step,
+    primaries born below the tracking cut (e+ still annihilate at rest), energies at the top of the grid."""
+    desc, prim = W.get(4, 16)
+    p = {k: v.copy() for k, v in prim.items()}
+    if case == "none":
+        p = {k: v[:0] for k, v in p.items()}
+    elif case == "one":
+        p = {k: v[:1] for k, v in p.items()}
+    elif case == "escape_at_once":
+        p["pos"][:, 2] = 149.99
+        p["dir"][:] = np.array([0.0, 0.0, 1.0])
+    elif case == "positrons_below_cut":
+        p["ptype"][:] = 2
+        p["E"][:] = 0.0005
+    elif case == "photons_below_cut":
+        p["ptype"][:] = 0
+        p["E"][:] = 0.0005
+    elif case == "grid_top":
+        p = {k: v[:2] for k, v in p.items()}
+        p["E"][:] = 1e5
+    G, O = emx.Problem(desc), emo.Problem(desc)
+    o = O.transport(p, desc["seed"])
+    g = G.transport(G.upload_primaries(p), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 21)
+    assert g["E_in"] == pytest.approx(o["E_in"], rel=1e-14, abs=0.0)
+    for k in ("steps", "tracks", "inter"):
+        a, b = o[k].astype(np.float64), g[k].astype(np.float64)
+        assert np.all(np.abs(a - b) <= 1e-3 * a + 3.0), (k, o[k], g[k])
+    if case in ("none", "escape_at_once", "positrons_below_cut", "photons_below_cut"):
+        assert np.array_equal(g["steps"], o["steps"]) and np.array_equal(g["tracks"], o["tracks"])
+        assert np.array_equal(G.read_step_hist(), o["step_hist"])
+    for k in ("escaped", "below_cut", "looper"):
+        assert g[k] == pytest.approx(o[k], rel=1e-3, abs=1e-9), k
+    assert g["edep"].sum() == pytest.approx(o["edep"].sum(), rel=1e-3, abs=1e-9)
+    assert g["stalls"] == 0
+
+
 def test_hopelessly_small_workspace_is_an_error_not_a_hang(emx):
     """R7: 100 GeV showers in 384 slots with 1000 stack records dead-lock (every live track waits for room on a
     full stack, and stalled warps keep pushing and retiring tombstones).  The loop must notice that no step is
