@@ -11,16 +11,10 @@
 
 #if defined(__CUDACC__)
 #define EMX_HD __host__ __device__ __forceinline__
-// shared, out-of-line building blocks: the fused step kernel is instruction-cache bound when everything is
-// inlined (345 KB of SASS), so the routines with many call sites exist once
-#ifndef EMX_OUTLINE
-#define EMX_OUTLINE 0
-#endif
-#if EMX_OUTLINE
-#define EMX_NI inline __host__ __device__ __noinline__
-#else
+// the larger building blocks (samplers, propagation, lookups).  Out-of-line copies were tried against the
+// instruction-fetch stalls of the first fused kernel and lost to the call ABI and spills:
+// everything is inlined, and one kernel per pool and phase keeps the code small instead
 #define EMX_NI __host__ __device__ __forceinline__
-#endif
 #else
 #define EMX_HD inline
 #define EMX_NI inline

@@ -1,9 +1,10 @@
-// emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the fused
-// per-type step kernel (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
+// emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the per-type step
+// kernels (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
 //
 // One ITERATION = k_plan (admission + refill plan) -> k_fill -> k_move -> per pool (e+, e-, gamma):
-// k_step_pool<PT> (phase A) -> k_interact<PT> (phase B).  Nothing returns to the host
-// between iterations: pool sizes, stack tops and the done flag live in the device control block.
+// k_step_pool<PT> (phase A) -> k_interact<PT> (phase B).  Eight iterations and k_loop_condition form the body
+// of a graph WHILE node: nothing returns to the host during a transport; pool sizes, stack tops and the done
+// flag live in the device control block.
 #include <cuda_runtime.h>
 #include "emx_kernels.h"
 #include "emx_step.h"
@@ -444,10 +445,10 @@ __global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// A1-A8 + A10: one step of every live track.  One PERSISTENT launch per pool (e+, e-, gamma): the grid is a
-// fixed number of single-warp blocks (16 per SM: what 128 registers per thread allow) and each warp pulls
-// 32-slot chunks of the pool from a device-side work counter until none are left.  A warp never waits for
-// another warp: there is no block-wide barrier and no shared memory.  One pool per launch keeps the code of a
+// A1-A8 + A10: one step of every live track.  One PERSISTENT launch per pool and phase: the grid is a fixed
+// number of 128-thread blocks (16 warps per SM: what 128 registers per thread allow) whose four warps work
+// independently, each pulling 32-slot chunks of the pool from a device-side work counter until none are
+// left.  A warp never waits for another warp: there is no block-wide barrier and no shared memory.  One pool per launch keeps the code of a
 // single particle type in the instruction caches (a merged kernel for the three types was instruction-fetch
 // bound: profiles/r1_v2_*); the three launches are parallel branches of the iteration graph.
 //   per lane: the track is read once, stepped in registers (step<PT>) and written once;
@@ -785,12 +786,6 @@ __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uin
         vol0 = t.vol;
         step0 = t.step;
         pend = step_pre<PT>(P, seed, t, o, fs, budget);
-#if defined(EMX_ONE_PHASE)
-        if (pend >= 0) {
-            step_interact<PT>(P, seed, t, o, pend);
-            pend = -1;
-        }
-#endif
         if (PT != kGamma && o.suspended) {
             // the propagation continues in the next iteration: park position, direction, surface flag and the
             // loop variables; nothing else of the step has happened yet
