@@ -110,6 +110,8 @@ typedef struct {
     emo_physics ph;
     double B[3];                 /* tesla */
     double Bmag, Bhat[3];
+    int field_kind;              /* 0 uniform; 1 solenoid with fringe (emo_set_field_fringe) */
+    double fringe_z0, fringe_a;  /* cm */
     double lnE0, dlnE, inv_dlnE; /* grid: x_j = lnE0 + j*dlnE */
     int built;
 } emo_problem;
@@ -176,6 +178,16 @@ int emo_add_material(emo_problem *p, int n_elem, const int *Z, const double *A, 
 int emo_add_surface(emo_problem *p, int type, double v);
 int emo_add_volume(emo_problem *p, int n_faces, const int *surf, const int *sense, int material, int tally);
 int emo_set_field(emo_problem *p, double Bx, double By, double Bz);
+/* Non-uniform field ("propagation of particles through arbitrary magnetic fields"): a solenoid
+ * along z whose field falls off towards its ends, B(x) = |B| g(x) with
+ *   f(z) = 1 / (1 + exp((|z| - z0) / a)),   g = (-x f'(z) / 2, -y f'(z) / 2, f(z)),   f' = -sign(z) f (1 - f) / a
+ * (the radial part makes div B = 0 to first order in r).  Needs a field set along +-z; returns -1 otherwise. */
+int emo_set_field_fringe(emo_problem *p, double z0_cm, double a_cm);
+/* g(x) of the field set on p (Bhat for the uniform field) */
+void emo_field_profile(const emo_problem *p, const double x[3], double g[3]);
+/* step doubling as emo_rk4_doubling, the field evaluated at the stage positions */
+void emo_rk4_doubling_map(const emo_problem *p, const double x[3], const double u[3], double kappa, double h,
+                          double x1[3], double u1[3], double *err);
 int emo_set_physics(emo_problem *p, const emo_physics *ph);
 int emo_set_cuts(emo_problem *p, int material, double Tcut, double kcut); /* explicit energies */
 int emo_build_tables(emo_problem *p);

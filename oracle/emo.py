@@ -70,7 +70,9 @@ def lib():
             "emo_gauss_legendre": (None, [i, dp, dp]),
             "emo_create": (p, []), "emo_destroy": (None, [p]),
             "emo_add_material": (i, [p, i, ip, dp, dp, d, d]), "emo_add_surface": (i, [p, i, d]),
-            "emo_add_volume": (i, [p, i, ip, ip, i, i]), "emo_set_field": (i, [p, d, d, d]),
+            "emo_add_volume": (i, [p, i, ip, ip, i, i]), "emo_set_field": (i, [p, d, d, d]), "emo_set_field_fringe": (i, [p, d, d]),
+            "emo_field_profile": (None, [p, dp, dp]),
+            "emo_rk4_doubling_map": (None, [p, dp, dp, d, d, dp, dp, dp]),
             "emo_set_physics": (i, [p, C.POINTER(Physics)]), "emo_set_cuts": (i, [p, i, d, d]),
             "emo_build_tables": (i, [p]), "emo_get_table": (i, [p, i, i, dp, i]),
             "emo_get_material_info": (i, [p, i, dp]), "emo_lookup": (d, [p, i, i, d]),
@@ -136,6 +138,8 @@ class Problem:
             assert L.emo_add_volume(self.h, len(s), _ip(s), _ip(e), vol["material"], vol["tally"]) >= 0
         B = desc.get("field", (0.0, 0.0, 0.0))
         L.emo_set_field(self.h, *[float(b) for b in B])
+        if desc.get("field_fringe"):
+            assert L.emo_set_field_fringe(self.h, *[float(v) for v in desc["field_fringe"]]) == 0
         ph = physics_from_dict(desc["physics"])
         assert L.emo_set_physics(self.h, C.byref(ph)) == 0
         for im, m in enumerate(desc["materials"]):

@@ -1,5 +1,5 @@
 /* ORACLE (test infrastructure).  Charged-track propagation in a uniform magnetic
- * field ("on-device propagation of particles through arbitrary
+ * field, or in a solenoid field with a fringe ("on-device propagation of particles through arbitrary
  * magnetic fields ... different integration algorithms"; BASELINE.json
  * configs[3]: "adaptive RK4 (1e-6 mm miss-distance tolerance)").  The paper gives
  * no algorithm: classical RK4 with step doubling (Press et al.) plus a chord /
@@ -46,6 +46,50 @@ void emo_rk4_doubling(const double x[3], const double u[3], double kappa, const 
     u1[0] /= n; u1[1] /= n; u1[2] /= n;
 }
 
+/* ---- non-uniform field: the same integrator with the field taken at the stage positions ---- */
+void emo_field_profile(const emo_problem *p, const double x[3], double g[3]) {
+    if (p->field_kind == 0) { g[0] = p->Bhat[0]; g[1] = p->Bhat[1]; g[2] = p->Bhat[2]; return; }
+    const double az = fabs(x[2]);
+    const double f = 1.0 / (1.0 + exp((az - p->fringe_z0) / p->fringe_a));
+    const double sg = x[2] > 0.0 ? 1.0 : (x[2] < 0.0 ? -1.0 : 0.0);
+    const double fp = -sg * f * (1.0 - f) / p->fringe_a;
+    g[0] = -0.5 * x[0] * fp * p->Bhat[2];
+    g[1] = -0.5 * x[1] * fp * p->Bhat[2];
+    g[2] = f * p->Bhat[2];
+}
+
+static void rk4_map(const emo_problem *p, const double x[3], const double u[3], double kappa, double h,
+                    double xo[3], double uo[3]) {
+    double g[3], k1x[3], k1u[3], k2x[3], k2u[3], k3x[3], k3u[3], k4x[3], k4u[3], xt[3], ut[3];
+    emo_field_profile(p, x, g);
+    rhs(u, kappa, g, k1x, k1u);
+    for (int i = 0; i < 3; ++i) { xt[i] = x[i] + 0.5 * h * k1x[i]; ut[i] = u[i] + 0.5 * h * k1u[i]; }
+    emo_field_profile(p, xt, g);
+    rhs(ut, kappa, g, k2x, k2u);
+    for (int i = 0; i < 3; ++i) { xt[i] = x[i] + 0.5 * h * k2x[i]; ut[i] = u[i] + 0.5 * h * k2u[i]; }
+    emo_field_profile(p, xt, g);
+    rhs(ut, kappa, g, k3x, k3u);
+    for (int i = 0; i < 3; ++i) { xt[i] = x[i] + h * k3x[i]; ut[i] = u[i] + h * k3u[i]; }
+    emo_field_profile(p, xt, g);
+    rhs(ut, kappa, g, k4x, k4u);
+    for (int i = 0; i < 3; ++i) {
+        xo[i] = x[i] + (h / 6.0) * (k1x[i] + 2.0 * k2x[i] + 2.0 * k3x[i] + k4x[i]);
+        uo[i] = u[i] + (h / 6.0) * (k1u[i] + 2.0 * k2u[i] + 2.0 * k3u[i] + k4u[i]);
+    }
+}
+
+void emo_rk4_doubling_map(const emo_problem *p, const double x[3], const double u[3], double kappa, double h,
+                          double x1[3], double u1[3], double *err) {
+    double xf[3], uf[3], xm[3], um[3];
+    rk4_map(p, x, u, kappa, h, xf, uf);
+    rk4_map(p, x, u, kappa, 0.5 * h, xm, um);
+    rk4_map(p, xm, um, kappa, 0.5 * h, x1, u1);
+    double dx = xf[0] - x1[0], dy = xf[1] - x1[1], dz = xf[2] - x1[2];
+    *err = sqrt(dx * dx + dy * dy + dz * dz);
+    double n = sqrt(u1[0] * u1[0] + u1[1] * u1[1] + u1[2] * u1[2]);
+    u1[0] /= n; u1[1] /= n; u1[2] /= n;
+}
+
 /* propagate up to s_max inside cell `vol`; returns the arc length travelled,
  * *hit = surface reached (-1: none).  x, u are updated in place. */
 double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x[3], double u[3],
@@ -60,7 +104,8 @@ double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x
         double rem = s_max - s_done;
         if (h > rem) h = rem;
         double x1[3], u1[3], err;
-        emo_rk4_doubling(x, u, kappa, p->Bhat, h, x1, u1, &err);
+        if (p->field_kind == 0) emo_rk4_doubling(x, u, kappa, p->Bhat, h, x1, u1, &err);
+        else emo_rk4_doubling_map(p, x, u, kappa, h, x1, u1, &err);
         if (err > eps && h > 1e-9) {
             double f = 0.9 * pow(eps / err, 0.2);
             h *= (f > 0.2 ? f : 0.2);

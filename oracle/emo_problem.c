@@ -82,6 +82,13 @@ int emo_set_field(emo_problem *p, double Bx, double By, double Bz) {
     p->B[0] = Bx; p->B[1] = By; p->B[2] = Bz;
     p->Bmag = sqrt(Bx * Bx + By * By + Bz * Bz);
     for (int i = 0; i < 3; ++i) p->Bhat[i] = p->Bmag > 0.0 ? p->B[i] / p->Bmag : 0.0;
+    p->field_kind = 0;
+    return 0;
+}
+
+int emo_set_field_fringe(emo_problem *p, double z0_cm, double a_cm) {
+    if (!(p->Bmag > 0.0) || p->B[0] != 0.0 || p->B[1] != 0.0 || !(z0_cm > 0.0) || !(a_cm > 0.0)) return -1;
+    p->field_kind = 1; p->fringe_z0 = z0_cm; p->fringe_a = a_cm;
     return 0;
 }
 

@@ -190,7 +190,17 @@ def config5(n=100000, n_zbins=28, half_length=700.0):
     return desc, _prim(n, 0, 1000.0, (0, 0, 0), d, 0, -1)
 
 
-CONFIGS = [config0, config1, config2, config3, config4, config5]
+def config6(n=20000):
+    """SURVEY 8(f) f4, "non-uniform field maps" ("arbitrary magnetic fields"): the barrel of config
+    4 in a solenoid field that falls off towards the ends of the barrel, B_z(0, z) = 4 T / (1 + exp((|z| - 100
+    cm) / 15 cm)), with the radial component that keeps div B = 0 to first order in r (include/emx.h:
+    emx_set_field_fringe).  Same primaries as config 4."""
+    desc, prim = config4(n)
+    desc.update(name="config6_barrel_fringe_field", seed=6, field_fringe=(100.0, 15.0))
+    return desc, prim
+
+
+CONFIGS = [config0, config1, config2, config3, config4, config5, config6]
 
 
 def get(k, n=None):

@@ -255,3 +255,93 @@ def test_field_landing_regression_state(emo):
     t.E = 0.003987383479174055; t.vol = 104; t.surf = -1; t.ptype = 1; t.alive = 1
     r = P.step_batch((emo.Track * 1)(t), 3)[0]
     assert r.action == 3 and r.trk.surf == 107 and abs(r.trk.x[1] + 30.0) <= 1e-7 and r.trk.alive == 0
+
+
+# ---------------- non-uniform field: solenoid with a fringe ----------------
+
+def _fringe_problem(emo, z0=100.0, a=15.0):
+    desc, _ = W.get(6, 4)
+    desc = dict(desc)
+    desc["field_fringe"] = (z0, a)
+    return emo.Problem(desc)
+
+
+def test_fringe_field_profile_closed_forms(emo):
+    """g(x): on the axis only B_z, equal to 1/2 at |z| = z0 and to the logistic elsewhere; even in z; the radial
+    part points outwards where the field falls off (beyond the centre) and div g = 0 by central differences."""
+    P = _fringe_problem(emo)
+    L = emo.lib()
+
+    def g(x):
+        out = np.zeros(3)
+        L.emo_field_profile(P.h, emo._dp(np.asarray(x, dtype=np.float64)), emo._dp(out))
+        return out
+    assert g([0, 0, 100.0]) == pytest.approx([0, 0, 0.5], abs=1e-15)
+    assert g([0, 0, -100.0]) == pytest.approx([0, 0, 0.5], abs=1e-15)
+    assert g([0, 0, 130.0])[2] == pytest.approx(1.0 / (1.0 + math.exp(2.0)), rel=1e-14)
+    assert g([0, 0, 0.0])[2] == pytest.approx(1.0 / (1.0 + math.exp(-100.0 / 15.0)), rel=1e-14)
+    a, b = g([3.0, -2.0, 120.0]), g([3.0, -2.0, -120.0])
+    assert a[2] == b[2] and a[0] == -b[0] and a[1] == -b[1]
+    assert a[0] > 0 and a[1] < 0                                   # field lines open up where B_z decreases
+    x0, h = np.array([7.0, -4.0, 95.0]), 1e-4
+    div = sum((g(x0 + h * e)[k] - g(x0 - h * e)[k]) / (2 * h) for k, e in enumerate(np.eye(3)))
+    assert abs(div) < 1e-9
+
+
+def test_fringe_integrator_reduces_to_the_uniform_one(emo):
+    """With the fringe pushed out to |z| = 1e9 cm the profile is exactly (0, 0, 1) and the stage-position
+    integrator must give bit-identical results to the uniform-field one."""
+    P = _fringe_problem(emo, z0=1e9, a=1.0)
+    L = emo.lib()
+    rng = np.random.default_rng(7)
+    Bhat = np.array([0.0, 0.0, 1.0])
+    for _ in range(50):
+        x = rng.normal(0, 50, 3)
+        u = rng.normal(0, 1, 3)
+        u /= np.linalg.norm(u)
+        kappa, h = rng.choice([-1, 1]) * 10 ** rng.uniform(-4, 0), 10 ** rng.uniform(-3, 1)
+        x1, u1, x2, u2 = np.zeros(3), np.zeros(3), np.zeros(3), np.zeros(3)
+        e1, e2 = emo.C.c_double(), emo.C.c_double()
+        L.emo_rk4_doubling(emo._dp(x), emo._dp(u), kappa, emo._dp(Bhat), h, emo._dp(x1), emo._dp(u1), emo.C.byref(e1))
+        L.emo_rk4_doubling_map(P.h, emo._dp(x), emo._dp(u), kappa, h, emo._dp(x2), emo._dp(u2), emo.C.byref(e2))
+        assert np.array_equal(x1, x2) and np.array_equal(u1, u2) and e1.value == e2.value
+
+
+def test_fringe_trajectory_against_an_independent_integrator(emo):
+    """A 50 MeV electron from the centre of the barrel through the fringe region: the oracle's adaptive RK4
+    (inside the vacuum core, no boundary in reach) against scipy's DOP853 at rtol 1e-12 on the same equation
+    of motion written out here.  Tolerance: field_eps (1e-7 cm) per accepted substep."""
+    from scipy.integrate import solve_ivp
+    P = _fringe_problem(emo)
+    L = emo.lib()
+    z0, a, Bmag = 100.0, 15.0, 4.0
+    E = 50.0
+    ME = 0.51099895                                                  # MeV
+    pm = math.sqrt(E * (E + 2 * ME))
+    kappa = -1.0 * 2.99792458e-3 * Bmag / pm
+
+    def rhs(s, y):
+        x, u = y[:3], y[3:]
+        f = 1.0 / (1.0 + math.exp((abs(x[2]) - z0) / a))
+        fp = -math.copysign(1.0, x[2]) * f * (1 - f) / a if x[2] != 0 else 0.0
+        g = np.array([-0.5 * x[0] * fp, -0.5 * x[1] * fp, f])
+        return np.concatenate([u, kappa * np.cross(u, g)])
+    x = np.array([0.5, 0.2, 60.0])
+    u = np.array([0.03, 0.02, 1.0])
+    u /= np.linalg.norm(u)
+    s_max = 80.0                                                     # stays inside r < 5 cm, |z| < 150
+    ref = solve_ivp(rhs, (0, s_max), np.concatenate([x, u]), method="DOP853", rtol=1e-12, atol=1e-14)
+    xo, uo = x.copy(), u.copy()
+    surf = emo.C.c_int(-1)
+    hit = emo.C.c_int(-1)
+    vol = P.locate(x)
+    s = L.emo_propagate_field(P.h, vol, emo.C.byref(surf), emo._dp(xo), emo._dp(uo), kappa, s_max, emo.C.byref(hit))
+    assert hit.value == -1 and s == pytest.approx(s_max, rel=1e-13)
+    assert np.linalg.norm(xo - ref.y[:3, -1]) < 2e-5                 # ~100 substeps of 1e-7 cm local error
+    assert np.linalg.norm(uo - ref.y[3:, -1]) < 1e-6
+    # and it differs from the uniform-field trajectory by far more than that (the test sees the fringe)
+    Pu = emo.Problem(W.get(4, 4)[0])
+    xu, uu = x.copy(), u.copy()
+    surf2, hit2 = emo.C.c_int(-1), emo.C.c_int(-1)
+    L.emo_propagate_field(Pu.h, vol, emo.C.byref(surf2), emo._dp(xu), emo._dp(uu), kappa, s_max, emo.C.byref(hit2))
+    assert np.linalg.norm(xu - xo) > 1e-3

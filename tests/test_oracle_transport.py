@@ -259,7 +259,7 @@ def test_steps_per_track_histogram_config0(emo):
     assert int((np.arange(emo.NHIST) * r["step_hist"][0]).sum()) == int(r["steps"][0])
 
 
-@pytest.mark.parametrize("cfg,n", [(1, 40), (2, 6), (3, 6), (4, 24), (5, 60)])
+@pytest.mark.parametrize("cfg,n", [(1, 40), (2, 6), (3, 6), (4, 24), (5, 60), (6, 24)])
 def test_energy_closure_per_event(emo, cfg, n):
     desc, prim = W.get(cfg, n)
     P = emo.Problem(desc)
