@@ -182,6 +182,14 @@ int emx_add_volume(emx_problem *p, int n_faces, const int *surf, const int *sens
 /* Uniform magnetic field in tesla; all zero = no field. */
 int emx_set_field(emx_problem *p, double Bx_T, double By_T, double Bz_T);
 
+/* Non-uniform field ("propagation of particles through arbitrary magnetic fields"):
+ * turns the field set with emx_set_field, which must point along +-z, into a solenoid field that falls off
+ * towards the ends:  B(x) = |B| g(x),  f(z) = 1 / (1 + exp((|z| - z0) / a)),
+ * g = (-x f'(z) / 2, -y f'(z) / 2, f(z)),  f' = -sign(z) f (1 - f) / a  (div B = 0 to first order in r).
+ * The adaptive RK4 then takes the field at its stage positions.  z0, a in cm, both > 0; EMX_E_ARG otherwise or
+ * when the field is not along z.  emx_set_field resets to a uniform field.  Invalidates the tables. */
+int emx_set_field_fringe(emx_problem *p, double z0_cm, double a_cm);
+
 int emx_get_physics(const emx_problem *p, emx_physics *out);
 int emx_set_physics(emx_problem *p, const emx_physics *ph);
 

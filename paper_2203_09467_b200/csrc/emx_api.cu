@@ -253,6 +253,19 @@ int emx_set_field(emx_problem *p, double Bx, double By, double Bz) {
     p->hp.B[0] = Bx;
     p->hp.B[1] = By;
     p->hp.B[2] = Bz;
+    p->hp.field_kind = 0;
+    p->hp.built = false;
+    return EMX_OK;
+}
+
+int emx_set_field_fringe(emx_problem *p, double z0_cm, double a_cm) {
+    if (!p) return fail(p, EMX_E_ARG, "emx_set_field_fringe: null problem");
+    if (p->hp.B[0] != 0.0 || p->hp.B[1] != 0.0 || p->hp.B[2] == 0.0)
+        return fail(p, EMX_E_ARG, "emx_set_field_fringe: set a field along z first (emx_set_field)");
+    if (!(z0_cm > 0.0) || !(a_cm > 0.0)) return fail(p, EMX_E_ARG, "emx_set_field_fringe: z0 and a must be > 0");
+    p->hp.field_kind = 1;
+    p->hp.fringe_z0 = z0_cm;
+    p->hp.fringe_a = a_cm;
     p->hp.built = false;
     return EMX_OK;
 }
@@ -368,6 +381,9 @@ int emx_build_tables(emx_problem *p, void *stream) {
     const double bm = sqrt(hp.B[0] * hp.B[0] + hp.B[1] * hp.B[1] + hp.B[2] * hp.B[2]);
     P.Bmag = bm;
     for (int i = 0; i < 3; ++i) P.Bhat[i] = bm > 0.0 ? hp.B[i] / bm : 0.0;
+    P.field_kind = hp.field_kind;
+    P.fringe_z0 = hp.fringe_z0;
+    P.fringe_a = hp.fringe_a;
     P.lnE0 = g.lnE0;
     P.dlnE = g.dlnE;
     P.inv_dlnE = g.inv_dlnE;

@@ -47,8 +47,13 @@ EMX_HD void step_one(const Params &P, uint64_t seed, const emx_track &in, emx_st
     fs.attempt = 0;
     const int whole = P.ph.max_substeps;  // the hook runs the whole step in one call
     if (in.ptype == kGamma) step<kGamma>(P, seed, t, o, fs, whole);
-    else if (in.ptype == kElectron) step<kElectron>(P, seed, t, o, fs, whole);
-    else step<kPositron>(P, seed, t, o, fs, whole);
+    else if (P.field_kind == 0) {
+        if (in.ptype == kElectron) step<kElectron>(P, seed, t, o, fs, whole);
+        else step<kPositron>(P, seed, t, o, fs, whole);
+    } else {
+        if (in.ptype == kElectron) step<kElectron, true>(P, seed, t, o, fs, whole);
+        else step<kPositron, true>(P, seed, t, o, fs, whole);
+    }
 
     put3(r.trk.x, t.x);
     put3(r.trk.u, t.u);

@@ -62,6 +62,8 @@ struct Params {
     const int *nb2_off;     // per surface S: cells that do not list S at all (the only other cells that can match)
     const int *nb2_list;
     double Bmag, Bhat[3];
+    int field_kind;               // 0 uniform; 1 solenoid with fringe (emx_set_field_fringe)
+    double fringe_z0, fringe_a;   // cm
     double lnE0, dlnE, inv_dlnE;  // grid: x_j = lnE0 + j * dlnE
 };
 

@@ -1,4 +1,5 @@
-// emx_field.h -- charged-track propagation in a uniform magnetic field (step A5 of DESIGN.md).
+// emx_field.h -- charged-track propagation in a magnetic field, uniform or a solenoid with a fringe (step A5
+// of DESIGN.md).
 // PAPER.md:144 "on-device propagation of particles through arbitrary magnetic fields ... different
 // integration algorithms"; BASELINE.json configs[3]: "adaptive RK4 (1e-6 mm miss-distance tolerance)".
 // Algorithm (C9): classical RK4 with step doubling for the local error, plus a chord /
@@ -31,13 +32,59 @@ EMX_HD void rk4_step(const Vec3 &x, const Vec3 &u, double kappa, const double B[
     uo.z = u.z + h6 * (k1u.z + 2.0 * k2u.z + 2.0 * k3u.z + k4u.z);
 }
 
-// one step of h against two of h/2: err = |x_full - x_half|, result = half-step state, u renormalised
-EMX_NI void rk4_doubling(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, Vec3 &x1, Vec3 &u1,
+// ---- non-uniform field (include/emx.h: emx_set_field_fringe): B(x) = Bmag g(x), a solenoid along z whose
+// field falls off towards its ends, with the radial part that keeps div B = 0 to first order in r
+EMX_HD void field_profile(const Params &P, const Vec3 &x, double g[3]) {
+    const double az = fabs(x.z);
+    const double f = 1.0 / (1.0 + m_exp((az - P.fringe_z0) / P.fringe_a));
+    const double sg = x.z > 0.0 ? 1.0 : (x.z < 0.0 ? -1.0 : 0.0);
+    const double fp = -sg * f * (1.0 - f) / P.fringe_a;
+    g[0] = -0.5 * x.x * fp * P.Bhat[2];
+    g[1] = -0.5 * x.y * fp * P.Bhat[2];
+    g[2] = f * P.Bhat[2];
+}
+
+// classical RK4 with the field taken at the stage positions (x-stages: dx/ds = u)
+EMX_HD void rk4_step_map(const Params &P, const Vec3 &x, const Vec3 &u, double kappa, double h, Vec3 &xo, Vec3 &uo) {
+    double g[3];
+    field_profile(P, x, g);
+    const Vec3 k1u = lorentz(u, kappa, g);
+    const Vec3 x2 = x + (0.5 * h) * u;
+    const Vec3 u2 = u + (0.5 * h) * k1u;
+    field_profile(P, x2, g);
+    const Vec3 k2u = lorentz(u2, kappa, g);
+    const Vec3 x3 = x + (0.5 * h) * u2;
+    const Vec3 u3 = u + (0.5 * h) * k2u;
+    field_profile(P, x3, g);
+    const Vec3 k3u = lorentz(u3, kappa, g);
+    const Vec3 x4 = x + h * u3;
+    const Vec3 u4 = u + h * k3u;
+    field_profile(P, x4, g);
+    const Vec3 k4u = lorentz(u4, kappa, g);
+    const double h6 = h / 6.0;
+    xo.x = x.x + h6 * (u.x + 2.0 * u2.x + 2.0 * u3.x + u4.x);
+    xo.y = x.y + h6 * (u.y + 2.0 * u2.y + 2.0 * u3.y + u4.y);
+    xo.z = x.z + h6 * (u.z + 2.0 * u2.z + 2.0 * u3.z + u4.z);
+    uo.x = u.x + h6 * (k1u.x + 2.0 * k2u.x + 2.0 * k3u.x + k4u.x);
+    uo.y = u.y + h6 * (k1u.y + 2.0 * k2u.y + 2.0 * k3u.y + k4u.y);
+    uo.z = u.z + h6 * (k1u.z + 2.0 * k2u.z + 2.0 * k3u.z + k4u.z);
+}
+
+// one step of h against two of h/2: err = |x_full - x_half|, result = half-step state, u renormalised.
+// MAP: the field is evaluated at the stage positions (non-uniform field); else it is P.Bhat everywhere
+template <bool MAP>
+EMX_NI void rk4_doubling(const Params &P, const Vec3 &x, const Vec3 &u, double kappa, double h, Vec3 &x1, Vec3 &u1,
                          double &err) {
     Vec3 xf, uf, xm, um;
-    rk4_step(x, u, kappa, B, h, xf, uf);
-    rk4_step(x, u, kappa, B, 0.5 * h, xm, um);
-    rk4_step(xm, um, kappa, B, 0.5 * h, x1, u1);
+    if (MAP) {
+        rk4_step_map(P, x, u, kappa, h, xf, uf);
+        rk4_step_map(P, x, u, kappa, 0.5 * h, xm, um);
+        rk4_step_map(P, xm, um, kappa, 0.5 * h, x1, u1);
+    } else {
+        rk4_step(x, u, kappa, P.Bhat, h, xf, uf);
+        rk4_step(x, u, kappa, P.Bhat, 0.5 * h, xm, um);
+        rk4_step(xm, um, kappa, P.Bhat, 0.5 * h, x1, u1);
+    }
     err = norm(xf - x1);
     const double n = norm(u1);
     u1.x /= n;
@@ -57,6 +104,7 @@ struct FieldState {
 // The substep loop of C9 runs for at most `budget` attempts per call; if it is not finished by then,
 // `suspended` is set and fs holds the loop variables, so that the next call continues the SAME sequence of
 // substeps: slicing changes when the work is done, never its result.  budget >= max_substeps: one call.
+template <bool MAP>
 EMX_NI double propagate_field(const Params &P, int vol, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
                               int &hit, FieldState &fs, int budget, bool &suspended) {
     const double eps = P.ph.field_eps;
@@ -91,7 +139,7 @@ EMX_NI double propagate_field(const Params &P, int vol, int &on_surf, Vec3 &x, V
         if (h > rem) h = rem;
         Vec3 x1, u1;
         double err;
-        rk4_doubling(x, u, kappa, P.Bhat, h, x1, u1, err);
+        rk4_doubling<MAP>(P, x, u, kappa, h, x1, u1, err);
         if (err > eps && h > 1e-9) {  // too inaccurate: shrink and retry
             const double f = 0.9 * m_pow(eps / err, 0.2);
             h *= (f > 0.2 ? f : 0.2);

@@ -17,6 +17,8 @@ struct HostProblem {
     std::vector<Volume> vol;
     emx_physics ph;
     double B[3] = {0.0, 0.0, 0.0};
+    int field_kind = 0;  // 0 uniform, 1 solenoid with fringe
+    double fringe_z0 = 0.0, fringe_a = 0.0;
     int n_tally = 0;
     bool built = false;
     std::string err;

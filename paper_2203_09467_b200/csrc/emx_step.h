@@ -135,7 +135,8 @@ EMX_HD void finish_step(const Params &P, Track &t, StepOut &o) {
     }
 }
 
-template <int PT>
+// MAP: the magnetic field is non-uniform (evaluated at the stage positions of the integrator)
+template <int PT, bool MAP = false>
 EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
     const emx_physics &ph = P.ph;
     o.action = EMX_A_NONE;
@@ -225,7 +226,7 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
         const double q = (PT == kElectron) ? -1.0 : 1.0;
         const double kappa = q * kCB * P.Bmag / pm;
         bool susp;
-        s = propagate_field(P, vol, t.surf, t.x, t.u, kappa, s_phys, hit, fs, budget, susp);
+        s = propagate_field<MAP>(P, vol, t.surf, t.x, t.u, kappa, s_phys, hit, fs, budget, susp);
         if (susp) {  // x, u, surf and fs hold the progress; the step continues in the next iteration
             o.suspended = 1;
             return -1;
@@ -408,9 +409,9 @@ EMX_HD void step_interact(const Params &P, uint64_t seed, Track &t, StepOut &o, 
 }
 
 // the whole step in one call
-template <int PT>
+template <int PT, bool MAP = false>
 EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
-    const int proc = step_pre<PT>(P, seed, t, o, fs, budget);
+    const int proc = step_pre<PT, MAP>(P, seed, t, o, fs, budget);
     if (proc >= 0) step_interact<PT>(P, seed, t, o, proc);
 }
 

@@ -46,7 +46,7 @@ class StepResult(C.Structure):
                 ("n_draws", C.c_int32), ("null_int", C.c_int32), ("rest", C.c_int32)]
 
 
-EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "emx_add_volume", "emx_set_field",
+EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "emx_add_volume", "emx_set_field", "emx_set_field_fringe",
            "emx_get_physics", "emx_set_physics", "emx_set_cuts", "emx_build_tables", "emx_get_table",
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
            "emx_set_primary_offset", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
@@ -70,7 +70,7 @@ def lib():
         sig = {
             "emx_create": (i, [C.POINTER(vp)]), "emx_destroy": (None, [vp]),
             "emx_add_material": (i, [vp, i, vp, vp, vp, d, d]), "emx_add_surface": (i, [vp, i, d]),
-            "emx_add_volume": (i, [vp, i, vp, vp, i, i]), "emx_set_field": (i, [vp, d, d, d]),
+            "emx_add_volume": (i, [vp, i, vp, vp, i, i]), "emx_set_field": (i, [vp, d, d, d]), "emx_set_field_fringe": (i, [vp, d, d]),
             "emx_get_physics": (i, [vp, C.POINTER(Physics)]), "emx_set_physics": (i, [vp, C.POINTER(Physics)]),
             "emx_set_cuts": (i, [vp, i, d, d]), "emx_build_tables": (i, [vp, vp]),
             "emx_get_table": (i, [vp, i, i, vp, i]), "emx_get_material_info": (i, [vp, i, vp]),
@@ -149,6 +149,8 @@ class Problem:
             self._check(L.emx_add_volume(h, len(s), _hp(s), _hp(e), vol["material"], vol["tally"]))
         B = desc.get("field", (0.0, 0.0, 0.0))
         self._check(L.emx_set_field(h, float(B[0]), float(B[1]), float(B[2])))
+        if desc.get("field_fringe"):
+            self._check(L.emx_set_field_fringe(h, float(desc["field_fringe"][0]), float(desc["field_fringe"][1])))
         ph = Physics()
         for k, _ in Physics._fields_:
             setattr(ph, k, desc["physics"][k])

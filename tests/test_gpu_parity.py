@@ -111,7 +111,7 @@ def test_tables_match_the_oracle(emx, emo, cfg):
 
 # ---------------- level 2: single step ----------------
 
-@pytest.mark.parametrize("cfg,n", [(0, 20000), (1, 40000), (2, 40000), (3, 40000), (4, 40000), (5, 20000)])
+@pytest.mark.parametrize("cfg,n", [(0, 20000), (1, 40000), (2, 40000), (3, 40000), (4, 40000), (5, 20000), (6, 40000)])
 def test_single_step_parity(emx, emo, cfg, n):
     desc, _ = W.get(cfg, 4)
     G, O = emx.Problem(desc), emo.Problem(desc)
@@ -123,15 +123,18 @@ def test_single_step_parity(emx, emo, cfg, n):
     # field steps that end because the substep budget ran out (action TRUNC) return "whatever was travelled":
     # the sum of ~1000 adaptive substeps whose sizes depend on pow() of an ill-conditioned error estimate, so
     # they agree only to ~1e-9; they are compared separately and counted
-    field = cfg in (3, 4)
+    field = cfg in (3, 4, 6)
     trunc = (ref["action"] == 4) & (got["action"] == 4) & (np.array([t.ptype for t in tr]) != 0) & field
     n_bad, worst, rep = states.compare_steps(ref, got, E_in, skip=trunc)
     # level 1: action, process, secondary counts and ids, draw counts, cells: bit-exact.  States whose
     # outcome hinges on a comparison within rounding of equality may differ; they are counted (expected 0)
     assert n_bad <= (2 if field else 0), rep
     big = {k: v for k, v in rep.items() if isinstance(v, float) and v > 1e-13}
-    # level 2: 1e-12; multi-substep field steps accumulate up to ~100 substeps of rounding: 1e-11
-    assert worst <= (1e-11 if field else RTOL2), big
+    # level 2: 1e-12; multi-substep field steps accumulate up to ~100 substeps of rounding: 1e-11.  In the
+    # non-uniform field (config 6) the error estimate, and with it the sequence of substeps, varies along the
+    # path, so two runs of the same algorithm reach a boundary at points up to the landing tolerance
+    # field_eps = 1e-7 cm apart (|ds| / s ~ 1e-9 .. 1e-8, directions rotated by kappa ds): 1e-6
+    assert worst <= (1e-6 if cfg == 6 else 1e-11 if field else RTOL2), big
     if trunc.any():
         _, w2, rep2 = states.compare_steps(ref, got, E_in, skip=~trunc)
         assert w2 <= 1e-6, rep2
@@ -150,7 +153,7 @@ def _per_primary_se(o):
 
 
 @pytest.mark.parametrize("cfg,n,n_slots", [(0, 1000, 1024), (1, 300, 1 << 16), (2, 24, 1 << 16), (3, 24, 1 << 16),
-                                           (4, 48, 1 << 16), (1, 64, 1024), (5, 400, 1 << 16)])
+                                           (4, 48, 1 << 16), (1, 64, 1024), (5, 400, 1 << 16), (6, 48, 1 << 16)])
 def test_transport_parity_and_energy_closure(emx, emo, cfg, n, n_slots):
     desc, prim = W.get(cfg, n)
     G, O = emx.Problem(desc), emo.Problem(desc)
@@ -319,11 +322,33 @@ def test_kept_iteration_graph_is_dropped_when_an_argument_changes(emx):
     assert np.array_equal(d["steps"], a1["steps"])
 
 
+def test_fringe_field_changes_the_result_and_uniform_limit_does_not(emx):
+    """The fringe pushed out to |z| = 1e9 cm is the uniform field: same counters as config 4 (the stage-position
+    integrator then does the same arithmetic); the real fringe of config 6 gives other histories."""
+    d4, prim = W.get(4, 32)
+    d6, _ = W.get(6, 32)
+    far = dict(d6)
+    far["field_fringe"] = (1e9, 1.0)
+    kw = dict(n_slots=1 << 14, queue_capacity=1 << 20)
+    res = []
+    for desc in (d4, far, d6):
+        G = emx.Problem(desc)
+        res.append(G.transport(G.upload_primaries(prim), 4, **kw))
+    assert np.array_equal(res[0]["steps"], res[1]["steps"]) and np.array_equal(res[0]["inter"], res[1]["inter"])
+    assert np.allclose(res[0]["edep"], res[1]["edep"], rtol=1e-11, atol=1e-9)
+    assert not np.array_equal(res[0]["steps"], res[2]["steps"])
+    assert res[2]["edep"].sum() + res[2]["escaped"] + res[2]["looper"] == pytest.approx(res[2]["E_in"], rel=1e-9)
+
+
 def test_error_paths(emx):
     import ctypes as C
     L = emx.lib()
     h = C.c_void_p()
     assert L.emx_create(C.byref(h)) == 0
+    assert L.emx_set_field_fringe(h, 100.0, 15.0) == -1      # no field along z set
+    assert L.emx_set_field(h, 0.0, 1.0, 0.0) == 0 and L.emx_set_field_fringe(h, 100.0, 15.0) == -1
+    assert L.emx_set_field(h, 0.0, 0.0, 2.0) == 0 and L.emx_set_field_fringe(h, 100.0, -1.0) == -1
+    assert L.emx_set_field_fringe(h, 100.0, 15.0) == 0
     assert L.emx_add_surface(h, 9, 1.0) == -1
     assert L.emx_build_tables(h, None) == -2           # no volume
     assert b"volume" in L.emx_last_error(h)
