@@ -46,6 +46,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--primaries", type=int, default=0, help="0 = the config's full count")
+    ap.add_argument("--slots", type=int, default=0, help="track slots (0 = the config's: 2^20 for config 4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--shard", action="store_true",
@@ -56,6 +57,8 @@ def parse():
 
 def workload(args):
     desc, prim = W.get(args.config) if args.primaries <= 0 else W.get(args.config, args.primaries)
+    if getattr(args, "slots", 0) > 0:
+        desc = dict(desc, n_slots=int(args.slots))
     return desc, prim
 
 
