@@ -1,6 +1,7 @@
 """bench.py -- track-steps/s and primaries/s of the EM-shower step loop on B200 (BASELINE.json `metric`).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--primaries n] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--primaries n] [--slots s] [--shard]
+                    [--impl reference]
 
 One "step" = one pass of the whole hot path (refill, step kernels, secondaries, tallies, until no track is
 left) over one batch of synthetic primaries: by default the full BASELINE config 4 ("throughput stress":
@@ -8,7 +9,8 @@ barrel detector in a 4 T field, 100 000 primaries of 1-100 GeV, 2^20 track slots
 single-GPU configuration.  Inputs are seeded and synthetic (paper_2203_09467_b200/workloads.py).
 `value` is device-timed with the primaries already resident in HBM; `e2e` is the same metric through
 emx_transport_host with HOST buffers (uploads and the tally read-back inside the timed region).
-N > 1 (torchrun): independent replicas, one per GPU, different seeds ("replicas only").
+N > 1 (torchrun): independent replicas, one per GPU, different seeds (the default), or with
+--shard ONE workload cut by primaries over the ranks with a final all-reduce of the tallies (strong scaling).
 `--impl reference` times the oracle (plain fp64 C, oracle/) on the host cores on a bounded sample.
 """
 import argparse
