@@ -256,6 +256,24 @@ def test_hopelessly_small_workspace_is_an_error_not_a_hang(emx):
     assert ok["edep"].sum() + ok["escaped"] + ok["looper"] == pytest.approx(ok["E_in"], rel=1e-9)
 
 
+def test_transport_on_a_side_stream_is_ordered_after_the_work_queued_on_it(emx):
+    """The `stream` argument: primaries uploaded on a non-default torch stream are consumed by a transport on
+    that same stream without any synchronisation in between (the library's internal streams are ordered after
+    the caller's stream, and the caller's stream after them)."""
+    import torch
+    desc, prim = W.get(2, 12)
+    G = emx.Problem(desc)
+    ref = G.transport(G.upload_primaries(prim), desc["seed"], n_slots=1 << 13, queue_capacity=1 << 18)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        pd = G.upload_primaries(prim)
+        a = G.transport(pd, desc["seed"], n_slots=1 << 13, queue_capacity=1 << 18)
+        b = G.transport_host(prim, desc["seed"], n_slots=1 << 13, queue_capacity=1 << 18)
+    for r in (a, b):
+        assert np.array_equal(r["steps"], ref["steps"]) and np.array_equal(r["inter"], ref["inter"])
+        assert np.allclose(r["edep"], ref["edep"], rtol=1e-11, atol=1e-9)
+
+
 def test_results_do_not_depend_on_slots_or_host_entry(emx):
     desc, prim = W.get(2, 12)
     G = emx.Problem(desc)
