@@ -50,13 +50,15 @@ enum { EMO_P_COMPTON = 0, EMO_P_PHOTO = 1, EMO_P_PAIR = 2, EMO_P_MOLLER = 3,
 #define EMO_M_ANNIH 32u
 
 /* step limiter ("action") */
-enum { EMO_A_NONE = 0, EMO_A_DISCRETE = 1, EMO_A_LOSS = 2, EMO_A_BOUNDARY = 3, EMO_A_TRUNC = 4 };
+enum { EMO_A_NONE = 0, EMO_A_DISCRETE = 1, EMO_A_LOSS = 2, EMO_A_BOUNDARY = 3, EMO_A_TRUNC = 4,
+       EMO_A_MSC = 5 /* the multiple-scattering step limit (DESIGN.md R-MSC) */ };
 
 /* table kinds per material (each n_E doubles) */
 enum { EMO_T_COMPTON = 0, EMO_T_PHOTO, EMO_T_PAIR, EMO_T_MOLLER, EMO_T_BREMS_EM,
        EMO_T_DEDX_EM, EMO_T_RANGE_EM, EMO_T_BHABHA, EMO_T_BREMS_EP, EMO_T_ANNIH,
        EMO_T_DEDX_EP, EMO_T_RANGE_EP, EMO_T_PAIR_ELEM0, /* + element index */
-       EMO_NTABLE = EMO_T_PAIR_ELEM0 + EMO_MAX_ELEM };
+       EMO_T_MSC = EMO_T_PAIR_ELEM0 + EMO_MAX_ELEM,     /* 1/lambda_1, inverse first transport mean free path of e+- */
+       EMO_NTABLE };
 
 /* surface types */
 enum { EMO_S_PX = 0, EMO_S_PY = 1, EMO_S_PZ = 2, EMO_S_CZ = 3 };
@@ -100,6 +102,9 @@ typedef struct {
     double vacuum_step;          /* cm */
     int max_steps;               /* per track */
     int deposit_e_at_creation;   /* config 0: every e- is deposited at birth */
+    int msc;                     /* 1: multiple scattering of e+- (DESIGN.md R-MSC) */
+    double msc_fr;               /* step limit s <= max(msc_fr * max(R, lambda_1), msc_smin) */
+    double msc_smin;             /* cm */
 } emo_physics;
 
 typedef struct {
@@ -135,6 +140,7 @@ typedef struct {
     double below_cut;            /* part of edep that came from tracking-cut kills/births */
     double escaped, looper;
     double s;                    /* step length travelled */
+    double msc_tau;              /* path length / lambda_1 used for the deflection of this step (0: none) */
     int n_draws;                 /* uniform draws consumed */
     int null_int;                /* 1 if the discrete interaction was kinematically null */
     int rest;                    /* 1 if an e+ annihilated at rest in this step */
@@ -169,6 +175,10 @@ double emo_brems_Sigma(double T, double kc, double X0); /* 1/cm */
 double emo_brems_dedx(double T, double kc, double X0);  /* MeV/cm */
 double emo_dedx_col(const emo_material *m, int ptype, double T, double Tcut); /* MeV/cm; Tcut<=0: unrestricted */
 void   emo_gauss_legendre(int n, double *x, double *w); /* nodes/weights on [-1,1] */
+/* multiple scattering (DESIGN.md R-MSC) */
+double emo_msc_screening(int Z, double T);              /* Moliere screening parameter A */
+double emo_msc_sigma1(int Z, double Amass, double T);   /* first transport cross section, cm2 per atom */
+double emo_msc_one_minus_mu(double tau, double xi);     /* 1 - cos(theta) of a step of s = tau * lambda_1 */
 
 /* ---- problem.c ---- */
 emo_problem *emo_create(void);
@@ -219,6 +229,7 @@ int  emo_moller(emo_rng *r, double T, double Tcut, const double u[3], double *Td
 int  emo_bhabha(emo_rng *r, double T, double Tcut, const double u[3], double *Td, double ud[3], double *T1, double u1[3]);
 void emo_annih_flight(emo_rng *r, double T, const double u[3], double *k1, double u1[3], double *k2, double u2[3]);
 void emo_annih_rest(emo_rng *r, double u1[3], double u2[3]);
+void emo_msc_deflect(emo_rng *r, double tau, const double u[3], double out[3]);
 
 /* ---- transport.c ---- */
 void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step_result *out);

@@ -13,7 +13,7 @@ from . import build as _build
 
 MAX_ELEM, MAX_FACES, NPROC, PER_PRIM, NHIST = 4, 8, 8, 11, 96
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
-           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3"]
+           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc"]
 T = {n: i for i, n in enumerate(T_NAMES)}
 ME = 0.51099895000
 
@@ -22,7 +22,8 @@ class Physics(C.Structure):
     _fields_ = [("process_mask", C.c_uint), ("E_min", C.c_double), ("E_max", C.c_double), ("n_E", C.c_int),
                 ("E_trk", C.c_double), ("prod_cut_cm", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("lin_loss", C.c_double), ("field_eps", C.c_double), ("max_substeps", C.c_int),
-                ("vacuum_step", C.c_double), ("max_steps", C.c_int), ("deposit_e_at_creation", C.c_int)]
+                ("vacuum_step", C.c_double), ("max_steps", C.c_int), ("deposit_e_at_creation", C.c_int),
+                ("msc", C.c_int), ("msc_fr", C.c_double), ("msc_smin", C.c_double)]
 
 
 class Track(C.Structure):
@@ -35,7 +36,7 @@ class StepResult(C.Structure):
     _fields_ = [("trk", Track), ("action", C.c_int), ("process", C.c_int), ("n_sec", C.c_int),
                 ("sec", Track * 4), ("sec_ord", C.c_int * 4), ("edep", C.c_double), ("edep_vol", C.c_int),
                 ("below_cut", C.c_double), ("escaped", C.c_double), ("looper", C.c_double), ("s", C.c_double),
-                ("n_draws", C.c_int), ("null_int", C.c_int), ("rest", C.c_int)]
+                ("msc_tau", C.c_double), ("n_draws", C.c_int), ("null_int", C.c_int), ("rest", C.c_int)]
 
 
 class Rng(C.Structure):
@@ -68,6 +69,8 @@ def lib():
             "emo_moller_dcs": (d, [d, d]), "emo_bhabha_dcs": (d, [d, d]),
             "emo_brems_Sigma": (d, [d, d, d]), "emo_brems_dedx": (d, [d, d, d]),
             "emo_gauss_legendre": (None, [i, dp, dp]),
+            "emo_msc_screening": (d, [i, d]), "emo_msc_sigma1": (d, [i, d, d]), "emo_msc_one_minus_mu": (d, [d, d]),
+            "emo_msc_deflect": (None, [C.POINTER(Rng), d, dp, dp]),
             "emo_create": (p, []), "emo_destroy": (None, [p]),
             "emo_add_material": (i, [p, i, ip, dp, dp, d, d]), "emo_add_surface": (i, [p, i, d]),
             "emo_add_volume": (i, [p, i, ip, ip, i, i]), "emo_set_field": (i, [p, d, d, d]), "emo_set_field_fringe": (i, [p, d, d]),

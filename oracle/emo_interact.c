@@ -224,3 +224,14 @@ void emo_annih_rest(emo_rng *r, double u1[3], double u2[3]) {
     u1[0] = s * cos(phi); u1[1] = s * sin(phi); u1[2] = mu;
     u2[0] = -u1[0]; u2[1] = -u1[1]; u2[2] = -u1[2];
 }
+
+/* ---- multiple-scattering deflection (DESIGN.md R-MSC) ----
+ * tau = path length in units of the first transport mean free path.  Draws: xi_1 (polar), xi_2 (azimuth).
+ * The sine comes from t = 1 - mu as sqrt(t (2 - t)), never from sqrt(1 - mu^2). */
+void emo_msc_deflect(emo_rng *r, double tau, const double u[3], double out[3]) {
+    double x1 = emo_next(r), x2 = emo_next(r);
+    double t = emo_msc_one_minus_mu(tau, x1);
+    double s2 = t * (2.0 - t);
+    double phi = 2.0 * EMO_PI * x2;
+    rotate_cs(u, 1.0 - t, s2 > 0.0 ? sqrt(s2) : 0.0, cos(phi), sin(phi), out);
+}

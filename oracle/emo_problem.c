@@ -18,6 +18,7 @@ emo_problem *emo_create(void) {
     ph->alpha_R = 0.2; ph->rho_R = 0.1; ph->lin_loss = 0.01;
     ph->field_eps = 1e-7; ph->max_substeps = 1000; ph->vacuum_step = 1e3;
     ph->max_steps = 10000; ph->deposit_e_at_creation = 0;
+    ph->msc = 0; ph->msc_fr = 0.2; ph->msc_smin = 1e-3;
     return p;
 }
 
@@ -94,6 +95,7 @@ int emo_set_field_fringe(emo_problem *p, double z0_cm, double a_cm) {
 
 int emo_set_physics(emo_problem *p, const emo_physics *ph) {
     if (ph->n_E < 2 || !(ph->E_max > ph->E_min) || !(ph->E_min > 0.0)) return -1;
+    if (ph->msc && (!(ph->msc_fr > 0.0) || !(ph->msc_smin > 0.0))) return -1;
     p->ph = *ph; p->built = 0;
     return 0;
 }
@@ -199,6 +201,11 @@ int emo_build_tables(emo_problem *p) {
                 double s = emo_brems_Sigma(E, m->kcut, m->X0);
                 T[EMO_T_BREMS_EM * n + j] = s;
                 T[EMO_T_BREMS_EP * n + j] = s;
+            }
+            if (ph->msc) {                                 /* 1/lambda_1 = sum_i n_i sigma_1(Z_i, E) (R-MSC) */
+                double s = 0.0;
+                for (int i = 0; i < m->n_elem; ++i) s += m->n_i[i] * emo_msc_sigma1(m->Z[i], m->A[i], E);
+                T[EMO_T_MSC * n + j] = s;
             }
             T[EMO_T_DEDX_EM * n + j] = dedx_total(m, EMO_ELECTRON, E, m->Tcut, m->kcut);
             T[EMO_T_DEDX_EP * n + j] = dedx_total(m, EMO_POSITRON, E, m->Tcut, m->kcut);

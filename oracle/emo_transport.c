@@ -68,6 +68,8 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
     if (t->E < ph->E_trk) { kill_below(&c, t->E); out->n_draws = (int)c.rng.n; return; }
 
     double Sig[3] = {0, 0, 0}, Stot = 0.0, D = 0.0, R = 0.0, s_phys, s_loss = INFINITY;
+    const int msc = (ph->msc && pt != EMO_GAMMA && mat >= 0);   /* multiple scattering applies (R-MSC) */
+    double iL0 = 0.0;                                            /* 1/lambda_1 at the pre-step energy */
     int nproc = 0, procs[3] = {-1, -1, -1};
     int action;
     const double E = t->E;
@@ -104,6 +106,14 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
             if (R <= ph->rho_R) s_loss = R;
             else s_loss = ph->alpha_R * R + ph->rho_R * (1.0 - ph->alpha_R) * (2.0 - ph->rho_R / R);
             if (s_loss < s_phys) { s_phys = s_loss; action = EMO_A_LOSS; }
+        }
+        if (msc) {
+            /* R-MSC step limit: s <= max(f_r max(R, lambda_1), s_min) */
+            iL0 = emo_lookup(p, mat, EMO_T_MSC, E);
+            double big = (iL0 > 0.0 && 1.0 / iL0 > R) ? 1.0 / iL0 : R;
+            double s_msc = ph->msc_fr * big;
+            if (s_msc < ph->msc_smin) s_msc = ph->msc_smin;
+            if (s_msc < s_phys) { s_phys = s_msc; action = EMO_A_MSC; }
         }
     }
 
@@ -157,6 +167,17 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
         t->vol = nv;
     } else {
         t->surf = -1;
+    }
+
+    /* 7b. multiple-scattering deflection at the end of the step (R-MSC): <cos> = exp(-Int ds / lambda_1), the
+     * integral by the trapezoid rule over the pre-step and post-loss energies; two draws, always consumed */
+    if (msc) {
+        double iL1 = emo_lookup(p, mat, EMO_T_MSC, t->E);
+        double tau = 0.5 * (iL0 + iL1) * s;
+        double u1[3];
+        emo_msc_deflect(&c.rng, tau, t->u, u1);
+        t->u[0] = u1[0]; t->u[1] = u1[1]; t->u[2] = u1[2];
+        out->msc_tau = tau;
     }
 
     /* 8. discrete */

@@ -211,3 +211,48 @@ double emo_dedx_col(const emo_material *m, int ptype, double T, double Tcut) {
     if (del < 0.0) del = 0.0;
     return 2.0 * EMO_PI * EMO_RE * EMO_RE * EMO_ME * m->n_e / b2 * (lg + F - del);
 }
+
+/* ---- multiple scattering of e+- (PAPER.md:111 names Urban / WentzelVI, "in progress", no formulas;
+ * DESIGN.md R-MSC is the reading) ----
+ * Single elastic scattering: screened Rutherford (Wentzel) per atom,
+ *   dsigma/dOmega = Z (Z + 1) r_e^2 (m_e c^2 / (beta p c))^2 / (1 - cos(theta) + 2 A)^2
+ * (Z + 1 instead of Z: scattering off the atomic electrons), with Moliere's screening parameter
+ *   A = (hbar / (2 p a_TF))^2 (1.13 + 3.76 (alpha Z / beta)^2),  a_TF = 0.88534 a_0 Z^(-1/3),
+ * i.e. hbar / (p a_TF) = alpha Z^(1/3) m_e c^2 / (0.88534 p c). */
+double emo_msc_screening(int Z, double T) {
+    double pc2 = T * (T + 2.0 * EMO_ME);                 /* (p c)^2 */
+    double Et = T + EMO_ME;
+    double beta2 = pc2 / (Et * Et);
+    double h = EMO_ALPHA * cbrt((double)Z) * EMO_ME / 0.88534;
+    double az = EMO_ALPHA * Z;
+    return 0.25 * h * h / pc2 * (1.13 + 3.76 * az * az / beta2);
+}
+
+/* first transport cross section sigma_1 = Int (1 - cos(theta)) dsigma over 0 <= t = 1 - cos(theta) <= t_m.
+ * The finite nucleus ends the Rutherford law at theta_max = hbar / (p R_N), R_N = 1.4 fm A^(1/3) (the sharp
+ * cutoff of the textbook treatment, Jackson section 13.6): t_m = min(2, theta_max^2 / 2).  With
+ * Int_0^t_m t / (t + 2A)^2 dt = ln(1 + t_m / (2A)) - t_m / (t_m + 2A):
+ *   sigma_1 = 2 pi Z (Z + 1) r_e^2 (m_e c^2 / (beta p c))^2 (ln(1 + t_m / (2A)) - t_m / (t_m + 2A)) */
+double emo_msc_sigma1(int Z, double Amass, double T) {
+    double pc2 = T * (T + 2.0 * EMO_ME);
+    double bpc = pc2 / (T + EMO_ME);                     /* beta p c */
+    double A = emo_msc_screening(Z, T);
+    double c = EMO_RE * EMO_ME / bpc;
+    double lam = EMO_RE * EMO_ME / EMO_ALPHA;            /* hbar c, MeV cm */
+    double RN = 1.4e-13 * cbrt(Amass);
+    double tm = 0.5 * lam * lam / (pc2 * RN * RN);
+    if (tm > 2.0) tm = 2.0;
+    return 2.0 * EMO_PI * (double)Z * (Z + 1.0) * c * c * (log1p(tm / (2.0 * A)) - tm / (tm + 2.0 * A));
+}
+
+/* Deflection after a path s = tau lambda_1: Lewis' theory gives <cos(theta)> = exp(-tau) exactly; the angle is
+ * drawn from the Henyey-Greenstein density p(mu) ~ (1 - g^2) / (1 + g^2 - 2 g mu)^(3/2), whose mean cosine is
+ * g, with g = exp(-tau).  Inverse of its distribution function, xi = F(mu), written for 1 - mu so that nothing
+ * cancels as g -> 1:  a = 1 - g,  S = (1 + g) a / (a + 2 g xi),  1 - mu = a (1 - xi) (S + a) / (a + 2 g xi). */
+double emo_msc_one_minus_mu(double tau, double xi) {
+    double g = exp(-tau), a = -expm1(-tau);
+    double den = a + 2.0 * g * xi;
+    double S = (1.0 + g) * a / den;
+    double t = a * (1.0 - xi) * (S + a) / den;
+    return t < 0.0 ? 0.0 : (t > 2.0 ? 2.0 : t);
+}
