@@ -84,6 +84,7 @@ extern "C" {
 #define EMX_A_LOSS 2
 #define EMX_A_BOUNDARY 3
 #define EMX_A_TRUNC 4 /* vacuum step cap / field substeps exhausted */
+#define EMX_A_MSC 5   /* multiple-scattering step limit (emx_physics.msc) */
 
 /* table kinds per material, each n_E doubles on the log grid */
 #define EMX_T_COMPTON 0
@@ -99,7 +100,8 @@ extern "C" {
 #define EMX_T_DEDX_EP 10
 #define EMX_T_RANGE_EP 11
 #define EMX_T_PAIR_ELEM0 12 /* + element index: n_i * sigma_pair(Z_i) for element selection */
-#define EMX_NTABLE (EMX_T_PAIR_ELEM0 + EMX_MAX_ELEM)
+#define EMX_T_MSC (EMX_T_PAIR_ELEM0 + EMX_MAX_ELEM) /* 1 / lambda_1: inverse first transport mean free path of e+-, 1/cm */
+#define EMX_NTABLE (EMX_T_MSC + 1)
 
 typedef struct emx_problem emx_problem; /* opaque, owned by the library */
 
@@ -118,6 +120,14 @@ typedef struct {
     double vacuum_step;         /* cm: step cap in vacuum */
     int32_t max_steps;          /* per track; then the track is killed into looper_lost */
     int32_t deposit_e_at_creation; /* 1: every e- is deposited where it is born (BASELINE configs[0]) */
+    /* Multiple scattering of e+- (Table 2: "Multiple scattering: Urban, WentzelVI", in progress
+     * there, no formula printed; DESIGN.md R-MSC).  msc = 1: 1/lambda_1 is tabulated from the screened-Rutherford
+     * transport cross section (Moliere screening, nuclear-size cutoff); a step of e+- in matter is limited to
+     * max(msc_fr * max(range, lambda_1), msc_smin) and ends with a deflection drawn from the Henyey-Greenstein
+     * law of mean cosine exp(-s (1/lambda_1(E) + 1/lambda_1(E')) / 2) (two draws, taken right after draw 0). */
+    int32_t msc;
+    double msc_fr;              /* > 0 */
+    double msc_smin;            /* cm, > 0 */
 } emx_physics;
 
 /* run totals (PAPER.md:176 energy deposition; Fig. 5 diagnostics PAPER.md:204-212) */
@@ -154,6 +164,7 @@ typedef struct {
     double below_cut;       /* part of edep from tracking-cut kills / births */
     double escaped, looper;
     double s;               /* step length travelled, cm */
+    double msc_tau;         /* path length / lambda_1 behind this step's multiple-scattering deflection (0: none) */
     int32_t n_draws;        /* uniforms consumed */
     int32_t null_int;
     int32_t rest;           /* e+ annihilated at rest in this step */

@@ -281,6 +281,8 @@ int emx_set_physics(emx_problem *p, const emx_physics *ph) {
     if (ph->n_E < 2 || !(ph->E_max > ph->E_min) || !(ph->E_min > 0.0) || ph->max_steps < 1 || ph->max_substeps < 1 ||
         !(ph->field_eps > 0.0) || !(ph->vacuum_step > 0.0))
         return fail(p, EMX_E_ARG, "emx_set_physics: invalid grid or limits");
+    if (ph->msc && (!(ph->msc_fr > 0.0) || !(ph->msc_smin > 0.0)))
+        return fail(p, EMX_E_ARG, "emx_set_physics: multiple scattering needs msc_fr > 0 and msc_smin > 0");
     p->hp.ph = *ph;
     p->hp.built = false;
     return EMX_OK;

@@ -47,12 +47,22 @@ EMX_HD void step_one(const Params &P, uint64_t seed, const emx_track &in, emx_st
     fs.attempt = 0;
     const int whole = P.ph.max_substeps;  // the hook runs the whole step in one call
     if (in.ptype == kGamma) step<kGamma>(P, seed, t, o, fs, whole);
-    else if (P.field_kind == 0) {
-        if (in.ptype == kElectron) step<kElectron>(P, seed, t, o, fs, whole);
-        else step<kPositron>(P, seed, t, o, fs, whole);
+    else if (!P.ph.msc) {
+        if (P.field_kind == 0) {
+            if (in.ptype == kElectron) step<kElectron>(P, seed, t, o, fs, whole);
+            else step<kPositron>(P, seed, t, o, fs, whole);
+        } else {
+            if (in.ptype == kElectron) step<kElectron, true>(P, seed, t, o, fs, whole);
+            else step<kPositron, true>(P, seed, t, o, fs, whole);
+        }
     } else {
-        if (in.ptype == kElectron) step<kElectron, true>(P, seed, t, o, fs, whole);
-        else step<kPositron, true>(P, seed, t, o, fs, whole);
+        if (P.field_kind == 0) {
+            if (in.ptype == kElectron) step<kElectron, false, true>(P, seed, t, o, fs, whole);
+            else step<kPositron, false, true>(P, seed, t, o, fs, whole);
+        } else {
+            if (in.ptype == kElectron) step<kElectron, true, true>(P, seed, t, o, fs, whole);
+            else step<kPositron, true, true>(P, seed, t, o, fs, whole);
+        }
     }
 
     put3(r.trk.x, t.x);
@@ -92,6 +102,7 @@ EMX_HD void step_one(const Params &P, uint64_t seed, const emx_track &in, emx_st
     r.escaped = o.escaped;
     r.looper = o.looper;
     r.s = o.s;
+    r.msc_tau = o.msc_tau;
     r.n_draws = o.n_draws;
     r.null_int = o.null_int;
     r.rest = o.rest;

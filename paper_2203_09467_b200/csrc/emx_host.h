@@ -38,6 +38,9 @@ struct HostProblem {
         ph.vacuum_step = 1e3;
         ph.max_steps = 10000;
         ph.deposit_e_at_creation = 0;
+        ph.msc = 0;
+        ph.msc_fr = 0.2;
+        ph.msc_smin = 1e-3;
     }
 };
 

@@ -49,6 +49,26 @@ EMX_HD double clamp1(double m) { return m > 1.0 ? 1.0 : (m < -1.0 ? -1.0 : m); }
 // exact inverse CDF of p(mu) ~ (1 - beta mu)^-2 (R30)
 EMX_HD double boosted_iso(double xi, double beta) { return clamp1((2.0 * xi - 1.0 + beta) / (beta * (2.0 * xi - 1.0) + 1.0)); }
 
+// ---- multiple-scattering deflection after a path of tau transport mean free paths (R-MSC): polar angle from
+// the Henyey-Greenstein law with mean cosine g = exp(-tau) (Lewis: <cos> = exp(-tau) exactly), azimuth uniform.
+// Inverse distribution function written for t = 1 - mu so that nothing cancels as g -> 1:
+//   a = 1 - g, S = (1 + g) a / (a + 2 g xi), t = a (1 - xi) (S + a) / (a + 2 g xi).   Draws: polar, azimuth.
+EMX_HD double msc_one_minus_mu(double tau, double xi) {
+    const double g = m_exp(-tau), a = -expm1(-tau);
+    const double den = a + 2.0 * g * xi;
+    const double S = (1.0 + g) * a / den;
+    const double t = a * (1.0 - xi) * (S + a) / den;
+    return t < 0.0 ? 0.0 : (t > 2.0 ? 2.0 : t);
+}
+EMX_NI Vec3 msc_deflect(Rng &r, double tau, const Vec3 &u) {
+    const double x1 = r.next(), x2 = r.next();
+    const double t = msc_one_minus_mu(tau, x1);
+    const double s2 = t * (2.0 - t);
+    double sp, cp;
+    sincos_(2.0 * kPi * x2, sp, cp);
+    return rotate(u, 1.0 - t, s2 > 0.0 ? sqrt(s2) : 0.0, cp, sp);
+}
+
 // ---- Compton, Klein-Nishina (C6.1): photon E -> E1 along u1, electron Te along ue
 EMX_NI void compton(Rng &r, double E, const Vec3 &u, double &E1, Vec3 &u1, double &Te, Vec3 &ue) {
     const double k = E / kMe;

@@ -35,6 +35,7 @@ struct StepOut {
     int rest_alloc;      // at-rest annihilation photons allocated (ordinals 2, 3), directions +-rest_u
     Vec3 rest_u;
     double edep, below_cut, escaped, looper, s;
+    double msc_tau;      // path / lambda_1 of this step's multiple-scattering deflection (level-2 hook)
     int n_draws, null_int, rest;
     int suspended;       // field propagation parked for the next iteration: nothing else of the step happened
 };
@@ -136,7 +137,9 @@ EMX_HD void finish_step(const Params &P, Track &t, StepOut &o) {
 }
 
 // MAP: the magnetic field is non-uniform (evaluated at the stage positions of the integrator)
-template <int PT, bool MAP = false>
+// MSC: multiple scattering of e+- is switched on (emx_physics.msc; its own instantiation, so that the kernels
+// of a problem without it carry none of its registers)
+template <int PT, bool MAP = false, bool MSC = false>
 EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
     const emx_physics &ph = P.ph;
     o.action = EMX_A_NONE;
@@ -145,6 +148,7 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
     o.s1.ptype = -1;
     o.rest_alloc = 0;
     o.edep = o.below_cut = o.escaped = o.looper = o.s = 0.0;
+    o.msc_tau = 0.0;
     o.n_draws = o.null_int = o.rest = 0;
     o.suspended = 0;
     Rng rng;
@@ -160,6 +164,8 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
     }
 
     double Sig0 = 0.0, Sig1 = 0.0, Sig2 = 0.0, Stot = 0.0, D = 0.0, R = 0.0, s_phys;
+    const bool msc = MSC && (PT != kGamma) && mat >= 0;     // multiple scattering applies (R-MSC)
+    double iL0 = 0.0;                                       // 1 / lambda_1 at the pre-step energy
     const double *Rtab = nullptr;
     int action;
     const double E = t.E;
@@ -200,6 +206,16 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
             if (s_loss < s_phys) {
                 s_phys = s_loss;
                 action = EMX_A_LOSS;
+            }
+            if (msc) {  // R-MSC step limit: s <= max(f_r max(R, lambda_1), s_min)
+                iL0 = interp(table(P, mat, EMX_T_MSC), g);
+                const double big = (iL0 > 0.0 && 1.0 / iL0 > R) ? 1.0 / iL0 : R;
+                double s_msc = ph.msc_fr * big;
+                if (s_msc < ph.msc_smin) s_msc = ph.msc_smin;
+                if (s_msc < s_phys) {
+                    s_phys = s_msc;
+                    action = EMX_A_MSC;
+                }
             }
         }
     }
@@ -280,6 +296,15 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
         t.surf = -1;
     }
 
+    // 7b. multiple-scattering deflection at the end of the step (R-MSC): <cos> = exp(-Int ds / lambda_1), the
+    // integral by the trapezoid rule over the pre-step and post-loss energies; draws 1 and 2, always consumed
+    if (msc) {
+        const double iL1 = interp(table(P, mat, EMX_T_MSC), grid_pos(P, t.E));
+        const double tau = 0.5 * (iL0 + iL1) * s;
+        t.u = msc_deflect(rng, tau, t.u);
+        o.msc_tau = tau;
+    }
+
     // 8. discrete interaction: select with the pre-step cross sections, interact at the post-loss energy (R21)
     if (action == EMX_A_DISCRETE) {
         const double target = rng.next() * Stot;
@@ -313,8 +338,10 @@ EMX_HD void step_interact(const Params &P, uint64_t seed, Track &t, StepOut &o, 
     const emx_physics &ph = P.ph;
     Rng rng;
     rng.init(seed, t.prim, t.tid, t.step);
-    rng.n = 2u;  // draws 0 (interaction length) and 1 (process selection) were used by step_pre
     const int mat = P.vol[t.vol].material;
+    // draws 0 (interaction length) and 1 (process selection) were used by step_pre, and two more in between
+    // by the multiple-scattering deflection of an e+- (R-MSC)
+    rng.n = (PT != kGamma && ph.msc) ? 4u : 2u;
     const Material &m = P.mat[mat];
     const double E1 = t.E;
     const Vec3 u0 = t.u;
@@ -409,9 +436,9 @@ EMX_HD void step_interact(const Params &P, uint64_t seed, Track &t, StepOut &o, 
 }
 
 // the whole step in one call
-template <int PT, bool MAP = false>
+template <int PT, bool MAP = false, bool MSC = false>
 EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
-    const int proc = step_pre<PT, MAP>(P, seed, t, o, fs, budget);
+    const int proc = step_pre<PT, MAP, MSC>(P, seed, t, o, fs, budget);
     if (proc >= 0) step_interact<PT>(P, seed, t, o, proc);
 }
 

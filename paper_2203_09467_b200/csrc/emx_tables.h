@@ -105,6 +105,10 @@ EMX_HD void table_pass3(const TableCtx &c, int im, int j) {
     const double sb = (mask & EMX_M_BREMS) ? brems_Sigma(E, m.kcut, m.X0) : 0.0;
     T[EMX_T_BREMS_EM * n + j] = sb;
     T[EMX_T_BREMS_EP * n + j] = sb;
+    double il = 0.0;  // 1 / lambda_1 = sum_i n_i sigma_1(Z_i) (R-MSC)
+    if (c.ph.msc)
+        for (int i = 0; i < m.n_elem; ++i) il += m.n_i[i] * msc_sigma1(m.Z[i], m.A[i], E);
+    T[EMX_T_MSC * n + j] = il;
     T[EMX_T_DEDX_EM * n + j] = dedx_total(m, kElectron, E, m.Tcut, m.kcut);
     T[EMX_T_DEDX_EP * n + j] = dedx_total(m, kPositron, E, m.Tcut, m.kcut);
     T[EMX_T_RANGE_EM * n + j] = range_bin(c, m, kElectron, m.Tcut, m.kcut, j);

@@ -172,6 +172,32 @@ EMX_HD double dedx_col(const Material &m, int ptype, double T, double Tcut) {
     return 2.0 * kPi * kRe * kRe * kMe * m.n_e / b2 * (lg + F - del);
 }
 
+// ---- multiple scattering of e+- (DESIGN.md R-MSC; PAPER.md:111 names the models, prints no formula) ----
+// Screened Rutherford law per atom, dsigma/dOmega = Z (Z + 1) re^2 (me / (beta p))^2 / (t + 2 A)^2 with
+// t = 1 - cos(theta); Moliere: 4 A = chi_0^2 (1.13 + 3.76 (alpha Z / beta)^2), chi_0 = hbar / (p a_TF),
+// a_TF = 0.88534 a_0 Z^(-1/3).  Lengths via hbar c = re me / alpha and a_0 = re / alpha^2.
+EMX_HD double msc_screening(int Z, double T) {
+    const double p2 = T * (T + 2.0 * kMe);
+    const double inv_beta2 = (T + kMe) * (T + kMe) / p2;
+    const double az = kAlpha * (double)Z;
+    const double chi0 = kAlpha * kMe * cbrt((double)Z) / (0.88534 * sqrt(p2));
+    return 0.25 * chi0 * chi0 * (1.13 + 3.76 * az * az * inv_beta2);
+}
+// first transport cross section, cm2 per atom: the law integrated with weight t up to
+// t_m = min(2, theta_max^2 / 2), theta_max = hbar / (p R_N), R_N = 1.4e-13 cm A^(1/3) (finite nucleus):
+//   sigma_1 = 2 pi Z (Z + 1) (re me / (beta p))^2 (ln(1 + t_m / 2A) - t_m / (t_m + 2A))
+EMX_HD double msc_sigma1(int Z, double Amass, double T) {
+    const double p2 = T * (T + 2.0 * kMe);
+    const double A2 = 2.0 * msc_screening(Z, T);
+    const double hbarc = kRe * kMe / kAlpha;
+    const double th_max = hbarc / (sqrt(p2) * 1.4e-13 * cbrt(Amass));
+    double tm = 0.5 * th_max * th_max;
+    if (tm > 2.0) tm = 2.0;
+    const double c = kRe * kMe * (T + kMe) / p2;
+    const double zz = (double)Z;
+    return 2.0 * kPi * zz * (zz + 1.0) * c * c * (log1p(tm / A2) - tm / (tm + A2));
+}
+
 EMX_HD double dedx_total(const Material &m, int ptype, double T, double Tcut, double kcut) {
     return dedx_col(m, ptype, T, Tcut) + brems_dedx(T, kcut, m.X0);
 }

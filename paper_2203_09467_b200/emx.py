@@ -13,9 +13,9 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("EMX_LIB_PATH") or os.path.join(HERE, "libemx.so")   # override: kernel experiments
-MAX_ELEM, MAX_FACES, NPROC, NTABLE, NHIST = 4, 8, 8, 16, 96
+MAX_ELEM, MAX_FACES, NPROC, NTABLE, NHIST = 4, 8, 8, 17, 96
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
-           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3"]
+           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc"]
 T = {n: i for i, n in enumerate(T_NAMES)}
 
 
@@ -23,7 +23,8 @@ class Physics(C.Structure):
     _fields_ = [("process_mask", C.c_uint32), ("E_min", C.c_double), ("E_max", C.c_double), ("n_E", C.c_int32),
                 ("E_trk", C.c_double), ("prod_cut_cm", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("lin_loss", C.c_double), ("field_eps", C.c_double), ("max_substeps", C.c_int32),
-                ("vacuum_step", C.c_double), ("max_steps", C.c_int32), ("deposit_e_at_creation", C.c_int32)]
+                ("vacuum_step", C.c_double), ("max_steps", C.c_int32), ("deposit_e_at_creation", C.c_int32),
+                ("msc", C.c_int32), ("msc_fr", C.c_double), ("msc_smin", C.c_double)]
 
 
 class Scalars(C.Structure):
@@ -43,7 +44,7 @@ class StepResult(C.Structure):
     _fields_ = [("trk", Track), ("action", C.c_int32), ("process", C.c_int32), ("n_sec", C.c_int32),
                 ("sec", Track * 4), ("sec_ord", C.c_int32 * 4), ("edep", C.c_double), ("edep_vol", C.c_int32),
                 ("below_cut", C.c_double), ("escaped", C.c_double), ("looper", C.c_double), ("s", C.c_double),
-                ("n_draws", C.c_int32), ("null_int", C.c_int32), ("rest", C.c_int32)]
+                ("msc_tau", C.c_double), ("n_draws", C.c_int32), ("null_int", C.c_int32), ("rest", C.c_int32)]
 
 
 EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "emx_add_volume", "emx_set_field", "emx_set_field_fringe",

@@ -91,9 +91,19 @@ def test_refill_compaction_order_is_bit_exact(emx, n_live, capacity, n_queue, p_
 
 # ---------------- tables ----------------
 
-@pytest.mark.parametrize("cfg", [0, 1, 2, 4])
+def _workload(cfg, n):
+    """W.get, plus 37 = config 3 (calorimeter in a 1 T field) with multiple scattering switched on and 47 = config 4
+    (barrel, 4 T) with it: the deflection at the end of a curved step"""
+    if cfg in (37, 47):
+        desc, prim = W.get(cfg // 10, n)
+        desc = dict(desc, physics=dict(desc["physics"], msc=1, msc_fr=0.2, msc_smin=1e-3), seed=cfg)
+        return desc, prim
+    return W.get(cfg, n)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 4, 7, 47])
 def test_tables_match_the_oracle(emx, emo, cfg):
-    desc, _ = W.get(cfg, 4)
+    desc, _ = _workload(cfg, 4)
     G, O = emx.Problem(desc), emo.Problem(desc)
     worst = 0.0
     for im in range(len(desc["materials"])):
@@ -111,9 +121,10 @@ def test_tables_match_the_oracle(emx, emo, cfg):
 
 # ---------------- level 2: single step ----------------
 
-@pytest.mark.parametrize("cfg,n", [(0, 20000), (1, 40000), (2, 40000), (3, 40000), (4, 40000), (5, 20000), (6, 40000)])
+@pytest.mark.parametrize("cfg,n", [(0, 20000), (1, 40000), (2, 40000), (3, 40000), (4, 40000), (5, 20000), (6, 40000),
+                                   (7, 40000), (37, 40000), (47, 40000)])
 def test_single_step_parity(emx, emo, cfg, n):
-    desc, _ = W.get(cfg, 4)
+    desc, _ = _workload(cfg, 4)
     G, O = emx.Problem(desc), emo.Problem(desc)
     tr = states.random_states(emo, O, desc, n, seed=1000 + cfg)
     ref = states.result_arrays(O.step_batch(tr, desc["seed"]))
@@ -123,7 +134,7 @@ def test_single_step_parity(emx, emo, cfg, n):
     # field steps that end because the substep budget ran out (action TRUNC) return "whatever was travelled":
     # the sum of ~1000 adaptive substeps whose sizes depend on pow() of an ill-conditioned error estimate, so
     # they agree only to ~1e-9; they are compared separately and counted
-    field = cfg in (3, 4, 6)
+    field = cfg in (3, 4, 6, 37, 47)
     trunc = (ref["action"] == 4) & (got["action"] == 4) & (np.array([t.ptype for t in tr]) != 0) & field
     n_bad, worst, rep = states.compare_steps(ref, got, E_in, skip=trunc)
     # level 1: action, process, secondary counts and ids, draw counts, cells: bit-exact.  States whose
@@ -140,8 +151,13 @@ def test_single_step_parity(emx, emo, cfg, n):
         assert w2 <= 1e-6, rep2
         assert trunc.sum() <= n // 100
     # coverage of the branches
-    acts = np.bincount(ref["action"], minlength=5)
+    acts = np.bincount(ref["action"], minlength=6)
     assert acts[1] > 0 and (cfg == 0 or acts[3] > 0)
+    if cfg in (7, 37, 47):      # multiple scattering: the step limit was hit, deflections happened before interactions
+        assert acts[5] > 0 and (ref["msc_tau"][ref["action"] == 1] > 0).any() and (ref["msc_tau"][ref["action"] == 3] > 0).any()
+        assert np.all(ref["n_draws"][(ref["msc_tau"] > 0) & (ref["action"] == 1)] >= 4)
+    else:
+        assert acts[5] == 0 and not ref["msc_tau"].any()
 
 
 # ---------------- level 3: transport ----------------
@@ -153,9 +169,10 @@ def _per_primary_se(o):
 
 
 @pytest.mark.parametrize("cfg,n,n_slots", [(0, 1000, 1024), (1, 300, 1 << 16), (2, 24, 1 << 16), (3, 24, 1 << 16),
-                                           (4, 48, 1 << 16), (1, 64, 1024), (5, 400, 1 << 16), (6, 48, 1 << 16)])
+                                           (4, 48, 1 << 16), (1, 64, 1024), (5, 400, 1 << 16), (6, 48, 1 << 16),
+                                           (7, 24, 1 << 16), (37, 24, 1 << 16), (47, 48, 1 << 16)])
 def test_transport_parity_and_energy_closure(emx, emo, cfg, n, n_slots):
-    desc, prim = W.get(cfg, n)
+    desc, prim = _workload(cfg, n)
     G, O = emx.Problem(desc), emo.Problem(desc)
     o = O.transport(prim, desc["seed"], per_primary=True)
     g = G.transport(G.upload_primaries(prim), desc["seed"], n_slots=n_slots, queue_capacity=1 << 20)
