@@ -58,6 +58,7 @@ enum { EMO_T_COMPTON = 0, EMO_T_PHOTO, EMO_T_PAIR, EMO_T_MOLLER, EMO_T_BREMS_EM,
        EMO_T_DEDX_EM, EMO_T_RANGE_EM, EMO_T_BHABHA, EMO_T_BREMS_EP, EMO_T_ANNIH,
        EMO_T_DEDX_EP, EMO_T_RANGE_EP, EMO_T_PAIR_ELEM0, /* + element index */
        EMO_T_MSC = EMO_T_PAIR_ELEM0 + EMO_MAX_ELEM,     /* 1/lambda_1, inverse first transport mean free path of e+- */
+       EMO_T_VAR_EM, EMO_T_VAR_EP,                      /* d(variance of the restricted collision loss)/ds, MeV2/cm */
        EMO_NTABLE };
 
 /* surface types */
@@ -105,6 +106,7 @@ typedef struct {
     int msc;                     /* 1: multiple scattering of e+- (DESIGN.md R-MSC) */
     double msc_fr;               /* step limit s <= max(msc_fr * max(R, lambda_1), msc_smin) */
     double msc_smin;             /* cm */
+    int fluct;                   /* 1: energy-loss fluctuations of e+- (DESIGN.md R-FLUCT) */
 } emo_physics;
 
 typedef struct {
@@ -175,6 +177,11 @@ double emo_brems_Sigma(double T, double kc, double X0); /* 1/cm */
 double emo_brems_dedx(double T, double kc, double X0);  /* MeV/cm */
 double emo_dedx_col(const emo_material *m, int ptype, double T, double Tcut); /* MeV/cm; Tcut<=0: unrestricted */
 void   emo_gauss_legendre(int n, double *x, double *w); /* nodes/weights on [-1,1] */
+/* second moment of the energy transfers below the production threshold, Int_0^Tup W^2 dsigma, MeV2 cm2 per
+ * electron (DESIGN.md R-FLUCT); ptype EMO_ELECTRON: Moller, Tup = min(Tcut, T/2); EMO_POSITRON: Bhabha, min(Tcut, T) */
+double emo_loss_second_moment(int ptype, double T, double Tcut);
+/* fluctuated loss: mean dE, variance V, the two uniforms; energy E bounds it (DESIGN.md R-FLUCT) */
+double emo_fluctuate_loss(double dE, double V, double E, double xi1, double xi2);
 /* multiple scattering (DESIGN.md R-MSC) */
 double emo_msc_screening(int Z, double T);              /* Moliere screening parameter A */
 double emo_msc_sigma1(int Z, double Amass, double T);   /* first transport cross section, cm2 per atom */

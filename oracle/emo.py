@@ -13,7 +13,7 @@ from . import build as _build
 
 MAX_ELEM, MAX_FACES, NPROC, PER_PRIM, NHIST = 4, 8, 8, 11, 96
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
-           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc"]
+           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc", "var_em", "var_ep"]
 T = {n: i for i, n in enumerate(T_NAMES)}
 ME = 0.51099895000
 
@@ -23,7 +23,7 @@ class Physics(C.Structure):
                 ("E_trk", C.c_double), ("prod_cut_cm", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("lin_loss", C.c_double), ("field_eps", C.c_double), ("max_substeps", C.c_int),
                 ("vacuum_step", C.c_double), ("max_steps", C.c_int), ("deposit_e_at_creation", C.c_int),
-                ("msc", C.c_int), ("msc_fr", C.c_double), ("msc_smin", C.c_double)]
+                ("msc", C.c_int), ("msc_fr", C.c_double), ("msc_smin", C.c_double), ("fluct", C.c_int)]
 
 
 class Track(C.Structure):
@@ -69,6 +69,7 @@ def lib():
             "emo_moller_dcs": (d, [d, d]), "emo_bhabha_dcs": (d, [d, d]),
             "emo_brems_Sigma": (d, [d, d, d]), "emo_brems_dedx": (d, [d, d, d]),
             "emo_gauss_legendre": (None, [i, dp, dp]),
+            "emo_loss_second_moment": (d, [i, d, d]), "emo_fluctuate_loss": (d, [d, d, d, d, d]),
             "emo_msc_screening": (d, [i, d]), "emo_msc_sigma1": (d, [i, d, d]), "emo_msc_one_minus_mu": (d, [d, d]),
             "emo_msc_deflect": (None, [C.POINTER(Rng), d, dp, dp]),
             "emo_create": (p, []), "emo_destroy": (None, [p]),

@@ -18,7 +18,7 @@ emo_problem *emo_create(void) {
     ph->alpha_R = 0.2; ph->rho_R = 0.1; ph->lin_loss = 0.01;
     ph->field_eps = 1e-7; ph->max_substeps = 1000; ph->vacuum_step = 1e3;
     ph->max_steps = 10000; ph->deposit_e_at_creation = 0;
-    ph->msc = 0; ph->msc_fr = 0.2; ph->msc_smin = 1e-3;
+    ph->msc = 0; ph->msc_fr = 0.2; ph->msc_smin = 1e-3; ph->fluct = 0;
     return p;
 }
 
@@ -206,6 +206,10 @@ int emo_build_tables(emo_problem *p) {
                 double s = 0.0;
                 for (int i = 0; i < m->n_elem; ++i) s += m->n_i[i] * emo_msc_sigma1(m->Z[i], m->A[i], E);
                 T[EMO_T_MSC * n + j] = s;
+            }
+            if (ph->fluct) {                               /* variance of the loss per unit path (R-FLUCT) */
+                T[EMO_T_VAR_EM * n + j] = m->n_e * emo_loss_second_moment(EMO_ELECTRON, E, m->Tcut);
+                T[EMO_T_VAR_EP * n + j] = m->n_e * emo_loss_second_moment(EMO_POSITRON, E, m->Tcut);
             }
             T[EMO_T_DEDX_EM * n + j] = dedx_total(m, EMO_ELECTRON, E, m->Tcut, m->kcut);
             T[EMO_T_DEDX_EP * n + j] = dedx_total(m, EMO_POSITRON, E, m->Tcut, m->kcut);

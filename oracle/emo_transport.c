@@ -139,14 +139,21 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
 
     /* 6. continuous loss (e+- in matter) */
     if (pt != EMO_GAMMA && mat >= 0) {
-        double dE;
+        double dE, f1 = 0.0, f2 = 0.0;
+        if (ph->fluct) { f1 = emo_next(&c.rng); f2 = emo_next(&c.rng); }          /* R-FLUCT: always consumed */
         if (action == EMO_A_LOSS && R <= ph->rho_R && full) dE = E;              /* range stop */
-        else if (s * D <= ph->lin_loss * E) dE = s * D;
         else {
-            double E2 = emo_range_inverse(p, mat, pt == EMO_ELECTRON ? EMO_T_RANGE_EM : EMO_T_RANGE_EP, R - s);
-            dE = E - E2;
-            if (dE < 0.0) dE = 0.0;
-            if (dE > E) dE = E;
+            if (s * D <= ph->lin_loss * E) dE = s * D;
+            else {
+                double E2 = emo_range_inverse(p, mat, pt == EMO_ELECTRON ? EMO_T_RANGE_EM : EMO_T_RANGE_EP, R - s);
+                dE = E - E2;
+                if (dE < 0.0) dE = 0.0;
+                if (dE > E) dE = E;
+            }
+            if (ph->fluct && dE > 0.0) {                                         /* R-FLUCT */
+                double V = s * emo_lookup(p, mat, pt == EMO_ELECTRON ? EMO_T_VAR_EM : EMO_T_VAR_EP, E);
+                dE = emo_fluctuate_loss(dE, V, E, f1, f2);
+            }
         }
         t->E = E - dE;
         out->edep += dE;

@@ -256,3 +256,40 @@ double emo_msc_one_minus_mu(double tau, double xi) {
     double t = a * (1.0 - xi) * (S + a) / den;
     return t < 0.0 ? 0.0 : (t > 2.0 ? 2.0 : t);
 }
+
+/* ---- energy-loss fluctuations of e+- (DESIGN.md R-FLUCT; PAPER.md:111 lists "energy loss" with the e+-
+ * processes, PAPER.md:114 (ii) continuous slowing down) ----
+ * The collisions with energy transfer W below the production threshold make up the continuous loss; the
+ * variance of their sum over a path s is s n_e Int_0^Tup W^2 (dsigma/dW) dW (Bohr; the collisions are
+ * independent).  With eps = W/T and the Moller / Bhabha laws above (x = Tup/T):
+ *   Moller:  T^2 pre [c0 x^3/3 + x + (x/(1-x) + x + 2 ln(1-x)) + c (x + ln(1-x))],  c0 = (g-1)^2/g^2, c = (2g-1)/g^2
+ *   Bhabha:  T^2 pre [x/b2 - B1 x^2/2 + B2 x^3/3 - B3 x^4/4 + B4 x^5/5]
+ * (term by term the integrals of eps^2 times the laws; leading term pre T^2 x = 2 pi re^2 me Tup / beta^2). */
+double emo_loss_second_moment(int ptype, double T, double Tcut) {
+    double g = T / EMO_ME + 1.0, g2 = g * g, b2 = 1.0 - 1.0 / g2;
+    if (ptype == EMO_ELECTRON) {
+        double x = Tcut / T;
+        if (x > 0.5) x = 0.5;
+        double pre = 2.0 * EMO_PI * EMO_RE * EMO_RE / (b2 * (g - 1.0));
+        double c0 = (g - 1.0) * (g - 1.0) / g2, c = (2.0 * g - 1.0) / g2;
+        double L = log1p(-x);
+        return T * T * pre * (c0 * x * x * x / 3.0 + x + (x / (1.0 - x) + x + 2.0 * L) + c * (x + L));
+    } else {
+        double x = Tcut / T, B1, B2, B3, B4;
+        if (x > 1.0) x = 1.0;
+        bhabha_B(g, &B1, &B2, &B3, &B4);
+        double pre = 2.0 * EMO_PI * EMO_RE * EMO_RE / (g - 1.0);
+        double x2 = x * x;
+        return T * T * pre * (x / b2 - 0.5 * B1 * x2 + B2 * x2 * x / 3.0 - 0.25 * B3 * x2 * x2 + 0.2 * B4 * x2 * x2 * x);
+    }
+}
+
+/* The fluctuated loss of a step: normal about the mean dE with variance V (Box-Muller from the two uniforms:
+ * z = sqrt(-2 ln xi1) cos(2 pi xi2)), kept inside [0, min(2 dE, E)] by clamping -- symmetric about the mean
+ * unless the mean is more than half of E, so the mean loss stays dE. */
+double emo_fluctuate_loss(double dE, double V, double E, double xi1, double xi2) {
+    double z = sqrt(-2.0 * log(xi1)) * cos(2.0 * EMO_PI * xi2);
+    double d = dE + sqrt(V) * z;
+    double hi = 2.0 * dE < E ? 2.0 * dE : E;
+    return d < 0.0 ? 0.0 : (d > hi ? hi : d);
+}

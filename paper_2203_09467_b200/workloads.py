@@ -27,7 +27,7 @@ def physics(**kw):
     ph = dict(process_mask=63, E_min=1e-3, E_max=1e4, n_E=256, E_trk=1e-3, prod_cut_cm=0.07,
               alpha_R=0.2, rho_R=0.1, lin_loss=0.01, field_eps=1e-7, max_substeps=1000,
               vacuum_step=1e3, max_steps=10000, deposit_e_at_creation=0,
-              msc=0, msc_fr=0.2, msc_smin=1e-3)
+              msc=0, msc_fr=0.2, msc_smin=1e-3, fluct=0)
     ph.update(kw)
     return ph
 
@@ -202,11 +202,12 @@ def config6(n=20000):
 
 
 def config7(n=10000):
-    """SURVEY 8(f) f2, multiple scattering of e+- (Urban / WentzelVI "in progress"): the sampling
-    calorimeter and beam of config 2 with the multiple-scattering step limit and deflection of DESIGN.md R-MSC
-    switched on (f_r = 0.2, s_min = 10 um)."""
+    """SURVEY 8(f) f2, multiple scattering of e+- (Urban / WentzelVI "in progress") and energy-loss
+    fluctuations: the sampling calorimeter and beam of config 2 with the multiple-scattering step limit and
+    deflection of DESIGN.md R-MSC (f_r = 0.2, s_min = 10 um) and the fluctuations of R-FLUCT switched on."""
     desc, prim = config2(n)
-    desc.update(name="config7_calorimeter_msc", seed=7, physics=physics(msc=1, msc_fr=0.2, msc_smin=1e-3))
+    desc.update(name="config7_calorimeter_msc", seed=7,
+                physics=physics(msc=1, msc_fr=0.2, msc_smin=1e-3, fluct=1))
     return desc, prim
 
 
