@@ -101,7 +101,9 @@ extern "C" {
 #define EMX_T_RANGE_EP 11
 #define EMX_T_PAIR_ELEM0 12 /* + element index: n_i * sigma_pair(Z_i) for element selection */
 #define EMX_T_MSC (EMX_T_PAIR_ELEM0 + EMX_MAX_ELEM) /* 1 / lambda_1: inverse first transport mean free path of e+-, 1/cm */
-#define EMX_NTABLE (EMX_T_MSC + 1)
+#define EMX_T_VAR_EM (EMX_T_MSC + 1) /* d(variance of the restricted collision loss)/ds of e-, MeV2/cm */
+#define EMX_T_VAR_EP (EMX_T_MSC + 2) /* ... of e+ */
+#define EMX_NTABLE (EMX_T_MSC + 3)
 
 typedef struct emx_problem emx_problem; /* opaque, owned by the library */
 
@@ -128,6 +130,12 @@ typedef struct {
     int32_t msc;
     double msc_fr;              /* > 0 */
     double msc_smin;            /* cm, > 0 */
+    /* Energy-loss fluctuations of e+- (PAPER.md:114 ii continuous slowing down; DESIGN.md R-FLUCT).  fluct = 1:
+     * the variance of the collisions below the production threshold per unit path, n_e Int_0^Tup W^2 dsigma of the
+     * Moller / Bhabha laws, is tabulated (EMX_T_VAR_*); the continuous loss of a step is drawn from the normal law
+     * about its mean with that variance times s, clamped to [0, min(2 mean, E)] (two draws, taken right after
+     * draw 0 and before those of the multiple scattering); a range stop is not fluctuated. */
+    int32_t fluct;
 } emx_physics;
 
 /* run totals (PAPER.md:176 energy deposition; Fig. 5 diagnostics PAPER.md:204-212) */

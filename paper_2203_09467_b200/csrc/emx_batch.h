@@ -47,7 +47,7 @@ EMX_HD void step_one(const Params &P, uint64_t seed, const emx_track &in, emx_st
     fs.attempt = 0;
     const int whole = P.ph.max_substeps;  // the hook runs the whole step in one call
     if (in.ptype == kGamma) step<kGamma>(P, seed, t, o, fs, whole);
-    else if (!P.ph.msc) {
+    else if (!P.ph.msc && !P.ph.fluct) {
         if (P.field_kind == 0) {
             if (in.ptype == kElectron) step<kElectron>(P, seed, t, o, fs, whole);
             else step<kPositron>(P, seed, t, o, fs, whole);

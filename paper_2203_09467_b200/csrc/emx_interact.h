@@ -49,6 +49,16 @@ EMX_HD double clamp1(double m) { return m > 1.0 ? 1.0 : (m < -1.0 ? -1.0 : m); }
 // exact inverse CDF of p(mu) ~ (1 - beta mu)^-2 (R30)
 EMX_HD double boosted_iso(double xi, double beta) { return clamp1((2.0 * xi - 1.0 + beta) / (beta * (2.0 * xi - 1.0) + 1.0)); }
 
+// ---- fluctuated continuous loss of a step (R-FLUCT): normal about the mean dE with variance V (Box-Muller:
+// z = sqrt(-2 ln xi1) cos(2 pi xi2)), clamped to [0, min(2 dE, E)]
+EMX_NI double fluctuate_loss(double dE, double V, double E, double xi1, double xi2) {
+    double sp, cp;
+    sincos_(2.0 * kPi * xi2, sp, cp);
+    const double d = dE + sqrt(V) * (sqrt(-2.0 * m_log(xi1)) * cp);
+    const double hi = 2.0 * dE < E ? 2.0 * dE : E;
+    return d < 0.0 ? 0.0 : (d > hi ? hi : d);
+}
+
 // ---- multiple-scattering deflection after a path of tau transport mean free paths (R-MSC): polar angle from
 // the Henyey-Greenstein law with mean cosine g = exp(-tau) (Lewis: <cos> = exp(-tau) exactly), azimuth uniform.
 // Inverse distribution function written for t = 1 - mu so that nothing cancels as g -> 1:

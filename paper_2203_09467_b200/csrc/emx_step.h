@@ -137,9 +137,10 @@ EMX_HD void finish_step(const Params &P, Track &t, StepOut &o) {
 }
 
 // MAP: the magnetic field is non-uniform (evaluated at the stage positions of the integrator)
-// MSC: multiple scattering of e+- is switched on (emx_physics.msc; its own instantiation, so that the kernels
-// of a problem without it carry none of its registers)
-template <int PT, bool MAP = false, bool MSC = false>
+// EXT: the condensed-history extensions of e+- -- multiple scattering (emx_physics.msc) and / or energy-loss
+// fluctuations (emx_physics.fluct) -- are switched on (their own instantiation, so that the kernels of a problem
+// without them carry none of their registers)
+template <int PT, bool MAP = false, bool EXT = false>
 EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
     const emx_physics &ph = P.ph;
     o.action = EMX_A_NONE;
@@ -164,7 +165,7 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
     }
 
     double Sig0 = 0.0, Sig1 = 0.0, Sig2 = 0.0, Stot = 0.0, D = 0.0, R = 0.0, s_phys;
-    const bool msc = MSC && (PT != kGamma) && mat >= 0;     // multiple scattering applies (R-MSC)
+    const bool msc = EXT && (PT != kGamma) && ph.msc && mat >= 0;  // multiple scattering applies (R-MSC)
     double iL0 = 0.0;                                       // 1 / lambda_1 at the pre-step energy
     const double *Rtab = nullptr;
     int action;
@@ -259,16 +260,27 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
 
     // 6. continuous loss (e+- in matter)
     if (PT != kGamma && mat >= 0) {
-        double dE;
+        double dE, f1 = 0.0, f2 = 0.0;
+        const bool fl = EXT && ph.fluct;  // energy-loss fluctuations (R-FLUCT): two draws, always consumed
+        if (fl) {
+            f1 = rng.next();
+            f2 = rng.next();
+        }
         if (action == EMX_A_LOSS && R <= ph.rho_R && full) {
             dE = E;  // range stop
-        } else if (s * D <= ph.lin_loss * E) {
-            dE = s * D;
         } else {
-            const double E2 = range_inverse(P, Rtab, R - s);
-            dE = E - E2;
-            if (dE < 0.0) dE = 0.0;
-            if (dE > E) dE = E;
+            if (s * D <= ph.lin_loss * E) {
+                dE = s * D;
+            } else {
+                const double E2 = range_inverse(P, Rtab, R - s);
+                dE = E - E2;
+                if (dE < 0.0) dE = 0.0;
+                if (dE > E) dE = E;
+            }
+            if (fl && dE > 0.0) {
+                const double V = s * interp(table(P, mat, PT == kElectron ? EMX_T_VAR_EM : EMX_T_VAR_EP), grid_pos(P, E));
+                dE = fluctuate_loss(dE, V, E, f1, f2);
+            }
         }
         t.E = E - dE;
         o.edep += dE;
@@ -339,9 +351,9 @@ EMX_HD void step_interact(const Params &P, uint64_t seed, Track &t, StepOut &o, 
     Rng rng;
     rng.init(seed, t.prim, t.tid, t.step);
     const int mat = P.vol[t.vol].material;
-    // draws 0 (interaction length) and 1 (process selection) were used by step_pre, and two more in between
-    // by the multiple-scattering deflection of an e+- (R-MSC)
-    rng.n = (PT != kGamma && ph.msc) ? 4u : 2u;
+    // draws 0 (interaction length) and the process selection were used by step_pre, and in between two each by
+    // the energy-loss fluctuation (R-FLUCT) and the multiple-scattering deflection (R-MSC) of an e+-
+    rng.n = (PT != kGamma) ? 2u + (ph.fluct ? 2u : 0u) + (ph.msc ? 2u : 0u) : 2u;
     const Material &m = P.mat[mat];
     const double E1 = t.E;
     const Vec3 u0 = t.u;
@@ -436,9 +448,9 @@ EMX_HD void step_interact(const Params &P, uint64_t seed, Track &t, StepOut &o, 
 }
 
 // the whole step in one call
-template <int PT, bool MAP = false, bool MSC = false>
+template <int PT, bool MAP = false, bool EXT = false>
 EMX_HD void step(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldState &fs, int budget) {
-    const int proc = step_pre<PT, MAP, MSC>(P, seed, t, o, fs, budget);
+    const int proc = step_pre<PT, MAP, EXT>(P, seed, t, o, fs, budget);
     if (proc >= 0) step_interact<PT>(P, seed, t, o, proc);
 }
 

@@ -109,6 +109,8 @@ EMX_HD void table_pass3(const TableCtx &c, int im, int j) {
     if (c.ph.msc)
         for (int i = 0; i < m.n_elem; ++i) il += m.n_i[i] * msc_sigma1(m.Z[i], m.A[i], E);
     T[EMX_T_MSC * n + j] = il;
+    T[EMX_T_VAR_EM * n + j] = c.ph.fluct ? m.n_e * loss_second_moment(kElectron, E, m.Tcut) : 0.0;  // R-FLUCT
+    T[EMX_T_VAR_EP * n + j] = c.ph.fluct ? m.n_e * loss_second_moment(kPositron, E, m.Tcut) : 0.0;
     T[EMX_T_DEDX_EM * n + j] = dedx_total(m, kElectron, E, m.Tcut, m.kcut);
     T[EMX_T_DEDX_EP * n + j] = dedx_total(m, kPositron, E, m.Tcut, m.kcut);
     T[EMX_T_RANGE_EM * n + j] = range_bin(c, m, kElectron, m.Tcut, m.kcut, j);

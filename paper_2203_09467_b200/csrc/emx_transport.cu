@@ -741,7 +741,7 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
 // Lanes whose step ends here (boundary, loss-limited, truncated, killed) are committed; lanes with an
 // interaction pending are committed as far as they got and filed in the list of their process, so that
 // k_interact runs every interactor on full warps (B:north_star "partitioned by next action").
-template <int PT, bool MAP, bool MSC>
+template <int PT, bool MAP, bool EXT>
 __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
                                              int n_live, int budget) {
     Ctl *c = w.ctl;
@@ -785,7 +785,7 @@ __device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uin
         t.alive = 1;
         vol0 = t.vol;
         step0 = t.step;
-        pend = step_pre<PT, MAP, MSC>(P, seed, t, o, fs, budget);
+        pend = step_pre<PT, MAP, EXT>(P, seed, t, o, fs, budget);
         if (PT != kGamma && o.suspended) {
             // the propagation continues in the next iteration: park position, direction, surface flag and the
             // loop variables; nothing else of the step has happened yet
@@ -880,7 +880,7 @@ __device__ __forceinline__ WarpAcc interact_chunk(const Params &P, const Work &w
     return epilogue<PT, false>(P, w, seed, tally, i, active, false, false, -1, t, o, vol0, step0);
 }
 
-template <int PT, bool MAP, bool MSC = false>
+template <int PT, bool MAP, bool EXT = false>
 __global__ void __launch_bounds__(kStepBlock, kStepWarpsPerSM * 32 / kStepBlock) k_step_pool(const __grid_constant__ Params P,
                                                                   const __grid_constant__ Work w, uint64_t seed,
                                                                   double *tally) {
@@ -899,7 +899,7 @@ __global__ void __launch_bounds__(kStepBlock, kStepWarpsPerSM * 32 / kStepBlock)
         const int k = __shfl_sync(0xffffffffu, k_next, 0);
         if (k >= total) break;
         if (lane == 0) k_next = atomicAdd(&c->work_ctr3[PT], 1);
-        const WarpAcc d = pre_chunk<PT, MAP, MSC>(P, w, seed, tally, k << 5, nl, budget);
+        const WarpAcc d = pre_chunk<PT, MAP, EXT>(P, w, seed, tally, k << 5, nl, budget);
         acc.n += d.n;
         acc.d += d.d;
     }
@@ -991,11 +991,11 @@ extern "C" int emx_debug_timeline(unsigned long long *host, int clear) {
 }
 #endif
 
-// phase A of a charged pool: the instantiation for the kind of field set on the problem, with or without
-// multiple scattering
+// phase A of a charged pool: the instantiation for the kind of field set on the problem, with or without the
+// condensed-history extensions (multiple scattering, energy-loss fluctuations)
 template <int PT>
 static void launch_phase_a(const Params &P, const Work &w, uint64_t seed, double *tally, int g, cudaStream_t st) {
-    if (!P.ph.msc) {
+    if (!P.ph.msc && !P.ph.fluct) {
         if (P.field_kind == 0) k_step_pool<PT, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
         else k_step_pool<PT, true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
     } else {

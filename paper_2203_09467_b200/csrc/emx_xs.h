@@ -172,6 +172,28 @@ EMX_HD double dedx_col(const Material &m, int ptype, double T, double Tcut) {
     return 2.0 * kPi * kRe * kRe * kMe * m.n_e / b2 * (lg + F - del);
 }
 
+// ---- energy-loss fluctuations (DESIGN.md R-FLUCT): second moment of the transfers W = eps T below the
+// production threshold, Int_0^x eps^2 (dsigma/deps) deps T^2, cm2 MeV2 per electron, x = min(Tcut/T, 1/2 | 1).
+// Moller law pre (c0 + 1/eps^2 - c/eps + 1/(1-eps)^2 - c/(1-eps)), Bhabha law pre (1/(b2 eps^2) - B1/eps + B2
+// - B3 eps + B4 eps^2) (C5.5, C5.6), integrated term by term.
+EMX_HD double loss_second_moment(int ptype, double T, double Tcut) {
+    const double g = T / kMe + 1.0, g2 = g * g, b2 = 1.0 - 1.0 / g2;
+    double x = Tcut / T;
+    if (ptype == kElectron) {
+        if (x > 0.5) x = 0.5;
+        const double pre = 2.0 * kPi * kRe * kRe / (b2 * (g - 1.0));
+        const double c0 = (g - 1.0) * (g - 1.0) / g2, c = (2.0 * g - 1.0) / g2;
+        const double L = log1p(-x);
+        return T * T * pre * (c0 * x * x * x / 3.0 + x + (x / (1.0 - x) + x + 2.0 * L) + c * (x + L));
+    }
+    if (x > 1.0) x = 1.0;
+    const double y = 1.0 / (g + 1.0), t = 1.0 - 2.0 * y;
+    const double B1 = 2.0 - y * y, B2 = t * (3.0 + y * y), B4 = t * t * t, B3 = t * t + B4;
+    const double pre = 2.0 * kPi * kRe * kRe / (g - 1.0);
+    const double x2 = x * x;
+    return T * T * pre * (x / b2 - 0.5 * B1 * x2 + B2 * x2 * x / 3.0 - 0.25 * B3 * x2 * x2 + 0.2 * B4 * x2 * x2 * x);
+}
+
 // ---- multiple scattering of e+- (DESIGN.md R-MSC; PAPER.md:111 names the models, prints no formula) ----
 // Screened Rutherford law per atom, dsigma/dOmega = Z (Z + 1) re^2 (me / (beta p))^2 / (t + 2 A)^2 with
 // t = 1 - cos(theta); Moliere: 4 A = chi_0^2 (1.13 + 3.76 (alpha Z / beta)^2), chi_0 = hbar / (p a_TF),

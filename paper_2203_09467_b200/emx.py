@@ -13,9 +13,9 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("EMX_LIB_PATH") or os.path.join(HERE, "libemx.so")   # override: kernel experiments
-MAX_ELEM, MAX_FACES, NPROC, NTABLE, NHIST = 4, 8, 8, 17, 96
+MAX_ELEM, MAX_FACES, NPROC, NTABLE, NHIST = 4, 8, 8, 19, 96
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
-           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc"]
+           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc", "var_em", "var_ep"]
 T = {n: i for i, n in enumerate(T_NAMES)}
 
 
@@ -24,7 +24,7 @@ class Physics(C.Structure):
                 ("E_trk", C.c_double), ("prod_cut_cm", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("lin_loss", C.c_double), ("field_eps", C.c_double), ("max_substeps", C.c_int32),
                 ("vacuum_step", C.c_double), ("max_steps", C.c_int32), ("deposit_e_at_creation", C.c_int32),
-                ("msc", C.c_int32), ("msc_fr", C.c_double), ("msc_smin", C.c_double)]
+                ("msc", C.c_int32), ("msc_fr", C.c_double), ("msc_smin", C.c_double), ("fluct", C.c_int32)]
 
 
 class Scalars(C.Structure):
