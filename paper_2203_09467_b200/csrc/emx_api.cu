@@ -59,6 +59,7 @@ struct emx_problem {
     long slice_above = -1;  // < 0: n_slots / 32
     int slice_budget = 2;
     int warps_per_sm[3] = {16, 16, 8};  // gamma, e-, e+ (the e+ pool holds 8 % of the slots)
+    double pool_frac[3] = {0.0, 0.0, 0.0};  // EMX_POOL_FRAC: share of the slots per pool (0: the default split)
 };
 
 namespace {
@@ -119,10 +120,18 @@ struct Carve {
     }
 };
 
+// with multiple scattering the charged tracks take ~7x the steps: measured on config 7, +24 % over the split above
+const double kPoolFracMsc[3] = {0.25, 0.63, 0.12};
+// share of the track slots per pool: the knob if set, else the default split for the physics of the problem
+// (the split decides when a step is taken, never its result)
+static const double *pool_split(const emx_problem *p) {
+    return p->pool_frac[0] > 0.0 ? p->pool_frac : (p->hp.ph.msc ? kPoolFracMsc : kPoolFrac);
+}
+
 // carve the caller's workspace; with base == nullptr only the size is computed
-size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
+size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log, const double *pool_frac) {
     Carve c{base};
-    split3(n_slots, kPoolFrac, w.cap);
+    split3(n_slots, pool_frac, w.cap);
     split3(qcap, kQueueFrac, w.qcap);
     w.ctl = c.take<Ctl>(1);
     w.log = c.take<uint32_t>(2 * (size_t)max_log);
@@ -186,6 +195,11 @@ int emx_create(emx_problem **out) {
     if (const char *e = getenv("EMX_SLICE_BUDGET")) p->slice_budget = atoi(e) > 0 ? atoi(e) : p->slice_budget;
     if (const char *e = getenv("EMX_SLICE_ABOVE")) p->slice_above = atol(e);
     if (const char *e = getenv("EMX_LOOP_NODE")) p->loop_node = atoi(e);
+    if (const char *e = getenv("EMX_POOL_FRAC")) {
+        double f[3] = {0, 0, 0};
+        if (sscanf(e, "%lf,%lf,%lf", &f[0], &f[1], &f[2]) == 3 && f[0] > 0 && f[1] > 0 && f[2] > 0)
+            for (int k = 0; k < 3; ++k) p->pool_frac[k] = f[k] / (f[0] + f[1] + f[2]);
+    }
     if (const char *e = getenv("EMX_WARPS_PER_SM")) sscanf(e, "%d,%d,%d", &p->warps_per_sm[0], &p->warps_per_sm[1], &p->warps_per_sm[2]);
     *out = p;
     return EMX_OK;
@@ -432,7 +446,7 @@ size_t emx_workspace_bytes(const emx_problem *p, long n_slots, long queue_capaci
     // pools hold fewer than 2^21 slots each (packed list counters): n_slots <= 2^21
     if (!p || n_slots < 1 || queue_capacity < 1 || n_slots > (1L << 21) || queue_capacity > (1L << 30)) return 0;
     Work w;
-    return carve_work(nullptr, n_slots, queue_capacity, w, kMaxLog);
+    return carve_work(nullptr, n_slots, queue_capacity, w, kMaxLog, pool_split(p));
 }
 
 int emx_reset_tallies(emx_problem *p, void *stream) {
@@ -446,7 +460,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     if (pr.first + pr.n > 0x100000000LL) return fail(p, EMX_E_ARG, "emx_transport: primary indices beyond 2^32");
     Work w;
     memset(&w, 0, sizeof(w));  // compared bytewise with the arguments of the kept graph
-    const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog);
+    const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog, pool_split(p));
     if (need > workspace_bytes) return fail(p, EMX_E_CAPACITY, "emx_transport: workspace smaller than emx_workspace_bytes()");
     // admission limits (R8): about 20 MeV of shower energy in flight per queued record at the peak of
     // the queue (measured on configs 1-4), with a factor 4 of headroom below the capacity

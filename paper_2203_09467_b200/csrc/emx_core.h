@@ -59,7 +59,7 @@ struct Params {
     const double *tab;      // [n_mat][EMX_NTABLE][n_E]
     const int *nb_off;      // neighbour candidates: cells having face (S, sense); index 2*S + (sense > 0)
     const int *nb_list;
-    const int *nb2_off;     // per surface S: cells that do not list S at all (the only other cells that can match)
+    const int *nb2_off;     // per (S, sense): cells that do not list S at all (the only other cells that can match)
     const int *nb2_list;
     double Bmag, Bhat[3];
     int field_kind;               // 0 uniform; 1 solenoid with fringe (emx_set_field_fringe)

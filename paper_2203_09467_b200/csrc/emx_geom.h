@@ -101,7 +101,9 @@ EMX_HD bool cell_matches(const Params &P, int cid, const Vec3 &x, const Vec3 &u,
 // sense can never agree, so only two precomputed lists (ascending id) have to be looked at: the cells that
 // list (S, newsense) -- in a world tiled without overlap the answer is one of them -- and, if none of those
 // matches (edges and corners where another surface lies within the tolerance), the cells that do not list S
-// at all.  For a world tiled without overlap this returns the id of the full scan in id order.
+// at all.  For a world tiled without overlap this returns the id of the full scan in id order.  Both lists leave
+// out the cells that a parallel face of their own keeps on the other side of S (emx_host.h never_across): the
+// scan would reject them anyway, and a track leaving the world finds nothing to test.
 EMX_NI int neighbour(const Params &P, const Vec3 &x, const Vec3 &u, int S) {
     const int newsense = surf_g(P.surf_type[S], x, u) > 0.0 ? 1 : -1;
     const int k = 2 * S + (newsense > 0 ? 1 : 0);
@@ -109,7 +111,7 @@ EMX_NI int neighbour(const Params &P, const Vec3 &x, const Vec3 &u, int S) {
         const int cid = P.nb_list[j];
         if (cell_matches(P, cid, x, u, S, newsense)) return cid;
     }
-    for (int j = P.nb2_off[S], e = P.nb2_off[S + 1]; j < e; ++j) {
+    for (int j = P.nb2_off[k], e = P.nb2_off[k + 1]; j < e; ++j) {
         const int cid = P.nb2_list[j];
         if (cell_matches(P, cid, x, u, S, newsense)) return cid;
     }

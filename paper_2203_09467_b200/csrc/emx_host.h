@@ -75,9 +75,31 @@ inline bool derive_material(Material &m, int n_elem, const int *Z, const double 
     return true;
 }
 
-// nb_off[2 S + (sense > 0)] .. nb_off[2 S + (sense > 0) + 1]: cells listing (S, sense), ascending id
+// Can cell c hold points just across S on its `sense` side?  Not if one of its own faces is a surface of the same
+// family (same axis plane, or z-cylinder) that keeps the cell on the other side of S by more than `margin`: with
+// sense = +1 the point has f_S >= -eps, and a face (v_f <= v_S - margin, sense -1) wants f_f < 0 where
+// f_f >= margin - eps > 0 (mirror image for sense = -1).  The point crossing S lies within the landing tolerance
+// eps = field_eps of S (C9), margin = max(1e-6, 10 eps) cm, so cell_matches() would reject exactly
+// these cells at that face: leaving them out of the candidate lists cannot change what neighbour() returns.
+inline bool never_across(const HostProblem &hp, int c, int S, int sense, double margin) {
+    const Volume &v = hp.vol[c];
+    const int tS = hp.surf_type[S];
+    const double vS = hp.surf_v[S];
+    for (int i = 0; i < v.n_faces; ++i) {
+        const int Sf = v.surf[i];
+        if (Sf == S || hp.surf_type[Sf] != tS) continue;
+        const double vf = hp.surf_v[Sf];
+        if (sense > 0 && v.sense[i] < 0 && vf <= vS - margin) return true;
+        if (sense < 0 && v.sense[i] > 0 && vf >= vS + margin) return true;
+    }
+    return false;
+}
+
+// nb_off[2 S + (sense > 0)] .. nb_off[2 S + (sense > 0) + 1]: cells listing (S, sense), ascending id, without the
+// cells that can never lie across S on that side
 inline void build_neighbour_lists(const HostProblem &hp, std::vector<int> &off, std::vector<int> &list) {
     const int ns = (int)hp.surf_type.size();
+    const double margin = fmax(1e-6, 10.0 * hp.ph.field_eps);
     off.assign(2 * ns + 1, 0);
     list.clear();
     for (int k = 0; k < 2 * ns; ++k) {
@@ -87,7 +109,7 @@ inline void build_neighbour_lists(const HostProblem &hp, std::vector<int> &off, 
             const Volume &v = hp.vol[c];
             for (int i = 0; i < v.n_faces; ++i)
                 if (v.surf[i] == S && v.sense[i] == sense) {
-                    list.push_back(c);
+                    if (!never_across(hp, c, S, sense, margin)) list.push_back(c);
                     break;
                 }
         }
@@ -95,21 +117,25 @@ inline void build_neighbour_lists(const HostProblem &hp, std::vector<int> &off, 
     off[2 * ns] = (int)list.size();
 }
 
-// off2[S] .. off2[S + 1]: cells that do not list S with either sense, ascending id
+// off2[2 S + (sense > 0)] .. off2[2 S + (sense > 0) + 1]: cells that do not list S with either sense, ascending id,
+// again without the cells that can never lie across S on that side (a track leaving the world through an outer
+// surface finds both lists empty instead of testing every cell of the problem)
 inline void build_nonlisting_lists(const HostProblem &hp, std::vector<int> &off2, std::vector<int> &list2) {
     const int ns = (int)hp.surf_type.size();
-    off2.assign(ns + 1, 0);
+    const double margin = fmax(1e-6, 10.0 * hp.ph.field_eps);
+    off2.assign(2 * ns + 1, 0);
     list2.clear();
-    for (int S = 0; S < ns; ++S) {
-        off2[S] = (int)list2.size();
+    for (int k = 0; k < 2 * ns; ++k) {
+        const int S = k / 2, sense = (k & 1) ? 1 : -1;
+        off2[k] = (int)list2.size();
         for (int c = 0; c < (int)hp.vol.size(); ++c) {
             const Volume &v = hp.vol[c];
             bool lists = false;
             for (int i = 0; i < v.n_faces; ++i) lists = lists || (v.surf[i] == S);
-            if (!lists) list2.push_back(c);
+            if (!lists && !never_across(hp, c, S, sense, margin)) list2.push_back(c);
         }
     }
-    off2[ns] = (int)list2.size();
+    off2[2 * ns] = (int)list2.size();
 }
 
 struct GridConsts {
