@@ -167,6 +167,7 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
     double Sig0 = 0.0, Sig1 = 0.0, Sig2 = 0.0, Stot = 0.0, D = 0.0, R = 0.0, s_phys;
     const bool msc = EXT && (PT != kGamma) && ph.msc && mat >= 0;  // multiple scattering applies (R-MSC)
     double iL0 = 0.0;                                       // 1 / lambda_1 at the pre-step energy
+    double var0 = 0.0;                                      // variance of the loss per unit path at the pre-step energy
     const double *Rtab = nullptr;
     int action;
     const double E = t.E;
@@ -208,6 +209,7 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
                 s_phys = s_loss;
                 action = EMX_A_LOSS;
             }
+            if (EXT && ph.fluct) var0 = interp(table(P, mat, PT == kElectron ? EMX_T_VAR_EM : EMX_T_VAR_EP), g);
             if (msc) {  // R-MSC step limit: s <= max(f_r max(R, lambda_1), s_min)
                 iL0 = interp(table(P, mat, EMX_T_MSC), g);
                 const double big = (iL0 > 0.0 && 1.0 / iL0 > R) ? 1.0 / iL0 : R;
@@ -278,8 +280,7 @@ EMX_HD int step_pre(const Params &P, uint64_t seed, Track &t, StepOut &o, FieldS
                 if (dE > E) dE = E;
             }
             if (fl && dE > 0.0) {
-                const double V = s * interp(table(P, mat, PT == kElectron ? EMX_T_VAR_EM : EMX_T_VAR_EP), grid_pos(P, E));
-                dE = fluctuate_loss(dE, V, E, f1, f2);
+                dE = fluctuate_loss(dE, s * var0, E, f1, f2);
             }
         }
         t.E = E - dE;
