@@ -323,6 +323,9 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
         const long long ng = c->n_live[0], ne = c->n_live[1], np = c->n_live[2];
         const long long live = ng + ne + np;
         const long long queued = (long long)c->q_top[0] + c->q_top[1] + c->q_top[2];
+        // a track pushes at most 4 records in an iteration (two products and two at-rest photons): where even that
+        // fits, the step kernels reserve with one atomic and no look at the top first
+        for (int p = 0; p < 3; ++p) c->q_safe[p] = ((long long)c->q_top[p] + 4LL * live <= (long long)w.qcap[p]) ? 1 : 0;
         if ((unsigned long long)live > c->peak_live) c->peak_live = (unsigned long long)live;
         if ((unsigned long long)queued > c->peak_queue) c->peak_queue = (unsigned long long)queued;
         if (c->iter < (unsigned long long)w.max_log) {
@@ -514,22 +517,27 @@ __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, i
     int r0 = -1;
     if (lane == 0) {
         const int cap = w.qcap[ty];
-        int old = *(volatile int *)&c->q_top[ty];
-        if ((long long)old + cnt + kReserveSlack <= (long long)cap) {
+        if (__ldg(&c->q_safe[ty])) {
+            // k_plan's guarantee for this iteration: one round trip to the top instead of two
             r0 = atomicAdd(&c->q_top[ty], cnt);
-        } else if (cap < 8 * kReserveSlack) {
-            // small stack: exact accounting by compare-and-swap
-            while (old + cnt <= cap) {
-                const int prev = atomicCAS(&c->q_top[ty], old, old + cnt);
-                if (prev == old) {
-                    r0 = old;
-                    break;
+        } else {
+            int old = *(volatile int *)&c->q_top[ty];
+            if ((long long)old + cnt + kReserveSlack <= (long long)cap) {
+                r0 = atomicAdd(&c->q_top[ty], cnt);
+            } else if (cap < 8 * kReserveSlack) {
+                // small stack: exact accounting by compare-and-swap
+                while (old + cnt <= cap) {
+                    const int prev = atomicCAS(&c->q_top[ty], old, old + cnt);
+                    if (prev == old) {
+                        r0 = old;
+                        break;
+                    }
+                    old = prev;
                 }
-                old = prev;
             }
+            // large stack within kReserveSlack of its capacity: treated as full (thousands of warps spinning on
+            // one compare-and-swap cost 10x the iteration; the last 2 % of a large stack are not worth it)
         }
-        // large stack within kReserveSlack of its capacity: treated as full (thousands of warps spinning on one
-        // compare-and-swap cost 10x the iteration; the last 2 % of a large stack are not worth it)
     }
     return __shfl_sync(0xffffffffu, r0, 0);
 }

@@ -48,6 +48,7 @@ struct Ctl {
     int n_live[3];
     int q_top[3];
     int m_step[3];  // tracks to step this iteration (= n_live)
+    int q_safe[3];  // set by k_plan: stack p cannot overflow in this iteration whatever the step kernels push
     PoolPlan plan[3];
     int done, error, had_live;
     int idle_iters;  // consecutive iterations without progress although tracks are live (R7)
