@@ -488,10 +488,6 @@ __device__ __forceinline__ void push_record(const QueueSoA &q, int r, const Vec3
     EMX_ST(&q.surf[r], -1);
 }
 
-#ifndef EMX_TALLY_GROUPS
-#define EMX_TALLY_GROUPS 3
-#endif
-
 __device__ __forceinline__ double warp_sum(double v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
@@ -684,21 +680,11 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     }
 
     // ---- A10: per-volume tally.  Lanes with the same tally id are summed with shuffles; one atomic per group.
-    // A warp whose lanes are spread over more than EMX_TALLY_GROUPS tally ids (a finely segmented calorimeter)
-    // would pay a whole warp reduction per id: there every lane adds its own deposit.
+    // (Letting the lanes of a warp that is spread over many ids add their deposits one by one saves the reductions
+    // -- +2 % on configs 2 and 7 -- but serialises on the few tally addresses of configs 4 and 5: -40 %.)
     {
         const int tl = (commit && o.edep != 0.0) ? P.vol[vol0].tally : -1;
         unsigned m = __ballot_sync(0xffffffffu, tl >= 0);
-#if EMX_TALLY_GROUPS < 32
-        if (m) {
-            const unsigned same = __match_any_sync(0xffffffffu, tl);
-            const unsigned lead = __ballot_sync(0xffffffffu, tl >= 0 && lane == __ffs(same) - 1);
-            if (__popc(lead) > EMX_TALLY_GROUPS) {
-                if (tl >= 0) atomicAdd(&tally[tl], o.edep);
-                m = 0u;
-            }
-        }
-#endif
         while (m) {
             const int leader = __ffs(m) - 1;
             const int key = __shfl_sync(0xffffffffu, tl, leader);
