@@ -708,6 +708,20 @@ int emx_set_primary_offset(emx_problem *p, long first) {
     return EMX_OK;
 }
 
+int emx_set_pool_split(emx_problem *p, double fg, double fe, double fp) {
+    if (!p) return fail(p, EMX_E_ARG, "emx_set_pool_split: null problem");
+    if (fg == 0.0 && fe == 0.0 && fp == 0.0) {
+        p->pool_frac[0] = p->pool_frac[1] = p->pool_frac[2] = 0.0;
+        return EMX_OK;
+    }
+    if (!(fg > 0.0) || !(fe > 0.0) || !(fp > 0.0)) return fail(p, EMX_E_ARG, "emx_set_pool_split: every share must be > 0");
+    const double s = fg + fe + fp;
+    p->pool_frac[0] = fg / s;
+    p->pool_frac[1] = fe / s;
+    p->pool_frac[2] = fp / s;
+    return EMX_OK;
+}
+
 int emx_read_tallies(const emx_problem *cp, double *edep_host, emx_scalars *out) {
     emx_problem *p = const_cast<emx_problem *>(cp);
     if (!p || !p->hp.built) return fail(p, EMX_E_STATE, "emx_read_tallies: tables not built");

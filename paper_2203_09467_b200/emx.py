@@ -50,7 +50,7 @@ class StepResult(C.Structure):
 EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "emx_add_volume", "emx_set_field", "emx_set_field_fringe",
            "emx_get_physics", "emx_set_physics", "emx_set_cuts", "emx_build_tables", "emx_get_table",
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
-           "emx_set_primary_offset", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
+           "emx_set_primary_offset", "emx_set_pool_split", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
            "emx_get_iteration_log", "emx_get_iteration_times",
            "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_last_error",
            "emx_version"]
@@ -81,7 +81,7 @@ def lib():
             "emx_reset_tallies": (i, [vp, vp]), "emx_read_tallies": (i, [vp, vp, C.POINTER(Scalars)]),
             "emx_last_transport_ms": (d, [vp]), "emx_get_iteration_log": (l, [vp, vp, l]),
             "emx_get_iteration_times": (l, [vp, vp, l]),
-            "emx_get_lanes": (i, [vp, vp]), "emx_read_step_hist": (i, [vp, vp]), "emx_set_primary_offset": (i, [vp, l]),
+            "emx_get_lanes": (i, [vp, vp]), "emx_read_step_hist": (i, [vp, vp]), "emx_set_primary_offset": (i, [vp, l]), "emx_set_pool_split": (i, [vp, d, d, d]),
             "emx_set_profile": (i, [vp, i]), "emx_get_profile": (i, [vp, vp, vp, vp]),
             "emx_step_batch": (i, [vp, u64, l, vp, vp, vp]),
             "emx_philox_batch": (i, [l, vp, vp, vp, vp]),
@@ -150,6 +150,8 @@ class Problem:
             self._check(L.emx_add_volume(h, len(s), _hp(s), _hp(e), vol["material"], vol["tally"]))
         B = desc.get("field", (0.0, 0.0, 0.0))
         self._check(L.emx_set_field(h, float(B[0]), float(B[1]), float(B[2])))
+        if desc.get("pool_split") and not os.environ.get("EMX_POOL_FRAC"):      # scheduling hint of the workload
+            self._check(L.emx_set_pool_split(h, *[float(v) for v in desc["pool_split"]]))
         if desc.get("field_fringe"):
             self._check(L.emx_set_field_fringe(h, float(desc["field_fringe"][0]), float(desc["field_fringe"][1])))
         ph = Physics()

@@ -308,6 +308,13 @@ def test_results_do_not_depend_on_slots_or_host_entry(emx):
     assert np.array_equal(a["steps"], b["steps"]) and np.array_equal(a["tracks"], b["tracks"])
     assert np.allclose(a["edep"], b["edep"], rtol=1e-11, atol=1e-9)
     assert a["iterations"] != b["iterations"] or a["peak_live"] != b["peak_live"]
+    # nor on how the slots are shared among the three pools (emx_set_pool_split)
+    G2 = emx.Problem(dict(desc, pool_split=(20, 60, 20)))
+    c = G2.transport(G2.upload_primaries(prim), desc["seed"], n_slots=1 << 12, queue_capacity=1 << 18)
+    assert np.array_equal(a["steps"], c["steps"]) and np.array_equal(a["tracks"], c["tracks"])
+    assert np.array_equal(a["inter"], c["inter"])
+    assert np.allclose(a["edep"], c["edep"], rtol=1e-11, atol=1e-9)
+    assert a["iterations"] != c["iterations"] or a["peak_live"] != c["peak_live"]
 
 
 def test_shards_of_the_primaries_sum_to_the_whole(emx):

@@ -62,6 +62,16 @@ def test_host_side_argument_checks_without_a_device(L):
     assert L.emx_set_physics(h, C.byref(ph)) == -1
     assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) > (1 << 20) * 85 + (1 << 26) * 76 * 0.9
     assert L.emx_workspace_bytes(h, 0, 10) == 0
+    # pool split: shares must be positive; it moves bytes between the pools' arrays (the charged pools carry 20 B
+    # more per slot), (0, 0, 0) restores the default
+    L.emx_set_pool_split.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
+    w0 = L.emx_workspace_bytes(h, 1 << 20, 1 << 26)
+    assert L.emx_set_pool_split(h, 40.0, -1.0, 10.0) == -1 and L.emx_set_pool_split(h, 0.0, 1.0, 1.0) == -1
+    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) == w0
+    assert L.emx_set_pool_split(h, 20.0, 70.0, 10.0) == 0
+    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) > w0
+    assert L.emx_set_pool_split(h, 0.0, 0.0, 0.0) == 0
+    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) == w0
     # compute calls before the tables are built are refused with EMX_E_STATE
     assert L.emx_read_tallies(h, None, None) == -2
     assert L.emx_step_batch(h, 0, 0, None, None, None) == -2
