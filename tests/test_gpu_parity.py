@@ -435,12 +435,15 @@ def test_scheduling_knobs_do_not_change_results(emx, monkeypatch):
     assert runs[0]["iterations"] != runs[1]["iterations"]       # the schedules did differ
 
 
-def test_full_size_bench_configuration(emx, emo):
+@pytest.mark.parametrize("cfg", [4, 7])
+def test_full_size_bench_configuration(emx, emo, cfg):
     """BASELINE config 4 in full (100 000 primaries, 2^20 slots, 2^26 records: what bench.py times), against
     the oracle on all host cores.  With keyed random numbers the histories are the same, so the integer
     counters agree to a few parts per million (a comparison within rounding of equality may flip in
-    3.6e9 steps) and every tally within 1e-6; energy closes to 1e-9."""
-    desc, prim = W.get(4)
+    3.6e9 steps) and every tally within 1e-6; energy closes to 1e-9.  The same for config 7 in full (10 000
+    showers of 10 GeV with multiple scattering and energy-loss fluctuations, 1.5e9 steps), as bench.py --config 7
+    times it."""
+    desc, prim = W.get(cfg)
     G = emx.Problem(desc)
     g = G.transport(G.upload_primaries(prim), desc["seed"])
     assert g["stalls"] == 0
