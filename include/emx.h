@@ -319,6 +319,14 @@ int emx_philox_batch(long n, const uint32_t *ctr4, const uint32_t *key2, uint32_
 int emx_draw_batch(uint64_t seed, long n, const uint32_t *prim, const uint64_t *tid, const uint32_t *step,
                    const uint32_t *nn, double *u, uint64_t *child, void *stream);
 
+/* Level-1 hook for the relocation after a boundary crossing (C8; HOST only, needs no device and no
+ * tables): the candidate cells, in the order they are tested, for a track that has crossed `surface` towards
+ * its `sense` side (+1: f > 0, -1: f < 0).  which = 0: the cells that list (surface, sense); which = 1: the cells
+ * that do not list the surface at all.  Both lists leave out the cells a parallel face of their own keeps on the
+ * other side of the surface by more than max(1e-6 cm, 10 field_eps).  Writes min(count, cap) cell ids to
+ * host_out (may be NULL with cap = 0) and returns count, or EMX_E_ARG. */
+int emx_neighbour_candidates(const emx_problem *p, int surface, int sense, int which, int32_t *host_out, int cap);
+
 /* Level-1 hook for the refill / compaction step: applies one refill pass to a pool
  * of `n_live` slots whose alive flags are alive[n_live] (uint8, DEVICE) with `n_queue` queued records and
  * room for `capacity` slots, and writes, for every slot index < new_n_live, src[i] (int32, DEVICE,

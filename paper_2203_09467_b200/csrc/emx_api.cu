@@ -708,6 +708,20 @@ int emx_set_primary_offset(emx_problem *p, long first) {
     return EMX_OK;
 }
 
+int emx_neighbour_candidates(const emx_problem *cp, int surface, int sense, int which, int32_t *host_out, int cap) {
+    emx_problem *p = const_cast<emx_problem *>(cp);
+    if (!p || surface < 0 || surface >= (int)p->hp.surf_type.size() || (sense != 1 && sense != -1) || (which != 0 && which != 1) ||
+        cap < 0 || (cap > 0 && !host_out))
+        return fail(p, EMX_E_ARG, "emx_neighbour_candidates: invalid argument");
+    std::vector<int> off, list;
+    if (which == 0) build_neighbour_lists(p->hp, off, list);
+    else build_nonlisting_lists(p->hp, off, list);
+    const int k = 2 * surface + (sense > 0 ? 1 : 0);
+    const int n = off[k + 1] - off[k];
+    for (int j = 0; j < n && j < cap; ++j) host_out[j] = list[off[k] + j];
+    return n;
+}
+
 int emx_set_pool_split(emx_problem *p, double fg, double fe, double fp) {
     if (!p) return fail(p, EMX_E_ARG, "emx_set_pool_split: null problem");
     if (fg == 0.0 && fe == 0.0 && fp == 0.0) {

@@ -50,7 +50,7 @@ class StepResult(C.Structure):
 EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "emx_add_volume", "emx_set_field", "emx_set_field_fringe",
            "emx_get_physics", "emx_set_physics", "emx_set_cuts", "emx_build_tables", "emx_get_table",
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
-           "emx_set_primary_offset", "emx_set_pool_split", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
+           "emx_set_primary_offset", "emx_set_pool_split", "emx_neighbour_candidates", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
            "emx_get_iteration_log", "emx_get_iteration_times",
            "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_last_error",
            "emx_version"]
@@ -81,7 +81,7 @@ def lib():
             "emx_reset_tallies": (i, [vp, vp]), "emx_read_tallies": (i, [vp, vp, C.POINTER(Scalars)]),
             "emx_last_transport_ms": (d, [vp]), "emx_get_iteration_log": (l, [vp, vp, l]),
             "emx_get_iteration_times": (l, [vp, vp, l]),
-            "emx_get_lanes": (i, [vp, vp]), "emx_read_step_hist": (i, [vp, vp]), "emx_set_primary_offset": (i, [vp, l]), "emx_set_pool_split": (i, [vp, d, d, d]),
+            "emx_get_lanes": (i, [vp, vp]), "emx_read_step_hist": (i, [vp, vp]), "emx_set_primary_offset": (i, [vp, l]), "emx_set_pool_split": (i, [vp, d, d, d]), "emx_neighbour_candidates": (i, [vp, i, i, i, vp, i]),
             "emx_set_profile": (i, [vp, i]), "emx_get_profile": (i, [vp, vp, vp, vp]),
             "emx_step_batch": (i, [vp, u64, l, vp, vp, vp]),
             "emx_philox_batch": (i, [l, vp, vp, vp, vp]),
@@ -258,6 +258,15 @@ class Problem:
                     null_int=int(sc.null_int), track_steps=int(sc.track_steps), stalls=int(sc.stalls),
                     iterations=int(sc.iterations), peak_live=int(sc.peak_live), peak_queue=int(sc.peak_queue),
                     ms=lib().emx_last_transport_ms(self.h))
+
+    def neighbour_candidates(self, surface, sense, which):
+        """cells tested, in order, after crossing `surface` towards `sense` (which = 0: listing it, 1: not listing it)"""
+        n = lib().emx_neighbour_candidates(self.h, int(surface), int(sense), int(which), None, 0)
+        if n < 0:
+            self._check(n)
+        out = np.zeros(max(n, 1), dtype=np.int32)
+        lib().emx_neighbour_candidates(self.h, int(surface), int(sense), int(which), out.ctypes.data, n)
+        return out[:n]
 
     def set_primary_offset(self, first):
         """the primaries of the following transports are primaries first, first + 1, ... of a longer list"""
