@@ -32,13 +32,21 @@ METRIC, UNIT = "track_steps_per_sec", "track-steps/s"
 # (x, u, E, tid, prim, step, vol, surf = 80 B) and written once (x, u, E, step, vol, surf, alive = 69 B);
 # per secondary one 76-byte record is written.
 B_STEP, B_SEC = 80 + 69, 76
-# dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the committed `ncu --set full` capture
-# of a saturated iteration (profiles/r1_final_step_kernels_full.md)
-TRAFFIC_PER_LAUNCH = {"k_step_pool<gamma>": 23.6e6, "k_step_pool<e->": 44.8e6, "k_step_pool<e+>": 8.6e6,
-                      "k_interact<gamma>": 26.9e6, "k_interact<e->": 26.6e6, "k_interact<e+>": 6.7e6}
-# sm__inst_executed_pipe_fp64 (fraction of peak) of the same capture: how far the kernels are from the fp64 ALU roof
-FP64_PIPE_NCU = {"k_step_pool<gamma>": 0.146, "k_step_pool<e->": 0.258, "k_step_pool<e+>": 0.114,
-                 "k_interact<gamma>": 0.136, "k_interact<e->": 0.094, "k_interact<e+>": 0.070}
+# Per workload, from the committed `ncu --set full` capture of one saturated iteration of that workload:
+# traffic = dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes); fp64 = sm__inst_executed_pipe_fp64 as a
+# fraction of peak (how far the kernels are from the fp64 ALU roof).  Workloads without a capture report null.
+NCU = {
+    4: {"source": "profiles/r1_final_step_kernels_full.md",
+        "traffic": {"k_step_pool<gamma>": 28.1e6, "k_step_pool<e->": 53.7e6, "k_step_pool<e+>": 10.7e6,
+                    "k_interact<gamma>": 33.8e6, "k_interact<e->": 30.9e6, "k_interact<e+>": 8.3e6},
+        "fp64": {"k_step_pool<gamma>": 0.146, "k_step_pool<e->": 0.268, "k_step_pool<e+>": 0.122,
+                 "k_interact<gamma>": 0.146, "k_interact<e->": 0.107, "k_interact<e+>": 0.071}},
+    7: {"source": "profiles/r1_config7_neighbour.md",
+        "traffic": {"k_step_pool<gamma>": 9.65e6, "k_step_pool<e->": 71.0e6, "k_step_pool<e+>": 3.99e6,
+                    "k_interact<gamma>": 9.05e6, "k_interact<e->": 9.37e6, "k_interact<e+>": 2.0e6},
+        "fp64": {"k_step_pool<gamma>": 0.083, "k_step_pool<e->": 0.111, "k_step_pool<e+>": 0.066,
+                 "k_interact<gamma>": 0.042, "k_interact<e->": 0.026, "k_interact<e+>": 0.012}},
+}
 
 
 def parse():
@@ -280,8 +288,9 @@ def run_ours(args):
     ach = alg_bytes / k_s / 1e9 if k_s > 0 else 0.0
     n_launch = max(rp["iterations"], 1)
     roof = {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-            "traffic": TRAFFIC_PER_LAUNCH.get(names[dom]),
-            "fp64_pipe_frac_ncu": FP64_PIPE_NCU.get(names[dom]),
+            "traffic": NCU.get(args.config, {}).get("traffic", {}).get(names[dom]),
+            "fp64_pipe_frac_ncu": NCU.get(args.config, {}).get("fp64", {}).get(names[dom]),
+            "ncu_source": NCU.get(args.config, {}).get("source"),
             "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s",
             "algorithmic_bytes_per_launch": alg_bytes / n_launch, "avg_launch_ms": kms[dom] / n_launch,
             "kernel_ms_profiled_pass": dict(zip(names + ["refill", "all_step_kernels"], [float(v) for v in kms])),
