@@ -35,7 +35,7 @@
 #define EMO_RE 2.8179403262e-13       /* cm */
 #define EMO_ALPHA 7.2973525693e-3
 #define EMO_NA 6.02214076e23          /* 1/mol */
-#define EMO_CB 2.99792458e-3          /* curvature: kappa[1/cm] = q*CB*B[T]/p[MeV/c] */
+#define EMO_CB 2.99792458             /* curvature: kappa[1/cm] = q*CB*B[T]/p[MeV/c]: r = p/(qB), 1e6 eV/c / (c * 1 T) = 0.333564 cm */
 #define EMO_PI 3.14159265358979323846
 
 /* process bits (process_mask) and process ids (counters, step results) */
