@@ -27,7 +27,7 @@ constexpr double kMe = 0.51099895000;       // electron mass, MeV
 constexpr double kRe = 2.8179403262e-13;    // classical electron radius, cm
 constexpr double kAlpha = 7.2973525693e-3;  // fine-structure constant
 constexpr double kNa = 6.02214076e23;       // Avogadro, 1/mol
-constexpr double kCB = 2.99792458e-3;       // curvature [1/cm] = q * kCB * B[T] / p[MeV/c]
+constexpr double kCB = 2.99792458;          // curvature [1/cm] = q * kCB * B[T] / p[MeV/c] (r = 0.33356 cm at 1 MeV/c, 1 T)
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kInf = __builtin_huge_val(); // +inf
 
