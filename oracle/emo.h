@@ -146,6 +146,7 @@ typedef struct {
     int n_draws;                 /* uniform draws consumed */
     int null_int;                /* 1 if the discrete interaction was kinematically null */
     int rest;                    /* 1 if an e+ annihilated at rest in this step */
+    int n_sub;                   /* substep attempts of the field propagation (0: straight move) */
 } emo_step_result;
 
 #define EMO_NHIST 96
@@ -223,6 +224,8 @@ void emo_rk4_doubling(const double x[3], const double u[3], double kappa, const 
                       double x1[3], double u1[3], double *err);
 double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x[3], double u[3],
                            double kappa, double s_max, int *hit);
+double emo_propagate_field_n(const emo_problem *p, int vol, int *surf_io, double x[3], double u[3],
+                             double kappa, double s_max, int *hit, int *n_sub);
 
 /* ---- interact.c : samplers; draws come from a callback-free draw cursor ---- */
 typedef struct { uint64_t seed; uint32_t prim; uint64_t tid; uint32_t step; uint32_t n; } emo_rng;

@@ -36,7 +36,7 @@ class StepResult(C.Structure):
     _fields_ = [("trk", Track), ("action", C.c_int), ("process", C.c_int), ("n_sec", C.c_int),
                 ("sec", Track * 4), ("sec_ord", C.c_int * 4), ("edep", C.c_double), ("edep_vol", C.c_int),
                 ("below_cut", C.c_double), ("escaped", C.c_double), ("looper", C.c_double), ("s", C.c_double),
-                ("msc_tau", C.c_double), ("n_draws", C.c_int), ("null_int", C.c_int), ("rest", C.c_int)]
+                ("msc_tau", C.c_double), ("n_draws", C.c_int), ("null_int", C.c_int), ("rest", C.c_int), ("n_sub", C.c_int)]
 
 
 class Rng(C.Structure):

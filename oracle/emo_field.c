@@ -94,13 +94,23 @@ void emo_rk4_doubling_map(const emo_problem *p, const double x[3], const double 
  * *hit = surface reached (-1: none).  x, u are updated in place. */
 double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x[3], double u[3],
                            double kappa, double s_max, int *hit) {
+    int n_sub;
+    return emo_propagate_field_n(p, vol, surf_io, x, u, kappa, s_max, hit, &n_sub);
+}
+
+/* the same, also counting the substep attempts (passes of the loop) in *n_sub: instrumentation for the level-2
+ * parity bound (the rounding of a step grows with its substeps), no arithmetic of its own */
+double emo_propagate_field_n(const emo_problem *p, int vol, int *surf_io, double x[3], double u[3],
+                             double kappa, double s_max, int *hit, int *n_sub) {
     const double eps = p->ph.field_eps;
     double s_done = 0.0;
     int surf = *surf_io;
     double h = 0.25 / fabs(kappa);
     if (s_max < h) h = s_max;
     *hit = -1;
+    *n_sub = 0;
     for (int attempt = 0; attempt < p->ph.max_substeps; ++attempt) {
+        *n_sub += 1;
         double rem = s_max - s_done;
         if (h > rem) h = rem;
         double x1[3], u1[3], err;

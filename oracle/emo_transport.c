@@ -131,7 +131,7 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
         double q = (pt == EMO_ELECTRON) ? -1.0 : 1.0;
         double kappa = q * EMO_CB * p->Bmag / pm;
         int sf = t->surf;
-        s = emo_propagate_field(p, vol, &sf, t->x, t->u, kappa, s_phys, &hit);
+        s = emo_propagate_field_n(p, vol, &sf, t->x, t->u, kappa, s_phys, &hit, &out->n_sub);
         if (hit >= 0) { action = EMO_A_BOUNDARY; full = 0; }
         else if (!(s >= s_phys * (1.0 - 1e-14))) { action = EMO_A_TRUNC; full = 0; }
     }
