@@ -28,25 +28,33 @@ sys.path.insert(0, ROOT)
 from paper_2203_09467_b200 import workloads as W  # noqa: E402
 
 METRIC, UNIT = "track_steps_per_sec", "track-steps/s"
-# algorithmic DRAM bytes of the step kernel: per track-step the slot is read once
-# (x, u, E, tid, prim, step, vol, surf = 80 B) and written once (x, u, E, step, vol, surf, alive = 69 B);
-# per secondary one 76-byte record is written.
-B_STEP, B_SEC = 80 + 69, 76
-# Per workload, from the committed `ncu --set full` capture of one saturated iteration of that workload:
-# traffic = dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes); fp64 = sm__inst_executed_pipe_fp64 as a
-# fraction of peak (how far the kernels are from the fp64 ALU roof).  Workloads without a capture report null.
-NCU = {
-    4: {"source": "profiles/r1_final_step_kernels_full.md",
-        "traffic": {"k_step_pool<gamma>": 28.1e6, "k_step_pool<e->": 53.7e6, "k_step_pool<e+>": 10.7e6,
-                    "k_interact<gamma>": 33.8e6, "k_interact<e->": 30.9e6, "k_interact<e+>": 8.3e6},
-        "fp64": {"k_step_pool<gamma>": 0.146, "k_step_pool<e->": 0.268, "k_step_pool<e+>": 0.122,
-                 "k_interact<gamma>": 0.146, "k_interact<e->": 0.107, "k_interact<e+>": 0.071}},
-    7: {"source": "profiles/r1_config7_neighbour.md",
-        "traffic": {"k_step_pool<gamma>": 9.65e6, "k_step_pool<e->": 71.0e6, "k_step_pool<e+>": 3.99e6,
-                    "k_interact<gamma>": 9.05e6, "k_interact<e->": 9.37e6, "k_interact<e+>": 2.0e6},
-        "fp64": {"k_step_pool<gamma>": 0.083, "k_step_pool<e->": 0.111, "k_step_pool<e+>": 0.066,
-                 "k_interact<gamma>": 0.042, "k_interact<e->": 0.026, "k_interact<e+>": 0.012}},
+# Algorithmic bytes per unit of each step kernel (five 16-byte words per slot -- (x, y), (z, ux),
+# (uy, uz), (E, track id), (prim, step, vol, surf) -- plus one-byte flags; 80-byte stack records).  Units = the slots
+# the kernel processed, counted by the kernel itself (emx_get_lanes).
+B_STAGE = {
+    "k_a<gamma>": 82 + 50,        # slot read (5 words, alive, stage) + (x, y), (z, ux), ids, alive, stage written
+    "k_a<charged>": 83 + 66,      # + ptype read; + (E, id) written
+    "k_a0": 35 + 10,              # (E, id), ids, stage, ptype read; s_phys, act, stage written
+    "k_field": 91 + 62,           # slot + s_phys, act, ptype, stage read; 3 words + path, surface hit, act, stage written
+    "k_a2": 97 + 34,              # slot + act, path, hit, stage, alive, ptype read; (E, id), ids, alive, stage written
+    "k_b<gamma>": 4 + 81 + 66,    # list entry + slot read; (z, ux), (uy, uz), (E, id), ids, alive, stage written
+    "k_b<charged>": 4 + 82 + 66,
 }
+B_SEC = 80                        # one stack record per secondary, written by the phase-B kernels
+
+
+def load_ncu_profile(config):
+    """ncu-derived constants of the committed capture of this workload (profiles/r2_ncu_config<k>.json, written by
+    `python -m paper_2203_09467_b200.diagnostics.ncu_extract` from the .ncu-rep): DRAM bytes per launch and fp64
+    instructions per unit of each kernel.  None when no capture of this workload is committed."""
+    path = os.path.join(ROOT, "profiles", "r2_ncu_config%d.json" % config)
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        d["file"] = os.path.relpath(path, ROOT)
+        return d
+    except (OSError, ValueError):
+        return None
 
 
 def parse():
@@ -217,7 +225,7 @@ def run_ours(args):
     if rank == 0:
         clocks.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    tot = dict(steps=0, sec=0, kms=np.zeros(4), launches=0, per_type=np.zeros(3), sec_type=np.zeros(3), iters=0)
+    tot = dict(steps=0, sec=0, launches=0, per_type=np.zeros(3), sec_type=np.zeros(3), iters=0)
     barrier()
     ev0.record()
     for _ in range(args.steps):
@@ -243,7 +251,6 @@ def run_ours(args):
     G.set_profile(True)
     rp = G.transport(pdev, seed)
     prof = G.profile()
-    tot["kms"] = np.array(prof["ms"])
     prof_ms = rp["ms"]
     G.set_profile(False)
 
@@ -265,19 +272,18 @@ def run_ours(args):
         return
 
     value = all_steps / (ms * 1e-3)
-    # roofline of the dominant kernel.  The profiled pass brackets each of the six step kernels of every
-    # iteration with CUDA events; the dominant one is the kernel with the largest total.  Its algorithmic
-    # bytes = the track slots it processed (counted by the kernel) x bytes per slot.
-    names = ["k_step_pool<gamma>", "k_step_pool<e->", "k_step_pool<e+>", "k_interact<gamma>", "k_interact<e->",
-             "k_interact<e+>"]
-    kms = tot["kms"]                      # ms of the profiled pass per kernel
-    dom = int(np.argmax(kms[:6]))
+    # roofline of the dominant kernel.  The profiled pass brackets every step kernel of every iteration with CUDA
+    # events; the dominant one is the kernel with the largest total.  Its algorithmic bytes = the track slots it
+    # processed (counted by the kernel) x bytes per slot (B_STAGE).
+    names = list(emx.STAGES)
+    kms = prof["ms"]                      # ms of the profiled pass per kernel
+    dom = max(names, key=lambda k: kms[k])
     lanes = float(prof["lanes"][dom])
     n_sec = float(tot["sec_type"].sum()) / args.steps
-    if dom < 3:
-        alg_bytes = lanes * B_STEP        # phase A: slot read (80 B) + written back (69 B)
-    else:
-        alg_bytes = lanes * (B_STEP + 4) + n_sec * B_SEC * (lanes / max(sum(prof["lanes"][3:6]), 1.0))
+    alg_bytes = lanes * B_STAGE[dom]
+    if dom.startswith("k_b"):
+        nb = float(prof["lanes"]["k_b<gamma>"] + prof["lanes"]["k_b<charged>"])
+        alg_bytes += n_sec * B_SEC * (lanes / max(nb, 1.0))
     k_s = kms[dom] * 1e-3
     peaks = {}
     try:
@@ -287,18 +293,29 @@ def run_ours(args):
     peak = float(peaks.get("hbm_gbs", 6650.0))
     ach = alg_bytes / k_s / 1e9 if k_s > 0 else 0.0
     n_launch = max(rp["iterations"], 1)
-    roof = {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-            "traffic": NCU.get(args.config, {}).get("traffic", {}).get(names[dom]),
-            "fp64_pipe_frac_ncu": NCU.get(args.config, {}).get("fp64", {}).get(names[dom]),
-            "ncu_source": NCU.get(args.config, {}).get("source"),
+    ncu = load_ncu_profile(args.config)
+    kn = (ncu or {}).get("kernels", {}).get(dom, {})
+    all_bytes = sum(float(prof["lanes"][k]) * B_STAGE[k] for k in names) + n_sec * B_SEC
+    roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "traffic": kn.get("dram_bytes_per_launch"),
             "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s",
             "algorithmic_bytes_per_launch": alg_bytes / n_launch, "avg_launch_ms": kms[dom] / n_launch,
-            "kernel_ms_profiled_pass": dict(zip(names + ["refill", "all_step_kernels"], [float(v) for v in kms])),
+            "units_per_launch": lanes / n_launch,
+            "kernel_ms_profiled_pass": {k: float(v) for k, v in kms.items()},
             "kernel_share_of_profiled_pass": float(kms[dom] / prof_ms), "profiled_pass_ms": prof_ms,
-            "all_step_kernels": {"achieved_GBs": float((sum(prof["lanes"][:3]) * B_STEP + sum(prof["lanes"][3:6]) * (B_STEP + 4)
-                                                        + n_sec * B_SEC) / (kms[7] * 1e-3) / 1e9)},
-            "note": "not HBM-bound on B200: the 95 MB track store stays in the 126 MB L2 (traffic < algorithmic "
-                    "bytes); the step kernels are latency / divergence bound, see DESIGN.md section 7"}
+            "all_step_kernels": {"achieved_GBs": float(all_bytes / (kms["all_step_kernels"] * 1e-3) / 1e9)},
+            "ncu_capture": None if ncu is None else {"file": ncu["file"], "build": ncu.get("build"), "measured_by_this_run": False}}
+    # the roofs that actually bind (profiles/r2_peaks.md): the propagation kernel is fp64 arithmetic, the track
+    # store lives in L2.  fp64 work = instructions per substep attempt from the committed capture x the attempts
+    # this run counted; L2 bytes = the algorithmic bytes (the store is L2-resident: DRAM traffic is below them)
+    pk = (ncu or {}).get("peaks", {})
+    if dom == "k_field" and kn.get("fp64_inst_per_attempt") and pk.get("fp64_tinst_per_s"):
+        work = float(kn["fp64_inst_per_attempt"]) * float(prof["attempts"])
+        roof["alu"] = {"bound": "alu", "achieved": work / k_s / 1e12, "peak": pk["fp64_tinst_per_s"] / 1e12,
+                       "unit": "T fp64 thread-instructions/s", "frac": work / k_s / pk["fp64_tinst_per_s"],
+                       "attempts_per_launch": float(prof["attempts"]) / n_launch}
+    if pk.get("l2_gbs"):
+        roof["l2"] = {"achieved": ach, "peak": pk["l2_gbs"], "unit": "GB/s", "frac": ach / pk["l2_gbs"]}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -309,7 +326,8 @@ def run_ours(args):
            "primaries_per_sec": n_prim * args.steps * world / (ms * 1e-3),
            "iterations_per_step": tot["iters"] / args.steps, "peak_live": last["peak_live"], "peak_queue": last["peak_queue"],
            "e2e": {"value": all_e2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-           "gpu_launches": int(tot["launches"]), "clocks": clk, "roofline": roof}
+           "gpu_launches": int(tot["launches"]), "clocks": clk, "roofline": roof,
+           "field_attempts_per_step": float(prof["attempts"])}
     if not args.no_cpu_baseline and world == 1:
         threads = os.cpu_count() or 1
         n_s = oracle_sample_size(desc, prim, threads)

@@ -176,6 +176,7 @@ typedef struct {
     int32_t n_draws;        /* uniforms consumed */
     int32_t null_int;
     int32_t rest;           /* e+ annihilated at rest in this step */
+    int32_t n_sub;          /* substep attempts of the field propagation behind this step (0: straight move) */
 } emx_step_result;
 
 /* ---- problem description (host side; arrays are HOST pointers, copied during the call) ---- */
@@ -246,11 +247,18 @@ int emx_transport(emx_problem *p, long n_primaries, const int *ptype, const doub
                   long n_slots, long queue_capacity, void *workspace, size_t workspace_bytes, void *stream);
 
 /* Same call with every primary array in HOST memory (pageable or pinned): uploads on `stream`,
- * transports, and leaves the tallies readable.  This is the end-to-end entry bench.py times as `e2e`. */
+ * transports, and leaves the tallies readable.  This is the end-to-end entry bench.py times as `e2e`.
+ * The primaries are staged in the caller's workspace: workspace_bytes must be at least
+ * emx_workspace_bytes(n_slots, queue_capacity) + emx_staging_bytes(n_primaries) (EMX_E_CAPACITY otherwise); the
+ * library allocates nothing. */
 int emx_transport_host(emx_problem *p, long n_primaries, const int *ptype, const double *E,
                        const double *pos3, const double *dir3, const int *start_vol, const int *start_surf,
                        uint64_t seed, long n_slots, long queue_capacity, void *workspace,
                        size_t workspace_bytes, void *stream);
+
+/* Bytes emx_transport_host needs behind the workspace proper to stage n_primaries primaries (52 bytes each,
+ * every array 256-byte aligned). */
+size_t emx_staging_bytes(long n_primaries);
 
 int emx_reset_tallies(emx_problem *p, void *stream);
 
@@ -261,13 +269,26 @@ int emx_reset_tallies(emx_problem *p, void *stream);
  * Default 0.  first + n must stay below 2^32 (EMX_E_ARG otherwise, here or in emx_transport). */
 int emx_set_primary_offset(emx_problem *p, long first);
 
-/* Share of the track slots given to the photon, electron and positron pools (the number of
- * track slots and the queue are what bounds a run; one pool per particle type).  The three
- * numbers are normalised to their sum; all must be > 0 (EMX_E_ARG otherwise).  The split decides WHEN a track
- * is stepped, never what its steps compute: results do not depend on it.  It enters emx_workspace_bytes, so set
- * it before sizing the workspace.  Default: 50 / 42 / 8, with multiple scattering 25 / 63 / 12; (0, 0, 0)
- * restores the default.  Measured optimum on one B200: 40 / 50 / 10 for the barrel of config 4 (+2.5 %). */
-int emx_set_pool_split(emx_problem *p, double f_gamma, double f_electron, double f_positron);
+/* Scheduling of the loop (track slots, queued initializers, time per step iteration).  Nothing
+ * here changes what a step computes: histories are keyed by (seed, primary, track id, step), so the counters of a
+ * run are the same under every schedule and its tallies are the same up to the order of their sums.
+ *   loop_node      1 (default): the whole loop is one CUDA graph with a WHILE node; 0: graphs of 8 iterations
+ *                  launched in batches with a look at the done flag in between (also the fallback when the driver
+ *                  refuses conditional nodes).
+ *   slice_min / slice_max / slice_above   time slicing of the field propagation: while more
+ *                  than slice_above tracks are live (< 0: n_slots / 32), a propagation that has used slice_min
+ *                  substep attempts in this iteration is parked for the next one as soon as its pool has no
+ *                  unstarted track left, and after slice_max attempts in any case.  Defaults 2 / 16 / -1.
+ *   blocks_per_sm  persistent 128-thread blocks per SM of each step kernel, in the order k_a<gamma>,
+ *                  k_a<charged>, k_a0, k_field, k_a2, k_b<gamma>, k_b<charged> (entry 7 unused); 0 = default. */
+typedef struct {
+    int32_t loop_node;
+    int32_t slice_min, slice_max;
+    int64_t slice_above;
+    int32_t blocks_per_sm[8];
+} emx_schedule;
+int emx_get_schedule(const emx_problem *p, emx_schedule *out);
+int emx_set_schedule(emx_problem *p, const emx_schedule *in);
 
 /* edep_host[n_tally] (MeV per tally id) and the run totals, copied to HOST memory. */
 int emx_read_tallies(const emx_problem *p, double *edep_host, emx_scalars *out);
@@ -282,18 +303,20 @@ int emx_read_step_hist(const emx_problem *p, uint64_t *hist_host);
 double emx_last_transport_ms(const emx_problem *p);
 
 /* Per-kernel timing of the loop.  Normally emx_transport runs the whole loop as ONE CUDA graph (a WHILE node
- * whose body is 8 iterations, the pools' step kernels as parallel branches, and a kernel that sets the node's
- * condition from the done flag) on internal streams ordered after `stream`.  With
- * profiling on (on = 1) it launches kernel by kernel on `stream` instead and brackets every launch with
- * CUDA events on that stream.  emx_get_profile: ms8[8] = milliseconds of the last transport spent in
- * { phase A (k_step_pool) gamma, e-, e+, phase B (k_interact) gamma, e-, e+, refill (k_plan + k_fill +
- * k_move), all step kernels }; *launches = kernels launched by the last transport (always counted);
- * *iterations_launched = iterations run, empty ones included (>= iterations needed: the done flag is looked at
- * once per 8 iterations in the graph, once per batch of launches otherwise).  emx_get_lanes: lanes6[6] = track slots processed by { phase A gamma, e-, e+, phase B gamma, e-, e+ }
- * over the last transport (the units of each kernel's algorithmic bytes).  Output pointers may be NULL. */
+ * whose body is 8 iterations, the two pools' kernel chains as parallel branches, and a kernel that sets the node's
+ * condition from the done flag) on internal streams ordered after `stream`.  on = 1: the kernels are launched
+ * one by one on `stream` instead and every launch is bracketed by CUDA events on that stream; on = 2: launched
+ * one by one without the events (what a profiler can list).  emx_get_profile: ms9[9] = milliseconds of the last
+ * transport spent in { k_a<gamma>, k_a<charged> (no field), k_a0, k_field, k_a2 (field), k_b<gamma>,
+ * k_b<charged>, refill (k_plan + k_fill + k_move), all step kernels }; *launches = kernels launched by the last
+ * transport (always counted); *iterations_launched = iterations run, empty ones included (>= iterations needed:
+ * the done flag is looked at once per 8 iterations in the graph, once per batch of launches otherwise).
+ * emx_get_lanes: lanes8[0..6] = track slots processed by those seven kernels over the last transport (the units
+ * of each kernel's algorithmic bytes), lanes8[7] = substep attempts of the field propagation.  Output pointers
+ * may be NULL. */
 int emx_set_profile(emx_problem *p, int on);
-int emx_get_profile(const emx_problem *p, double *ms8, long *launches, long *iterations_launched);
-int emx_get_lanes(const emx_problem *p, uint64_t *lanes6);
+int emx_get_profile(const emx_problem *p, double *ms9, long *launches, long *iterations_launched);
+int emx_get_lanes(const emx_problem *p, uint64_t *lanes8);
 
 /* Per-iteration diagnostics of the last transport (Fig. 5): up to `max_iter` rows of
  * { live tracks, queued initializers } as uint32 pairs in HOST memory; returns rows written. */

@@ -38,7 +38,7 @@ struct emx_problem {
     // optional per-kernel timing of the loop (emx_set_profile)
     bool profile = false;
     std::vector<cudaEvent_t> prof_ev;
-    double prof_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // phase A gamma, e-, e+; phase B gamma, e-, e+; refill; all step kernels
+    double prof_ms[kNStages + 2] = {0};  // the step kernels by stage (emx_kernels.h), refill, all step kernels
     int n_sm = 148;
     long launches = 0, iterations_launched = 0;
     std::vector<float> iter_ms;  // per iteration: refill ms, step ms (profiling on)
@@ -53,13 +53,11 @@ struct emx_problem {
     Primaries graph_pr;
     uint64_t graph_seed = 0;
     unsigned long long graph_gen = 0, params_gen = 1;
-    int loop_node = 1;         // 1: the whole loop is one graph with a WHILE node; 0: flat graphs + host polling
     bool graph_is_loop = false;
     bool use_graph = true;
-    long slice_above = -1;  // < 0: n_slots / 32
-    int slice_budget = 2;
-    int warps_per_sm[3] = {16, 16, 8};  // gamma, e-, e+ (the e+ pool holds 8 % of the slots)
-    double pool_frac[3] = {0.0, 0.0, 0.0};  // EMX_POOL_FRAC: share of the slots per pool (0: the default split)
+    emx_schedule sched;        // emx_set_schedule: when work is done, never what it computes
+    // production thresholds given with emx_set_cuts (< 0: derive from the cut length at every build)
+    std::vector<double> user_Tcut, user_kcut;
 };
 
 namespace {
@@ -93,20 +91,7 @@ void free_device(emx_problem *p) {
     p->hp.built = false;
 }
 
-// split n into three pool sizes (gamma, e-, e+), each a multiple of kChunk
-void split3(long n, const double f[3], int out[3]) {
-    long used = 0;
-    for (int k = 0; k < 3; ++k) {
-        long v = (long)((double)n * f[k]) / kChunk * kChunk;
-        if (v < kChunk) v = kChunk;
-        out[k] = (int)v;
-        used += v;
-    }
-    (void)used;
-}
-
-const double kPoolFrac[3] = {0.50, 0.42, 0.08};   // measured live mix of the workloads
-const double kQueueFrac[3] = {0.30, 0.60, 0.10};  // e- secondaries dominate the queued records in every config
+const double kQueueFrac[kPools] = {0.30, 0.70};  // e+- secondaries dominate the queued records in every config
 
 struct Carve {
     char *base;
@@ -120,61 +105,60 @@ struct Carve {
     }
 };
 
-// with multiple scattering the charged tracks take ~7x the steps: measured on config 7, +24 % over the split above
-const double kPoolFracMsc[3] = {0.25, 0.63, 0.12};
-// share of the track slots per pool: the knob if set, else the default split for the physics of the problem
-// (the split decides when a step is taken, never its result)
-static const double *pool_split(const emx_problem *p) {
-    return p->pool_frac[0] > 0.0 ? p->pool_frac : (p->hp.ph.msc ? kPoolFracMsc : kPoolFrac);
+// stack capacities: the two shares of queue_capacity, each at least one chunk
+void split_queue(long qcap, int out[kPools]) {
+    for (int k = 0; k < kPools; ++k) {
+        long v = (long)((double)qcap * kQueueFrac[k]);
+        if (v < kChunk) v = kChunk;
+        out[k] = (int)v;
+    }
 }
 
 // carve the caller's workspace; with base == nullptr only the size is computed
-size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log, const double *pool_frac) {
+size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
     Carve c{base};
-    split3(n_slots, pool_frac, w.cap);
-    split3(qcap, kQueueFrac, w.qcap);
+    int nch = (int)((n_slots + kChunk - 1) / kChunk);
+    if (nch < 2) nch = 2;  // one chunk per pool at least
+    w.n_chunks = nch;
+    w.slot_cap = nch * kChunk;
+    w.pool_reserve = nch / 32 > 1 ? nch / 32 : 1;
+    split_queue(qcap, w.qcap);
     w.ctl = c.take<Ctl>(1);
     w.log = c.take<uint32_t>(2 * (size_t)max_log);
     w.max_log = max_log;
-    for (int p = 0; p < 3; ++p) {
-        const size_t n = (size_t)w.cap[p], nch = n / kChunk + 1;
-        TrackSoA &t = w.trk[p];
-        t.x = c.take<double>(n); t.y = c.take<double>(n); t.z = c.take<double>(n);
-        t.ux = c.take<double>(n); t.uy = c.take<double>(n); t.uz = c.take<double>(n);
-        t.E = c.take<double>(n);
-        t.tid = c.take<uint64_t>(n);
-        t.prim = c.take<uint32_t>(n); t.step = c.take<uint32_t>(n);
-        t.vol = c.take<int>(n); t.surf = c.take<int>(n);
-        t.alive = c.take<uint8_t>(n);
-        t.pend = c.take<uint8_t>(n);
-        if (p != 0) {
-            t.fs_s = c.take<double>(n);
-            t.fs_h = c.take<double>(n);
-            t.fs_a = c.take<int>(n);
-        } else {
-            t.fs_s = t.fs_h = nullptr;
-            t.fs_a = nullptr;
-        }
-        w.chunk_dead[p] = c.take<int>(nch);
-        w.chunk_off[p] = c.take<int>(nch);
+    const size_t n = (size_t)nch * kChunk;
+    Store &t = w.st;
+    t.xy = c.take<double2>(n); t.zu = c.take<double2>(n); t.uu = c.take<double2>(n);
+    t.Et = c.take<double2>(n);
+    t.id = c.take<int4>(n);
+    t.alive = c.take<uint8_t>(n); t.stage = c.take<uint8_t>(n); t.ptype = c.take<uint8_t>(n); t.act = c.take<uint8_t>(n);
+    t.s_phys = c.take<double>(n); t.s_done = c.take<double>(n); t.h_try = c.take<double>(n);
+    t.att = c.take<int>(n);
+    w.free_list = c.take<int>((size_t)nch);
+    for (int p = 0; p < kPools; ++p) {
+        w.ctab[p] = c.take<int>((size_t)nch);
+        w.chunk_dead[p] = c.take<int>((size_t)nch + 1);
+        w.chunk_off[p] = c.take<int>((size_t)nch + 1);
         w.hole_idx[p] = c.take<int>(n);
-        for (int k = 0; k < 3; ++k) w.ilist[p][k] = c.take<int>(n);
+        for (int k = 0; k < kMaxLists; ++k) w.ilist[p][k] = (p == kPoolGamma && k == 3) ? nullptr : c.take<int>(n);
     }
-    // everything above (track store, scan arrays, interaction lists: about 110 MB at 2^20 slots) is touched in
-    // every iteration and is kept together; the stacks follow.  (A persisting-L2 access-policy window over
-    // this region was tried: 83 MB can be set aside on B200, and it was 9 % slower.)
-    w.hot_bytes = align_up(c.off, 256);
-    for (int p = 0; p < 3; ++p) {
+    // everything above (track store, scan arrays, interaction lists: about 150 MB of addresses at 2^20 slots, of
+    // which an iteration touches what the live tracks need) is kept together; the stacks follow
+    for (int p = 0; p < kPools; ++p) {
         const size_t q = (size_t)w.qcap[p];
-        QueueSoA &s = w.q[p];
-        s.x = c.take<double>(q); s.y = c.take<double>(q); s.z = c.take<double>(q);
-        s.ux = c.take<double>(q); s.uy = c.take<double>(q); s.uz = c.take<double>(q);
-        s.E = c.take<double>(q);
-        s.tid = c.take<uint64_t>(q);
-        s.prim = c.take<uint32_t>(q);
-        s.vol = c.take<int>(q); s.surf = c.take<int>(q);
+        Stack &s = w.q[p];
+        s.xy = c.take<double2>(q); s.zu = c.take<double2>(q); s.uu = c.take<double2>(q);
+        s.Et = c.take<double2>(q);
+        s.id = c.take<int4>(q);
     }
     return align_up(c.off, 256);
+}
+
+// staging area of emx_transport_host behind the workspace proper: the six primary arrays (4 + 8 + 24 + 24 + 4 + 4
+// bytes per primary)
+size_t staging_bytes(long n) {
+    const size_t nn = (size_t)(n > 0 ? n : 1);
+    return align_up(nn * 4, 256) * 3 + align_up(nn * 8, 256) + 2 * align_up(nn * 24, 256);
 }
 
 constexpr int kMaxLog = 1 << 16;
@@ -191,16 +175,11 @@ int emx_create(emx_problem **out) {
     if (!out) return fail(nullptr, EMX_E_ARG, "emx_create: null output");
     emx_problem *p = new (std::nothrow) emx_problem();
     if (!p) return fail(nullptr, EMX_E_NOMEM, "emx_create: out of memory");
-    // tuning knobs of the scheduler (they never change a result, only when work is done)
-    if (const char *e = getenv("EMX_SLICE_BUDGET")) p->slice_budget = atoi(e) > 0 ? atoi(e) : p->slice_budget;
-    if (const char *e = getenv("EMX_SLICE_ABOVE")) p->slice_above = atol(e);
-    if (const char *e = getenv("EMX_LOOP_NODE")) p->loop_node = atoi(e);
-    if (const char *e = getenv("EMX_POOL_FRAC")) {
-        double f[3] = {0, 0, 0};
-        if (sscanf(e, "%lf,%lf,%lf", &f[0], &f[1], &f[2]) == 3 && f[0] > 0 && f[1] > 0 && f[2] > 0)
-            for (int k = 0; k < 3; ++k) p->pool_frac[k] = f[k] / (f[0] + f[1] + f[2]);
-    }
-    if (const char *e = getenv("EMX_WARPS_PER_SM")) sscanf(e, "%d,%d,%d", &p->warps_per_sm[0], &p->warps_per_sm[1], &p->warps_per_sm[2]);
+    p->sched.loop_node = 1;
+    p->sched.slice_min = 2;
+    p->sched.slice_max = 16;
+    p->sched.slice_above = -1;
+    for (int k = 0; k < 8; ++k) p->sched.blocks_per_sm[k] = 0;
     *out = p;
     return EMX_OK;
 }
@@ -227,6 +206,8 @@ int emx_add_material(emx_problem *p, int n_elem, const int *Z, const double *A, 
     if (!derive_material(m, n_elem, Z, A, mass_frac, density_g_cm3, mean_exc_energy_eV))
         return fail(p, EMX_E_ARG, "emx_add_material: invalid element list, density or mean excitation energy");
     p->hp.mat.push_back(m);
+    p->user_Tcut.push_back(-1.0);
+    p->user_kcut.push_back(-1.0);
     p->hp.built = false;
     return (int)p->hp.mat.size() - 1;
 }
@@ -304,8 +285,8 @@ int emx_set_physics(emx_problem *p, const emx_physics *ph) {
 
 int emx_set_cuts(emx_problem *p, int material, double Tcut, double kcut) {
     if (!p || material < 0 || material >= (int)p->hp.mat.size()) return fail(p, EMX_E_ARG, "emx_set_cuts: unknown material");
-    p->hp.mat[material].Tcut = Tcut;
-    p->hp.mat[material].kcut = kcut;
+    p->user_Tcut[material] = Tcut;  // < 0: back to the cut-length conversion
+    p->user_kcut[material] = kcut;
     p->hp.built = false;
     return EMX_OK;
 }
@@ -316,9 +297,14 @@ int emx_build_tables(emx_problem *p, void *stream) {
     if (!p) return fail(p, EMX_E_ARG, "emx_build_tables: null problem");
     HostProblem &hp = p->hp;
     if (hp.vol.empty()) return fail(p, EMX_E_STATE, "emx_build_tables: no volume defined");
-    for (const Material &m : hp.mat)
-        if (!(hp.ph.prod_cut_cm > 0.0) && (m.Tcut < 0.0 || m.kcut < 0.0))
+    // every build starts from what the caller set: the thresholds a previous build derived from another cut length
+    // or another grid must not survive it
+    for (size_t im = 0; im < hp.mat.size(); ++im) {
+        hp.mat[im].Tcut = p->user_Tcut[im];
+        hp.mat[im].kcut = p->user_kcut[im];
+        if (!(hp.ph.prod_cut_cm > 0.0) && (hp.mat[im].Tcut < 0.0 || hp.mat[im].kcut < 0.0))
             return fail(p, EMX_E_STATE, "emx_build_tables: no production cut length and no explicit cut energies");
+    }
     cudaStream_t st = (cudaStream_t)stream;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
@@ -442,12 +428,17 @@ int emx_get_material_info(const emx_problem *p, int material, double *o) {
     return EMX_OK;
 }
 
-size_t emx_workspace_bytes(const emx_problem *p, long n_slots, long queue_capacity) {
-    // pools hold fewer than 2^21 slots each (packed list counters): n_slots <= 2^21
-    if (!p || n_slots < 1 || queue_capacity < 1 || n_slots > (1L << 21) || queue_capacity > (1L << 30)) return 0;
-    Work w;
-    return carve_work(nullptr, n_slots, queue_capacity, w, kMaxLog, pool_split(p));
+static bool sizes_ok(long n_slots, long queue_capacity) {
+    return n_slots >= 1 && queue_capacity >= 1 && n_slots <= (1L << 22) && queue_capacity <= (1L << 30);
 }
+
+size_t emx_workspace_bytes(const emx_problem *p, long n_slots, long queue_capacity) {
+    if (!p || !sizes_ok(n_slots, queue_capacity)) return 0;
+    Work w;
+    return carve_work(nullptr, n_slots, queue_capacity, w, kMaxLog);
+}
+
+size_t emx_staging_bytes(long n_primaries) { return n_primaries < 0 ? 0 : staging_bytes(n_primaries); }
 
 int emx_reset_tallies(emx_problem *p, void *stream) {
     if (!p || !p->hp.built) return fail(p, EMX_E_STATE, "emx_reset_tallies: tables not built");
@@ -455,21 +446,42 @@ int emx_reset_tallies(emx_problem *p, void *stream) {
     return EMX_OK;
 }
 
+// blocks of the persistent step kernels: blocks_per_sm of the schedule, else what the compiled kernel's launch
+// bounds allow, shared between the chains that run side by side
+static void size_grids(const emx_problem *p, Work &w) {
+    // defaults per stage (kStage*): 128-thread blocks per SM
+    static const int kDefault[kNStages] = {3, 4, 8, 5, 5, 3, 3};
+    for (int k = 0; k < kNStages; ++k) {
+        int b = p->sched.blocks_per_sm[k] > 0 ? p->sched.blocks_per_sm[k] : kDefault[k];
+        if (b > 16) b = 16;
+        w.grid[k] = p->n_sm * b;
+    }
+    w.grid[7] = 0;
+    // what all resident warps of the step kernels can ask of a stack at the same time: 64 warps per SM,
+    // 32 lanes x 4 records each
+    w.reserve_slack = p->n_sm * 64 * 128;
+}
+
 static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, long n_slots, long queue_capacity,
                             void *workspace, size_t workspace_bytes, cudaStream_t st) {
     if (pr.first + pr.n > 0x100000000LL) return fail(p, EMX_E_ARG, "emx_transport: primary indices beyond 2^32");
+    if (!sizes_ok(n_slots, queue_capacity))
+        return fail(p, EMX_E_ARG, "emx_transport: n_slots must be in [1, 2^22] and queue_capacity in [1, 2^30]");
     Work w;
     memset(&w, 0, sizeof(w));  // compared bytewise with the arguments of the kept graph
-    const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog, pool_split(p));
+    const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog);
     if (need > workspace_bytes) return fail(p, EMX_E_CAPACITY, "emx_transport: workspace smaller than emx_workspace_bytes()");
     // admission limits (R8): about 20 MeV of shower energy in flight per queued record at the peak of
     // the queue (measured on configs 1-4), with a factor 4 of headroom below the capacity
     w.n_primaries = pr.n;
     w.wave = (int)(n_slots / 256 < 256 ? 256 : (n_slots / 256 > 4096 ? 4096 : n_slots / 256));
     w.inflight_cap = 5.0 * (double)queue_capacity;
-    w.slice_above = p->slice_above >= 0 ? p->slice_above : n_slots / 32;
-    w.slice_budget = p->slice_budget;
-    for (int k = 0; k < 3; ++k) w.warps_per_sm[k] = p->warps_per_sm[k];
+    w.slice_above = p->sched.slice_above >= 0 ? p->sched.slice_above : n_slots / 32;
+    w.slice_min = p->sched.slice_min > 0 ? p->sched.slice_min : 1;
+    w.slice_max = p->sched.slice_max >= w.slice_min ? p->sched.slice_max : w.slice_min;
+    size_grids(p, w);
+    const bool field = p->P.Bmag != 0.0;
+    const int per_iter = launches_per_iteration(field);
     CU(cudaEventRecord(p->ev0, st));
     CU(launch_init(w, pr, st));
     p->launches = 1;
@@ -478,8 +490,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     p->iter_ms.clear();
     if (p->use_graph && !p->profile) {
         // ---- device-driven path: kIterPerGraph iterations captured once as a CUDA graph; inside an iteration
-        // the three step kernels are parallel branches, so the tail of one pool overlaps the start of the next.
-        // The host only looks at the done flag between graph launches.
+        // the two pools' chains are parallel branches.  The host only looks at the done flag between graph launches.
         constexpr int kIterPerGraph = 8;
         CU(cudaEventRecord(p->evIn, st));
         CU(cudaStreamWaitEvent(p->s0, p->evIn, 0));
@@ -488,24 +499,21 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         memset(&prz, 0, sizeof(prz));
         prz.n = pr.n; prz.ptype = pr.ptype; prz.E = pr.E; prz.pos3 = pr.pos3; prz.dir3 = pr.dir3;
         prz.vol = pr.vol; prz.surf = pr.surf; prz.first = pr.first;
+        const bool want_loop = p->sched.loop_node != 0;
         const bool keep = p->graph_exec && p->graph_gen == p->params_gen && p->graph_seed == seed &&
-                          p->graph_is_loop == (p->loop_node != 0) &&
+                          p->graph_is_loop == want_loop &&
                           memcmp(&p->graph_w, &w, sizeof(Work)) == 0 && memcmp(&p->graph_pr, &prz, sizeof(Primaries)) == 0;
-        // kIterPerGraph iterations of the loop, captured from s0 (fork / join over s1, s2)
+        // kIterPerGraph iterations of the loop, captured from s0 (fork / join over s1)
         auto capture_iterations = [&]() -> cudaError_t {
             cudaError_t e = cudaSuccess;
             for (int k = 0; k < kIterPerGraph && e == cudaSuccess; ++k) {
                 e = launch_refill(w, pr, p->s0);
                 if (e == cudaSuccess) e = cudaEventRecord(p->evFork, p->s0);
                 if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s1, p->evFork, 0);
-                if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s2, p->evFork, 0);
-                if (e == cudaSuccess) e = launch_step_pool(kPositron, p->P, w, seed, p->d_tally, p->n_sm, p->s1);
-                if (e == cudaSuccess) e = launch_step_pool(kElectron, p->P, w, seed, p->d_tally, p->n_sm, p->s2);
-                if (e == cudaSuccess) e = launch_step_pool(kGamma, p->P, w, seed, p->d_tally, p->n_sm, p->s0);
+                if (e == cudaSuccess) e = launch_step_pool(kPoolCharged, p->P, w, seed, p->d_tally, p->s1);
+                if (e == cudaSuccess) e = launch_step_pool(kPoolGamma, p->P, w, seed, p->d_tally, p->s0);
                 if (e == cudaSuccess) e = cudaEventRecord(p->evJ1, p->s1);
-                if (e == cudaSuccess) e = cudaEventRecord(p->evJ2, p->s2);
                 if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s0, p->evJ1, 0);
-                if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s0, p->evJ2, 0);
             }
             return e;
         };
@@ -514,7 +522,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
             p->graph_exec = nullptr;
             cudaGraph_t graph = nullptr;
             bool looped = false;
-            if (p->loop_node) {
+            if (want_loop) {
                 // the whole loop as ONE graph: a WHILE node whose body is kIterPerGraph iterations followed by
                 // a one-thread kernel that sets the node's condition from the done flag -- nothing returns to
                 // the host until the transport is over
@@ -547,7 +555,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
                     if (graph) cudaGraphDestroy(graph);
                     graph = nullptr;
                     p->graph_exec = nullptr;
-                    p->loop_node = 0;
+                    p->sched.loop_node = 0;
                     ce = cudaSuccess;
                 }
             }
@@ -574,14 +582,14 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
             if (ce == cudaSuccess) ce = cudaStreamSynchronize(p->s0);
             if (ce == cudaSuccess) {
                 const long bodies = (long)((p->h_ctl->iter + kIterPerGraph) / kIterPerGraph);  // the last one finds done
-                p->launches += bodies * (kIterPerGraph * kLaunchesPerIteration + 1);
+                p->launches += bodies * (kIterPerGraph * per_iter + 1);
                 p->iterations_launched += bodies * kIterPerGraph;
             }
         } else {
             int batch = 1;
             for (;;) {
                 for (int k = 0; k < batch && ce == cudaSuccess; ++k) ce = cudaGraphLaunch(exec, p->s0);
-                p->launches += (long)batch * kIterPerGraph * kLaunchesPerIteration;
+                p->launches += (long)batch * kIterPerGraph * per_iter;
                 p->iterations_launched += (long)batch * kIterPerGraph;
                 if (ce == cudaSuccess) ce = cudaMemcpyAsync(p->h_ctl, w.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, p->s0);
                 if (ce == cudaSuccess) ce = cudaStreamSynchronize(p->s0);
@@ -597,50 +605,50 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
         CU(cudaEventRecord(p->evOut, p->s0));
         CU(cudaStreamWaitEvent(st, p->evOut, 0));
     } else {
-    int batch = 8;
-    for (;;) {
-        size_t ne = 0;
-        if (p->profile) {
-            while (p->prof_ev.size() < (size_t)batch * 8) {
-                cudaEvent_t e;
-                CU(cudaEventCreate(&e));
-                p->prof_ev.push_back(e);
-            }
-        }
-        for (int k = 0; k < batch; ++k) {
-            if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
-            CU(launch_refill(w, pr, st));
+        // ---- plain stream launches, kernel by kernel on the caller's stream (what a profiler can list); with
+        // profiling on every kernel is bracketed by CUDA events
+        static const int kNoField[] = {kStageACharged, kStageBCharged, kStageAGamma, kStageBGamma};
+        static const int kField[] = {kStageA0, kStageField, kStageA2, kStageBCharged, kStageAGamma, kStageBGamma};
+        const int *order = field ? kField : kNoField;
+        const int n_stage = field ? 6 : 4;
+        const int ev_per_iter = n_stage + 2;
+        int batch = 8;
+        for (;;) {
+            size_t ne = 0;
             if (p->profile) {
-                for (int pt = 2; pt >= 0; --pt)
-                    for (int ph = 0; ph < 2; ++ph) {
-                        CU(cudaEventRecord(p->prof_ev[ne++], st));
-                        CU(launch_phase(pt, ph, p->P, w, seed, p->d_tally, p->n_sm, st));
-                    }
-                CU(cudaEventRecord(p->prof_ev[ne++], st));
-            } else {
-                CU(launch_step(p->P, w, seed, p->d_tally, p->n_sm, st));
+                while (p->prof_ev.size() < (size_t)batch * ev_per_iter) {
+                    cudaEvent_t e;
+                    CU(cudaEventCreate(&e));
+                    p->prof_ev.push_back(e);
+                }
             }
-        }
-        p->launches += (long)batch * kLaunchesPerIteration;
-        p->iterations_launched += batch;
-        CU(cudaMemcpyAsync(p->h_ctl, w.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
-        if (p->profile)
             for (int k = 0; k < batch; ++k) {
-                float ms;
-                const cudaEvent_t *e = &p->prof_ev[(size_t)k * 8];
-                CU(cudaEventElapsedTime(&ms, e[0], e[1])); p->prof_ms[6] += ms; p->iter_ms.push_back(ms);
-                int q = 1;
-                for (int pt = 2; pt >= 0; --pt)
-                    for (int ph = 0; ph < 2; ++ph, ++q) {
-                        CU(cudaEventElapsedTime(&ms, e[q], e[q + 1]));
-                        p->prof_ms[3 * ph + pt] += ms;
-                    }
-                CU(cudaEventElapsedTime(&ms, e[1], e[7])); p->prof_ms[7] += ms; p->iter_ms.push_back(ms);
+                if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
+                CU(launch_refill(w, pr, st));
+                for (int q = 0; q < n_stage; ++q) {
+                    if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
+                    CU(launch_stage(order[q], p->P, w, seed, p->d_tally, st));
+                }
+                if (p->profile) CU(cudaEventRecord(p->prof_ev[ne++], st));
             }
-        if (p->h_ctl->done || p->h_ctl->error) break;
-        if (batch < 64) batch *= 2;
-    }
+            p->launches += (long)batch * per_iter;
+            p->iterations_launched += batch;
+            CU(cudaMemcpyAsync(p->h_ctl, w.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            if (p->profile)
+                for (int k = 0; k < batch; ++k) {
+                    float ms;
+                    const cudaEvent_t *e = &p->prof_ev[(size_t)k * ev_per_iter];
+                    CU(cudaEventElapsedTime(&ms, e[0], e[1])); p->prof_ms[kNStages] += ms; p->iter_ms.push_back(ms);
+                    for (int q = 0; q < n_stage; ++q) {
+                        CU(cudaEventElapsedTime(&ms, e[1 + q], e[2 + q]));
+                        p->prof_ms[order[q]] += ms;
+                    }
+                    CU(cudaEventElapsedTime(&ms, e[1], e[1 + n_stage])); p->prof_ms[kNStages + 1] += ms; p->iter_ms.push_back(ms);
+                }
+            if (p->h_ctl->done || p->h_ctl->error) break;
+            if (batch < 64) batch *= 2;
+        }
     }
     CU(cudaEventRecord(p->ev1, st));
     CU(cudaEventSynchronize(p->ev1));
@@ -652,6 +660,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     const size_t nlog = (size_t)(p->last_ctl.iter < (unsigned long long)kMaxLog ? p->last_ctl.iter : kMaxLog);
     p->iter_log.resize(2 * nlog);
     if (nlog) CU(cudaMemcpy(p->iter_log.data(), w.log, 2 * nlog * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    if (p->last_ctl.error == EMX_E_ARG) return fail(p, EMX_E_ARG, "emx_transport: a primary's particle code is outside 0..2");
     if (p->last_ctl.error) return fail(p, p->last_ctl.error, "emx_transport: secondary stacks full, no track can be stepped");
     return EMX_OK;
 }
@@ -672,13 +681,16 @@ int emx_transport_host(emx_problem *p, long n, const int *ptype, const double *E
     if (!p || !p->hp.built) return fail(p, EMX_E_STATE, "emx_transport_host: tables not built");
     if (n < 0 || (n > 0 && (!ptype || !E || !pos3 || !dir3 || !start_vol)) || !workspace)
         return fail(p, EMX_E_ARG, "emx_transport_host: invalid argument");
+    if (!sizes_ok(n_slots, queue_capacity))
+        return fail(p, EMX_E_ARG, "emx_transport_host: n_slots must be in [1, 2^22] and queue_capacity in [1, 2^30]");
     cudaStream_t st = (cudaStream_t)stream;
-    // staging area for the primaries: 4 + 8 + 24 + 24 + 4 + 4 bytes each
+    // the primaries are staged in the caller's workspace, behind the part emx_workspace_bytes() describes
+    Work w0;
+    const size_t body = carve_work(nullptr, n_slots, queue_capacity, w0, kMaxLog);
+    if (body + staging_bytes(n) > workspace_bytes)
+        return fail(p, EMX_E_CAPACITY, "emx_transport_host: workspace smaller than emx_workspace_bytes() + emx_staging_bytes()");
     const size_t nn = (size_t)(n ? n : 1);
-    char *d = nullptr;
-    const size_t bytes = align_up(nn * 4, 256) * 3 + align_up(nn * 8, 256) + 2 * align_up(nn * 24, 256);
-    CU(cudaMalloc(&d, bytes));
-    Carve c{d};
+    Carve c{(char *)workspace + body};
     int *d_pt = c.take<int>(nn), *d_vol = c.take<int>(nn), *d_surf = c.take<int>(nn);
     double *d_E = c.take<double>(nn), *d_pos = c.take<double>(3 * nn), *d_dir = c.take<double>(3 * nn);
     cudaError_t e = cudaSuccess;
@@ -691,14 +703,9 @@ int emx_transport_host(emx_problem *p, long n, const int *ptype, const double *E
     up(d_E, E, (size_t)n * 8);
     up(d_pos, pos3, (size_t)n * 24);
     up(d_dir, dir3, (size_t)n * 24);
-    int rc;
-    if (e != cudaSuccess) rc = fail_cuda(p, e, "emx_transport_host: upload");
-    else {
-        Primaries pr{n, d_pt, d_E, d_pos, d_dir, d_vol, start_surf ? d_surf : nullptr, p->prim_first};
-        rc = transport_device(p, pr, seed, n_slots, queue_capacity, workspace, workspace_bytes, st);
-    }
-    cudaFree(d);
-    return rc;
+    if (e != cudaSuccess) return fail_cuda(p, e, "emx_transport_host: upload");
+    Primaries pr{n, d_pt, d_E, d_pos, d_dir, d_vol, start_surf ? d_surf : nullptr, p->prim_first};
+    return transport_device(p, pr, seed, n_slots, queue_capacity, workspace, body, st);
 }
 
 int emx_set_primary_offset(emx_problem *p, long first) {
@@ -722,17 +729,20 @@ int emx_neighbour_candidates(const emx_problem *cp, int surface, int sense, int 
     return n;
 }
 
-int emx_set_pool_split(emx_problem *p, double fg, double fe, double fp) {
-    if (!p) return fail(p, EMX_E_ARG, "emx_set_pool_split: null problem");
-    if (fg == 0.0 && fe == 0.0 && fp == 0.0) {
-        p->pool_frac[0] = p->pool_frac[1] = p->pool_frac[2] = 0.0;
-        return EMX_OK;
-    }
-    if (!(fg > 0.0) || !(fe > 0.0) || !(fp > 0.0)) return fail(p, EMX_E_ARG, "emx_set_pool_split: every share must be > 0");
-    const double s = fg + fe + fp;
-    p->pool_frac[0] = fg / s;
-    p->pool_frac[1] = fe / s;
-    p->pool_frac[2] = fp / s;
+int emx_get_schedule(const emx_problem *p, emx_schedule *out) {
+    if (!p || !out) return EMX_E_ARG;
+    *out = p->sched;
+    return EMX_OK;
+}
+
+int emx_set_schedule(emx_problem *p, const emx_schedule *in) {
+    if (!p || !in) return fail(p, EMX_E_ARG, "emx_set_schedule: null argument");
+    if (in->slice_min < 1 || in->slice_max < in->slice_min)
+        return fail(p, EMX_E_ARG, "emx_set_schedule: need 1 <= slice_min <= slice_max");
+    for (int k = 0; k < 8; ++k)
+        if (in->blocks_per_sm[k] < 0 || in->blocks_per_sm[k] > 16)
+            return fail(p, EMX_E_ARG, "emx_set_schedule: blocks_per_sm outside 0..16");
+    p->sched = *in;
     return EMX_OK;
 }
 
@@ -765,9 +775,9 @@ int emx_set_profile(emx_problem *p, int on) {
     return EMX_OK;
 }
 
-int emx_get_profile(const emx_problem *p, double *ms4, long *launches, long *iterations_launched) {  // ms4: 8 doubles
+int emx_get_profile(const emx_problem *p, double *ms9, long *launches, long *iterations_launched) {
     if (!p) return EMX_E_ARG;
-    if (ms4) for (int k = 0; k < 8; ++k) ms4[k] = p->prof_ms[k];
+    if (ms9) for (int k = 0; k < kNStages + 2; ++k) ms9[k] = p->prof_ms[k];
     if (launches) *launches = p->launches;
     if (iterations_launched) *iterations_launched = p->iterations_launched;
     return EMX_OK;
@@ -781,10 +791,18 @@ long emx_get_iteration_log(const emx_problem *p, uint32_t *host_out, long max_it
     return n;
 }
 
-int emx_get_lanes(const emx_problem *p, uint64_t *lanes6) {
-    if (!p || !lanes6 || !p->have_ctl) return EMX_E_ARG;
-    for (int ph = 0; ph < 2; ++ph)
-        for (int pt = 0; pt < 3; ++pt) lanes6[3 * ph + pt] = p->last_ctl.lanes[ph][pt];
+int emx_get_lanes(const emx_problem *p, uint64_t *lanes8) {
+    if (!p || !lanes8 || !p->have_ctl) return EMX_E_ARG;
+    const Ctl &c = p->last_ctl;
+    const bool field = p->P.Bmag != 0.0;
+    lanes8[kStageAGamma] = c.lanes[2][kPoolGamma];
+    lanes8[kStageACharged] = field ? 0ull : c.lanes[2][kPoolCharged];
+    lanes8[kStageA0] = c.lanes[0][kPoolCharged];
+    lanes8[kStageField] = c.lanes[1][kPoolCharged];
+    lanes8[kStageA2] = field ? c.lanes[2][kPoolCharged] : 0ull;
+    lanes8[kStageBGamma] = c.lanes[3][kPoolGamma];
+    lanes8[kStageBCharged] = c.lanes[3][kPoolCharged];
+    lanes8[7] = c.attempts;
     return EMX_OK;
 }
 
@@ -837,16 +855,11 @@ int emx_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *ali
     int *scratch = nullptr;
     const size_t ints = refill_plan_scratch_ints(capacity);
     CU(cudaMalloc(&scratch, ints * sizeof(int)));
-    cudaError_t e = launch_refill_plan(n_live, capacity, n_queue, alive, src, scratch, st);
+    const Ctl *d_ctl = nullptr;
+    cudaError_t e = launch_refill_plan(n_live, capacity, n_queue, alive, src, scratch, &d_ctl, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     Ctl hc;
-    if (e == cudaSuccess) {
-        // the control block sits behind the three int arrays (see launch_refill_plan)
-        const size_t nch = (size_t)(capacity + kChunk - 1) / kChunk + 1;
-        int *q = scratch + 2 * nch + capacity;
-        q += (16 - ((uintptr_t)q / 4) % 16) % 16;
-        e = cudaMemcpy(&hc, q, sizeof(Ctl), cudaMemcpyDeviceToHost);
-    }
+    if (e == cudaSuccess) e = cudaMemcpy(&hc, d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost);
     cudaFree(scratch);
     if (e != cudaSuccess) return fail_cuda(p, e, "emx_refill_plan");
     counts_host[0] = hc.plan[0].n_final;

@@ -42,27 +42,15 @@ EMX_HD void step_one(const Params &P, uint64_t seed, const emx_track &in, emx_st
     t.surf = in.surf;
     t.alive = 1;
     StepOut o;
-    FieldState fs;
-    fs.s_done = fs.h = 0.0;
-    fs.attempt = 0;
-    const int whole = P.ph.max_substeps;  // the hook runs the whole step in one call
-    if (in.ptype == kGamma) step<kGamma>(P, seed, t, o, fs, whole);
+    int n_sub = 0;
+    const int pt = in.ptype;
+    if (pt == kGamma) step<false>(P, seed, pt, t, o, n_sub);
     else if (!P.ph.msc && !P.ph.fluct) {
-        if (P.field_kind == 0) {
-            if (in.ptype == kElectron) step<kElectron>(P, seed, t, o, fs, whole);
-            else step<kPositron>(P, seed, t, o, fs, whole);
-        } else {
-            if (in.ptype == kElectron) step<kElectron, true>(P, seed, t, o, fs, whole);
-            else step<kPositron, true>(P, seed, t, o, fs, whole);
-        }
+        if (P.field_kind == 0) step<true, false, false>(P, seed, pt, t, o, n_sub);
+        else step<true, true, false>(P, seed, pt, t, o, n_sub);
     } else {
-        if (P.field_kind == 0) {
-            if (in.ptype == kElectron) step<kElectron, false, true>(P, seed, t, o, fs, whole);
-            else step<kPositron, false, true>(P, seed, t, o, fs, whole);
-        } else {
-            if (in.ptype == kElectron) step<kElectron, true, true>(P, seed, t, o, fs, whole);
-            else step<kPositron, true, true>(P, seed, t, o, fs, whole);
-        }
+        if (P.field_kind == 0) step<true, false, true>(P, seed, pt, t, o, n_sub);
+        else step<true, true, true>(P, seed, pt, t, o, n_sub);
     }
 
     put3(r.trk.x, t.x);
@@ -106,6 +94,7 @@ EMX_HD void step_one(const Params &P, uint64_t seed, const emx_track &in, emx_st
     r.n_draws = o.n_draws;
     r.null_int = o.null_int;
     r.rest = o.rest;
+    r.n_sub = n_sub;
 }
 
 }  // namespace emx

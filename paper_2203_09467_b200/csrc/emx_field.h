@@ -4,32 +4,53 @@
 // integration algorithms"; BASELINE.json configs[3]: "adaptive RK4 (1e-6 mm miss-distance tolerance)".
 // Algorithm (C9): classical RK4 with step doubling for the local error, plus a chord /
 // secant search for the boundary landing point.  y = (x, u), dy/ds = (u, kappa u x Bhat).
+//
+// The substep loop of C9 is written as ONE ATTEMPT per call (field_attempt): the propagation kernel keeps every
+// lane of a warp busy with one attempt of SOME track and hands a lane a new track as soon as its own is done,
+// so tracks that need 1 and tracks that need 1000 attempts share a warp without idling it.
 #pragma once
 #include "emx_core.h"
 #include "emx_geom.h"
 
 namespace emx {
 
+// AX: direction of a uniform field.  0 / 1 / 2: along +-x / +-y / +-z, the sign folded into kappa by the caller
+// (Bhat = b e_a, b = +-1: kappa (u x Bhat) = (kappa b)(u x e_a) exactly, every product with the zero components
+// of Bhat being an exact zero) -- the same numbers as the general formula with a third of the arithmetic;
+// 3: any direction.
+constexpr int kAxisAny = 3;
+
+template <int AX>
 EMX_HD Vec3 lorentz(const Vec3 &u, double kappa, const double B[3]) {
+    if (AX == 0) return {0.0, kappa * u.z, -(kappa * u.y)};
+    if (AX == 1) return {-(kappa * u.z), 0.0, kappa * u.x};
+    if (AX == 2) return {kappa * u.y, -(kappa * u.x), 0.0};
     return {kappa * (u.y * B[2] - u.z * B[1]), kappa * (u.z * B[0] - u.x * B[2]), kappa * (u.x * B[1] - u.y * B[0])};
 }
 
+// u + f k, leaving the component along an axis-aligned field alone (its k is an exact zero)
+template <int AX>
+EMX_HD Vec3 stage_u(const Vec3 &u, double f, const Vec3 &k) {
+    return {AX == 0 ? u.x : u.x + f * k.x, AX == 1 ? u.y : u.y + f * k.y, AX == 2 ? u.z : u.z + f * k.z};
+}
+
 // one classical RK4 step of length h.  dx/ds = u, so the x-stages are the u-stage arguments.
+template <int AX>
 EMX_HD void rk4_step(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, Vec3 &xo, Vec3 &uo) {
-    const Vec3 k1u = lorentz(u, kappa, B);
-    const Vec3 u2 = u + (0.5 * h) * k1u;
-    const Vec3 k2u = lorentz(u2, kappa, B);
-    const Vec3 u3 = u + (0.5 * h) * k2u;
-    const Vec3 k3u = lorentz(u3, kappa, B);
-    const Vec3 u4 = u + h * k3u;
-    const Vec3 k4u = lorentz(u4, kappa, B);
+    const Vec3 k1u = lorentz<AX>(u, kappa, B);
+    const Vec3 u2 = stage_u<AX>(u, 0.5 * h, k1u);
+    const Vec3 k2u = lorentz<AX>(u2, kappa, B);
+    const Vec3 u3 = stage_u<AX>(u, 0.5 * h, k2u);
+    const Vec3 k3u = lorentz<AX>(u3, kappa, B);
+    const Vec3 u4 = stage_u<AX>(u, h, k3u);
+    const Vec3 k4u = lorentz<AX>(u4, kappa, B);
     const double h6 = h / 6.0;
     xo.x = x.x + h6 * (u.x + 2.0 * u2.x + 2.0 * u3.x + u4.x);
     xo.y = x.y + h6 * (u.y + 2.0 * u2.y + 2.0 * u3.y + u4.y);
     xo.z = x.z + h6 * (u.z + 2.0 * u2.z + 2.0 * u3.z + u4.z);
-    uo.x = u.x + h6 * (k1u.x + 2.0 * k2u.x + 2.0 * k3u.x + k4u.x);
-    uo.y = u.y + h6 * (k1u.y + 2.0 * k2u.y + 2.0 * k3u.y + k4u.y);
-    uo.z = u.z + h6 * (k1u.z + 2.0 * k2u.z + 2.0 * k3u.z + k4u.z);
+    uo.x = AX == 0 ? u.x : u.x + h6 * (k1u.x + 2.0 * k2u.x + 2.0 * k3u.x + k4u.x);
+    uo.y = AX == 1 ? u.y : u.y + h6 * (k1u.y + 2.0 * k2u.y + 2.0 * k3u.y + k4u.y);
+    uo.z = AX == 2 ? u.z : u.z + h6 * (k1u.z + 2.0 * k2u.z + 2.0 * k3u.z + k4u.z);
 }
 
 // ---- non-uniform field (include/emx.h: emx_set_field_fringe): B(x) = Bmag g(x), a solenoid along z whose
@@ -48,19 +69,19 @@ EMX_HD void field_profile(const Params &P, const Vec3 &x, double g[3]) {
 EMX_HD void rk4_step_map(const Params &P, const Vec3 &x, const Vec3 &u, double kappa, double h, Vec3 &xo, Vec3 &uo) {
     double g[3];
     field_profile(P, x, g);
-    const Vec3 k1u = lorentz(u, kappa, g);
+    const Vec3 k1u = lorentz<kAxisAny>(u, kappa, g);
     const Vec3 x2 = x + (0.5 * h) * u;
     const Vec3 u2 = u + (0.5 * h) * k1u;
     field_profile(P, x2, g);
-    const Vec3 k2u = lorentz(u2, kappa, g);
+    const Vec3 k2u = lorentz<kAxisAny>(u2, kappa, g);
     const Vec3 x3 = x + (0.5 * h) * u2;
     const Vec3 u3 = u + (0.5 * h) * k2u;
     field_profile(P, x3, g);
-    const Vec3 k3u = lorentz(u3, kappa, g);
+    const Vec3 k3u = lorentz<kAxisAny>(u3, kappa, g);
     const Vec3 x4 = x + h * u3;
     const Vec3 u4 = u + h * k3u;
     field_profile(P, x4, g);
-    const Vec3 k4u = lorentz(u4, kappa, g);
+    const Vec3 k4u = lorentz<kAxisAny>(u4, kappa, g);
     const double h6 = h / 6.0;
     xo.x = x.x + h6 * (u.x + 2.0 * u2.x + 2.0 * u3.x + u4.x);
     xo.y = x.y + h6 * (u.y + 2.0 * u2.y + 2.0 * u3.y + u4.y);
@@ -71,8 +92,8 @@ EMX_HD void rk4_step_map(const Params &P, const Vec3 &x, const Vec3 &u, double k
 }
 
 // one step of h against two of h/2: err = |x_full - x_half|, result = half-step state, u renormalised.
-// MAP: the field is evaluated at the stage positions (non-uniform field); else it is P.Bhat everywhere
-template <bool MAP>
+// MAP: the field is evaluated at the stage positions (non-uniform field); else it is uniform along AX
+template <bool MAP, int AX>
 EMX_NI void rk4_doubling(const Params &P, const Vec3 &x, const Vec3 &u, double kappa, double h, Vec3 &x1, Vec3 &u1,
                          double &err) {
     Vec3 xf, uf, xm, um;
@@ -81,9 +102,9 @@ EMX_NI void rk4_doubling(const Params &P, const Vec3 &x, const Vec3 &u, double k
         rk4_step_map(P, x, u, kappa, 0.5 * h, xm, um);
         rk4_step_map(P, xm, um, kappa, 0.5 * h, x1, u1);
     } else {
-        rk4_step(x, u, kappa, P.Bhat, h, xf, uf);
-        rk4_step(x, u, kappa, P.Bhat, 0.5 * h, xm, um);
-        rk4_step(xm, um, kappa, P.Bhat, 0.5 * h, x1, u1);
+        rk4_step<AX>(x, u, kappa, P.Bhat, h, xf, uf);
+        rk4_step<AX>(x, u, kappa, P.Bhat, 0.5 * h, xm, um);
+        rk4_step<AX>(xm, um, kappa, P.Bhat, 0.5 * h, x1, u1);
     }
     err = norm(xf - x1);
     const double n = norm(u1);
@@ -92,100 +113,118 @@ EMX_NI void rk4_doubling(const Params &P, const Vec3 &x, const Vec3 &u, double k
     u1.z /= n;
 }
 
-// Progress of a propagation that is spread over several iterations of the loop: the
-// arc length done, the current trial step and the substep attempts used.  attempt == 0: none in progress.
+// Loop variables of a propagation: the arc length done, the current trial step and the substep attempts used.
+// They live in registers while a lane works on the track and in the slot while the track is parked between two
+// iterations of the loop; either way the SAME sequence of substeps is taken: when the attempts are made never
+// changes a result.
 struct FieldState {
     double s_done, h;
     int attempt;
 };
 
-// Propagate up to s_max inside cell `vol`.  Returns the arc length travelled so far; hit = surface reached
-// (-1 none).  x, u are updated; on_surf is the surface the track sits on (updated when suspended).
-// The substep loop of C9 runs for at most `budget` attempts per call; if it is not finished by then,
-// `suspended` is set and fs holds the loop variables, so that the next call continues the SAME sequence of
-// substeps: slicing changes when the work is done, never its result.  budget >= max_substeps: one call.
-template <bool MAP>
-EMX_NI double propagate_field(const Params &P, int vol, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
-                              int &hit, FieldState &fs, int budget, bool &suspended) {
+EMX_HD void field_begin(double kappa, double s_max, FieldState &fs) {
+    fs.s_done = 0.0;
+    fs.h = 0.25 / fabs(kappa);
+    if (s_max < fs.h) fs.h = s_max;
+    fs.attempt = 0;
+}
+
+// ONE attempt of the substep loop of C9 inside cell `vol`, towards the arc length s_max.  x, u, on_surf (the surface
+// the track sits on) and fs are updated.  Returns true when the propagation is over: s = arc length travelled,
+// hit = surface reached (-1 none: s_max travelled, or the max_substeps attempts of the step are used up).
+template <bool MAP, int AX>
+EMX_NI bool field_attempt(const Params &P, int vol, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
+                          FieldState &fs, int &hit, double &s) {
     const double eps = P.ph.field_eps;
-    double s_done;
-    int surf = on_surf;
-    double h;
-    int attempt;
-    if (fs.attempt > 0) {  // resume
-        s_done = fs.s_done;
-        h = fs.h;
-        attempt = fs.attempt;
-    } else {
-        s_done = 0.0;
-        h = 0.25 / fabs(kappa);
-        if (s_max < h) h = s_max;
-        attempt = 0;
-    }
+    const double rem = s_max - fs.s_done;
+    double h = fs.h;
+    if (h > rem) h = rem;
+    Vec3 x1, u1;
+    double err;
+    rk4_doubling<MAP, AX>(P, x, u, kappa, h, x1, u1, err);
     hit = -1;
-    suspended = false;
-    const int max_attempts = P.ph.max_substeps;
-    const int stop_at = (budget < max_attempts - attempt) ? attempt + budget : max_attempts;
-    for (; attempt < max_attempts; ++attempt) {
-        if (attempt >= stop_at) {  // out of budget for this iteration: park the loop variables
-            fs.s_done = s_done;
-            fs.h = h;
-            fs.attempt = attempt;
-            on_surf = surf;
-            suspended = true;
-            return s_done;
-        }
-        const double rem = s_max - s_done;
-        if (h > rem) h = rem;
-        Vec3 x1, u1;
-        double err;
-        rk4_doubling<MAP>(P, x, u, kappa, h, x1, u1, err);
-        if (err > eps && h > 1e-9) {  // too inaccurate: shrink and retry
-            const double f = 0.9 * m_pow(eps / err, 0.2);
-            h *= (f > 0.2 ? f : 0.2);
-            continue;
-        }
+    if (err > eps && h > 1e-9) {  // too inaccurate: shrink and retry
+        const double f = 0.9 * m_pow(eps / err, 0.2);
+        h *= (f > 0.2 ? f : 0.2);
+    } else {
         const Vec3 c = x1 - x;
         const double L = norm(c);
         if (!(L > 0.0)) {
-            s_done += h;
-            break;
+            fs.s_done += h;
+            s = fs.s_done;
+            return true;
         }
         const Vec3 cd = {c.x / L, c.y / L, c.z / L};
         int S;
-        const double d = distance_to_boundary(P, vol, x, cd, surf, S);
+        const double d = distance_to_boundary(P, vol, x, cd, on_surf, S);
         if (d <= eps) {
             // chord bends back across the surface the track sits on: shorten and retry
-            if (d == 0.0 && S == surf && h > 1e-9) {
+            if (d == 0.0 && S == on_surf && h > 1e-9) {
                 h *= 0.5;
-                continue;
+            } else {
+                hit = S;  // immediate (re-)crossing, nothing more travelled
+                s = fs.s_done;
+                return true;
             }
-            hit = S;  // immediate (re-)crossing, nothing more travelled
-            fs.attempt = 0;
-            return s_done;
-        }
-        if (d > L + eps) {  // chord ends inside the cell, clear of S: accept
+        } else if (d > L + eps) {  // chord ends inside the cell, clear of S: accept
             x = x1;
             u = u1;
-            s_done += h;
-            surf = -1;
-            if (s_done >= s_max * (1.0 - 1e-14)) break;
+            fs.s_done += h;
+            on_surf = -1;
+            if (fs.s_done >= s_max * (1.0 - 1e-14)) {
+                s = fs.s_done;
+                return true;
+            }
             const double e = err > eps / 3125.0 ? err : eps / 3125.0;
             const double f = 0.9 * m_pow(eps / e, 0.2);
             h *= (f < 5.0 ? f : 5.0);
-            continue;
-        }
-        if (L - d <= eps) {  // |L - d| <= eps: landed on S, just past it or just short of it
+        } else if (L - d <= eps) {  // |L - d| <= eps: landed on S, just past it or just short of it
             x = x1;
             u = u1;
             hit = S;
-            fs.attempt = 0;
-            return s_done + h;
+            s = fs.s_done + h;
+            return true;
+        } else {
+            h *= d / L;  // secant: aim the chord end at S
         }
-        h *= d / L;  // secant: aim the chord end at S
     }
-    fs.attempt = 0;
-    return s_done;
+    fs.h = h;
+    fs.attempt += 1;
+    if (fs.attempt >= P.ph.max_substeps) {  // the step's attempts are used up: whatever was travelled
+        s = fs.s_done;
+        return true;
+    }
+    return false;
+}
+
+// the axis of a uniform field (host and device): 0 / 1 / 2 with sign b = Bhat[axis], or kAxisAny
+EMX_HD int field_axis(const double Bhat[3]) {
+    for (int a = 0; a < 3; ++a) {
+        const int i = (a + 1) % 3, j = (a + 2) % 3;
+        if (Bhat[i] == 0.0 && Bhat[j] == 0.0 && (Bhat[a] == 1.0 || Bhat[a] == -1.0)) return a;
+    }
+    return kAxisAny;
+}
+
+// The whole propagation in one call (level-2 hook; the loop's kernel calls field_attempt itself).
+template <bool MAP>
+EMX_NI double propagate_field(const Params &P, int vol, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
+                              int &hit, int &n_attempts) {
+    FieldState fs;
+    field_begin(kappa, s_max, fs);
+    double s = 0.0;
+    const int ax = MAP ? kAxisAny : field_axis(P.Bhat);
+    const double kb = ax == kAxisAny ? kappa : kappa * P.Bhat[ax];
+    bool done = false;
+    n_attempts = 0;
+    while (!done) {
+        if (MAP || ax == kAxisAny) done = field_attempt<MAP, kAxisAny>(P, vol, on_surf, x, u, kappa, s_max, fs, hit, s);
+        else if (ax == 0) done = field_attempt<false, 0>(P, vol, on_surf, x, u, kb, s_max, fs, hit, s);
+        else if (ax == 1) done = field_attempt<false, 1>(P, vol, on_surf, x, u, kb, s_max, fs, hit, s);
+        else done = field_attempt<false, 2>(P, vol, on_surf, x, u, kb, s_max, fs, hit, s);
+        ++n_attempts;
+    }
+    return s;
 }
 
 }  // namespace emx

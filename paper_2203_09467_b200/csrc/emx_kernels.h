@@ -24,22 +24,33 @@ struct Primaries {
     long long first;        // primary index of element 0 (emx_set_primary_offset): element i is primary first + i
 };
 
+// the step kernels by stage (index of Work::grid, of emx_get_profile's milliseconds and of emx_get_lanes)
+enum : int {
+    kStageAGamma = 0,    // k_a<gamma>: limits + straight move + finish
+    kStageACharged = 1,  // k_a<charged>: the same for e+- when there is no field
+    kStageA0 = 2,        // k_a0: limits of e+- (field)
+    kStageField = 3,     // k_field: adaptive RK4 propagation of e+-
+    kStageA2 = 4,        // k_a2: finish of e+- (field)
+    kStageBGamma = 5,    // k_b<gamma>: Compton, photoelectric, pair production
+    kStageBCharged = 6,  // k_b<charged>: Moller, Bhabha, bremsstrahlung, annihilation
+    kNStages = 7
+};
+
 // resets the control block, totals the injected energy
 cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st);
-// one iteration of the loop = launch_refill (k_plan, k_fill, k_move) then
-// launch_step (one persistent kernel per pool); tally = device edep array
+// one iteration of the loop = launch_refill (k_plan, k_fill, k_move) then the two pools' chains
+// (launch_step_pool, or stage by stage with launch_stage); tally = device edep array
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st);
 // sets the condition of a graph WHILE node (handle from cudaGraphConditionalHandleCreate): go on unless done
 cudaError_t launch_loop_condition(const Work &w, unsigned long long handle, cudaStream_t st);
-cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st);
-cudaError_t launch_phase(int pt, int phase, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
-                         cudaStream_t st);
-cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
-                             cudaStream_t st);
-constexpr int kLaunchesPerIteration = 9;  // 3 refill kernels + 3 x (phase A + phase B)
+cudaError_t launch_stage(int stage, const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st);
+cudaError_t launch_step_pool(int pool, const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st);
+cudaError_t step_kernel_regs(int stage, bool field, int *regs);
+// kernels launched per iteration: 3 refill kernels + the stages of the two chains
+inline int launches_per_iteration(bool field) { return 3 + 2 + (field ? 4 : 2); }
 // level-1 hook: the refill index logic alone on a caller-supplied alive[] (see include/emx.h)
 cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
-                               int *scratch, cudaStream_t st);
+                               int *scratch, const Ctl **ctl_out, cudaStream_t st);
 size_t refill_plan_scratch_ints(long capacity);
 
 }  // namespace emx

@@ -1,107 +1,82 @@
-// emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the per-type step
-// kernels (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
+// emx_transport.cu -- the loop kernels: primary loading, refill / compaction (A0, A9), the step kernels
+// (A1-A8, A10) and loop control (A12).  DESIGN.md section 5.
 //
-// One ITERATION = k_plan (admission + refill plan) -> k_fill -> k_move -> per pool (e+, e-, gamma):
-// k_step_pool<PT> (phase A) -> k_interact<PT> (phase B).  Eight iterations and k_loop_condition form the body
-// of a graph WHILE node: nothing returns to the host during a transport; pool sizes, stack tops and the done
-// flag live in the device control block.
+// One ITERATION = k_plan (admission, refill plan, chunk trading) -> k_fill -> k_move -> per pool
+//   photons:          k_a<gamma>  (limits + straight move + finish)                        -> k_b<gamma>
+//   e+-, no field:    k_a<charged>                                                        -> k_b<charged>
+//   e+-, in a field:  k_a0 (limits) -> k_field (adaptive RK4, lanes refilled) -> k_a2 (finish) -> k_b<charged>
+// The two pools' chains are parallel branches of the iteration graph.  Eight iterations and k_loop_condition form
+// the body of a graph WHILE node: nothing returns to the host during a transport; pool sizes, stack tops and
+// the done flag live in the device control block.
 #include <cuda_runtime.h>
 #include "emx_kernels.h"
 #include "emx_step.h"
+#include "emx_diag.h"
 
 namespace emx {
 
 // stack records are written once and read once: streaming stores / loads (evict-first) keep them from
 // displacing the track store in L2
-#ifndef EMX_STREAM_HINTS
-#define EMX_STREAM_HINTS 1
-#endif
-#if EMX_STREAM_HINTS
-#define EMX_ST(p, v) __stcs((p), (v))
-#define EMX_LD(p) __ldcs((p))
-#else
-#define EMX_ST(p, v) (*(p) = (v))
-#define EMX_LD(p) (*(p))
-#endif
+__device__ __forceinline__ void st_cs(double2 *p, double2 v) { __stcs(p, v); }
+__device__ __forceinline__ void st_cs(int4 *p, int4 v) { __stcs(p, v); }
+__device__ __forceinline__ double2 ld_cs(const double2 *p) { return __ldcs(p); }
+__device__ __forceinline__ int4 ld_cs(const int4 *p) { return __ldcs(p); }
 
-__device__ __forceinline__ void load_record(const QueueSoA &q, int r, const TrackSoA &t, int i) {
-    t.x[i] = EMX_LD(&q.x[r]);
-    t.y[i] = EMX_LD(&q.y[r]);
-    t.z[i] = EMX_LD(&q.z[r]);
-    t.ux[i] = EMX_LD(&q.ux[r]);
-    t.uy[i] = EMX_LD(&q.uy[r]);
-    t.uz[i] = EMX_LD(&q.uz[r]);
-    t.E[i] = EMX_LD(&q.E[r]);
-    t.tid[i] = (uint64_t)EMX_LD((const unsigned long long *)&q.tid[r]);
-    t.prim[i] = EMX_LD(&q.prim[r]);
-    t.step[i] = 0u;
-    t.vol[i] = EMX_LD(&q.vol[r]);
-    t.surf[i] = EMX_LD(&q.surf[r]);
-    t.alive[i] = 2;  // 2 = filled in this refill pass (k_move still ranks it as a hole)
-    if (t.fs_a) t.fs_a[i] = 0;
-    if (t.pend) t.pend[i] = 0;
+__device__ __forceinline__ double2 pack_Et(double E, uint64_t tid) { return make_double2(E, __longlong_as_double((long long)tid)); }
+__device__ __forceinline__ uint64_t tid_of(double2 Et) { return (uint64_t)__double_as_longlong(Et.y); }
+
+// A0: record r of stack `pool` becomes the track in physical slot s
+template <int POOL>
+__device__ __forceinline__ void load_record(const Work &w, int r, int s) {
+    const Stack &q = w.q[POOL];
+    const Store &t = w.st;
+    t.xy[s] = ld_cs(&q.xy[r]);
+    t.zu[s] = ld_cs(&q.zu[r]);
+    t.uu[s] = ld_cs(&q.uu[r]);
+    t.Et[s] = ld_cs(&q.Et[r]);
+    const int4 id = ld_cs(&q.id[r]);  // prim, vol, surf, ptype
+    t.id[s] = make_int4(id.x, 0, id.y, id.z);
+    if (POOL == kPoolCharged) t.ptype[s] = (uint8_t)id.w;
+    t.alive[s] = 2;  // 2 = filled in this refill pass (k_move still ranks it as a hole)
+    t.stage[s] = kStFresh;
 }
 
-__device__ __forceinline__ void move_slot(const TrackSoA &t, int from, int to) {
-    t.x[to] = t.x[from];
-    t.y[to] = t.y[from];
-    t.z[to] = t.z[from];
-    t.ux[to] = t.ux[from];
-    t.uy[to] = t.uy[from];
-    t.uz[to] = t.uz[from];
-    t.E[to] = t.E[from];
-    t.tid[to] = t.tid[from];
-    t.prim[to] = t.prim[from];
-    t.step[to] = t.step[from];
-    t.vol[to] = t.vol[from];
-    t.surf[to] = t.surf[from];
+template <int POOL>
+__device__ __forceinline__ void move_slot(const Work &w, int from, int to) {
+    const Store &t = w.st;
+    t.xy[to] = t.xy[from];
+    t.zu[to] = t.zu[from];
+    t.uu[to] = t.uu[from];
+    t.Et[to] = t.Et[from];
+    t.id[to] = t.id[from];
+    t.stage[to] = t.stage[from];
     t.alive[to] = 2;
-    if (t.pend) t.pend[to] = t.pend[from];
-    if (t.fs_a) {
-        t.fs_s[to] = t.fs_s[from];
-        t.fs_h[to] = t.fs_h[from];
-        t.fs_a[to] = t.fs_a[from];
+    if (POOL == kPoolCharged) {  // a propagation may be parked in the slot
+        t.ptype[to] = t.ptype[from];
+        t.act[to] = t.act[from];
+        t.s_phys[to] = t.s_phys[from];
+        t.s_done[to] = t.s_done[from];
+        t.h_try[to] = t.h_try[from];
+        t.att[to] = t.att[from];
     }
 }
-
-// Optional timeline of the iteration graph (diagnostics, -DEMX_TIMELINE): first block start / last block end
-// of every kernel node, from %globaltimer, for iterations [EMX_TL_FIRST, EMX_TL_FIRST + kTlN).
-#ifdef EMX_TIMELINE
-#ifndef EMX_TL_FIRST
-#define EMX_TL_FIRST 2500
-#endif
-constexpr int kTlN = 64;
-__device__ unsigned long long g_tl[kTlN][9][4];  // min start, max end, sum of block times, blocks
-__device__ __forceinline__ void tl_mark(const Work &w, int node, int which, int iter_off) {
-    __shared__ unsigned long long s_t0;
-    if (threadIdx.x != 0) return;
-    const long long it = (long long)w.ctl->iter - iter_off - EMX_TL_FIRST;
-    if (it < 0 || it >= kTlN) return;
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    atomicMax(&g_tl[it][node][which], which == 0 ? ~t : t);
-    if (which == 0) s_t0 = t;
-    else {
-        atomicAdd(&g_tl[it][node][2], t - s_t0);
-        atomicAdd(&g_tl[it][node][3], 1ull);
-    }
-}
-#define EMX_TL(w, node, which, off) tl_mark(w, node, which, off)
-#else
-#define EMX_TL(w, node, which, off) ((void)0)
-#endif
 
 // ------------------------------------------------------------------------------------------------
-// Loop start: clear the control block, total the injected energy and the primaries per type.
+// Loop start: clear the control block, total the injected energy and the primaries per type, hand every
+// chunk of the store to the free list.
 __global__ void __launch_bounds__(1024) k_init(Work w, Primaries pr) {
     __shared__ int s_cnt[3][32];
     __shared__ double s_E[32];
+    __shared__ int s_bad;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     Ctl *c = w.ctl;
+    if (tid == 0) s_bad = 0;
+    __syncthreads();
     int cnt[3] = {0, 0, 0};
     double ein = 0.0;
     for (long i = tid; i < pr.n; i += blockDim.x) {
         const int pt = pr.ptype[i];
+        if (pt < 0 || pt > 2) s_bad = 1;
         cnt[0] += (pt == 0);
         cnt[1] += (pt == 1);
         cnt[2] += (pt == 2);
@@ -125,43 +100,52 @@ __global__ void __launch_bounds__(1024) k_init(Work w, Primaries pr) {
             z.tracks[p] = (unsigned long long)t;
         }
         z.E_in = e;
+        z.n_free = w.n_chunks;
+        if (s_bad) {  // a particle code outside 0..2: nothing is transported
+            z.error = EMX_E_ARG;
+            z.done = 1;
+        }
         *c = z;
     }
-    for (int p = 0; p < 3; ++p)
-        for (int k = tid; k <= w.cap[p] / kChunk; k += blockDim.x) w.chunk_dead[p][k] = 0;
+    for (int k = tid; k < w.n_chunks; k += blockDim.x) w.free_list[k] = w.n_chunks - 1 - k;  // chunk 0 on top
+    for (int p = 0; p < kPools; ++p)
+        for (int k = tid; k <= w.n_chunks; k += blockDim.x) w.chunk_dead[p][k] = 0;
 }
 
 // A0, first half: admission of primaries (R8).  Done by the one block of k_plan at the start of every iteration.  While the
 // shower energy in flight and the stacks are below their soft limits, the next `wave` primaries are pushed
-// onto the stacks of their types, lowest index on top, so they enter the pools in ascending order at the
+// onto the stacks of their pools, lowest index on top, so they enter the pools in ascending order at the
 // refill that follows.  Histories do not depend on when a primary is admitted (keyed RNG, C2); admission only
 // bounds the number of queued records (the queue had to hold 2.5e7 initializers).
-__device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) {
-    __shared__ int s_cnt[3][32];
-    __shared__ int s_total[3], s_base[3];
+// Returns (to every thread) the number of primaries admitted.
+__device__ __forceinline__ int admit_block(const Work &w, const Primaries &pr) {
+    __shared__ int s_cnt[kPools][32];
+    __shared__ int s_total[kPools], s_base[kPools];
     __shared__ double s_E[32];
-    __shared__ int s_go;
+    __shared__ long long s_A;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
     Ctl *c = w.ctl;
-    if (c->done) return;
+    if (c->done) return 0;
     const long long next = c->next_primary;
-    if (next >= pr.n) return;
+    if (next >= pr.n) return 0;
     const double inflight = c->E_admitted - (c->edep_total + c->escaped + c->looper);
-    if (inflight >= w.inflight_cap) return;
-    for (int p = 0; p < 3; ++p)
-        if (4LL * c->q_top[p] >= (long long)w.qcap[p]) return;  // a stack is a quarter full: let it drain first
-    const long long A = (pr.n - next) < (long long)w.wave ? (pr.n - next) : (long long)w.wave;
-    // pass 1: counts per type and energy of the window
-    int cnt[3] = {0, 0, 0};
+    if (inflight >= w.inflight_cap) return 0;
+    long long A = (pr.n - next) < (long long)w.wave ? (pr.n - next) : (long long)w.wave;
+    for (int p = 0; p < kPools; ++p) {
+        if (c->q_top[p] > 0 && 4LL * c->q_top[p] >= (long long)w.qcap[p]) return 0;  // a quarter full: let it drain first
+        const long long room = (long long)w.qcap[p] - c->q_top[p];
+        if (A > room) A = room;  // a wave never asks a stack for more than it can hold (no count exceeds A)
+    }
+    if (A <= 0) return 0;
+    // pass 1: energy of the window and its primaries per pool
+    int cnt[kPools] = {0, 0};
     double ein = 0.0;
     for (long long k = tid; k < A; k += blockDim.x) {
         const int pt = pr.ptype[next + k];
-        cnt[0] += (pt == 0);
-        cnt[1] += (pt == 1);
-        cnt[2] += (pt == 2);
+        cnt[pool_of(pt)] += 1;
         ein += pr.E[next + k] + (pt == kPositron ? 2.0 * kMe : 0.0);
     }
-    for (int p = 0; p < 3; ++p) {
+    for (int p = 0; p < kPools; ++p) {
         int v = cnt[p];
         for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
         if (lane == 0) s_cnt[p][wid] = v;
@@ -170,49 +154,41 @@ __device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) 
     if (lane == 0) s_E[wid] = ein;
     __syncthreads();
     if (tid == 0) {
-        int go = 1;
-        for (int p = 0; p < 3; ++p) {
+        for (int p = 0; p < kPools; ++p) {
             int t = 0;
             for (int k = 0; k < nw; ++k) t += s_cnt[p][k];
             s_total[p] = t;
             s_base[p] = 0;
-            if (c->q_top[p] + t > w.qcap[p]) go = 0;  // no room: try again in a later iteration
         }
-        s_go = go;
+        s_A = A;
     }
     __syncthreads();
-    if (!s_go) return;
-    // pass 2: stable rank of each primary inside its type, tile by tile
+    // pass 2: stable rank of each primary inside its pool, tile by tile
     for (long long base = 0; base < A; base += blockDim.x) {
         const long long k = base + tid;
         const long long i = next + k;
         const int pt = (k < A) ? pr.ptype[i] : -1;
+        const int pl = pt >= 0 ? pool_of(pt) : -1;
         int rank = 0;
-        for (int p = 0; p < 3; ++p) {
-            const unsigned b = __ballot_sync(0xffffffffu, pt == p);
+        for (int p = 0; p < kPools; ++p) {
+            const unsigned b = __ballot_sync(0xffffffffu, pl == p);
             if (lane == 0) s_cnt[p][wid] = __popc(b);
-            if (pt == p) rank = __popc(b & ((1u << lane) - 1u));
+            if (pl == p) rank = __popc(b & ((1u << lane) - 1u));
         }
         __syncthreads();
-        if (pt >= 0) {
-            int before = s_base[pt];
-            for (int q = 0; q < wid; ++q) before += s_cnt[pt][q];
-            const int r = c->q_top[pt] + s_total[pt] - 1 - (before + rank);  // lowest index on top
-            const QueueSoA &q = w.q[pt];
-            q.x[r] = pr.pos3[3 * i];
-            q.y[r] = pr.pos3[3 * i + 1];
-            q.z[r] = pr.pos3[3 * i + 2];
-            q.ux[r] = pr.dir3[3 * i];
-            q.uy[r] = pr.dir3[3 * i + 1];
-            q.uz[r] = pr.dir3[3 * i + 2];
-            q.E[r] = pr.E[i];
-            q.tid[r] = 0ull;
-            q.prim[r] = (uint32_t)(pr.first + i);
-            q.vol[r] = pr.vol[i];
-            q.surf[r] = pr.surf ? pr.surf[i] : -1;
+        if (pl >= 0) {
+            int before = s_base[pl];
+            for (int q = 0; q < wid; ++q) before += s_cnt[pl][q];
+            const int r = c->q_top[pl] + s_total[pl] - 1 - (before + rank);  // lowest index on top
+            const Stack &q = w.q[pl];
+            q.xy[r] = make_double2(pr.pos3[3 * i], pr.pos3[3 * i + 1]);
+            q.zu[r] = make_double2(pr.pos3[3 * i + 2], pr.dir3[3 * i]);
+            q.uu[r] = make_double2(pr.dir3[3 * i + 1], pr.dir3[3 * i + 2]);
+            q.Et[r] = pack_Et(pr.E[i], 0ull);
+            q.id[r] = make_int4((int)(uint32_t)(pr.first + i), pr.vol[i], pr.surf ? pr.surf[i] : -1, pt);
         }
         __syncthreads();
-        if (tid < 3) {
+        if (tid < kPools) {
             int t = 0;
             for (int q = 0; q < nw; ++q) t += s_cnt[tid][q];
             s_base[tid] += t;
@@ -222,10 +198,11 @@ __device__ __forceinline__ void admit_block(const Work &w, const Primaries &pr) 
     if (tid == 0) {
         double e = 0.0;
         for (int k = 0; k < nw; ++k) e += s_E[k];
-        for (int p = 0; p < 3; ++p) c->q_top[p] += s_total[p];
+        for (int p = 0; p < kPools; ++p) c->q_top[p] += s_total[p];
         c->next_primary = next + A;
         c->E_admitted += e;
     }
+    return (int)s_A;
 }
 
 cudaError_t launch_init(const Work &w, const Primaries &pr, cudaStream_t st) {
@@ -238,26 +215,30 @@ constexpr int kPatience = 64;  // iterations without progress before the loop gi
 
 // ------------------------------------------------------------------------------------------------
 // A9 / A12: refill plan and loop control.  One block.  Per pool: exclusive prefix sum of the per-chunk
-// dead counts the step kernel left behind -> rank of every hole; then the sizes of the refill:
+// dead counts the step kernels left behind -> rank of every hole; then the sizes of the refill:
 //   a      holes filled from the stack (hole k, ascending slot index, takes record [q - 1 - k]),
 //   h - a  holes left when the stack is dry: the live range shrinks to n_new and the live tracks above
 //          n_new move into the remaining holes below it (j-th live track from the end -> j-th such hole),
-//   extra  records appended above the old range when the stack holds more than the holes.
+//   extra  records appended above the old range when the stack holds more than the holes -- as far as the pool
+//          has room, and room is what the pools TRADE here: chunks beyond a pool's range go to the free list, and
+//          the free chunks go to the pools in proportion to what their stacks could fill (the
+//          track slots are the resource; no per-workload split of them is needed).
 __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
-    constexpr int kGroupWarps = 10;  // warps 0-9 scan the gamma pool, 10-19 e-, 20-29 e+ (side by side)
-    __shared__ int s_warp[3][kGroupWarps];
+    constexpr int kGroupWarps = 16;  // warps 0-15 scan the photon pool, 16-31 the charged pool (side by side)
+    __shared__ int s_warp[kPools][kGroupWarps];
+    __shared__ int s_h[kPools], s_grant[kPools], s_owned[kPools], s_free;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     Ctl *c = w.ctl;
     if (c->done) return;
     EMX_TL(w, 0, 0, 0);
-    admit_block(w, pr);
+    const int admitted = admit_block(w, pr);
     __syncthreads();
-    const int p = wid / kGroupWarps, wig = wid % kGroupWarps;  // pool of this warp, warp index in its group
-    if (p < 3) {
-        const int gt = wig * 32 + lane;  // thread index in the group
+    {
+        const int p = wid / kGroupWarps, wig = wid % kGroupWarps;  // pool of this warp, warp index in its group
+        const int gt = wig * 32 + lane;                            // thread index in the group
         const int n_old = c->n_live[p];
         const int nch = (n_old + kChunk - 1) / kChunk;
-        constexpr int kPer = 8;  // chunks per thread: one pass of a group covers 2560 chunks
+        constexpr int kPer = 8;  // chunks per thread: one pass of a group covers 4096 chunks
         int carry = 0;           // dead slots before this pass (every thread of the group keeps its own copy)
         for (int base = 0; base < nch; base += kGroupWarps * 32 * kPer) {
             const int k0 = base + gt * kPer;
@@ -293,39 +274,89 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
             carry += total;
             asm volatile("bar.sync %0, %1;" ::"r"(p + 1), "r"(kGroupWarps * 32) : "memory");
         }
-        if (gt == 0) {
-            const int h = carry;
-            const int q = c->q_top[p];
-            const int a = h < q ? h : q;
-            const int n_new = n_old - (h - a);
-            int extra = 0;
-            if (h == a) {
-                extra = q - a;
-                const int room = w.cap[p] - n_old;
-                if (extra > room) extra = room;
-            }
-            PoolPlan pl;
-            pl.n_old = n_old;
-            pl.h = h;
-            pl.a = a;
-            pl.n_new = n_new;
-            pl.extra = extra;
-            pl.n_final = n_new + extra;
-            pl.q_old = q;
-            pl.q_new = q - a - extra;
-            c->plan[p] = pl;
-            c->n_live[p] = pl.n_final;
-            c->q_top[p] = pl.q_new;
-        }
+        if (gt == 0) s_h[p] = carry;
     }
     __syncthreads();
     if (tid == 0) {
-        const long long ng = c->n_live[0], ne = c->n_live[1], np = c->n_live[2];
-        const long long live = ng + ne + np;
-        const long long queued = (long long)c->q_top[0] + c->q_top[1] + c->q_top[2];
+        // the two refills, and how many chunks each pool holds after this iteration
+        int a[kPools], n_new[kPools], want_extra[kPools], base[kPools], d[kPools], g[kPools];
+        for (int p = 0; p < kPools; ++p) {
+            const int n_old = c->n_live[p], h = s_h[p], q = c->q_top[p];
+            a[p] = h < q ? h : q;
+            n_new[p] = n_old - (h - a[p]);
+            want_extra[p] = (h == a[p]) ? q - a[p] : 0;
+            // a pool keeps the chunks of its old range through this iteration (k_move still reads its tail)
+            base[p] = (n_old + kChunk - 1) / kChunk;
+            // ... and never grows into the last pool_reserve chunks of the store, so that the other pool can always start
+            const long long top = (long long)n_new[p] + want_extra[p];
+            long long want = (top + kChunk - 1) / kChunk;
+            if (want > w.n_chunks - w.pool_reserve) want = w.n_chunks - w.pool_reserve;
+            d[p] = want > base[p] ? (int)want - base[p] : 0;
+        }
+        const int avail = w.n_chunks - base[0] - base[1];
+        if (d[0] + d[1] <= avail) {
+            g[0] = d[0];
+            g[1] = d[1];
+        } else {
+            g[0] = (int)((long long)avail * d[0] / (d[0] + d[1]));
+            g[1] = avail - g[0];
+        }
+        for (int p = 0; p < kPools; ++p) {
+            const int n_old = c->n_live[p], h = s_h[p], q = c->q_top[p];
+            const int grant = base[p] + g[p];
+            int extra = want_extra[p];
+            long long room = (long long)grant * kChunk;
+            if (room > w.slot_cap) room = w.slot_cap;
+            room -= n_old;
+            if (extra > room) extra = (int)room;
+            PoolPlan pl;
+            pl.n_old = n_old;
+            pl.h = h;
+            pl.a = a[p];
+            pl.n_new = n_new[p];
+            pl.extra = extra;
+            pl.n_final = n_new[p] + extra;
+            pl.q_old = q;
+            pl.q_new = q - a[p] - extra;
+            c->plan[p] = pl;
+            c->n_live[p] = pl.n_final;
+            c->q_top[p] = pl.q_new;
+            s_grant[p] = grant;
+            s_owned[p] = c->owned[p];
+        }
+        s_free = c->n_free;
+    }
+    __syncthreads();
+    // chunk trading: first every pool returns what it holds beyond its grant, then takes what it is short of
+    for (int p = 0; p < kPools; ++p) {
+        const int own = s_owned[p], grant = s_grant[p], nf = s_free;
+        for (int k = tid; k < own - grant; k += blockDim.x) w.free_list[nf + k] = w.ctab[p][grant + k];
+        __syncthreads();
+        if (tid == 0 && own > grant) {
+            s_free = nf + (own - grant);
+            s_owned[p] = grant;
+        }
+        __syncthreads();
+    }
+    for (int p = 0; p < kPools; ++p) {
+        const int own = s_owned[p], grant = s_grant[p], nf = s_free;
+        for (int k = tid; k < grant - own; k += blockDim.x) w.ctab[p][own + k] = w.free_list[nf - 1 - k];
+        __syncthreads();
+        if (tid == 0 && grant > own) {
+            s_free = nf - (grant - own);
+            s_owned[p] = grant;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        for (int p = 0; p < kPools; ++p) c->owned[p] = s_owned[p];
+        c->n_free = s_free;
+        const long long ng = c->n_live[0], nc = c->n_live[1];
+        const long long live = ng + nc;
+        const long long queued = (long long)c->q_top[0] + c->q_top[1];
         // a track pushes at most 4 records in an iteration (two products and two at-rest photons): where even that
         // fits, the step kernels reserve with one atomic and no look at the top first
-        for (int p = 0; p < 3; ++p) c->q_safe[p] = ((long long)c->q_top[p] + 4LL * live <= (long long)w.qcap[p]) ? 1 : 0;
+        for (int p = 0; p < kPools; ++p) c->q_safe[p] = ((long long)c->q_top[p] + 4LL * live <= (long long)w.qcap[p]) ? 1 : 0;
         if ((unsigned long long)live > c->peak_live) c->peak_live = (unsigned long long)live;
         if ((unsigned long long)queued > c->peak_queue) c->peak_queue = (unsigned long long)queued;
         if (c->iter < (unsigned long long)w.max_log) {
@@ -334,32 +365,34 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
         }
         if (live == 0 && c->next_primary >= w.n_primaries) {
             c->done = 1;
-            c->m_step[0] = c->m_step[1] = c->m_step[2] = 0;
+            c->m_step[0] = c->m_step[1] = 0;
         } else {
             c->iter += 1;
             // R7: a step whose secondaries do not fit on the stacks is not committed and is re-executed in a
             // later iteration with the same (tid, step) and hence the same draws.  Progress = steps committed or
             // field propagations advanced; retiring a tombstone is none (stalled warps can push and retire
-            // tombstones for ever).  kPatience iterations in a row without progress although tracks are live:
-            // the stacks are too small for this problem
+            // tombstones for ever).  kPatience iterations in a row without progress although tracks are live --
+            // or with nothing live, nothing queued and no primary admitted -- : the stacks are too small
             c->m_step[0] = (int)ng;
-            c->m_step[1] = (int)ne;
-            c->m_step[2] = (int)np;
+            c->m_step[1] = (int)nc;
             EMX_TL(w, 0, 1, 1);
-            c->idle_iters = (c->had_live && c->progress == 0ull) ? c->idle_iters + 1 : 0;
+            const bool stuck = (c->had_live && c->progress == 0ull) || (live == 0 && admitted == 0);
+            c->idle_iters = stuck ? c->idle_iters + 1 : 0;
             if (c->idle_iters >= kPatience) {
                 c->error = EMX_E_CAPACITY;
                 c->done = 1;
             }
             c->had_live = live > 0 ? 1 : 0;
-            // time slicing of the field propagation: with many tracks in flight a track may use only a few
-            // substep attempts per iteration (the rest of its step continues next iteration), so that no warp
-            // holds an iteration open for hundreds of substeps; with few tracks left latency matters more
-            c->field_budget = live > w.slice_above ? w.slice_budget : 0x7fffffff;
+            // time slicing of the field propagation: with many tracks in flight a track may be parked after a few
+            // substep attempts (the rest of its step continues next iteration), so that no propagation holds an
+            // iteration open; with few tracks left latency matters more and every propagation runs to its end
+            c->field_min = live > w.slice_above ? w.slice_min : 0x7fffffff;
             c->progress = 0ull;
-            c->work_ctr3[0] = c->work_ctr3[1] = c->work_ctr3[2] = 0;
-            c->work_ctrB[0] = c->work_ctrB[1] = c->work_ctrB[2] = 0;
-            for (int a = 0; a < 3; ++a) c->icount64[a] = 0ull;
+            c->work_a[0] = c->work_a[1] = 0;
+            c->work_b[0] = c->work_b[1] = 0;
+            c->work_0 = c->work_f = 0;
+            for (int p = 0; p < kPools; ++p)
+                for (int k = 0; k < kMaxLists; ++k) c->icount[p][k] = 0;
         }
     }
 }
@@ -379,151 +412,164 @@ __device__ __forceinline__ int rank_in_chunk(bool dead, int *s_w) {
 constexpr int kRefillBlocks = 1184;  // per pool: 8 x 148 blocks, grid-stride over the chunks
 
 // A0: fill holes from the stack, list the holes that are left, append records above the old range
-__global__ void __launch_bounds__(kChunk) k_fill(Work w, int32_t *dbg_src) {
-    __shared__ int s_w[kChunk / 32];
-    const int p = blockIdx.y;
+template <int POOL>
+__device__ __forceinline__ void fill_pool(const Work &w, int32_t *dbg_src, int *s_w) {
     const Ctl *c = w.ctl;
-    if (c->done) return;
-    const PoolPlan pl = c->plan[p];
+    const PoolPlan pl = c->plan[POOL];
     const int top = pl.n_old > pl.n_final ? pl.n_old : pl.n_final;
     const int nch_old = (pl.n_old + kChunk - 1) / kChunk;
-    const TrackSoA &t = w.trk[p];
-    EMX_TL(w, 1, 0, 1);
+    const Store &t = w.st;
     for (int ch = blockIdx.x; ch * kChunk < top; ch += gridDim.x) {  // grid-stride over 128-slot chunks
         const int base = ch * kChunk;
         if (ch < nch_old && base + kChunk <= pl.n_old) {  // chunk inside the old range: skip it if nothing died
-            const int d0 = w.chunk_off[p][ch];
-            const int d1 = (ch + 1 < nch_old) ? w.chunk_off[p][ch + 1] : pl.h;
+            const int d0 = w.chunk_off[POOL][ch];
+            const int d1 = (ch + 1 < nch_old) ? w.chunk_off[POOL][ch + 1] : pl.h;
             if (d1 == d0) continue;
         }
         const int i = base + threadIdx.x;
-        const bool dead = (i < pl.n_old) && (t.alive[i] == 0);
-        const int k = w.chunk_off[p][ch < nch_old ? ch : 0] + rank_in_chunk(dead, s_w);
+        const int s = w.ctab[POOL][ch] * kChunk + threadIdx.x;
+        const bool dead = (i < pl.n_old) && (t.alive[s] == 0);
+        const int k = w.chunk_off[POOL][ch < nch_old ? ch : 0] + rank_in_chunk(dead, s_w);
         if (dead) {
             if (k < pl.a) {
                 const int r = pl.q_old - 1 - k;
-                if (dbg_src) { dbg_src[i] = r; t.alive[i] = 2; }
-                else load_record(w.q[p], r, t, i);
+                if (dbg_src) { dbg_src[i] = r; t.alive[s] = 2; }
+                else load_record<POOL>(w, r, s);
             } else {
-                w.hole_idx[p][k - pl.a] = i;
+                w.hole_idx[POOL][k - pl.a] = i;
             }
         } else if (i >= pl.n_old && i < pl.n_old + pl.extra) {
             const int r = pl.q_old - 1 - pl.a - (i - pl.n_old);
-            if (dbg_src) { dbg_src[i] = r; t.alive[i] = 2; }
-            else load_record(w.q[p], r, t, i);
+            if (dbg_src) { dbg_src[i] = r; t.alive[s] = 2; }
+            else load_record<POOL>(w, r, s);
         }
     }
+}
+__global__ void __launch_bounds__(kChunk) k_fill(Work w, int32_t *dbg_src) {
+    __shared__ int s_w[kChunk / 32];
+    if (w.ctl->done) return;
+    EMX_TL(w, 1, 0, 1);
+    if (blockIdx.y == 0) fill_pool<kPoolGamma>(w, dbg_src, s_w);
+    else fill_pool<kPoolCharged>(w, dbg_src, s_w);
     EMX_TL(w, 1, 1, 1);
 }
 
 // A9: tail compaction when the stack ran dry: live tracks at or above n_new move into the holes below it
-__global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
-    __shared__ int s_w[kChunk / 32];
-    const int p = blockIdx.y;
+template <int POOL>
+__device__ __forceinline__ void move_pool(const Work &w, int32_t *dbg_src, int *s_w) {
     const Ctl *c = w.ctl;
-    if (c->done) return;
-    const PoolPlan pl = c->plan[p];
-    EMX_TL(w, 2, 0, 1);
-    if (pl.h == pl.a) {  // nothing to compact
-        EMX_TL(w, 2, 1, 1);
-        return;
-    }
-    const TrackSoA &t = w.trk[p];
+    const PoolPlan pl = c->plan[POOL];
+    if (pl.h == pl.a) return;  // nothing to compact
+    const Store &t = w.st;
     // grid-stride over the chunks that overlap the tail [n_new, n_old)
     for (int ch = pl.n_new / kChunk + blockIdx.x; ch * kChunk < pl.n_old; ch += gridDim.x) {
         const int i = ch * kChunk + threadIdx.x;
+        const int s = w.ctab[POOL][ch] * kChunk + threadIdx.x;
         const bool in = i < pl.n_old;
-        const uint8_t al = in ? t.alive[i] : (uint8_t)1;
+        const uint8_t al = in ? t.alive[s] : (uint8_t)1;
         const bool dead = al != 1;  // holes of this pass, whether k_fill has refilled them (2) or not (0)
-        const int dead_before = w.chunk_off[p][ch] + rank_in_chunk(dead, s_w);
+        const int dead_before = w.chunk_off[POOL][ch] + rank_in_chunk(dead, s_w);
         if (in && !dead && i >= pl.n_new) {
             const int dead_after = pl.h - dead_before;      // dead slots in (i, n_old)
             const int j = (pl.n_old - 1 - i) - dead_after;  // live tracks in (i, n_old)
-            const int dest = w.hole_idx[p][j];
-            if (dbg_src) { dbg_src[dest] = -2 - i; t.alive[dest] = 2; }
-            else move_slot(t, i, dest);
+            const int dest = w.hole_idx[POOL][j];
+            if (dbg_src) { dbg_src[dest] = -2 - i; t.alive[phys_slot(w, POOL, dest)] = 2; }
+            else move_slot<POOL>(w, s, phys_slot(w, POOL, dest));
         }
     }
+}
+__global__ void __launch_bounds__(kChunk) k_move(Work w, int32_t *dbg_src) {
+    __shared__ int s_w[kChunk / 32];
+    if (w.ctl->done) return;
+    EMX_TL(w, 2, 0, 1);
+    if (blockIdx.y == 0) move_pool<kPoolGamma>(w, dbg_src, s_w);
+    else move_pool<kPoolCharged>(w, dbg_src, s_w);
     EMX_TL(w, 2, 1, 1);
 }
 
 // ------------------------------------------------------------------------------------------------
-// A1-A8 + A10: one step of every live track.  One PERSISTENT launch per pool and phase: the grid is a fixed
-// number of 128-thread blocks (16 warps per SM: what 128 registers per thread allow) whose four warps work
-// independently, each pulling 32-slot chunks of the pool from a device-side work counter until none are
-// left.  A warp never waits for another warp: there is no block-wide barrier and no shared memory.  One pool per launch keeps the code of a
-// single particle type in the instruction caches (a merged kernel for the three types was instruction-fetch
-// bound: profiles/r1_v2_*); the three launches are parallel branches of the iteration graph.
-//   per lane: the track is read once, stepped in registers (step<PT>) and written once;
-//   secondaries go straight onto the typed stacks: the warp counts its records per type with ballots, one
-//   lane reserves the range with one atomic per type ("atomic addition to unambiguously reserve
-//   one or more items") and the lanes write consecutive records;
+// A1-A8 + A10: one step of every live track.  PERSISTENT launches: a fixed number of 128-thread blocks whose
+// four warps work independently, each pulling 32-slot groups of the pool from a device-side work counter until
+// none are left.  A warp never waits for another warp: no block-wide barrier, no shared memory.  One pool and
+// one stage per kernel keeps its code in the instruction caches and its registers few enough for 20-32 warps
+// per SM (the fused kernel of round 1 held 128 registers and 16 warps; profiles/r2_*).
+//   secondaries go straight onto the stacks: the warp counts its records per pool, one lane reserves the range
+//   with one atomic ("atomic addition to unambiguously reserve one or more items") and the lanes
+//   write consecutive records;
 //   tallies: lanes that deposit into the same tally are reduced with warp shuffles and one lane issues the
 //   fp64 atomic (north_star "warp-shuffle reductions for tallies"); run counters are kept in registers, one
-//   counter per lane, across all chunks of the warp and flushed once at the end of the launch.
-#ifndef EMX_WARPS_PER_SM
-#define EMX_WARPS_PER_SM 16
-#endif
-constexpr int kStepWarpsPerSM = EMX_WARPS_PER_SM;
-// warps of a step-kernel block are independent (no barrier, no shared memory); they are grouped four to a
-// block only because block dispatch is what an idle iteration costs (~2.4 ns per block, 21 000 single-warp
-// blocks per iteration = 50 us)
-#ifndef EMX_STEP_BLOCK
-#define EMX_STEP_BLOCK 128
-#endif
-constexpr int kStepBlock = EMX_STEP_BLOCK;
+//   counter per lane, across all groups of the warp and flushed once at the end of the launch.
+constexpr int kStepBlock = 128;
 
-__device__ __forceinline__ void push_record(const QueueSoA &q, int r, const Vec3 &x, const Vec3 &u, double E,
-                                            uint64_t tid, uint32_t prim, int vol) {
-    EMX_ST(&q.x[r], x.x);
-    EMX_ST(&q.y[r], x.y);
-    EMX_ST(&q.z[r], x.z);
-    EMX_ST(&q.ux[r], u.x);
-    EMX_ST(&q.uy[r], u.y);
-    EMX_ST(&q.uz[r], u.z);
-    EMX_ST(&q.E[r], E);
-    EMX_ST((unsigned long long *)&q.tid[r], (unsigned long long)tid);
-    EMX_ST(&q.prim[r], prim);
-    EMX_ST(&q.vol[r], vol);
-    EMX_ST(&q.surf[r], -1);
+template <int POOL>
+__device__ __forceinline__ void push_record(const Work &w, int r, const Vec3 &x, const Vec3 &u, double E, uint64_t tid,
+                                            uint32_t prim, int vol, int ptype) {
+    const Stack &q = w.q[POOL];
+    st_cs(&q.xy[r], make_double2(x.x, x.y));
+    st_cs(&q.zu[r], make_double2(x.z, u.x));
+    st_cs(&q.uu[r], make_double2(u.y, u.z));
+    st_cs(&q.Et[r], pack_Et(E, tid));
+    st_cs(&q.id[r], make_int4((int)prim, vol, -1, ptype));
 }
 
 __device__ __forceinline__ double warp_sum(double v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+__device__ __forceinline__ int warp_scan_incl(int v, int lane) {
+    for (int d = 1; d < 32; d <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += t;
+    }
+    return v;
+}
 
 // per-warp accumulators, spread over the lanes: lane k owns integer counter k (0..7 interactions by process,
-// 8 null interactions, 9..11 tracks created by type, 12..14 steps by type, 15 progress, 16 stalls) and lanes
-// 0..3 own the doubles escaped, below_cut, looper, deposited
+// 8 null interactions, 9..11 tracks created by type, 12..14 steps by type, 15 progress, 16 stalls, 17 slots
+// processed) and lanes 0..3 own the doubles escaped, below_cut, looper, deposited
 struct WarpAcc {
     unsigned long long n;
     double d;
 };
+__device__ __forceinline__ void flush_acc(Ctl *c, const WarpAcc &acc, int lane, unsigned long long *lanes_ctr) {
+    if (acc.n) {
+        unsigned long long *dst = lane < 8    ? &c->inter[lane]
+                                  : lane == 8 ? &c->null_int
+                                  : lane < 12 ? &c->tracks[lane - 9]
+                                  : lane < 15 ? &c->steps[lane - 12]
+                                  : lane == 15 ? &c->progress
+                                               : &c->stalls;
+        if (lane <= 16) atomicAdd(dst, acc.n);
+        if (lane == 17) atomicAdd(lanes_ctr, acc.n);
+    }
+    if (acc.d != 0.0 && lane < 4) {
+        double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
+        atomicAdd(dst, acc.d);
+    }
+}
 
-// Reserve `cnt` records (warp total) on stack ty; returns the base index or -1 when the stack is full.
-// Far from the capacity one atomicAdd does it: kReserveSlack bounds what all resident warps of
-// the three step kernels can request at the same time (one outstanding reservation of <= 96 records each), so
+// Reserve `cnt` records (warp total) on stack `pool`; returns the base index or -1 when the stack is full.
+// Far from the capacity one atomicAdd does it: w.reserve_slack bounds what all resident warps of
+// the step kernels can request at the same time (one outstanding reservation of <= 128 records each), so
 // the top cannot pass the capacity.  Near the capacity a small stack (tests) is reserved by compare-and-swap,
-// which never moves the top past the capacity; a large stack is simply treated as full.  Nothing is ever rolled back: an add-then-subtract scheme lets a
-// reservation succeed above a top that a concurrent failure has inflated, and strands its records.
-constexpr int kReserveSlack = 148 * 3 * 32 * 96;
-
-__device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, int lane) {
+// which never moves the top past the capacity; a large stack is simply treated as full.  Nothing is ever rolled
+// back: an add-then-subtract scheme lets a reservation succeed above a top that a concurrent failure has
+// inflated, and strands its records.
+__device__ __forceinline__ int reserve(Ctl *c, const Work &w, int pool, int cnt, int lane) {
     int r0 = -1;
     if (lane == 0) {
-        const int cap = w.qcap[ty];
-        if (__ldg(&c->q_safe[ty])) {
+        const int cap = w.qcap[pool];
+        if (__ldg(&c->q_safe[pool])) {
             // k_plan's guarantee for this iteration: one round trip to the top instead of two
-            r0 = atomicAdd(&c->q_top[ty], cnt);
+            r0 = atomicAdd(&c->q_top[pool], cnt);
         } else {
-            int old = *(volatile int *)&c->q_top[ty];
-            if ((long long)old + cnt + kReserveSlack <= (long long)cap) {
-                r0 = atomicAdd(&c->q_top[ty], cnt);
-            } else if (cap < 8 * kReserveSlack) {
+            int old = *(volatile int *)&c->q_top[pool];
+            if ((long long)old + cnt + w.reserve_slack <= (long long)cap) {
+                r0 = atomicAdd(&c->q_top[pool], cnt);
+            } else if ((long long)cap < 8LL * w.reserve_slack) {
                 // small stack: exact accounting by compare-and-swap
                 while (old + cnt <= cap) {
-                    const int prev = atomicCAS(&c->q_top[ty], old, old + cnt);
+                    const int prev = atomicCAS(&c->q_top[pool], old, old + cnt);
                     if (prev == old) {
                         r0 = old;
                         break;
@@ -531,7 +577,7 @@ __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int ty, int cnt, i
                     old = prev;
                 }
             }
-            // large stack within kReserveSlack of its capacity: treated as full (thousands of warps spinning on
+            // large stack within the slack of its capacity: treated as full (thousands of warps spinning on
             // one compare-and-swap cost 10x the iteration; the last 2 % of a large stack are not worth it)
         }
     }
@@ -548,69 +594,62 @@ __device__ __forceinline__ int step_bin(uint32_t n) {
     return b < EMX_NHIST ? b : EMX_NHIST - 1;
 }
 
-// index of process `proc` among the processes of particle type PT (the order of C7.8), and back
-template <int PT>
+// index of process `proc` among the interaction lists of its pool, and back
+template <int POOL>
 __device__ __forceinline__ int proc_slot(int proc) {
-    if (PT == kGamma) return proc == EMX_P_COMPTON ? 0 : (proc == EMX_P_PHOTO ? 1 : 2);
-    if (PT == kElectron) return proc == EMX_P_MOLLER ? 0 : 1;
-    return proc == EMX_P_BHABHA ? 0 : (proc == EMX_P_BREMS ? 1 : 2);
+    if (POOL == kPoolGamma) return proc == EMX_P_COMPTON ? 0 : (proc == EMX_P_PHOTO ? 1 : 2);
+    return proc == EMX_P_MOLLER ? 0 : (proc == EMX_P_BHABHA ? 1 : (proc == EMX_P_BREMS ? 2 : 3));
 }
-template <int PT>
+template <int POOL>
 __device__ __forceinline__ int slot_proc(int k) {
-    if (PT == kGamma) return k == 0 ? EMX_P_COMPTON : (k == 1 ? EMX_P_PHOTO : EMX_P_PAIR);
-    if (PT == kElectron) return k == 0 ? EMX_P_MOLLER : EMX_P_BREMS;
-    return k == 0 ? EMX_P_BHABHA : (k == 1 ? EMX_P_BREMS : EMX_P_ANNIH);
+    if (POOL == kPoolGamma) return k == 0 ? EMX_P_COMPTON : (k == 1 ? EMX_P_PHOTO : EMX_P_PAIR);
+    return k == 0 ? EMX_P_MOLLER : (k == 1 ? EMX_P_BHABHA : (k == 2 ? EMX_P_BREMS : EMX_P_ANNIH));
 }
 
-// What both step kernels do with a lane's result: reserve and write the secondaries (A8), write the track
+// what of the slot a kernel's epilogue has to write back
+enum : int { kWrX = 1, kWrU = 2, kWrE = 4 };
+
+// What the finishing kernels do with a lane's result: reserve and write the secondaries (A8), write the track
 // back, tally (A10), count.  `pend` >= 0: the lane's step is not finished -- its interaction `pend` was
-// selected and waits for k_interact; only what has happened so far (move, continuous loss) is committed.
-template <int PT, bool CONSEC>
-__device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint64_t seed, double *tally, int i,
-                                            bool active, bool tomb, bool parked, int pend, Track &t, StepOut &o,
-                                            int vol0, uint32_t step0) {
+// selected and waits for k_b; only what has happened so far (move, continuous loss) is committed.
+// i = pool-local slot, s = physical slot, pt = particle type of the lane's track.
+template <int POOL, int WR, bool CONSEC>
+__device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint64_t seed, double *tally, int i, int s,
+                                            int pt, bool active, bool tomb, int pend, Track &t, StepOut &o, int vol0,
+                                            uint32_t step0) {
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
-    const TrackSoA &ts = w.trk[PT];
-    // ---- A8: secondaries -> typed stacks.  When a stack cannot take the warp's records the lanes that needed
+    const Store &ts = w.st;
+    // ---- A8: secondaries -> stacks.  When a stack cannot take the warp's records the lanes that needed
     // it STALL: nothing of their step is committed (R7).  Records a stalled lane did obtain
-    // for another type become tombstones (E < 0), which the next refill loads and this kernel retires.
+    // on the other stack become tombstones (E < 0), which the next refill loads and the step kernels retire.
     const int ng = (o.s0.ptype == kGamma) + (o.s1.ptype == kGamma) + 2 * o.rest_alloc;
-    const int ne = (o.s0.ptype == kElectron);  // only ordinal 0 is ever an electron
-    const int np = (o.s1.ptype == kPositron);  // only the pair positron
+    const int nc = (o.s0.ptype == kElectron) + (o.s1.ptype == kPositron);  // ordinal 0 an e-, ordinal 1 the pair e+
     bool stall = false;
-    int r_e = -1, r_p = -1, r_g = -1;
-    unsigned b = __ballot_sync(0xffffffffu, ne);
-    if (b) {
-        const int r0 = reserve(c, w, kElectron, __popc(b), lane);
-        if (ne) {
-            if (r0 < 0) stall = true;
-            else r_e = r0 + __popc(b & lt);
-        }
-    }
-    if (PT == kGamma) {  // only photons make positrons
-        b = __ballot_sync(0xffffffffu, np);
+    int r_c = -1, r_g = -1;
+    {
+        const unsigned b = __ballot_sync(0xffffffffu, nc > 0);
         if (b) {
-            const int r0 = reserve(c, w, kPositron, __popc(b), lane);
-            if (np) {
+            int inc = nc;
+            if (POOL == kPoolGamma) inc = warp_scan_incl(nc, lane);  // 0..2 per lane (pair production)
+            else inc = __popc(b & lt) + nc;                          // 0..1 per lane
+            const int tot = POOL == kPoolGamma ? __shfl_sync(0xffffffffu, inc, 31) : __popc(b);
+            const int r0 = reserve(c, w, kPoolCharged, tot, lane);
+            if (nc) {
                 if (r0 < 0) stall = true;
-                else r_p = r0 + __popc(b & lt);
+                else r_c = r0 + inc - nc;
             }
         }
     }
-    if (PT != kGamma) {  // only e+- make photons: 0..3 per lane -> inclusive warp scan of the counts
-        b = __ballot_sync(0xffffffffu, ng > 0);
+    if (POOL == kPoolCharged) {  // only e+- make photons: 0..3 per lane
+        const unsigned b = __ballot_sync(0xffffffffu, ng > 0);
         if (b) {
-            int inc = ng;
-            for (int d = 1; d < 32; d <<= 1) {
-                const int v = __shfl_up_sync(0xffffffffu, inc, d);
-                if (lane >= d) inc += v;
-            }
-            const int r0 = reserve(c, w, kGamma, __shfl_sync(0xffffffffu, inc, 31), lane);
+            const int inc = warp_scan_incl(ng, lane);
+            const int r0 = reserve(c, w, kPoolGamma, __shfl_sync(0xffffffffu, inc, 31), lane);
             if (ng) {
                 if (r0 < 0) stall = true;
                 else r_g = r0 + inc - ng;
@@ -618,65 +657,62 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
         }
     }
     if (stall) {
-        if (r_e >= 0) w.q[kElectron].E[r_e] = -1.0;
-        if (r_p >= 0) w.q[kPositron].E[r_p] = -1.0;
+        if (r_c >= 0)
+            for (int k = 0; k < nc; ++k) w.q[kPoolCharged].Et[r_c + k] = make_double2(-1.0, 0.0);
         if (r_g >= 0)
-            for (int k = 0; k < ng; ++k) w.q[kGamma].E[r_g + k] = -1.0;
+            for (int k = 0; k < ng; ++k) w.q[kPoolGamma].Et[r_g + k] = make_double2(-1.0, 0.0);
     } else {
-        if (ne) push_record(w.q[kElectron], r_e, t.x, o.s0.u, o.s0.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 0u),
-                            t.prim, t.vol);
-        if (np) push_record(w.q[kPositron], r_p, t.x, o.s1.u, o.s1.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 1u),
-                            t.prim, t.vol);
-        if (ng) {
-            const QueueSoA &q = w.q[kGamma];
+        const uint32_t k0 = (uint32_t)seed;
+        if (nc) {
+            int r = r_c;
+            if (o.s0.ptype == kElectron)
+                push_record<kPoolCharged>(w, r++, t.x, o.s0.u, o.s0.E, child_tid(k0, t.prim, t.tid, step0, 0u), t.prim, t.vol, kElectron);
+            if (o.s1.ptype == kPositron)
+                push_record<kPoolCharged>(w, r++, t.x, o.s1.u, o.s1.E, child_tid(k0, t.prim, t.tid, step0, 1u), t.prim, t.vol, kPositron);
+        }
+        if (POOL == kPoolCharged && ng) {
             int r = r_g;
             if (o.s0.ptype == kGamma)
-                push_record(q, r++, t.x, o.s0.u, o.s0.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 0u), t.prim, t.vol);
+                push_record<kPoolGamma>(w, r++, t.x, o.s0.u, o.s0.E, child_tid(k0, t.prim, t.tid, step0, 0u), t.prim, t.vol, kGamma);
             if (o.s1.ptype == kGamma)
-                push_record(q, r++, t.x, o.s1.u, o.s1.E, child_tid((uint32_t)seed, t.prim, t.tid, step0, 1u), t.prim, t.vol);
+                push_record<kPoolGamma>(w, r++, t.x, o.s1.u, o.s1.E, child_tid(k0, t.prim, t.tid, step0, 1u), t.prim, t.vol, kGamma);
             if (o.rest_alloc) {
                 const Vec3 mu = {-o.rest_u.x, -o.rest_u.y, -o.rest_u.z};
-                push_record(q, r++, t.x, o.rest_u, kMe, child_tid((uint32_t)seed, t.prim, t.tid, step0, 2u), t.prim, t.vol);
-                push_record(q, r++, t.x, mu, kMe, child_tid((uint32_t)seed, t.prim, t.tid, step0, 3u), t.prim, t.vol);
+                push_record<kPoolGamma>(w, r++, t.x, o.rest_u, kMe, child_tid(k0, t.prim, t.tid, step0, 2u), t.prim, t.vol, kGamma);
+                push_record<kPoolGamma>(w, r++, t.x, mu, kMe, child_tid(k0, t.prim, t.tid, step0, 3u), t.prim, t.vol, kGamma);
             }
         }
     }
-    const bool commit = active && !tomb && !stall && !parked;
+    const bool commit = active && !tomb && !stall;
 
     // ---- write the track back (A5-A7 results); tid and prim never change
     if (commit) {
-        ts.x[i] = t.x.x;
-        ts.y[i] = t.x.y;
-        ts.z[i] = t.x.z;
-        ts.ux[i] = t.u.x;
-        ts.uy[i] = t.u.y;
-        ts.uz[i] = t.u.z;
-        ts.E[i] = t.E;
-        ts.step[i] = t.step;
-        ts.vol[i] = t.vol;
-        ts.surf[i] = t.surf;
-        if (PT != kGamma) ts.fs_a[i] = 0;
-        ts.pend[i] = (uint8_t)(pend >= 0 ? 1 + pend : 0);
+        if (WR & kWrX) ts.xy[s] = make_double2(t.x.x, t.x.y);
+        if (WR & (kWrX | kWrU)) ts.zu[s] = make_double2(t.x.z, t.u.x);
+        if (WR & kWrU) ts.uu[s] = make_double2(t.u.y, t.u.z);
+        if (WR & kWrE) ts.Et[s] = pack_Et(t.E, t.tid);
+        ts.id[s] = make_int4((int)t.prim, (int)t.step, t.vol, t.surf);
+        ts.stage[s] = (uint8_t)(pend >= 0 ? kStPend + pend : kStFresh);
     }
     const bool died = active && (tomb || (commit && !t.alive));
-    if (active) ts.alive[i] = (uint8_t)(died ? 0 : 1);
+    if (active) ts.alive[s] = (uint8_t)(died ? 0 : 1);
     // steps-per-track histogram: a track that ends here took step0 + 1 steps; lanes with the same bin share
     // one atomic (most tracks end after a few steps: per-lane atomics on those few bins cost 70 % more time)
     {
         const bool ended = died && !tomb;
         const unsigned be = __ballot_sync(0xffffffffu, ended);
         if (ended) {
-            const int hb = step_bin(step0 + 1u);
+            const int hb = step_bin(step0 + 1u) + EMX_NHIST * pt;
             const unsigned m = __match_any_sync(be, hb);
-            if (lane == __ffs(m) - 1) atomicAdd(&c->hist[PT][hb], (unsigned long long)__popc(m));
+            if (lane == __ffs(m) - 1) atomicAdd(&c->hist[0][hb], (unsigned long long)__popc(m));
         }
     }
     // dead slots per 128-slot chunk, for the refill plan (A9)
     if (CONSEC) {  // the warp's lanes are 32 consecutive slots of one chunk
         const unsigned bd = __ballot_sync(0xffffffffu, died);
-        if (bd && lane == 0) atomicAdd(&w.chunk_dead[PT][i / kChunk], __popc(bd));
+        if (bd && lane == 0) atomicAdd(&w.chunk_dead[POOL][i / kChunk], __popc(bd));
     } else if (died) {
-        atomicAdd(&w.chunk_dead[PT][i / kChunk], 1);
+        atomicAdd(&w.chunk_dead[POOL][i / kChunk], 1);
     }
 
     // ---- A10: per-volume tally.  Lanes with the same tally id are summed with shuffles; one atomic per group.
@@ -690,8 +726,8 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
             const int key = __shfl_sync(0xffffffffu, tl, leader);
             const bool mine = (tl == key);
             const unsigned grp = __ballot_sync(0xffffffffu, mine);
-            const double s = warp_sum(mine ? o.edep : 0.0);
-            if (lane == leader) atomicAdd(&tally[key], s);
+            const double sum = warp_sum(mine ? o.edep : 0.0);
+            if (lane == leader) atomicAdd(&tally[key], sum);
             m &= ~grp;
         }
     }
@@ -724,20 +760,24 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
         }
         const unsigned n_rest = __popc(__ballot_sync(0xffffffffu, commit && o.rest));
         if (lane == EMX_P_REST) add += n_rest;
-        const unsigned n_e = __popc(__ballot_sync(0xffffffffu, commit && ne));
-        const unsigned n_p = __popc(__ballot_sync(0xffffffffu, commit && np));
+        const unsigned n_e = __popc(__ballot_sync(0xffffffffu, commit && o.s0.ptype == kElectron));
+        const unsigned n_p = __popc(__ballot_sync(0xffffffffu, commit && o.s1.ptype == kPositron));
         unsigned n_g = commit ? (unsigned)ng : 0u;
         for (int o2 = 16; o2 > 0; o2 >>= 1) n_g += __shfl_xor_sync(0xffffffffu, n_g, o2);
+        const bool stepped = commit && pend < 0;  // completed steps
         const unsigned n_commit = __popc(__ballot_sync(0xffffffffu, commit));
-        const unsigned n_done = __popc(__ballot_sync(0xffffffffu, commit && pend < 0));  // completed steps
-        const unsigned n_parked = __popc(__ballot_sync(0xffffffffu, parked));
+        const unsigned n_s0 = __popc(__ballot_sync(0xffffffffu, stepped && pt == kGamma));
+        const unsigned n_s1 = __popc(__ballot_sync(0xffffffffu, stepped && pt == kElectron));
+        const unsigned n_s2 = __popc(__ballot_sync(0xffffffffu, stepped && pt == kPositron));
         const unsigned n_stall = __popc(__ballot_sync(0xffffffffu, active && stall));
         const unsigned n_active = __popc(__ballot_sync(0xffffffffu, active));
         if (lane == 9) add = n_g;
         if (lane == 10) add = n_e;
         if (lane == 11) add = n_p;
-        if (lane == 12 + PT) add = n_done;
-        if (lane == 15) add = n_commit + n_parked;
+        if (lane == 12) add = n_s0;
+        if (lane == 13) add = n_s1;
+        if (lane == 14) add = n_s2;
+        if (lane == 15) add = n_commit;
         if (lane == 16) add = n_stall;
         if (lane == 17) add = n_active;
         acc.n += add;
@@ -745,249 +785,381 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     return acc;
 }
 
-// one pool per launch: the code of a single particle type stays resident in the instruction caches
-
-// Phase A of a chunk: items 1-7 of C7 and the selection of the discrete process for 32 consecutive slots.
+// ---- phase A of a group of 32 consecutive slots.
+// FUSED: stages a0, a1 (straight move) and a2 in registers (photons; e+- without a field).
+// else:  stage a2 alone, for the slots whose move the propagation kernel has finished.
 // Lanes whose step ends here (boundary, loss-limited, truncated, killed) are committed; lanes with an
 // interaction pending are committed as far as they got and filed in the list of their process, so that
-// k_interact runs every interactor on full warps (B:north_star "partitioned by next action").
-template <int PT, bool MAP, bool EXT>
-__device__ __forceinline__ WarpAcc pre_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
-                                             int n_live, int budget) {
+// k_b runs every interactor on full warps (B:north_star "partitioned by next action").
+template <int POOL, bool EXT, bool FUSED>
+__device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
+                                           int n_live) {
+    constexpr bool CH = POOL == kPoolCharged;
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const int i = base + lane;
-    const TrackSoA &ts = w.trk[PT];
-    const bool active = i < n_live;
+    const Store &ts = w.st;
+    const int s = w.ctab[POOL][base / kChunk] * kChunk + (i % kChunk);
+    const bool in = i < n_live;
     Track t;
     StepOut o;
-    int vol0 = 0;
+    int vol0 = 0, pt = CH ? kElectron : kGamma;
     uint32_t step0 = 0;
-    // every field of the slot is loaded up front, whether or not the lane turns out to need it (tombstone, stalled
-    // interaction, no propagation in progress): one round trip to L2 instead of a chain of four dependent ones
+    int stage = kStFresh, al = 1;
     double E0 = 0.0;
-    uint8_t pend_b = 0;
-    FieldState fs;
-    fs.s_done = fs.h = 0.0;
-    fs.attempt = 0;
-    if (active) {
-        E0 = ts.E[i];
-        pend_b = ts.pend[i];
-        t.x = {ts.x[i], ts.y[i], ts.z[i]};
-        t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
-        t.tid = ts.tid[i];
-        t.prim = ts.prim[i];
-        t.step = ts.step[i];
-        t.vol = ts.vol[i];
-        t.surf = ts.surf[i];
-        if (PT != kGamma) {
-            fs.attempt = ts.fs_a[i];
-            fs.s_done = ts.fs_s[i];
-            fs.h = ts.fs_h[i];
-        }
+    if (in) {
+        al = ts.alive[s];
+        stage = ts.stage[s];
+        const double2 Et = ts.Et[s];
+        E0 = Et.x;
+        t.tid = tid_of(Et);
+        if (CH) pt = ts.ptype[s];
     }
-    const bool tomb = active && E0 < 0.0;  // tombstone record: retire the slot without stepping
-    const int pend_in = (active && !tomb) ? (int)pend_b - 1 : -1;  // interaction still waiting (stalled)
+    const bool tomb = in && E0 < 0.0;  // tombstone record: retire the slot without stepping
+    const bool waiting = in && !tomb && stage >= kStPend;  // interaction selected earlier and stalled: file it again
+    const bool go = in && !tomb && (FUSED ? stage == kStFresh : stage == kStMoved);
     int pend = -1;
-    if (active && !tomb && pend_in < 0) {
+    clear_out(o);
+    t.alive = 1;
+    if (go) {
+        const int4 id = ts.id[s];
+        const double2 xy = ts.xy[s], zu = ts.zu[s], uu = ts.uu[s];
+        t.x = {xy.x, xy.y, zu.x};
+        t.u = {zu.y, uu.x, uu.y};
         t.E = E0;
-        t.alive = 1;
+        t.prim = (uint32_t)id.x;
+        t.step = (uint32_t)id.y;
+        t.vol = id.z;
+        t.surf = id.w;
         vol0 = t.vol;
         step0 = t.step;
-        pend = step_pre<PT, MAP, EXT>(P, seed, t, o, fs, budget);
-        if (PT != kGamma && o.suspended) {
-            // the propagation continues in the next iteration: park position, direction, surface flag and the
-            // loop variables; nothing else of the step has happened yet
-            ts.x[i] = t.x.x;
-            ts.y[i] = t.x.y;
-            ts.z[i] = t.x.z;
-            ts.ux[i] = t.u.x;
-            ts.uy[i] = t.u.y;
-            ts.uz[i] = t.u.z;
-            ts.surf[i] = t.surf;
-            ts.fs_s[i] = fs.s_done;
-            ts.fs_h[i] = fs.h;
-            ts.fs_a[i] = fs.attempt;
-            o.s0.ptype = o.s1.ptype = -1;
-            o.rest_alloc = 0;
-            o.process = -1;
-            o.edep = o.below_cut = o.escaped = o.looper = 0.0;
-            o.null_int = o.rest = 0;
-            t.alive = 1;
+        Carry cy;
+        if (FUSED) {
+            step_a0<CH, EXT>(P, seed, pt, t, cy);
+            if (cy.action != kActCut) move_straight(P, t, cy);
+        } else {
+            cy.action = ts.act[s];
+            cy.s = ts.s_done[s];
+            cy.hit = ts.att[s];
+            cy.s_phys = 0.0;
         }
-    } else {
-        o.s0.ptype = o.s1.ptype = -1;
-        o.rest_alloc = 0;
-        o.process = -1;
-        o.edep = o.below_cut = o.escaped = o.looper = 0.0;
-        o.null_int = o.rest = 0;
-        o.suspended = 0;
-        t.alive = 1;
+        pend = step_a2<CH, EXT>(P, seed, pt, t, o, cy);
     }
-    const bool parked = active && !tomb && (PT != kGamma) && o.suspended;
-    const bool waiting = pend_in >= 0;  // nothing to do in this phase
-
-    // file the lanes with a pending interaction (new or stalled) in the list of their process.  The three list
-    // counters of a pool are packed into one 64-bit word (21 bits each; pools hold fewer than 2^21 slots, checked
-    // by the host), so one atomic per warp reserves the entries of all three lists.  It is issued BEFORE the
-    // epilogue and its result is used after it: the round trip to L2 runs under the epilogue's work.
-    const int pk = waiting ? proc_slot<PT>(pend_in) : (pend >= 0 && !parked ? proc_slot<PT>(pend) : -1);
-    const unsigned b0 = __ballot_sync(0xffffffffu, pk == 0);
-    const unsigned b1 = __ballot_sync(0xffffffffu, pk == 1);
-    const unsigned b2 = __ballot_sync(0xffffffffu, pk == 2);
-    unsigned long long lbase = 0ull;
-    if ((b0 | b1 | b2) && lane == 0)
-        lbase = atomicAdd(&c->icount64[PT], (unsigned long long)__popc(b0) | ((unsigned long long)__popc(b1) << 21) |
-                                               ((unsigned long long)__popc(b2) << 42));
-
-    WarpAcc acc = epilogue<PT, true>(P, w, seed, tally, i, active && !waiting, tomb, parked, pend, t, o, vol0, step0);
-
-    if (b0 | b1 | b2) {
-        lbase = __shfl_sync(0xffffffffu, lbase, 0);
-        if (pk >= 0) {
-            const unsigned bk = pk == 0 ? b0 : (pk == 1 ? b1 : b2);
-            const int r0 = (int)((lbase >> (21 * pk)) & 0x1fffffull);
-            w.ilist[PT][pk][r0 + __popc(bk & lt)] = i;
+    // file the lanes with a pending interaction (new or stalled) in the list of their process: one atomic per
+    // warp and non-empty list
+    const int pk = waiting ? proc_slot<POOL>(stage - kStPend) : (pend >= 0 ? proc_slot<POOL>(pend) : -1);
+    constexpr int nk = CH ? 4 : 3;
+    int my_base = 0;
+    unsigned my_mask = 0;
+#pragma unroll
+    for (int k = 0; k < nk; ++k) {
+        const unsigned b = __ballot_sync(0xffffffffu, pk == k);
+        if (b) {
+            int r0 = 0;
+            if (lane == 0) r0 = atomicAdd(&c->icount[POOL][k], __popc(b));
+            r0 = __shfl_sync(0xffffffffu, r0, 0);
+            if (pk == k) {
+                my_base = r0;
+                my_mask = b;
+            }
         }
     }
+    // FUSED: position moved here; a2: position and direction were written by the propagation kernel, the
+    // direction changes again only through multiple scattering
+    constexpr int WR = FUSED ? (kWrX | (CH ? kWrE : 0) | (CH && EXT ? kWrU : 0)) : (kWrE | (EXT ? kWrU : 0));
+    WarpAcc acc = epilogue<POOL, WR, true>(P, w, seed, tally, i, s, pt, go || tomb, tomb, pend, t, o, vol0, step0);
+    if (pk >= 0) w.ilist[POOL][pk][my_base + __popc(my_mask & lt)] = i;
+    // a track the refill has just moved and that no kernel finishes in this iteration (parked propagation, stalled
+    // interaction) still carries the mark of the refill pass
+    if (in && !(go || tomb) && al == 2) ts.alive[s] = 1;
     return acc;
 }
 
-// Phase B of a chunk: 32 tracks of pool PT waiting for the same interactor (list k of the pool).
-template <int PT>
-__device__ __forceinline__ WarpAcc interact_chunk(const Params &P, const Work &w, uint64_t seed, double *tally, int k,
-                                                  int first, int n_list) {
-    const int lane = threadIdx.x & 31;
-    const int idx = first + lane;
-    const TrackSoA &ts = w.trk[PT];
-    const bool active = idx < n_list;
-    const int i = active ? w.ilist[PT][k][idx] : 0;
-    Track t;
-    StepOut o;
-    o.action = EMX_A_DISCRETE;
-    o.process = -1;
-    o.s0.ptype = o.s1.ptype = -1;
-    o.rest_alloc = 0;
-    o.edep = o.below_cut = o.escaped = o.looper = o.s = 0.0;
-    o.n_draws = o.null_int = o.rest = o.suspended = 0;
-    int vol0 = 0;
-    uint32_t step0 = 0;
-    t.alive = 1;
-    if (active) {
-        t.x = {ts.x[i], ts.y[i], ts.z[i]};
-        t.u = {ts.ux[i], ts.uy[i], ts.uz[i]};
-        t.E = ts.E[i];
-        t.tid = ts.tid[i];
-        t.prim = ts.prim[i];
-        t.step = ts.step[i];
-        t.vol = ts.vol[i];
-        t.surf = -1;
-        vol0 = t.vol;
-        step0 = t.step;
-        step_interact<PT>(P, seed, t, o, slot_proc<PT>(k));
-    }
-    return epilogue<PT, false>(P, w, seed, tally, i, active, false, false, -1, t, o, vol0, step0);
-}
-
-template <int PT, bool MAP, bool EXT = false>
-__global__ void __launch_bounds__(kStepBlock, kStepWarpsPerSM * 32 / kStepBlock) k_step_pool(const __grid_constant__ Params P,
-                                                                  const __grid_constant__ Work w, uint64_t seed,
-                                                                  double *tally) {
+// the persistent loop of the dense phase-A kernels
+template <int POOL, bool EXT, bool FUSED>
+__device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, uint64_t seed, double *tally, int node) {
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
-    const int nl = c->m_step[PT];
+    const int nl = c->m_step[POOL];
     const int total = (nl + 31) >> 5;
-    const int budget = c->field_budget;
-    EMX_TL(w, 3 + PT, 0, 1);
+    EMX_TL(w, node, 0, 1);
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
     int k_next = 0;
-    if (lane == 0) k_next = atomicAdd(&c->work_ctr3[PT], 1);
+    if (lane == 0) k_next = atomicAdd(&c->work_a[POOL], 1);
     for (;;) {
         const int k = __shfl_sync(0xffffffffu, k_next, 0);
         if (k >= total) break;
-        if (lane == 0) k_next = atomicAdd(&c->work_ctr3[PT], 1);
-        const WarpAcc d = pre_chunk<PT, MAP, EXT>(P, w, seed, tally, k << 5, nl, budget);
+        if (lane == 0) k_next = atomicAdd(&c->work_a[POOL], 1);
+        const WarpAcc d = a_group<POOL, EXT, FUSED>(P, w, seed, tally, k << 5, nl);
         acc.n += d.n;
         acc.d += d.d;
     }
-    if (acc.n) {
-        unsigned long long *dst = lane < 8    ? &c->inter[lane]
-                                  : lane == 8 ? &c->null_int
-                                  : lane < 12 ? &c->tracks[lane - 9]
-                                  : lane < 15 ? &c->steps[lane - 12]
-                                  : lane == 15 ? &c->progress
-                                               : &c->stalls;
-        if (lane <= 16) atomicAdd(dst, acc.n);
-        if (lane == 17) atomicAdd(&c->lanes[0][PT], acc.n);
-    }
-    EMX_TL(w, 3 + PT, 1, 1);
-    if (acc.d != 0.0 && lane < 4) {
-        double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
-        atomicAdd(dst, acc.d);
-    }
+    flush_acc(c, acc, lane, &c->lanes[2][POOL]);
+    EMX_TL(w, node, 1, 1);
 }
 
-// Phase B: the interactors.  Persistent single-warp blocks pull 32-entry chunks of the pool's process lists;
-// a warp runs ONE interactor on (up to) 32 tracks that all selected it.
-#ifndef EMX_WARPS_B
-#define EMX_WARPS_B EMX_WARPS_PER_SM
+#ifndef EMX_BLOCKS_A
+#define EMX_BLOCKS_A 4   // resident 128-thread blocks per SM the dense phase-A kernels are compiled for
 #endif
-template <int PT>
-__global__ void __launch_bounds__(kStepBlock, EMX_WARPS_B * 32 / kStepBlock) k_interact(const __grid_constant__ Params P,
-                                                                 const __grid_constant__ Work w, uint64_t seed,
-                                                                 double *tally) {
+#ifndef EMX_BLOCKS_A2
+#define EMX_BLOCKS_A2 5
+#endif
+#ifndef EMX_BLOCKS_B
+#define EMX_BLOCKS_B 4
+#endif
+#ifndef EMX_BLOCKS_F
+#define EMX_BLOCKS_F 5
+#endif
+#ifndef EMX_BLOCKS_0
+#define EMX_BLOCKS_0 8
+#endif
+
+template <int POOL, bool EXT>
+__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_A) k_a(const __grid_constant__ Params P, const __grid_constant__ Work w,
+                                                                uint64_t seed, double *tally) {
+    a_kernel_body<POOL, EXT, true>(P, w, seed, tally, 3 + POOL);
+}
+template <bool EXT>
+__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_A2) k_a2(const __grid_constant__ Params P, const __grid_constant__ Work w,
+                                                                  uint64_t seed, double *tally) {
+    a_kernel_body<kPoolCharged, EXT, false>(P, w, seed, tally, 4);
+}
+
+// ---- stage a0 of the charged pool when there is a field: limits of every fresh track (dense, nothing but
+// per-lane work).  A track below the tracking cut goes straight to stage a2.
+template <bool EXT>
+__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_0) k_a0(const __grid_constant__ Params P, const __grid_constant__ Work w,
+                                                                 uint64_t seed) {
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
-    constexpr int nk = (PT == kElectron) ? 2 : 3;
+    const int nl = c->m_step[kPoolCharged];
+    const int total = (nl + 31) >> 5;
+    const Store &ts = w.st;
+    EMX_TL(w, 7, 0, 1);
+    unsigned long long n_done = 0;
+    int k_next = 0;
+    if (lane == 0) k_next = atomicAdd(&c->work_0, 1);
+    for (;;) {
+        const int k = __shfl_sync(0xffffffffu, k_next, 0);
+        if (k >= total) break;
+        if (lane == 0) k_next = atomicAdd(&c->work_0, 1);
+        const int i = (k << 5) + lane;
+        if (i >= nl) continue;
+        const int s = phys_slot(w, kPoolCharged, i);
+        if (ts.stage[s] != kStFresh) continue;
+        const double2 Et = ts.Et[s];
+        if (Et.x < 0.0) continue;  // tombstone: stage a2 retires it
+        const int4 id = ts.id[s];
+        Track t;
+        t.E = Et.x;
+        t.tid = tid_of(Et);
+        t.prim = (uint32_t)id.x;
+        t.step = (uint32_t)id.y;
+        t.vol = id.z;
+        Carry cy;
+        step_a0<true, EXT>(P, seed, ts.ptype[s], t, cy);
+        ts.s_phys[s] = cy.s_phys;
+        ts.act[s] = (uint8_t)cy.action;
+        ts.stage[s] = (uint8_t)(cy.action == kActCut ? kStMoved : kStReady);
+        n_done += 1;
+    }
+    for (int o = 16; o > 0; o >>= 1) n_done += __shfl_xor_sync(0xffffffffu, n_done, o);
+    if (lane == 0 && n_done) atomicAdd(&c->lanes[0][kPoolCharged], n_done);
+    EMX_TL(w, 7, 1, 1);
+}
+
+// ---- stage a1 of the charged pool in a field: the adaptive RK4 of C9, ONE ATTEMPT of the substep loop per pass
+// of the warp.  A lane whose track is done (or parked) takes the next track of the pool in the same pass, so the
+// warp stays full whether a propagation needs 1 attempt or 1000 (a lane that runs the whole loop of its own
+// track idles 31 others for as long as the longest of them lasts: the e- kernel of round 1 spent 212 of the 311 us
+// of an iteration that way once the field had its true strength).  A track may be parked after field_min
+// attempts once the pool has no track left to hand out (or after slice_max attempts): its loop variables go to
+// the slot and the next iteration continues the SAME sequence of substeps.
+template <bool MAP, int AX>
+__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid_constant__ Params P, const __grid_constant__ Work w) {
+    Ctl *c = w.ctl;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    const int nl = c->m_step[kPoolCharged];
+    const int min_att = c->field_min, max_att = w.slice_max;
+    const Store &ts = w.st;
+    EMX_TL(w, 8, 0, 1);
+    bool have = false, dry = false;
+    int s = 0, vol = 0, surf = -1, used = 0, act = 0;
+    Vec3 x = {0.0, 0.0, 0.0}, u = {0.0, 0.0, 1.0};
+    double kappa = 1.0, s_max = 0.0;
+    FieldState fs;
+    fs.s_done = fs.h = 0.0;
+    fs.attempt = 0;
+    unsigned n_att = 0, n_trk = 0;
+    for (;;) {
+        // hand the idle lanes the next slots of the pool
+        unsigned need = __ballot_sync(0xffffffffu, !have && !dry);
+        while (need) {
+            const int leader = __ffs(need) - 1;
+            int i0 = 0;
+            if (lane == leader) i0 = atomicAdd(&c->work_f, __popc(need));
+            i0 = __shfl_sync(0xffffffffu, i0, leader);
+            if (!have && !dry) {
+                const int i = i0 + __popc(need & lt);
+                if (i >= nl) {
+                    dry = true;
+                } else {
+                    s = phys_slot(w, kPoolCharged, i);
+                    const int stage = ts.stage[s];
+                    if (stage == kStReady || stage == kStParked) {
+                        const double2 xy = ts.xy[s], zu = ts.zu[s], uu = ts.uu[s];
+                        const int4 id = ts.id[s];
+                        x = {xy.x, xy.y, zu.x};
+                        u = {zu.y, uu.x, uu.y};
+                        vol = id.z;
+                        surf = id.w;
+                        s_max = ts.s_phys[s];
+                        act = ts.act[s];
+                        kappa = curvature(P, ts.ptype[s], ts.Et[s].x);
+                        if (!MAP && AX != kAxisAny) kappa *= P.Bhat[AX];
+                        if (stage == kStReady) {
+                            field_begin(kappa, s_max, fs);
+                        } else {
+                            fs.s_done = ts.s_done[s];
+                            fs.h = ts.h_try[s];
+                            fs.attempt = ts.att[s];
+                        }
+                        have = true;
+                        used = 0;
+                        n_trk += 1;
+                    }
+                }
+            }
+            need = __ballot_sync(0xffffffffu, !have && !dry);
+        }
+        if (!__ballot_sync(0xffffffffu, have)) break;
+        const bool pool_dry = __ballot_sync(0xffffffffu, dry) != 0u;
+        if (have) {
+            int hit;
+            double sres;
+            const bool done = field_attempt<MAP, AX>(P, vol, surf, x, u, kappa, s_max, fs, hit, sres);
+            used += 1;
+            n_att += 1;
+            if (done) {
+                Carry cy;
+                cy.s_phys = s_max;
+                cy.action = act;
+                field_move_done(cy, sres, hit);
+                ts.xy[s] = make_double2(x.x, x.y);
+                ts.zu[s] = make_double2(x.z, u.x);
+                ts.uu[s] = make_double2(u.y, u.z);
+                ts.s_done[s] = cy.s;
+                ts.att[s] = cy.hit;
+                ts.act[s] = (uint8_t)cy.action;
+                ts.stage[s] = kStMoved;
+                have = false;
+            } else if (used >= min_att && (pool_dry || used >= max_att)) {
+                ts.xy[s] = make_double2(x.x, x.y);
+                ts.zu[s] = make_double2(x.z, u.x);
+                ts.uu[s] = make_double2(u.y, u.z);
+                reinterpret_cast<int *>(ts.id)[4 * (size_t)s + 3] = surf;
+                ts.s_done[s] = fs.s_done;
+                ts.h_try[s] = fs.h;
+                ts.att[s] = fs.attempt;
+                ts.stage[s] = kStParked;
+                have = false;
+            }
+        }
+    }
+    unsigned long long a = n_att, b = n_trk;
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+    }
+    if (lane == 0 && a) {
+        atomicAdd(&c->progress, a);
+        atomicAdd(&c->attempts, a);
+        atomicAdd(&c->lanes[1][kPoolCharged], b);
+    }
+    EMX_TL(w, 8, 1, 1);
+}
+
+// ---- phase B of a group: 32 tracks of a pool waiting for the same interactor (list k of the pool).
+template <int POOL>
+__device__ __forceinline__ WarpAcc b_group(const Params &P, const Work &w, uint64_t seed, double *tally, int k, int first,
+                                           int n_list) {
+    constexpr bool CH = POOL == kPoolCharged;
+    const int lane = threadIdx.x & 31;
+    const int idx = first + lane;
+    const Store &ts = w.st;
+    const bool active = idx < n_list;
+    const int i = active ? w.ilist[POOL][k][idx] : 0;
+    const int s = active ? phys_slot(w, POOL, i) : 0;
+    Track t;
+    StepOut o;
+    clear_out(o);
+    o.action = EMX_A_DISCRETE;
+    int vol0 = 0, pt = CH ? kElectron : kGamma;
+    uint32_t step0 = 0;
+    t.alive = 1;
+    if (active) {
+        const double2 xy = ts.xy[s], zu = ts.zu[s], uu = ts.uu[s], Et = ts.Et[s];
+        const int4 id = ts.id[s];
+        if (CH) pt = ts.ptype[s];
+        t.x = {xy.x, xy.y, zu.x};
+        t.u = {zu.y, uu.x, uu.y};
+        t.E = Et.x;
+        t.tid = tid_of(Et);
+        t.prim = (uint32_t)id.x;
+        t.step = (uint32_t)id.y;
+        t.vol = id.z;
+        t.surf = -1;
+        vol0 = t.vol;
+        step0 = t.step;
+        step_interact<CH>(P, seed, pt, t, o, slot_proc<POOL>(k));
+    }
+    return epilogue<POOL, kWrU | kWrE, false>(P, w, seed, tally, i, s, pt, active, false, -1, t, o, vol0, step0);
+}
+
+// Phase B: the interactors.  Persistent warps pull 32-entry groups of the pool's process lists; a warp runs ONE
+// interactor on (up to) 32 tracks that all selected it.
+template <int POOL>
+__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_B) k_b(const __grid_constant__ Params P, const __grid_constant__ Work w,
+                                                                uint64_t seed, double *tally) {
+    Ctl *c = w.ctl;
+    const int lane = threadIdx.x & 31;
+    constexpr int nk = (POOL == kPoolCharged) ? 4 : 3;
     // order in which the lists are worked off.  The stacks are LIFO, so what is pushed LAST is refilled
     // first: photons run pair production first (its leptons are the most energetic secondaries and go to the
-    // bottom of this iteration's records) and photoelectric absorption last.  Keeping low-energy tracks on top
-    // is what keeps the queue short ("preferentially selecting lower-energy particles").
-    const int ord0 = (PT == kGamma) ? 2 : 0, ord1 = (PT == kGamma) ? 0 : 1, ord2 = (PT == kGamma) ? 1 : 2;
-    int n[3], cb[4];
+    // bottom of this iteration's records) and photoelectric absorption last; e+- run bremsstrahlung and
+    // annihilation before the knock-on electrons.  Keeping low-energy tracks on top is what keeps the queue
+    // short ("preferentially selecting lower-energy particles").
+    const int ord[4] = {POOL == kPoolGamma ? 2 : 2, POOL == kPoolGamma ? 0 : 3, POOL == kPoolGamma ? 1 : 0, 1};
+    int n[4], cb[5];
     cb[0] = 0;
-    const unsigned long long packed = c->icount64[PT];
-    n[0] = (int)((packed >> (21 * ord0)) & 0x1fffffull);
-    n[1] = (int)((packed >> (21 * ord1)) & 0x1fffffull);
-    n[2] = ord2 < nk ? (int)((packed >> (21 * ord2)) & 0x1fffffull) : 0;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) cb[k + 1] = cb[k] + ((n[k] + 31) >> 5);
-    const int total = cb[3];
-    EMX_TL(w, 6 + PT, 0, 1);
+    for (int k = 0; k < 4; ++k) {
+        n[k] = k < nk ? c->icount[POOL][ord[k]] : 0;
+        cb[k + 1] = cb[k] + ((n[k] + 31) >> 5);
+    }
+    const int total = cb[4];
+    EMX_TL(w, 5 + POOL, 0, 1);
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
     int k_next = 0;
-    if (lane == 0 && total > 0) k_next = atomicAdd(&c->work_ctrB[PT], 1);
+    if (lane == 0 && total > 0) k_next = atomicAdd(&c->work_b[POOL], 1);
     for (;;) {
         const int ch = __shfl_sync(0xffffffffu, k_next, 0);
         if (ch >= total) break;
-        if (lane == 0) k_next = atomicAdd(&c->work_ctrB[PT], 1);
+        if (lane == 0) k_next = atomicAdd(&c->work_b[POOL], 1);
         // one call site: the interactor code exists once per kernel
-        const int sel = ch < cb[1] ? 0 : (ch < cb[2] ? 1 : 2);
-        const int kk = sel == 0 ? ord0 : (sel == 1 ? ord1 : ord2);
-        const WarpAcc d = interact_chunk<PT>(P, w, seed, tally, kk, (ch - cb[sel]) << 5, n[sel]);
+        const int sel = ch < cb[1] ? 0 : (ch < cb[2] ? 1 : (ch < cb[3] ? 2 : 3));
+        const WarpAcc d = b_group<POOL>(P, w, seed, tally, ord[sel], (ch - cb[sel]) << 5, n[sel]);
         acc.n += d.n;
         acc.d += d.d;
     }
-    if (acc.n) {
-        unsigned long long *dst = lane < 8    ? &c->inter[lane]
-                                  : lane == 8 ? &c->null_int
-                                  : lane < 12 ? &c->tracks[lane - 9]
-                                  : lane < 15 ? &c->steps[lane - 12]
-                                  : lane == 15 ? &c->progress
-                                               : &c->stalls;
-        if (lane <= 16) atomicAdd(dst, acc.n);
-        if (lane == 17) atomicAdd(&c->lanes[1][PT], acc.n);
-    }
-    EMX_TL(w, 6 + PT, 1, 1);
-    if (acc.d != 0.0 && lane < 4) {
-        double *dst = lane == 0 ? &c->escaped : lane == 1 ? &c->below_cut : lane == 2 ? &c->looper : &c->edep_total;
-        atomicAdd(dst, acc.d);
-    }
+    flush_acc(c, acc, lane, &c->lanes[3][POOL]);
+    EMX_TL(w, 5 + POOL, 1, 1);
 }
 
 #ifdef EMX_TIMELINE
@@ -1001,22 +1173,12 @@ extern "C" int emx_debug_timeline(unsigned long long *host, int clear) {
 }
 #endif
 
-// phase A of a charged pool: the instantiation for the kind of field set on the problem, with or without the
-// condensed-history extensions (multiple scattering, energy-loss fluctuations)
-template <int PT>
-static void launch_phase_a(const Params &P, const Work &w, uint64_t seed, double *tally, int g, cudaStream_t st) {
-    if (!P.ph.msc && !P.ph.fluct) {
-        if (P.field_kind == 0) k_step_pool<PT, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-        else k_step_pool<PT, true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-    } else {
-        if (P.field_kind == 0) k_step_pool<PT, false, true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-        else k_step_pool<PT, true, true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-    }
-}
+// ------------------------------------------------------------------------------------------------
+// launchers
 
 cudaError_t launch_refill(const Work &w, const Primaries &pr, cudaStream_t st) {
     k_plan<<<1, kPlanThreads, 0, st>>>(w, pr);
-    const dim3 g3(kRefillBlocks, 3);
+    const dim3 g3(kRefillBlocks, kPools);
     k_fill<<<g3, kChunk, 0, st>>>(w, nullptr);
     k_move<<<g3, kChunk, 0, st>>>(w, nullptr);
     return cudaGetLastError();
@@ -1031,99 +1193,143 @@ cudaError_t launch_loop_condition(const Work &w, unsigned long long handle, cuda
     return cudaGetLastError();
 }
 
-cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
-                             cudaStream_t st);
+static bool ext_on(const Params &P) { return P.ph.msc || P.ph.fluct; }
 
-// blocks of a pool's persistent step kernels: warps_per_sm warps per SM, which pull chunks until the pool is done
-static int step_grid(const Work &w, int pt, int n_sm) {
-    return n_sm * (w.warps_per_sm[pt] > 0 ? w.warps_per_sm[pt] : kStepWarpsPerSM) * 32 / kStepBlock;
-}
-
-cudaError_t launch_step(const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm, cudaStream_t st) {
-    for (int pt = 2; pt >= 0; --pt) {
-        const cudaError_t e = launch_step_pool(pt, P, w, seed, tally, n_sm, st);
-        if (e != cudaSuccess) return e;
+// the kernels of one pool's chain, one by one (kStage*: emx_kernels.h)
+cudaError_t launch_stage(int stage, const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st) {
+    const int g = w.grid[stage];
+    const bool ext = ext_on(P);
+    switch (stage) {
+    case kStageAGamma:
+        k_a<kPoolGamma, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        break;
+    case kStageACharged:  // no field: limits + straight move + finish
+        if (ext) k_a<kPoolCharged, true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        else k_a<kPoolCharged, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        break;
+    case kStageA0:
+        if (ext) k_a0<true><<<g, kStepBlock, 0, st>>>(P, w, seed);
+        else k_a0<false><<<g, kStepBlock, 0, st>>>(P, w, seed);
+        break;
+    case kStageField: {
+        const int ax = P.field_kind == 0 ? field_axis(P.Bhat) : kAxisAny;
+        if (P.field_kind != 0) k_field<true, kAxisAny><<<g, kStepBlock, 0, st>>>(P, w);
+        else if (ax == 0) k_field<false, 0><<<g, kStepBlock, 0, st>>>(P, w);
+        else if (ax == 1) k_field<false, 1><<<g, kStepBlock, 0, st>>>(P, w);
+        else if (ax == 2) k_field<false, 2><<<g, kStepBlock, 0, st>>>(P, w);
+        else k_field<false, kAxisAny><<<g, kStepBlock, 0, st>>>(P, w);
+        break;
+    }
+    case kStageA2:
+        if (ext) k_a2<true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        else k_a2<false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        break;
+    case kStageBGamma:
+        k_b<kPoolGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        break;
+    case kStageBCharged:
+        k_b<kPoolCharged><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        break;
+    default:
+        return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
 }
 
-// one phase of one pool (profiling path: every kernel bracketed by events)
-cudaError_t launch_phase(int pt, int phase, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
-                         cudaStream_t st) {
-    const int g = step_grid(w, pt, n_sm);
-    if (phase == 0) {
-        if (pt == kGamma) k_step_pool<kGamma, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-        else if (pt == kElectron) launch_phase_a<kElectron>(P, w, seed, tally, g, st);
-        else launch_phase_a<kPositron>(P, w, seed, tally, g, st);
+// the step kernels of one pool on its stream (fork / join branches of the iteration graph)
+cudaError_t launch_step_pool(int pool, const Params &P, const Work &w, uint64_t seed, double *tally, cudaStream_t st) {
+    cudaError_t e = cudaSuccess;
+    if (pool == kPoolGamma) {
+        e = launch_stage(kStageAGamma, P, w, seed, tally, st);
+        if (e == cudaSuccess) e = launch_stage(kStageBGamma, P, w, seed, tally, st);
     } else {
-        if (pt == kGamma) k_interact<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-        else if (pt == kElectron) k_interact<kElectron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-        else k_interact<kPositron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        if (P.Bmag == 0.0) {
+            e = launch_stage(kStageACharged, P, w, seed, tally, st);
+        } else {
+            e = launch_stage(kStageA0, P, w, seed, tally, st);
+            if (e == cudaSuccess) e = launch_stage(kStageField, P, w, seed, tally, st);
+            if (e == cudaSuccess) e = launch_stage(kStageA2, P, w, seed, tally, st);
+        }
+        if (e == cudaSuccess) e = launch_stage(kStageBCharged, P, w, seed, tally, st);
     }
-    return cudaGetLastError();
+    return e;
 }
 
-// the step kernels of one pool on its own stream (fork / join branches of the iteration graph)
-cudaError_t launch_step_pool(int pt, const Params &P, const Work &w, uint64_t seed, double *tally, int n_sm,
-                             cudaStream_t st) {
-    // persistent single-warp blocks per SM for this pool: the three pools' kernels run side by side, so each
-    // gets a share of the 16 warps per SM that fit
-    const int g = step_grid(w, pt, n_sm);
-    if (pt == kGamma) {
-        k_step_pool<kGamma, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-        k_interact<kGamma><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-    } else if (pt == kElectron) {
-        launch_phase_a<kElectron>(P, w, seed, tally, g, st);
-        k_interact<kElectron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-    } else {
-        launch_phase_a<kPositron>(P, w, seed, tally, g, st);
-        k_interact<kPositron><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+// registers per thread of the step kernels as compiled (for sizing the persistent grids)
+cudaError_t step_kernel_regs(int stage, bool field, int *regs) {
+    cudaFuncAttributes a;
+    cudaError_t e;
+    switch (stage) {
+    case kStageAGamma: e = cudaFuncGetAttributes(&a, k_a<kPoolGamma, false>); break;
+    case kStageACharged: e = cudaFuncGetAttributes(&a, k_a<kPoolCharged, false>); break;
+    case kStageA0: e = cudaFuncGetAttributes(&a, k_a0<false>); break;
+    case kStageField: e = cudaFuncGetAttributes(&a, k_field<false, 2>); break;
+    case kStageA2: e = cudaFuncGetAttributes(&a, k_a2<false>); break;
+    case kStageBGamma: e = cudaFuncGetAttributes(&a, k_b<kPoolGamma>); break;
+    default: e = cudaFuncGetAttributes(&a, k_b<kPoolCharged>); break;
     }
-    return cudaGetLastError();
+    (void)field;
+    if (e == cudaSuccess) *regs = a.numRegs;
+    return e;
 }
 
 // ------------------------------------------------------------------------------------------------
 // level-1 hook: the refill index logic (k_plan, k_fill, k_move) on a caller-supplied alive[] array
 __global__ void k_hook_init(Work w, int n_live, int n_queue) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid == 0) {
         Ctl z = Ctl();
         z.n_live[0] = n_live;
         z.q_top[0] = n_queue;
+        z.owned[0] = w.n_chunks;  // the one pool of the hook owns every chunk, in order
         *w.ctl = z;
+    }
+    for (int k = tid; k < w.n_chunks; k += gridDim.x * blockDim.x) {
+        w.ctab[0][k] = k;
+        w.ctab[1][k] = 0;
     }
 }
 __global__ void __launch_bounds__(kChunk) k_count_dead(Work w, int n_live) {
     const int i = blockIdx.x * kChunk + threadIdx.x;
-    const int n = __syncthreads_count(i < n_live && w.trk[0].alive[i] == 0);
+    const int n = __syncthreads_count(i < n_live && w.st.alive[i] == 0);
     if (threadIdx.x == 0) w.chunk_dead[0][blockIdx.x] = n;
 }
 
 size_t refill_plan_scratch_ints(long capacity) {
     const size_t nch = (size_t)(capacity + kChunk - 1) / kChunk + 1;
-    return 2 * nch + (size_t)capacity + (sizeof(Ctl) + 3) / 4 + 64 + ((size_t)capacity + 3) / 4 + 64;
+    return 6 * nch + (size_t)capacity + (sizeof(Ctl) + 3) / 4 + 64 + (nch * kChunk + 3) / 4 + 64;
 }
 
 cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
-                               int *scratch, cudaStream_t st) {
+                               int *scratch, const Ctl **ctl_out, cudaStream_t st) {
     const size_t nch = (size_t)(capacity + kChunk - 1) / kChunk + 1;
     Work w = Work();
     int *p = scratch;
     w.chunk_dead[0] = p; p += nch;
     w.chunk_off[0] = p; p += nch;
+    w.chunk_dead[1] = w.chunk_dead[0];  // the second pool of the hook is empty
+    w.chunk_off[1] = w.chunk_off[0];
+    w.ctab[0] = p; p += nch;
+    w.ctab[1] = p; p += nch;
+    w.free_list = p; p += 2 * nch;
     w.hole_idx[0] = p; p += capacity;
+    w.hole_idx[1] = w.hole_idx[0];
     p += (16 - ((uintptr_t)p / 4) % 16) % 16;  // 64-byte alignment for the control block
     w.ctl = (Ctl *)p; p += (sizeof(Ctl) + 3) / 4;
-    w.trk[0].alive = (uint8_t *)p;
-    w.cap[0] = (int)capacity;
-    w.cap[1] = w.cap[2] = 0;
-    w.qcap[0] = w.qcap[1] = w.qcap[2] = 0x7fffffff;
+    *ctl_out = w.ctl;
+    w.st.alive = (uint8_t *)p;
+    w.n_chunks = (int)((capacity + kChunk - 1) / kChunk);
+    w.slot_cap = (int)capacity;
+    w.pool_reserve = 0;
+    w.qcap[0] = w.qcap[1] = 0x7fffffff;
     w.log = nullptr;
     w.max_log = 0;
     w.n_primaries = 0;
-    cudaMemsetAsync(w.trk[0].alive, 0, (size_t)capacity, st);
-    if (n_live > 0) cudaMemcpyAsync(w.trk[0].alive, alive, (size_t)n_live, cudaMemcpyDeviceToDevice, st);
+    cudaMemsetAsync(w.st.alive, 0, nch * kChunk, st);
+    if (n_live > 0) cudaMemcpyAsync(w.st.alive, alive, (size_t)n_live, cudaMemcpyDeviceToDevice, st);
     cudaMemsetAsync(src, 0xFF, (size_t)capacity * sizeof(int32_t), st);
-    k_hook_init<<<1, 32, 0, st>>>(w, (int)n_live, (int)n_queue);
+    cudaMemsetAsync(w.chunk_dead[0], 0, 2 * nch * sizeof(int), st);
+    k_hook_init<<<8, 256, 0, st>>>(w, (int)n_live, (int)n_queue);
     const unsigned g = (unsigned)((n_live + kChunk - 1) / kChunk);
     if (g) k_count_dead<<<g, kChunk, 0, st>>>(w, (int)n_live);
     Primaries none = Primaries();

@@ -2,36 +2,55 @@
 // params/state split), the secondary stacks ("stack allocator", PAPER.md:204
 // "track initializers"), and the loop's control block.  DESIGN.md section 5.
 //
-// The store is split into one POOL per particle type (gamma, e-, e+): a track never changes type, so each
-// pool is stepped by a kernel instantiated for that type -- particle type is the coarsest "next action"
-// and partitioning by it removes the largest source of warp divergence.  Inside a pool the live tracks
-// always occupy the dense prefix [0, n_live): the refill pass fills holes from the pool's LIFO stack and,
-// when the stack runs dry, from the tail of the pool, so every field access is a coalesced 8-byte stream.
+// Two POOLS share one physical store: photons, and e- / e+ ("charged": the two differ in the sign of the
+// curvature, in which tables they read and in the rest-mass bookkeeping, not in the shape of their step).  A
+// track never changes pool, so each pool is stepped by kernels instantiated for it -- the pool is the coarsest
+// "next action", and partitioning by it removes the largest source of warp divergence.  The store is cut into
+// chunks of 128 slots; a pool OWNS a set of chunks through its chunk table (pool-local chunk -> physical chunk)
+// and k_plan moves free chunks to the pool that needs them, so the split of the slots follows the live mix of
+// the workload by itself.  In pool-local numbering the live tracks always occupy the dense prefix [0, n_live):
+// the refill fills holes from the pool's LIFO stack and, when the stack runs dry, from the tail of the pool, so
+// every access of a warp is a coalesced 16-byte-per-lane stream inside one chunk.
 #pragma once
+#include <cuda_runtime.h>
 #include "emx_core.h"
 
 namespace emx {
 
-constexpr int kChunk = 128;  // slots per thread block of the step / refill kernels
+constexpr int kChunk = 128;  // slots per chunk (and per thread block of the refill kernels)
+constexpr int kPools = 2;
+enum : int { kPoolGamma = 0, kPoolCharged = 1 };
+EMX_HD int pool_of(int ptype) { return ptype == kGamma ? kPoolGamma : kPoolCharged; }
 
-struct TrackSoA {
-    double *x, *y, *z, *ux, *uy, *uz, *E;
-    uint64_t *tid;
-    uint32_t *prim, *step;
-    int *vol, *surf;
-    uint8_t *alive;
-    uint8_t *pend;  // 0, or 1 + process id of the interaction selected by phase A and not yet run
-    // field propagation in progress (charged pools only; null for gamma): arc length done, trial step,
-    // substep attempts used (0 = none in progress)
-    double *fs_s, *fs_h;
-    int *fs_a;
+// where a live track is in its step
+enum : int {
+    kStFresh = 0,   // needs limits (stage a0)
+    kStReady = 1,   // limits known, move not started (charged pool in a field)
+    kStParked = 2,  // field propagation in progress
+    kStMoved = 3,   // move done, needs stage a2
+    kStPend = 8     // + process id: interaction selected, waits for the interactor (or stalled on a full stack)
 };
 
-struct QueueSoA {  // secondary / primary initializer records (76 B per record)
-    double *x, *y, *z, *ux, *uy, *uz, *E;
-    uint64_t *tid;
-    uint32_t *prim;
-    int *vol, *surf;
+// Track store, indexed by PHYSICAL slot.  Fields that are read and written together share a 16-byte word, so a
+// lane moves its slot with five vector accesses: (x, y), (z, ux), (uy, uz), (E, track id), (prim, step, vol, surf).
+struct Store {
+    double2 *xy, *zu, *uu;
+    double2 *Et;  // .x = E (MeV), .y = the 64 bits of the track id
+    int4 *id;     // .x prim, .y step, .z vol, .w surf
+    uint8_t *alive;  // 0 dead, 1 alive, 2 filled / moved in this refill pass
+    uint8_t *stage;  // kSt*
+    uint8_t *ptype;  // charged pool: kElectron / kPositron
+    uint8_t *act;    // EMX_A_* of the current step (from stage a0, overridden by the move), or kActCut
+    // the move of the current step: step limit of the physics; arc length done (after the move: path travelled);
+    // trial step of the propagation; substep attempts used (after the move: surface hit, -1 none)
+    double *s_phys, *s_done, *h_try;
+    int *att;
+};
+
+// secondary / primary initializer record (80 bytes): same packing, .id = (prim, vol, surf, ptype)
+struct Stack {
+    double2 *xy, *zu, *uu, *Et;
+    int4 *id;
 };
 
 struct PoolPlan {
@@ -44,38 +63,47 @@ struct PoolPlan {
     int q_old, q_new;
 };
 
+constexpr int kMaxLists = 4;  // interaction lists per pool: gamma Compton / photo / pair; charged Moller / Bhabha / brems / annihilation
+
 struct Ctl {
-    int n_live[3];
-    int q_top[3];
-    int m_step[3];  // tracks to step this iteration (= n_live)
-    int q_safe[3];  // set by k_plan: stack p cannot overflow in this iteration whatever the step kernels push
-    PoolPlan plan[3];
+    int n_live[kPools];
+    int q_top[kPools];
+    int m_step[kPools];  // tracks to step this iteration (= n_live)
+    int q_safe[kPools];  // set by k_plan: stack p cannot overflow in this iteration whatever the step kernels push
+    PoolPlan plan[kPools];
+    int owned[kPools];   // chunks in each pool's chunk table
+    int n_free;          // chunks on the free list
     int done, error, had_live;
-    int idle_iters;  // consecutive iterations without progress although tracks are live (R7)
-    int work_ctr3[3];  // next 32-slot chunk of each pool's step kernel (phase A)
-    int work_ctrB[3];  // next 32-entry chunk of each pool's interaction lists (phase B)
-    unsigned long long icount64[3];  // entries in the interaction lists of each pool, 3 x 21 bits packed
-    int field_budget;  // substep attempts per track and iteration (time slicing of the field propagation)
+    int idle_iters;      // consecutive iterations without progress although tracks are live (R7)
+    int work_a[kPools];  // next 32-slot group of each pool for the dense phase-A kernel (stages a0 .. a2, or a2 alone)
+    int work_0;          // ... for the limits kernel of the charged pool (field)
+    int work_f;          // next slot of the charged pool for the propagation kernel
+    int work_b[kPools];  // next 32-entry group of each pool's interaction lists (phase B)
+    int icount[kPools][kMaxLists];  // entries in the interaction lists
+    int field_min;       // substep attempts a track is given per iteration before it may be parked
     unsigned long long iter;
-    unsigned long long progress;  // steps committed + tombstones retired in the current iteration (R7)
+    unsigned long long progress;  // steps committed + propagations advanced in the current iteration (R7)
     long long next_primary;       // primaries [0, next_primary) have been admitted
     double E_admitted;            // energy of the admitted primaries (e+ with their 2 me)
     double edep_total;            // all energy deposited so far (every cell, tallied or not)
     double escaped, below_cut, looper, E_in;
     unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls, peak_live, peak_queue;
-    unsigned long long lanes[2][3];  // track slots processed by phase A / phase B kernels, per pool
+    unsigned long long lanes[4][kPools];  // slots processed by the kernels a0 / field / a (or a2) / b, per pool
+    unsigned long long attempts;          // substep attempts of the field propagation
     unsigned long long hist[3][EMX_NHIST];  // tracks by type and by the bin of the steps they took
 };
 
 struct Work {
-    TrackSoA trk[3];
-    QueueSoA q[3];
-    int cap[3];   // slots per pool
-    int qcap[3];  // records per stack
-    int *chunk_dead[3];
-    int *chunk_off[3];
-    int *hole_idx[3];
-    int *ilist[3][3];  // slots waiting for an interactor, [pool][process slot], capacity cap[pool] each
+    Store st;
+    Stack q[kPools];
+    int n_chunks;         // physical chunks of the store
+    int qcap[kPools];     // records per stack
+    int *ctab[kPools];    // chunk tables, n_chunks entries each
+    int *free_list;       // n_chunks entries
+    int *chunk_dead[kPools];  // per pool-local chunk: slots that died in the last iteration
+    int *chunk_off[kPools];   // ... exclusive prefix sum of it
+    int *hole_idx[kPools];
+    int *ilist[kPools][kMaxLists];  // pool-local slots waiting for an interactor, n_slots entries each
     Ctl *ctl;
     uint32_t *log;  // per iteration: live, queued
     int max_log;
@@ -84,14 +112,22 @@ struct Work {
     long long n_primaries;
     int wave;
     double inflight_cap;
-    size_t hot_bytes;       // leading part of the workspace that holds the track store, scan arrays and lists
-    int warps_per_sm[3];    // persistent step-kernel warps per SM, per pool
     long long slice_above;  // live tracks above which the field propagation is time-sliced
-    int slice_budget;       // substep attempts per track and iteration while sliced
+    int slice_min;          // substep attempts per track and iteration before parking while sliced
+    int slice_max;          // ... after which a track is parked even if the pool still has work
+    int grid[8];            // blocks of the persistent step kernels, by stage (emx_kernels.h: kStage*)
+    int reserve_slack;      // records all resident warps can request at the same time (see reserve())
+    int slot_cap;           // slots a pool may hold at most (= n_chunks * kChunk; smaller in the refill hook)
+    int pool_reserve;       // chunks a pool never takes, so that the other pool can always start (n_chunks / 32, >= 1)
 };
 
-// bytes of one slot / one record, for the workspace carve-up and the roofline arithmetic
-constexpr size_t kSlotBytes = 7 * 8 + 8 + 4 + 4 + 4 + 4 + 1;  // + 20 B in the charged pools (field progress)
-constexpr size_t kRecordBytes = 7 * 8 + 8 + 4 + 4 + 4;
+// physical slot of pool-local slot i
+__device__ __forceinline__ int phys_slot(const Work &w, int pool, int i) {
+    return (w.ctab[pool][i / kChunk] * kChunk) | (i % kChunk);
+}
+
+// bytes of one slot / one record, for the roofline arithmetic
+constexpr size_t kSlotBytes = 5 * 16 + 4;   // + 28 B of propagation state in the charged pool
+constexpr size_t kRecordBytes = 5 * 16;
 
 }  // namespace emx

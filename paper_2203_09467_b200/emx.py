@@ -12,8 +12,10 @@ import weakref
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("EMX_LIB_PATH") or os.path.join(HERE, "libemx.so")   # override: kernel experiments
+LIB_PATH = os.path.join(HERE, "libemx.so")
 MAX_ELEM, MAX_FACES, NPROC, NTABLE, NHIST = 4, 8, 8, 19, 96
+# the step kernels in the order of emx_get_profile / emx_get_lanes / emx_schedule.blocks_per_sm
+STAGES = ["k_a<gamma>", "k_a<charged>", "k_a0", "k_field", "k_a2", "k_b<gamma>", "k_b<charged>"]
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
            "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc", "var_em", "var_ep"]
 T = {n: i for i, n in enumerate(T_NAMES)}
@@ -34,6 +36,11 @@ class Scalars(C.Structure):
                 ("iterations", C.c_uint64), ("peak_live", C.c_uint64), ("peak_queue", C.c_uint64)]
 
 
+class Schedule(C.Structure):
+    _fields_ = [("loop_node", C.c_int32), ("slice_min", C.c_int32), ("slice_max", C.c_int32), ("slice_above", C.c_int64),
+                ("blocks_per_sm", C.c_int32 * 8)]
+
+
 class Track(C.Structure):
     _fields_ = [("x", C.c_double * 3), ("u", C.c_double * 3), ("E", C.c_double), ("tid", C.c_uint64),
                 ("prim", C.c_uint32), ("step", C.c_uint32), ("vol", C.c_int32), ("surf", C.c_int32),
@@ -44,13 +51,14 @@ class StepResult(C.Structure):
     _fields_ = [("trk", Track), ("action", C.c_int32), ("process", C.c_int32), ("n_sec", C.c_int32),
                 ("sec", Track * 4), ("sec_ord", C.c_int32 * 4), ("edep", C.c_double), ("edep_vol", C.c_int32),
                 ("below_cut", C.c_double), ("escaped", C.c_double), ("looper", C.c_double), ("s", C.c_double),
-                ("msc_tau", C.c_double), ("n_draws", C.c_int32), ("null_int", C.c_int32), ("rest", C.c_int32)]
+                ("msc_tau", C.c_double), ("n_draws", C.c_int32), ("null_int", C.c_int32), ("rest", C.c_int32),
+                ("n_sub", C.c_int32)]
 
 
 EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "emx_add_volume", "emx_set_field", "emx_set_field_fringe",
            "emx_get_physics", "emx_set_physics", "emx_set_cuts", "emx_build_tables", "emx_get_table",
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
-           "emx_set_primary_offset", "emx_set_pool_split", "emx_neighbour_candidates", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
+           "emx_staging_bytes", "emx_set_primary_offset", "emx_get_schedule", "emx_set_schedule", "emx_neighbour_candidates", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
            "emx_get_iteration_log", "emx_get_iteration_times",
            "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_last_error",
            "emx_version"]
@@ -81,7 +89,8 @@ def lib():
             "emx_reset_tallies": (i, [vp, vp]), "emx_read_tallies": (i, [vp, vp, C.POINTER(Scalars)]),
             "emx_last_transport_ms": (d, [vp]), "emx_get_iteration_log": (l, [vp, vp, l]),
             "emx_get_iteration_times": (l, [vp, vp, l]),
-            "emx_get_lanes": (i, [vp, vp]), "emx_read_step_hist": (i, [vp, vp]), "emx_set_primary_offset": (i, [vp, l]), "emx_set_pool_split": (i, [vp, d, d, d]), "emx_neighbour_candidates": (i, [vp, i, i, i, vp, i]),
+            "emx_get_lanes": (i, [vp, vp]), "emx_read_step_hist": (i, [vp, vp]), "emx_set_primary_offset": (i, [vp, l]), "emx_staging_bytes": (C.c_size_t, [l]),
+            "emx_get_schedule": (i, [vp, C.POINTER(Schedule)]), "emx_set_schedule": (i, [vp, C.POINTER(Schedule)]), "emx_neighbour_candidates": (i, [vp, i, i, i, vp, i]),
             "emx_set_profile": (i, [vp, i]), "emx_get_profile": (i, [vp, vp, vp, vp]),
             "emx_step_batch": (i, [vp, u64, l, vp, vp, vp]),
             "emx_philox_batch": (i, [l, vp, vp, vp, vp]),
@@ -150,8 +159,6 @@ class Problem:
             self._check(L.emx_add_volume(h, len(s), _hp(s), _hp(e), vol["material"], vol["tally"]))
         B = desc.get("field", (0.0, 0.0, 0.0))
         self._check(L.emx_set_field(h, float(B[0]), float(B[1]), float(B[2])))
-        if desc.get("pool_split") and not os.environ.get("EMX_POOL_FRAC"):      # scheduling hint of the workload
-            self._check(L.emx_set_pool_split(h, *[float(v) for v in desc["pool_split"]]))
         if desc.get("field_fringe"):
             self._check(L.emx_set_field_fringe(h, float(desc["field_fringe"][0]), float(desc["field_fringe"][1])))
         ph = Physics()
@@ -199,14 +206,16 @@ class Problem:
         self._check(lib().emx_get_material_info(self.h, material, _hp(o)))
         return dict(n_e=o[0], I=o[1], hwp=o[2], X0=o[3], Tcut=o[4], kcut=o[5], rho=o[6], n_elem=int(o[7]))
 
-    def workspace(self, n_slots, queue_capacity):
-        """A torch uint8 CUDA tensor of emx_workspace_bytes(); cached per (n_slots, queue_capacity)."""
+    def workspace(self, n_slots, queue_capacity, n_staged=0):
+        """A torch uint8 CUDA tensor of emx_workspace_bytes() (+ emx_staging_bytes(n_staged) for
+        emx_transport_host); cached per (n_slots, queue_capacity) and grown when more staging is asked for."""
         torch = _torch()
         key = (int(n_slots), int(queue_capacity))
-        if self._ws is None or self._ws[0] != key:
-            nb = lib().emx_workspace_bytes(self.h, key[0], key[1])
-            if nb == 0:
-                raise EmxError("emx_workspace_bytes: invalid sizes")
+        nb = lib().emx_workspace_bytes(self.h, key[0], key[1])
+        if nb == 0:
+            raise EmxError("emx_workspace_bytes: invalid sizes")
+        nb += lib().emx_staging_bytes(int(n_staged)) if n_staged else 0
+        if self._ws is None or self._ws[0] != key or self._ws[1].numel() < nb:
             self._ws = None
             self._ws = (key, torch.empty(nb, dtype=torch.uint8, device="cuda"))
         return self._ws[1]
@@ -237,7 +246,7 @@ class Problem:
         L = lib()
         n_slots = n_slots or self.desc["n_slots"]
         queue_capacity = queue_capacity or self.desc["queue_capacity"]
-        ws = self.workspace(n_slots, queue_capacity)
+        ws = self.workspace(n_slots, queue_capacity, n_staged=len(prim["E"]))
         st = _stream()
         if reset:
             self._check(L.emx_reset_tallies(self.h, st))
@@ -278,19 +287,34 @@ class Problem:
         self._check(lib().emx_read_step_hist(self.h, _hp(h)))
         return h
 
+    def set_schedule(self, **kw):
+        """emx_set_schedule: loop_node, slice_min, slice_max, slice_above, blocks_per_sm (dict stage name -> blocks
+        or a list of 7).  Only what is named changes.  A schedule never changes a result."""
+        sc = Schedule()
+        self._check(lib().emx_get_schedule(self.h, C.byref(sc)))
+        for k, v in kw.items():
+            if k == "blocks_per_sm":
+                items = v.items() if isinstance(v, dict) else zip(STAGES, v)
+                for name, b in items:
+                    sc.blocks_per_sm[STAGES.index(name)] = int(b)
+            else:
+                setattr(sc, k, int(v))
+        self._check(lib().emx_set_schedule(self.h, C.byref(sc)))
+
     def set_profile(self, on):
         self._check(lib().emx_set_profile(self.h, int(on)))
 
     def profile(self):
-        """dict(ms=[A gamma, A e-, A e+, B gamma, B e-, B e+, refill, all step kernels], lanes=[same six],
-        launches, iterations_launched) of the last transport"""
-        ms = (C.c_double * 8)()
+        """dict(ms = {stage: ms, "refill": ms, "all_step_kernels": ms}, lanes = {stage: slots processed},
+        attempts = substep attempts of the field propagation, launches, iterations_launched) of the last transport"""
+        ms = (C.c_double * 9)()
         nl, ni = C.c_long(), C.c_long()
         self._check(lib().emx_get_profile(self.h, C.cast(ms, C.c_void_p), C.cast(C.byref(nl), C.c_void_p),
                                           C.cast(C.byref(ni), C.c_void_p)))
-        lanes = (C.c_uint64 * 6)()
+        lanes = (C.c_uint64 * 8)()
         lib().emx_get_lanes(self.h, C.cast(lanes, C.c_void_p))
-        return dict(ms=list(ms), lanes=list(lanes), launches=nl.value, iterations_launched=ni.value)
+        return dict(ms=dict(zip(STAGES + ["refill", "all_step_kernels"], list(ms))), lanes=dict(zip(STAGES, list(lanes)[:7])),
+                    attempts=int(lanes[7]), launches=nl.value, iterations_launched=ni.value)
 
     def iteration_times(self, max_iter=1 << 16):
         """(n, 2) float32: refill ms, step-kernel ms per iteration of the last transport (profiling on)"""

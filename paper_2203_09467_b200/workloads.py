@@ -145,7 +145,7 @@ def config4(n=100000):
             vols.append(dict(surf=[i - 1, i, nc, nc + 1], sense=[1, -1, 1, -1], material=mats[i], tally=t))
     desc = dict(name="config4_barrel_stress", seed=4, materials=[SI, PBWO4, BRASS, PVT], surfaces=surfaces,
                 volumes=vols, field=(0.0, 0.0, 4.0), physics=physics(E_max=1e5),
-                n_slots=1 << 20, queue_capacity=1 << 26, pool_split=(40, 50, 10))
+                n_slots=1 << 20, queue_capacity=1 << 26)
     rng = np.random.default_rng(4)
     xi = rng.random(size=(n, 3))
     mu = 2.0 * xi[:, 0] - 1.0

@@ -98,7 +98,7 @@ def result_arrays(res):
         vol=t["vol"].copy(), surf=t["surf"].copy(), alive=t["alive"].copy(), action=a["action"].copy(),
         process=a["process"].copy(), n_sec=a["n_sec"].copy(), edep=a["edep"].copy(),
         below_cut=a["below_cut"].copy(), escaped=a["escaped"].copy(), looper=a["looper"].copy(),
-        s=a["s"].copy(), msc_tau=a["msc_tau"].copy(), n_draws=a["n_draws"].copy(), null_int=a["null_int"].copy(), rest=a["rest"].copy(),
+        s=a["s"].copy(), n_sub=a["n_sub"].copy(), msc_tau=a["msc_tau"].copy(), n_draws=a["n_draws"].copy(), null_int=a["null_int"].copy(), rest=a["rest"].copy(),
         sec_E=sec["E"].copy(), sec_u=sec["u"].copy(), sec_x=sec["x"].copy(), sec_tid=sec["tid"].copy(),
         sec_ptype=sec["ptype"].copy(), sec_ord=a["sec_ord"].copy(), sec_vol=sec["vol"].copy(),
         sec_prim=sec["prim"].copy(), sec_surf=sec["surf"].copy())

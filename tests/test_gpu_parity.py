@@ -308,13 +308,12 @@ def test_results_do_not_depend_on_slots_or_host_entry(emx):
     assert np.array_equal(a["steps"], b["steps"]) and np.array_equal(a["tracks"], b["tracks"])
     assert np.allclose(a["edep"], b["edep"], rtol=1e-11, atol=1e-9)
     assert a["iterations"] != b["iterations"] or a["peak_live"] != b["peak_live"]
-    # nor on how the slots are shared among the three pools (emx_set_pool_split)
-    G2 = emx.Problem(dict(desc, pool_split=(20, 60, 20)))
-    c = G2.transport(G2.upload_primaries(prim), desc["seed"], n_slots=1 << 12, queue_capacity=1 << 18)
+    # nor on how many slots there are for the two pools to share (256: one chunk each; the pools trade chunks)
+    c = G.transport(G.upload_primaries(prim), desc["seed"], n_slots=256, queue_capacity=1 << 18)
     assert np.array_equal(a["steps"], c["steps"]) and np.array_equal(a["tracks"], c["tracks"])
     assert np.array_equal(a["inter"], c["inter"])
     assert np.allclose(a["edep"], c["edep"], rtol=1e-11, atol=1e-9)
-    assert a["iterations"] != c["iterations"] or a["peak_live"] != c["peak_live"]
+    assert c["peak_live"] <= 256 and c["iterations"] > a["iterations"]
 
 
 def test_shards_of_the_primaries_sum_to_the_whole(emx):
@@ -410,18 +409,21 @@ def test_error_paths(emx):
     L.emx_destroy(h)
 
 
-def test_scheduling_knobs_do_not_change_results(emx, monkeypatch):
-    """Time slicing of the field propagation (substep budget per iteration) and the launch paths (the loop as
-    one graph with a WHILE node, flat iteration graphs polled by the host, plain stream launches, profiled
-    launches) only change WHEN work is done: counters are equal, tallies equal up to summation order."""
+def test_scheduling_knobs_do_not_change_results(emx):
+    """Time slicing of the field propagation (attempts per iteration before a track may be parked), the grids of
+    the persistent kernels and the launch paths (the loop as one graph with a WHILE node, flat iteration graphs
+    polled by the host, plain stream launches, profiled launches) only change WHEN work is done: counters are
+    equal, tallies equal up to summation order."""
     desc, prim = W.get(4, 64)
     runs, hists = [], []
-    for budget, mode, loop_node in (("2", 0, "1"), ("100000", 0, "1"), ("7", 2, "1"), ("2", 1, "1"), ("2", 0, "0")):
-        monkeypatch.setenv("EMX_SLICE_BUDGET", budget)
-        monkeypatch.setenv("EMX_SLICE_ABOVE", "0")
-        monkeypatch.setenv("EMX_LOOP_NODE", loop_node)      # 0: flat iteration graphs polled by the host
+    variants = (dict(slice_min=2, slice_max=16), dict(slice_min=1000, slice_max=1000), dict(slice_min=1, slice_max=1),
+                dict(slice_min=3, slice_max=7, profile=2), dict(profile=1), dict(loop_node=0),
+                dict(blocks_per_sm={"k_field": 1, "k_a2": 2, "k_b<gamma>": 1}))
+    for v in variants:
+        v = dict(v)
         G = emx.Problem(desc)
-        G.set_profile(mode)
+        G.set_profile(v.pop("profile", 0))
+        G.set_schedule(slice_above=0, **v)
         runs.append(G.transport(G.upload_primaries(prim), desc["seed"], n_slots=1 << 14, queue_capacity=1 << 20))
         hists.append(G.read_step_hist())
     assert all(np.array_equal(hists[0], h) for h in hists[1:])
@@ -432,7 +434,7 @@ def test_scheduling_knobs_do_not_change_results(emx, monkeypatch):
         assert a["null_int"] == b["null_int"]
         assert np.allclose(a["edep"], b["edep"], rtol=1e-11, atol=1e-9)
         assert b["escaped"] == pytest.approx(a["escaped"], rel=1e-11)
-    assert runs[0]["iterations"] != runs[1]["iterations"]       # the schedules did differ
+    assert runs[0]["iterations"] != runs[1]["iterations"] or runs[0]["iterations"] != runs[2]["iterations"]   # the schedules did differ
 
 
 @pytest.mark.parametrize("cfg", [4, 7])

@@ -60,18 +60,25 @@ def test_host_side_argument_checks_without_a_device(L):
     assert (ph.n_E, ph.alpha_R, ph.rho_R, ph.max_steps) == (256, 0.2, 0.1, 10000)
     ph.n_E = 1
     assert L.emx_set_physics(h, C.byref(ph)) == -1
-    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) > (1 << 20) * 85 + (1 << 26) * 76 * 0.9
-    assert L.emx_workspace_bytes(h, 0, 10) == 0
-    # pool split: shares must be positive; it moves bytes between the pools' arrays (the charged pools carry 20 B
-    # more per slot), (0, 0, 0) restores the default
-    L.emx_set_pool_split.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
-    w0 = L.emx_workspace_bytes(h, 1 << 20, 1 << 26)
-    assert L.emx_set_pool_split(h, 40.0, -1.0, 10.0) == -1 and L.emx_set_pool_split(h, 0.0, 1.0, 1.0) == -1
-    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) == w0
-    assert L.emx_set_pool_split(h, 20.0, 70.0, 10.0) == 0
-    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) > w0
-    assert L.emx_set_pool_split(h, 0.0, 0.0, 0.0) == 0
-    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) == w0
+    assert L.emx_workspace_bytes(h, 1 << 20, 1 << 26) > (1 << 20) * 84 + (1 << 26) * 80 * 0.9
+    assert L.emx_workspace_bytes(h, 0, 10) == 0 and L.emx_workspace_bytes(h, (1 << 22) + 1, 10) == 0
+    L.emx_staging_bytes.restype, L.emx_staging_bytes.argtypes = C.c_size_t, [C.c_long]
+    assert L.emx_staging_bytes(100000) >= 100000 * 68 and L.emx_staging_bytes(0) > 0
+    # the schedule: defaults, validation (it never changes a result, so there is nothing else to check without a GPU)
+    sc = emx.Schedule()
+    assert L.emx_get_schedule(h, C.byref(sc)) == 0
+    assert (sc.loop_node, sc.slice_min, sc.slice_above) == (1, 2, -1) and sc.slice_max >= sc.slice_min
+    sc.slice_min = 0
+    assert L.emx_set_schedule(h, C.byref(sc)) == -1
+    sc.slice_min, sc.slice_max = 4, 3
+    assert L.emx_set_schedule(h, C.byref(sc)) == -1
+    sc.slice_max = 8
+    sc.blocks_per_sm[3] = 17
+    assert L.emx_set_schedule(h, C.byref(sc)) == -1
+    sc.blocks_per_sm[3] = 4
+    assert L.emx_set_schedule(h, C.byref(sc)) == 0
+    sc2 = emx.Schedule()
+    assert L.emx_get_schedule(h, C.byref(sc2)) == 0 and (sc2.slice_min, sc2.slice_max, sc2.blocks_per_sm[3]) == (4, 8, 4)
     # compute calls before the tables are built are refused with EMX_E_STATE
     assert L.emx_read_tallies(h, None, None) == -2
     assert L.emx_step_batch(h, 0, 0, None, None, None) == -2
