@@ -35,10 +35,18 @@ void emo_rotate(const double u[3], double mu, double phi, double out[3]) {
 static double beta_of(double T) { return sqrt(T * (T + 2.0 * EMO_ME)) / (T + EMO_ME); }
 static double clamp1(double m) { return m > 1.0 ? 1.0 : (m < -1.0 ? -1.0 : m); }
 
-/* exact inverse CDF of p(mu) ~ (1 - beta mu)^-2 */
-static double boosted_iso(double xi, double beta) {
-    return clamp1((2.0 * xi - 1.0 + beta) / (beta * (2.0 * xi - 1.0) + 1.0));
+/* Exact inverse CDF of p(mu) ~ (1 - beta mu)^-2 (R30), returned as t = 1 - mu for a lepton of kinetic energy T:
+ * mu = (v + beta) / (beta v + 1), v = 2 xi - 1, gives 1 - mu = (1 - beta)(1 - v) / (1 + beta v).  With
+ * 1 - beta = 1 / (gamma^2 (1 + beta)) and 1 + beta v = (1 - beta) + 2 beta xi nothing cancels: the emission angle,
+ * which is ~1/gamma, keeps full relative precision at every energy (forming 1 - mu from a
+ * rounded mu loses a factor gamma^2). */
+static double boosted_iso_t(double xi, double T) {
+    double g = T / EMO_ME + 1.0, b = beta_of(T);
+    double omb = 1.0 / (g * g * (1.0 + b));
+    double t = 2.0 * omb * (1.0 - xi) / (omb + 2.0 * b * xi);
+    return t < 0.0 ? 0.0 : (t > 2.0 ? 2.0 : t);
 }
+static double sin_of_t(double t) { double s2 = t * (2.0 - t); return s2 > 0.0 ? sqrt(s2) : 0.0; }
 
 /* ---- Compton (Klein-Nishina) ---- */
 void emo_compton(emo_rng *r, double E, const double u[3], double *E1, double u1[3], double *Te, double ue[3]) {
@@ -60,8 +68,9 @@ void emo_compton(emo_rng *r, double E, const double u[3], double *E1, double u1[
     rotate_cs(u, mu, s, cos(phi), sin(phi), u1);
     *E1 = eps * E;
     *Te = E - *E1;
-    for (int i = 0; i < 3; ++i) ue[i] = E * u[i] - (*E1) * u1[i];
-    normalise(ue, u);
+    /* momentum balance E u = E1 u1 + p_e u_e with u1 = mu u + s e: p_e u_e = (E - E1 mu) u - E1 s e, and
+     * E - E1 mu = Te + E1 t carries no cancellation */
+    rotate_cs(u, *Te + (*E1) * t, -(*E1) * s, cos(phi), sin(phi), ue);
 }
 
 /* ---- photoelectron direction: p(mu) ~ (1-mu^2)/(1-beta mu)^4 (Sauter, leading term) ---- */
@@ -118,12 +127,12 @@ int emo_pair(emo_rng *r, int Z, double E, const double u[3], double *Tm, double 
     double tp = E - tm - 2.0 * EMO_ME;
     if (tp < 0.0) tp = 0.0;
     *Tm = tm; *Tp = tp;
-    double mum = boosted_iso(emo_next(r), beta_of(tm));
-    double mup = boosted_iso(emo_next(r), beta_of(tp));
+    double t_m = boosted_iso_t(emo_next(r), tm);
+    double t_p = boosted_iso_t(emo_next(r), tp);
     double phi = 2.0 * EMO_PI * emo_next(r);
     double cp = cos(phi), sp = sin(phi);
-    rotate_cs(u, mum, sqrt((1.0 - mum) * (1.0 + mum)), cp, sp, um);
-    rotate_cs(u, mup, sqrt((1.0 - mup) * (1.0 + mup)), -cp, -sp, up);
+    rotate_cs(u, 1.0 - t_m, sin_of_t(t_m), cp, sp, um);
+    rotate_cs(u, 1.0 - t_p, sin_of_t(t_p), -cp, -sp, up);
     return 1;
 }
 
@@ -138,13 +147,15 @@ int emo_brems(emo_rng *r, double T, double kc, const double u[3], double *k, dou
         double y = kk / T;
         if ((4.0 / 3.0) * x2 <= 4.0 / 3.0 - 4.0 * y / 3.0 + y * y) break;
     }
-    double mu = boosted_iso(emo_next(r), beta_of(T));
+    double t = boosted_iso_t(emo_next(r), T), sn = sin_of_t(t);
     double phi = 2.0 * EMO_PI * emo_next(r);
-    rotate_cs(u, mu, sqrt((1.0 - mu) * (1.0 + mu)), cos(phi), sin(phi), ug);
+    double cp = cos(phi), sp = sin(phi);
+    rotate_cs(u, 1.0 - t, sn, cp, sp, ug);
     double p = sqrt(T * (T + 2.0 * EMO_ME));
     *k = kk; *T1 = T - kk;
-    for (int i = 0; i < 3; ++i) u1[i] = p * u[i] - kk * ug[i];
-    normalise(u1, u);
+    /* recoil p u - k u_gamma = (p - k mu) u - k s e, with p - k mu = (p - T) + T1 + k t and
+     * p - T = 2 me T / (p + T): no difference of nearly equal numbers */
+    rotate_cs(u, 2.0 * EMO_ME * T / (p + T) + *T1 + kk * t, -kk * sn, cp, sp, u1);
     return 1;
 }
 
@@ -152,11 +163,15 @@ int emo_brems(emo_rng *r, double T, double kc, const double u[3], double *k, dou
 static void knock_on(emo_rng *r, double T, double Td, const double u[3], double ud[3], double *T1, double u1[3]) {
     double p = sqrt(T * (T + 2.0 * EMO_ME)), pd = sqrt(Td * (Td + 2.0 * EMO_ME));
     double mu = clamp1(Td * (T + 2.0 * EMO_ME) / (p * pd));
+    /* sin^2 = 1 - mu^2 = 2 me (T - Td) / (T (Td + 2 me)) in closed form */
+    double s2 = 2.0 * EMO_ME * (T - Td) / (T * (Td + 2.0 * EMO_ME));
+    double sn = s2 > 0.0 ? sqrt(s2) : 0.0;
     double phi = 2.0 * EMO_PI * emo_next(r);
-    rotate_cs(u, mu, sqrt((1.0 - mu) * (1.0 + mu)), cos(phi), sin(phi), ud);
+    double cp = cos(phi), sp = sin(phi);
+    rotate_cs(u, mu, sn, cp, sp, ud);
     *T1 = T - Td;
-    for (int i = 0; i < 3; ++i) u1[i] = p * u[i] - pd * ud[i];
-    normalise(u1, u);
+    /* primary: p u - pd u_delta = (p - pd mu) u - pd s e, p - pd mu = (T - Td)(T + 2 me) / p */
+    rotate_cs(u, (*T1) * (T + 2.0 * EMO_ME) / p, -pd * sn, cp, sp, u1);
 }
 
 /* ---- Moller ---- */
@@ -207,20 +222,25 @@ void emo_annih_flight(emo_rng *r, double T, const double u[3], double *k1, doubl
     }
     double Etot = T + 2.0 * EMO_ME;
     double kk = eps * Etot;
-    double mu = clamp1((eps * (g + 1.0) - 1.0) / (eps * sqrt(g * g - 1.0)));
+    double pg = sqrt(g * g - 1.0);                                  /* p / me */
+    double mu = clamp1((eps * (g + 1.0) - 1.0) / (eps * pg));
+    /* sin^2 = 1 - mu^2 = (2 (g + 1) eps (1 - eps) - 1) / (eps^2 (g^2 - 1)) in closed form */
+    double s2 = (2.0 * (g + 1.0) * eps * (1.0 - eps) - 1.0) / (eps * eps * (g * g - 1.0));
+    double sn = s2 > 0.0 ? sqrt(s2) : 0.0;
     double phi = 2.0 * EMO_PI * emo_next(r);
-    rotate_cs(u, mu, sqrt((1.0 - mu) * (1.0 + mu)), cos(phi), sin(phi), u1);
-    double p = sqrt(T * (T + 2.0 * EMO_ME));
+    double cp = cos(phi), sp = sin(phi);
+    rotate_cs(u, mu, sn, cp, sp, u1);
     *k1 = kk; *k2 = Etot - kk;
-    for (int i = 0; i < 3; ++i) u2[i] = p * u[i] - kk * u1[i];
-    normalise(u2, u);
+    /* second photon: p u - k1 u1 = (p - k1 mu) u - k1 s e, p - k1 mu = me (g + 1) ((1 - eps)(g + 1) - 1) / sqrt(g^2 - 1) */
+    rotate_cs(u, EMO_ME * (g + 1.0) * ((1.0 - eps) * (g + 1.0) - 1.0) / pg, -kk * sn, cp, sp, u2);
 }
 
 /* ---- annihilation at rest: two back-to-back me photons, isotropic ---- */
 void emo_annih_rest(emo_rng *r, double u1[3], double u2[3]) {
-    double mu = 2.0 * emo_next(r) - 1.0;
+    double xi = emo_next(r);
+    double mu = 2.0 * xi - 1.0;
     double phi = 2.0 * EMO_PI * emo_next(r);
-    double s = sqrt((1.0 - mu) * (1.0 + mu));
+    double s = 2.0 * sqrt(xi * (1.0 - xi));                        /* sqrt((1 - mu)(1 + mu)) without the cancellation */
     u1[0] = s * cos(phi); u1[1] = s * sin(phi); u1[2] = mu;
     u2[0] = -u1[0]; u2[1] = -u1[1]; u2[2] = -u1[2];
 }
