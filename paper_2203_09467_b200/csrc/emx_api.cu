@@ -134,7 +134,9 @@ size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
     t.alive = c.take<uint8_t>(n); t.stage = c.take<uint8_t>(n); t.ptype = c.take<uint8_t>(n); t.act = c.take<uint8_t>(n);
     t.s_phys = c.take<double>(n); t.s_done = c.take<double>(n); t.h_try = c.take<double>(n);
     t.att = c.take<int>(n);
+    t.kap = c.take<double>(n);
     w.free_list = c.take<int>((size_t)nch);
+    w.rtab = c.take<int>((size_t)nch);
     for (int p = 0; p < kPools; ++p) {
         w.ctab[p] = c.take<int>((size_t)nch);
         w.chunk_dead[p] = c.take<int>((size_t)nch + 1);

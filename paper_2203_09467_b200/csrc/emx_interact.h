@@ -46,8 +46,20 @@ EMX_HD Vec3 rotate_mu_phi(const Vec3 &u, double mu, double phi) {
 
 EMX_HD double beta_of(double T) { return sqrt(T * (T + 2.0 * kMe)) / (T + kMe); }
 EMX_HD double clamp1(double m) { return m > 1.0 ? 1.0 : (m < -1.0 ? -1.0 : m); }
-// exact inverse CDF of p(mu) ~ (1 - beta mu)^-2 (R30)
-EMX_HD double boosted_iso(double xi, double beta) { return clamp1((2.0 * xi - 1.0 + beta) / (beta * (2.0 * xi - 1.0) + 1.0)); }
+// Exact inverse CDF of p(mu) ~ (1 - beta mu)^-2 (R30) for a lepton of kinetic energy T, as t = 1 - mu:
+// mu = (v + beta) / (beta v + 1), v = 2 xi - 1  =>  t = (1 - beta)(1 - v) / (1 + beta v)
+//    = 2 (1 - beta)(1 - xi) / ((1 - beta) + 2 beta xi),  1 - beta = 1 / (gamma^2 (1 + beta)).
+// Nothing cancels, so the emission angle (~1/gamma) keeps its relative precision at every energy.
+EMX_HD double boosted_iso_t(double xi, double T) {
+    const double g = T / kMe + 1.0, b = beta_of(T);
+    const double omb = 1.0 / (g * g * (1.0 + b));
+    const double t = 2.0 * omb * (1.0 - xi) / (omb + 2.0 * b * xi);
+    return t < 0.0 ? 0.0 : (t > 2.0 ? 2.0 : t);
+}
+EMX_HD double sin_of_t(double t) {
+    const double s2 = t * (2.0 - t);
+    return s2 > 0.0 ? sqrt(s2) : 0.0;
+}
 
 // ---- fluctuated continuous loss of a step (R-FLUCT): normal about the mean dE with variance V (Box-Muller:
 // z = sqrt(-2 ln xi1) cos(2 pi xi2)), clamped to [0, min(2 dE, E)]
@@ -100,8 +112,9 @@ EMX_NI void compton(Rng &r, double E, const Vec3 &u, double &E1, Vec3 &u1, doubl
     u1 = rotate(u, mu, s, cp, sp);
     E1 = eps * E;
     Te = E - E1;
-    ue = E * u - E1 * u1;
-    normalise(ue, u);
+    // momentum balance E u = E1 u1 + p_e u_e with u1 = mu u + s e: p_e u_e = (E - E1 mu) u - E1 s e, and
+    // E - E1 mu = Te + E1 t carries no cancellation
+    ue = rotate(u, Te + E1 * t, -E1 * s, cp, sp);
 }
 
 // ---- photoelectron direction, leading Sauter term p(mu) ~ (1 - mu^2) / (1 - beta mu)^4 (C6.2)
@@ -162,12 +175,12 @@ EMX_NI bool pair_production(Rng &r, int Z, double E, const Vec3 &u, double &Tm, 
     if (tp < 0.0) tp = 0.0;
     Tm = tm;
     Tp = tp;
-    const double mum = boosted_iso(r.next(), beta_of(tm));
-    const double mup = boosted_iso(r.next(), beta_of(tp));
+    const double t_m = boosted_iso_t(r.next(), tm);
+    const double t_p = boosted_iso_t(r.next(), tp);
     double sp, cp;
     sincos_(2.0 * kPi * r.next(), sp, cp);
-    um = rotate(u, mum, sqrt((1.0 - mum) * (1.0 + mum)), cp, sp);
-    up = rotate(u, mup, sqrt((1.0 - mup) * (1.0 + mup)), -cp, -sp);
+    um = rotate(u, 1.0 - t_m, sin_of_t(t_m), cp, sp);
+    up = rotate(u, 1.0 - t_p, sin_of_t(t_p), -cp, -sp);
     return true;
 }
 
@@ -183,13 +196,16 @@ EMX_NI bool bremsstrahlung(Rng &r, double T, double kc, const Vec3 &u, double &k
         const double y = kk / T;
         if ((4.0 / 3.0) * x2 <= 4.0 / 3.0 - 4.0 * y / 3.0 + y * y) break;
     }
-    const double mu = boosted_iso(r.next(), beta_of(T));
-    ug = rotate_mu_phi(u, mu, 2.0 * kPi * r.next());
+    const double t = boosted_iso_t(r.next(), T), sn = sin_of_t(t);
+    double sp, cp;
+    sincos_(2.0 * kPi * r.next(), sp, cp);
+    ug = rotate(u, 1.0 - t, sn, cp, sp);
     const double p = sqrt(T * (T + 2.0 * kMe));
     k = kk;
     T1 = T - kk;
-    u1 = p * u - kk * ug;
-    normalise(u1, u);
+    // recoil p u - k u_gamma = (p - k mu) u - k s e, with p - k mu = (p - T) + T1 + k t and
+    // p - T = 2 me T / (p + T): no difference of nearly equal numbers
+    u1 = rotate(u, 2.0 * kMe * T / (p + T) + T1 + kk * t, -kk * sn, cp, sp);
     return true;
 }
 
@@ -197,10 +213,15 @@ EMX_NI bool bremsstrahlung(Rng &r, double T, double kc, const Vec3 &u, double &k
 EMX_NI void knock_on(Rng &r, double T, double Td, const Vec3 &u, Vec3 &ud, double &T1, Vec3 &u1) {
     const double p = sqrt(T * (T + 2.0 * kMe)), pd = sqrt(Td * (Td + 2.0 * kMe));
     const double mu = clamp1(Td * (T + 2.0 * kMe) / (p * pd));
-    ud = rotate_mu_phi(u, mu, 2.0 * kPi * r.next());
+    // sin^2 = 1 - mu^2 = 2 me (T - Td) / (T (Td + 2 me)) in closed form
+    const double s2 = 2.0 * kMe * (T - Td) / (T * (Td + 2.0 * kMe));
+    const double sn = s2 > 0.0 ? sqrt(s2) : 0.0;
+    double sp, cp;
+    sincos_(2.0 * kPi * r.next(), sp, cp);
+    ud = rotate(u, mu, sn, cp, sp);
     T1 = T - Td;
-    u1 = p * u - pd * ud;
-    normalise(u1, u);
+    // primary: p u - pd u_delta = (p - pd mu) u - pd s e, p - pd mu = (T - Td)(T + 2 me) / p
+    u1 = rotate(u, T1 * (T + 2.0 * kMe) / p, -pd * sn, cp, sp);
 }
 
 EMX_NI bool moller(Rng &r, double T, double Tcut, const Vec3 &u, double &Td, Vec3 &ud, double &T1, Vec3 &u1) {
@@ -250,21 +271,27 @@ EMX_NI void annih_flight(Rng &r, double T, const Vec3 &u, double &k1, Vec3 &u1, 
     }
     const double Etot = T + 2.0 * kMe;
     const double kk = eps * Etot;
-    const double mu = clamp1((eps * (g + 1.0) - 1.0) / (eps * sqrt(g * g - 1.0)));
-    u1 = rotate_mu_phi(u, mu, 2.0 * kPi * r.next());
-    const double p = sqrt(T * (T + 2.0 * kMe));
+    const double pg = sqrt(g * g - 1.0);  // p / me
+    const double mu = clamp1((eps * (g + 1.0) - 1.0) / (eps * pg));
+    // sin^2 = 1 - mu^2 = (2 (g + 1) eps (1 - eps) - 1) / (eps^2 (g^2 - 1)) in closed form
+    const double s2 = (2.0 * (g + 1.0) * eps * (1.0 - eps) - 1.0) / (eps * eps * (g * g - 1.0));
+    const double sn = s2 > 0.0 ? sqrt(s2) : 0.0;
+    double sp, cp;
+    sincos_(2.0 * kPi * r.next(), sp, cp);
+    u1 = rotate(u, mu, sn, cp, sp);
     k1 = kk;
     k2 = Etot - kk;
-    u2 = p * u - kk * u1;
-    normalise(u2, u);
+    // second photon: p u - k1 u1 = (p - k1 mu) u - k1 s e, p - k1 mu = me (g + 1) ((1 - eps)(g + 1) - 1) / sqrt(g^2 - 1)
+    u2 = rotate(u, kMe * (g + 1.0) * ((1.0 - eps) * (g + 1.0) - 1.0) / pg, -kk * sn, cp, sp);
 }
 
 // ---- annihilation at rest: two back-to-back me photons, isotropic (C6.6, R12/R25)
 EMX_NI void annih_rest(Rng &r, Vec3 &u1, Vec3 &u2) {
-    const double mu = 2.0 * r.next() - 1.0;
+    const double xi = r.next();
+    const double mu = 2.0 * xi - 1.0;
     double sp, cp;
     sincos_(2.0 * kPi * r.next(), sp, cp);
-    const double s = sqrt((1.0 - mu) * (1.0 + mu));
+    const double s = 2.0 * sqrt(xi * (1.0 - xi));  // sqrt((1 - mu)(1 + mu)) without the cancellation
     u1 = {s * cp, s * sp, mu};
     u2 = {-u1.x, -u1.y, -u1.z};
 }

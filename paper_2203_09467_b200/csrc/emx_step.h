@@ -219,8 +219,9 @@ EMX_HD void finish_step(const Params &P, int pt, Track &t, StepOut &o) {
 
 // ---- stage a0: items 1-4 (tracking cut, lookup, limits; draw 0).  Fills c.s_phys and c.action.
 // EXT: multiple scattering and / or energy-loss fluctuations are on.
+// L receives the table values of item 3 (left alone below the cut and in vacuum) for a caller that runs stage a2 next.
 template <bool CH, bool EXT>
-EMX_HD void step_a0(const Params &P, uint64_t seed, int pt, const Track &t, Carry &c) {
+EMX_HD void step_a0(const Params &P, uint64_t seed, int pt, const Track &t, Carry &c, Lookup &L) {
     const emx_physics &ph = P.ph;
     const int mat = P.vol[t.vol].material;
     c.s = 0.0;
@@ -232,7 +233,6 @@ EMX_HD void step_a0(const Params &P, uint64_t seed, int pt, const Track &t, Carr
         c.s_phys = ph.vacuum_step;
         c.action = EMX_A_TRUNC;
     } else {  // 3. lookup, 4. limits
-        Lookup L;
         lookup_tables<CH, EXT>(P, pt, mat, t.E, L);
         const double xi = draw_at(seed, t.prim, t.tid, t.step, 0u);
         step_limits<CH, EXT>(P, L, xi, c.s_phys, c.action);
@@ -273,8 +273,9 @@ EMX_HD void field_move_done(Carry &c, double s, int hit) {
 
 // ---- stage a2: items 6, 7, 7b and the selection of item 8.  t.E is still the pre-step energy.  Returns the process
 // id (EMX_P_*) if an interaction is pending (step_interact finishes the step), else -1 and the step is complete.
-template <bool CH, bool EXT>
-EMX_HD int step_a2(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o, const Carry &c) {
+// HAVE_L: L already holds the table values of stage a0 (same slot, same energy); else they are looked up again.
+template <bool CH, bool EXT, bool HAVE_L = false>
+EMX_HD int step_a2(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o, const Carry &c, Lookup &L) {
     const emx_physics &ph = P.ph;
     clear_out(o);
     Rng rng;
@@ -288,11 +289,12 @@ EMX_HD int step_a2(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o,
     const int action = c.action;
     const double s = c.s;
     const double E = t.E;
-    Lookup L;
-    L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.var0 = 0.0;
-    L.Rtab = nullptr;
+    if (!HAVE_L) {
+        L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.var0 = 0.0;
+        L.Rtab = nullptr;
+    }
     if (mat >= 0) {
-        lookup_tables<CH, EXT>(P, pt, mat, E, L);
+        if (!HAVE_L) lookup_tables<CH, EXT>(P, pt, mat, E, L);
         (void)rng.next();  // draw 0 was the interaction length (stage a1); this also restores the block's second half
     }
     const bool msc = CH && EXT && ph.msc && mat >= 0;  // multiple scattering applies (R-MSC)
@@ -488,8 +490,11 @@ EMX_HD void step_interact(const Params &P, uint64_t seed, int pt, Track &t, Step
 template <bool CH, bool MAP = false, bool EXT = false>
 EMX_HD void step(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o, int &n_sub) {
     Carry c;
+    Lookup L;
+    L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.var0 = 0.0;
+    L.Rtab = nullptr;
     n_sub = 0;
-    step_a0<CH, EXT>(P, seed, pt, t, c);
+    step_a0<CH, EXT>(P, seed, pt, t, c, L);
     if (c.action != kActCut) {
         if (!CH || P.Bmag == 0.0) {
             move_straight(P, t, c);
@@ -499,7 +504,7 @@ EMX_HD void step(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o, i
             field_move_done(c, s, hit);
         }
     }
-    const int proc = step_a2<CH, EXT>(P, seed, pt, t, o, c);
+    const int proc = step_a2<CH, EXT, true>(P, seed, pt, t, o, c, L);
     if (proc >= 0) step_interact<CH>(P, seed, pt, t, o, proc);
 }
 

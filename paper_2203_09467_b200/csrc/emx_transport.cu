@@ -58,6 +58,7 @@ __device__ __forceinline__ void move_slot(const Work &w, int from, int to) {
         t.s_done[to] = t.s_done[from];
         t.h_try[to] = t.h_try[from];
         t.att[to] = t.att[from];
+        t.kap[to] = t.kap[from];
     }
 }
 
@@ -340,7 +341,11 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
     }
     for (int p = 0; p < kPools; ++p) {
         const int own = s_owned[p], grant = s_grant[p], nf = s_free;
-        for (int k = tid; k < grant - own; k += blockDim.x) w.ctab[p][own + k] = w.free_list[nf - 1 - k];
+        for (int k = tid; k < grant - own; k += blockDim.x) {
+            const int ch = w.free_list[nf - 1 - k];
+            w.ctab[p][own + k] = ch;
+            w.rtab[ch] = own + k;
+        }
         __syncthreads();
         if (tid == 0 && grant > own) {
             s_free = nf - (grant - own);
@@ -365,7 +370,9 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
         }
         if (live == 0 && c->next_primary >= w.n_primaries) {
             c->done = 1;
-            c->m_step[0] = c->m_step[1] = 0;
+            c->m_step[0] = c->m_step[1] = 0;  // the iterations still queued behind this one find nothing to do
+            for (int p = 0; p < kPools; ++p)
+                for (int k = 0; k < kMaxLists; ++k) c->icount[p][k] = 0;
         } else {
             c->iter += 1;
             // R7: a step whose secondaries do not fit on the stacks is not committed and is re-executed in a
@@ -381,6 +388,7 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
             if (c->idle_iters >= kPatience) {
                 c->error = EMX_E_CAPACITY;
                 c->done = 1;
+                c->m_step[0] = c->m_step[1] = 0;  // nothing more is stepped (k_plan returns at once from now on)
             }
             c->had_live = live > 0 ? 1 : 0;
             // time slicing of the field propagation: with many tracks in flight a track may be parked after a few
@@ -388,9 +396,7 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
             // iteration open; with few tracks left latency matters more and every propagation runs to its end
             c->field_min = live > w.slice_above ? w.slice_min : 0x7fffffff;
             c->progress = 0ull;
-            c->work_a[0] = c->work_a[1] = 0;
-            c->work_b[0] = c->work_b[1] = 0;
-            c->work_0 = c->work_f = 0;
+            c->work_f = 0;
             for (int p = 0; p < kPools; ++p)
                 for (int k = 0; k < kMaxLists; ++k) c->icount[p][k] = 0;
         }
@@ -555,33 +561,22 @@ __device__ __forceinline__ void flush_acc(Ctl *c, const WarpAcc &acc, int lane, 
 // which never moves the top past the capacity; a large stack is simply treated as full.  Nothing is ever rolled
 // back: an add-then-subtract scheme lets a reservation succeed above a top that a concurrent failure has
 // inflated, and strands its records.
-__device__ __forceinline__ int reserve(Ctl *c, const Work &w, int pool, int cnt, int lane) {
-    int r0 = -1;
-    if (lane == 0) {
-        const int cap = w.qcap[pool];
-        if (__ldg(&c->q_safe[pool])) {
-            // k_plan's guarantee for this iteration: one round trip to the top instead of two
-            r0 = atomicAdd(&c->q_top[pool], cnt);
-        } else {
-            int old = *(volatile int *)&c->q_top[pool];
-            if ((long long)old + cnt + w.reserve_slack <= (long long)cap) {
-                r0 = atomicAdd(&c->q_top[pool], cnt);
-            } else if ((long long)cap < 8LL * w.reserve_slack) {
-                // small stack: exact accounting by compare-and-swap
-                while (old + cnt <= cap) {
-                    const int prev = atomicCAS(&c->q_top[pool], old, old + cnt);
-                    if (prev == old) {
-                        r0 = old;
-                        break;
-                    }
-                    old = prev;
-                }
-            }
-            // large stack within the slack of its capacity: treated as full (thousands of warps spinning on
-            // one compare-and-swap cost 10x the iteration; the last 2 % of a large stack are not worth it)
+__device__ __forceinline__ int reserve(Ctl *c, const Work &w, int pool, int cnt, bool safe) {
+    const int cap = w.qcap[pool];
+    if (safe) return atomicAdd(&c->q_top[pool], cnt);  // k_plan's guarantee for this iteration: one round trip to the top
+    int old = *(volatile int *)&c->q_top[pool];
+    if ((long long)old + cnt + w.reserve_slack <= (long long)cap) return atomicAdd(&c->q_top[pool], cnt);
+    if ((long long)cap < 8LL * w.reserve_slack) {
+        // small stack: exact accounting by compare-and-swap
+        while (old + cnt <= cap) {
+            const int prev = atomicCAS(&c->q_top[pool], old, old + cnt);
+            if (prev == old) return old;
+            old = prev;
         }
     }
-    return __shfl_sync(0xffffffffu, r0, 0);
+    // large stack within the slack of its capacity: treated as full (thousands of warps spinning on
+    // one compare-and-swap cost 10x the iteration; the last 2 % of a large stack are not worth it)
+    return -1;
 }
 
 // bin of the steps-per-track histogram (include/emx.h: EMX_NHIST)
@@ -616,7 +611,7 @@ enum : int { kWrX = 1, kWrU = 2, kWrE = 4 };
 template <int POOL, int WR, bool CONSEC>
 __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint64_t seed, double *tally, int i, int s,
                                             int pt, bool active, bool tomb, int pend, Track &t, StepOut &o, int vol0,
-                                            uint32_t step0) {
+                                            uint32_t step0, int safe) {
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
@@ -632,27 +627,37 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     bool stall = false;
     int r_c = -1, r_g = -1;
     {
-        const unsigned b = __ballot_sync(0xffffffffu, nc > 0);
-        if (b) {
-            int inc = nc;
-            if (POOL == kPoolGamma) inc = warp_scan_incl(nc, lane);  // 0..2 per lane (pair production)
-            else inc = __popc(b & lt) + nc;                          // 0..1 per lane
-            const int tot = POOL == kPoolGamma ? __shfl_sync(0xffffffffu, inc, 31) : __popc(b);
-            const int r0 = reserve(c, w, kPoolCharged, tot, lane);
-            if (nc) {
-                if (r0 < 0) stall = true;
-                else r_c = r0 + inc - nc;
+        // warp totals and each lane's offset: charged records 0..2 per lane from photons (pair production), 0..1
+        // from e+-; photons 0..3 per lane, from e+- only.  Lane 0 reserves on the charged stack and lane 1 on the
+        // photon stack in the same instruction, so the two round trips overlap.
+        const unsigned bc = __ballot_sync(0xffffffffu, nc > 0);
+        const unsigned bg = POOL == kPoolCharged ? __ballot_sync(0xffffffffu, ng > 0) : 0u;
+        if (bc | bg) {
+            int inc_c = 0, tot_c = 0, inc_g = 0, tot_g = 0;
+            if (bc) {
+                if (POOL == kPoolGamma) {
+                    inc_c = warp_scan_incl(nc, lane);
+                    tot_c = __shfl_sync(0xffffffffu, inc_c, 31);
+                } else {
+                    inc_c = __popc(bc & lt) + nc;
+                    tot_c = __popc(bc);
+                }
             }
-        }
-    }
-    if (POOL == kPoolCharged) {  // only e+- make photons: 0..3 per lane
-        const unsigned b = __ballot_sync(0xffffffffu, ng > 0);
-        if (b) {
-            const int inc = warp_scan_incl(ng, lane);
-            const int r0 = reserve(c, w, kPoolGamma, __shfl_sync(0xffffffffu, inc, 31), lane);
+            if (bg) {
+                inc_g = warp_scan_incl(ng, lane);
+                tot_g = __shfl_sync(0xffffffffu, inc_g, 31);
+            }
+            int r0 = -1;
+            const int my_cnt = lane == 0 ? tot_c : (lane == 1 ? tot_g : 0);
+            if (my_cnt) r0 = reserve(c, w, 1 - lane, my_cnt, (safe >> (1 - lane)) & 1);  // lane 0: kPoolCharged, lane 1: kPoolGamma
+            const int r0c = __shfl_sync(0xffffffffu, r0, 0), r0g = __shfl_sync(0xffffffffu, r0, 1);
+            if (nc) {
+                if (r0c < 0) stall = true;
+                else r_c = r0c + inc_c - nc;
+            }
             if (ng) {
-                if (r0 < 0) stall = true;
-                else r_g = r0 + inc - ng;
+                if (r0g < 0) stall = true;
+                else r_g = r0g + inc_g - ng;
             }
         }
     }
@@ -711,8 +716,8 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     if (CONSEC) {  // the warp's lanes are 32 consecutive slots of one chunk
         const unsigned bd = __ballot_sync(0xffffffffu, died);
         if (bd && lane == 0) atomicAdd(&w.chunk_dead[POOL][i / kChunk], __popc(bd));
-    } else if (died) {
-        atomicAdd(&w.chunk_dead[POOL][i / kChunk], 1);
+    } else if (died) {  // phase B works on physical slots: the chunk's place in the pool comes from the reverse table
+        atomicAdd(&w.chunk_dead[POOL][w.rtab[s / kChunk]], 1);
     }
 
     // ---- A10: per-volume tally.  Lanes with the same tally id are summed with shuffles; one atomic per group.
@@ -793,7 +798,7 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
 // k_b runs every interactor on full warps (B:north_star "partitioned by next action").
 template <int POOL, bool EXT, bool FUSED>
 __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
-                                           int n_live) {
+                                           int n_live, int safe) {
     constexpr bool CH = POOL == kPoolCharged;
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
@@ -835,8 +840,11 @@ __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint6
         vol0 = t.vol;
         step0 = t.step;
         Carry cy;
+        Lookup L;
+        L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.var0 = 0.0;
+        L.Rtab = nullptr;
         if (FUSED) {
-            step_a0<CH, EXT>(P, seed, pt, t, cy);
+            step_a0<CH, EXT>(P, seed, pt, t, cy, L);
             if (cy.action != kActCut) move_straight(P, t, cy);
         } else {
             cy.action = ts.act[s];
@@ -844,32 +852,28 @@ __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint6
             cy.hit = ts.att[s];
             cy.s_phys = 0.0;
         }
-        pend = step_a2<CH, EXT>(P, seed, pt, t, o, cy);
+        pend = step_a2<CH, EXT, FUSED>(P, seed, pt, t, o, cy, L);
     }
     // file the lanes with a pending interaction (new or stalled) in the list of their process: one atomic per
     // warp and non-empty list
     const int pk = waiting ? proc_slot<POOL>(stage - kStPend) : (pend >= 0 ? proc_slot<POOL>(pend) : -1);
+    // (lane k reserves the entries of list k; the atomics are in flight while the epilogue runs)
     constexpr int nk = CH ? 4 : 3;
-    int my_base = 0;
     unsigned my_mask = 0;
+    int list_cnt = 0, list_r0 = 0;
 #pragma unroll
     for (int k = 0; k < nk; ++k) {
         const unsigned b = __ballot_sync(0xffffffffu, pk == k);
-        if (b) {
-            int r0 = 0;
-            if (lane == 0) r0 = atomicAdd(&c->icount[POOL][k], __popc(b));
-            r0 = __shfl_sync(0xffffffffu, r0, 0);
-            if (pk == k) {
-                my_base = r0;
-                my_mask = b;
-            }
-        }
+        if (pk == k) my_mask = b;
+        if (lane == k) list_cnt = __popc(b);
     }
+    if (list_cnt) list_r0 = atomicAdd(&c->icount[POOL][lane], list_cnt);
     // FUSED: position moved here; a2: position and direction were written by the propagation kernel, the
     // direction changes again only through multiple scattering
     constexpr int WR = FUSED ? (kWrX | (CH ? kWrE : 0) | (CH && EXT ? kWrU : 0)) : (kWrE | (EXT ? kWrU : 0));
-    WarpAcc acc = epilogue<POOL, WR, true>(P, w, seed, tally, i, s, pt, go || tomb, tomb, pend, t, o, vol0, step0);
-    if (pk >= 0) w.ilist[POOL][pk][my_base + __popc(my_mask & lt)] = i;
+    WarpAcc acc = epilogue<POOL, WR, true>(P, w, seed, tally, i, s, pt, go || tomb, tomb, pend, t, o, vol0, step0, safe);
+    const int my_base = __shfl_sync(0xffffffffu, list_r0, pk >= 0 ? pk : 0);
+    if (pk >= 0) w.ilist[POOL][pk][my_base + __popc(my_mask & lt)] = s;
     // a track the refill has just moved and that no kernel finishes in this iteration (parked propagation, stalled
     // interaction) still carries the mark of the refill pass
     if (in && !(go || tomb) && al == 2) ts.alive[s] = 1;
@@ -883,17 +887,15 @@ __device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, ui
     const int lane = threadIdx.x & 31;
     const int nl = c->m_step[POOL];
     const int total = (nl + 31) >> 5;
+    const int safe = c->q_safe[0] | (c->q_safe[1] << 1);
     EMX_TL(w, node, 0, 1);
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
-    int k_next = 0;
-    if (lane == 0) k_next = atomicAdd(&c->work_a[POOL], 1);
-    for (;;) {
-        const int k = __shfl_sync(0xffffffffu, k_next, 0);
-        if (k >= total) break;
-        if (lane == 0) k_next = atomicAdd(&c->work_a[POOL], 1);
-        const WarpAcc d = a_group<POOL, EXT, FUSED>(P, w, seed, tally, k << 5, nl);
+    // the groups of a dense kernel cost about the same: a fixed stride per warp, no work counter
+    const int n_warps = gridDim.x * (kStepBlock / 32);
+    for (int k = blockIdx.x * (kStepBlock / 32) + (threadIdx.x >> 5); k < total; k += n_warps) {
+        const WarpAcc d = a_group<POOL, EXT, FUSED>(P, w, seed, tally, k << 5, nl, safe);
         acc.n += d.n;
         acc.d += d.d;
     }
@@ -938,14 +940,11 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_0) k_a0(const __grid_co
     const int nl = c->m_step[kPoolCharged];
     const int total = (nl + 31) >> 5;
     const Store &ts = w.st;
+    const int ax = P.field_kind == 0 ? field_axis(P.Bhat) : kAxisAny;
     EMX_TL(w, 7, 0, 1);
     unsigned long long n_done = 0;
-    int k_next = 0;
-    if (lane == 0) k_next = atomicAdd(&c->work_0, 1);
-    for (;;) {
-        const int k = __shfl_sync(0xffffffffu, k_next, 0);
-        if (k >= total) break;
-        if (lane == 0) k_next = atomicAdd(&c->work_0, 1);
+    const int n_warps = gridDim.x * (kStepBlock / 32);
+    for (int k = blockIdx.x * (kStepBlock / 32) + (threadIdx.x >> 5); k < total; k += n_warps) {
         const int i = (k << 5) + lane;
         if (i >= nl) continue;
         const int s = phys_slot(w, kPoolCharged, i);
@@ -960,10 +959,24 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_0) k_a0(const __grid_co
         t.step = (uint32_t)id.y;
         t.vol = id.z;
         Carry cy;
-        step_a0<true, EXT>(P, seed, ts.ptype[s], t, cy);
-        ts.s_phys[s] = cy.s_phys;
+        Lookup L;
+        const int pt = ts.ptype[s];
+        step_a0<true, EXT>(P, seed, pt, t, cy, L);
         ts.act[s] = (uint8_t)cy.action;
-        ts.stage[s] = (uint8_t)(cy.action == kActCut ? kStMoved : kStReady);
+        if (cy.action == kActCut) {
+            ts.stage[s] = kStMoved;
+        } else {  // the propagation starts here: curvature and the first trial step (C9)
+            double kappa = curvature(P, pt, t.E);
+            if (ax != kAxisAny) kappa *= P.Bhat[ax];
+            FieldState fs;
+            field_begin(kappa, cy.s_phys, fs);
+            ts.s_phys[s] = cy.s_phys;
+            ts.kap[s] = kappa;
+            ts.s_done[s] = fs.s_done;
+            ts.h_try[s] = fs.h;
+            ts.att[s] = fs.attempt;
+            ts.stage[s] = kStParked;
+        }
         n_done += 1;
     }
     for (int o = 16; o > 0; o >>= 1) n_done += __shfl_xor_sync(0xffffffffu, n_done, o);
@@ -1009,8 +1022,7 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid
                     dry = true;
                 } else {
                     s = phys_slot(w, kPoolCharged, i);
-                    const int stage = ts.stage[s];
-                    if (stage == kStReady || stage == kStParked) {
+                    if (ts.stage[s] == kStParked) {
                         const double2 xy = ts.xy[s], zu = ts.zu[s], uu = ts.uu[s];
                         const int4 id = ts.id[s];
                         x = {xy.x, xy.y, zu.x};
@@ -1019,15 +1031,10 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid
                         surf = id.w;
                         s_max = ts.s_phys[s];
                         act = ts.act[s];
-                        kappa = curvature(P, ts.ptype[s], ts.Et[s].x);
-                        if (!MAP && AX != kAxisAny) kappa *= P.Bhat[AX];
-                        if (stage == kStReady) {
-                            field_begin(kappa, s_max, fs);
-                        } else {
-                            fs.s_done = ts.s_done[s];
-                            fs.h = ts.h_try[s];
-                            fs.attempt = ts.att[s];
-                        }
+                        kappa = ts.kap[s];
+                        fs.s_done = ts.s_done[s];
+                        fs.h = ts.h_try[s];
+                        fs.attempt = ts.att[s];
                         have = true;
                         used = 0;
                         n_trk += 1;
@@ -1086,14 +1093,14 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid
 // ---- phase B of a group: 32 tracks of a pool waiting for the same interactor (list k of the pool).
 template <int POOL>
 __device__ __forceinline__ WarpAcc b_group(const Params &P, const Work &w, uint64_t seed, double *tally, int k, int first,
-                                           int n_list) {
+                                           int n_list, int safe) {
     constexpr bool CH = POOL == kPoolCharged;
     const int lane = threadIdx.x & 31;
     const int idx = first + lane;
     const Store &ts = w.st;
     const bool active = idx < n_list;
-    const int i = active ? w.ilist[POOL][k][idx] : 0;
-    const int s = active ? phys_slot(w, POOL, i) : 0;
+    const int s = active ? w.ilist[POOL][k][idx] : 0;
+    const int i = 0;  // phase B does not need the pool-local index
     Track t;
     StepOut o;
     clear_out(o);
@@ -1117,7 +1124,7 @@ __device__ __forceinline__ WarpAcc b_group(const Params &P, const Work &w, uint6
         step0 = t.step;
         step_interact<CH>(P, seed, pt, t, o, slot_proc<POOL>(k));
     }
-    return epilogue<POOL, kWrU | kWrE, false>(P, w, seed, tally, i, s, pt, active, false, -1, t, o, vol0, step0);
+    return epilogue<POOL, kWrU | kWrE, false>(P, w, seed, tally, i, s, pt, active, false, -1, t, o, vol0, step0, safe);
 }
 
 // Phase B: the interactors.  Persistent warps pull 32-entry groups of the pool's process lists; a warp runs ONE
@@ -1142,19 +1149,16 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_B) k_b(const __grid_con
         cb[k + 1] = cb[k] + ((n[k] + 31) >> 5);
     }
     const int total = cb[4];
+    const int safe = c->q_safe[0] | (c->q_safe[1] << 1);
     EMX_TL(w, 5 + POOL, 0, 1);
     WarpAcc acc;
     acc.n = 0ull;
     acc.d = 0.0;
-    int k_next = 0;
-    if (lane == 0 && total > 0) k_next = atomicAdd(&c->work_b[POOL], 1);
-    for (;;) {
-        const int ch = __shfl_sync(0xffffffffu, k_next, 0);
-        if (ch >= total) break;
-        if (lane == 0) k_next = atomicAdd(&c->work_b[POOL], 1);
+    const int n_warps = gridDim.x * (kStepBlock / 32);
+    for (int ch = blockIdx.x * (kStepBlock / 32) + (threadIdx.x >> 5); ch < total; ch += n_warps) {
         // one call site: the interactor code exists once per kernel
         const int sel = ch < cb[1] ? 0 : (ch < cb[2] ? 1 : (ch < cb[3] ? 2 : 3));
-        const WarpAcc d = b_group<POOL>(P, w, seed, tally, ord[sel], (ch - cb[sel]) << 5, n[sel]);
+        const WarpAcc d = b_group<POOL>(P, w, seed, tally, ord[sel], (ch - cb[sel]) << 5, n[sel], safe);
         acc.n += d.n;
         acc.d += d.d;
     }
@@ -1287,6 +1291,7 @@ __global__ void k_hook_init(Work w, int n_live, int n_queue) {
     for (int k = tid; k < w.n_chunks; k += gridDim.x * blockDim.x) {
         w.ctab[0][k] = k;
         w.ctab[1][k] = 0;
+        w.rtab[k] = k;
     }
 }
 __global__ void __launch_bounds__(kChunk) k_count_dead(Work w, int n_live) {
@@ -1297,7 +1302,7 @@ __global__ void __launch_bounds__(kChunk) k_count_dead(Work w, int n_live) {
 
 size_t refill_plan_scratch_ints(long capacity) {
     const size_t nch = (size_t)(capacity + kChunk - 1) / kChunk + 1;
-    return 6 * nch + (size_t)capacity + (sizeof(Ctl) + 3) / 4 + 64 + (nch * kChunk + 3) / 4 + 64;
+    return 7 * nch + (size_t)capacity + (sizeof(Ctl) + 3) / 4 + 64 + (nch * kChunk + 3) / 4 + 64;
 }
 
 cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
@@ -1312,6 +1317,7 @@ cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const u
     w.ctab[0] = p; p += nch;
     w.ctab[1] = p; p += nch;
     w.free_list = p; p += 2 * nch;
+    w.rtab = p; p += nch;
     w.hole_idx[0] = p; p += capacity;
     w.hole_idx[1] = w.hole_idx[0];
     p += (16 - ((uintptr_t)p / 4) % 16) % 16;  // 64-byte alignment for the control block

@@ -25,8 +25,7 @@ EMX_HD int pool_of(int ptype) { return ptype == kGamma ? kPoolGamma : kPoolCharg
 // where a live track is in its step
 enum : int {
     kStFresh = 0,   // needs limits (stage a0)
-    kStReady = 1,   // limits known, move not started (charged pool in a field)
-    kStParked = 2,  // field propagation in progress
+    kStParked = 2,  // charged pool in a field: limits known, propagation not started or in progress
     kStMoved = 3,   // move done, needs stage a2
     kStPend = 8     // + process id: interaction selected, waits for the interactor (or stalled on a full stack)
 };
@@ -45,6 +44,7 @@ struct Store {
     // trial step of the propagation; substep attempts used (after the move: surface hit, -1 none)
     double *s_phys, *s_done, *h_try;
     int *att;
+    double *kap;     // curvature of the current step (sign of the charge and of an axis-aligned field folded in)
 };
 
 // secondary / primary initializer record (80 bytes): same packing, .id = (prim, vol, surf, ptype)
@@ -75,10 +75,7 @@ struct Ctl {
     int n_free;          // chunks on the free list
     int done, error, had_live;
     int idle_iters;      // consecutive iterations without progress although tracks are live (R7)
-    int work_a[kPools];  // next 32-slot group of each pool for the dense phase-A kernel (stages a0 .. a2, or a2 alone)
-    int work_0;          // ... for the limits kernel of the charged pool (field)
-    int work_f;          // next slot of the charged pool for the propagation kernel
-    int work_b[kPools];  // next 32-entry group of each pool's interaction lists (phase B)
+    int work_f;          // next slot of the charged pool for the propagation kernel (the dense kernels stride)
     int icount[kPools][kMaxLists];  // entries in the interaction lists
     int field_min;       // substep attempts a track is given per iteration before it may be parked
     unsigned long long iter;
@@ -100,10 +97,11 @@ struct Work {
     int qcap[kPools];     // records per stack
     int *ctab[kPools];    // chunk tables, n_chunks entries each
     int *free_list;       // n_chunks entries
+    int *rtab;            // physical chunk -> its index in the owning pool's chunk table
     int *chunk_dead[kPools];  // per pool-local chunk: slots that died in the last iteration
     int *chunk_off[kPools];   // ... exclusive prefix sum of it
     int *hole_idx[kPools];
-    int *ilist[kPools][kMaxLists];  // pool-local slots waiting for an interactor, n_slots entries each
+    int *ilist[kPools][kMaxLists];  // PHYSICAL slots waiting for an interactor, n_slots entries each
     Ctl *ctl;
     uint32_t *log;  // per iteration: live, queued
     int max_log;

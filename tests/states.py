@@ -105,19 +105,72 @@ def result_arrays(res):
 
 
 ME = 0.51099895
+EPS = 2.0 ** -52          # fp64 unit roundoff (spacing at 1)
+RTOL2 = 1e-12             # level 2 of BASELINE.json north_star
 
 
-def compare_steps(ref, got, E_in, skip=None):
+def step_tolerances(desc, tracks, ref):
+    """Per-state level-2 tolerances, DERIVED from the arithmetic of the step, as multiples of
+    nothing observed: every entry is RTOL2 for a step without field substeps and without fluctuated loss.
+
+    Field steps (n = substep attempts, from the oracle's own count).  Both implementations run the same IEEE
+    operations, but their libm differs in the last bit, so after the first substep the two positions differ by
+    ~EPS |x|.  The error estimate err = |x_full - x_half| is a difference of nearly equal positions: its relative
+    difference is EPS |x| / err, the next trial step h differs by a fifth of that (h ~ err^-1/5), and the RK4
+    truncation error of a substep (err / 15, fifth order in h) changes by 5 dh/h err / 15 = EPS |x| / 15: per substep
+    the end point moves by <= EPS |x| along the helix and the direction by <= |kappa| EPS |x|, whatever err is.
+      positions, path length   RTOL2 + 4 n EPS                       (relative to X = max(|x|, s))
+      directions               RTOL2 + n EPS X |kappa|
+    A step cut short by the substep budget (action TRUNC) returns s = sum of its n trial steps, each carrying
+    dh/h <= EPS |x| / (5 err) with err >= field_eps / 3125 where h still grows: ds/s <= 625 EPS X / field_eps, and
+    the direction turns by |kappa| ds.  In a NON-UNIFORM field the error estimate varies along the path, the two
+    substep sequences drift apart by the same dh/h and a boundary is reached at points up to the landing tolerance
+    apart: ds <= 2 field_eps for a step that ends on a surface.
+    Energy-loss fluctuations: the fluctuated loss can take most of E, the post-loss energy E' = E - dE carries
+    EPS E / E' of relative rounding and everything the interactor computes from E' inherits it: scale E / E'."""
+    n = len(tracks)
+    ph = desc["physics"]
+    B = float(np.linalg.norm(desc.get("field", (0.0, 0.0, 0.0))))
+    E = np.array([t.E for t in tracks])
+    pt = np.array([t.ptype for t in tracks])
+    nsub = ref["n_sub"].astype(np.float64)
+    p = np.sqrt(E * (E + 2 * ME))
+    kappa = np.where(pt != 0, 2.99792458 * B / np.maximum(p, 1e-300), 0.0)
+    fin = np.isfinite(ref["s"])
+    X = np.maximum(np.linalg.norm(ref["x"], axis=1), np.where(fin, np.abs(ref["s"]), 0.0))
+    tol_x = RTOL2 + 4 * nsub * EPS
+    tol_u = RTOL2 + nsub * EPS * X * kappa
+    tol_E = np.full(n, RTOL2)
+    eps_f = ph["field_eps"]
+    trunc = (ref["action"] == 4) & (nsub >= ph["max_substeps"])
+    ds_rel = 625 * EPS * X / eps_f                      # of s
+    s_abs = np.where(fin, np.abs(ref["s"]), 0.0)
+    tol_x = np.where(trunc, tol_x + ds_rel * s_abs / np.maximum(X, 1e-300), tol_x)
+    tol_u = np.where(trunc, tol_u + kappa * ds_rel * s_abs, tol_u)
+    if desc.get("field_fringe"):
+        moved = nsub > 1
+        tol_x = np.where(moved, tol_x + 2 * eps_f / np.maximum(X, 1e-300), tol_x)
+        tol_u = np.where(moved, tol_u + kappa * 2 * eps_f, tol_u)
+    if ph.get("fluct"):
+        e_post = np.maximum(E - ref["edep"], 0.0)
+        scale = np.where((pt != 0) & (e_post > 0), np.minimum(E / np.maximum(e_post, 1e-300), 1e6), 1.0)
+        tol_E = tol_E * scale
+        tol_u = tol_u * scale
+    return dict(x=tol_x, u=tol_u, E=tol_E, trunc=trunc)
+
+
+def compare_steps(ref, got, E_in, tol=None, skip=None):
     """Level-1/2 comparison of two result dicts for the same input states (E_in = their energies).
     Integers must be equal.  Energies are compared on the scale of the step's input energy
     (E' = E - dE is a difference, so its own magnitude is not the scale of its rounding error; DESIGN.md
-    section 6), lengths relative to themselves, positions relative to max(|x|, s), unit vectors absolutely.
-    Directions are divided by 1 + 2e-3 gamma (gamma = E_in / me): emission angles are ~1/gamma and are
-    formed from 1 - mu, so their rounding error is ~ eps_mach gamma.  `skip` masks states excluded from the
-    floating-point comparison (they still count for the integers).
-    Returns (n_int_mismatch, worst_rel, report) over all states."""
+    section 6), path lengths and positions relative to X = max(|x|, s), unit vectors absolutely.  `tol` =
+    step_tolerances(...) (default: RTOL2 everywhere).  `skip` masks states excluded from the floating-point
+    comparison (they still count for the integers).
+    Returns (n_int_mismatch, worst error / tolerance, report) over all states."""
     n = len(ref["E"])
-    int_keys = ("step", "vol", "surf", "alive", "action", "process", "n_sec", "n_draws", "null_int", "rest")
+    if tol is None:
+        tol = dict(x=np.full(n, RTOL2), u=np.full(n, RTOL2), E=np.full(n, RTOL2))
+    int_keys = ("step", "vol", "surf", "alive", "action", "process", "n_sec", "n_draws", "null_int", "rest", "n_sub")
     bad = np.zeros(n, dtype=bool)
     report = {}
     for k in int_keys:
@@ -131,40 +184,31 @@ def compare_steps(ref, got, E_in, skip=None):
         if m.any():
             report[k] = int(m.sum())
         bad |= m
-    worst = 0.0
-    tiny = 1e-300
-
-    def rel(a, b, scale=None):
-        sc = np.maximum(np.abs(a), tiny) if scale is None else scale
-        return np.abs(a - b) / sc
-
     ok = ~bad
     if skip is not None:
         ok &= ~np.asarray(skip, dtype=bool)
     Es = np.asarray(E_in, dtype=np.float64)[ok]
-    cond = 1.0 + 2e-3 * Es / ME
+    tx, tu, tE = tol["x"][ok], tol["u"][ok], tol["E"][ok]
+
+    def ratio(err, t):
+        r = err / t
+        return float(r.max()) if r.size else 0.0
+
     for k in ("E", "edep", "below_cut", "escaped", "looper"):
-        r = rel(ref[k][ok], got[k][ok], np.maximum(np.abs(ref[k][ok]), Es))
-        w = float(r.max()) if r.size else 0.0
-        report["rel_" + k] = w
-        worst = max(worst, w)
+        err = np.abs(ref[k][ok] - got[k][ok]) / np.maximum(np.abs(ref[k][ok]), Es)
+        report["E:" + k] = ratio(err, tE)
     fin = np.isfinite(ref["s"][ok])
-    r = rel(ref["s"][ok][fin], got["s"][ok][fin])
-    report["rel_s"] = float(r.max()) if r.size else 0.0
-    r = rel(ref["msc_tau"][ok][fin], got["msc_tau"][ok][fin])
-    report["rel_msc_tau"] = float(r.max()) if r.size else 0.0
-    xs = np.maximum(np.linalg.norm(ref["x"][ok], axis=1), np.where(fin, np.abs(ref["s"][ok]), 0.0))
-    d = np.linalg.norm(ref["x"][ok] - got["x"][ok], axis=1)
-    d = d[fin] / np.maximum(xs[fin], 1e-30)
-    report["rel_x"] = float(d.max()) if d.size else 0.0
-    d = np.linalg.norm(ref["u"][ok] - got["u"][ok], axis=1) / cond
-    report["abs_u"] = float(d.max()) if d.size else 0.0
-    r = rel(ref["sec_E"][ok], got["sec_E"][ok], np.maximum(np.abs(ref["sec_E"][ok]), Es[:, None]))
-    report["rel_sec_E"] = float(r.max()) if r.size else 0.0
-    d = np.linalg.norm(ref["sec_u"][ok] - got["sec_u"][ok], axis=2) / cond[:, None]
-    report["abs_sec_u"] = float(d.max()) if d.size else 0.0
-    d = np.linalg.norm(ref["sec_x"][ok] - got["sec_x"][ok], axis=2)
-    d = d[fin] / np.maximum(xs[fin], 1e-30)[:, None]
-    report["rel_sec_x"] = float(d.max()) if d.size else 0.0
-    worst = max(report[k] for k in report if k.startswith("rel_") or k.startswith("abs_"))
+    X = np.maximum(np.maximum(np.linalg.norm(ref["x"][ok], axis=1), np.where(fin, np.abs(ref["s"][ok]), 0.0)), 1e-300)
+    report["s"] = ratio((np.abs(ref["s"][ok] - got["s"][ok]) / X)[fin], tx[fin])
+    mt = np.maximum(np.abs(ref["msc_tau"][ok]), 1e-300)
+    report["msc_tau"] = ratio(np.abs(ref["msc_tau"][ok] - got["msc_tau"][ok]) / mt, tx)
+    report["x"] = ratio((np.linalg.norm(ref["x"][ok] - got["x"][ok], axis=1) / X)[fin], tx[fin])
+    report["u"] = ratio(np.linalg.norm(ref["u"][ok] - got["u"][ok], axis=1), tu)
+    err = np.abs(ref["sec_E"][ok] - got["sec_E"][ok]) / np.maximum(np.abs(ref["sec_E"][ok]), Es[:, None])
+    report["sec_E"] = ratio(err.max(axis=1) if err.size else err, tE)
+    err = np.linalg.norm(ref["sec_u"][ok] - got["sec_u"][ok], axis=2)
+    report["sec_u"] = ratio(err.max(axis=1) if err.size else err, tu)
+    err = np.linalg.norm(ref["sec_x"][ok] - got["sec_x"][ok], axis=2) / X[:, None]
+    report["sec_x"] = ratio(err.max(axis=1)[fin] if err.size else err, tx[fin])
+    worst = max(v for k, v in report.items() if isinstance(v, float))
     return int(bad.sum()), worst, report
