@@ -279,13 +279,23 @@ int emx_set_primary_offset(emx_problem *p, long first);
  *                  than slice_above tracks are live (< 0: n_slots / 32), a propagation that has used slice_min
  *                  substep attempts in this iteration is parked for the next one as soon as its pool has no
  *                  unstarted track left, and after slice_max attempts in any case.  Defaults 2 / 16 / -1.
+ *   mev_per_slot   primaries are admitted while the shower energy in flight (admitted - deposited - escaped) is below
+ *                  mev_per_slot x n_slots: the energy in flight is what fills the slots and, beyond them, the queue
+ *                  (PAPER.md:204-206).  <= 0: 20 MeV.
+ *   admit_below    primaries are admitted (in waves of n_slots / 256, 256..4096) only while fewer records than this
+ *                  wait on the stacks (the queue is the memory limit); <= 0: 2 n_slots.
  *   blocks_per_sm  persistent 128-thread blocks per SM of each step kernel, in the order k_a<gamma>,
- *                  k_a<charged>, k_a0, k_field, k_a2, k_b<gamma>, k_b<charged> (entry 7 unused); 0 = default. */
+ *                  k_a<charged>, k_a0, k_field, k_a2, k_b<gamma>, k_b<charged>; 0 = default.  Entry 7 is a switch:
+ *                  1 = k_field stages the geometry's face table in shared memory instead of reading it through L1
+ *                  (measured 1-3 % SLOWER on B200, profiles/r2_staging.md: kept for that comparison). */
 typedef struct {
     int32_t loop_node;
     int32_t slice_min, slice_max;
     int64_t slice_above;
     int32_t blocks_per_sm[8];
+    int64_t admit_below;
+    int32_t mev_per_slot;
+    int32_t reserved;
 } emx_schedule;
 int emx_get_schedule(const emx_problem *p, emx_schedule *out);
 int emx_set_schedule(emx_problem *p, const emx_schedule *in);

@@ -21,6 +21,7 @@ struct emx_problem {
     int *d_surf_type = nullptr;
     double *d_surf_v = nullptr;
     Volume *d_vol = nullptr;
+    Face *d_faces = nullptr;
     double *d_tab = nullptr;
     double *d_scratch = nullptr;
     int *d_nb_off = nullptr, *d_nb_list = nullptr, *d_nb2_off = nullptr, *d_nb2_list = nullptr;
@@ -91,8 +92,6 @@ void free_device(emx_problem *p) {
     p->hp.built = false;
 }
 
-const double kQueueFrac[kPools] = {0.30, 0.70};  // e+- secondaries dominate the queued records in every config
-
 struct Carve {
     char *base;
     size_t off = 0;
@@ -105,15 +104,6 @@ struct Carve {
     }
 };
 
-// stack capacities: the two shares of queue_capacity, each at least one chunk
-void split_queue(long qcap, int out[kPools]) {
-    for (int k = 0; k < kPools; ++k) {
-        long v = (long)((double)qcap * kQueueFrac[k]);
-        if (v < kChunk) v = kChunk;
-        out[k] = (int)v;
-    }
-}
-
 // carve the caller's workspace; with base == nullptr only the size is computed
 size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
     Carve c{base};
@@ -122,7 +112,7 @@ size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
     w.n_chunks = nch;
     w.slot_cap = nch * kChunk;
     w.pool_reserve = nch / 32 > 1 ? nch / 32 : 1;
-    split_queue(qcap, w.qcap);
+    w.qtotal = (int)qcap;
     w.ctl = c.take<Ctl>(1);
     w.log = c.take<uint32_t>(2 * (size_t)max_log);
     w.max_log = max_log;
@@ -146,9 +136,9 @@ size_t carve_work(char *base, long n_slots, long qcap, Work &w, int max_log) {
     }
     // everything above (track store, scan arrays, interaction lists: about 150 MB of addresses at 2^20 slots, of
     // which an iteration touches what the live tracks need) is kept together; the stacks follow
-    for (int p = 0; p < kPools; ++p) {
-        const size_t q = (size_t)w.qcap[p];
-        Stack &s = w.q[p];
+    {
+        const size_t q = (size_t)w.qtotal;
+        Stack &s = w.q;
         s.xy = c.take<double2>(q); s.zu = c.take<double2>(q); s.uu = c.take<double2>(q);
         s.Et = c.take<double2>(q);
         s.id = c.take<int4>(q);
@@ -181,6 +171,9 @@ int emx_create(emx_problem **out) {
     p->sched.slice_min = 2;
     p->sched.slice_max = 16;
     p->sched.slice_above = -1;
+    p->sched.admit_below = 0;
+    p->sched.mev_per_slot = 0;
+    p->sched.reserved = 0;
     for (int k = 0; k < 8; ++k) p->sched.blocks_per_sm[k] = 0;
     *out = p;
     return EMX_OK;
@@ -324,6 +317,7 @@ int emx_build_tables(emx_problem *p, void *stream) {
         p->d_surf_type = cv.take<int>(ns ? ns : 1);
         p->d_surf_v = cv.take<double>(ns ? ns : 1);
         p->d_vol = cv.take<Volume>(nv);
+        p->d_faces = cv.take<Face>(nv * EMX_MAX_FACES);
         p->d_tab = cv.take<double>((nm ? nm : 1) * EMX_NTABLE * n);
         p->d_scratch = cv.take<double>((nm ? nm : 1) * n);
         p->d_nb_off = cv.take<int>(nb_off.size());
@@ -344,6 +338,20 @@ int emx_build_tables(emx_problem *p, void *stream) {
         CU(cudaMemcpyAsync(p->d_surf_v, hp.surf_v.data(), ns * sizeof(double), cudaMemcpyHostToDevice, st));
     }
     CU(cudaMemcpyAsync(p->d_vol, hp.vol.data(), nv * sizeof(Volume), cudaMemcpyHostToDevice, st));
+    std::vector<Face> faces(nv * EMX_MAX_FACES);  // the cells' face lists resolved against the surface table
+    memset(faces.data(), 0, faces.size() * sizeof(Face));
+    for (size_t iv = 0; iv < nv; ++iv) {
+        const Volume &v = hp.vol[iv];
+        for (int i = 0; i < v.n_faces; ++i) {
+            Face &f = faces[iv * EMX_MAX_FACES + i];
+            f.S = v.surf[i];
+            f.v = hp.surf_v[v.surf[i]];
+            f.type = (int8_t)hp.surf_type[v.surf[i]];
+            f.sense = (int8_t)v.sense[i];
+        }
+        faces[iv * EMX_MAX_FACES].n = (int16_t)v.n_faces;
+    }
+    CU(cudaMemcpyAsync(p->d_faces, faces.data(), faces.size() * sizeof(Face), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(p->d_nb_off, nb_off.data(), nb_off.size() * sizeof(int), cudaMemcpyHostToDevice, st));
     if (!nb_list.empty())
         CU(cudaMemcpyAsync(p->d_nb_list, nb_list.data(), nb_list.size() * sizeof(int), cudaMemcpyHostToDevice, st));
@@ -377,6 +385,7 @@ int emx_build_tables(emx_problem *p, void *stream) {
     P.surf_type = p->d_surf_type;
     P.surf_v = p->d_surf_v;
     P.vol = p->d_vol;
+    P.faces = p->d_faces;
     P.tab = p->d_tab;
     P.nb_off = p->d_nb_off;
     P.nb_list = p->d_nb_list;
@@ -452,7 +461,7 @@ int emx_reset_tallies(emx_problem *p, void *stream) {
 // bounds allow, shared between the chains that run side by side
 static void size_grids(const emx_problem *p, Work &w) {
     // defaults per stage (kStage*): 128-thread blocks per SM
-    static const int kDefault[kNStages] = {3, 4, 8, 5, 5, 3, 3};
+    static const int kDefault[kNStages] = {4, 4, 8, 5, 5, 4, 4};
     for (int k = 0; k < kNStages; ++k) {
         int b = p->sched.blocks_per_sm[k] > 0 ? p->sched.blocks_per_sm[k] : kDefault[k];
         if (b > 16) b = 16;
@@ -473,15 +482,16 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     memset(&w, 0, sizeof(w));  // compared bytewise with the arguments of the kept graph
     const size_t need = carve_work((char *)workspace, n_slots, queue_capacity, w, kMaxLog);
     if (need > workspace_bytes) return fail(p, EMX_E_CAPACITY, "emx_transport: workspace smaller than emx_workspace_bytes()");
-    // admission limits (R8): about 20 MeV of shower energy in flight per queued record at the peak of
-    // the queue (measured on configs 1-4), with a factor 4 of headroom below the capacity
+    // admission limits (R8): the shower energy in flight is what fills the slots and then the queue
     w.n_primaries = pr.n;
     w.wave = (int)(n_slots / 256 < 256 ? 256 : (n_slots / 256 > 4096 ? 4096 : n_slots / 256));
-    w.inflight_cap = 5.0 * (double)queue_capacity;
+    w.inflight_cap = (p->sched.mev_per_slot > 0 ? (double)p->sched.mev_per_slot : 20.0) * (double)n_slots;
+    w.admit_below = p->sched.admit_below > 0 ? p->sched.admit_below : 2 * n_slots;
     w.slice_above = p->sched.slice_above >= 0 ? p->sched.slice_above : n_slots / 32;
     w.slice_min = p->sched.slice_min > 0 ? p->sched.slice_min : 1;
     w.slice_max = p->sched.slice_max >= w.slice_min ? p->sched.slice_max : w.slice_min;
     size_grids(p, w);
+    w.stage_faces = p->sched.blocks_per_sm[7] == 1 ? 1 : 0;  // entry 7 of the schedule: 1 switches the staging on
     const bool field = p->P.Bmag != 0.0;
     const int per_iter = launches_per_iteration(field);
     CU(cudaEventRecord(p->ev0, st));

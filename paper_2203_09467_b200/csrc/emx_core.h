@@ -47,6 +47,16 @@ struct Volume {
     int material, tally;
 };
 
+// One face of a cell with everything the navigation needs in one 16-byte word: the cells' face lists resolved
+// against the surface table once, on the host (faces[vol * EMX_MAX_FACES + i]; n of face 0 = faces of the cell)
+struct Face {
+    double v;      // plane position or cylinder radius
+    int S;         // surface id
+    int8_t type;   // EMX_S_*
+    int8_t sense;  // side of the surface the cell is on
+    int16_t n;     // face 0 only: number of faces of the cell
+};
+
 // Read-only problem data ("params" in the paper's params/state split), passed to
 // kernels by value; the pointers refer to the problem's one small device block.
 struct Params {
@@ -56,6 +66,7 @@ struct Params {
     const int *surf_type;
     const double *surf_v;
     const Volume *vol;
+    const Face *faces;      // [n_vol][EMX_MAX_FACES]
     const double *tab;      // [n_mat][EMX_NTABLE][n_E]
     const int *nb_off;      // neighbour candidates: cells having face (S, sense); index 2*S + (sense > 0)
     const int *nb_list;

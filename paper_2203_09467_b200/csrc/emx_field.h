@@ -133,11 +133,12 @@ EMX_HD void field_begin(double kappa, double s_max, FieldState &fs) {
     fs.attempt = 0;
 }
 
-// ONE attempt of the substep loop of C9 inside cell `vol`, towards the arc length s_max.  x, u, on_surf (the surface
+// ONE attempt of the substep loop of C9 inside one cell, towards the arc length s_max.  x, u, on_surf (the surface
 // the track sits on) and fs are updated.  Returns true when the propagation is over: s = arc length travelled,
 // hit = surface reached (-1 none: s_max travelled, or the max_substeps attempts of the step are used up).
+// cell = the faces of the track's cell (Params::faces, or the kernel's copy of it in shared memory).
 template <bool MAP, int AX>
-EMX_NI bool field_attempt(const Params &P, int vol, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
+EMX_NI bool field_attempt(const Params &P, const Face *cell, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
                           FieldState &fs, int &hit, double &s) {
     const double eps = P.ph.field_eps;
     const double rem = s_max - fs.s_done;
@@ -165,7 +166,7 @@ EMX_NI bool field_attempt(const Params &P, int vol, int &on_surf, Vec3 &x, Vec3 
         }
         const Vec3 cd = {c.x / L, c.y / L, c.z / L};
         int S;
-        const double d = distance_to_boundary(P, vol, x, cd, on_surf, S);
+        const double d = distance_to_faces(cell, x, cd, on_surf, S);
         if (d <= eps) {
             // chord bends back across the surface the track sits on: shorten and retry
             if (d == 0.0 && S == on_surf && h > 1e-9) {
@@ -231,11 +232,12 @@ EMX_NI double propagate_field(const Params &P, int vol, int &on_surf, Vec3 &x, V
     const double kb = ax == kAxisAny ? kappa : kappa * P.Bhat[ax];
     bool done = false;
     n_attempts = 0;
+    const Face *cell = P.faces + (size_t)vol * EMX_MAX_FACES;
     while (!done) {
-        if (MAP || ax == kAxisAny) done = field_attempt<MAP, kAxisAny>(P, vol, on_surf, x, u, kappa, s_max, fs, hit, s);
-        else if (ax == 0) done = field_attempt<false, 0>(P, vol, on_surf, x, u, kb, s_max, fs, hit, s);
-        else if (ax == 1) done = field_attempt<false, 1>(P, vol, on_surf, x, u, kb, s_max, fs, hit, s);
-        else done = field_attempt<false, 2>(P, vol, on_surf, x, u, kb, s_max, fs, hit, s);
+        if (MAP || ax == kAxisAny) done = field_attempt<MAP, kAxisAny>(P, cell, on_surf, x, u, kappa, s_max, fs, hit, s);
+        else if (ax == 0) done = field_attempt<false, 0>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
+        else if (ax == 1) done = field_attempt<false, 1>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
+        else done = field_attempt<false, 2>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
         ++n_attempts;
     }
     return s;

@@ -17,27 +17,27 @@ EMX_HD double surf_g(int type, const Vec3 &x, const Vec3 &u) {
     return comp(u, type);
 }
 
-// Distance along u from x to the nearest face of cell `vol`; on_surf = surface the track is flagged on
-// (-1 none).  Returns +inf and hit = -1 when no face is ahead.  Ties -> lowest surface id.
-EMX_NI double distance_to_boundary(const Params &P, int vol, const Vec3 &x, const Vec3 &u, int on_surf, int &hit) {
-    const Volume &c = P.vol[vol];
+// Distance along u from x to the nearest face of the cell whose faces are cell[0 .. cell[0].n); on_surf = surface
+// the track is flagged on (-1 none).  Returns +inf and hit = -1 when no face is ahead.  Ties -> lowest surface id.
+EMX_NI double distance_to_faces(const Face *cell, const Vec3 &x, const Vec3 &u, int on_surf, int &hit) {
     double best = kInf;
     int bs = -1;
     // cylinder coefficients shared by every CZ face of the cell
     const double a = u.x * u.x + u.y * u.y;
     const double b = x.x * u.x + x.y * u.y;
     const double rr = x.x * x.x + x.y * x.y;
-    const int nf = c.n_faces;
+    const int nf = cell[0].n;
     for (int i = 0; i < nf; ++i) {
-        const int S = c.surf[i];
-        const int type = P.surf_type[S];
-        const double v = P.surf_v[S];
+        const Face f = cell[i];
+        const int S = f.S;
+        const int type = f.type;
+        const double v = f.v;
         double d = -1.0;
         bool have = false;
         if (S == on_surf) {
             const double g = (type == EMX_S_CZ) ? 2.0 * b : comp(u, type);
             const int ns = g > 0.0 ? 1 : -1;
-            if (ns != c.sense[i]) {  // heading back across the surface it sits on
+            if (ns != f.sense) {  // heading back across the surface it sits on
                 d = 0.0;
                 have = true;
             } else if (type == EMX_S_CZ && a > 0.0) {  // on the cylinder: c0 = 0 exactly, roots 0 and -2b/a
@@ -73,25 +73,29 @@ EMX_NI double distance_to_boundary(const Params &P, int vol, const Vec3 &x, cons
     hit = bs;
     return best;
 }
+EMX_HD double distance_to_boundary(const Params &P, int vol, const Vec3 &x, const Vec3 &u, int on_surf, int &hit) {
+    return distance_to_faces(P.faces + (size_t)vol * EMX_MAX_FACES, x, u, on_surf, hit);
+}
 
 // does cell c contain the point just across S (entered with sense `newsense`)?  Faces within the
 // tolerance take their sense from the direction of motion (C8).
 EMX_HD bool cell_matches(const Params &P, int cid, const Vec3 &x, const Vec3 &u, int S, int newsense) {
-    const Volume &c = P.vol[cid];
-    for (int i = 0; i < c.n_faces; ++i) {
-        const int Sf = c.surf[i];
+    const Face *cell = P.faces + (size_t)cid * EMX_MAX_FACES;
+    const int nf = cell[0].n;
+    for (int i = 0; i < nf; ++i) {
+        const Face fc = cell[i];
         int sn;
-        if (Sf == S) {
+        if (fc.S == S) {
             sn = newsense;
         } else {
-            const int type = P.surf_type[Sf];
-            const double v = P.surf_v[Sf];
+            const int type = fc.type;
+            const double v = fc.v;
             const double f = surf_f(type, v, x);
             const double tol = (type == EMX_S_CZ) ? 2e-9 * v : 1e-9;
             if (fabs(f) <= tol) sn = surf_g(type, x, u) > 0.0 ? 1 : -1;
             else sn = f > 0.0 ? 1 : -1;
         }
-        if (sn != c.sense[i]) return false;
+        if (sn != fc.sense) return false;
     }
     return true;
 }

@@ -27,8 +27,9 @@ __device__ __forceinline__ uint64_t tid_of(double2 Et) { return (uint64_t)__doub
 
 // A0: record r of stack `pool` becomes the track in physical slot s
 template <int POOL>
-__device__ __forceinline__ void load_record(const Work &w, int r, int s) {
-    const Stack &q = w.q[POOL];
+__device__ __forceinline__ void load_record(const Work &w, int r_stack, int s) {
+    const Stack &q = w.q;
+    const int r = qrec(w, POOL, r_stack);
     const Store &t = w.st;
     t.xy[s] = ld_cs(&q.xy[r]);
     t.zu[s] = ld_cs(&q.zu[r]);
@@ -119,23 +120,24 @@ __global__ void __launch_bounds__(1024) k_init(Work w, Primaries pr) {
 // refill that follows.  Histories do not depend on when a primary is admitted (keyed RNG, C2); admission only
 // bounds the number of queued records (the queue had to hold 2.5e7 initializers).
 // Returns (to every thread) the number of primaries admitted.
-__device__ __forceinline__ int admit_block(const Work &w, const Primaries &pr) {
+__device__ __forceinline__ int admit_block(const Work &w, const Primaries &pr, Ctl *c) {
     __shared__ int s_cnt[kPools][32];
     __shared__ int s_total[kPools], s_base[kPools];
     __shared__ double s_E[32];
     __shared__ long long s_A;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
-    Ctl *c = w.ctl;
     if (c->done) return 0;
     const long long next = c->next_primary;
     if (next >= pr.n) return 0;
     const double inflight = c->E_admitted - (c->edep_total + c->escaped + c->looper);
     if (inflight >= w.inflight_cap) return 0;
     long long A = (pr.n - next) < (long long)w.wave ? (pr.n - next) : (long long)w.wave;
-    for (int p = 0; p < kPools; ++p) {
-        if (c->q_top[p] > 0 && 4LL * c->q_top[p] >= (long long)w.qcap[p]) return 0;  // a quarter full: let it drain first
-        const long long room = (long long)w.qcap[p] - c->q_top[p];
-        if (A > room) A = room;  // a wave never asks a stack for more than it can hold (no count exceeds A)
+    {
+        const long long queued = (long long)c->q_top[0] + c->q_top[1];
+        if (queued > 0 && 4LL * queued >= (long long)w.qtotal) return 0;  // the arena is a quarter full: let it drain first
+        if (queued >= w.admit_below) return 0;  // enough records wait to keep every slot busy: more would only sit in HBM
+        const long long room = (long long)w.qtotal - queued;
+        if (A > room) A = room;  // a wave never asks for more than the arena can hold
     }
     if (A <= 0) return 0;
     // pass 1: energy of the window and its primaries per pool
@@ -180,8 +182,8 @@ __device__ __forceinline__ int admit_block(const Work &w, const Primaries &pr) {
         if (pl >= 0) {
             int before = s_base[pl];
             for (int q = 0; q < wid; ++q) before += s_cnt[pl][q];
-            const int r = c->q_top[pl] + s_total[pl] - 1 - (before + rank);  // lowest index on top
-            const Stack &q = w.q[pl];
+            const int r = qrec(w, pl, c->q_top[pl] + s_total[pl] - 1 - (before + rank));  // lowest index on top
+            const Stack &q = w.q;
             q.xy[r] = make_double2(pr.pos3[3 * i], pr.pos3[3 * i + 1]);
             q.zu[r] = make_double2(pr.pos3[3 * i + 2], pr.dir3[3 * i]);
             q.uu[r] = make_double2(pr.dir3[3 * i + 1], pr.dir3[3 * i + 2]);
@@ -228,11 +230,16 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
     constexpr int kGroupWarps = 16;  // warps 0-15 scan the photon pool, 16-31 the charged pool (side by side)
     __shared__ int s_warp[kPools][kGroupWarps];
     __shared__ int s_h[kPools], s_grant[kPools], s_owned[kPools], s_free;
+    // the loop state is worked on in shared memory: one coalesced read and one write of the head of the control block
+    // instead of a chain of dependent round trips to L2 for every field thread 0 touches
+    __shared__ unsigned long long s_head[kCtlHead / 8];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    Ctl *c = w.ctl;
-    if (c->done) return;
+    if (w.ctl->done) return;
+    for (int k = tid; k < (int)(kCtlHead / 8); k += blockDim.x) s_head[k] = reinterpret_cast<const unsigned long long *>(w.ctl)[k];
+    __syncthreads();
+    Ctl *c = reinterpret_cast<Ctl *>(s_head);
     EMX_TL(w, 0, 0, 0);
-    const int admitted = admit_block(w, pr);
+    const int admitted = admit_block(w, pr, c);
     __syncthreads();
     {
         const int p = wid / kGroupWarps, wig = wid % kGroupWarps;  // pool of this warp, warp index in its group
@@ -361,7 +368,7 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
         const long long queued = (long long)c->q_top[0] + c->q_top[1];
         // a track pushes at most 4 records in an iteration (two products and two at-rest photons): where even that
         // fits, the step kernels reserve with one atomic and no look at the top first
-        for (int p = 0; p < kPools; ++p) c->q_safe[p] = ((long long)c->q_top[p] + 4LL * live <= (long long)w.qcap[p]) ? 1 : 0;
+        c->q_safe[0] = c->q_safe[1] = (queued + 4LL * live <= (long long)w.qtotal) ? 1 : 0;
         if ((unsigned long long)live > c->peak_live) c->peak_live = (unsigned long long)live;
         if ((unsigned long long)queued > c->peak_queue) c->peak_queue = (unsigned long long)queued;
         if (c->iter < (unsigned long long)w.max_log) {
@@ -401,6 +408,8 @@ __global__ void __launch_bounds__(1024) k_plan(Work w, Primaries pr) {
                 for (int k = 0; k < kMaxLists; ++k) c->icount[p][k] = 0;
         }
     }
+    __syncthreads();
+    for (int k = tid; k < (int)(kCtlHead / 8); k += blockDim.x) reinterpret_cast<unsigned long long *>(w.ctl)[k] = s_head[k];
 }
 
 // rank of slot i among the dead slots of its chunk (exclusive), for a block that covers one chunk
@@ -510,7 +519,8 @@ constexpr int kStepBlock = 128;
 template <int POOL>
 __device__ __forceinline__ void push_record(const Work &w, int r, const Vec3 &x, const Vec3 &u, double E, uint64_t tid,
                                             uint32_t prim, int vol, int ptype) {
-    const Stack &q = w.q[POOL];
+    const Stack &q = w.q;
+    r = qrec(w, POOL, r);
     st_cs(&q.xy[r], make_double2(x.x, x.y));
     st_cs(&q.zu[r], make_double2(x.z, u.x));
     st_cs(&q.uu[r], make_double2(u.y, u.z));
@@ -554,28 +564,35 @@ __device__ __forceinline__ void flush_acc(Ctl *c, const WarpAcc &acc, int lane, 
     }
 }
 
-// Reserve `cnt` records (warp total) on stack `pool`; returns the base index or -1 when the stack is full.
+// Reserve `cnt` records (warp total) on stack `pool`; returns the base index or -1 when the arena is full.
 // Far from the capacity one atomicAdd does it: w.reserve_slack bounds what all resident warps of
 // the step kernels can request at the same time (one outstanding reservation of <= 128 records each), so
-// the top cannot pass the capacity.  Near the capacity a small stack (tests) is reserved by compare-and-swap,
-// which never moves the top past the capacity; a large stack is simply treated as full.  Nothing is ever rolled
+// the stacks cannot meet.  Near the capacity a small arena (tests) is reserved by compare-and-swap,
+// which never lets the two tops pass the capacity; a large arena is simply treated as full.  Nothing is ever rolled
 // back: an add-then-subtract scheme lets a reservation succeed above a top that a concurrent failure has
 // inflated, and strands its records.
 __device__ __forceinline__ int reserve(Ctl *c, const Work &w, int pool, int cnt, bool safe) {
-    const int cap = w.qcap[pool];
-    if (safe) return atomicAdd(&c->q_top[pool], cnt);  // k_plan's guarantee for this iteration: one round trip to the top
-    int old = *(volatile int *)&c->q_top[pool];
-    if ((long long)old + cnt + w.reserve_slack <= (long long)cap) return atomicAdd(&c->q_top[pool], cnt);
-    if ((long long)cap < 8LL * w.reserve_slack) {
-        // small stack: exact accounting by compare-and-swap
-        while (old + cnt <= cap) {
-            const int prev = atomicCAS(&c->q_top[pool], old, old + cnt);
-            if (prev == old) return old;
+    // the two tops are the halves of one 64-bit word: one atomic moves one of them and returns both, so "do the two
+    // stacks still fit the arena" is always decided on a consistent pair
+    unsigned long long *tops = reinterpret_cast<unsigned long long *>(&c->q_top[0]);
+    const int sh = 32 * pool;
+    const unsigned long long inc = (unsigned long long)cnt << sh;
+    const long long cap = w.qtotal;
+    if (safe) return (int)((atomicAdd(tops, inc) >> sh) & 0xffffffffull);  // k_plan's guarantee for this iteration
+    unsigned long long old = *(volatile unsigned long long *)tops;
+    long long used = (long long)(old & 0xffffffffull) + (long long)(old >> 32);
+    if (used + cnt + w.reserve_slack <= cap) return (int)((atomicAdd(tops, inc) >> sh) & 0xffffffffull);
+    if (cap < 8LL * w.reserve_slack) {
+        // small arena: exact accounting by compare-and-swap
+        while (used + cnt <= cap) {
+            const unsigned long long prev = atomicCAS(tops, old, old + inc);
+            if (prev == old) return (int)((old >> sh) & 0xffffffffull);
             old = prev;
+            used = (long long)(old & 0xffffffffull) + (long long)(old >> 32);
         }
     }
-    // large stack within the slack of its capacity: treated as full (thousands of warps spinning on
-    // one compare-and-swap cost 10x the iteration; the last 2 % of a large stack are not worth it)
+    // large arena within the slack of its capacity: treated as full (thousands of warps spinning on
+    // one compare-and-swap cost 10x the iteration; the last 2 % of a large arena are not worth it)
     return -1;
 }
 
@@ -663,9 +680,9 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
     }
     if (stall) {
         if (r_c >= 0)
-            for (int k = 0; k < nc; ++k) w.q[kPoolCharged].Et[r_c + k] = make_double2(-1.0, 0.0);
+            for (int k = 0; k < nc; ++k) w.q.Et[qrec(w, kPoolCharged, r_c + k)] = make_double2(-1.0, 0.0);
         if (r_g >= 0)
-            for (int k = 0; k < ng; ++k) w.q[kPoolGamma].Et[r_g + k] = make_double2(-1.0, 0.0);
+            for (int k = 0; k < ng; ++k) w.q.Et[qrec(w, kPoolGamma, r_g + k)] = make_double2(-1.0, 0.0);
     } else {
         const uint32_t k0 = (uint32_t)seed;
         if (nc) {
@@ -992,7 +1009,18 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_0) k_a0(const __grid_co
 // attempts once the pool has no track left to hand out (or after slice_max attempts): its loop variables go to
 // the slot and the next iteration continues the SAME sequence of substeps.
 template <bool MAP, int AX>
-__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid_constant__ Params P, const __grid_constant__ Work w) {
+__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid_constant__ Params P, const __grid_constant__ Work w,
+                                                                    int stage_faces) {
+    // the face table of the whole geometry (16 B per face) is staged in shared memory when it fits: every attempt
+    // reads the faces of its cell (B:north_star "shared-memory ... staging of the hot table slices")
+    extern __shared__ double2 s_faces2[];
+    const Face *faces = P.faces;
+    if (stage_faces) {
+        const double2 *src = reinterpret_cast<const double2 *>(P.faces);
+        for (int k = threadIdx.x; k < P.n_vol * EMX_MAX_FACES; k += blockDim.x) s_faces2[k] = src[k];
+        __syncthreads();
+        faces = reinterpret_cast<const Face *>(s_faces2);
+    }
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -1048,7 +1076,7 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid
         if (have) {
             int hit;
             double sres;
-            const bool done = field_attempt<MAP, AX>(P, vol, surf, x, u, kappa, s_max, fs, hit, sres);
+            const bool done = field_attempt<MAP, AX>(P, faces + vol * EMX_MAX_FACES, surf, x, u, kappa, s_max, fs, hit, sres);
             used += 1;
             n_att += 1;
             if (done) {
@@ -1217,11 +1245,15 @@ cudaError_t launch_stage(int stage, const Params &P, const Work &w, uint64_t see
         break;
     case kStageField: {
         const int ax = P.field_kind == 0 ? field_axis(P.Bhat) : kAxisAny;
-        if (P.field_kind != 0) k_field<true, kAxisAny><<<g, kStepBlock, 0, st>>>(P, w);
-        else if (ax == 0) k_field<false, 0><<<g, kStepBlock, 0, st>>>(P, w);
-        else if (ax == 1) k_field<false, 1><<<g, kStepBlock, 0, st>>>(P, w);
-        else if (ax == 2) k_field<false, 2><<<g, kStepBlock, 0, st>>>(P, w);
-        else k_field<false, kAxisAny><<<g, kStepBlock, 0, st>>>(P, w);
+        // shared-memory copy of the face table: up to 40 KB per block (5 blocks per SM stay resident)
+        const size_t fb = (size_t)P.n_vol * EMX_MAX_FACES * sizeof(Face);
+        const int stage = (w.stage_faces && fb <= 40 * 1024) ? 1 : 0;
+        const size_t sm = stage ? fb : 0;
+        if (P.field_kind != 0) k_field<true, kAxisAny><<<g, kStepBlock, sm, st>>>(P, w, stage);
+        else if (ax == 0) k_field<false, 0><<<g, kStepBlock, sm, st>>>(P, w, stage);
+        else if (ax == 1) k_field<false, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);
+        else if (ax == 2) k_field<false, 2><<<g, kStepBlock, sm, st>>>(P, w, stage);
+        else k_field<false, kAxisAny><<<g, kStepBlock, sm, st>>>(P, w, stage);
         break;
     }
     case kStageA2:
@@ -1327,7 +1359,7 @@ cudaError_t launch_refill_plan(long n_live, long capacity, long n_queue, const u
     w.n_chunks = (int)((capacity + kChunk - 1) / kChunk);
     w.slot_cap = (int)capacity;
     w.pool_reserve = 0;
-    w.qcap[0] = w.qcap[1] = 0x7fffffff;
+    w.qtotal = 0x7fffffff;
     w.log = nullptr;
     w.max_log = 0;
     w.n_primaries = 0;

@@ -13,6 +13,7 @@
 // every access of a warp is a coalesced 16-byte-per-lane stream inside one chunk.
 #pragma once
 #include <cuda_runtime.h>
+#include <cstddef>
 #include "emx_core.h"
 
 namespace emx {
@@ -67,7 +68,7 @@ constexpr int kMaxLists = 4;  // interaction lists per pool: gamma Compton / pho
 
 struct Ctl {
     int n_live[kPools];
-    int q_top[kPools];
+    int q_top[kPools];   // records on each stack; the pair is also updated as ONE 64-bit word (8-byte aligned here)
     int m_step[kPools];  // tracks to step this iteration (= n_live)
     int q_safe[kPools];  // set by k_plan: stack p cannot overflow in this iteration whatever the step kernels push
     PoolPlan plan[kPools];
@@ -84,17 +85,22 @@ struct Ctl {
     double E_admitted;            // energy of the admitted primaries (e+ with their 2 me)
     double edep_total;            // all energy deposited so far (every cell, tallied or not)
     double escaped, below_cut, looper, E_in;
-    unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls, peak_live, peak_queue;
+    unsigned long long peak_live, peak_queue;
+    // ---- everything above is the loop state k_plan works on (it copies it to shared memory and back: kCtlHead);
+    // below are run totals that only the step kernels add to
+    unsigned long long steps[3], tracks[3], inter[EMX_NPROC], null_int, stalls;
     unsigned long long lanes[4][kPools];  // slots processed by the kernels a0 / field / a (or a2) / b, per pool
     unsigned long long attempts;          // substep attempts of the field propagation
     unsigned long long hist[3][EMX_NHIST];  // tracks by type and by the bin of the steps they took
 };
 
+constexpr size_t kCtlHead = offsetof(Ctl, steps);  // bytes of the loop state at the start of Ctl (a multiple of 8)
+
 struct Work {
     Store st;
-    Stack q[kPools];
+    Stack q;              // ONE arena for both stacks: photons grow up from record 0, e+- down from the last record
     int n_chunks;         // physical chunks of the store
-    int qcap[kPools];     // records per stack
+    int qtotal;           // records in the arena (what the two stacks may hold together)
     int *ctab[kPools];    // chunk tables, n_chunks entries each
     int *free_list;       // n_chunks entries
     int *rtab;            // physical chunk -> its index in the owning pool's chunk table
@@ -106,9 +112,11 @@ struct Work {
     uint32_t *log;  // per iteration: live, queued
     int max_log;
     // admission of primaries (R8): up to `wave` primaries enter per iteration while the energy in
-    // flight (admitted - deposited - escaped) is below inflight_cap and no stack is more than a quarter full
+    // flight (admitted - deposited - escaped) is below inflight_cap, fewer than admit_below records are queued and
+    // the arena is less than a quarter full
     long long n_primaries;
     int wave;
+    long long admit_below;  // no primaries are admitted while this many records are queued
     double inflight_cap;
     long long slice_above;  // live tracks above which the field propagation is time-sliced
     int slice_min;          // substep attempts per track and iteration before parking while sliced
@@ -116,8 +124,12 @@ struct Work {
     int grid[8];            // blocks of the persistent step kernels, by stage (emx_kernels.h: kStage*)
     int reserve_slack;      // records all resident warps can request at the same time (see reserve())
     int slot_cap;           // slots a pool may hold at most (= n_chunks * kChunk; smaller in the refill hook)
+    int stage_faces;        // 1: k_field keeps the geometry's face table in shared memory (emx_schedule)
     int pool_reserve;       // chunks a pool never takes, so that the other pool can always start (n_chunks / 32, >= 1)
 };
+
+// record r (counted from the bottom of its stack) of pool's stack in the shared arena
+__device__ __forceinline__ int qrec(const Work &w, int pool, int r) { return pool == kPoolGamma ? r : w.qtotal - 1 - r; }
 
 // physical slot of pool-local slot i
 __device__ __forceinline__ int phys_slot(const Work &w, int pool, int i) {

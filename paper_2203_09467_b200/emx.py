@@ -38,7 +38,7 @@ class Scalars(C.Structure):
 
 class Schedule(C.Structure):
     _fields_ = [("loop_node", C.c_int32), ("slice_min", C.c_int32), ("slice_max", C.c_int32), ("slice_above", C.c_int64),
-                ("blocks_per_sm", C.c_int32 * 8)]
+                ("blocks_per_sm", C.c_int32 * 8), ("admit_below", C.c_int64), ("mev_per_slot", C.c_int32), ("reserved", C.c_int32)]
 
 
 class Track(C.Structure):
@@ -289,11 +289,13 @@ class Problem:
 
     def set_schedule(self, **kw):
         """emx_set_schedule: loop_node, slice_min, slice_max, slice_above, blocks_per_sm (dict stage name -> blocks
-        or a list of 7).  Only what is named changes.  A schedule never changes a result."""
+        or a list of 7), stage_faces (bool).  Only what is named changes.  A schedule never changes a result."""
         sc = Schedule()
         self._check(lib().emx_get_schedule(self.h, C.byref(sc)))
         for k, v in kw.items():
-            if k == "blocks_per_sm":
+            if k == "stage_faces":
+                sc.blocks_per_sm[7] = 1 if v else 0
+            elif k == "blocks_per_sm":
                 items = v.items() if isinstance(v, dict) else zip(STAGES, v)
                 for name, b in items:
                     sc.blocks_per_sm[STAGES.index(name)] = int(b)

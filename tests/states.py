@@ -114,18 +114,25 @@ def step_tolerances(desc, tracks, ref):
     nothing observed: every entry is RTOL2 for a step without field substeps and without fluctuated loss.
 
     Field steps (n = substep attempts, from the oracle's own count).  Both implementations run the same IEEE
-    operations, but their libm differs in the last bit, so after the first substep the two positions differ by
-    ~EPS |x|.  The error estimate err = |x_full - x_half| is a difference of nearly equal positions: its relative
-    difference is EPS |x| / err, the next trial step h differs by a fifth of that (h ~ err^-1/5), and the RK4
-    truncation error of a substep (err / 15, fifth order in h) changes by 5 dh/h err / 15 = EPS |x| / 15: per substep
-    the end point moves by <= EPS |x| along the helix and the direction by <= |kappa| EPS |x|, whatever err is.
-      positions, path length   RTOL2 + 4 n EPS                       (relative to X = max(|x|, s))
-      directions               RTOL2 + n EPS X |kappa|
+    operations, but their libm differs in the last bit, so after the first rescaling of h the two positions differ by
+    a rounding, EPS |x|.  The error estimate err = |x_full - x_half| is a difference of two positions that each carry
+    a few such roundings (take 8 EPS |x| for the difference), so err differs by 8 EPS |x| / err relative, the next
+    trial step by a fifth of that (h ~ err^-1/5), and the RK4 truncation error of the substep (err / 15, fifth order in
+    h) by 5 dh/h err / 15 < 8 EPS |x|: per substep the end point moves by < 8 EPS |x| along the helix and the
+    direction by < |kappa| 8 EPS |x|, whatever err is.  With X = max(|x|, s):
+      positions, path length   RTOL2 + 8 n EPS              (relative to X)
+      directions               RTOL2 + 8 n EPS X |kappa|
+      energies                 RTOL2 + (path tolerance) X / s    (the loss of the step is proportional to its path)
     A step cut short by the substep budget (action TRUNC) returns s = sum of its n trial steps, each carrying
-    dh/h <= EPS |x| / (5 err) with err >= field_eps / 3125 where h still grows: ds/s <= 625 EPS X / field_eps, and
-    the direction turns by |kappa| ds.  In a NON-UNIFORM field the error estimate varies along the path, the two
-    substep sequences drift apart by the same dh/h and a boundary is reached at points up to the landing tolerance
-    apart: ds <= 2 field_eps for a step that ends on a surface.
+    dh/h <= 8 EPS |x| / (5 err) with err >= field_eps / 3125 where h still grows: ds/s <= 5000 EPS X / field_eps, and
+    the direction turns by |kappa| ds.
+    In a NON-UNIFORM field the error estimate changes along the path, so the two sequences of substeps do not stay
+    within roundings of each other: each run realises its own truncation errors (<= field_eps / 15 per accepted
+    substep, in position and again through the direction it leaves the substep with) and lands on a surface within
+    field_eps of it along its own chord: |dx| <= 4 (n / 15 + 1) field_eps.
+    Its TRUNC steps (the 1000-attempt emergency exit, vacuum only: no loss) stop at arc lengths that depend on all
+    1000 step sizes: several end points are correct (they lie on the same curve), so only ds <= 5e-2 s is asked, with
+    the position and direction differences that follow from ds.
     Energy-loss fluctuations: the fluctuated loss can take most of E, the post-loss energy E' = E - dE carries
     EPS E / E' of relative rounding and everything the interactor computes from E' inherits it: scale E / E'."""
     n = len(tracks)
@@ -137,20 +144,18 @@ def step_tolerances(desc, tracks, ref):
     p = np.sqrt(E * (E + 2 * ME))
     kappa = np.where(pt != 0, 2.99792458 * B / np.maximum(p, 1e-300), 0.0)
     fin = np.isfinite(ref["s"])
-    X = np.maximum(np.linalg.norm(ref["x"], axis=1), np.where(fin, np.abs(ref["s"]), 0.0))
-    tol_x = RTOL2 + 4 * nsub * EPS
-    tol_u = RTOL2 + nsub * EPS * X * kappa
-    tol_E = np.full(n, RTOL2)
-    eps_f = ph["field_eps"]
-    trunc = (ref["action"] == 4) & (nsub >= ph["max_substeps"])
-    ds_rel = 625 * EPS * X / eps_f                      # of s
     s_abs = np.where(fin, np.abs(ref["s"]), 0.0)
-    tol_x = np.where(trunc, tol_x + ds_rel * s_abs / np.maximum(X, 1e-300), tol_x)
-    tol_u = np.where(trunc, tol_u + kappa * ds_rel * s_abs, tol_u)
+    X = np.maximum(np.maximum(np.linalg.norm(ref["x"], axis=1), s_abs), 1e-300)
+    eps_f = ph["field_eps"]
+    path = 8 * nsub * EPS                               # relative to X
+    trunc = (ref["action"] == 4) & (nsub >= ph["max_substeps"])
+    path = np.where(trunc, path + 5000 * EPS * X / eps_f * s_abs / X, path)
     if desc.get("field_fringe"):
-        moved = nsub > 1
-        tol_x = np.where(moved, tol_x + 2 * eps_f / np.maximum(X, 1e-300), tol_x)
-        tol_u = np.where(moved, tol_u + kappa * 2 * eps_f, tol_u)
+        path = np.where(nsub > 1, path + 4 * (nsub / 15 + 1) * eps_f / X, path)
+        path = np.where(trunc, path + 5e-2 * s_abs / X, path)
+    tol_x = RTOL2 + path
+    tol_u = RTOL2 + kappa * path * X
+    tol_E = RTOL2 + np.where(s_abs > 0, path * X / np.maximum(s_abs, 1e-300), 0.0)
     if ph.get("fluct"):
         e_post = np.maximum(E - ref["edep"], 0.0)
         scale = np.where((pt != 0) & (e_post > 0), np.minimum(E / np.maximum(e_post, 1e-300), 1e6), 1.0)

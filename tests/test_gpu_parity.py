@@ -139,11 +139,11 @@ def test_single_step_parity(emx, emo, cfg, n):
     tol = states.step_tolerances(desc, tr, ref)
     n_bad, worst, rep = states.compare_steps(ref, got, E_in, tol)
     assert n_bad == 0, rep
-    assert worst <= 1.0, rep
-    plain = (ref["n_sub"] == 0) & (tol["E"] == states.RTOL2)
+    assert worst <= 1.0, {k: v for k, v in rep.items() if isinstance(v, float) and v > 0.5}
+    plain = (ref["n_sub"] == 0) & (tol["E"] == states.RTOL2)      # the plain 1e-12 of north_star holds for these
     assert plain.sum() > n // 4 and np.all(tol["u"][plain] == states.RTOL2) and np.all(tol["x"][plain] == states.RTOL2)
     if cfg in (3, 4, 6, 37, 47):
-        assert tol["trunc"].sum() <= n // 8 and (ref["n_sub"] > 1).sum() > n // 10
+        assert tol["trunc"].sum() <= n // 6 and (ref["n_sub"] > 1).sum() > n // 10
     # coverage of the branches
     acts = np.bincount(ref["action"], minlength=6)
     assert acts[1] > 0 and (cfg == 0 or acts[3] > 0)
@@ -209,12 +209,12 @@ def test_full_stack_stalls_do_not_change_the_physics(emx, emo):
     G = emx.Problem(desc)
     pd = G.upload_primaries(prim)
     a = G.transport(pd, desc["seed"], n_slots=4096, queue_capacity=1 << 20)
-    b = G.transport(pd, desc["seed"], n_slots=4096, queue_capacity=6000)
+    b = G.transport(pd, desc["seed"], n_slots=4096, queue_capacity=3000)
     assert b["stalls"] > 0 and a["stalls"] == 0
     assert np.array_equal(a["steps"], b["steps"]) and np.array_equal(a["inter"], b["inter"])
     assert np.array_equal(a["tracks"], b["tracks"])
     assert b["edep"].sum() == pytest.approx(a["edep"].sum(), rel=1e-12)
-    assert b["peak_queue"] <= 6000 * 1.01 + 384
+    assert b["peak_queue"] <= 3000 * 1.01 + 384
     hb = G.read_step_hist()
     G.transport(pd, desc["seed"], n_slots=4096, queue_capacity=1 << 20)
     assert np.array_equal(hb, G.read_step_hist())      # stalled steps are not counted twice

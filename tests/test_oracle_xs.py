@@ -189,6 +189,58 @@ def test_unrestricted_collision_loss_reduces_to_icru37(emo, T):
     assert P.table(0, "dedx_ep")[0] - rad == pytest.approx(pre * (lg + Fp - dl), rel=1e-11)
 
 
+def _one_material(emo, mat, T, **over):
+    """problem of one material whose energy grid starts exactly at T, no production threshold below T"""
+    from paper_2203_09467_b200 import workloads as W
+    m = dict(mat, Tcut=1e9, kcut=1e9, **over)
+    d = dict(materials=[m], surfaces=[], volumes=[dict(surf=[], sense=[], material=0, tally=0)],
+             field=(0, 0, 0), physics=W.physics(E_min=T, E_max=2 * T, n_E=2))
+    return emo.Problem(d)
+
+
+def test_printed_collision_stopping_powers(emo):
+    """SURVEY C5.8 pin (iii): the printed unrestricted (dE/dx)_col / rho, density effect zero (golden file)."""
+    from paper_2203_09467_b200 import workloads as W
+    mats = {"Pb": W.PB, "lAr": W.LAR, "Si": W.SI}
+    rows = golden("dedx_collision_unrestricted.txt")
+    assert len(rows) == 5
+    for name, I_eV, T, want in rows:
+        T = float(T)
+        assert mats[name]["I_eV"] == float(I_eV)
+        P = _one_material(emo, mats[name], T)
+        mi = P.material_info(0)
+        got = (P.table(0, "dedx_em")[0] - T / mi["X0"]) / mi["rho"]
+        assert abs(got - float(want)) < 0.6e-4, (name, T, got)          # every printed digit
+
+
+def test_density_effect_gives_the_fermi_plateau(emo):
+    """Density effect (R23), pinned by what it is FOR: once it is on, the collision loss no longer depends
+    on the mean excitation energy I (Fermi plateau: only the electron density enters, through the plasma energy),
+    and it switches on where hbar omega_p beta gamma = sqrt(e) I.  Below the onset two values of I differ by the
+    Bethe logarithm, 2 ln(I_a / I_b) times the prefactor.  A wrong coefficient of the logarithm of delta, a
+    missing beta gamma or a wrong onset fails one of the three."""
+    from paper_2203_09467_b200 import workloads as W
+    Ia, Ib = 823.0, 500.0
+    hwp = _one_material(emo, W.PB, 1.0).material_info(0)["hwp"]                       # MeV
+    onset = {I: math.sqrt(math.e) * I * 1e-6 / hwp for I in (Ia, Ib)}              # beta gamma at the onset
+    for T in (0.5, 2.0, 5.0, 10.5, 11.2, 20.0, 100.0, 1e3, 1e4):
+        g = T / ME + 1
+        bg = math.sqrt(g * g - 1)
+        b2 = 1 - 1 / (g * g)
+        pa, pb = _one_material(emo, W.PB, T, I_eV=Ia), _one_material(emo, W.PB, T, I_eV=Ib)
+        for kind in ("dedx_em", "dedx_ep"):
+            va, vb = pa.table(0, kind)[0], pb.table(0, kind)[0]
+            if bg > max(onset.values()) * (1 + 1e-9):
+                assert va == pytest.approx(vb, rel=1e-12), (T, kind)
+            elif bg < min(onset.values()):
+                pre = 2 * math.pi * RE * RE * ME * pa.material_info(0)["n_e"] / b2
+                assert vb - va == pytest.approx(pre * 2 * math.log(Ia / Ib), rel=1e-9), (T, kind)
+            else:
+                assert vb > va
+    # the onset for I = 823 eV sits between T = 10.5 and 11.2 MeV (beta gamma = 22.2): both sides are sampled above
+    assert (10.5 / ME + 1) ** 2 - 1 < onset[Ia] ** 2 < (11.2 / ME + 1) ** 2 - 1
+
+
 @pytest.mark.parametrize("T,Tcut", [(10.0, 1.0), (1.0, 0.1), (1e3, 0.35), (5.0, 2.0)])
 def test_restricted_loss_derivative_equals_cut_times_dcs(emo, T, Tcut):
     """d(dE/dx)_col / dT_cut = n_e T_cut dsigma/dT_delta(T_cut): ties dE/dx to the Moller/Bhabha DCS."""
