@@ -369,6 +369,27 @@ int emx_neighbour_candidates(const emx_problem *p, int surface, int sense, int w
 int emx_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
                     long *counts_host, void *stream);
 
+/* The same hook for callers that may not allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): identical arguments and results, but the scratch of the refill kernels
+ * (chunk tables, hole list, control block, a padded copy of alive[]) lives in a file-scope device array of the
+ * library instead of a block that emx_refill_plan allocates and frees on every call.  The call allocates nothing:
+ * no cudaMalloc, cudaFree or allocating library routine, on the host or on the device.
+ *   limit       capacity <= emx_refill_plan_static_max() = 65536 slots; a larger capacity returns EMX_E_CAPACITY
+ *               with a text naming the limit (use emx_refill_plan there).  The array is 345 KB; every GPU that loads
+ *               the library holds it until the process exits.
+ *   set-up      the device address of the array is looked up once per device (cudaGetSymbolAddress with that device
+ *               current) on the first call there; emx_refill_plan_static_setup() does the lookup for the current
+ *               device ahead of time and returns EMX_OK or EMX_E_CUDA / EMX_E_ARG (device ordinal above 63).
+ *   sharing     every call on a device uses the SAME array.  It keeps the previous call's contents, so each call
+ *               clears the part it uses first (on `stream`).  Calls whose GPU work overlaps -- different streams,
+ *               or different host threads -- race on it: serialise them.  Calls on one stream are safe, and the
+ *               function returns only after its own work on `stream` is complete.
+ * alive, src: DEVICE, owned by the caller; counts_host: HOST. */
+int emx_refill_plan_static(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
+                           long *counts_host, void *stream);
+long emx_refill_plan_static_max(void);
+int emx_refill_plan_static_setup(void);
+
 const char *emx_last_error(const emx_problem *p);
 const char *emx_version(void);
 

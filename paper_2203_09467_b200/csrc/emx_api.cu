@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 #include "emx_host.h"
@@ -877,6 +878,87 @@ int emx_refill_plan(long n_live, long capacity, long n_queue, const uint8_t *ali
     counts_host[0] = hc.plan[0].n_final;
     counts_host[1] = hc.plan[0].q_new;
     counts_host[2] = hc.plan[0].h - hc.plan[0].a;
+    return EMX_OK;
+}
+
+}  // extern "C"
+
+// ---- emx_refill_plan_static: the refill hook for callers that cannot allocate (include/emx.h) ----
+// Same kernels as emx_refill_plan; their scratch (chunk tables, hole list, control block, a padded copy of the alive
+// flags) lives in ONE file-scope device array instead of a cudaMalloc'ed block.  Every GPU that loads libemx holds the
+// array until the process exits; every call shares it.
+namespace {
+constexpr long kStaticPlanMaxCapacity = 1L << 16;  // slots: what emx_refill_plan_static accepts
+constexpr size_t static_plan_ints(long capacity) {  // the layout of launch_refill_plan (emx_transport.cu)
+    return 7 * ((size_t)(capacity + kChunk - 1) / kChunk + 1) + (size_t)capacity + (sizeof(Ctl) + 3) / 4 + 64 +
+           (((size_t)(capacity + kChunk - 1) / kChunk + 1) * kChunk + 3) / 4 + 64;
+}
+constexpr size_t kStaticPlanInts = static_plan_ints(kStaticPlanMaxCapacity);  // 345 KB
+}  // namespace
+
+static __device__ __align__(256) int g_static_plan_scratch[kStaticPlanInts];
+
+namespace {
+constexpr int kMaxDevices = 64;
+int *g_static_plan_ptr[kMaxDevices];  // device address of the array on each device, looked up once
+std::mutex g_static_plan_mu;
+
+// The array's name is a host-side stand-in in host code: its device address comes from the runtime, once per device,
+// with that device current.
+int static_plan_scratch(int **out) {
+    emx_problem *p = nullptr;
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(p, EMX_E_ARG, "emx_refill_plan_static: device ordinal above 63");
+    std::lock_guard<std::mutex> lock(g_static_plan_mu);
+    if (!g_static_plan_ptr[dev]) {
+        void *a = nullptr;
+        CU(cudaGetSymbolAddress(&a, g_static_plan_scratch));
+        if (!a) return fail(p, EMX_E_CUDA, "emx_refill_plan_static: no device address for the scratch array");
+        g_static_plan_ptr[dev] = static_cast<int *>(a);
+    }
+    *out = g_static_plan_ptr[dev];
+    return EMX_OK;
+}
+}  // namespace
+
+extern "C" {
+
+long emx_refill_plan_static_max(void) { return kStaticPlanMaxCapacity; }
+
+int emx_refill_plan_static_setup(void) {
+    int *scratch = nullptr;
+    return static_plan_scratch(&scratch);
+}
+
+int emx_refill_plan_static(long n_live, long capacity, long n_queue, const uint8_t *alive, int32_t *src,
+                           long *counts_host, void *stream) {
+    emx_problem *p = nullptr;
+    if (n_live < 0 || capacity < n_live || capacity < 1 || n_queue < 0 || (n_live > 0 && !alive) || !src || !counts_host ||
+        n_queue > (1L << 30))
+        return fail(p, EMX_E_ARG, "emx_refill_plan_static: invalid argument");
+    if (capacity > kStaticPlanMaxCapacity || refill_plan_scratch_ints(capacity) > kStaticPlanInts) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "emx_refill_plan_static: capacity %ld is above the %ld slots the static scratch holds "
+                 "(use emx_refill_plan)", capacity, kStaticPlanMaxCapacity);
+        g_err = buf;
+        return EMX_E_CAPACITY;
+    }
+    int *scratch = nullptr;
+    const int rc = static_plan_scratch(&scratch);
+    if (rc != EMX_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps what the last call left in it: everything this call uses starts from zero
+    CU(cudaMemsetAsync(scratch, 0, refill_plan_scratch_ints(capacity) * sizeof(int), st));
+    const Ctl *d_ctl = nullptr;
+    cudaError_t e = launch_refill_plan(n_live, capacity, n_queue, alive, src, scratch, &d_ctl, st);
+    PoolPlan plan = PoolPlan();  // three counts come back through a plain host struct: no staging buffer of ours
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&plan, &d_ctl->plan[0], sizeof(PoolPlan), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(p, e, "emx_refill_plan_static");
+    counts_host[0] = plan.n_final;
+    counts_host[1] = plan.q_new;
+    counts_host[2] = plan.h - plan.a;
     return EMX_OK;
 }
 

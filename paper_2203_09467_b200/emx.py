@@ -60,7 +60,8 @@ EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
            "emx_staging_bytes", "emx_set_primary_offset", "emx_get_schedule", "emx_set_schedule", "emx_neighbour_candidates", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
            "emx_get_iteration_log", "emx_get_iteration_times",
-           "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_last_error",
+           "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_refill_plan_static", "emx_refill_plan_static_max",
+           "emx_refill_plan_static_setup", "emx_last_error",
            "emx_version"]
 
 _lib = None
@@ -96,6 +97,8 @@ def lib():
             "emx_philox_batch": (i, [l, vp, vp, vp, vp]),
             "emx_draw_batch": (i, [u64, l, vp, vp, vp, vp, vp, vp, vp]),
             "emx_refill_plan": (i, [l, l, l, vp, vp, vp, vp]),
+            "emx_refill_plan_static": (i, [l, l, l, vp, vp, vp, vp]),
+            "emx_refill_plan_static_max": (l, []), "emx_refill_plan_static_setup": (i, []),
             "emx_last_error": (C.c_char_p, [vp]), "emx_version": (C.c_char_p, []),
         }
         for name, (res, args) in sig.items():
@@ -373,14 +376,20 @@ def draw_batch(seed, prim, tid, step, nn):
     return u.cpu().numpy(), ch.cpu().numpy().view(np.uint64)
 
 
-def refill_plan(alive, capacity, n_queue):
-    """Level-1 hook: returns (src[capacity] int32, (new_n_live, new_n_queue, n_unfilled_holes))."""
+def refill_plan(alive, capacity, n_queue, static=False):
+    """Level-1 hook: returns (src[capacity] int32, (new_n_live, new_n_queue, n_unfilled_holes)).
+    static=True: emx_refill_plan_static, the variant that allocates nothing (capacity <= refill_plan_static_max())."""
     torch = _torch()
     a = torch.from_numpy(_np(alive, np.uint8)).cuda()
     src = torch.empty(capacity, dtype=torch.int32, device="cuda")
     counts = (C.c_long * 3)()
-    rc = lib().emx_refill_plan(len(alive), capacity, n_queue, C.c_void_p(a.data_ptr()) if len(alive) else None,
-                               C.c_void_p(src.data_ptr()), C.cast(counts, C.c_void_p), _stream())
+    name = "emx_refill_plan_static" if static else "emx_refill_plan"
+    rc = getattr(lib(), name)(len(alive), capacity, n_queue, C.c_void_p(a.data_ptr()) if len(alive) else None,
+                              C.c_void_p(src.data_ptr()), C.cast(counts, C.c_void_p), _stream())
     if rc < 0:
-        raise EmxError("emx_refill_plan %d: %s" % (rc, (lib().emx_last_error(None) or b"").decode()))
+        raise EmxError("%s %d: %s" % (name, rc, (lib().emx_last_error(None) or b"").decode()))
     return src.cpu().numpy(), tuple(counts)
+
+
+def refill_plan_static_max():
+    return int(lib().emx_refill_plan_static_max())
