@@ -59,6 +59,7 @@ enum { EMO_T_COMPTON = 0, EMO_T_PHOTO, EMO_T_PAIR, EMO_T_MOLLER, EMO_T_BREMS_EM,
        EMO_T_DEDX_EP, EMO_T_RANGE_EP, EMO_T_PAIR_ELEM0, /* + element index */
        EMO_T_MSC = EMO_T_PAIR_ELEM0 + EMO_MAX_ELEM,     /* 1/lambda_1, inverse first transport mean free path of e+- */
        EMO_T_VAR_EM, EMO_T_VAR_EP,                      /* d(variance of the restricted collision loss)/ds, MeV2/cm */
+       EMO_T_MSC2,                                      /* 1/lambda_2, inverse second transport mean free path (msc = 2) */
        EMO_NTABLE };
 
 /* surface types */
@@ -103,7 +104,8 @@ typedef struct {
     double vacuum_step;          /* cm */
     int max_steps;               /* per track */
     int deposit_e_at_creation;   /* config 0: every e- is deposited at birth */
-    int msc;                     /* 1: multiple scattering of e+- (DESIGN.md R-MSC) */
+    int msc;                     /* 1: multiple scattering of e+- (DESIGN.md R-MSC); 2: also the path-length
+                                  * correction and the lateral displacement of Lewis' theory (DESIGN.md R-MSC2) */
     double msc_fr;               /* step limit s <= max(msc_fr * max(R, lambda_1), msc_smin) */
     double msc_smin;             /* cm */
     int fluct;                   /* 1: energy-loss fluctuations of e+- (DESIGN.md R-FLUCT) */
@@ -187,6 +189,12 @@ double emo_fluctuate_loss(double dE, double V, double E, double xi1, double xi2)
 double emo_msc_screening(int Z, double T);              /* Moliere screening parameter A */
 double emo_msc_sigma1(int Z, double Amass, double T);   /* first transport cross section, cm2 per atom */
 double emo_msc_one_minus_mu(double tau, double xi);     /* 1 - cos(theta) of a step of s = tau * lambda_1 */
+/* DESIGN.md R-MSC2: second transport cross section; Lewis' mean geometric length <z> and mean square lateral
+ * displacement <x^2 + y^2> of a true path t (il1 = 1/lambda_1, il2 = 1/lambda_2, both 1/cm) */
+double emo_msc_sigma2(int Z, double Amass, double T);   /* Int (1 - P_2(cos theta)) dsigma, cm2 per atom */
+double emo_msc_phi3(double x);                          /* (x^2/2 - x + 1 - exp(-x)) / x^3 */
+double emo_msc_geom_length(double t, double il1);       /* cm */
+double emo_msc_lateral_r2(double t, double il1, double il2); /* cm2 */
 
 /* ---- problem.c ---- */
 emo_problem *emo_create(void);

@@ -13,7 +13,7 @@ from . import build as _build
 
 MAX_ELEM, MAX_FACES, NPROC, PER_PRIM, NHIST = 4, 8, 8, 11, 96
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
-           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc", "var_em", "var_ep"]
+           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc", "var_em", "var_ep", "msc2"]
 T = {n: i for i, n in enumerate(T_NAMES)}
 ME = 0.51099895000
 
@@ -71,6 +71,8 @@ def lib():
             "emo_gauss_legendre": (None, [i, dp, dp]),
             "emo_loss_second_moment": (d, [i, d, d]), "emo_fluctuate_loss": (d, [d, d, d, d, d]),
             "emo_msc_screening": (d, [i, d]), "emo_msc_sigma1": (d, [i, d, d]), "emo_msc_one_minus_mu": (d, [d, d]),
+            "emo_msc_sigma2": (d, [i, d, d]), "emo_msc_phi3": (d, [d]), "emo_msc_geom_length": (d, [d, d]),
+            "emo_msc_lateral_r2": (d, [d, d, d]),
             "emo_msc_deflect": (None, [C.POINTER(Rng), d, dp, dp]),
             "emo_create": (p, []), "emo_destroy": (None, [p]),
             "emo_add_material": (i, [p, i, ip, dp, dp, d, d]), "emo_add_surface": (i, [p, i, d]),

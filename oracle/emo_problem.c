@@ -95,6 +95,7 @@ int emo_set_field_fringe(emo_problem *p, double z0_cm, double a_cm) {
 
 int emo_set_physics(emo_problem *p, const emo_physics *ph) {
     if (ph->n_E < 2 || !(ph->E_max > ph->E_min) || !(ph->E_min > 0.0)) return -1;
+    if (ph->msc < 0 || ph->msc > 2) return -1;
     if (ph->msc && (!(ph->msc_fr > 0.0) || !(ph->msc_smin > 0.0))) return -1;
     p->ph = *ph; p->built = 0;
     return 0;
@@ -206,6 +207,11 @@ int emo_build_tables(emo_problem *p) {
                 double s = 0.0;
                 for (int i = 0; i < m->n_elem; ++i) s += m->n_i[i] * emo_msc_sigma1(m->Z[i], m->A[i], E);
                 T[EMO_T_MSC * n + j] = s;
+                if (ph->msc == 2) {                        /* 1/lambda_2 (R-MSC2) */
+                    double s2 = 0.0;
+                    for (int i = 0; i < m->n_elem; ++i) s2 += m->n_i[i] * emo_msc_sigma2(m->Z[i], m->A[i], E);
+                    T[EMO_T_MSC2 * n + j] = s2;
+                }
             }
             if (ph->fluct) {                               /* variance of the loss per unit path (R-FLUCT) */
                 T[EMO_T_VAR_EM * n + j] = m->n_e * emo_loss_second_moment(EMO_ELECTRON, E, m->Tcut);

@@ -69,6 +69,7 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
 
     double Sig[3] = {0, 0, 0}, Stot = 0.0, D = 0.0, R = 0.0, s_phys, s_loss = INFINITY;
     const int msc = (ph->msc && pt != EMO_GAMMA && mat >= 0);   /* multiple scattering applies (R-MSC) */
+    const int msc2 = (msc && ph->msc == 2);                      /* ... with Lewis' spatial moments (R-MSC2) */
     double iL0 = 0.0;                                            /* 1/lambda_1 at the pre-step energy */
     int nproc = 0, procs[3] = {-1, -1, -1};
     int action;
@@ -117,24 +118,28 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
         }
     }
 
-    /* 5. geometry / move */
+    /* 5. geometry / move.  R-MSC2: s_phys is the TRUE path length t of the step; the track is moved by the mean
+     * geometric length z(t) = lambda_1 (1 - exp(-t / lambda_1)) of Lewis' theory (lambda_1 at the pre-step energy).
+     * A move cut short after the geometric length g < z(t) stands for the true length t g / z(t). */
+    double s_move = msc2 ? emo_msc_geom_length(s_phys, iL0) : s_phys;
     double s;
     int hit = -1;
     int full = 1;                         /* the full s_phys was travelled */
     if (pt == EMO_GAMMA || p->Bmag == 0.0) {
         double d = emo_distance(p, vol, t->x, t->u, t->surf, &hit);
-        if (d <= s_phys) { s = d; action = EMO_A_BOUNDARY; full = 0; }
-        else { s = s_phys; hit = -1; }
+        if (d <= s_move) { s = d; action = EMO_A_BOUNDARY; full = 0; }
+        else { s = s_move; hit = -1; }
         for (int i = 0; i < 3; ++i) t->x[i] += s * t->u[i];
     } else {
         double pm = sqrt(E * (E + 2.0 * EMO_ME));
         double q = (pt == EMO_ELECTRON) ? -1.0 : 1.0;
         double kappa = q * EMO_CB * p->Bmag / pm;
         int sf = t->surf;
-        s = emo_propagate_field_n(p, vol, &sf, t->x, t->u, kappa, s_phys, &hit, &out->n_sub);
+        s = emo_propagate_field_n(p, vol, &sf, t->x, t->u, kappa, s_move, &hit, &out->n_sub);
         if (hit >= 0) { action = EMO_A_BOUNDARY; full = 0; }
-        else if (!(s >= s_phys * (1.0 - 1e-14))) { action = EMO_A_TRUNC; full = 0; }
+        else if (!(s >= s_move * (1.0 - 1e-14))) { action = EMO_A_TRUNC; full = 0; }
     }
+    if (msc2) s = full ? s_phys : s_phys * (s / s_move);   /* from here on s is the true path length */
     out->s = s;
 
     /* 6. continuous loss (e+- in matter) */
@@ -181,10 +186,33 @@ void emo_step(const emo_problem *p, uint64_t seed, const emo_track *in, emo_step
     if (msc) {
         double iL1 = emo_lookup(p, mat, EMO_T_MSC, t->E);
         double tau = 0.5 * (iL0 + iL1) * s;
-        double u1[3];
-        emo_msc_deflect(&c.rng, tau, t->u, u1);
+        double u0[3] = { t->u[0], t->u[1], t->u[2] }, u1[3];
+        emo_msc_deflect(&c.rng, tau, u0, u1);
         t->u[0] = u1[0]; t->u[1] = u1[1]; t->u[2] = u1[2];
         out->msc_tau = tau;
+        /* R-MSC2 lateral displacement: along the transverse part of the new direction, d = u1 - (u0.u1) u0 with
+         * |d| = sin(theta), by rho = sqrt(3 <r^2> / (2 (1 - g^2))) sin(theta): for the Henyey-Greenstein angle
+         * <sin^2(theta)> = (2/3)(1 - g^2), g = exp(-tau), so <rho^2> is Lewis' <x^2 + y^2> of the true path s
+         * (lambda_1, lambda_2 averaged over the pre-step and post-loss energies like tau).  No draw of its own.
+         * The track stays inside its cell: rho <= 0.9 x the distance to the cell's boundary along d; a step that
+         * ended ON a boundary is not displaced. */
+        if (msc2 && action != EMO_A_BOUNDARY) {
+            double il1 = 0.5 * (iL0 + iL1);
+            double il2 = 0.5 * (emo_lookup(p, mat, EMO_T_MSC2, E) + emo_lookup(p, mat, EMO_T_MSC2, t->E));
+            double r2 = emo_msc_lateral_r2(s, il1, il2);
+            double om = -expm1(-2.0 * tau);
+            double mu = u0[0] * u1[0] + u0[1] * u1[1] + u0[2] * u1[2];
+            double d[3] = { u1[0] - mu * u0[0], u1[1] - mu * u0[1], u1[2] - mu * u0[2] };
+            double dn = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            if (r2 > 0.0 && om > 0.0 && dn > 0.0) {
+                double rho = sqrt(1.5 * r2 / om) * dn;
+                double dh[3] = { d[0] / dn, d[1] / dn, d[2] / dn };
+                int hs;
+                double lim = 0.9 * emo_distance(p, t->vol, t->x, dh, -1, &hs);
+                if (rho > lim) rho = lim;
+                for (int i = 0; i < 3; ++i) t->x[i] += rho * dh[i];
+            }
+        }
     }
 
     /* 8. discrete */

@@ -245,6 +245,70 @@ double emo_msc_sigma1(int Z, double Amass, double T) {
     return 2.0 * EMO_PI * (double)Z * (Z + 1.0) * c * c * (log1p(tm / (2.0 * A)) - tm / (tm + 2.0 * A));
 }
 
+/* ---- DESIGN.md R-MSC2: what Lewis' theory (H. W. Lewis, Phys. Rev. 78 (1950) 526) fixes about the SPATIAL
+ * displacement of a true path t in an unbounded medium of constant transport mean free paths lambda_1, lambda_2
+ * (lambda_l^-1 = n Int (1 - P_l(cos theta)) dsigma), start at the origin along +z, tau = t / lambda_1,
+ * kappa = lambda_1 / lambda_2:
+ *   <z>         = lambda_1 (1 - exp(-tau))
+ *   <x^2 + y^2> = (4 lambda_1^2 / 3) [ tau - (kappa + 1) / kappa + kappa / (kappa - 1) exp(-tau)
+ *                                      - exp(-kappa tau) / (kappa (kappa - 1)) ]
+ * Both hold for ANY single-scattering law.  The multiple-scattering step of the transport moves the track by <z>
+ * along its direction instead of by t, and displaces it sideways so that the mean square displacement is Lewis'. */
+
+/* second transport cross section of the screened Rutherford law of emo_msc_sigma1, same cutoff t_m:
+ * 1 - P_2(mu) = (3/2)(1 - mu^2) = 3 t - (3/2) t^2, t = 1 - mu, and with
+ *   I_1 = Int_0^t_m t   / (t + 2A)^2 dt = ln(1 + t_m / 2A) - t_m / (t_m + 2A)
+ *   I_2 = Int_0^t_m t^2 / (t + 2A)^2 dt = t_m - 4A ln(1 + t_m / 2A) + 2A t_m / (t_m + 2A)
+ * sigma_2 = 2 pi Z (Z + 1) r_e^2 (m_e c^2 / (beta p c))^2 (3 I_1 - (3/2) I_2) */
+double emo_msc_sigma2(int Z, double Amass, double T) {
+    double pc2 = T * (T + 2.0 * EMO_ME);
+    double bpc = pc2 / (T + EMO_ME);
+    double A = emo_msc_screening(Z, T);
+    double c = EMO_RE * EMO_ME / bpc;
+    double lam = EMO_RE * EMO_ME / EMO_ALPHA;
+    double RN = 1.4e-13 * cbrt(Amass);
+    double tm = 0.5 * lam * lam / (pc2 * RN * RN);
+    if (tm > 2.0) tm = 2.0;
+    double lg = log1p(tm / (2.0 * A)), fr = tm / (tm + 2.0 * A);
+    double I1 = lg - fr;
+    double I2 = tm - 4.0 * A * lg + 2.0 * A * fr;
+    return 2.0 * EMO_PI * (double)Z * (Z + 1.0) * c * c * (3.0 * I1 - 1.5 * I2);
+}
+
+/* phi_3(x) = (x^2/2 - x + 1 - exp(-x)) / x^3 = 1/6 - x/24 + x^2/120 - ...: the plain expression loses everything to
+ * cancellation for small x, so below x = 0.5 the series is summed (terms x^n / (n + 3)!, n <= 14: the next is below
+ * 1e-19) */
+double emo_msc_phi3(double x) {
+    if (x < 0.5) {
+        double s = 0.0, term = 1.0 / 6.0;
+        for (int n = 0; n <= 14; ++n) { s += term; term *= -x / (double)(n + 4); }
+        return s;
+    }
+    return (0.5 * x * x - x - expm1(-x)) / (x * x * x);
+}
+
+/* <z> = lambda_1 (1 - exp(-tau)) = t (1 - exp(-tau)) / tau */
+double emo_msc_geom_length(double t, double il1) {
+    double tau = t * il1;
+    if (!(tau > 0.0)) return t;
+    return t * (-expm1(-tau) / tau);
+}
+
+/* Lewis' <x^2 + y^2>.  The bracket is O(tau^3) for small tau: written with phi_3 it is
+ *   tau^3 (kappa / (kappa - 1)) (kappa phi_3(kappa tau) - phi_3(tau)),
+ * which does not cancel there (kappa > 1 for every forward-peaked law), and lambda_1^2 tau^3 = t^2 tau.  For
+ * tau >= 1 it is the other way round -- the two phi_3 agree in their leading 1 / (2 x) and the printed form is the
+ * well-conditioned one. */
+double emo_msc_lateral_r2(double t, double il1, double il2) {
+    double tau = t * il1;
+    if (!(tau > 0.0) || !(il2 > il1)) return 0.0;
+    double kap = il2 / il1;
+    if (tau < 1.0)
+        return (4.0 / 3.0) * t * t * tau * (kap / (kap - 1.0)) * (kap * emo_msc_phi3(kap * tau) - emo_msc_phi3(tau));
+    double br = tau - (kap + 1.0) / kap + (kap * exp(-tau) - exp(-kap * tau) / kap) / (kap - 1.0);
+    return (4.0 / 3.0) * br / (il1 * il1);
+}
+
 /* Deflection after a path s = tau lambda_1: Lewis' theory gives <cos(theta)> = exp(-tau) exactly; the angle is
  * drawn from the Henyey-Greenstein density p(mu) ~ (1 - g^2) / (1 + g^2 - 2 g mu)^(3/2), whose mean cosine is
  * g, with g = exp(-tau).  Inverse of its distribution function, xi = F(mu), written for 1 - mu so that nothing
