@@ -103,7 +103,8 @@ extern "C" {
 #define EMX_T_MSC (EMX_T_PAIR_ELEM0 + EMX_MAX_ELEM) /* 1 / lambda_1: inverse first transport mean free path of e+-, 1/cm */
 #define EMX_T_VAR_EM (EMX_T_MSC + 1) /* d(variance of the restricted collision loss)/ds of e-, MeV2/cm */
 #define EMX_T_VAR_EP (EMX_T_MSC + 2) /* ... of e+ */
-#define EMX_NTABLE (EMX_T_MSC + 3)
+#define EMX_T_MSC2 (EMX_T_MSC + 3) /* 1 / lambda_2: inverse second transport mean free path of e+- (msc = 2), 1/cm */
+#define EMX_NTABLE (EMX_T_MSC + 4)
 
 typedef struct emx_problem emx_problem; /* opaque, owned by the library */
 
@@ -126,7 +127,12 @@ typedef struct {
      * there, no formula printed; DESIGN.md R-MSC).  msc = 1: 1/lambda_1 is tabulated from the screened-Rutherford
      * transport cross section (Moliere screening, nuclear-size cutoff); a step of e+- in matter is limited to
      * max(msc_fr * max(range, lambda_1), msc_smin) and ends with a deflection drawn from the Henyey-Greenstein
-     * law of mean cosine exp(-s (1/lambda_1(E) + 1/lambda_1(E')) / 2) (two draws, taken right after draw 0). */
+     * law of mean cosine exp(-s (1/lambda_1(E) + 1/lambda_1(E')) / 2) (two draws, taken right after draw 0).
+     * msc = 2 (DESIGN.md R-MSC2) adds the spatial moments of Lewis' theory: 1/lambda_2 is tabulated too
+     * (EMX_T_MSC2); the step limits are TRUE path lengths t and the track is moved by the mean geometric length
+     * lambda_1 (1 - exp(-t / lambda_1)); after the deflection a step that did not end on a boundary is shifted
+     * sideways, along the transverse part of the new direction, with the mean square <x^2 + y^2> of the theory,
+     * at most 0.9 of the way to the cell's boundary.  emx_step_result.s and the energy loss refer to the true path. */
     int32_t msc;
     double msc_fr;              /* > 0 */
     double msc_smin;            /* cm, > 0 */
@@ -343,6 +349,14 @@ long emx_get_iteration_times(const emx_problem *p, float *host_out, long max_ite
  * in[n] and out[n] are DEVICE pointers (AoS). */
 int emx_step_batch(emx_problem *p, uint64_t seed, long n, const emx_track *in, emx_step_result *out,
                    void *stream);
+
+/* Level-2 parity hook for ONE substep of the field propagation (C9): for each of n states
+ * (x, u, curvature kappa [1/cm, signed], trial step h [cm]) one RK4 step of h against two of h / 2 in the problem's
+ * field, exactly as the propagation kernel runs it -- x1, u1 = state after the two half steps (u1 normalised),
+ * err = |x_full - x_half|.  All pointers DEVICE; x3, u3, x1, u1 hold 3 n doubles (xyz per state).  EMX_E_STATE
+ * when no field is set. */
+int emx_field_substep_batch(emx_problem *p, long n, const double *x3, const double *u3, const double *kappa,
+                            const double *h, double *x1, double *u1, double *err, void *stream);
 
 /* Level-1 parity hooks (integer work).  All pointers DEVICE.
  * emx_philox_batch: out[4i..4i+3] = Philox4x32-10(ctr[4i..], key[2i..]).

@@ -272,6 +272,7 @@ int emx_set_physics(emx_problem *p, const emx_physics *ph) {
     if (ph->n_E < 2 || !(ph->E_max > ph->E_min) || !(ph->E_min > 0.0) || ph->max_steps < 1 || ph->max_substeps < 1 ||
         !(ph->field_eps > 0.0) || !(ph->vacuum_step > 0.0))
         return fail(p, EMX_E_ARG, "emx_set_physics: invalid grid or limits");
+    if (ph->msc < 0 || ph->msc > 2) return fail(p, EMX_E_ARG, "emx_set_physics: msc is 0, 1 or 2");
     if (ph->msc && (!(ph->msc_fr > 0.0) || !(ph->msc_smin > 0.0)))
         return fail(p, EMX_E_ARG, "emx_set_physics: multiple scattering needs msc_fr > 0 and msc_smin > 0");
     p->hp.ph = *ph;
@@ -394,6 +395,7 @@ int emx_build_tables(emx_problem *p, void *stream) {
     P.nb2_list = p->d_nb2_list;
     const double bm = sqrt(hp.B[0] * hp.B[0] + hp.B[1] * hp.B[1] + hp.B[2] * hp.B[2]);
     P.Bmag = bm;
+    P.field_eps_floor = hp.ph.field_eps / 3125.0;
     for (int i = 0; i < 3; ++i) P.Bhat[i] = bm > 0.0 ? hp.B[i] / bm : 0.0;
     P.field_kind = hp.field_kind;
     P.fringe_z0 = hp.fringe_z0;
@@ -840,6 +842,16 @@ int emx_step_batch(emx_problem *p, uint64_t seed, long n, const emx_track *in, e
     if (!p || !p->hp.built) return fail(p, EMX_E_STATE, "emx_step_batch: tables not built");
     if (n < 0 || (n > 0 && (!in || !out))) return fail(p, EMX_E_ARG, "emx_step_batch: invalid argument");
     CU(launch_step_batch(p->P, seed, n, in, out, (cudaStream_t)stream));
+    return EMX_OK;
+}
+
+int emx_field_substep_batch(emx_problem *p, long n, const double *x3, const double *u3, const double *kappa,
+                            const double *h, double *x1, double *u1, double *err, void *stream) {
+    if (!p || !p->hp.built) return fail(p, EMX_E_STATE, "emx_field_substep_batch: tables not built");
+    if (n < 0 || (n > 0 && (!x3 || !u3 || !kappa || !h || !x1 || !u1 || !err)))
+        return fail(p, EMX_E_ARG, "emx_field_substep_batch: invalid argument");
+    if (p->P.Bmag <= 0.0) return fail(p, EMX_E_STATE, "emx_field_substep_batch: no field set");
+    CU(launch_field_substep_batch(p->P, n, x3, u3, kappa, h, x1, u1, err, (cudaStream_t)stream));
     return EMX_OK;
 }
 

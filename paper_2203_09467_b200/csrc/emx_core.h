@@ -73,6 +73,7 @@ struct Params {
     const int *nb2_off;     // per (S, sense): cells that do not list S at all (the only other cells that can match)
     const int *nb2_list;
     double Bmag, Bhat[3];
+    double field_eps_floor;       // ph.field_eps / 3125: the error below which a substep grows by the full factor 5 (C9)
     int field_kind;               // 0 uniform; 1 solenoid with fringe (emx_set_field_fringe)
     double fringe_z0, fringe_a;   // cm
     double lnE0, dlnE, inv_dlnE;  // grid: x_j = lnE0 + j * dlnE

@@ -35,8 +35,9 @@ EMX_HD Vec3 stage_u(const Vec3 &u, double f, const Vec3 &k) {
 }
 
 // one classical RK4 step of length h.  dx/ds = u, so the x-stages are the u-stage arguments.
+// h6 = h / 6 (the caller divides once per substep: (h / 2) / 6 = (h / 6) / 2 exactly)
 template <int AX>
-EMX_HD void rk4_step(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, Vec3 &xo, Vec3 &uo) {
+EMX_HD void rk4_step(const Vec3 &x, const Vec3 &u, double kappa, const double B[3], double h, double h6, Vec3 &xo, Vec3 &uo) {
     const Vec3 k1u = lorentz<AX>(u, kappa, B);
     const Vec3 u2 = stage_u<AX>(u, 0.5 * h, k1u);
     const Vec3 k2u = lorentz<AX>(u2, kappa, B);
@@ -44,7 +45,6 @@ EMX_HD void rk4_step(const Vec3 &x, const Vec3 &u, double kappa, const double B[
     const Vec3 k3u = lorentz<AX>(u3, kappa, B);
     const Vec3 u4 = stage_u<AX>(u, h, k3u);
     const Vec3 k4u = lorentz<AX>(u4, kappa, B);
-    const double h6 = h / 6.0;
     xo.x = x.x + h6 * (u.x + 2.0 * u2.x + 2.0 * u3.x + u4.x);
     xo.y = x.y + h6 * (u.y + 2.0 * u2.y + 2.0 * u3.y + u4.y);
     xo.z = x.z + h6 * (u.z + 2.0 * u2.z + 2.0 * u3.z + u4.z);
@@ -102,9 +102,10 @@ EMX_NI void rk4_doubling(const Params &P, const Vec3 &x, const Vec3 &u, double k
         rk4_step_map(P, x, u, kappa, 0.5 * h, xm, um);
         rk4_step_map(P, xm, um, kappa, 0.5 * h, x1, u1);
     } else {
-        rk4_step<AX>(x, u, kappa, P.Bhat, h, xf, uf);
-        rk4_step<AX>(x, u, kappa, P.Bhat, 0.5 * h, xm, um);
-        rk4_step<AX>(xm, um, kappa, P.Bhat, 0.5 * h, x1, u1);
+        const double h6 = h / 6.0, hh6 = 0.5 * h6;
+        rk4_step<AX>(x, u, kappa, P.Bhat, h, h6, xf, uf);
+        rk4_step<AX>(x, u, kappa, P.Bhat, 0.5 * h, hh6, xm, um);
+        rk4_step<AX>(xm, um, kappa, P.Bhat, 0.5 * h, hh6, x1, u1);
     }
     err = norm(xf - x1);
     const double n = norm(u1);
@@ -113,9 +114,27 @@ EMX_NI void rk4_doubling(const Params &P, const Vec3 &x, const Vec3 &u, double k
     u1.z /= n;
 }
 
-// x^(1/5) for the step-size control, x in [3e-10, 3125]: exp(log(x) / 5), within 2 ulp (|log x| <= 22, so the error of
-// the logarithm enters the exponent below 1e-15) at 0.4 of the cost of pow()
-EMX_HD double fifth_root(double x) { return m_exp(0.2 * m_log(x)); }
+// x^(1/5) for the step-size control, x in [1e-30, 1e30], within 1 ulp: r ~ x^(-1/5) from a single-precision seed of
+// the special-function unit (relative error below 1e-5) and two Newton steps r <- r (6 - x r^5) / 5 (each squares the
+// error times 3: 3e-10, then below rounding), y = x r^4, and one Newton step of y^5 = x with 1 / (5 y^4) = r^4 / 5
+// whose residual comes out of one fused multiply-add.  30 instructions against the 110 of exp(log(x) / 5), which was
+// 30 % of all instructions of the propagation kernel (profiles/r2_field_hotspots.md).
+EMX_HD double fifth_root(double x) {
+#if defined(__CUDA_ARCH__)
+    double r = (double)__powf((float)x, -0.2f);
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const double r2 = r * r, r4 = r2 * r2;
+        r = r * (0.2 * fma(-x, r4 * r, 6.0));
+    }
+    const double r2 = r * r, r4 = r2 * r2;
+    const double y = x * r4;
+    const double y2 = y * y;
+    return fma(-0.2 * r4, fma(y2 * y2, y, -x), y);
+#else
+    return pow(x, 0.2);
+#endif
+}
 
 // Loop variables of a propagation: the arc length done, the current trial step and the substep attempts used.
 // They live in registers while a lane works on the track and in the slot while the track is parked between two
@@ -185,7 +204,7 @@ EMX_NI bool field_attempt(const Params &P, const Face *cell, int &on_surf, Vec3 
                 s = fs.s_done;
                 return true;
             }
-            const double e = err > eps / 3125.0 ? err : eps / 3125.0;
+            const double e = err > P.field_eps_floor ? err : P.field_eps_floor;
             ratio = eps / e;
             rescale = 2;
         } else if (L - d <= eps) {  // |L - d| <= eps: landed on S, just past it or just short of it

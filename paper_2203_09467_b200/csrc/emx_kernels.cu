@@ -48,6 +48,32 @@ cudaError_t launch_step_batch(const Params &P, uint64_t seed, long n, const emx_
     return cudaGetLastError();
 }
 
+// ONE substep of the field propagation (rk4_doubling as k_field runs it: the axis specialisation of a uniform
+// field with the sign of the field folded into the curvature, or the field map at the stage positions)
+__global__ void k_field_substep_batch(Params P, long n, const double *x3, const double *u3, const double *kappa,
+                                      const double *h, double *x1, double *u1, double *err) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const Vec3 x = {x3[3 * i], x3[3 * i + 1], x3[3 * i + 2]}, u = {u3[3 * i], u3[3 * i + 1], u3[3 * i + 2]};
+    Vec3 xo, uo;
+    double e;
+    const int ax = P.field_kind == 0 ? field_axis(P.Bhat) : kAxisAny;
+    if (P.field_kind != 0) rk4_doubling<true, kAxisAny>(P, x, u, kappa[i], h[i], xo, uo, e);
+    else if (ax == 0) rk4_doubling<false, 0>(P, x, u, kappa[i] * P.Bhat[0], h[i], xo, uo, e);
+    else if (ax == 1) rk4_doubling<false, 1>(P, x, u, kappa[i] * P.Bhat[1], h[i], xo, uo, e);
+    else if (ax == 2) rk4_doubling<false, 2>(P, x, u, kappa[i] * P.Bhat[2], h[i], xo, uo, e);
+    else rk4_doubling<false, kAxisAny>(P, x, u, kappa[i], h[i], xo, uo, e);
+    put3(x1 + 3 * i, xo);
+    put3(u1 + 3 * i, uo);
+    err[i] = e;
+}
+cudaError_t launch_field_substep_batch(const Params &P, long n, const double *x3, const double *u3, const double *kappa,
+                                       const double *h, double *x1, double *u1, double *err, cudaStream_t st) {
+    if (n <= 0) return cudaSuccess;
+    k_field_substep_batch<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(P, n, x3, u3, kappa, h, x1, u1, err);
+    return cudaGetLastError();
+}
+
 __global__ void k_philox_batch(long n, const uint32_t *ctr, const uint32_t *key, uint32_t *out) {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;

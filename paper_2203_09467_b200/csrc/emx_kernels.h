@@ -11,6 +11,8 @@ struct TableCtx;
 cudaError_t launch_build_tables(const TableCtx &c, cudaStream_t st);
 cudaError_t launch_step_batch(const Params &P, uint64_t seed, long n, const emx_track *in, emx_step_result *out,
                               cudaStream_t st);
+cudaError_t launch_field_substep_batch(const Params &P, long n, const double *x3, const double *u3, const double *kappa,
+                                       const double *h, double *x1, double *u1, double *err, cudaStream_t st);
 cudaError_t launch_philox_batch(long n, const uint32_t *ctr, const uint32_t *key, uint32_t *out, cudaStream_t st);
 cudaError_t launch_draw_batch(uint64_t seed, long n, const uint32_t *prim, const uint64_t *tid, const uint32_t *step,
                               const uint32_t *nn, double *u, uint64_t *child, cudaStream_t st);

@@ -54,8 +54,9 @@ struct StepOut {
 // what stage a1 hands to stage a2
 constexpr int kActCut = 7;  // internal action code: the track was below the tracking cut at the start of the step
 struct Carry {
-    double s_phys;  // step limit of the physics (kept while a propagation is parked)
-    double s;       // path travelled
+    double s_phys;  // limit of the move: the step limit of the physics (R-MSC2: its geometric length); kept while a
+                    // propagation is parked
+    double s;       // path travelled by the move
     int action;     // EMX_A_* after the move (BOUNDARY / TRUNC override the physics limit), or kActCut
     int hit;        // surface reached, -1 none
 };
@@ -97,13 +98,14 @@ EMX_HD const double *table(const Params &P, int mat, int kind) {
 struct Lookup {
     double Sig0, Sig1, Sig2, Stot, D, R;
     double iL0;   // 1 / lambda_1 (R-MSC)
+    double iL20;  // 1 / lambda_2 (R-MSC2)
     double var0;  // variance of the loss per unit path (R-FLUCT)
     const double *Rtab;
 };
 template <bool CH, bool EXT>
 EMX_HD void lookup_tables(const Params &P, int pt, int mat, double E, Lookup &L) {
     const GridPos g = grid_pos(P, E);
-    L.D = L.R = L.iL0 = L.var0 = 0.0;
+    L.D = L.R = L.iL0 = L.iL20 = L.var0 = 0.0;
     L.Rtab = nullptr;
     if (!CH) {
         L.Sig0 = interp(table(P, mat, EMX_T_COMPTON), g);
@@ -121,6 +123,7 @@ EMX_HD void lookup_tables(const Params &P, int pt, int mat, double E, Lookup &L)
         L.Stot = em ? (L.Sig0 + L.Sig1) : (L.Sig0 + L.Sig1 + L.Sig2);
         if (EXT && P.ph.fluct) L.var0 = interp(table(P, mat, em ? EMX_T_VAR_EM : EMX_T_VAR_EP), g);
         if (EXT && P.ph.msc) L.iL0 = interp(table(P, mat, EMX_T_MSC), g);
+        if (EXT && P.ph.msc == 2) L.iL20 = interp(table(P, mat, EMX_T_MSC2), g);
     }
 }
 
@@ -236,6 +239,8 @@ EMX_HD void step_a0(const Params &P, uint64_t seed, int pt, const Track &t, Carr
         lookup_tables<CH, EXT>(P, pt, mat, t.E, L);
         const double xi = draw_at(seed, t.prim, t.tid, t.step, 0u);
         step_limits<CH, EXT>(P, L, xi, c.s_phys, c.action);
+        // R-MSC2: the limits are true path lengths; what the move is limited by is the geometric length of the step
+        if (CH && EXT && ph.msc == 2) c.s_phys = msc_geom_length(c.s_phys, L.iL0);
     }
 }
 
@@ -287,17 +292,27 @@ EMX_HD int step_a2(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o,
     }
     const int mat = P.vol[t.vol].material;
     const int action = c.action;
-    const double s = c.s;
+    double s = c.s;
     const double E = t.E;
     if (!HAVE_L) {
-        L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.var0 = 0.0;
+        L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.iL20 = L.var0 = 0.0;
         L.Rtab = nullptr;
     }
+    double xi0 = 0.5;
     if (mat >= 0) {
         if (!HAVE_L) lookup_tables<CH, EXT>(P, pt, mat, E, L);
-        (void)rng.next();  // draw 0 was the interaction length (stage a1); this also restores the block's second half
+        xi0 = rng.next();  // draw 0 was the interaction length (stage a1); this also restores the block's second half
     }
     const bool msc = CH && EXT && ph.msc && mat >= 0;  // multiple scattering applies (R-MSC)
+    if (msc && ph.msc == 2) {
+        // R-MSC2: c.s is the geometric length of the move; from here on s is the TRUE path length -- the limit of the
+        // physics (the same evaluation as stage a0's) if the move was completed, else in proportion
+        double t_phys;
+        int a0;
+        step_limits<CH, EXT>(P, L, xi0, t_phys, a0);
+        const bool full = action != EMX_A_BOUNDARY && action != EMX_A_TRUNC;
+        s = full ? t_phys : t_phys * (c.s / msc_geom_length(t_phys, L.iL0));
+    }
     o.s = s;
 
     // 6. continuous loss (e+- in matter)
@@ -352,10 +367,35 @@ EMX_HD int step_a2(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o,
     // 7b. multiple-scattering deflection at the end of the step (R-MSC): <cos> = exp(-Int ds / lambda_1), the
     // integral by the trapezoid rule over the pre-step and post-loss energies; two draws, always consumed
     if (msc) {
-        const double iL1 = interp(table(P, mat, EMX_T_MSC), grid_pos(P, t.E));
+        const GridPos g1 = grid_pos(P, t.E);
+        const double iL1 = interp(table(P, mat, EMX_T_MSC), g1);
         const double tau = 0.5 * (L.iL0 + iL1) * s;
-        t.u = msc_deflect(rng, tau, t.u);
+        const Vec3 u0 = t.u;
+        t.u = msc_deflect(rng, tau, u0);
         o.msc_tau = tau;
+        // R-MSC2 lateral displacement along the transverse part d of the new direction (|d| = sin(theta)) by
+        // rho = sqrt(3 <r^2> / (2 (1 - g^2))) |d|: <rho^2> = Lewis' <x^2 + y^2> for the Henyey-Greenstein angle
+        // (<sin^2> = (2/3)(1 - g^2), g = exp(-tau)); at most 0.9 of the way to the cell's boundary; none after a
+        // step that ended on a boundary
+        if (ph.msc == 2 && action != EMX_A_BOUNDARY) {
+            const double il1 = 0.5 * (L.iL0 + iL1);
+            const double il2 = 0.5 * (L.iL20 + interp(table(P, mat, EMX_T_MSC2), g1));
+            const double r2 = msc_lateral_r2(s, il1, il2);
+            const double om = -expm1(-2.0 * tau);
+            const double mu = u0.x * t.u.x + u0.y * t.u.y + u0.z * t.u.z;
+            const Vec3 d = {t.u.x - mu * u0.x, t.u.y - mu * u0.y, t.u.z - mu * u0.z};
+            const double dn = norm(d);
+            if (r2 > 0.0 && om > 0.0 && dn > 0.0) {
+                double rho = sqrt(1.5 * r2 / om) * dn;
+                const Vec3 dh = {d.x / dn, d.y / dn, d.z / dn};
+                int hs;
+                const double lim = 0.9 * distance_to_boundary(P, t.vol, t.x, dh, -1, hs);
+                if (rho > lim) rho = lim;
+                t.x.x += rho * dh.x;
+                t.x.y += rho * dh.y;
+                t.x.z += rho * dh.z;
+            }
+        }
     }
 
     // 8. discrete interaction: select with the pre-step cross sections, interact at the post-loss energy (R21)
@@ -491,7 +531,7 @@ template <bool CH, bool MAP = false, bool EXT = false>
 EMX_HD void step(const Params &P, uint64_t seed, int pt, Track &t, StepOut &o, int &n_sub) {
     Carry c;
     Lookup L;
-    L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.var0 = 0.0;
+    L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.iL20 = L.var0 = 0.0;
     L.Rtab = nullptr;
     n_sub = 0;
     step_a0<CH, EXT>(P, seed, pt, t, c, L);

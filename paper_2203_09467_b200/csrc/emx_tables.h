@@ -109,6 +109,10 @@ EMX_HD void table_pass3(const TableCtx &c, int im, int j) {
     if (c.ph.msc)
         for (int i = 0; i < m.n_elem; ++i) il += m.n_i[i] * msc_sigma1(m.Z[i], m.A[i], E);
     T[EMX_T_MSC * n + j] = il;
+    double il2 = 0.0;  // 1 / lambda_2 (R-MSC2)
+    if (c.ph.msc == 2)
+        for (int i = 0; i < m.n_elem; ++i) il2 += m.n_i[i] * msc_sigma2(m.Z[i], m.A[i], E);
+    T[EMX_T_MSC2 * n + j] = il2;
     T[EMX_T_VAR_EM * n + j] = c.ph.fluct ? m.n_e * loss_second_moment(kElectron, E, m.Tcut) : 0.0;  // R-FLUCT
     T[EMX_T_VAR_EP * n + j] = c.ph.fluct ? m.n_e * loss_second_moment(kPositron, E, m.Tcut) : 0.0;
     T[EMX_T_DEDX_EM * n + j] = dedx_total(m, kElectron, E, m.Tcut, m.kcut);

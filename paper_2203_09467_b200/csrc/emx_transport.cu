@@ -858,7 +858,7 @@ __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint6
         step0 = t.step;
         Carry cy;
         Lookup L;
-        L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.var0 = 0.0;
+        L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.iL20 = L.var0 = 0.0;
         L.Rtab = nullptr;
         if (FUSED) {
             step_a0<CH, EXT>(P, seed, pt, t, cy, L);
@@ -885,9 +885,9 @@ __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint6
         if (lane == k) list_cnt = __popc(b);
     }
     if (list_cnt) list_r0 = atomicAdd(&c->icount[POOL][lane], list_cnt);
-    // FUSED: position moved here; a2: position and direction were written by the propagation kernel, the
-    // direction changes again only through multiple scattering
-    constexpr int WR = FUSED ? (kWrX | (CH ? kWrE : 0) | (CH && EXT ? kWrU : 0)) : (kWrE | (EXT ? kWrU : 0));
+    // FUSED: position moved here; a2: position and direction were written by the propagation kernel and change
+    // again only through multiple scattering (deflection; lateral displacement of R-MSC2)
+    constexpr int WR = FUSED ? (kWrX | (CH ? kWrE : 0) | (CH && EXT ? kWrU : 0)) : (kWrE | (EXT ? (kWrU | kWrX) : 0));
     WarpAcc acc = epilogue<POOL, WR, true>(P, w, seed, tally, i, s, pt, go || tomb, tomb, pend, t, o, vol0, step0, safe);
     const int my_base = __shfl_sync(0xffffffffu, list_r0, pk >= 0 ? pk : 0);
     if (pk >= 0) w.ilist[POOL][pk][my_base + __popc(my_mask & lt)] = s;

@@ -220,6 +220,53 @@ EMX_HD double msc_sigma1(int Z, double Amass, double T) {
     return 2.0 * kPi * zz * (zz + 1.0) * c * c * (log1p(tm / A2) - tm / (tm + A2));
 }
 
+// ---- DESIGN.md R-MSC2: the spatial moments of Lewis' theory (Phys. Rev. 78 (1950) 526) for a true path t,
+// tau = t / lambda_1, kappa = lambda_1 / lambda_2:  <z> = lambda_1 (1 - exp(-tau)),
+// <x^2 + y^2> = (4 lambda_1^2 / 3) (tau - (kappa + 1) / kappa + kappa exp(-tau) / (kappa - 1) - exp(-kappa tau) / (kappa (kappa - 1)))
+// second transport cross section, cm2 per atom: the law of msc_sigma1 integrated with weight
+// 1 - P_2 = 3 t - (3/2) t^2 up to t_m:  I_1 = ln(1 + t_m / 2A) - t_m / (t_m + 2A),
+// I_2 = t_m - 4A ln(1 + t_m / 2A) + 2A t_m / (t_m + 2A),  sigma_2 = 2 pi Z (Z + 1) (re me / (beta p))^2 (3 I_1 - 3 I_2 / 2)
+EMX_HD double msc_sigma2(int Z, double Amass, double T) {
+    const double p2 = T * (T + 2.0 * kMe);
+    const double A2 = 2.0 * msc_screening(Z, T);
+    const double hbarc = kRe * kMe / kAlpha;
+    const double th_max = hbarc / (sqrt(p2) * 1.4e-13 * cbrt(Amass));
+    double tm = 0.5 * th_max * th_max;
+    if (tm > 2.0) tm = 2.0;
+    const double c = kRe * kMe * (T + kMe) / p2;
+    const double zz = (double)Z;
+    const double lg = log1p(tm / A2), fr = tm / (tm + A2);
+    const double I1 = lg - fr;
+    const double I2 = tm - 2.0 * A2 * lg + A2 * fr;
+    return 2.0 * kPi * zz * (zz + 1.0) * c * c * (3.0 * I1 - 1.5 * I2);
+}
+// phi_3(x) = (x^2 / 2 - x + 1 - exp(-x)) / x^3: series below x = 1/2 (the plain form cancels), 15 terms
+EMX_HD double msc_phi3(double x) {
+    if (x < 0.5) {
+        double s = 0.0, term = 1.0 / 6.0;
+        for (int n = 0; n <= 14; ++n) {
+            s += term;
+            term *= -x / (double)(n + 4);
+        }
+        return s;
+    }
+    return (0.5 * x * x - x - expm1(-x)) / (x * x * x);
+}
+EMX_HD double msc_geom_length(double t, double il1) {
+    const double tau = t * il1;
+    if (!(tau > 0.0)) return t;
+    return t * (-expm1(-tau) / tau);
+}
+// <x^2 + y^2>: with phi_3 for tau < 1 (the printed bracket is O(tau^3) and cancels), as printed for tau >= 1
+EMX_HD double msc_lateral_r2(double t, double il1, double il2) {
+    const double tau = t * il1;
+    if (!(tau > 0.0) || !(il2 > il1)) return 0.0;
+    const double kap = il2 / il1;
+    if (tau < 1.0) return (4.0 / 3.0) * t * t * tau * (kap / (kap - 1.0)) * (kap * msc_phi3(kap * tau) - msc_phi3(tau));
+    const double br = tau - (kap + 1.0) / kap + (kap * exp(-tau) - exp(-kap * tau) / kap) / (kap - 1.0);
+    return (4.0 / 3.0) * br / (il1 * il1);
+}
+
 EMX_HD double dedx_total(const Material &m, int ptype, double T, double Tcut, double kcut) {
     return dedx_col(m, ptype, T, Tcut) + brems_dedx(T, kcut, m.X0);
 }

@@ -2,6 +2,7 @@
 
     python -m paper_2203_09467_b200.diagnostics.ncu_extract REPORT.ncu-rep [--md OUT.md] [--json OUT.json]
                                                             [--config 4] [--build TEXT] [--command TEXT]
+                                                            [--fp64-csv FIELD.csv --fp64-json FIELD.json]
 
 Reads the report with `ncu -i REPORT --page raw --csv` (ncu must be on PATH; no GPU needed) and writes
   --md    one table, a column per captured launch: duration, grid, registers, warp instructions, lanes active per
@@ -11,6 +12,10 @@ Reads the report with `ncu -i REPORT --page raw --csv` (ncu must be on PATH; no 
           as `roofline.traffic` and uses for `roofline.alu` (it divides the fp64 instructions of k_field by the
           substep attempts of the captured launch, which the caller passes with --attempts, or leaves them per
           launch).  The measured peaks of profiles/r2_peaks.json, if present, are copied in under "peaks".
+  --fp64-csv / --fp64-json  the two outputs of the diagnostics/field_work.py pass (ncu's per-launch counter list and
+          the run's attempt count): the fp64 instructions of ALL k_field launches of that run divided by its substep
+          attempts give `fp64_inst_per_attempt` of k_field, which is what `roofline.alu` multiplies with the attempts
+          bench.py counts live.
 Never used by the product path or the tests.
 """
 import argparse
@@ -95,6 +100,33 @@ def num(v):
         return None
 
 
+def per_attempt(csv_path, json_path):
+    """sums of the counters over every k_field launch of the field_work.py run, per substep attempt of that run"""
+    with open(json_path) as f:
+        run = json.loads(f.read().strip().splitlines()[-1])
+    with open(csv_path) as f:
+        lines = [ln for ln in f if not ln.startswith("==")]
+    rows = list(csv.reader(lines))
+    hdr = rows[0]
+    ik, im, iv = hdr.index("Kernel Name"), hdr.index("Metric Name"), hdr.index("Metric Value")
+    tot, launches = {}, set()
+    for r in rows[1:]:
+        if len(r) <= iv or "k_field" not in r[ik]:
+            continue
+        v = num(r[iv])
+        if v is None:
+            continue
+        tot[r[im]] = tot.get(r[im], 0.0) + v
+        launches.add(r[0])
+    fp64 = sum(tot.get(m, 0.0) for m in ("smsp__sass_thread_inst_executed_op_dfma_pred_on.sum",
+                                         "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum",
+                                         "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum"))
+    att = float(run["attempts"])
+    return {"fp64_inst_per_attempt": fp64 / att, "thread_inst_per_attempt": tot.get("smsp__thread_inst_executed.sum", 0.0) / att,
+            "warp_inst_per_attempt": tot.get("smsp__inst_executed.sum", 0.0) / att,
+            "per_attempt_from": {"run": run, "k_field_launches": len(launches), "fp64_thread_inst": fp64}}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("report")
@@ -105,6 +137,8 @@ def main():
     ap.add_argument("--command", default="")
     ap.add_argument("--attempts", type=float, default=0.0, help="substep attempts of the captured k_field launch")
     ap.add_argument("--title", default="")
+    ap.add_argument("--fp64-csv")
+    ap.add_argument("--fp64-json")
     a = ap.parse_args()
     hdr, data = read_raw(a.report)
     idx = {h: i for i, h in enumerate(hdr)}
@@ -156,6 +190,8 @@ def main():
                 k["attempts_in_launch"] = a.attempts
                 k["fp64_inst_per_attempt"] = fp64 / a.attempts
             kernels[name] = k
+        if a.fp64_csv and a.fp64_json and "k_field" in kernels:
+            kernels["k_field"].update(per_attempt(a.fp64_csv, a.fp64_json))
         out = {"config": a.config, "build": a.build, "report": os.path.basename(a.report), "command": a.command, "kernels": kernels}
         peaks = os.path.join(os.path.dirname(os.path.abspath(a.json)), "r2_peaks.json")
         if os.path.exists(peaks):

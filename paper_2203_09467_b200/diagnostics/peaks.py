@@ -15,7 +15,6 @@ import sys
 import tempfile
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-CMD = "python -m paper_2203_09467_b200.diagnostics.peaks --json profiles/r2_peaks.json --md profiles/r2_peaks.md"
 
 
 def main():
@@ -33,6 +32,7 @@ def main():
     for r in runs[1:]:
         for k in ("fp64_dfma_tinst_per_s", "fp64_tinst_per_s", "fp64_tflops_fma", "l2_read_gbs", "l2_gbs"):
             best[k] = max(best[k], r[k])
+    CMD = "python -m paper_2203_09467_b200.diagnostics.peaks " + " ".join(sys.argv[1:])
     best["command"] = CMD
     best["runs"] = runs
     if a.json:

@@ -13,11 +13,11 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libemx.so")
-MAX_ELEM, MAX_FACES, NPROC, NTABLE, NHIST = 4, 8, 8, 19, 96
+MAX_ELEM, MAX_FACES, NPROC, NTABLE, NHIST = 4, 8, 8, 20, 96
 # the step kernels in the order of emx_get_profile / emx_get_lanes / emx_schedule.blocks_per_sm
 STAGES = ["k_a<gamma>", "k_a<charged>", "k_a0", "k_field", "k_a2", "k_b<gamma>", "k_b<charged>"]
 T_NAMES = ["compton", "photo", "pair", "moller", "brems_em", "dedx_em", "range_em", "bhabha", "brems_ep",
-           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc", "var_em", "var_ep"]
+           "annih", "dedx_ep", "range_ep", "pair_elem0", "pair_elem1", "pair_elem2", "pair_elem3", "msc", "var_em", "var_ep", "msc2"]
 T = {n: i for i, n in enumerate(T_NAMES)}
 
 
@@ -60,7 +60,7 @@ EXPORTS = ["emx_create", "emx_destroy", "emx_add_material", "emx_add_surface", "
            "emx_get_material_info", "emx_n_tally", "emx_workspace_bytes", "emx_transport", "emx_transport_host",
            "emx_staging_bytes", "emx_set_primary_offset", "emx_get_schedule", "emx_set_schedule", "emx_neighbour_candidates", "emx_reset_tallies", "emx_read_tallies", "emx_read_step_hist", "emx_last_transport_ms", "emx_set_profile", "emx_get_profile", "emx_get_lanes",
            "emx_get_iteration_log", "emx_get_iteration_times",
-           "emx_step_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_refill_plan_static", "emx_refill_plan_static_max",
+           "emx_step_batch", "emx_field_substep_batch", "emx_philox_batch", "emx_draw_batch", "emx_refill_plan", "emx_refill_plan_static", "emx_refill_plan_static_max",
            "emx_refill_plan_static_setup", "emx_last_error",
            "emx_version"]
 
@@ -97,6 +97,7 @@ def lib():
             "emx_philox_batch": (i, [l, vp, vp, vp, vp]),
             "emx_draw_batch": (i, [u64, l, vp, vp, vp, vp, vp, vp, vp]),
             "emx_refill_plan": (i, [l, l, l, vp, vp, vp, vp]),
+            "emx_field_substep_batch": (i, [vp, l, vp, vp, vp, vp, vp, vp, vp, vp]),
             "emx_refill_plan_static": (i, [l, l, l, vp, vp, vp, vp]),
             "emx_refill_plan_static_max": (l, []), "emx_refill_plan_static_setup": (i, []),
             "emx_last_error": (C.c_char_p, [vp]), "emx_version": (C.c_char_p, []),
@@ -347,6 +348,19 @@ class Problem:
         C.memmove(out, host.ctypes.data, n * C.sizeof(StepResult))
         del host
         return out
+
+
+def field_substep_batch(problem, x, u, kappa, h):
+    """Level-2 hook: one rk4_doubling substep per state in the problem's field.  Returns (x1, u1, err)."""
+    torch = _torch()
+    n = len(kappa)
+    dev = lambda a: torch.from_numpy(_np(a, np.float64)).cuda()
+    xd, ud, kd, hd = dev(x), dev(u), dev(kappa), dev(h)
+    x1, u1 = torch.empty(n, 3, dtype=torch.float64, device="cuda"), torch.empty(n, 3, dtype=torch.float64, device="cuda")
+    err = torch.empty(n, dtype=torch.float64, device="cuda")
+    ptr = lambda t: C.c_void_p(t.data_ptr())
+    problem._check(lib().emx_field_substep_batch(problem.h, n, ptr(xd), ptr(ud), ptr(kd), ptr(hd), ptr(x1), ptr(u1), ptr(err), _stream()))
+    return x1.cpu().numpy(), u1.cpu().numpy(), err.cpu().numpy()
 
 
 def philox_batch(ctr, key):

@@ -331,3 +331,42 @@ def test_paper_verification_problem_geometry(emo):
     assert len(r["edep"]) == 28
     assert r["edep"].sum() + r["escaped"] + r["looper"] == pytest.approx(r["E_in"], rel=1e-11)
     assert r["edep"][13] + r["edep"][14] > 0.4 * r["E_in"]            # isotropic source: most energy near z = 0
+
+
+def test_longitudinal_shower_profile_of_1_gev_electrons_in_lead(emo):
+    """Shower shape pinned by what cascade theory and the PDG review fix (SURVEY C13 keeps the
+    rest of the aggregate physics "parity unpinned"): in units of the radiation length t = z / X0 the longitudinal
+    profile of an electron-induced shower peaks at t_max = ln(E / E_c) - 0.5 with E_c = 610 MeV / (Z + 1.24)
+    (PDG, "Passage of particles through matter", electromagnetic cascades: Rossi's critical energy for solids and the
+    shower-maximum rule), and 95 % of the energy lies within t_max + 0.08 Z + 9.6 radiation lengths (same review,
+    longitudinal containment).  300 showers of 1 GeV in 60 lead slabs of X0 / 2, 1 m wide."""
+    X0 = emo.Problem(W.config1(1)[0]).material_info(0)["X0"]
+    nz, dz = 60, 0.5 * X0
+    surfaces = [(W.PX, -50.0), (W.PX, 50.0), (W.PY, -50.0), (W.PY, 50.0)] + [(W.PZ, k * dz) for k in range(nz + 1)]
+    volumes = [dict(surf=[0, 1, 2, 3, 4 + k, 5 + k], sense=[1, -1, 1, -1, 1, -1], material=0, tally=k) for k in range(nz)]
+    desc = dict(name="pb_slabs", seed=11, materials=[W.PB], surfaces=surfaces, volumes=volumes, field=(0.0, 0.0, 0.0),
+                physics=W.physics(), n_slots=1 << 16, queue_capacity=1 << 20)
+    n = 300
+    prim = W._prim(n, 1, 1000.0, (0, 0, 0), (0, 0, 1), 0, 4)
+    r = emo.Problem(desc).transport(prim, 11)
+    prof = r["edep"] / r["edep"].sum()
+    assert r["edep"].sum() + r["escaped"] == pytest.approx(r["E_in"], rel=1e-9)
+    assert r["escaped"] / r["E_in"] < 0.01                                # 30 X0 deep, 1 m wide
+    t = (np.arange(nz) + 0.5) * 0.5                                       # slab centres in radiation lengths
+    Ec = 610.0 / (82 + 1.24)
+    t_max = math.log(1000.0 / Ec) - 0.5                                   # 4.41
+    # maximum of the profile: vertex of the parabola through the highest slab and its neighbours
+    k = int(np.argmax(prof))
+    y0, y1, y2 = prof[k - 1], prof[k], prof[k + 1]
+    peak = t[k] + 0.5 * 0.5 * (y0 - y2) / (y0 - 2 * y1 + y2)
+    assert abs(peak - t_max) < 1.0, (peak, t_max)
+    # a gamma-distribution profile t^(a-1) e^(-b t) with b = 0.5 (lead, 1 GeV) has its mean 1 / b beyond the maximum
+    mean = float((t * prof).sum())
+    assert t_max + 1.0 < mean < t_max + 3.5, (mean, t_max)
+    L95 = t_max + 0.08 * 82 + 9.6                                         # 20.6 X0
+    inside = float(prof[t < L95].sum())
+    assert 0.92 < inside < 0.99, inside
+    # and the profile rises to its maximum and falls after it (smoothed over 3 slabs: 300 showers fluctuate)
+    sm = np.convolve(prof, np.ones(3) / 3, mode="valid")
+    ks = int(np.argmax(sm))
+    assert np.all(np.diff(sm[:ks + 1]) > 0) and np.all(np.diff(sm[ks + 3:ks + 30]) < 0)
