@@ -109,6 +109,7 @@ typedef struct {
     double msc_fr;               /* step limit s <= max(msc_fr * max(R, lambda_1), msc_smin) */
     double msc_smin;             /* cm */
     int fluct;                   /* 1: energy-loss fluctuations of e+- (DESIGN.md R-FLUCT) */
+    int integrator;              /* field propagation: 0 classical RK4 with step doubling (R-C9), 1 Dormand-Prince 5(4) (R-INT) */
 } emo_physics;
 
 typedef struct {
@@ -211,6 +212,9 @@ int emo_set_field(emo_problem *p, double Bx, double By, double Bz);
 int emo_set_field_fringe(emo_problem *p, double z0_cm, double a_cm);
 /* g(x) of the field set on p (Bhat for the uniform field) */
 void emo_field_profile(const emo_problem *p, const double x[3], double g[3]);
+/* Dormand-Prince 5(4) step (DESIGN.md R-INT): x1, u1 = fifth-order solution (u1 normalised), err = |x_5 - x_4| */
+void emo_dp45(const emo_problem *p, const double x[3], const double u[3], double kappa, double h,
+              double x1[3], double u1[3], double *err);
 /* step doubling as emo_rk4_doubling, the field evaluated at the stage positions */
 void emo_rk4_doubling_map(const emo_problem *p, const double x[3], const double u[3], double kappa, double h,
                           double x1[3], double u1[3], double *err);

@@ -23,7 +23,8 @@ class Physics(C.Structure):
                 ("E_trk", C.c_double), ("prod_cut_cm", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("lin_loss", C.c_double), ("field_eps", C.c_double), ("max_substeps", C.c_int),
                 ("vacuum_step", C.c_double), ("max_steps", C.c_int), ("deposit_e_at_creation", C.c_int),
-                ("msc", C.c_int), ("msc_fr", C.c_double), ("msc_smin", C.c_double), ("fluct", C.c_int)]
+                ("msc", C.c_int), ("msc_fr", C.c_double), ("msc_smin", C.c_double), ("fluct", C.c_int),
+                ("integrator", C.c_int)]
 
 
 class Track(C.Structure):
@@ -79,6 +80,7 @@ def lib():
             "emo_add_volume": (i, [p, i, ip, ip, i, i]), "emo_set_field": (i, [p, d, d, d]), "emo_set_field_fringe": (i, [p, d, d]),
             "emo_field_profile": (None, [p, dp, dp]),
             "emo_rk4_doubling_map": (None, [p, dp, dp, d, d, dp, dp, dp]),
+            "emo_dp45": (None, [p, dp, dp, d, d, dp, dp, dp]),
             "emo_set_physics": (i, [p, C.POINTER(Physics)]), "emo_set_cuts": (i, [p, i, d, d]),
             "emo_build_tables": (i, [p]), "emo_get_table": (i, [p, i, i, dp, i]),
             "emo_get_material_info": (i, [p, i, dp]), "emo_lookup": (d, [p, i, i, d]),

@@ -90,6 +90,49 @@ void emo_rk4_doubling_map(const emo_problem *p, const double x[3], const double 
     u1[0] /= n; u1[1] /= n; u1[2] /= n;
 }
 
+/* ---- second integrator (DESIGN.md R-INT; "different integration algorithms"): the embedded pair of
+ * Dormand and Prince, J. Comput. Appl. Math. 6 (1980) 19, RK5(4)7M.  Seven stages (the seventh is the fifth-order
+ * solution itself), the fifth-order solution is advanced, err = |x_5 - x_4| = h |sum_i e_i k_i^x| (positions only, as
+ * for the step doubling), u renormalised.  The field is taken at the stage positions (emo_field_profile returns the
+ * constant direction of a uniform field).  Sums run over j ascending from 0.0. */
+static const double DP_A[7][6] = {
+    { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 },
+    { 1.0 / 5.0, 0.0, 0.0, 0.0, 0.0, 0.0 },
+    { 3.0 / 40.0, 9.0 / 40.0, 0.0, 0.0, 0.0, 0.0 },
+    { 44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0, 0.0, 0.0, 0.0 },
+    { 19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0, 0.0, 0.0 },
+    { 9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0.0 },
+    { 35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0 } };
+static const double DP_E[7] = { 71.0 / 57600.0, 0.0, -71.0 / 16695.0, 71.0 / 1920.0, -17253.0 / 339200.0, 22.0 / 525.0,
+                                -1.0 / 40.0 };
+
+void emo_dp45(const emo_problem *p, const double x[3], const double u[3], double kappa, double h,
+              double x1[3], double u1[3], double *err) {
+    double kx[7][3], ku[7][3], xs[3], us[3], g[3];
+    for (int s = 0; s < 7; ++s) {
+        for (int i = 0; i < 3; ++i) {
+            double ax = 0.0, au = 0.0;
+            for (int j = 0; j < s; ++j) { ax += DP_A[s][j] * kx[j][i]; au += DP_A[s][j] * ku[j][i]; }
+            xs[i] = x[i] + h * ax;
+            us[i] = u[i] + h * au;
+        }
+        emo_field_profile(p, xs, g);
+        rhs(us, kappa, g, kx[s], ku[s]);
+    }
+    /* xs, us of the seventh stage are the fifth-order solution */
+    double e[3];
+    for (int i = 0; i < 3; ++i) {
+        double a = 0.0;
+        for (int j = 0; j < 7; ++j) a += DP_E[j] * kx[j][i];
+        e[i] = h * a;
+        x1[i] = xs[i];
+        u1[i] = us[i];
+    }
+    *err = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+    double n = sqrt(u1[0] * u1[0] + u1[1] * u1[1] + u1[2] * u1[2]);
+    u1[0] /= n; u1[1] /= n; u1[2] /= n;
+}
+
 /* propagate up to s_max inside cell `vol`; returns the arc length travelled,
  * *hit = surface reached (-1: none).  x, u are updated in place. */
 double emo_propagate_field(const emo_problem *p, int vol, int *surf_io, double x[3], double u[3],
@@ -114,7 +157,8 @@ double emo_propagate_field_n(const emo_problem *p, int vol, int *surf_io, double
         double rem = s_max - s_done;
         if (h > rem) h = rem;
         double x1[3], u1[3], err;
-        if (p->field_kind == 0) emo_rk4_doubling(x, u, kappa, p->Bhat, h, x1, u1, &err);
+        if (p->ph.integrator == 1) emo_dp45(p, x, u, kappa, h, x1, u1, &err);
+        else if (p->field_kind == 0) emo_rk4_doubling(x, u, kappa, p->Bhat, h, x1, u1, &err);
         else emo_rk4_doubling_map(p, x, u, kappa, h, x1, u1, &err);
         if (err > eps && h > 1e-9) {
             double f = 0.9 * pow(eps / err, 0.2);

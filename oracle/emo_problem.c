@@ -18,7 +18,7 @@ emo_problem *emo_create(void) {
     ph->alpha_R = 0.2; ph->rho_R = 0.1; ph->lin_loss = 0.01;
     ph->field_eps = 1e-7; ph->max_substeps = 1000; ph->vacuum_step = 1e3;
     ph->max_steps = 10000; ph->deposit_e_at_creation = 0;
-    ph->msc = 0; ph->msc_fr = 0.2; ph->msc_smin = 1e-3; ph->fluct = 0;
+    ph->msc = 0; ph->msc_fr = 0.2; ph->msc_smin = 1e-3; ph->fluct = 0; ph->integrator = 0;
     return p;
 }
 
@@ -96,6 +96,7 @@ int emo_set_field_fringe(emo_problem *p, double z0_cm, double a_cm) {
 int emo_set_physics(emo_problem *p, const emo_physics *ph) {
     if (ph->n_E < 2 || !(ph->E_max > ph->E_min) || !(ph->E_min > 0.0)) return -1;
     if (ph->msc < 0 || ph->msc > 2) return -1;
+    if (ph->integrator < 0 || ph->integrator > 1) return -1;
     if (ph->msc && (!(ph->msc_fr > 0.0) || !(ph->msc_smin > 0.0))) return -1;
     p->ph = *ph; p->built = 0;
     return 0;

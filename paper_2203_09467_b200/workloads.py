@@ -27,7 +27,7 @@ def physics(**kw):
     ph = dict(process_mask=63, E_min=1e-3, E_max=1e4, n_E=256, E_trk=1e-3, prod_cut_cm=0.07,
               alpha_R=0.2, rho_R=0.1, lin_loss=0.01, field_eps=1e-7, max_substeps=1000,
               vacuum_step=1e3, max_steps=10000, deposit_e_at_creation=0,
-              msc=0, msc_fr=0.2, msc_smin=1e-3, fluct=0)
+              msc=0, msc_fr=0.2, msc_smin=1e-3, fluct=0, integrator=0)
     ph.update(kw)
     return ph
 
