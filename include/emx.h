@@ -142,6 +142,10 @@ typedef struct {
      * about its mean with that variance times s, clamped to [0, min(2 mean, E)] (two draws, taken right after
      * draw 0 and before those of the multiple scattering); a range stop is not fluctuated. */
     int32_t fluct;
+    /* Integrator of the field propagation ("different integration algorithms"): 0 = classical RK4 with step
+     * doubling (C9; what B:configs names), 1 = the embedded Dormand-Prince 5(4) pair (DESIGN.md R-INT) --
+     * same step-size rule, boundary search and landing tolerance, fewer and longer substeps on smooth stretches. */
+    int32_t integrator;
 } emx_physics;
 
 /* run totals (PAPER.md:176 energy deposition; Fig. 5 diagnostics PAPER.md:204-212) */

@@ -273,6 +273,7 @@ int emx_set_physics(emx_problem *p, const emx_physics *ph) {
         !(ph->field_eps > 0.0) || !(ph->vacuum_step > 0.0))
         return fail(p, EMX_E_ARG, "emx_set_physics: invalid grid or limits");
     if (ph->msc < 0 || ph->msc > 2) return fail(p, EMX_E_ARG, "emx_set_physics: msc is 0, 1 or 2");
+    if (ph->integrator < 0 || ph->integrator > 1) return fail(p, EMX_E_ARG, "emx_set_physics: integrator is 0 or 1");
     if (ph->msc && (!(ph->msc_fr > 0.0) || !(ph->msc_smin > 0.0)))
         return fail(p, EMX_E_ARG, "emx_set_physics: multiple scattering needs msc_fr > 0 and msc_smin > 0");
     p->hp.ph = *ph;

@@ -114,6 +114,70 @@ EMX_NI void rk4_doubling(const Params &P, const Vec3 &x, const Vec3 &u, double k
     u1.z /= n;
 }
 
+// ---- second integrator (DESIGN.md R-INT; "different integration algorithms"): the embedded pair of Dormand
+// and Prince (RK5(4)7M, J. Comput. Appl. Math. 6 (1980) 19).  Seven stages with the field at the stage positions, the
+// fifth-order solution (= the state of the seventh stage) is advanced, err = |x_5 - x_4| = h |sum_i e_i k_i^x|, u
+// renormalised.  Stage sums in ascending order (terms with a zero coefficient left out: they add a signed zero).
+template <bool MAP, int AX>
+EMX_NI void dp45_step(const Params &P, const Vec3 &x, const Vec3 &u, double kappa, double h, Vec3 &x1, Vec3 &u1, double &err) {
+    constexpr double A[7][6] = {{0.0, 0.0, 0.0, 0.0, 0.0, 0.0},
+                                {1.0 / 5.0, 0.0, 0.0, 0.0, 0.0, 0.0},
+                                {3.0 / 40.0, 9.0 / 40.0, 0.0, 0.0, 0.0, 0.0},
+                                {44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0, 0.0, 0.0, 0.0},
+                                {19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0, 0.0, 0.0},
+                                {9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0.0},
+                                {35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0}};
+    constexpr double E[7] = {71.0 / 57600.0, 0.0, -71.0 / 16695.0, 71.0 / 1920.0, -17253.0 / 339200.0, 22.0 / 525.0, -1.0 / 40.0};
+    Vec3 kx[7], ku[7];  // dx/ds = the stage direction, du/ds = kappa u x Bhat at the stage
+    Vec3 xs = x, us = u;
+#pragma unroll
+    for (int s = 0; s < 7; ++s) {
+        if (s > 0) {
+            Vec3 ax = {0.0, 0.0, 0.0}, au = {0.0, 0.0, 0.0};
+#pragma unroll
+            for (int j = 0; j < s; ++j) {
+                if (A[s][j] == 0.0) continue;
+                ax.x += A[s][j] * kx[j].x;
+                ax.y += A[s][j] * kx[j].y;
+                ax.z += A[s][j] * kx[j].z;
+                if (AX != 0) au.x += A[s][j] * ku[j].x;
+                if (AX != 1) au.y += A[s][j] * ku[j].y;
+                if (AX != 2) au.z += A[s][j] * ku[j].z;
+            }
+            xs = {x.x + h * ax.x, x.y + h * ax.y, x.z + h * ax.z};
+            us = {AX == 0 ? u.x : u.x + h * au.x, AX == 1 ? u.y : u.y + h * au.y, AX == 2 ? u.z : u.z + h * au.z};
+        }
+        kx[s] = us;
+        if (MAP) {
+            double g[3];
+            field_profile(P, xs, g);
+            ku[s] = lorentz<kAxisAny>(us, kappa, g);
+        } else {
+            ku[s] = lorentz<AX>(us, kappa, P.Bhat);
+        }
+    }
+    Vec3 e = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int j = 0; j < 7; ++j) {
+        if (E[j] == 0.0) continue;
+        e.x += E[j] * kx[j].x;
+        e.y += E[j] * kx[j].y;
+        e.z += E[j] * kx[j].z;
+    }
+    e = {h * e.x, h * e.y, h * e.z};
+    err = norm(e);
+    x1 = xs;
+    const double n = norm(us);
+    u1 = {us.x / n, us.y / n, us.z / n};
+}
+
+// one substep with integrator INTEG (0: step doubling, 1: Dormand-Prince)
+template <bool MAP, int AX, int INTEG>
+EMX_HD void field_substep(const Params &P, const Vec3 &x, const Vec3 &u, double kappa, double h, Vec3 &x1, Vec3 &u1, double &err) {
+    if (INTEG == 1) dp45_step<MAP, AX>(P, x, u, kappa, h, x1, u1, err);
+    else rk4_doubling<MAP, AX>(P, x, u, kappa, h, x1, u1, err);
+}
+
 // x^(1/5) for the step-size control, x in [1e-30, 1e30], within 1 ulp: r ~ x^(-1/5) from a single-precision seed of
 // the special-function unit (relative error below 1e-5) and two Newton steps r <- r (6 - x r^5) / 5 (each squares the
 // error times 3: 3e-10, then below rounding), y = x r^4, and one Newton step of y^5 = x with 1 / (5 y^4) = r^4 / 5
@@ -156,7 +220,7 @@ EMX_HD void field_begin(double kappa, double s_max, FieldState &fs) {
 // the track sits on) and fs are updated.  Returns true when the propagation is over: s = arc length travelled,
 // hit = surface reached (-1 none: s_max travelled, or the max_substeps attempts of the step are used up).
 // cell = the faces of the track's cell (Params::faces, or the kernel's copy of it in shared memory).
-template <bool MAP, int AX>
+template <bool MAP, int AX, int INTEG = 0>
 EMX_NI bool field_attempt(const Params &P, const Face *cell, int &on_surf, Vec3 &x, Vec3 &u, double kappa, double s_max,
                           FieldState &fs, int &hit, double &s) {
     const double eps = P.ph.field_eps;
@@ -165,7 +229,7 @@ EMX_NI bool field_attempt(const Params &P, const Face *cell, int &on_surf, Vec3 
     if (h > rem) h = rem;
     Vec3 x1, u1;
     double err;
-    rk4_doubling<MAP, AX>(P, x, u, kappa, h, x1, u1, err);
+    field_substep<MAP, AX, INTEG>(P, x, u, kappa, h, x1, u1, err);
     hit = -1;
     // the two places of C9 that rescale h by 0.9 (eps / e)^(1/5) -- shrink after a rejected substep, grow after an
     // accepted one -- share ONE evaluation of the power, so that lanes which shrink and lanes which grow do not
@@ -253,7 +317,12 @@ EMX_NI double propagate_field(const Params &P, int vol, int &on_surf, Vec3 &x, V
     n_attempts = 0;
     const Face *cell = P.faces + (size_t)vol * EMX_MAX_FACES;
     while (!done) {
-        if (MAP || ax == kAxisAny) done = field_attempt<MAP, kAxisAny>(P, cell, on_surf, x, u, kappa, s_max, fs, hit, s);
+        if (P.ph.integrator == 1) {
+            if (MAP || ax == kAxisAny) done = field_attempt<MAP, kAxisAny, 1>(P, cell, on_surf, x, u, kappa, s_max, fs, hit, s);
+            else if (ax == 0) done = field_attempt<false, 0, 1>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
+            else if (ax == 1) done = field_attempt<false, 1, 1>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
+            else done = field_attempt<false, 2, 1>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
+        } else if (MAP || ax == kAxisAny) done = field_attempt<MAP, kAxisAny>(P, cell, on_surf, x, u, kappa, s_max, fs, hit, s);
         else if (ax == 0) done = field_attempt<false, 0>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
         else if (ax == 1) done = field_attempt<false, 1>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);
         else done = field_attempt<false, 2>(P, cell, on_surf, x, u, kb, s_max, fs, hit, s);

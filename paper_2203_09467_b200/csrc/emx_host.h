@@ -41,6 +41,7 @@ struct HostProblem {
         ph.msc = 0;
         ph.msc_fr = 0.2;
         ph.msc_smin = 1e-3;
+        ph.integrator = 0;
         ph.fluct = 0;
     }
 };

@@ -58,7 +58,13 @@ __global__ void k_field_substep_batch(Params P, long n, const double *x3, const 
     Vec3 xo, uo;
     double e;
     const int ax = P.field_kind == 0 ? field_axis(P.Bhat) : kAxisAny;
-    if (P.field_kind != 0) rk4_doubling<true, kAxisAny>(P, x, u, kappa[i], h[i], xo, uo, e);
+    if (P.ph.integrator == 1) {
+        if (P.field_kind != 0) dp45_step<true, kAxisAny>(P, x, u, kappa[i], h[i], xo, uo, e);
+        else if (ax == 0) dp45_step<false, 0>(P, x, u, kappa[i] * P.Bhat[0], h[i], xo, uo, e);
+        else if (ax == 1) dp45_step<false, 1>(P, x, u, kappa[i] * P.Bhat[1], h[i], xo, uo, e);
+        else if (ax == 2) dp45_step<false, 2>(P, x, u, kappa[i] * P.Bhat[2], h[i], xo, uo, e);
+        else dp45_step<false, kAxisAny>(P, x, u, kappa[i], h[i], xo, uo, e);
+    } else if (P.field_kind != 0) rk4_doubling<true, kAxisAny>(P, x, u, kappa[i], h[i], xo, uo, e);
     else if (ax == 0) rk4_doubling<false, 0>(P, x, u, kappa[i] * P.Bhat[0], h[i], xo, uo, e);
     else if (ax == 1) rk4_doubling<false, 1>(P, x, u, kappa[i] * P.Bhat[1], h[i], xo, uo, e);
     else if (ax == 2) rk4_doubling<false, 2>(P, x, u, kappa[i] * P.Bhat[2], h[i], xo, uo, e);

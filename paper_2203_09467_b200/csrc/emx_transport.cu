@@ -1008,7 +1008,7 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_0) k_a0(const __grid_co
 // of an iteration that way once the field had its true strength).  A track may be parked after field_min
 // attempts once the pool has no track left to hand out (or after slice_max attempts): its loop variables go to
 // the slot and the next iteration continues the SAME sequence of substeps.
-template <bool MAP, int AX>
+template <bool MAP, int AX, int INTEG = 0>
 __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid_constant__ Params P, const __grid_constant__ Work w,
                                                                     int stage_faces) {
     // the face table of the whole geometry (16 B per face) is staged in shared memory when it fits: every attempt
@@ -1076,7 +1076,7 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid
         if (have) {
             int hit;
             double sres;
-            const bool done = field_attempt<MAP, AX>(P, faces + vol * EMX_MAX_FACES, surf, x, u, kappa, s_max, fs, hit, sres);
+            const bool done = field_attempt<MAP, AX, INTEG>(P, faces + vol * EMX_MAX_FACES, surf, x, u, kappa, s_max, fs, hit, sres);
             used += 1;
             n_att += 1;
             if (done) {
@@ -1249,7 +1249,13 @@ cudaError_t launch_stage(int stage, const Params &P, const Work &w, uint64_t see
         const size_t fb = (size_t)P.n_vol * EMX_MAX_FACES * sizeof(Face);
         const int stage = (w.stage_faces && fb <= 40 * 1024) ? 1 : 0;
         const size_t sm = stage ? fb : 0;
-        if (P.field_kind != 0) k_field<true, kAxisAny><<<g, kStepBlock, sm, st>>>(P, w, stage);
+        if (P.ph.integrator == 1) {  // Dormand-Prince 5(4) (DESIGN.md R-INT): instantiations of their own
+            if (P.field_kind != 0) k_field<true, kAxisAny, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);
+            else if (ax == 0) k_field<false, 0, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);
+            else if (ax == 1) k_field<false, 1, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);
+            else if (ax == 2) k_field<false, 2, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);
+            else k_field<false, kAxisAny, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);
+        } else if (P.field_kind != 0) k_field<true, kAxisAny><<<g, kStepBlock, sm, st>>>(P, w, stage);
         else if (ax == 0) k_field<false, 0><<<g, kStepBlock, sm, st>>>(P, w, stage);
         else if (ax == 1) k_field<false, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);
         else if (ax == 2) k_field<false, 2><<<g, kStepBlock, sm, st>>>(P, w, stage);

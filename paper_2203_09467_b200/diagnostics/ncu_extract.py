@@ -49,6 +49,13 @@ ROWS = [
     ("lts__t_sector_hit_rate.pct", "L2 hit (%)", 1),
     ("l1tex__t_sector_hit_rate.pct", "L1 hit (%)", 1),
     ("l1tex__data_pipe_lsu_wavefronts_mem_lg.sum", "L1 wavefronts, global + local (M)", 1e-6),
+    ("l1tex__t_requests_pipe_lsu_mem_global_op_ld.sum", "global load requests = warp-level load instructions (M)", 1e-6),
+    ("l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum", "global load sectors of 32 B (M)", 1e-6),
+    ("l1tex__t_requests_pipe_lsu_mem_global_op_st.sum", "global store requests (M)", 1e-6),
+    ("l1tex__t_sectors_pipe_lsu_mem_global_op_st.sum", "global store sectors (M)", 1e-6),
+    ("l1tex__t_requests_pipe_lsu_mem_local_op_ld.sum", "local (spill) load requests (M)", 1e-6),
+    ("l1tex__t_requests_pipe_lsu_mem_local_op_st.sum", "local (spill) store requests (M)", 1e-6),
+    ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", "shared-memory wavefronts (M)", 1e-6),
     ("smsp__inst_executed_op_global_ld.sum", "global load instructions (M)", 1e-6),
     ("smsp__inst_executed_op_global_st.sum", "global store instructions (M)", 1e-6),
     ("smsp__inst_executed_op_local_ld.sum", "local (spill) load instructions (M)", 1e-6),

@@ -26,7 +26,8 @@ class Physics(C.Structure):
                 ("E_trk", C.c_double), ("prod_cut_cm", C.c_double), ("alpha_R", C.c_double), ("rho_R", C.c_double),
                 ("lin_loss", C.c_double), ("field_eps", C.c_double), ("max_substeps", C.c_int32),
                 ("vacuum_step", C.c_double), ("max_steps", C.c_int32), ("deposit_e_at_creation", C.c_int32),
-                ("msc", C.c_int32), ("msc_fr", C.c_double), ("msc_smin", C.c_double), ("fluct", C.c_int32)]
+                ("msc", C.c_int32), ("msc_fr", C.c_double), ("msc_smin", C.c_double), ("fluct", C.c_int32),
+                ("integrator", C.c_int32)]
 
 
 class Scalars(C.Structure):

@@ -99,7 +99,8 @@ def _workload(cfg, n):
     lateral displacement), with / without / with fluctuations"""
     ext = {37: dict(msc=1, msc_fr=0.2, msc_smin=1e-3), 47: dict(msc=1, msc_fr=0.1, msc_smin=2e-3, fluct=1), 17: dict(fluct=1),
            27: dict(msc=2, msc_fr=0.2, msc_smin=1e-3, fluct=1), 38: dict(msc=2, msc_fr=0.2, msc_smin=1e-3),
-           48: dict(msc=2, msc_fr=0.1, msc_smin=2e-3, fluct=1)}
+           48: dict(msc=2, msc_fr=0.1, msc_smin=2e-3, fluct=1),
+           43: dict(integrator=1), 63: dict(integrator=1)}      # the Dormand-Prince integrator (R-INT): barrel at 4 T, fringe field
     if cfg in ext:
         desc, prim = W.get(cfg // 10, n)
         desc = dict(desc, physics=dict(desc["physics"], **ext[cfg]), seed=cfg)
@@ -128,7 +129,7 @@ def test_tables_match_the_oracle(emx, emo, cfg):
 # ---------------- level 2: single step ----------------
 
 @pytest.mark.parametrize("cfg,n", [(0, 20000), (1, 40000), (2, 40000), (3, 40000), (4, 40000), (5, 20000), (6, 40000),
-                                   (7, 40000), (17, 40000), (37, 40000), (47, 40000), (27, 40000), (38, 40000), (48, 40000)])
+                                   (7, 40000), (17, 40000), (37, 40000), (47, 40000), (27, 40000), (38, 40000), (48, 40000), (43, 40000), (63, 40000)])
 def test_single_step_parity(emx, emo, cfg, n):
     desc, _ = _workload(cfg, 4)
     G, O = emx.Problem(desc), emo.Problem(desc)
@@ -146,7 +147,7 @@ def test_single_step_parity(emx, emo, cfg, n):
     assert worst <= 1.0, {k: v for k, v in rep.items() if isinstance(v, float) and v > 0.5}
     plain = (ref["n_sub"] == 0) & (tol["E"] == states.RTOL2)      # the plain 1e-12 of north_star holds for these
     assert plain.sum() > n // 4 and np.all(tol["u"][plain] == states.RTOL2) and np.all(tol["x"][plain] == states.RTOL2)
-    if cfg in (3, 4, 6, 37, 47, 38, 48):
+    if cfg in (3, 4, 6, 37, 47, 38, 48, 43, 63):
         assert tol["trunc"].sum() <= n // 6 and (ref["n_sub"] > 1).sum() > n // 10
     # coverage of the branches
     acts = np.bincount(ref["action"], minlength=6)
@@ -171,16 +172,18 @@ def _per_primary_se(o):
     return o["per_prim_tally"].std(axis=0, ddof=1) / np.sqrt(n), o["per_prim"].std(axis=0, ddof=1) / np.sqrt(n)
 
 
+@pytest.mark.parametrize("integrator", [0, 1])
 @pytest.mark.parametrize("field,fringe", [((0.0, 1.0, 0.0), None), ((0.0, 0.0, -4.0), None), ((1.0, -2.0, 0.5), None),
                                           ((0.0, 0.0, 3.8), (120.0, 15.0))])
-def test_one_field_substep_at_1e_12(emx, emo, field, fringe):
-    """Level 2 for ONE substep of the propagation: rk4_doubling of the kernel (axis-specialised
-    for a field along +-x, +-y, +-z; general; field map) against the oracle's, state by state.  One substep is a
+def test_one_field_substep_at_1e_12(emx, emo, field, fringe, integrator):
+    """Level 2 for ONE substep of the propagation: rk4_doubling (integrator 0) and the Dormand-Prince
+    step (integrator 1) of the kernel (axis-specialised for a field along +-x, +-y, +-z; general; field map) against the
+    oracle's, state by state.  One substep is a
     fixed sequence of IEEE operations on both sides, so 1e-12 holds without any allowance: positions relative to
     max(|x|, h), directions absolute (unit vectors), and the error estimate -- a DIFFERENCE of two positions, so its
     rounding is that of the positions -- absolute on the same scale."""
     desc, _ = W.get(4, 4)
-    desc = dict(desc, field=field)
+    desc = dict(desc, field=field, physics=dict(desc["physics"], integrator=integrator))
     if fringe:
         desc["field_fringe"] = fringe
     G, O = emx.Problem(desc), emo.Problem(desc)
@@ -202,7 +205,9 @@ def test_one_field_substep_at_1e_12(emx, emo, field, fringe):
     for i in range(n):
         a = (x[i].ctypes.data_as(dp), u[i].ctypes.data_as(dp))
         o = (ox[i].ctypes.data_as(dp), ou[i].ctypes.data_as(dp), C.byref(e))
-        if fringe:
+        if integrator == 1:
+            L.emo_dp45(O.h, a[0], a[1], kappa[i], h[i], *o)
+        elif fringe:
             L.emo_rk4_doubling_map(O.h, a[0], a[1], kappa[i], h[i], *o)
         else:
             L.emo_rk4_doubling(a[0], a[1], kappa[i], Bhat.ctypes.data_as(dp), h[i], *o)
@@ -218,7 +223,7 @@ def test_one_field_substep_at_1e_12(emx, emo, field, fringe):
 @pytest.mark.parametrize("cfg,n,n_slots", [(0, 1000, 1024), (1, 300, 1 << 16), (2, 24, 1 << 16), (3, 24, 1 << 16),
                                            (4, 48, 1 << 16), (1, 64, 1024), (5, 400, 1 << 16), (6, 48, 1 << 16),
                                            (7, 24, 1 << 16), (17, 300, 1 << 16), (37, 24, 1 << 16), (47, 48, 1 << 16),
-                                           (27, 24, 1 << 16), (48, 48, 1 << 16)])
+                                           (27, 24, 1 << 16), (48, 48, 1 << 16), (43, 48, 1 << 16)])
 def test_transport_parity_and_energy_closure(emx, emo, cfg, n, n_slots):
     desc, prim = _workload(cfg, n)
     G, O = emx.Problem(desc), emo.Problem(desc)
