@@ -355,9 +355,10 @@ int emx_step_batch(emx_problem *p, uint64_t seed, long n, const emx_track *in, e
                    void *stream);
 
 /* Level-2 parity hook for ONE substep of the field propagation (C9): for each of n states
- * (x, u, curvature kappa [1/cm, signed], trial step h [cm]) one RK4 step of h against two of h / 2 in the problem's
- * field, exactly as the propagation kernel runs it -- x1, u1 = state after the two half steps (u1 normalised),
- * err = |x_full - x_half|.  All pointers DEVICE; x3, u3, x1, u1 hold 3 n doubles (xyz per state).  EMX_E_STATE
+ * (x, u, curvature kappa [1/cm, signed], trial step h [cm]) one substep of the problem's integrator in the problem's
+ * field, exactly as the propagation kernel runs it -- integrator 0: one RK4 step of h against two of h / 2, x1, u1 =
+ * state after the two half steps, err = |x_full - x_half|; integrator 1: one Dormand-Prince step, x1, u1 = fifth-order
+ * solution, err = |x_5 - x_4|; u1 normalised.  All pointers DEVICE; x3, u3, x1, u1 hold 3 n doubles (xyz per state).  EMX_E_STATE
  * when no field is set. */
 int emx_field_substep_batch(emx_problem *p, long n, const double *x3, const double *u3, const double *kappa,
                             const double *h, double *x1, double *u1, double *err, void *stream);
