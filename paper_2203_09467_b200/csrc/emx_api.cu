@@ -495,7 +495,7 @@ static int transport_device(emx_problem *p, const Primaries &pr, uint64_t seed, 
     w.slice_min = p->sched.slice_min > 0 ? p->sched.slice_min : 1;
     w.slice_max = p->sched.slice_max >= w.slice_min ? p->sched.slice_max : w.slice_min;
     size_grids(p, w);
-    w.stage_faces = p->sched.blocks_per_sm[7] == 1 ? 1 : 0;  // entry 7 of the schedule: 1 switches the staging on
+    w.stage_faces = p->sched.blocks_per_sm[7] & 3;  // entry 7 of the schedule: staging switches (bit 0 faces, bit 1 photon tables)
     const bool field = p->P.Bmag != 0.0;
     const int per_iter = launches_per_iteration(field);
     CU(cudaEventRecord(p->ev0, st));

@@ -102,15 +102,19 @@ struct Lookup {
     double var0;  // variance of the loss per unit path (R-FLUCT)
     const double *Rtab;
 };
+// gtab: the photon kernel's shared-memory copy of its three tables per material ([mat][3][n_E], emx_schedule entry 7
+// bit 1; nullptr: the tables are read from global memory through L1)
 template <bool CH, bool EXT>
-EMX_HD void lookup_tables(const Params &P, int pt, int mat, double E, Lookup &L) {
+EMX_HD void lookup_tables(const Params &P, int pt, int mat, double E, Lookup &L, const double *gtab = nullptr) {
     const GridPos g = grid_pos(P, E);
     L.D = L.R = L.iL0 = L.iL20 = L.var0 = 0.0;
     L.Rtab = nullptr;
     if (!CH) {
-        L.Sig0 = interp(table(P, mat, EMX_T_COMPTON), g);
-        L.Sig1 = interp(table(P, mat, EMX_T_PHOTO), g);
-        L.Sig2 = interp(table(P, mat, EMX_T_PAIR), g);
+        const size_t nE = (size_t)P.ph.n_E;
+        const double *T0 = gtab ? gtab + (size_t)mat * 3 * nE : table(P, mat, EMX_T_COMPTON);  // kinds 0, 1, 2 are adjacent
+        L.Sig0 = interp(T0, g);
+        L.Sig1 = interp(T0 + nE, g);
+        L.Sig2 = interp(T0 + 2 * nE, g);
         L.Stot = L.Sig0 + L.Sig1 + L.Sig2;
     } else {
         const bool em = (pt == kElectron);
@@ -224,7 +228,7 @@ EMX_HD void finish_step(const Params &P, int pt, Track &t, StepOut &o) {
 // EXT: multiple scattering and / or energy-loss fluctuations are on.
 // L receives the table values of item 3 (left alone below the cut and in vacuum) for a caller that runs stage a2 next.
 template <bool CH, bool EXT>
-EMX_HD void step_a0(const Params &P, uint64_t seed, int pt, const Track &t, Carry &c, Lookup &L) {
+EMX_HD void step_a0(const Params &P, uint64_t seed, int pt, const Track &t, Carry &c, Lookup &L, const double *gtab = nullptr) {
     const emx_physics &ph = P.ph;
     const int mat = P.vol[t.vol].material;
     c.s = 0.0;
@@ -236,7 +240,7 @@ EMX_HD void step_a0(const Params &P, uint64_t seed, int pt, const Track &t, Carr
         c.s_phys = ph.vacuum_step;
         c.action = EMX_A_TRUNC;
     } else {  // 3. lookup, 4. limits
-        lookup_tables<CH, EXT>(P, pt, mat, t.E, L);
+        lookup_tables<CH, EXT>(P, pt, mat, t.E, L, gtab);
         const double xi = draw_at(seed, t.prim, t.tid, t.step, 0u);
         step_limits<CH, EXT>(P, L, xi, c.s_phys, c.action);
         // R-MSC2: the limits are true path lengths; what the move is limited by is the geometric length of the step

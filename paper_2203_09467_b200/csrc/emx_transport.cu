@@ -815,7 +815,7 @@ __device__ __forceinline__ WarpAcc epilogue(const Params &P, const Work &w, uint
 // k_b runs every interactor on full warps (B:north_star "partitioned by next action").
 template <int POOL, bool EXT, bool FUSED>
 __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint64_t seed, double *tally, int base,
-                                           int n_live, int safe) {
+                                           int n_live, int safe, const double *gtab = nullptr) {
     constexpr bool CH = POOL == kPoolCharged;
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
@@ -861,7 +861,7 @@ __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint6
         L.Sig0 = L.Sig1 = L.Sig2 = L.Stot = L.D = L.R = L.iL0 = L.iL20 = L.var0 = 0.0;
         L.Rtab = nullptr;
         if (FUSED) {
-            step_a0<CH, EXT>(P, seed, pt, t, cy, L);
+            step_a0<CH, EXT>(P, seed, pt, t, cy, L, gtab);
             if (cy.action != kActCut) move_straight(P, t, cy);
         } else {
             cy.action = ts.act[s];
@@ -899,7 +899,8 @@ __device__ __forceinline__ WarpAcc a_group(const Params &P, const Work &w, uint6
 
 // the persistent loop of the dense phase-A kernels
 template <int POOL, bool EXT, bool FUSED>
-__device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, uint64_t seed, double *tally, int node) {
+__device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, uint64_t seed, double *tally, int node,
+                                              const double *gtab = nullptr) {
     Ctl *c = w.ctl;
     const int lane = threadIdx.x & 31;
     const int nl = c->m_step[POOL];
@@ -912,7 +913,7 @@ __device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, ui
     // the groups of a dense kernel cost about the same: a fixed stride per warp, no work counter
     const int n_warps = gridDim.x * (kStepBlock / 32);
     for (int k = blockIdx.x * (kStepBlock / 32) + (threadIdx.x >> 5); k < total; k += n_warps) {
-        const WarpAcc d = a_group<POOL, EXT, FUSED>(P, w, seed, tally, k << 5, nl, safe);
+        const WarpAcc d = a_group<POOL, EXT, FUSED>(P, w, seed, tally, k << 5, nl, safe, gtab);
         acc.n += d.n;
         acc.d += d.d;
     }
@@ -938,8 +939,20 @@ __device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, ui
 
 template <int POOL, bool EXT>
 __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_A) k_a(const __grid_constant__ Params P, const __grid_constant__ Work w,
-                                                                uint64_t seed, double *tally) {
-    a_kernel_body<POOL, EXT, true>(P, w, seed, tally, 3 + POOL);
+                                                                uint64_t seed, double *tally, int stage_tab) {
+    // photon pool, emx_schedule entry 7 bit 1: the three tables a photon step interpolates (Compton, photoelectric, pair:
+    // 3 x n_E doubles per material, adjacent kinds) are copied to shared memory first (B:north_star "shared-memory ...
+    // staging of the hot table slices"; measured, profiles/r2_staging.md)
+    extern __shared__ double s_gtab[];
+    const double *gtab = nullptr;
+    if (POOL == kPoolGamma && stage_tab) {
+        const int nE = P.ph.n_E, per = 3 * nE;
+        for (int k = threadIdx.x; k < P.n_mat * per; k += blockDim.x)
+            s_gtab[k] = P.tab[(size_t)(k / per) * EMX_NTABLE * nE + (k % per)];
+        __syncthreads();
+        gtab = s_gtab;
+    }
+    a_kernel_body<POOL, EXT, true>(P, w, seed, tally, 3 + POOL, gtab);
 }
 template <bool EXT>
 __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_A2) k_a2(const __grid_constant__ Params P, const __grid_constant__ Work w,
@@ -1232,12 +1245,16 @@ cudaError_t launch_stage(int stage, const Params &P, const Work &w, uint64_t see
     const int g = w.grid[stage];
     const bool ext = ext_on(P);
     switch (stage) {
-    case kStageAGamma:
-        k_a<kPoolGamma, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+    case kStageAGamma: {
+        // shared-memory copy of the photon tables: 3 x n_E doubles per material, up to 40 KB per block
+        const size_t tb = (size_t)P.n_mat * 3 * (size_t)P.ph.n_E * sizeof(double);
+        const int stage_tab = ((w.stage_faces & 2) && tb <= 40 * 1024) ? 1 : 0;
+        k_a<kPoolGamma, false><<<g, kStepBlock, stage_tab ? tb : 0, st>>>(P, w, seed, tally, stage_tab);
         break;
+    }
     case kStageACharged:  // no field: limits + straight move + finish
-        if (ext) k_a<kPoolCharged, true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
-        else k_a<kPoolCharged, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally);
+        if (ext) k_a<kPoolCharged, true><<<g, kStepBlock, 0, st>>>(P, w, seed, tally, 0);
+        else k_a<kPoolCharged, false><<<g, kStepBlock, 0, st>>>(P, w, seed, tally, 0);
         break;
     case kStageA0:
         if (ext) k_a0<true><<<g, kStepBlock, 0, st>>>(P, w, seed);
@@ -1247,7 +1264,7 @@ cudaError_t launch_stage(int stage, const Params &P, const Work &w, uint64_t see
         const int ax = P.field_kind == 0 ? field_axis(P.Bhat) : kAxisAny;
         // shared-memory copy of the face table: up to 40 KB per block (5 blocks per SM stay resident)
         const size_t fb = (size_t)P.n_vol * EMX_MAX_FACES * sizeof(Face);
-        const int stage = (w.stage_faces && fb <= 40 * 1024) ? 1 : 0;
+        const int stage = ((w.stage_faces & 1) && fb <= 40 * 1024) ? 1 : 0;
         const size_t sm = stage ? fb : 0;
         if (P.ph.integrator == 1) {  // Dormand-Prince 5(4) (DESIGN.md R-INT): instantiations of their own
             if (P.field_kind != 0) k_field<true, kAxisAny, 1><<<g, kStepBlock, sm, st>>>(P, w, stage);

@@ -124,7 +124,8 @@ struct Work {
     int grid[8];            // blocks of the persistent step kernels, by stage (emx_kernels.h: kStage*)
     int reserve_slack;      // records all resident warps can request at the same time (see reserve())
     int slot_cap;           // slots a pool may hold at most (= n_chunks * kChunk; smaller in the refill hook)
-    int stage_faces;        // 1: k_field keeps the geometry's face table in shared memory (emx_schedule)
+    int stage_faces;        // shared-memory staging switches (emx_schedule entry 7): bit 0 the face table in k_field, bit 1
+                            // the photon tables in k_a<gamma>
     int pool_reserve;       // chunks a pool never takes, so that the other pool can always start (n_chunks / 32, >= 1)
 };
 

@@ -22,6 +22,7 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--primaries", type=int, default=48)
     ap.add_argument("--stage-faces", type=int, default=0, help="1: k_field stages the face table in shared memory (emx_schedule)")
+    ap.add_argument("--stage-tables", type=int, default=0, help="1: k_a<gamma> stages the photon tables in shared memory")
     a = ap.parse_args()
     from .. import emx, workloads as W
     desc, prim = W.get(a.config, a.primaries)
@@ -30,11 +31,13 @@ def main():
     G.set_profile(2)
     if a.stage_faces:
         G.set_schedule(stage_faces=True)
+    if a.stage_tables:
+        G.set_schedule(stage_tables=True)
     r = G.transport(pd, desc["seed"])
     p = G.profile()
     print(json.dumps({"config": a.config, "primaries": a.primaries, "workload": desc["name"], "iterations": int(r["iterations"]),
                       "track_steps": int(r["track_steps"]), "attempts": float(p["attempts"]),
-                      "k_field_slots": float(p["lanes"]["k_field"]), "stage_faces": a.stage_faces, "ms": float(r["ms"]),
+                      "k_field_slots": float(p["lanes"]["k_field"]), "stage_faces": a.stage_faces, "stage_tables": a.stage_tables, "ms": float(r["ms"]),
                       "k_field_ms": float(p["ms"].get("k_field", 0.0))}))
     return 0
 

@@ -294,12 +294,14 @@ class Problem:
 
     def set_schedule(self, **kw):
         """emx_set_schedule: loop_node, slice_min, slice_max, slice_above, blocks_per_sm (dict stage name -> blocks
-        or a list of 7), stage_faces (bool).  Only what is named changes.  A schedule never changes a result."""
+        or a list of 7), stage_faces / stage_tables (bool: the shared-memory staging switches, both measured slower).  Only what is named changes.  A schedule never changes a result."""
         sc = Schedule()
         self._check(lib().emx_get_schedule(self.h, C.byref(sc)))
         for k, v in kw.items():
             if k == "stage_faces":
-                sc.blocks_per_sm[7] = 1 if v else 0
+                sc.blocks_per_sm[7] = (sc.blocks_per_sm[7] & ~1) | (1 if v else 0)
+            elif k == "stage_tables":
+                sc.blocks_per_sm[7] = (sc.blocks_per_sm[7] & ~2) | (2 if v else 0)
             elif k == "blocks_per_sm":
                 items = v.items() if isinstance(v, dict) else zip(STAGES, v)
                 for name, b in items:

@@ -502,14 +502,14 @@ def test_error_paths(emx):
 
 def test_scheduling_knobs_do_not_change_results(emx):
     """Time slicing of the field propagation (attempts per iteration before a track may be parked), the grids of
-    the persistent kernels and the launch paths (the loop as one graph with a WHILE node, flat iteration graphs
+    the persistent kernels, the shared-memory staging switches and the launch paths (the loop as one graph with a WHILE node, flat iteration graphs
     polled by the host, plain stream launches, profiled launches) only change WHEN work is done: counters are
     equal, tallies equal up to summation order."""
     desc, prim = W.get(4, 64)
     runs, hists = [], []
     variants = (dict(slice_min=2, slice_max=16), dict(slice_min=1000, slice_max=1000), dict(slice_min=1, slice_max=1),
                 dict(slice_min=3, slice_max=7, profile=2), dict(profile=1), dict(loop_node=0),
-                dict(blocks_per_sm={"k_field": 1, "k_a2": 2, "k_b<gamma>": 1}))
+                dict(blocks_per_sm={"k_field": 1, "k_a2": 2, "k_b<gamma>": 1}), dict(stage_faces=True, stage_tables=True))
     for v in variants:
         v = dict(v)
         G = emx.Problem(desc)
