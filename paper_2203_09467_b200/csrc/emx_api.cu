@@ -345,14 +345,21 @@ int emx_build_tables(emx_problem *p, void *stream) {
     memset(faces.data(), 0, faces.size() * sizeof(Face));
     for (size_t iv = 0; iv < nv; ++iv) {
         const Volume &v = hp.vol[iv];
-        for (int i = 0; i < v.n_faces; ++i) {
-            Face &f = faces[iv * EMX_MAX_FACES + i];
-            f.S = v.surf[i];
-            f.v = hp.surf_v[v.surf[i]];
-            f.type = (int8_t)hp.surf_type[v.surf[i]];
-            f.sense = (int8_t)v.sense[i];
-        }
-        faces[iv * EMX_MAX_FACES].n = (int16_t)v.n_faces;
+        // planes first, cylinders after (each group in the cell's own order): the distance routine runs one uniform loop
+        // per kind; the result does not depend on the order (ties go to the lowest surface id)
+        int k = 0, n_plane = 0;
+        for (int pass = 0; pass < 2; ++pass)
+            for (int i = 0; i < v.n_faces; ++i) {
+                const bool cyl = hp.surf_type[v.surf[i]] == EMX_S_CZ;
+                if (cyl != (pass == 1)) continue;
+                Face &f = faces[iv * EMX_MAX_FACES + k++];
+                f.S = v.surf[i];
+                f.v = hp.surf_v[v.surf[i]];
+                f.type = (int8_t)hp.surf_type[v.surf[i]];
+                f.sense = (int8_t)v.sense[i];
+                if (!cyl) n_plane += 1;
+            }
+        faces[iv * EMX_MAX_FACES].n = (int16_t)(v.n_faces | (n_plane << 8));  // low byte: faces, high byte: planes among them
     }
     CU(cudaMemcpyAsync(p->d_faces, faces.data(), faces.size() * sizeof(Face), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(p->d_nb_off, nb_off.data(), nb_off.size() * sizeof(int), cudaMemcpyHostToDevice, st));

@@ -54,7 +54,7 @@ struct Face {
     int S;         // surface id
     int8_t type;   // EMX_S_*
     int8_t sense;  // side of the surface the cell is on
-    int16_t n;     // face 0 only: number of faces of the cell
+    int16_t n;     // face 0 only: low byte = number of faces of the cell, high byte = how many of them are planes (they come first)
 };
 
 // Read-only problem data ("params" in the paper's params/state split), passed to

@@ -22,47 +22,64 @@ EMX_HD double surf_g(int type, const Vec3 &x, const Vec3 &u) {
 EMX_NI double distance_to_faces(const Face *cell, const Vec3 &x, const Vec3 &u, int on_surf, int &hit) {
     double best = kInf;
     int bs = -1;
-    // cylinder coefficients shared by every CZ face of the cell
-    const double a = u.x * u.x + u.y * u.y;
-    const double b = x.x * u.x + x.y * u.y;
-    const double rr = x.x * x.x + x.y * x.y;
-    const int nf = cell[0].n;
-    for (int i = 0; i < nf; ++i) {
+    const int nn = cell[0].n;
+    const int nf = nn & 0xff, np = (nn >> 8) & 0xff;
+    // planes (the table lists them first): one division each, the iterations are independent of one another
+#pragma unroll 2
+    for (int i = 0; i < np; ++i) {
         const Face f = cell[i];
         const int S = f.S;
         const int type = f.type;
+        double d = -1.0;
+        bool have = false;
+        const double ua = comp(u, type);
+        if (S == on_surf) {
+            const int ns = ua > 0.0 ? 1 : -1;
+            if (ns != f.sense) {  // heading back across the surface it sits on
+                d = 0.0;
+                have = true;
+            }
+        } else if (ua != 0.0) {
+            const double t = (f.v - comp(x, type)) / ua;
+            if (t > 0.0) { d = t; have = true; }
+        }
+        if (have && (d < best || (d == best && S < bs))) {
+            best = d;
+            bs = S;
+        }
+    }
+    // z-cylinders: coefficients shared by all of them
+    const double a = u.x * u.x + u.y * u.y;
+    const double b = x.x * u.x + x.y * u.y;
+    const double rr = x.x * x.x + x.y * x.y;
+#pragma unroll 2
+    for (int i = np; i < nf; ++i) {
+        const Face f = cell[i];
+        const int S = f.S;
         const double v = f.v;
         double d = -1.0;
         bool have = false;
         if (S == on_surf) {
-            const double g = (type == EMX_S_CZ) ? 2.0 * b : comp(u, type);
+            const double g = 2.0 * b;
             const int ns = g > 0.0 ? 1 : -1;
             if (ns != f.sense) {  // heading back across the surface it sits on
                 d = 0.0;
                 have = true;
-            } else if (type == EMX_S_CZ && a > 0.0) {  // on the cylinder: c0 = 0 exactly, roots 0 and -2b/a
+            } else if (a > 0.0) {  // on the cylinder: c0 = 0 exactly, roots 0 and -2b/a
                 const double r = -2.0 * b / a;
                 if (r > 0.0) { d = r; have = true; }
             }
-        } else if (type == EMX_S_CZ) {
-            if (a > 0.0) {
-                const double c0 = rr - v * v;
-                const double disc = b * b - a * c0;
-                if (disc >= 0.0) {
-                    const double sq = sqrt(disc);
-                    const double q = (b >= 0.0) ? -(b + sq) : -(b - sq);  // cancellation-free pair q/a, c0/q
-                    const double r1 = q / a;
-                    const double r2 = (q != 0.0) ? c0 / q : -1.0;
-                    const double lo = r1 < r2 ? r1 : r2, hi = r1 < r2 ? r2 : r1;
-                    if (lo > 0.0) { d = lo; have = true; }
-                    else if (hi > 0.0) { d = hi; have = true; }
-                }
-            }
-        } else {
-            const double ua = comp(u, type);
-            if (ua != 0.0) {
-                const double t = (v - comp(x, type)) / ua;
-                if (t > 0.0) { d = t; have = true; }
+        } else if (a > 0.0) {
+            const double c0 = rr - v * v;
+            const double disc = b * b - a * c0;
+            if (disc >= 0.0) {
+                const double sq = sqrt(disc);
+                const double q = (b >= 0.0) ? -(b + sq) : -(b - sq);  // cancellation-free pair q/a, c0/q
+                const double r1 = q / a;
+                const double r2 = (q != 0.0) ? c0 / q : -1.0;
+                const double lo = r1 < r2 ? r1 : r2, hi = r1 < r2 ? r2 : r1;
+                if (lo > 0.0) { d = lo; have = true; }
+                else if (hi > 0.0) { d = hi; have = true; }
             }
         }
         if (have && (d < best || (d == best && S < bs))) {
@@ -81,7 +98,7 @@ EMX_HD double distance_to_boundary(const Params &P, int vol, const Vec3 &x, cons
 // tolerance take their sense from the direction of motion (C8).
 EMX_HD bool cell_matches(const Params &P, int cid, const Vec3 &x, const Vec3 &u, int S, int newsense) {
     const Face *cell = P.faces + (size_t)cid * EMX_MAX_FACES;
-    const int nf = cell[0].n;
+    const int nf = cell[0].n & 0xff;
     for (int i = 0; i < nf; ++i) {
         const Face fc = cell[i];
         int sn;
