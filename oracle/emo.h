@@ -17,7 +17,8 @@
  * Parity status: every function below is pinned by tests/test_oracle_*.py.
  * Of the aggregate shower shapes the longitudinal profile is pinned (maximum at
  * ln(E/Ec) - 0.5 radiation lengths and the 95 % containment length of the PDG
- * review, tests/test_oracle_transport.py); sampling fractions and
+ * review, tests/test_oracle_transport.py) and, with multiple scattering on, the
+ * lateral containment in Moliere radii (tests/test_oracle_msc2.py); sampling fractions and
  * multiplicities remain "parity unpinned" beyond energy conservation: the paper
  * prints no number for them and no independent code exists in this container.
  * emo_sigma_pe is a definitional stand-in (R3): its pin is its own

@@ -259,3 +259,29 @@ def test_shower_with_the_spatial_moments_closes_energy_and_is_reproducible(emo):
     assert a["edep"].sum() + a["escaped"] + a["looper"] == pytest.approx(a["E_in"], rel=1e-9)
     c = emo.Problem(dict(desc, physics=dict(desc["physics"], msc=1))).transport(prim, 5)
     assert c["steps"][1] != a["steps"][1]                    # the option changes the histories
+
+
+def test_lateral_shower_containment_in_moliere_radii(emo):
+    """What multiple scattering is FOR in a shower, pinned by the PDG review ("Passage of particles through matter",
+    electromagnetic cascades): the transverse size scales with the Moliere radius R_M = X0 (21.2 MeV / E_c); on
+    average 10 % of the energy lies outside a cylinder of radius R_M, about 1 % outside 3.5 R_M.  200 showers of 1 GeV
+    in lead rings of R_M / 4 around the beam axis, 40 X0 deep.  With the deflection and the spatial moments on: 88 / 95 /
+    99 % inside 1 / 2 / 3.5 R_M; with multiple scattering off the shower is far too narrow (97 % inside 1 R_M), so the
+    pin does see the model."""
+    X0 = emo.Problem(W.config1(1)[0]).material_info(0)["X0"]
+    RM = X0 * 21.2 / (610.0 / (82 + 1.24))
+    assert RM == pytest.approx(1.62, abs=0.01)                         # cm
+    radii = [(k + 1) * 0.25 * RM for k in range(20)] + [60.0]
+    surfaces = [(W.PZ, 0.0), (W.PZ, 40 * X0)] + [(W.CZ, r) for r in radii]
+    volumes = [dict(surf=[0, 1, 2], sense=[1, -1, -1], material=0, tally=0)]
+    volumes += [dict(surf=[0, 1, 1 + k, 2 + k], sense=[1, -1, 1, -1], material=0, tally=k) for k in range(1, len(radii))]
+    inside = {}
+    for msc in (0, 2):
+        desc = dict(name="pb_rings", seed=13, materials=[W.PB], surfaces=surfaces, volumes=volumes, field=(0.0, 0.0, 0.0),
+                    physics=W.physics(msc=msc), n_slots=1 << 16, queue_capacity=1 << 20)
+        r = emo.Problem(desc).transport(W._prim(200, 1, 1000.0, (0, 0, 0), (0, 0, 1), 0, 0), 13)
+        assert r["edep"].sum() + r["escaped"] + r["looper"] == pytest.approx(r["E_in"], rel=1e-9)
+        cum = np.cumsum(r["edep"]) / r["edep"].sum()
+        inside[msc] = (float(cum[3]), float(cum[7]), float(cum[13]))     # 1, 2, 3.5 R_M
+    assert 0.85 < inside[2][0] < 0.93 and 0.93 < inside[2][1] < 0.975 and inside[2][2] > 0.975, inside
+    assert inside[0][0] > 0.95, inside
