@@ -924,6 +924,9 @@ __device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, ui
 #ifndef EMX_BLOCKS_A
 #define EMX_BLOCKS_A 4   // resident 128-thread blocks per SM the dense phase-A kernels are compiled for
 #endif
+#ifndef EMX_BLOCKS_AG
+#define EMX_BLOCKS_AG 5  // the photon instantiation of k_a: 102 registers (measured: -7 % for the kernel); e+- keep 4 blocks (128)
+#endif
 #ifndef EMX_BLOCKS_A2
 #define EMX_BLOCKS_A2 5
 #endif
@@ -931,14 +934,14 @@ __device__ __forceinline__ void a_kernel_body(const Params &P, const Work &w, ui
 #define EMX_BLOCKS_B 4
 #endif
 #ifndef EMX_BLOCKS_F
-#define EMX_BLOCKS_F 5
+#define EMX_BLOCKS_F 6  // uniform field: 80 registers; the field-map instantiations keep 96 (5 blocks)
 #endif
 #ifndef EMX_BLOCKS_0
 #define EMX_BLOCKS_0 8
 #endif
 
 template <int POOL, bool EXT>
-__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_A) k_a(const __grid_constant__ Params P, const __grid_constant__ Work w,
+__global__ void __launch_bounds__(kStepBlock, POOL == kPoolGamma ? EMX_BLOCKS_AG : EMX_BLOCKS_A) k_a(const __grid_constant__ Params P, const __grid_constant__ Work w,
                                                                 uint64_t seed, double *tally, int stage_tab) {
     // photon pool, emx_schedule entry 7 bit 1: the three tables a photon step interpolates (Compton, photoelectric, pair:
     // 3 x n_E doubles per material, adjacent kinds) are copied to shared memory first (B:north_star "shared-memory ...
@@ -1022,7 +1025,7 @@ __global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_0) k_a0(const __grid_co
 // attempts once the pool has no track left to hand out (or after slice_max attempts): its loop variables go to
 // the slot and the next iteration continues the SAME sequence of substeps.
 template <bool MAP, int AX, int INTEG = 0>
-__global__ void __launch_bounds__(kStepBlock, EMX_BLOCKS_F) k_field(const __grid_constant__ Params P, const __grid_constant__ Work w,
+__global__ void __launch_bounds__(kStepBlock, MAP ? 5 : EMX_BLOCKS_F) k_field(const __grid_constant__ Params P, const __grid_constant__ Work w,
                                                                     int stage_faces) {
     // the face table of the whole geometry (16 B per face) is staged in shared memory when it fits: every attempt
     // reads the faces of its cell (B:north_star "shared-memory ... staging of the hot table slices")
