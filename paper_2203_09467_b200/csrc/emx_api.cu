@@ -472,7 +472,7 @@ int emx_reset_tallies(emx_problem *p, void *stream) {
 // bounds allow, shared between the chains that run side by side
 static void size_grids(const emx_problem *p, Work &w) {
     // defaults per stage (kStage*): 128-thread blocks per SM
-    static const int kDefault[kNStages] = {5, 4, 8, 5, 5, 4, 4};
+    static const int kDefault[kNStages] = {5, 4, 6, 5, 5, 4, 4};
     for (int k = 0; k < kNStages; ++k) {
         int b = p->sched.blocks_per_sm[k] > 0 ? p->sched.blocks_per_sm[k] : kDefault[k];
         // the propagation kernels of a uniform field are compiled for 6 blocks per SM (80 registers), that of a field map for 5
