@@ -100,7 +100,8 @@ def _workload(cfg, n):
     ext = {37: dict(msc=1, msc_fr=0.2, msc_smin=1e-3), 47: dict(msc=1, msc_fr=0.1, msc_smin=2e-3, fluct=1), 17: dict(fluct=1),
            27: dict(msc=2, msc_fr=0.2, msc_smin=1e-3, fluct=1), 38: dict(msc=2, msc_fr=0.2, msc_smin=1e-3),
            48: dict(msc=2, msc_fr=0.1, msc_smin=2e-3, fluct=1),
-           43: dict(integrator=1), 63: dict(integrator=1)}      # the Dormand-Prince integrator (R-INT): barrel at 4 T, fringe field
+           43: dict(integrator=1), 63: dict(integrator=1),      # the Dormand-Prince integrator (R-INT): barrel at 4 T, fringe field
+           49: dict(msc=2, msc_fr=0.1, msc_smin=2e-3, fluct=1, integrator=1)}   # everything optional at once
     if cfg in ext:
         desc, prim = W.get(cfg // 10, n)
         desc = dict(desc, physics=dict(desc["physics"], **ext[cfg]), seed=cfg)
@@ -129,7 +130,7 @@ def test_tables_match_the_oracle(emx, emo, cfg):
 # ---------------- level 2: single step ----------------
 
 @pytest.mark.parametrize("cfg,n", [(0, 20000), (1, 40000), (2, 40000), (3, 40000), (4, 40000), (5, 20000), (6, 40000),
-                                   (7, 40000), (17, 40000), (37, 40000), (47, 40000), (27, 40000), (38, 40000), (48, 40000), (43, 40000), (63, 40000)])
+                                   (7, 40000), (17, 40000), (37, 40000), (47, 40000), (27, 40000), (38, 40000), (48, 40000), (43, 40000), (63, 40000), (49, 40000)])
 def test_single_step_parity(emx, emo, cfg, n):
     desc, _ = _workload(cfg, 4)
     G, O = emx.Problem(desc), emo.Problem(desc)
@@ -147,13 +148,13 @@ def test_single_step_parity(emx, emo, cfg, n):
     assert worst <= 1.0, {k: v for k, v in rep.items() if isinstance(v, float) and v > 0.5}
     plain = (ref["n_sub"] == 0) & (tol["E"] == states.RTOL2)      # the plain 1e-12 of north_star holds for these
     assert plain.sum() > n // 4 and np.all(tol["u"][plain] == states.RTOL2) and np.all(tol["x"][plain] == states.RTOL2)
-    if cfg in (3, 4, 6, 37, 47, 38, 48, 43, 63):
+    if cfg in (3, 4, 6, 37, 47, 38, 48, 43, 63, 49):
         assert tol["trunc"].sum() <= n // 6 and (ref["n_sub"] > 1).sum() > n // 10
     # coverage of the branches
     acts = np.bincount(ref["action"], minlength=6)
     assert acts[1] > 0 and (cfg == 0 or acts[3] > 0)
     fl = desc["physics"]["fluct"]
-    if cfg in (7, 37, 47, 27, 38, 48):      # multiple scattering: the step limit was hit, deflections happened before interactions
+    if cfg in (7, 37, 47, 27, 38, 48, 49):      # multiple scattering: the step limit was hit, deflections happened before interactions
         assert acts[5] > 0 and (ref["msc_tau"][ref["action"] == 1] > 0).any() and (ref["msc_tau"][ref["action"] == 3] > 0).any()
         assert np.all(ref["n_draws"][(ref["msc_tau"] > 0) & (ref["action"] == 1)] >= 4 + 2 * fl)
     else:
@@ -223,7 +224,7 @@ def test_one_field_substep_at_1e_12(emx, emo, field, fringe, integrator):
 @pytest.mark.parametrize("cfg,n,n_slots", [(0, 1000, 1024), (1, 300, 1 << 16), (2, 24, 1 << 16), (3, 24, 1 << 16),
                                            (4, 48, 1 << 16), (1, 64, 1024), (5, 400, 1 << 16), (6, 48, 1 << 16),
                                            (7, 24, 1 << 16), (17, 300, 1 << 16), (37, 24, 1 << 16), (47, 48, 1 << 16),
-                                           (27, 24, 1 << 16), (48, 48, 1 << 16), (43, 48, 1 << 16)])
+                                           (27, 24, 1 << 16), (48, 48, 1 << 16), (43, 48, 1 << 16), (49, 48, 1 << 16)])
 def test_transport_parity_and_energy_closure(emx, emo, cfg, n, n_slots):
     desc, prim = _workload(cfg, n)
     G, O = emx.Problem(desc), emo.Problem(desc)
