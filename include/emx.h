@@ -295,7 +295,8 @@ int emx_set_primary_offset(emx_problem *p, long first);
  *   admit_below    primaries are admitted (in waves of n_slots / 256, 256..4096) only while fewer records than this
  *                  wait on the stacks (the queue is the memory limit); <= 0: 2 n_slots.
  *   blocks_per_sm  persistent 128-thread blocks per SM of each step kernel, in the order k_a<gamma>,
- *                  k_a<charged>, k_a0, k_field, k_a2, k_b<gamma>, k_b<charged>; 0 = default.  Entry 7 holds two switches
+ *                  k_a<charged>, k_a0, k_field, k_a2, k_b<gamma>, k_b<charged>; 0 = default (5, 4, 6, 6 -- 5 with a field map --,
+ *                  5, 4, 4: what the kernels' registers allow).  Entry 7 holds two switches
  *                  for shared-memory staging of hot table slices: bit 0 = k_field copies the geometry's face table to
  *                  shared memory, bit 1 = k_a<gamma> copies the photon tables (3 per material) -- instead of reading
  *                  them through L1.  Both measured SLOWER on B200 (profiles/r2_staging.md) and kept for that comparison. */
